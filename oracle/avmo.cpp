@@ -1,0 +1,482 @@
+// avmo.cpp — ORACLE (test infrastructure; see avmo.h).  Plain serial C++17, fp64, one electron at a time,
+// written in the order and notation of SURVEY.md §8(c) steps S0-S9 (restated in DESIGN.md §3).
+// Compile: g++ -O2 -ffp-contract=off -std=c++17 -shared -fPIC (no fused multiply-add, no fast-math).
+// Shares nothing with paper_2509_15377_b200/csrc/.
+#include "avmo.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <string>
+#include <thread>
+#include <vector>
+
+namespace {
+
+// ---- constants (SURVEY.md §8(c) "Constants"; CODATA-2018: c = 29.9792458 cm/ns, mc^2 = 510998.95 eV) ----
+const double C2 = 0.05930969584745753;        // speed [cm/ns] = C2 * sqrt(energy [eV])
+const double INV_C2SQ = 284.28150518042008;   // energy = |v|^2 * INV_C2SQ
+const double KAPPA = 0.0017588200107589609;   // acceleration a = -KAPPA * E  [cm/ns^2 per V/cm]
+const double OMEGA1 = 175.88200107589608;     // cyclotron angular frequency per tesla [rad/ns/T]
+const double EXB_UNIT = 1.0e-5;               // v_d [cm/ns] = 1e-5 (E x B)/|B|^2, E in V/cm, B in T
+const double EPS_FLOOR = 1.0e-10;             // eV
+const double TWO_PI = 6.283185307179586;
+const uint32_t BLOCK_CHILD_ID = 0xFFFFFFFFu;
+const uint32_t N_STEP_LIMIT = 0xFFFFFFF0u;
+
+thread_local std::string g_err;
+
+// ---- Philox4x32-10 (Salmon et al., SC'11), SURVEY.md §8(c) "Uniforms" ------------------------------------
+void philox4x32_10(uint32_t c[4], uint32_t k0, uint32_t k1) {
+  const uint64_t M0 = 0xD2511F53ull, M1 = 0xCD9E8D57ull;
+  for (int round = 0; round < 10; ++round) {
+    uint64_t p0 = M0 * (uint64_t)c[0];
+    uint64_t p1 = M1 * (uint64_t)c[2];
+    uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+    uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+    uint32_t n0 = hi1 ^ c[1] ^ k0, n1 = lo1, n2 = hi0 ^ c[3] ^ k1, n3 = lo0;
+    c[0] = n0; c[1] = n1; c[2] = n2; c[3] = n3;
+    if (round < 9) { k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
+  }
+}
+
+void philox_block(uint64_t seed, uint64_t id, uint32_t n, uint32_t block, uint32_t w[4]) {
+  w[0] = n; w[1] = block; w[2] = (uint32_t)id; w[3] = (uint32_t)(id >> 32);
+  philox4x32_10(w, (uint32_t)seed, (uint32_t)(seed >> 32));
+}
+
+double to_unit(uint32_t hi, uint32_t lo) {           // ((x >> 12) + 0.5) * 2^-52, strictly inside (0,1)
+  uint64_t x = ((uint64_t)hi << 32) | (uint64_t)lo;
+  return ((double)(x >> 12) + 0.5) * 2.220446049250313e-16;
+}
+
+void uniform_pair(uint64_t seed, uint64_t id, uint32_t n, uint32_t block, double& ua, double& ub) {
+  uint32_t w[4];
+  philox_block(seed, id, n, block, w);
+  ua = to_unit(w[0], w[1]);
+  ub = to_unit(w[2], w[3]);
+}
+
+// ---- data ---------------------------------------------------------------------------------------------
+struct Gas {
+  int nb = 0, L = 0;
+  double e_max = 0, inv_de = 0, nu_hat = 0, inv_nu_hat = 0;
+  const double* cum = nullptr;
+  const uint8_t* type = nullptr;
+  const double *loss = nullptr, *recoil = nullptr, *w = nullptr;
+};
+
+struct Electron {
+  double x, y, z, t, e, kx, ky, kz;
+  uint64_t id;
+  uint32_t n, aval;
+  int32_t status;
+  double birth[5];
+};
+
+struct Tally {
+  std::vector<uint64_t> level;
+  uint64_t n_null = 0, n_real = 0, n_overflow = 0, n_steps = 0;
+  double sdx = 0, sdy = 0, sdz = 0, sdt = 0, sloss = 0;
+};
+
+bool load_gas(const avmo_gas_desc* d, Gas& g) {
+  if (!d || d->n_bins < 1 || d->n_levels < 1 || !(d->e_max_eV > 0) || !d->cum_rate || !d->level_type ||
+      !d->level_loss_eV || !d->level_recoil || !d->level_ob_w_eV) { g_err = "gas: null or empty field"; return false; }
+  g.nb = d->n_bins; g.L = d->n_levels; g.e_max = d->e_max_eV;
+  g.inv_de = (double)g.nb / g.e_max;
+  g.cum = d->cum_rate; g.type = d->level_type; g.loss = d->level_loss_eV; g.recoil = d->level_recoil; g.w = d->level_ob_w_eV;
+  double mx = 0;
+  for (int b = 0; b < g.nb; ++b) {
+    double prev = 0;
+    for (int l = 0; l < g.L; ++l) {
+      double c = g.cum[(size_t)b * g.L + l];
+      if (!(c >= prev)) { g_err = "gas: cum_rate decreases along levels"; return false; }
+      prev = c;
+    }
+    mx = std::max(mx, prev);
+  }
+  for (int l = 0; l < g.L; ++l) if (g.type[l] > 3) { g_err = "gas: bad level type"; return false; }
+  g.nu_hat = d->nu_hat > 0 ? d->nu_hat : mx;      // R4: one global null-collision rate
+  if (!(g.nu_hat > 0) || g.nu_hat < mx) { g_err = "gas: nu_hat must be >= max total rate and > 0"; return false; }
+  g.inv_nu_hat = 1.0 / g.nu_hat;
+  return true;
+}
+
+bool check_field(const avmo_field_desc* f) {
+  if (!f || !f->slabs || f->n_slabs < 1) { g_err = "field: no slabs"; return false; }
+  for (int i = 0; i < f->n_slabs; ++i) {
+    const avmo_slab& s = f->slabs[i];
+    if (!(s.z_hi > s.z_lo)) { g_err = "field: slab z_hi <= z_lo"; return false; }
+    if (i > 0 && s.z_lo != f->slabs[i - 1].z_hi) { g_err = "field: slabs not contiguous/ascending"; return false; }
+    if (s.kind == 1) {
+      if (!s.nodes || s.nx < 2 || s.ny < 2 || s.nz < 2) { g_err = "field: grid needs nodes and >=2 per axis"; return false; }
+      for (int a = 0; a < 3; ++a) if (!(s.spacing[a] > 0)) { g_err = "field: spacing"; return false; }
+      double ztop = s.origin[2] + (s.nz - 1) * s.spacing[2];
+      double tol = 1e-9 * s.spacing[2];
+      if (s.z_lo < s.origin[2] - tol || s.z_hi > ztop + tol) { g_err = "field: slab z-range outside its grid"; return false; }
+      if (s.bc_x < 0 || s.bc_x > 2 || s.bc_y < 0 || s.bc_y > 2) { g_err = "field: bc"; return false; }
+      if (s.bc_x && !(s.period_x > 0 && s.period_x <= (s.nx - 1) * s.spacing[0] * (1 + 1e-12))) { g_err = "field: period_x"; return false; }
+      if (s.bc_y && !(s.period_y > 0 && s.period_y <= (s.ny - 1) * s.spacing[1] * (1 + 1e-12))) { g_err = "field: period_y"; return false; }
+    } else if (s.kind != 0) { g_err = "field: kind"; return false; }
+  }
+  return true;
+}
+
+// R15: fold one coordinate into the stored cell.  Returns false when outside with bc none.
+// q = (x - origin) mod period (periodic) or mod 2P with reflection (mirror); flip = normal component changes sign.
+bool fold(double x, double origin, double h, int n, int bc, double P, double& q, bool& flip) {
+  flip = false;
+  q = x - origin;
+  if (bc == 0) return q >= 0.0 && q <= (n - 1) * h;
+  if (bc == 1) { q = q - P * std::floor(q / P); if (q >= P) q = 0.0; return true; }
+  double two_p = 2.0 * P;
+  q = q - two_p * std::floor(q / two_p);
+  if (q >= two_p) q = 0.0;
+  if (q > P) { q = two_p - q; flip = true; }
+  return true;
+}
+
+void cell(double q, double h, int n, int& i, double& w) {   // i = min(floor(q/h), n-2), w = q/h - i
+  double s = q / h;
+  i = (int)std::floor(s);
+  if (i > n - 2) i = n - 2;
+  if (i < 0) i = 0;
+  w = s - (double)i;
+}
+
+// S0 / R14 / R15: field and gas-mask at r.  Returns the slab index, or a negative status code
+// (-AVMO_LEFT_*) when r is outside the domain.
+int field_at(const avmo_field_desc* f, double x, double y, double z, double E[3], double& mask) {
+  const avmo_slab* S = f->slabs;
+  int ns = f->n_slabs;
+  if (z < S[0].z_lo) return -AVMO_LEFT_ZLO;
+  if (z > S[ns - 1].z_hi) return -AVMO_LEFT_ZHI;
+  if (x < f->xy_lo[0] || x > f->xy_hi[0] || y < f->xy_lo[1] || y > f->xy_hi[1]) return -AVMO_LEFT_XY;
+  if (!(z == z) || !(x == x) || !(y == y)) return -AVMO_LEFT_XY;
+  int si = ns - 1;
+  for (int i = 0; i < ns; ++i) if (z < S[i].z_hi) { si = i; break; }
+  const avmo_slab& s = S[si];
+  if (s.kind == 0) { E[0] = s.E[0]; E[1] = s.E[1]; E[2] = s.E[2]; mask = 1.0; return si; }
+  double qx, qy; bool fx, fy;
+  if (!fold(x, s.origin[0], s.spacing[0], s.nx, s.bc_x, s.period_x, qx, fx)) return -AVMO_LEFT_XY;
+  if (!fold(y, s.origin[1], s.spacing[1], s.ny, s.bc_y, s.period_y, qy, fy)) return -AVMO_LEFT_XY;
+  int i, j, k; double wx, wy, wz;
+  cell(qx, s.spacing[0], s.nx, i, wx);
+  cell(qy, s.spacing[1], s.ny, j, wy);
+  cell(z - s.origin[2], s.spacing[2], s.nz, k, wz);
+  double out[4];
+  for (int c = 0; c < 4; ++c) {
+    auto N = [&](int kk, int jj, int ii) { return (double)s.nodes[(((size_t)kk * s.ny + jj) * s.nx + ii) * 4 + c]; };
+    // lerp a + w (b - a): x, then y, then z
+    double c00 = N(k, j, i) + wx * (N(k, j, i + 1) - N(k, j, i));
+    double c10 = N(k, j + 1, i) + wx * (N(k, j + 1, i + 1) - N(k, j + 1, i));
+    double c01 = N(k + 1, j, i) + wx * (N(k + 1, j, i + 1) - N(k + 1, j, i));
+    double c11 = N(k + 1, j + 1, i) + wx * (N(k + 1, j + 1, i + 1) - N(k + 1, j + 1, i));
+    double c0 = c00 + wy * (c10 - c00);
+    double c1 = c01 + wy * (c11 - c01);
+    out[c] = c0 + wz * (c1 - c0);
+  }
+  E[0] = fx ? -out[0] : out[0];
+  E[1] = fy ? -out[1] : out[1];
+  E[2] = out[2];
+  mask = out[3];
+  return si;
+}
+
+struct StepOut {
+  int event = -2;      // -1 null, l >= 0 level, -2 terminated before the decision
+  int bin = -1;
+  bool child = false;
+  Electron c;
+};
+
+// One step S0-S9 for an in-domain, active electron.
+void step(const Gas& g, const avmo_field_desc* f, uint64_t seed, double t_max, Electron& el, StepOut& so, Tally* tl) {
+  so.event = -2; so.bin = -1; so.child = false;
+  // S0: field at r (held constant during the flight); B is a run constant.  R3: re-evaluated every step.
+  double E[3], m;
+  int si = field_at(f, el.x, el.y, el.z, E, m);
+  if (si < 0) { el.status = -si; return; }      // not in domain: caller error, reported as a status
+  // S1: the step's counter n_s; block 0 -> (u1, u2)
+  const uint32_t n_s = el.n;
+  double u1, u2;
+  uniform_pair(seed, el.id, n_s, 0, u1, u2);
+  // S2: free-flight time under the null-collision rate nu_hat
+  const double dt = -std::log(u1) * g.inv_nu_hat;
+  // S3: flight in constant E (and B)
+  const double sp = C2 * std::sqrt(el.e);
+  const double v0[3] = {sp * el.kx, sp * el.ky, sp * el.kz};
+  const double a[3] = {-KAPPA * E[0], -KAPPA * E[1], -KAPPA * E[2]};
+  const double r0[3] = {el.x, el.y, el.z};
+  double r1[3], v1[3];
+  const double Bn2 = f->B[0] * f->B[0] + f->B[1] * f->B[1] + f->B[2] * f->B[2];
+  if (Bn2 == 0.0) {
+    for (int i = 0; i < 3; ++i) {
+      r1[i] = r0[i] + v0[i] * dt + 0.5 * a[i] * dt * dt;
+      v1[i] = v0[i] + a[i] * dt;
+    }
+  } else {
+    const double Bn = std::sqrt(Bn2);
+    const double bh[3] = {f->B[0] / Bn, f->B[1] / Bn, f->B[2] / Bn};
+    const double omega = OMEGA1 * Bn;
+    const double a_b = a[0] * bh[0] + a[1] * bh[1] + a[2] * bh[2];
+    const double v_b = v0[0] * bh[0] + v0[1] * bh[1] + v0[2] * bh[2];
+    const double ExB[3] = {E[1] * f->B[2] - E[2] * f->B[1], E[2] * f->B[0] - E[0] * f->B[2], E[0] * f->B[1] - E[1] * f->B[0]};
+    double apar[3], vpar[3], vd[3], w0[3], bxw[3];
+    for (int i = 0; i < 3; ++i) {
+      apar[i] = a_b * bh[i];
+      vpar[i] = v_b * bh[i];
+      vd[i] = EXB_UNIT * ExB[i] / Bn2;
+      w0[i] = v0[i] - vpar[i] - vd[i];
+    }
+    bxw[0] = bh[1] * w0[2] - bh[2] * w0[1];
+    bxw[1] = bh[2] * w0[0] - bh[0] * w0[2];
+    bxw[2] = bh[0] * w0[1] - bh[1] * w0[0];
+    const double th = omega * dt;
+    const double sn = std::sin(th), cs = std::cos(th);
+    const double sh = std::sin(0.5 * th);
+    const double vers = 2.0 * sh * sh;               // 1 - cos(theta), cancellation-free
+    for (int i = 0; i < 3; ++i) {
+      v1[i] = vpar[i] + apar[i] * dt + vd[i] + w0[i] * cs + bxw[i] * sn;
+      r1[i] = r0[i] + vpar[i] * dt + 0.5 * apar[i] * dt * dt + vd[i] * dt + (w0[i] * sn + bxw[i] * vers) / omega;
+    }
+  }
+  // S4: new energy, direction, time, counter
+  const double s2 = v1[0] * v1[0] + v1[1] * v1[1] + v1[2] * v1[2];
+  const double e1 = std::max(s2 * INV_C2SQ, EPS_FLOOR);
+  double k1[3] = {el.kx, el.ky, el.kz};
+  if (s2 > 0.0) { const double nrm = std::sqrt(s2); k1[0] = v1[0] / nrm; k1[1] = v1[1] / nrm; k1[2] = v1[2] / nrm; }
+  const double t1 = el.t + dt;
+  if (tl) {
+    tl->n_steps++;
+    tl->sdx += r1[0] - r0[0]; tl->sdy += r1[1] - r0[1]; tl->sdz += r1[2] - r0[2]; tl->sdt += dt;
+  }
+  el.x = r1[0]; el.y = r1[1]; el.z = r1[2]; el.t = t1; el.e = e1; el.kx = k1[0]; el.ky = k1[1]; el.kz = k1[2];
+  el.n = n_s + 1;
+  // S5: terminate at r' — bounds, then material, then time limit (R13: no back-projection)
+  double E1[3], m1;
+  int s1 = field_at(f, r1[0], r1[1], r1[2], E1, m1);
+  if (s1 < 0) { el.status = -s1; return; }
+  if (m1 < 0.5) { el.status = AVMO_MATERIAL; return; }
+  if (t1 > t_max) { el.status = AVMO_TIME_LIMIT; return; }
+  if (el.n >= N_STEP_LIMIT) { el.status = AVMO_STEP_LIMIT; return; }
+  // S6: energy bin (R5: piecewise constant, clamp and count)
+  const double sb = e1 * g.inv_de;
+  int b;
+  if (sb >= (double)g.nb) { b = g.nb - 1; if (tl) tl->n_overflow++; } else b = (int)sb;
+  so.bin = b;
+  const double* row = g.cum + (size_t)b * g.L;
+  // S7: null or real (R7: one uniform decides both)
+  const double xr = u2 * g.nu_hat;
+  if (xr >= row[g.L - 1]) { so.event = -1; if (tl) tl->n_null++; return; }
+  // S8: level = smallest index with cum[b][l] > x
+  int l = 0;
+  while (row[l] <= xr) ++l;
+  so.event = l;
+  if (tl) { tl->n_real++; tl->level[l]++; }
+  // S9a: attachment
+  if (g.type[l] == AVMO_ATTACHMENT) { el.status = AVMO_ATTACHED; return; }
+  // S9b: deflection angles
+  double u3, u4;
+  uniform_pair(seed, el.id, n_s, 1, u3, u4);
+  const double ct = 1.0 - 2.0 * u3;
+  const double st = 2.0 * std::sqrt(u3 * (1.0 - u3));
+  const double phi = TWO_PI * u4;
+  const double sphi = std::sin(phi), cphi = std::cos(phi);
+  // S9c: energy after the collision
+  double e2;
+  if (g.type[l] == AVMO_ELASTIC) {
+    e2 = e1 * (1.0 - g.recoil[l] * (1.0 - ct));                    // R9
+    if (tl) tl->sloss += e1 - e2;
+  } else if (g.type[l] == AVMO_EXCITATION) {
+    e2 = std::max(e1 - g.loss[l], EPS_FLOOR);                      // R11
+    if (tl) tl->sloss += e1 - e2;
+  } else {                                                         // ionisation, R10 (Opal-Peterson-Beaty)
+    double u5, u6, u7, u8;
+    uniform_pair(seed, el.id, n_s, 2, u5, u6);
+    uniform_pair(seed, el.id, n_s, 3, u7, u8);
+    const double ea = std::max(e1 - g.loss[l], 0.0);
+    const double w = g.w[l];
+    const double es = w * std::tan(u5 * std::atan(ea / (2.0 * w)));
+    e2 = std::max(ea - es, EPS_FLOOR);
+    Electron& c = so.c;
+    c.x = r1[0]; c.y = r1[1]; c.z = r1[2]; c.t = t1;
+    c.e = std::max(es, EPS_FLOOR);
+    const double sc = 2.0 * std::sqrt(u6 * (1.0 - u6));
+    const double pc = TWO_PI * u7;
+    c.kx = sc * std::cos(pc); c.ky = sc * std::sin(pc); c.kz = 1.0 - 2.0 * u6;
+    uint32_t wd[4];
+    philox_block(seed, el.id, n_s, BLOCK_CHILD_ID, wd);             // R16: schedule-independent child id
+    c.id = (uint64_t)wd[0] + ((uint64_t)wd[1] << 32);
+    c.n = 0; c.aval = el.aval; c.status = AVMO_ACTIVE;
+    c.birth[0] = c.x; c.birth[1] = c.y; c.birth[2] = c.z; c.birth[3] = c.t; c.birth[4] = c.e;
+    so.child = true;
+    if (tl) tl->sloss += e1 - e2 - c.e;
+  }
+  el.e = e2;
+  // S9d: new direction — branch-free orthonormal basis about k' (Duff et al. 2017), then renormalise
+  const double sg = std::copysign(1.0, k1[2]);
+  const double A = -1.0 / (sg + k1[2]);
+  const double Bq = k1[0] * k1[1] * A;
+  const double b1[3] = {1.0 + sg * k1[0] * k1[0] * A, sg * Bq, -sg * k1[0]};
+  const double b2[3] = {Bq, sg + k1[1] * k1[1] * A, -k1[1]};
+  double k2[3];
+  for (int i = 0; i < 3; ++i) k2[i] = ct * k1[i] + st * (cphi * b1[i] + sphi * b2[i]);
+  const double nk = std::sqrt(k2[0] * k2[0] + k2[1] * k2[1] + k2[2] * k2[2]);
+  el.kx = k2[0] / nk; el.ky = k2[1] / nk; el.kz = k2[2] / nk;
+}
+
+struct Record { Electron el; };
+
+// The avalanche driver: transport until status != 0, push newly created electrons, repeat.
+// Serial: one electron at a time from a stack.  Order is irrelevant because draws are keyed by (id, n).
+void run_range(const Gas& g, const avmo_field_desc* f, const double* prim, int64_t p0, int64_t p1, uint64_t seed,
+               double t_max, std::vector<Electron>& done, Tally& tl) {
+  std::vector<Electron> stack;
+  StepOut so;
+  for (int64_t p = p0; p < p1; ++p) {
+    const double* q = prim + p * 8;
+    Electron el;
+    el.x = q[0]; el.y = q[1]; el.z = q[2]; el.t = q[3]; el.e = std::max(q[4], EPS_FLOOR);
+    double nk = std::sqrt(q[5] * q[5] + q[6] * q[6] + q[7] * q[7]);
+    if (!(nk > 0)) { el.kx = 0; el.ky = 0; el.kz = 1; } else { el.kx = q[5] / nk; el.ky = q[6] / nk; el.kz = q[7] / nk; }
+    el.id = (uint64_t)p; el.n = 0; el.aval = (uint32_t)p; el.status = AVMO_ACTIVE;
+    el.birth[0] = el.x; el.birth[1] = el.y; el.birth[2] = el.z; el.birth[3] = el.t; el.birth[4] = el.e;
+    // a-1: reject out-of-domain primaries (status set, endpoint = birth point)
+    double E[3], m;
+    int si = field_at(f, el.x, el.y, el.z, E, m);
+    if (si < 0) el.status = -si;
+    else if (m < 0.5) el.status = AVMO_MATERIAL;
+    else if (el.t > t_max) el.status = AVMO_TIME_LIMIT;
+    stack.push_back(el);
+    while (!stack.empty()) {
+      Electron cur = stack.back();
+      stack.pop_back();
+      while (cur.status == AVMO_ACTIVE) {
+        step(g, f, seed, t_max, cur, so, &tl);
+        if (so.child) stack.push_back(so.c);
+      }
+      done.push_back(cur);
+    }
+  }
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* avmo_last_error(void) { return g_err.c_str(); }
+
+void avmo_philox(uint64_t seed, uint64_t id, uint32_t n, uint32_t block, uint32_t out[4]) { philox_block(seed, id, n, block, out); }
+
+void avmo_uniform_pair(uint64_t seed, uint64_t id, uint32_t n, uint32_t block, double out[2]) {
+  uniform_pair(seed, id, n, block, out[0], out[1]);
+}
+
+int32_t avmo_field_eval(const avmo_field_desc* f, int64_t n, const double* r, double* E, double* mask, int32_t* slab) {
+  if (!check_field(f) || n < 0 || !r || !E || !mask || !slab) return AVMO_ERR_INVALID_ARG;
+  for (int64_t i = 0; i < n; ++i) {
+    double e[3] = {0, 0, 0}, m = 0;
+    int si = field_at(f, r[i], r[n + i], r[2 * n + i], e, m);
+    E[i] = e[0]; E[n + i] = e[1]; E[2 * n + i] = e[2]; mask[i] = m; slab[i] = si < 0 ? -1 : si;
+  }
+  return AVMO_OK;
+}
+
+int32_t avmo_step_batch(const avmo_gas_desc* gd, const avmo_field_desc* f, uint64_t seed, double t_max, int64_t n,
+                        const double* in, const uint64_t* id, const uint32_t* n_idx, double* out, int32_t* event,
+                        int32_t* status, int32_t* bin, double* child, uint64_t* child_id) {
+  Gas g;
+  if (!load_gas(gd, g) || !check_field(f)) return AVMO_ERR_INVALID_ARG;
+  if (n < 0 || !in || !id || !n_idx || !out || !event || !status || !bin || !child || !child_id) { g_err = "step_batch: null"; return AVMO_ERR_INVALID_ARG; }
+  StepOut so;
+  for (int64_t i = 0; i < n; ++i) {
+    Electron el;
+    el.x = in[i]; el.y = in[n + i]; el.z = in[2 * n + i]; el.t = in[3 * n + i]; el.e = in[4 * n + i];
+    el.kx = in[5 * n + i]; el.ky = in[6 * n + i]; el.kz = in[7 * n + i];
+    el.id = id[i]; el.n = n_idx[i]; el.aval = 0; el.status = AVMO_ACTIVE;
+    step(g, f, seed, t_max, el, so, nullptr);
+    out[i] = el.x; out[n + i] = el.y; out[2 * n + i] = el.z; out[3 * n + i] = el.t; out[4 * n + i] = el.e;
+    out[5 * n + i] = el.kx; out[6 * n + i] = el.ky; out[7 * n + i] = el.kz;
+    event[i] = so.event; status[i] = el.status; bin[i] = so.bin;
+    for (int c = 0; c < 8; ++c) child[c * n + i] = 0.0;
+    child_id[i] = 0;
+    if (so.child) {
+      const Electron& c = so.c;
+      child[i] = c.x; child[n + i] = c.y; child[2 * n + i] = c.z; child[3 * n + i] = c.t; child[4 * n + i] = c.e;
+      child[5 * n + i] = c.kx; child[6 * n + i] = c.ky; child[7 * n + i] = c.kz;
+      child_id[i] = c.id;
+    }
+  }
+  return AVMO_OK;
+}
+
+int32_t avmo_run(const avmo_gas_desc* gd, const avmo_field_desc* f, const double* prim, int64_t np,
+                 const avmo_run_opts* opts, avmo_outputs* o, int64_t* n_out) {
+  Gas g;
+  if (!load_gas(gd, g) || !check_field(f)) return AVMO_ERR_INVALID_ARG;
+  if (np < 0 || (np > 0 && !prim) || !opts || !o || !n_out || o->capacity < 0) { g_err = "run: null/negative"; return AVMO_ERR_INVALID_ARG; }
+  if (np > 0xFFFFFFFFll) { g_err = "run: too many primaries"; return AVMO_ERR_INVALID_ARG; }
+  int nt = std::max(1, opts->n_threads);
+  nt = (int)std::min<int64_t>(nt, std::max<int64_t>(np, 1));
+  std::vector<std::vector<Electron>> done(nt);
+  std::vector<Tally> tl(nt);
+  for (auto& t : tl) t.level.assign(g.L, 0);
+  if (nt == 1) {
+    run_range(g, f, prim, 0, np, opts->seed, opts->t_max, done[0], tl[0]);
+  } else {                       // timed multi-core baseline only: disjoint primary ranges, identical results
+    std::vector<std::thread> th;
+    for (int t = 0; t < nt; ++t) {
+      int64_t p0 = np * t / nt, p1 = np * (t + 1) / nt;
+      th.emplace_back([&, t, p0, p1] { run_range(g, f, prim, p0, p1, opts->seed, opts->t_max, done[t], tl[t]); });
+    }
+    for (auto& x : th) x.join();
+  }
+  // outputs
+  int64_t total = 0;
+  for (auto& d : done) total += (int64_t)d.size();
+  const int64_t cap = o->capacity;
+  if (o->per_avalanche) std::memset(o->per_avalanche, 0, sizeof(uint64_t) * 3 * (size_t)np);
+  int64_t w = 0;
+  for (auto& d : done)
+    for (auto& el : d) {
+      if (o->per_avalanche) {                 // a-12 / C11: ions = ionisations = endpoints - 1 per avalanche
+        o->per_avalanche[3 * (size_t)el.aval + 0]++;
+        if (el.status == AVMO_ATTACHED) o->per_avalanche[3 * (size_t)el.aval + 2]++;
+      }
+      if (w >= cap) { ++w; continue; }
+      if (o->id) o->id[w] = el.id;
+      if (o->avalanche) o->avalanche[w] = el.aval;
+      if (o->status) o->status[w] = el.status;
+      if (o->n_steps) o->n_steps[w] = el.n;
+      if (o->birth) for (int c = 0; c < 5; ++c) o->birth[c * cap + w] = el.birth[c];
+      if (o->end) {
+        const double e8[8] = {el.x, el.y, el.z, el.t, el.e, el.kx, el.ky, el.kz};
+        for (int c = 0; c < 8; ++c) o->end[c * cap + w] = e8[c];
+      }
+      ++w;
+    }
+  if (o->per_avalanche)
+    for (int64_t p = 0; p < np; ++p) o->per_avalanche[3 * p + 1] = o->per_avalanche[3 * p] > 0 ? o->per_avalanche[3 * p] - 1 : 0;
+  if (o->tallies_u64) {
+    for (int l = 0; l < g.L + 4; ++l) o->tallies_u64[l] = 0;
+    for (auto& t : tl) {
+      for (int l = 0; l < g.L; ++l) o->tallies_u64[l] += t.level[l];
+      o->tallies_u64[g.L] += t.n_null; o->tallies_u64[g.L + 1] += t.n_real;
+      o->tallies_u64[g.L + 2] += t.n_overflow; o->tallies_u64[g.L + 3] += t.n_steps;
+    }
+  }
+  if (o->tallies_f64) {
+    for (int c = 0; c < 5; ++c) o->tallies_f64[c] = 0;
+    for (auto& t : tl) {
+      o->tallies_f64[0] += t.sdx; o->tallies_f64[1] += t.sdy; o->tallies_f64[2] += t.sdz;
+      o->tallies_f64[3] += t.sdt; o->tallies_f64[4] += t.sloss;
+    }
+  }
+  *n_out = std::min(total, cap);
+  if (total > cap) { g_err = "run: capacity exceeded"; return AVMO_ERR_CAPACITY; }
+  return AVMO_OK;
+}
+
+}  // extern "C"

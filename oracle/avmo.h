@@ -1,0 +1,91 @@
+/* avmo — the ORACLE: plain, serial, slow, obviously-correct CPU implementation of microscopic electron
+ * avalanche transport (null-collision Monte Carlo).  TEST INFRASTRUCTURE ONLY: used by tests/,
+ * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs.  It shares no code with the
+ * CUDA path (paper_2509_15377_b200/csrc/) and the product never routes through it.
+ *
+ * What it follows.  The paper (arxiv 2509.15377, /root/reference/PAPER.md) describes the algorithm only in
+ * outline: "electron transport" for every active electron, then "stack processing", until every electron
+ * has a non-zero status (Fig. 2 at PAPER.md:89); it names its method's sources as the
+ * semi-classical null-collision Monte Carlo technique (ref [8]) over per-process cross
+ * sections (ref [9]).  Every numeric choice the paper leaves open is fixed by the readings
+ * R1-R20 and steps S0-S9 of SURVEY.md §8(c), restated in DESIGN.md §3; the functions below cite them.
+ *
+ * Units: cm, ns, eV, V/cm, tesla.  All arithmetic fp64; grid nodes are fp32 storage, fp64 arithmetic.
+ * All pointers are HOST pointers.  Parity status of each function: see DESIGN.md §5 (pins C1-C17);
+ * absolute values of the synthetic-gas results (gain, alpha, W of configs 1-5) are "parity unpinned"
+ * (no reference values exist anywhere) — they are pinned GPU-vs-oracle only.
+ */
+#ifndef AVMO_H
+#define AVMO_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { AVMO_OK = 0, AVMO_ERR_INVALID_ARG = -1, AVMO_ERR_CAPACITY = -2 };
+enum { AVMO_ELASTIC = 0, AVMO_EXCITATION = 1, AVMO_IONISATION = 2, AVMO_ATTACHMENT = 3 };
+enum { AVMO_ACTIVE = 0, AVMO_LEFT_ZLO = 1, AVMO_LEFT_ZHI = 2, AVMO_LEFT_XY = 3, AVMO_MATERIAL = 4,
+       AVMO_ATTACHED = 5, AVMO_TIME_LIMIT = 6, AVMO_STEP_LIMIT = 7 };
+
+typedef struct {
+  int32_t n_bins;  double e_max_eV;
+  int32_t n_levels;
+  const double*  cum_rate;        /* [n_bins][n_levels] ns^-1, non-decreasing along levels */
+  const uint8_t* level_type;
+  const double*  level_loss_eV;
+  const double*  level_recoil;
+  const double*  level_ob_w_eV;
+  double nu_hat;                  /* <= 0: max_b cum_rate[b][L-1] */
+} avmo_gas_desc;
+
+typedef struct {
+  double z_lo, z_hi;  int32_t kind;           /* 0 uniform, 1 grid */
+  double E[3];
+  const float* nodes;                          /* grid: [nz][ny][nx][4] = Ex,Ey,Ez,mask */
+  int32_t nx, ny, nz;  double origin[3], spacing[3];
+  int32_t bc_x, bc_y;                          /* 0 none, 1 periodic, 2 mirror */
+  double period_x, period_y;
+} avmo_slab;
+
+typedef struct { const avmo_slab* slabs; int32_t n_slabs; double B[3]; double xy_lo[2], xy_hi[2]; } avmo_field_desc;
+
+typedef struct { uint64_t seed; double t_max; int32_t n_threads; } avmo_run_opts;
+
+typedef struct {
+  int64_t capacity;
+  uint64_t* id; uint32_t* avalanche; int32_t* status; uint32_t* n_steps;
+  double* birth;            /* [5][capacity]: x0,y0,z0,t0,e0 */
+  double* end;              /* [8][capacity]: x1,y1,z1,t1,e1,kx,ky,kz */
+  uint64_t* per_avalanche;  /* [Np][3]: endpoints, ions, negative ions */
+  uint64_t* tallies_u64;    /* [n_levels+4]: per level, null, real, overflow, steps */
+  double*   tallies_f64;    /* [5]: sum dx,dy,dz over all flights, sum dt, sum energy loss */
+} avmo_outputs;
+
+/* Philox4x32-10 block for (seed, electron id, collision index n, block) -> 4 words / 2 uniforms. */
+void avmo_philox(uint64_t seed, uint64_t id, uint32_t n, uint32_t block, uint32_t out[4]);
+void avmo_uniform_pair(uint64_t seed, uint64_t id, uint32_t n, uint32_t block, double out[2]);
+
+/* Field at n points r[3][n] -> E[3][n], mask[n], slab[n] (-1 outside the domain / bounds). */
+int32_t avmo_field_eval(const avmo_field_desc*, int64_t n, const double* r, double* E, double* mask, int32_t* slab);
+
+/* One step S0-S9 each from given states (state [8][n] = x,y,z,t,e,kx,ky,kz).  Outputs: state_out [8][n];
+ * event[n]: -1 null collision, l>=0 selected level, -2 terminated before the collision decision;
+ * status[n]; bin[n] (-1 if not reached); child [8][n] + child_id[n] valid where level type is ionisation. */
+int32_t avmo_step_batch(const avmo_gas_desc*, const avmo_field_desc*, uint64_t seed, double t_max, int64_t n,
+                        const double* state_in, const uint64_t* id, const uint32_t* n_idx,
+                        double* state_out, int32_t* event, int32_t* status, int32_t* bin,
+                        double* child_out, uint64_t* child_id);
+
+/* Whole avalanches: stack driver.  primaries: [Np][8] AoS.  Returns AVMO_ERR_CAPACITY when more than
+ * `capacity` electrons are created (outputs then hold the first `capacity` finished ones). */
+int32_t avmo_run(const avmo_gas_desc*, const avmo_field_desc*, const double* primaries, int64_t n_primaries,
+                 const avmo_run_opts*, avmo_outputs*, int64_t* n_endpoints_out);
+
+const char* avmo_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

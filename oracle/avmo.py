@@ -1,0 +1,205 @@
+"""ctypes binding of the ORACLE (oracle/avmo.cpp).  TEST INFRASTRUCTURE: imported only by tests/,
+__graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs — never by the product package.
+
+`build()` compiles oracle/libavmo.so with g++ -O2 -ffp-contract=off (building the checker is not using it).
+Inputs are the plain-data descriptions of paper_2509_15377_b200.gen (GasTable, FieldDesc) and numpy arrays.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libavmo.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    src = os.path.join(_HERE, "avmo.cpp")
+    hdr = os.path.join(_HERE, "avmo.h")
+    if not force and os.path.exists(_SO) and os.path.getmtime(_SO) >= max(os.path.getmtime(src), os.path.getmtime(hdr)):
+        return _SO
+    cmd = ["g++", "-O2", "-ffp-contract=off", "-std=c++17", "-shared", "-fPIC", "-pthread", "-o", _SO, src]
+    subprocess.run(cmd, check=True, cwd=_HERE)
+    return _SO
+
+
+class GasDesc(C.Structure):
+    _fields_ = [("n_bins", C.c_int32), ("e_max_eV", C.c_double), ("n_levels", C.c_int32),
+                ("cum_rate", C.c_void_p), ("level_type", C.c_void_p), ("level_loss_eV", C.c_void_p),
+                ("level_recoil", C.c_void_p), ("level_ob_w_eV", C.c_void_p), ("nu_hat", C.c_double)]
+
+
+class SlabDesc(C.Structure):
+    _fields_ = [("z_lo", C.c_double), ("z_hi", C.c_double), ("kind", C.c_int32), ("E", C.c_double * 3),
+                ("nodes", C.c_void_p), ("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
+                ("origin", C.c_double * 3), ("spacing", C.c_double * 3), ("bc_x", C.c_int32), ("bc_y", C.c_int32),
+                ("period_x", C.c_double), ("period_y", C.c_double)]
+
+
+class FieldDescC(C.Structure):
+    _fields_ = [("slabs", C.POINTER(SlabDesc)), ("n_slabs", C.c_int32), ("B", C.c_double * 3),
+                ("xy_lo", C.c_double * 2), ("xy_hi", C.c_double * 2)]
+
+
+class RunOpts(C.Structure):
+    _fields_ = [("seed", C.c_uint64), ("t_max", C.c_double), ("n_threads", C.c_int32)]
+
+
+class Outputs(C.Structure):
+    _fields_ = [("capacity", C.c_int64), ("id", C.c_void_p), ("avalanche", C.c_void_p), ("status", C.c_void_p),
+                ("n_steps", C.c_void_p), ("birth", C.c_void_p), ("end", C.c_void_p), ("per_avalanche", C.c_void_p),
+                ("tallies_u64", C.c_void_p), ("tallies_f64", C.c_void_p)]
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = C.CDLL(_SO)
+        _lib.avmo_last_error.restype = C.c_char_p
+        _lib.avmo_run.restype = C.c_int32
+        _lib.avmo_step_batch.restype = C.c_int32
+        _lib.avmo_field_eval.restype = C.c_int32
+    return _lib
+
+
+def _p(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+class _Keep:
+    """Holds the numpy arrays a C descriptor points into."""
+
+    def __init__(self):
+        self.refs = []
+
+
+def gas_desc(gas) -> tuple:
+    k = _Keep()
+    cum = np.ascontiguousarray(gas.cum_rate, dtype=np.float64)
+    ty = np.ascontiguousarray(gas.level_type, dtype=np.uint8)
+    lo = np.ascontiguousarray(gas.level_loss, dtype=np.float64)
+    rc = np.ascontiguousarray(gas.level_recoil, dtype=np.float64)
+    w = np.ascontiguousarray(gas.level_ob_w, dtype=np.float64)
+    k.refs += [cum, ty, lo, rc, w]
+    d = GasDesc(int(gas.n_bins), float(gas.e_max), int(cum.shape[1]), _p(cum).value, _p(ty).value, _p(lo).value,
+                _p(rc).value, _p(w).value, float(gas.nu_hat))
+    return d, k
+
+
+def field_desc(field) -> tuple:
+    k = _Keep()
+    n = len(field.slabs)
+    arr = (SlabDesc * n)()
+    for i, s in enumerate(field.slabs):
+        a = arr[i]
+        a.z_lo, a.z_hi, a.kind = s.z_lo, s.z_hi, s.kind
+        a.E[:] = s.E
+        if s.nodes is not None:
+            nodes = np.ascontiguousarray(s.nodes, dtype=np.float32)
+            k.refs.append(nodes)
+            a.nodes = _p(nodes).value
+            a.nz, a.ny, a.nx = nodes.shape[:3]
+        a.origin[:] = s.origin
+        a.spacing[:] = s.spacing
+        a.bc_x, a.bc_y, a.period_x, a.period_y = s.bc_x, s.bc_y, s.period_x, s.period_y
+    k.refs.append(arr)
+    d = FieldDescC(arr, n, (C.c_double * 3)(*field.B), (C.c_double * 2)(*field.xy_lo), (C.c_double * 2)(*field.xy_hi))
+    return d, k
+
+
+def philox(seed, ident, n, block) -> np.ndarray:
+    out = (C.c_uint32 * 4)()
+    lib().avmo_philox(C.c_uint64(seed), C.c_uint64(ident), C.c_uint32(n), C.c_uint32(block), out)
+    return np.array(out[:], dtype=np.uint32)
+
+
+def uniform_pair(seed, ident, n, block):
+    out = (C.c_double * 2)()
+    lib().avmo_uniform_pair(C.c_uint64(seed), C.c_uint64(ident), C.c_uint32(n), C.c_uint32(block), out)
+    return out[0], out[1]
+
+
+def field_eval(field, r):
+    """r: [3, n] -> E [3, n], mask [n], slab [n]."""
+    r = np.ascontiguousarray(r, dtype=np.float64)
+    n = r.shape[1]
+    E = np.zeros((3, n)); m = np.zeros(n); sl = np.zeros(n, dtype=np.int32)
+    fd, _k = field_desc(field)
+    rc = lib().avmo_field_eval(C.byref(fd), C.c_int64(n), _p(r), _p(E), _p(m), _p(sl))
+    if rc != 0:
+        raise RuntimeError(lib().avmo_last_error().decode())
+    return E, m, sl
+
+
+@dataclass
+class StepResult:
+    state: np.ndarray      # [8, n]
+    event: np.ndarray
+    status: np.ndarray
+    bin: np.ndarray
+    child: np.ndarray      # [8, n]
+    child_id: np.ndarray
+
+
+def step_batch(gas, field, seed, state, ids, n_idx, t_max=float("inf")) -> StepResult:
+    state = np.ascontiguousarray(state, dtype=np.float64)
+    n = state.shape[1]
+    ids = np.ascontiguousarray(ids, dtype=np.uint64)
+    n_idx = np.ascontiguousarray(n_idx, dtype=np.uint32)
+    out = np.zeros((8, n)); ev = np.zeros(n, dtype=np.int32); st = np.zeros(n, dtype=np.int32)
+    bn = np.zeros(n, dtype=np.int32); ch = np.zeros((8, n)); cid = np.zeros(n, dtype=np.uint64)
+    gd, _kg = gas_desc(gas)
+    fd, _kf = field_desc(field)
+    rc = lib().avmo_step_batch(C.byref(gd), C.byref(fd), C.c_uint64(seed), C.c_double(t_max), C.c_int64(n), _p(state),
+                               _p(ids), _p(n_idx), _p(out), _p(ev), _p(st), _p(bn), _p(ch), _p(cid))
+    if rc != 0:
+        raise RuntimeError(lib().avmo_last_error().decode())
+    return StepResult(out, ev, st, bn, ch, cid)
+
+
+@dataclass
+class RunResult:
+    n: int
+    id: np.ndarray
+    avalanche: np.ndarray
+    status: np.ndarray
+    n_steps: np.ndarray
+    birth: np.ndarray           # [5, n]
+    end: np.ndarray             # [8, n]
+    per_avalanche: np.ndarray   # [Np, 3]
+    tallies_u64: np.ndarray     # [L+4]
+    tallies_f64: np.ndarray     # [5]
+    rc: int = 0
+
+    def sorted_by_id(self):
+        o = np.argsort(self.id, kind="stable")
+        return RunResult(self.n, self.id[o], self.avalanche[o], self.status[o], self.n_steps[o], self.birth[:, o],
+                         self.end[:, o], self.per_avalanche, self.tallies_u64, self.tallies_f64, self.rc)
+
+
+def run(gas, field, primaries, seed=0, t_max=float("inf"), capacity=None, n_threads=1, allow_overflow=False) -> RunResult:
+    prim = np.ascontiguousarray(primaries, dtype=np.float64)
+    np_ = prim.shape[0]
+    cap = int(capacity if capacity is not None else max(4 * np_, 1 << 16))
+    L = gas.n_levels
+    ident = np.zeros(cap, dtype=np.uint64); av = np.zeros(cap, dtype=np.uint32); st = np.zeros(cap, dtype=np.int32)
+    ns = np.zeros(cap, dtype=np.uint32); birth = np.zeros((5, cap)); end = np.zeros((8, cap))
+    pa = np.zeros((max(np_, 1), 3), dtype=np.uint64); tu = np.zeros(L + 4, dtype=np.uint64); tf = np.zeros(5)
+    gd, _kg = gas_desc(gas)
+    fd, _kf = field_desc(field)
+    o = Outputs(cap, _p(ident), _p(av), _p(st), _p(ns), _p(birth), _p(end), _p(pa), _p(tu), _p(tf))
+    opts = RunOpts(int(seed), float(t_max), int(n_threads))
+    n_out = C.c_int64(0)
+    rc = lib().avmo_run(C.byref(gd), C.byref(fd), _p(prim), C.c_int64(np_), C.byref(opts), C.byref(o), C.byref(n_out))
+    if rc == -2 and not allow_overflow:
+        raise MemoryError("oracle: capacity exceeded")
+    if rc not in (0, -2):
+        raise RuntimeError(lib().avmo_last_error().decode())
+    n = n_out.value
+    return RunResult(n, ident[:n], av[:n], st[:n], ns[:n], birth[:, :n], end[:, :n], pa[:np_], tu, tf, rc)
