@@ -1,0 +1,188 @@
+/* avm.h — C ABI of libavm: microscopic (collision-by-collision) electron avalanche transport on one B200.
+ *
+ * What the library computes.  The hot path of the paper "Accelerating Garfield++ with CUDA"
+ * (arxiv 2509.15377, PAPER.md): for every active electron an "electron transport" stage, then "stack
+ * processing" (finished electrons removed, newly created ones added), repeated until every electron has a
+ * non-zero status code (Fig. 2 at PAPER.md:89).  The transport stage is the semi-classical
+ * null-collision Monte Carlo technique the paper names as its method's source (refs [8], [9] at
+ * PAPER.md:189-190).  The paper prints no equations; every numeric choice is fixed by readings R1-R20 and
+ * steps S0-S9 of SURVEY.md §8(c), restated in DESIGN.md §3.
+ *
+ * Conventions.
+ *  - Units: cm, ns, eV, V/cm, tesla.  All arithmetic fp64; grid-map nodes are fp32 storage, fp64 arithmetic.
+ *  - Every function returns int32_t: AVM_OK or a negative AVM_ERR_*; avm_last_error() gives a thread-local
+ *    message.  No exception crosses the boundary.
+ *  - The library NEVER allocates device memory and has no CPU fallback: the caller provides every device
+ *    buffer and the CUDA stream (PyTorch in this repo: torch.empty(..., device="cuda"), stream handle).
+ *  - "host" / "device" is stated for every pointer.  Host arrays are borrowed for the duration of the call;
+ *    device buffers given at creation are borrowed until the matching destroy.
+ *  - Work is enqueued on the context's stream.  avm_run and avm_fetch synchronise that stream before they
+ *    return (a count is returned to the host); avm_step_batch and avm_field_eval do not.
+ *  - Random numbers: counter-based Philox4x32-10, counter = (n, block, id_lo, id_hi), key = (seed_lo,
+ *    seed_hi); n = the electron's collision index, id = its 64-bit id.  This replaces the paper's
+ *    pre-generated numbers selected by electron ID: results do not depend on scheduling.
+ */
+#ifndef AVM_H
+#define AVM_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { AVM_OK = 0, AVM_ERR_INVALID_ARG = -1, AVM_ERR_CAPACITY = -2, AVM_ERR_CUDA = -3, AVM_ERR_STATE = -4 };
+/* collision level types */
+enum { AVM_ELASTIC = 0, AVM_EXCITATION = 1, AVM_IONISATION = 2, AVM_ATTACHMENT = 3 };
+/* electron status codes: "non-zero status code" = finished */
+enum { AVM_ACTIVE = 0, AVM_LEFT_ZLO = 1, AVM_LEFT_ZHI = 2, AVM_LEFT_XY = 3, AVM_MATERIAL = 4,
+       AVM_ATTACHED = 5, AVM_TIME_LIMIT = 6, AVM_STEP_LIMIT = 7 };
+enum { AVM_MAX_LEVELS = 64, AVM_MAX_SLABS = 8 };
+
+typedef struct avm_ctx avm_ctx;
+typedef struct avm_gas avm_gas;
+typedef struct avm_field avm_field;
+
+/* Thread-local message of the last failing call on this thread ("" if none). */
+const char* avm_last_error(void);
+
+/* ---- context: "run on a chosen GPU" (SetRunModeOptions(mode, device)) ----------------
+ * device: CUDA ordinal.  cuda_stream: a cudaStream_t (NULL = the legacy default stream).  The context
+ * records device properties (SM count) used to size the persistent grid.  Fails with AVM_ERR_CUDA when the
+ * device is missing or is not compute capability 10.x. */
+int32_t avm_ctx_create(int32_t device, void* cuda_stream, avm_ctx** out);
+int32_t avm_ctx_destroy(avm_ctx*);
+/* Number of SMs of the context's device (grid sizing; reported by the bench). */
+int32_t avm_ctx_sm_count(const avm_ctx*);
+
+/* ---- gas: cumulative collision-rate tables ("GPU versions" of the Medium data; S6-S9) -------
+ * All pointers HOST.  cum_rate[b][l] = sum of the rates [ns^-1] of levels 0..l in energy bin b; bins are
+ * uniform on [0, e_max), bin = floor(e * n_bins / e_max), energies >= e_max use the last bin and are
+ * counted (R5).  Rates are piecewise constant per bin.  nu_hat is the null-collision rate (R4); it must be
+ * >= every cum_rate[b][n_levels-1]; <= 0 selects that maximum. */
+typedef struct {
+  int32_t n_bins;
+  double e_max_eV;
+  int32_t n_levels;               /* 1..AVM_MAX_LEVELS */
+  const double* cum_rate;         /* host [n_bins][n_levels], non-decreasing along levels */
+  const uint8_t* level_type;      /* host [n_levels], AVM_ELASTIC.. */
+  const double* level_loss_eV;    /* host [n_levels]: threshold = energy loss (excitation, ionisation) */
+  const double* level_recoil;     /* host [n_levels]: r = 2mM/(m+M)^2 (elastic) */
+  const double* level_ob_w_eV;    /* host [n_levels]: Opal-Beaty w (ionisation) */
+  double nu_hat;
+} avm_gas_desc;
+/* Bytes of device memory avm_gas_create needs for this table (0 on an invalid description). */
+size_t avm_gas_bytes(const avm_gas_desc*);
+/* Validates the table, lays it out in dev_buf (DEVICE, >= avm_gas_bytes, 256-byte aligned; borrowed until
+ * avm_gas_destroy) and uploads it on the context's stream.  Layout: DESIGN.md §4. */
+int32_t avm_gas_create(avm_ctx*, const avm_gas_desc*, void* dev_buf, size_t dev_bytes, avm_gas** out);
+int32_t avm_gas_destroy(avm_gas*);
+/* The resolved null-collision rate [ns^-1]. */
+double avm_gas_nu_hat(const avm_gas*);
+
+/* ---- field: uniform, uniform + B, or regular-grid map(s) (S0, R14, R15) ---------------------------------
+ * A stack of z-slabs, ascending and contiguous (slab[i].z_hi == slab[i+1].z_lo).  kind 0: uniform field
+ * vector E (the force on an electron is -E).  kind 1: regular grid of float4 nodes (Ex, Ey, Ez, gas-mask)
+ * laid out [nz][ny][nx][4], trilinear interpolation (x, then y, then z); mask < 0.5 = solid material, the
+ * electron is absorbed (R14).  bc 0: leaving the grid in x/y ends the electron (status 3); 1: periodic with
+ * the given period; 2: mirror-periodic — fold into [0, period], the field component normal to the mirror
+ * changes sign (R15).  B is one constant vector for the whole run (exact helical flight when non-zero).
+ * xy_lo/xy_hi: absorbing bounds in x and y (+-inf allowed). */
+typedef struct {
+  double z_lo, z_hi;
+  int32_t kind;
+  double E[3];
+  const float* nodes_dev;         /* DEVICE [nz][ny][nx][4], 16-byte aligned, borrowed until avm_field_destroy */
+  int32_t nx, ny, nz;
+  double origin[3], spacing[3];
+  int32_t bc_x, bc_y;
+  double period_x, period_y;
+} avm_slab;
+typedef struct {
+  const avm_slab* slabs;          /* host [n_slabs], 1..AVM_MAX_SLABS */
+  int32_t n_slabs;
+  double B[3];
+  double xy_lo[2], xy_hi[2];
+} avm_field_desc;
+int32_t avm_field_create(avm_ctx*, const avm_field_desc*, avm_field** out);
+int32_t avm_field_destroy(avm_field*);
+/* Field and gas-mask at n points.  r: DEVICE [3][n]; E: DEVICE [3][n]; mask: DEVICE [n]; slab: DEVICE [n]
+ * (-1 = outside the domain).  Asynchronous on the context's stream. */
+int32_t avm_field_eval(avm_ctx*, const avm_field*, int64_t n, const double* r, double* E, double* mask,
+                       int32_t* slab);
+
+/* ---- run: whole avalanches --------------------------------------------------------------
+ * Primaries: [n_primaries][8] = x, y, z, t, energy, kx, ky, kz (AoS).  HOST by default (the H2D copy is part
+ * of the call, as in the paper's timing convention); DEVICE with AVM_RUN_PRIMARIES_ON_DEVICE.
+ * Primary p gets id = p + id_offset and avalanche index p; secondaries get id = Philox(n_s, 0xFFFFFFFF, parent
+ * id) (R16) and inherit the avalanche index.  A primary outside the domain / inside material is finished at
+ * its birth point with the corresponding status. */
+enum { AVM_RUN_PRIMARIES_ON_DEVICE = 1u, AVM_RUN_NO_TALLIES = 2u };
+typedef struct {
+  uint64_t seed;
+  double t_max;                   /* ns; electrons with t > t_max stop with status 6 (+inf: none) */
+  uint32_t flags;
+  uint32_t max_iters_per_launch;  /* guard on the persistent kernel's loop (0 = default); the host relaunches */
+  uint64_t id_offset;             /* id of primary 0 (replicas / shards of one job use disjoint ranges) */
+  int32_t n_ctas_per_sm;          /* 0 = default */
+} avm_run_opts;
+
+/* Caller-provided DEVICE buffers; `capacity` = maximum number of electrons ever created (primaries +
+ * secondaries).  Slot s holds electron s for the whole run: while the electron is active its `end` column
+ * is its live state, afterwards its endpoint.  Slots are in creation order (primaries first); the order of
+ * secondaries is unspecified (compare after sorting by id, R17).  id, avalanche, status, n_steps and end are
+ * required; per_avalanche and tallies_* may be NULL; birth may be NULL only when tallies_f64 is NULL too
+ * (the flight sums are taken as sum over electrons of endpoint - birth point). */
+typedef struct {
+  int64_t capacity;
+  void* workspace;                /* DEVICE, >= avm_run_workspace_bytes(capacity), 256-byte aligned */
+  size_t workspace_bytes;
+  uint64_t* id;                   /* [capacity] */
+  uint32_t* avalanche;            /* [capacity] */
+  int32_t* status;                /* [capacity] */
+  uint32_t* n_steps;              /* [capacity] collision index n reached (real + null steps taken) */
+  double* birth;                  /* [5][capacity]: x0, y0, z0, t0, e0; may be NULL */
+  double* end;                    /* [8][capacity]: x1, y1, z1, t1, e1, kx, ky, kz */
+  uint64_t* per_avalanche;        /* [n_primaries][3]: endpoints, ions (= endpoints - 1), negative ions; may be NULL */
+  uint64_t* tallies_u64;          /* [n_levels + 4]: per level, null, real, energy overflow, steps; may be NULL */
+  double* tallies_f64;            /* [5]: sum dx, dy, dz over all flights, sum dt, sum energy loss; may be NULL */
+} avm_outputs;
+size_t avm_run_workspace_bytes(const avm_ctx*, int64_t capacity);
+/* Runs all avalanches to completion.  *n_endpoints_out = electrons created = endpoints written (<= capacity).
+ * AVM_ERR_CAPACITY: more than `capacity` electrons would exist; the run still terminates, outputs hold the
+ * electrons that fit (children that did not fit are dropped and counted in the message). */
+int32_t avm_run(avm_ctx*, const avm_gas*, const avm_field*, const double* primaries, int64_t n_primaries,
+                const avm_run_opts*, const avm_outputs*, int64_t* n_endpoints_out);
+/* Launch statistics of the last avm_run on this context: kernels launched, persistent-kernel launches. */
+int32_t avm_run_stats(const avm_ctx*, int64_t* n_kernel_launches, int64_t* n_transport_launches);
+
+/* Device -> host copy of the first n entries of every non-NULL array of `host` from the same-named array of
+ * `dev` ("retrieve the electron endpoints").  `host` is an avm_outputs whose pointers are HOST
+ * arrays with leading dimension host->capacity (workspace ignored); per_avalanche needs n_primaries,
+ * tallies_u64 needs n_levels (0 skips them).  Synchronises the stream. */
+int32_t avm_fetch(avm_ctx*, const avm_outputs* dev, int64_t n, int64_t n_primaries, int32_t n_levels,
+                  const avm_outputs* host);
+
+/* ---- parity hook: ONE step S0-S9 from each of n given states (no loop, no append) -----------------------
+ * All arrays DEVICE, length n ([8][n] for states = x,y,z,t,e,kx,ky,kz).  event: -1 null collision, l >= 0
+ * selected level, -2 terminated before the collision decision.  status: as above.  bin: energy bin used
+ * (-1 if not reached).  child/child_id: valid where the level is an ionisation, else zero. */
+int32_t avm_step_batch(avm_ctx*, const avm_gas*, const avm_field*, uint64_t seed, double t_max, int64_t n,
+                       const double* state_in, const uint64_t* id, const uint32_t* n_idx, double* state_out,
+                       int32_t* event, int32_t* status, int32_t* bin, double* child_out, uint64_t* child_id);
+
+/* Philox block (seed, id, n, block) -> words[4] and two uniforms, for n_items items.  All arrays DEVICE.
+ * Pin C1: lets the tests compare the device generator bit for bit. */
+int32_t avm_philox_batch(avm_ctx*, uint64_t seed, int64_t n_items, const uint64_t* id, const uint32_t* n_idx,
+                         const uint32_t* block, uint32_t* words_out /*[n_items][4]*/, double* u_out /*[n_items][2]*/);
+
+/* FP64 issue-rate probe: runs a chain of dependent-free DFMA streams (n_threads threads, iters iterations of
+ * 8 independent FMAs each) and writes the elapsed milliseconds; used by bench.py to measure the ALU roofline
+ * denominator on the box it runs on.  sink: DEVICE [n_threads] doubles. */
+int32_t avm_fp64_probe(avm_ctx*, int32_t n_blocks, int32_t n_threads_per_block, int64_t iters, double* sink,
+                       float* ms_out /*host*/);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,848 @@
+// avm.cu — kernels and the C ABI of libavm (include/avm.h) for sm_100a.
+//
+// Design: one persistent transport kernel.  Every electron owns a slot of the caller's SoA
+// output arrays for the whole run (live state while active, endpoint afterwards), so "stack processing"
+// moves no data: a finished electron frees its lane, a new one is appended by a
+// warp-aggregated atomic on the packed counter (total << 32 | done), and idle lanes pick up work through
+// tickets (lane holding ticket s runs the electron in slot s as soon as its status flag is published).
+// The run ends when done == total.  State stays in registers between collisions.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "avm_device.cuh"
+
+using namespace avm;
+
+namespace {
+
+thread_local std::string g_err;
+
+int32_t fail(int32_t code, const std::string& msg) { g_err = msg; return code; }
+#define AVM_CUDA(call)                                                                                  \
+  do {                                                                                                  \
+    cudaError_t e_ = (call);                                                                            \
+    if (e_ != cudaSuccess) return fail(AVM_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); \
+  } while (0)
+
+constexpr int kThreads = 256;          // threads per CTA of the transport kernel
+constexpr int kMinCtasPerSm = 2;       // register budget: 65536 / (256 * 2) = 128 registers per thread
+constexpr uint32_t kDefaultMaxIters = 1u << 16;
+constexpr int64_t kStageElectrons = 1 << 18;   // primaries staged per H2D chunk (16 MiB)
+constexpr size_t kCtlBytes = 4096;
+
+struct RunArrays {
+  uint32_t cap;
+  uint64_t* id;
+  uint32_t* aval;
+  int32_t* status;
+  uint32_t* nsteps;
+  double* birth;   // [5][cap] or null
+  double* end;     // [8][cap]
+};
+
+struct RunCtl {
+  unsigned long long counters;   // (electrons created << 32) | electrons finished
+  unsigned int q_head;           // tickets handed out beyond the static ones
+  unsigned int dropped;          // children that did not fit in `capacity`
+  unsigned long long n_null, n_real, n_overflow, n_steps;
+  unsigned long long level[AVM_MAX_LEVELS];
+  double sum_loss;
+  double sum_d[4];               // sum over electrons of (end - birth): dx, dy, dz, dt
+};
+static_assert(sizeof(RunCtl) <= kCtlBytes, "ctl block");
+
+__device__ __forceinline__ int ld_volatile_s32(const int* p) { return *(const volatile int*)p; }
+__device__ __forceinline__ unsigned long long ld_volatile_u64(const unsigned long long* p) {
+  return *(const volatile unsigned long long*)p;
+}
+
+// ---- one step S0-S9 in velocity form -------------------------------------------------------------------
+struct StepOut {
+  int event;        // -1 null, l >= 0 level, -2 terminated before the decision
+  int bin;
+  int status;       // 0 or the finishing status
+  bool spawn, overflow;
+  Child ch;
+  double e;         // energy after the step (e' for null/terminated, e'' after a collision)
+  double s2;        // |v'|^2 after the flight
+  double kx, ky, kz;  // direction after a real, non-attaching collision (else untouched)
+  double loss;
+};
+
+// In: electron (r, t, v, id, n) with the field (Ex,Ey,Ez) at r.  Out: state after the step; (Ex,Ey,Ez) = the
+// field at the new position (valid when status == 0), which is the next step's S0 (same point, R3).
+template <bool UNIFORM1, bool HASB>
+__device__ __forceinline__ void step_core(const DevGas& g, const DevField& f, const uint8_t* lv_type,
+                                          const double* lv_loss, const double* lv_recoil, const double* lv_w,
+                                          uint64_t seed, double t_max, uint64_t id, uint32_t& n, double& x, double& y,
+                                          double& z, double& t, double& vx, double& vy, double& vz, double& Ex,
+                                          double& Ey, double& Ez, StepOut& o) {
+  o.event = -2; o.bin = -1; o.status = 0; o.spawn = false; o.overflow = false; o.loss = 0.0;
+  const uint32_t n_s = n;                                   // S1
+  const U4 r0 = philox(seed, id, n_s, 0u);
+  const double u1 = to_unit(r0.w0, r0.w1), u2 = to_unit(r0.w2, r0.w3);
+  const double dt = -log(u1) * g.inv_nu_hat;                // S2
+  flight<HASB>(f, Ex, Ey, Ez, dt, x, y, z, vx, vy, vz);     // S3
+  const double s2 = vx * vx + vy * vy + vz * vz;            // S4
+  const double e1 = fmax(s2 * kInvC2Sq, kEpsFloor);
+  t = t + dt;
+  n = n_s + 1u;
+  o.s2 = s2; o.e = e1;
+  double mask;                                              // S5
+  const int si = field_at<UNIFORM1>(f, x, y, z, Ex, Ey, Ez, mask);
+  if (si < 0) { o.status = -si; return; }
+  if (mask < 0.5) { o.status = AVM_MATERIAL; return; }
+  if (t > t_max) { o.status = AVM_TIME_LIMIT; return; }
+  if (n >= kStepLimit) { o.status = AVM_STEP_LIMIT; return; }
+  const double sb = e1 * g.inv_de;                          // S6
+  int b;
+  if (sb >= (double)g.nb) { b = g.nb - 1; o.overflow = true; } else b = (int)sb;
+  o.bin = b;
+  const double xr = u2 * g.nu_hat;                          // S7
+  if (xr >= __ldg(g.nu_tot + b)) { o.event = -1; return; }
+  const int l = select_level(g, b, xr);                     // S8
+  o.event = l;
+  const int type = lv_type[l];
+  if (type == AVM_ATTACHMENT) { o.status = AVM_ATTACHED; return; }   // S9a
+  double kx = 0.0, ky = 0.0, kz = 1.0;
+  if (s2 > 0.0) { const double inv = 1.0 / sqrt(s2); kx = vx * inv; ky = vy * inv; kz = vz * inv; }
+  const double e2 = collide(seed, id, n_s, type, lv_loss[l], lv_recoil[l], lv_w[l], e1, kx, ky, kz, o.spawn, o.ch, o.loss);
+  o.e = e2; o.kx = kx; o.ky = ky; o.kz = kz;
+  const double sp = kC2 * sqrt(e2);
+  vx = sp * kx; vy = sp * ky; vz = sp * kz;
+}
+
+// ---- persistent transport kernel -------------------------------------------------------------------------
+template <bool UNIFORM1, bool HASB, bool TALLY>
+__global__ void __launch_bounds__(kThreads, kMinCtasPerSm)
+transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevField f, const RunArrays a,
+                 RunCtl* __restrict__ ctl, const uint64_t seed, const double t_max, const uint32_t max_iters,
+                 const uint32_t n_static_tickets) {
+  __shared__ double s_loss[AVM_MAX_LEVELS], s_recoil[AVM_MAX_LEVELS], s_w[AVM_MAX_LEVELS];
+  __shared__ uint8_t s_type[AVM_MAX_LEVELS];
+  __shared__ unsigned int s_hist[AVM_MAX_LEVELS];
+  for (int l = threadIdx.x; l < AVM_MAX_LEVELS; l += blockDim.x) {
+    const bool in = l < g.L;
+    s_loss[l] = in ? g.loss[l] : 0.0; s_recoil[l] = in ? g.recoil[l] : 0.0; s_w[l] = in ? g.w[l] : 1.0;
+    s_type[l] = in ? g.type[l] : 0; s_hist[l] = 0u;
+  }
+  __syncthreads();
+
+  const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+  const uint32_t cap = a.cap;
+  const size_t ld = cap;
+  // static tickets, warp-major across the grid: the first electrons fill whole warps, one warp per CTA first
+  uint32_t ticket = (warp * gridDim.x + blockIdx.x) * 32u + lane;
+  bool have = false;
+  double x = 0, y = 0, z = 0, t = 0, vx = 0, vy = 0, vz = 0, Ex = 0, Ey = 0, Ez = 0;
+  uint64_t id = 0;
+  uint32_t n = 0, slot = 0, aval = 0;
+  uint32_t c_null = 0, c_real = 0, c_steps = 0, c_over = 0;
+  double c_loss = 0.0;
+
+  for (uint32_t it = 0; it < max_iters; ++it) {
+    if (!have) {
+#pragma unroll 1
+      for (int tries = 0; tries < 4 && ticket < cap; ++tries) {
+        const int st = ld_volatile_s32(a.status + ticket);
+        if (st == 0) {                              // published and unfinished: this lane runs it
+          __threadfence();
+          slot = ticket;
+          x = __ldcg(a.end + slot); y = __ldcg(a.end + ld + slot); z = __ldcg(a.end + 2 * ld + slot);
+          t = __ldcg(a.end + 3 * ld + slot);
+          const double e = __ldcg(a.end + 4 * ld + slot);
+          const double sp = kC2 * sqrt(e);
+          vx = sp * __ldcg(a.end + 5 * ld + slot); vy = sp * __ldcg(a.end + 6 * ld + slot);
+          vz = sp * __ldcg(a.end + 7 * ld + slot);
+          id = __ldcg(a.id + slot);
+          n = __ldcg(a.nsteps + slot);
+          aval = __ldcg(a.aval + slot);
+          double m;
+          field_at<UNIFORM1>(f, x, y, z, Ex, Ey, Ez, m);     // S0 of its first step here (in-domain by construction)
+          have = true;
+          break;
+        }
+        if (st < 0) break;                          // not created yet: keep the ticket
+        ticket = n_static_tickets + atomicAdd(&ctl->q_head, 1u);   // finished in an earlier launch: next ticket
+      }
+    }
+    const unsigned act = __ballot_sync(0xFFFFFFFFu, have);
+    if (act == 0u) {                                // whole warp idle: poll for termination
+      unsigned long long c = 0ull;
+      if (lane == 0u) c = ld_volatile_u64(&ctl->counters);
+      c = __shfl_sync(0xFFFFFFFFu, c, 0);
+      if ((uint32_t)(c >> 32) == (uint32_t)c) break;
+      __nanosleep(200);
+      continue;
+    }
+    StepOut o;
+    o.status = 0; o.spawn = false;
+    if (have) {
+      step_core<UNIFORM1, HASB>(g, f, s_type, s_loss, s_recoil, s_w, seed, t_max, id, n, x, y, z, t, vx, vy, vz, Ex,
+                                Ey, Ez, o);
+      if (TALLY) {
+        ++c_steps;
+        if (o.overflow) ++c_over;
+        if (o.event == -1) ++c_null;
+        else if (o.event >= 0) { ++c_real; atomicAdd(&s_hist[o.event], 1u); c_loss += o.loss; }
+      }
+    }
+    // ---- append secondaries: one atomic per warp (a-9) ----
+    const unsigned sm = __ballot_sync(0xFFFFFFFFu, o.spawn);
+    if (sm) {
+      const int leader = __ffs(sm) - 1;
+      unsigned long long old = 0ull;
+      if ((int)lane == leader) old = atomicAdd(&ctl->counters, (unsigned long long)__popc(sm) << 32);
+      old = __shfl_sync(0xFFFFFFFFu, old, leader);
+      if (o.spawn) {
+        const uint64_t cs = (old >> 32) + (uint64_t)__popc(sm & ((1u << lane) - 1u));
+        if (cs < (uint64_t)cap) {
+          const uint32_t c = (uint32_t)cs;
+          double ckx, cky, ckz;
+          child_direction(o.ch.u6, o.ch.u7, ckx, cky, ckz);
+          __stcg(a.end + c, x); __stcg(a.end + ld + c, y); __stcg(a.end + 2 * ld + c, z); __stcg(a.end + 3 * ld + c, t);
+          __stcg(a.end + 4 * ld + c, o.ch.e);
+          __stcg(a.end + 5 * ld + c, ckx); __stcg(a.end + 6 * ld + c, cky); __stcg(a.end + 7 * ld + c, ckz);
+          __stcg(a.id + c, child_id_of(seed, id, n - 1u));
+          __stcg(a.aval + c, aval);
+          __stcg(a.nsteps + c, 0u);
+          if (a.birth) {
+            __stcg(a.birth + c, x); __stcg(a.birth + ld + c, y); __stcg(a.birth + 2 * ld + c, z);
+            __stcg(a.birth + 3 * ld + c, t); __stcg(a.birth + 4 * ld + c, o.ch.e);
+          }
+          __threadfence();
+          *(volatile int*)(a.status + c) = 0;       // publish
+        } else {                                    // no room: drop the child, count it as created and finished
+          atomicAdd(&ctl->dropped, 1u);
+          atomicAdd(&ctl->counters, 1ull);
+        }
+      }
+    }
+    // ---- retire finished electrons: endpoint write, one atomic per warp for `done`, one for new tickets ----
+    const bool fin = have && o.status != 0;
+    const unsigned fm = __ballot_sync(0xFFFFFFFFu, fin);
+    if (fm) {
+      const int leader = __ffs(fm) - 1;
+      unsigned int base = 0u;
+      if ((int)lane == leader) {
+        base = atomicAdd(&ctl->q_head, (unsigned int)__popc(fm));
+      }
+      base = __shfl_sync(0xFFFFFFFFu, base, leader);
+      if (fin) {
+        double kx = 0.0, ky = 0.0, kz = 1.0;
+        if (o.s2 > 0.0) { const double inv = 1.0 / sqrt(o.s2); kx = vx * inv; ky = vy * inv; kz = vz * inv; }
+        a.end[slot] = x; a.end[ld + slot] = y; a.end[2 * ld + slot] = z; a.end[3 * ld + slot] = t;
+        a.end[4 * ld + slot] = o.e; a.end[5 * ld + slot] = kx; a.end[6 * ld + slot] = ky; a.end[7 * ld + slot] = kz;
+        a.nsteps[slot] = n;
+        a.status[slot] = o.status;
+        have = false;
+        ticket = n_static_tickets + base + (uint32_t)__popc(fm & ((1u << lane) - 1u));
+      }
+      __syncwarp();
+      if ((int)lane == leader) { __threadfence(); atomicAdd(&ctl->counters, (unsigned long long)__popc(fm)); }
+    }
+  }
+
+  // guard expired with the electron still active: park its state in its slot (status stays 0); the next
+  // launch picks it up through the tickets.
+  if (have) {
+    const double s2 = vx * vx + vy * vy + vz * vz;
+    double kx = 0.0, ky = 0.0, kz = 1.0;
+    if (s2 > 0.0) { const double inv = 1.0 / sqrt(s2); kx = vx * inv; ky = vy * inv; kz = vz * inv; }
+    a.end[slot] = x; a.end[ld + slot] = y; a.end[2 * ld + slot] = z; a.end[3 * ld + slot] = t;
+    a.end[4 * ld + slot] = fmax(s2 * kInvC2Sq, kEpsFloor);
+    a.end[5 * ld + slot] = kx; a.end[6 * ld + slot] = ky; a.end[7 * ld + slot] = kz;
+    a.nsteps[slot] = n;
+  }
+  if (TALLY) {
+    // warp reduce the per-thread counters, one atomic per warp; level histogram per CTA
+    unsigned long long v0 = c_null, v1 = c_real, v2 = c_steps, v3 = c_over;
+    double v4 = c_loss;
+#pragma unroll
+    for (int o2 = 16; o2 > 0; o2 >>= 1) {
+      v0 += __shfl_down_sync(0xFFFFFFFFu, v0, o2); v1 += __shfl_down_sync(0xFFFFFFFFu, v1, o2);
+      v2 += __shfl_down_sync(0xFFFFFFFFu, v2, o2); v3 += __shfl_down_sync(0xFFFFFFFFu, v3, o2);
+      v4 += __shfl_down_sync(0xFFFFFFFFu, v4, o2);
+    }
+    if (lane == 0u) {
+      if (v0) atomicAdd(&ctl->n_null, v0);
+      if (v1) atomicAdd(&ctl->n_real, v1);
+      if (v2) atomicAdd(&ctl->n_steps, v2);
+      if (v3) atomicAdd(&ctl->n_overflow, v3);
+      if (v4 != 0.0) atomicAdd(&ctl->sum_loss, v4);
+    }
+    __syncthreads();
+    for (int l = threadIdx.x; l < g.L; l += blockDim.x)
+      if (s_hist[l]) atomicAdd(&ctl->level[l], (unsigned long long)s_hist[l]);
+  }
+}
+
+// ---- primary injection (a-1) -----------------------------------------------------------------------------
+template <bool UNIFORM1>
+__global__ void inject_kernel(const __grid_constant__ DevField f, const RunArrays a, RunCtl* ctl,
+                              const double* __restrict__ prim, const uint32_t p0, const uint32_t count,
+                              const uint64_t id_offset, const double t_max) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  unsigned long long add = 0ull;
+  if (i < count) {
+    const uint32_t p = p0 + i;
+    const double* q = prim + (size_t)i * 8;
+    const double x = q[0], y = q[1], z = q[2], t = q[3];
+    const double e = fmax(q[4], kEpsFloor);
+    double kx = q[5], ky = q[6], kz = q[7];
+    const double nk = sqrt(kx * kx + ky * ky + kz * kz);
+    if (!(nk > 0.0)) { kx = 0.0; ky = 0.0; kz = 1.0; } else { kx /= nk; ky /= nk; kz /= nk; }
+    double Ex, Ey, Ez, m = 1.0;
+    const int si = field_at<UNIFORM1>(f, x, y, z, Ex, Ey, Ez, m);
+    int st = 0;
+    if (si < 0) st = -si;
+    else if (m < 0.5) st = AVM_MATERIAL;
+    else if (t > t_max) st = AVM_TIME_LIMIT;
+    const size_t ld = a.cap;
+    a.end[p] = x; a.end[ld + p] = y; a.end[2 * ld + p] = z; a.end[3 * ld + p] = t; a.end[4 * ld + p] = e;
+    a.end[5 * ld + p] = kx; a.end[6 * ld + p] = ky; a.end[7 * ld + p] = kz;
+    if (a.birth) {
+      a.birth[p] = x; a.birth[ld + p] = y; a.birth[2 * ld + p] = z; a.birth[3 * ld + p] = t; a.birth[4 * ld + p] = e;
+    }
+    a.id[p] = id_offset + (uint64_t)p;
+    a.aval[p] = p;
+    a.nsteps[p] = 0u;
+    a.status[p] = st;
+    add = (1ull << 32) | (st != 0 ? 1ull : 0ull);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) add += __shfl_down_sync(0xFFFFFFFFu, add, o);
+  if ((threadIdx.x & 31u) == 0u && add) atomicAdd(&ctl->counters, add);
+}
+
+// ---- tallies derived from the endpoints (a-12) -----------------------------------------------------------
+__global__ void finalize_kernel(const RunArrays a, RunCtl* ctl, const uint32_t n, unsigned long long* per_aval,
+                                const uint32_t n_prim, const bool want_sums) {
+  double d[4] = {0.0, 0.0, 0.0, 0.0};
+  const size_t ld = a.cap;
+  for (uint32_t s = blockIdx.x * blockDim.x + threadIdx.x; s < n; s += gridDim.x * blockDim.x) {
+    if (per_aval) {
+      const uint32_t av = a.aval[s];
+      if (av < n_prim) {
+        atomicAdd(per_aval + 3 * (size_t)av, 1ull);
+        if (a.status[s] == AVM_ATTACHED) atomicAdd(per_aval + 3 * (size_t)av + 2, 1ull);
+      }
+    }
+    if (want_sums) {
+#pragma unroll
+      for (int c = 0; c < 4; ++c) d[c] += a.end[c * ld + s] - a.birth[c * ld + s];
+    }
+  }
+  if (want_sums) {
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+      double v = d[c];
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xFFFFFFFFu, v, o);
+      if ((threadIdx.x & 31u) == 0u && v != 0.0) atomicAdd(&ctl->sum_d[c], v);
+    }
+  }
+}
+
+__global__ void publish_kernel(const RunCtl* ctl, const int L, unsigned long long* per_aval, const uint32_t n_prim,
+                               unsigned long long* tallies_u64, double* tallies_f64) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (per_aval && i < n_prim) {
+    const unsigned long long e = per_aval[3 * (size_t)i];
+    per_aval[3 * (size_t)i + 1] = e > 0ull ? e - 1ull : 0ull;     // ions = ionisations = endpoints - 1 (C11)
+  }
+  if (i == 0u) {
+    if (tallies_u64) {
+      for (int l = 0; l < L; ++l) tallies_u64[l] = ctl->level[l];
+      tallies_u64[L] = ctl->n_null; tallies_u64[L + 1] = ctl->n_real;
+      tallies_u64[L + 2] = ctl->n_overflow; tallies_u64[L + 3] = ctl->n_steps;
+    }
+    if (tallies_f64) {
+      for (int c = 0; c < 4; ++c) tallies_f64[c] = ctl->sum_d[c];
+      tallies_f64[4] = ctl->sum_loss;
+    }
+  }
+}
+
+// ---- parity hooks ----------------------------------------------------------------------------------------
+template <bool UNIFORM1, bool HASB>
+__global__ void step_batch_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevField f,
+                                  const uint64_t seed, const double t_max, const int64_t n,
+                                  const double* __restrict__ in, const uint64_t* __restrict__ ids,
+                                  const uint32_t* __restrict__ n_idx, double* __restrict__ out,
+                                  int32_t* __restrict__ event, int32_t* __restrict__ status, int32_t* __restrict__ bin,
+                                  double* __restrict__ child, uint64_t* __restrict__ child_id) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  double x = in[i], y = in[n + i], z = in[2 * n + i], t = in[3 * n + i];
+  const double e = in[4 * n + i];
+  double kx = in[5 * n + i], ky = in[6 * n + i], kz = in[7 * n + i];
+  const uint64_t id = ids[i];
+  uint32_t nn = n_idx[i];
+  for (int c = 0; c < 8; ++c) child[c * n + i] = 0.0;
+  child_id[i] = 0ull;
+  double Ex, Ey, Ez, m;
+  const int si = field_at<UNIFORM1>(f, x, y, z, Ex, Ey, Ez, m);     // S0
+  if (si < 0) {                                                     // caller error: reported as a status
+    for (int c = 0; c < 8; ++c) out[c * n + i] = in[c * n + i];
+    event[i] = -2; status[i] = -si; bin[i] = -1;
+    return;
+  }
+  const double sp = kC2 * sqrt(e);
+  double vx = sp * kx, vy = sp * ky, vz = sp * kz;
+  StepOut o;
+  step_core<UNIFORM1, HASB>(g, f, g.type, g.loss, g.recoil, g.w, seed, t_max, id, nn, x, y, z, t, vx, vy, vz, Ex, Ey,
+                            Ez, o);
+  const bool collided = o.event >= 0 && o.status == 0;
+  if (collided) { kx = o.kx; ky = o.ky; kz = o.kz; }
+  else if (o.s2 > 0.0) { const double inv = 1.0 / sqrt(o.s2); kx = vx * inv; ky = vy * inv; kz = vz * inv; }
+  out[i] = x; out[n + i] = y; out[2 * n + i] = z; out[3 * n + i] = t; out[4 * n + i] = o.e;
+  out[5 * n + i] = kx; out[6 * n + i] = ky; out[7 * n + i] = kz;
+  event[i] = o.event; status[i] = o.status; bin[i] = o.bin;
+  if (o.spawn) {
+    double ckx, cky, ckz;
+    child_direction(o.ch.u6, o.ch.u7, ckx, cky, ckz);
+    child[i] = x; child[n + i] = y; child[2 * n + i] = z; child[3 * n + i] = t; child[4 * n + i] = o.ch.e;
+    child[5 * n + i] = ckx; child[6 * n + i] = cky; child[7 * n + i] = ckz;
+    child_id[i] = child_id_of(seed, id, nn - 1u);
+  }
+}
+
+__global__ void field_eval_kernel(const __grid_constant__ DevField f, const int64_t n, const double* __restrict__ r,
+                                  double* __restrict__ E, double* __restrict__ mask, int32_t* __restrict__ slab) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  double ex = 0.0, ey = 0.0, ez = 0.0, m = 0.0;
+  const int si = field_at<false>(f, r[i], r[n + i], r[2 * n + i], ex, ey, ez, m);
+  E[i] = ex; E[n + i] = ey; E[2 * n + i] = ez; mask[i] = m; slab[i] = si < 0 ? -1 : si;
+}
+
+__global__ void philox_batch_kernel(const uint64_t seed, const int64_t n, const uint64_t* __restrict__ id,
+                                    const uint32_t* __restrict__ n_idx, const uint32_t* __restrict__ block,
+                                    uint32_t* __restrict__ words, double* __restrict__ u) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const U4 w = philox(seed, id[i], n_idx[i], block[i]);
+  words[4 * i] = w.w0; words[4 * i + 1] = w.w1; words[4 * i + 2] = w.w2; words[4 * i + 3] = w.w3;
+  u[2 * i] = to_unit(w.w0, w.w1); u[2 * i + 1] = to_unit(w.w2, w.w3);
+}
+
+// FP64 issue-rate probe: 8 independent DFMA chains per thread.
+__global__ void __launch_bounds__(256) fp64_probe_kernel(const long long iters, double* sink) {
+  double a0 = 1.0 + threadIdx.x * 1e-9, a1 = a0 + 1e-3, a2 = a0 + 2e-3, a3 = a0 + 3e-3, a4 = a0 + 4e-3,
+         a5 = a0 + 5e-3, a6 = a0 + 6e-3, a7 = a0 + 7e-3;
+  const double m = 0.9999999, c = 1e-7;
+  for (long long i = 0; i < iters; ++i) {
+    a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+    a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+  }
+  sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+}
+
+}  // namespace
+
+// =================================================================================================================
+// Host side: handles and the C ABI
+// =================================================================================================================
+struct avm_ctx {
+  int device = 0;
+  cudaStream_t stream = nullptr;
+  int sm_count = 0;
+  unsigned long long* h_counters = nullptr;   // pinned: the one word the host reads per launch
+  int64_t n_kernel_launches = 0, n_transport_launches = 0;
+};
+struct avm_gas {
+  DevGas d{};
+  double nu_hat = 0.0;
+};
+struct avm_field {
+  DevField d{};
+  bool uniform1 = false;
+};
+
+namespace {
+
+bool valid_gas(const avm_gas_desc* d, double* max_rate) {
+  if (!d || d->n_bins < 1 || d->n_levels < 1 || d->n_levels > AVM_MAX_LEVELS || !(d->e_max_eV > 0) || !d->cum_rate ||
+      !d->level_type || !d->level_loss_eV || !d->level_recoil || !d->level_ob_w_eV) {
+    g_err = "gas: null pointer, empty table or n_levels > AVM_MAX_LEVELS";
+    return false;
+  }
+  double mx = 0.0;
+  const int L = d->n_levels;
+  for (int b = 0; b < d->n_bins; ++b) {
+    double prev = 0.0;
+    for (int l = 0; l < L; ++l) {
+      const double c = d->cum_rate[(size_t)b * L + l];
+      if (!(c >= prev)) { g_err = "gas: cum_rate decreases along levels (or is NaN / negative)"; return false; }
+      prev = c;
+    }
+    if (prev > mx) mx = prev;
+  }
+  for (int l = 0; l < L; ++l) {
+    if (d->level_type[l] > 3) { g_err = "gas: bad level type"; return false; }
+    if (d->level_type[l] == AVM_IONISATION && !(d->level_ob_w_eV[l] > 0)) { g_err = "gas: ionisation level needs w > 0"; return false; }
+  }
+  if (!(mx > 0.0) && !(d->nu_hat > 0.0)) { g_err = "gas: all rates are zero"; return false; }
+  if (d->nu_hat > 0.0 && d->nu_hat < mx) { g_err = "gas: nu_hat below the maximum total rate"; return false; }
+  if (max_rate) *max_rate = mx;
+  return true;
+}
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+struct GasLayout { size_t nu_tot, cum, loss, recoil, w, type, total; };
+GasLayout gas_layout(int nb, int L) {
+  GasLayout g;
+  size_t off = 0;
+  g.nu_tot = off; off = align_up(off + sizeof(double) * nb, 256);
+  g.cum = off;    off = align_up(off + sizeof(double) * (size_t)nb * L, 256);
+  g.loss = off;   off += sizeof(double) * AVM_MAX_LEVELS;
+  g.recoil = off; off += sizeof(double) * AVM_MAX_LEVELS;
+  g.w = off;      off += sizeof(double) * AVM_MAX_LEVELS;
+  g.type = off;   off = align_up(off + AVM_MAX_LEVELS, 256);
+  g.total = off;
+  return g;
+}
+
+template <typename K, typename... Args>
+cudaError_t launch(avm_ctx* ctx, K kernel, dim3 grid, dim3 block, Args... args) {
+  kernel<<<grid, block, 0, ctx->stream>>>(args...);
+  ctx->n_kernel_launches++;
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* avm_last_error(void) { return g_err.c_str(); }
+
+int32_t avm_ctx_create(int32_t device, void* cuda_stream, avm_ctx** out) {
+  if (!out) return fail(AVM_ERR_INVALID_ARG, "ctx_create: out is null");
+  *out = nullptr;
+  int n_dev = 0;
+  AVM_CUDA(cudaGetDeviceCount(&n_dev));
+  if (device < 0 || device >= n_dev) return fail(AVM_ERR_CUDA, "ctx_create: no such CUDA device");
+  AVM_CUDA(cudaSetDevice(device));
+  cudaDeviceProp prop;
+  AVM_CUDA(cudaGetDeviceProperties(&prop, device));
+  if (prop.major != 10) return fail(AVM_ERR_CUDA, "ctx_create: device is not compute capability 10.x (built for sm_100a only)");
+  avm_ctx* c = new (std::nothrow) avm_ctx();
+  if (!c) return fail(AVM_ERR_STATE, "ctx_create: out of host memory");
+  c->device = device;
+  c->stream = (cudaStream_t)cuda_stream;
+  c->sm_count = prop.multiProcessorCount;
+  cudaError_t e = cudaHostAlloc((void**)&c->h_counters, 64, cudaHostAllocDefault);
+  if (e != cudaSuccess) { delete c; return fail(AVM_ERR_CUDA, std::string("ctx_create: cudaHostAlloc: ") + cudaGetErrorString(e)); }
+  *out = c;
+  return AVM_OK;
+}
+
+int32_t avm_ctx_destroy(avm_ctx* c) {
+  if (!c) return AVM_OK;
+  if (c->h_counters) cudaFreeHost(c->h_counters);
+  delete c;
+  return AVM_OK;
+}
+
+int32_t avm_ctx_sm_count(const avm_ctx* c) { return c ? c->sm_count : 0; }
+
+size_t avm_gas_bytes(const avm_gas_desc* d) {
+  if (!d || d->n_bins < 1 || d->n_levels < 1 || d->n_levels > AVM_MAX_LEVELS) return 0;
+  return gas_layout(d->n_bins, d->n_levels).total;
+}
+
+int32_t avm_gas_create(avm_ctx* ctx, const avm_gas_desc* d, void* dev_buf, size_t dev_bytes, avm_gas** out) {
+  if (!ctx || !out) return fail(AVM_ERR_INVALID_ARG, "gas_create: null ctx/out");
+  *out = nullptr;
+  double mx = 0.0;
+  if (!valid_gas(d, &mx)) return AVM_ERR_INVALID_ARG;
+  const int nb = d->n_bins, L = d->n_levels;
+  const GasLayout lay = gas_layout(nb, L);
+  if (!dev_buf || dev_bytes < lay.total || ((uintptr_t)dev_buf & 255u)) return fail(AVM_ERR_INVALID_ARG, "gas_create: device buffer null, too small or not 256-byte aligned");
+  std::vector<unsigned char> h(lay.total, 0);
+  double* nu_tot = (double*)(h.data() + lay.nu_tot);
+  for (int b = 0; b < nb; ++b) nu_tot[b] = d->cum_rate[(size_t)b * L + L - 1];
+  std::memcpy(h.data() + lay.cum, d->cum_rate, sizeof(double) * (size_t)nb * L);
+  std::memcpy(h.data() + lay.loss, d->level_loss_eV, sizeof(double) * L);
+  std::memcpy(h.data() + lay.recoil, d->level_recoil, sizeof(double) * L);
+  std::memcpy(h.data() + lay.w, d->level_ob_w_eV, sizeof(double) * L);
+  std::memcpy(h.data() + lay.type, d->level_type, L);
+  AVM_CUDA(cudaSetDevice(ctx->device));
+  AVM_CUDA(cudaMemcpyAsync(dev_buf, h.data(), lay.total, cudaMemcpyHostToDevice, ctx->stream));
+  AVM_CUDA(cudaStreamSynchronize(ctx->stream));
+  avm_gas* g = new (std::nothrow) avm_gas();
+  if (!g) return fail(AVM_ERR_STATE, "gas_create: out of host memory");
+  unsigned char* base = (unsigned char*)dev_buf;
+  g->nu_hat = d->nu_hat > 0.0 ? d->nu_hat : mx;
+  g->d.nb = nb; g->d.L = L;
+  g->d.inv_de = (double)nb / d->e_max_eV;
+  g->d.nu_hat = g->nu_hat;
+  g->d.inv_nu_hat = 1.0 / g->nu_hat;
+  g->d.nu_tot = (const double*)(base + lay.nu_tot);
+  g->d.cum = (const double*)(base + lay.cum);
+  g->d.loss = (const double*)(base + lay.loss);
+  g->d.recoil = (const double*)(base + lay.recoil);
+  g->d.w = (const double*)(base + lay.w);
+  g->d.type = (const uint8_t*)(base + lay.type);
+  *out = g;
+  return AVM_OK;
+}
+
+int32_t avm_gas_destroy(avm_gas* g) { delete g; return AVM_OK; }
+double avm_gas_nu_hat(const avm_gas* g) { return g ? g->nu_hat : 0.0; }
+
+int32_t avm_field_create(avm_ctx* ctx, const avm_field_desc* d, avm_field** out) {
+  if (!ctx || !out) return fail(AVM_ERR_INVALID_ARG, "field_create: null ctx/out");
+  *out = nullptr;
+  if (!d || !d->slabs || d->n_slabs < 1 || d->n_slabs > AVM_MAX_SLABS) return fail(AVM_ERR_INVALID_ARG, "field_create: need 1..AVM_MAX_SLABS slabs");
+  const double inf = std::numeric_limits<double>::infinity();
+  avm_field* f = new (std::nothrow) avm_field();
+  if (!f) return fail(AVM_ERR_STATE, "field_create: out of host memory");
+  DevField& F = f->d;
+  F.n_slabs = d->n_slabs;
+  for (int i = 0; i < d->n_slabs; ++i) {
+    const avm_slab& s = d->slabs[i];
+    DevSlab& S = F.slab[i];
+    const char* bad = nullptr;
+    if (!(s.z_hi > s.z_lo)) bad = "field: slab z_hi <= z_lo";
+    else if (i > 0 && s.z_lo != d->slabs[i - 1].z_hi) bad = "field: slabs not contiguous/ascending";
+    else if (s.kind != 0 && s.kind != 1) bad = "field: kind";
+    S.z_lo = s.z_lo; S.z_hi = s.z_hi; S.kind = s.kind;
+    for (int a = 0; a < 3; ++a) S.E[a] = s.E[a];
+    if (!bad && s.kind == 1) {
+      if (!s.nodes_dev || s.nx < 2 || s.ny < 2 || s.nz < 2) bad = "field: grid needs device nodes and >= 2 nodes per axis";
+      else if ((uintptr_t)s.nodes_dev & 15u) bad = "field: nodes not 16-byte aligned";
+      else if (!(s.spacing[0] > 0 && s.spacing[1] > 0 && s.spacing[2] > 0)) bad = "field: spacing";
+      else if (s.bc_x < 0 || s.bc_x > 2 || s.bc_y < 0 || s.bc_y > 2) bad = "field: bc";
+      else {
+        const double ztop = s.origin[2] + (s.nz - 1) * s.spacing[2], tol = 1e-9 * s.spacing[2];
+        if (s.z_lo < s.origin[2] - tol || s.z_hi > ztop + tol) bad = "field: slab z-range outside its grid";
+        if (s.bc_x && !(s.period_x > 0 && s.period_x <= (s.nx - 1) * s.spacing[0] * (1 + 1e-12))) bad = "field: period_x";
+        if (s.bc_y && !(s.period_y > 0 && s.period_y <= (s.ny - 1) * s.spacing[1] * (1 + 1e-12))) bad = "field: period_y";
+      }
+      S.nodes = (const float4*)s.nodes_dev;
+      S.nx = s.nx; S.ny = s.ny; S.nz = s.nz;
+      const int bc[2] = {s.bc_x, s.bc_y};
+      const double per[2] = {s.period_x, s.period_y};
+      const int nn[2] = {s.nx, s.ny};
+      for (int a = 0; a < 3; ++a) { S.org[a] = s.origin[a]; S.inv_h[a] = 1.0 / s.spacing[a]; }
+      for (int a = 0; a < 2; ++a) {
+        S.bc[a] = bc[a];
+        S.span[a] = (nn[a] - 1) * s.spacing[a];
+        S.P[a] = bc[a] == 2 ? 2.0 * per[a] : per[a];
+        S.inv_P[a] = bc[a] ? 1.0 / S.P[a] : 0.0;
+        S.half[a] = bc[a] == 2 ? per[a] : inf;
+      }
+    }
+    if (bad) { delete f; return fail(AVM_ERR_INVALID_ARG, bad); }
+  }
+  F.z_lo = d->slabs[0].z_lo;
+  F.z_hi = d->slabs[d->n_slabs - 1].z_hi;
+  for (int a = 0; a < 2; ++a) { F.xy_lo[a] = d->xy_lo[a]; F.xy_hi[a] = d->xy_hi[a]; }
+  const double Bn2 = d->B[0] * d->B[0] + d->B[1] * d->B[1] + d->B[2] * d->B[2];
+  F.has_B = Bn2 != 0.0;
+  F.Bn2 = Bn2;
+  for (int a = 0; a < 3; ++a) F.B[a] = d->B[a];
+  if (F.has_B) {
+    const double Bn = std::sqrt(Bn2);
+    for (int a = 0; a < 3; ++a) F.bh[a] = d->B[a] / Bn;
+    F.omega = kOmega1 * Bn;
+    F.inv_omega = 1.0 / F.omega;
+  }
+  f->uniform1 = d->n_slabs == 1 && d->slabs[0].kind == 0;
+  *out = f;
+  return AVM_OK;
+}
+
+int32_t avm_field_destroy(avm_field* f) { delete f; return AVM_OK; }
+
+int32_t avm_field_eval(avm_ctx* ctx, const avm_field* f, int64_t n, const double* r, double* E, double* mask, int32_t* slab) {
+  if (!ctx || !f || n < 0 || (n > 0 && (!r || !E || !mask || !slab))) return fail(AVM_ERR_INVALID_ARG, "field_eval: null argument");
+  if (n == 0) return AVM_OK;
+  AVM_CUDA(cudaSetDevice(ctx->device));
+  AVM_CUDA(launch(ctx, field_eval_kernel, dim3((unsigned)((n + 255) / 256)), dim3(256), f->d, n, r, E, mask, slab));
+  return AVM_OK;
+}
+
+size_t avm_run_workspace_bytes(const avm_ctx*, int64_t capacity) {
+  if (capacity < 0) return 0;
+  const int64_t stage = capacity < kStageElectrons ? capacity : kStageElectrons;
+  return kCtlBytes + (size_t)stage * 8 * sizeof(double);
+}
+
+int32_t avm_run_stats(const avm_ctx* c, int64_t* n_kernel_launches, int64_t* n_transport_launches) {
+  if (!c) return fail(AVM_ERR_INVALID_ARG, "run_stats: null ctx");
+  if (n_kernel_launches) *n_kernel_launches = c->n_kernel_launches;
+  if (n_transport_launches) *n_transport_launches = c->n_transport_launches;
+  return AVM_OK;
+}
+
+namespace {
+typedef void (*TransportFn)(const DevGas, const DevField, const RunArrays, RunCtl*, const uint64_t, const double,
+                            const uint32_t, const uint32_t);
+TransportFn pick_transport(bool uniform1, bool has_b, bool tally) {
+  if (uniform1) {
+    if (has_b) return tally ? transport_kernel<true, true, true> : transport_kernel<true, true, false>;
+    return tally ? transport_kernel<true, false, true> : transport_kernel<true, false, false>;
+  }
+  if (has_b) return tally ? transport_kernel<false, true, true> : transport_kernel<false, true, false>;
+  return tally ? transport_kernel<false, false, true> : transport_kernel<false, false, false>;
+}
+}  // namespace
+
+int32_t avm_run(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, const double* primaries, int64_t np,
+                const avm_run_opts* opts, const avm_outputs* o, int64_t* n_out) {
+  if (!ctx || !gas || !field || !opts || !o || !n_out) return fail(AVM_ERR_INVALID_ARG, "run: null argument");
+  *n_out = 0;
+  if (np < 0 || (np > 0 && !primaries)) return fail(AVM_ERR_INVALID_ARG, "run: primaries");
+  if (o->capacity < np || o->capacity < 1 || o->capacity > 0x7FFFFFFFll) return fail(AVM_ERR_INVALID_ARG, "run: capacity must be in [max(1, n_primaries), 2^31)");
+  if (!o->id || !o->avalanche || !o->status || !o->n_steps || !o->end) return fail(AVM_ERR_INVALID_ARG, "run: id, avalanche, status, n_steps and end are required");
+  if (o->tallies_f64 && !o->birth) return fail(AVM_ERR_INVALID_ARG, "run: tallies_f64 needs birth");
+  if (!o->workspace || o->workspace_bytes < avm_run_workspace_bytes(ctx, o->capacity) || ((uintptr_t)o->workspace & 255u))
+    return fail(AVM_ERR_INVALID_ARG, "run: workspace null, too small or not 256-byte aligned");
+  AVM_CUDA(cudaSetDevice(ctx->device));
+  ctx->n_kernel_launches = 0; ctx->n_transport_launches = 0;
+  cudaStream_t st = ctx->stream;
+  RunCtl* ctl = (RunCtl*)o->workspace;
+  double* stage = (double*)((unsigned char*)o->workspace + kCtlBytes);
+  RunArrays a;
+  a.cap = (uint32_t)o->capacity; a.id = o->id; a.aval = o->avalanche; a.status = o->status; a.nsteps = o->n_steps;
+  a.birth = o->birth; a.end = o->end;
+  const bool tally = !(opts->flags & AVM_RUN_NO_TALLIES);
+  const bool on_dev = opts->flags & AVM_RUN_PRIMARIES_ON_DEVICE;
+
+  AVM_CUDA(cudaMemsetAsync(ctl, 0, kCtlBytes, st));
+  AVM_CUDA(cudaMemsetAsync(o->status, 0xFF, sizeof(int32_t) * (size_t)o->capacity, st));   // -1 = slot not created yet
+  if (o->per_avalanche && np > 0) AVM_CUDA(cudaMemsetAsync(o->per_avalanche, 0, sizeof(uint64_t) * 3 * (size_t)np, st));
+  // a-1: primaries in (H2D inside the call), chunked through the staging area
+  for (int64_t p0 = 0; p0 < np; p0 += kStageElectrons) {
+    const int64_t cnt = (np - p0) < kStageElectrons ? (np - p0) : kStageElectrons;
+    const double* src = primaries + p0 * 8;
+    if (!on_dev) {
+      AVM_CUDA(cudaMemcpyAsync(stage, src, sizeof(double) * 8 * (size_t)cnt, cudaMemcpyHostToDevice, st));
+      src = stage;
+    }
+    const dim3 grid((unsigned)((cnt + 255) / 256));
+    if (field->uniform1) AVM_CUDA(launch(ctx, inject_kernel<true>, grid, dim3(256), field->d, a, ctl, src, (uint32_t)p0, (uint32_t)cnt, opts->id_offset, opts->t_max));
+    else AVM_CUDA(launch(ctx, inject_kernel<false>, grid, dim3(256), field->d, a, ctl, src, (uint32_t)p0, (uint32_t)cnt, opts->id_offset, opts->t_max));
+  }
+  // persistent transport (a-2 .. a-11)
+  TransportFn fn = pick_transport(field->uniform1, field->d.has_B != 0, tally);
+  int occ = 0;
+  AVM_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kThreads, 0));
+  if (occ < 1) return fail(AVM_ERR_CUDA, "run: transport kernel does not fit on an SM");
+  if (opts->n_ctas_per_sm > 0 && opts->n_ctas_per_sm < occ) occ = opts->n_ctas_per_sm;
+  const unsigned grid = (unsigned)(ctx->sm_count * occ);
+  const uint32_t n_static = grid * kThreads;
+  const uint32_t max_iters = opts->max_iters_per_launch ? opts->max_iters_per_launch : kDefaultMaxIters;
+  unsigned long long c = 0ull;
+  const int64_t max_launches = 1ll << 20;
+  int64_t launches = 0;
+  for (;;) {
+    AVM_CUDA(cudaMemcpyAsync(ctx->h_counters, &ctl->counters, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    AVM_CUDA(cudaStreamSynchronize(st));
+    c = *ctx->h_counters;
+    if ((uint32_t)(c >> 32) == (uint32_t)c) break;              // a-11: every electron has a non-zero status
+    if (++launches > max_launches) return fail(AVM_ERR_STATE, "run: launch limit reached without termination");
+    AVM_CUDA(cudaMemsetAsync(&ctl->q_head, 0, sizeof(unsigned int), st));
+    fn<<<grid, kThreads, 0, st>>>(gas->d, field->d, a, ctl, opts->seed, opts->t_max, max_iters, n_static);
+    AVM_CUDA(cudaGetLastError());
+    ctx->n_kernel_launches++; ctx->n_transport_launches++;
+  }
+  const uint64_t total = c >> 32;
+  const uint32_t n_end = (uint32_t)(total < (uint64_t)a.cap ? total : (uint64_t)a.cap);
+  // a-12: tallies from the endpoints
+  const bool want_sums = o->tallies_f64 != nullptr;
+  if ((o->per_avalanche || want_sums) && n_end > 0) {
+    unsigned blocks = (n_end + 255u) / 256u;
+    const unsigned maxb = (unsigned)ctx->sm_count * 8u;
+    if (blocks > maxb) blocks = maxb;
+    AVM_CUDA(launch(ctx, finalize_kernel, dim3(blocks), dim3(256), a, ctl, n_end, (unsigned long long*)o->per_avalanche, (uint32_t)np, want_sums));
+  }
+  if (o->per_avalanche || o->tallies_u64 || o->tallies_f64) {
+    const unsigned blocks = (unsigned)((np > 0 ? np : 1) + 255) / 256;
+    AVM_CUDA(launch(ctx, publish_kernel, dim3(blocks), dim3(256), (const RunCtl*)ctl, gas->d.L, (unsigned long long*)o->per_avalanche, (uint32_t)np,
+                    (unsigned long long*)o->tallies_u64, o->tallies_f64));
+  }
+  unsigned int dropped = 0;
+  AVM_CUDA(cudaMemcpyAsync(ctx->h_counters + 1, &ctl->dropped, sizeof(unsigned int), cudaMemcpyDeviceToHost, st));
+  AVM_CUDA(cudaStreamSynchronize(st));
+  dropped = *(unsigned int*)(ctx->h_counters + 1);
+  *n_out = n_end;
+  if (dropped) return fail(AVM_ERR_CAPACITY, "run: capacity exceeded, " + std::to_string(dropped) + " secondaries dropped");
+  return AVM_OK;
+}
+
+int32_t avm_fetch(avm_ctx* ctx, const avm_outputs* dev, int64_t n, int64_t np, int32_t n_levels, const avm_outputs* host) {
+  if (!ctx || !dev || !host || n < 0 || n > dev->capacity || n > host->capacity) return fail(AVM_ERR_INVALID_ARG, "fetch: null argument or n beyond a capacity");
+  AVM_CUDA(cudaSetDevice(ctx->device));
+  cudaStream_t st = ctx->stream;
+#define AVM_D2H(dst, src, bytes) AVM_CUDA(cudaMemcpyAsync((dst), (src), (bytes), cudaMemcpyDeviceToHost, st))
+  if (n > 0) {
+    if (host->id && dev->id) AVM_D2H(host->id, dev->id, sizeof(uint64_t) * n);
+    if (host->avalanche && dev->avalanche) AVM_D2H(host->avalanche, dev->avalanche, sizeof(uint32_t) * n);
+    if (host->status && dev->status) AVM_D2H(host->status, dev->status, sizeof(int32_t) * n);
+    if (host->n_steps && dev->n_steps) AVM_D2H(host->n_steps, dev->n_steps, sizeof(uint32_t) * n);
+    if (host->birth && dev->birth)
+      AVM_CUDA(cudaMemcpy2DAsync(host->birth, sizeof(double) * host->capacity, dev->birth, sizeof(double) * dev->capacity, sizeof(double) * n, 5, cudaMemcpyDeviceToHost, st));
+    if (host->end && dev->end)
+      AVM_CUDA(cudaMemcpy2DAsync(host->end, sizeof(double) * host->capacity, dev->end, sizeof(double) * dev->capacity, sizeof(double) * n, 8, cudaMemcpyDeviceToHost, st));
+  }
+  if (host->per_avalanche && dev->per_avalanche && np > 0) AVM_D2H(host->per_avalanche, dev->per_avalanche, sizeof(uint64_t) * 3 * np);
+  if (host->tallies_u64 && dev->tallies_u64 && n_levels > 0) AVM_D2H(host->tallies_u64, dev->tallies_u64, sizeof(uint64_t) * (n_levels + 4));
+  if (host->tallies_f64 && dev->tallies_f64) AVM_D2H(host->tallies_f64, dev->tallies_f64, sizeof(double) * 5);
+#undef AVM_D2H
+  AVM_CUDA(cudaStreamSynchronize(st));
+  return AVM_OK;
+}
+
+int32_t avm_step_batch(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, uint64_t seed, double t_max, int64_t n,
+                       const double* in, const uint64_t* id, const uint32_t* n_idx, double* out, int32_t* event,
+                       int32_t* status, int32_t* bin, double* child, uint64_t* child_id) {
+  if (!ctx || !gas || !field || n < 0) return fail(AVM_ERR_INVALID_ARG, "step_batch: null argument");
+  if (n == 0) return AVM_OK;
+  if (!in || !id || !n_idx || !out || !event || !status || !bin || !child || !child_id) return fail(AVM_ERR_INVALID_ARG, "step_batch: null array");
+  AVM_CUDA(cudaSetDevice(ctx->device));
+  const dim3 grid((unsigned)((n + 127) / 128)), block(128);
+  const bool u = field->uniform1, b = field->d.has_B != 0;
+#define AVM_SB(U, B) AVM_CUDA(launch(ctx, step_batch_kernel<U, B>, grid, block, gas->d, field->d, seed, t_max, n, in, id, n_idx, out, event, status, bin, child, child_id))
+  if (u && b) AVM_SB(true, true); else if (u) AVM_SB(true, false); else if (b) AVM_SB(false, true); else AVM_SB(false, false);
+#undef AVM_SB
+  return AVM_OK;
+}
+
+int32_t avm_philox_batch(avm_ctx* ctx, uint64_t seed, int64_t n, const uint64_t* id, const uint32_t* n_idx,
+                         const uint32_t* block, uint32_t* words, double* u) {
+  if (!ctx || n < 0 || (n > 0 && (!id || !n_idx || !block || !words || !u))) return fail(AVM_ERR_INVALID_ARG, "philox_batch: null argument");
+  if (n == 0) return AVM_OK;
+  AVM_CUDA(cudaSetDevice(ctx->device));
+  AVM_CUDA(launch(ctx, philox_batch_kernel, dim3((unsigned)((n + 255) / 256)), dim3(256), seed, n, id, n_idx, block, words, u));
+  return AVM_OK;
+}
+
+int32_t avm_fp64_probe(avm_ctx* ctx, int32_t n_blocks, int32_t n_threads, int64_t iters, double* sink, float* ms_out) {
+  if (!ctx || n_blocks < 1 || n_threads < 32 || n_threads > 256 || iters < 1 || !sink || !ms_out) return fail(AVM_ERR_INVALID_ARG, "fp64_probe: bad argument");
+  AVM_CUDA(cudaSetDevice(ctx->device));
+  cudaEvent_t e0, e1;
+  AVM_CUDA(cudaEventCreate(&e0));
+  AVM_CUDA(cudaEventCreate(&e1));
+  fp64_probe_kernel<<<n_blocks, n_threads, 0, ctx->stream>>>(iters / 8 > 0 ? iters / 8 : 1, sink);   // warm-up
+  AVM_CUDA(cudaEventRecord(e0, ctx->stream));
+  fp64_probe_kernel<<<n_blocks, n_threads, 0, ctx->stream>>>(iters, sink);
+  AVM_CUDA(cudaEventRecord(e1, ctx->stream));
+  AVM_CUDA(cudaGetLastError());
+  AVM_CUDA(cudaEventSynchronize(e1));
+  AVM_CUDA(cudaEventElapsedTime(ms_out, e0, e1));
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  return AVM_OK;
+}
+
+}  // extern "C"

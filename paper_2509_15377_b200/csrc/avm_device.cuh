@@ -1,0 +1,269 @@
+// avm_device.cuh — device-side arithmetic of one transport step (S0-S9) for sm_100a.
+// Shared by the persistent transport kernel and the avm_step_batch parity hook, so the hook tests the
+// same code the run executes.  Shares nothing with oracle/ (the oracle has its own Philox, field and step).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "../../include/avm.h"
+
+namespace avm {
+
+// ---- constants (DESIGN.md §3 "Constants"; CODATA-2018 c = 29.9792458 cm/ns, mc^2 = 510998.95 eV) ------------
+constexpr double kC2 = 0.05930969584745753;        // speed [cm/ns] = kC2 * sqrt(energy [eV])
+constexpr double kInvC2Sq = 284.28150518042008;    // energy = |v|^2 * kInvC2Sq
+constexpr double kKappa = 0.0017588200107589609;   // a = -kKappa * E  [cm/ns^2 per V/cm]
+constexpr double kOmega1 = 175.88200107589608;     // rad/ns/T
+constexpr double kExBUnit = 1.0e-5;                // v_d [cm/ns] = 1e-5 (E x B)/|B|^2
+constexpr double kEpsFloor = 1.0e-10;              // eV
+constexpr uint32_t kBlockChildId = 0xFFFFFFFFu;
+constexpr uint32_t kStepLimit = 0xFFFFFFF0u;
+
+// ---- device-resident descriptions (passed by value as __grid_constant__ kernel parameters) -------------
+struct DevGas {
+  int nb, L;
+  double inv_de, nu_hat, inv_nu_hat;
+  const double* nu_tot;   // [nb]      total real-collision rate per bin (= cum[b][L-1])
+  const double* cum;      // [nb][L]   cumulative rates, row-major by bin
+  const double* loss;     // [L]
+  const double* recoil;   // [L]
+  const double* w;        // [L]
+  const uint8_t* type;    // [L]
+};
+
+struct DevSlab {
+  double z_lo, z_hi;
+  double E[3];
+  double org[3], inv_h[3], span[2];   // span = (n-1)*h in x, y (bc none)
+  double P[2], inv_P[2];              // fold period per axis (periodic: P; mirror: 2P) and its inverse
+  double half[2];                     // mirror: P (reflect when q > half); else +inf
+  const float4* nodes;
+  int kind, nx, ny, nz, bc[2];
+};
+
+struct DevField {
+  DevSlab slab[AVM_MAX_SLABS];
+  int n_slabs;
+  int has_B;
+  double z_lo, z_hi;
+  double xy_lo[2], xy_hi[2];
+  double B[3], bh[3], Bn2, omega, inv_omega;
+};
+
+// ---- Philox4x32-10 (Salmon et al., SC'11) — DESIGN.md §3 "Uniforms" --------------------------------------
+struct U4 { uint32_t w0, w1, w2, w3; };
+
+__device__ __forceinline__ U4 philox(uint64_t seed, uint64_t id, uint32_t n, uint32_t block) {
+  uint32_t c0 = n, c1 = block, c2 = (uint32_t)id, c3 = (uint32_t)(id >> 32);
+  uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+    const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+    c0 = hi1 ^ c1 ^ k0; c1 = lo1; c2 = hi0 ^ c3 ^ k1; c3 = lo0;
+    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+  }
+  return U4{c0, c1, c2, c3};
+}
+
+// u = ((x >> 12) + 0.5) * 2^-52 with x = hi:lo — strictly inside (0,1), exactly representable.
+__device__ __forceinline__ double to_unit(uint32_t hi, uint32_t lo) {
+  // Build the double 1.m directly: mantissa = top 52 bits of x, value in [1,2); subtract 1 and add 2^-53.
+  const uint32_t mh = hi >> 12, ml = (hi << 20) | (lo >> 12);
+  const double one_m = __hiloint2double((int)(0x3FF00000u | mh), (int)ml);   // 1 + (x>>12) 2^-52, exact
+  return (one_m - 1.0) + 1.1102230246251565e-16;                            // both steps exact
+}
+
+// ---- field (S0, R14, R15) -------------------------------------------------------------------------------
+__device__ __forceinline__ double f2d(float v) { return (double)v; }
+
+// Fold coordinate `q = x - org` of axis ax into the stored cell.  Returns false when outside with bc none.
+__device__ __forceinline__ bool fold_axis(const DevSlab& s, int ax, double x, double& q, bool& flip) {
+  flip = false;
+  q = x - s.org[ax];
+  const int bc = s.bc[ax];
+  if (bc == 0) return q >= 0.0 && q <= s.span[ax];
+  const double P = s.P[ax];
+  q = q - P * floor(q * s.inv_P[ax]);
+  if (q >= P || q < 0.0) q = 0.0;
+  if (q > s.half[ax]) { q = P - q; flip = true; }
+  return true;
+}
+
+__device__ __forceinline__ void cell_of(double s, int n, int& i, double& w) {
+  i = (int)floor(s);
+  i = min(i, n - 2);
+  i = max(i, 0);
+  w = s - (double)i;
+}
+
+__device__ __forceinline__ double lerp3(double c000, double c100, double c010, double c110, double c001,
+                                        double c101, double c011, double c111, double wx, double wy, double wz) {
+  const double c00 = c000 + wx * (c100 - c000);
+  const double c10 = c010 + wx * (c110 - c010);
+  const double c01 = c001 + wx * (c101 - c001);
+  const double c11 = c011 + wx * (c111 - c011);
+  const double c0 = c00 + wy * (c10 - c00);
+  const double c1 = c01 + wy * (c11 - c01);
+  return c0 + wz * (c1 - c0);
+}
+
+// Grid lookup inside slab s (z already known to lie in the slab).  Returns false when x/y leave a bc-none grid.
+__device__ __forceinline__ bool grid_at(const DevSlab& s, double x, double y, double z, double& Ex, double& Ey,
+                                        double& Ez, double& mask) {
+  double qx, qy;
+  bool fx, fy;
+  if (!fold_axis(s, 0, x, qx, fx)) return false;
+  if (!fold_axis(s, 1, y, qy, fy)) return false;
+  int i, j, k;
+  double wx, wy, wz;
+  cell_of(qx * s.inv_h[0], s.nx, i, wx);
+  cell_of(qy * s.inv_h[1], s.ny, j, wy);
+  cell_of((z - s.org[2]) * s.inv_h[2], s.nz, k, wz);
+  const float4* p = s.nodes + ((size_t)k * s.ny + j) * s.nx + i;
+  const size_t sy = (size_t)s.nx, sz = (size_t)s.nx * s.ny;
+  const float4 n000 = __ldg(p), n100 = __ldg(p + 1);
+  const float4 n010 = __ldg(p + sy), n110 = __ldg(p + sy + 1);
+  const float4 n001 = __ldg(p + sz), n101 = __ldg(p + sz + 1);
+  const float4 n011 = __ldg(p + sz + sy), n111 = __ldg(p + sz + sy + 1);
+  const double ex = lerp3(f2d(n000.x), f2d(n100.x), f2d(n010.x), f2d(n110.x), f2d(n001.x), f2d(n101.x), f2d(n011.x), f2d(n111.x), wx, wy, wz);
+  const double ey = lerp3(f2d(n000.y), f2d(n100.y), f2d(n010.y), f2d(n110.y), f2d(n001.y), f2d(n101.y), f2d(n011.y), f2d(n111.y), wx, wy, wz);
+  Ez = lerp3(f2d(n000.z), f2d(n100.z), f2d(n010.z), f2d(n110.z), f2d(n001.z), f2d(n101.z), f2d(n011.z), f2d(n111.z), wx, wy, wz);
+  mask = lerp3(f2d(n000.w), f2d(n100.w), f2d(n010.w), f2d(n110.w), f2d(n001.w), f2d(n101.w), f2d(n011.w), f2d(n111.w), wx, wy, wz);
+  Ex = fx ? -ex : ex;
+  Ey = fy ? -ey : ey;
+  return true;
+}
+
+// Field and mask at r.  Returns the slab index (>= 0) or -status when r is outside the domain.
+// UNIFORM1 = the field is one uniform slab (configs 1-3): no dispatch, no loads.
+template <bool UNIFORM1>
+__device__ __forceinline__ int field_at(const DevField& f, double x, double y, double z, double& Ex, double& Ey,
+                                        double& Ez, double& mask) {
+  if (z < f.z_lo) return -AVM_LEFT_ZLO;
+  if (z > f.z_hi) return -AVM_LEFT_ZHI;
+  // written so that NaN coordinates fail the test (status 3), like the oracle
+  if (!(x >= f.xy_lo[0] && x <= f.xy_hi[0] && y >= f.xy_lo[1] && y <= f.xy_hi[1] && z == z)) return -AVM_LEFT_XY;
+  if (UNIFORM1) {
+    Ex = f.slab[0].E[0]; Ey = f.slab[0].E[1]; Ez = f.slab[0].E[2]; mask = 1.0;
+    return 0;
+  }
+  int si = f.n_slabs - 1;
+  for (int i = f.n_slabs - 2; i >= 0; --i) if (z < f.slab[i].z_hi) si = i;
+  const DevSlab& s = f.slab[si];
+  if (s.kind == 0) { Ex = s.E[0]; Ey = s.E[1]; Ez = s.E[2]; mask = 1.0; return si; }
+  if (!grid_at(s, x, y, z, Ex, Ey, Ez, mask)) return -AVM_LEFT_XY;
+  return si;
+}
+
+// ---- S2-S3: free flight of duration dt in constant E (and B) from (r, v) ---------------------------------
+template <bool HASB>
+__device__ __forceinline__ void flight(const DevField& f, double Ex, double Ey, double Ez, double dt, double& x,
+                                       double& y, double& z, double& vx, double& vy, double& vz) {
+  const double ax = -kKappa * Ex, ay = -kKappa * Ey, az = -kKappa * Ez;
+  if (!HASB) {
+    const double h = 0.5 * dt * dt;
+    x = (x + vx * dt) + ax * h; y = (y + vy * dt) + ay * h; z = (z + vz * dt) + az * h;
+    vx = vx + ax * dt; vy = vy + ay * dt; vz = vz + az * dt;
+  } else {
+    const double bx = f.bh[0], by = f.bh[1], bz = f.bh[2];
+    const double a_b = ax * bx + ay * by + az * bz;
+    const double v_b = vx * bx + vy * by + vz * bz;
+    const double sc = kExBUnit / f.Bn2;
+    const double dx_ = sc * (Ey * f.B[2] - Ez * f.B[1]);      // E x B drift velocity
+    const double dy_ = sc * (Ez * f.B[0] - Ex * f.B[2]);
+    const double dz_ = sc * (Ex * f.B[1] - Ey * f.B[0]);
+    const double px = v_b * bx, py = v_b * by, pz = v_b * bz;  // v parallel
+    const double qx = a_b * bx, qy = a_b * by, qz = a_b * bz;  // a parallel
+    const double wx = vx - px - dx_, wy = vy - py - dy_, wz = vz - pz - dz_;
+    const double cx = by * wz - bz * wy, cy = bz * wx - bx * wz, cz = bx * wy - by * wx;   // b x w0
+    const double th = f.omega * dt;
+    double sh, ch;
+    sincos(0.5 * th, &sh, &ch);
+    const double sn = 2.0 * sh * ch, vers = 2.0 * sh * sh, cs = 1.0 - vers;
+    const double h = 0.5 * dt * dt, io = f.inv_omega;
+    x = x + px * dt + qx * h + dx_ * dt + (wx * sn + cx * vers) * io;
+    y = y + py * dt + qy * h + dy_ * dt + (wy * sn + cy * vers) * io;
+    z = z + pz * dt + qz * h + dz_ * dt + (wz * sn + cz * vers) * io;
+    vx = px + qx * dt + dx_ + wx * cs + cx * sn;
+    vy = py + qy * dt + dy_ + wy * cs + cy * sn;
+    vz = pz + qz * dt + dz_ + wz * cs + cz * sn;
+  }
+}
+
+// ---- S9: collision outcome ------------------------------------------------------------------------------
+struct Child { double e, u6, u7; };   // secondary: energy and the two uniforms of its isotropic direction
+
+// S9d: rotate unit vector k by polar (ct, st) and azimuth (cphi, sphi) about itself (Duff et al. 2017 basis).
+__device__ __forceinline__ void deflect(double& kx, double& ky, double& kz, double ct, double st, double cphi,
+                                        double sphi) {
+  const double sg = copysign(1.0, kz);
+  const double A = -1.0 / (sg + kz);
+  const double Bq = kx * ky * A;
+  const double b1x = 1.0 + sg * kx * kx * A, b1y = sg * Bq, b1z = -sg * kx;
+  const double b2x = Bq, b2y = sg + ky * ky * A, b2z = -ky;
+  const double nx = ct * kx + st * (cphi * b1x + sphi * b2x);
+  const double ny = ct * ky + st * (cphi * b1y + sphi * b2y);
+  const double nz = ct * kz + st * (cphi * b1z + sphi * b2z);
+  const double inv = 1.0 / sqrt(nx * nx + ny * ny + nz * nz);
+  kx = nx * inv; ky = ny * inv; kz = nz * inv;
+}
+
+__device__ __forceinline__ void child_direction(double u6, double u7, double& kx, double& ky, double& kz) {
+  const double sc = 2.0 * sqrt(u6 * (1.0 - u6));
+  double s, c;
+  sincospi(2.0 * u7, &s, &c);
+  kx = sc * c; ky = sc * s; kz = 1.0 - 2.0 * u6;
+}
+
+__device__ __forceinline__ uint64_t child_id_of(uint64_t seed, uint64_t id, uint32_t n_s) {
+  const U4 w = philox(seed, id, n_s, kBlockChildId);
+  return (uint64_t)w.w0 | ((uint64_t)w.w1 << 32);
+}
+
+// Real collision of level l at energy e1, direction k (unit).  type/loss/recoil/w are the level's parameters.
+// Returns the new energy; updates k; fills `ch` and returns spawn=true for an ionisation.  *loss_out = energy
+// leaving the electron population (tally).  Attachment is handled by the caller (S9a).
+__device__ __forceinline__ double collide(uint64_t seed, uint64_t id, uint32_t n_s, int type, double lv_loss,
+                                          double lv_recoil, double lv_w, double e1, double& kx, double& ky,
+                                          double& kz, bool& spawn, Child& ch, double& loss_out) {
+  const U4 r1 = philox(seed, id, n_s, 1u);
+  const double u3 = to_unit(r1.w0, r1.w1), u4 = to_unit(r1.w2, r1.w3);
+  const double ct = 1.0 - 2.0 * u3;
+  const double st = 2.0 * sqrt(u3 * (1.0 - u3));
+  double sphi, cphi;
+  sincospi(2.0 * u4, &sphi, &cphi);
+  double e2;
+  spawn = false;
+  if (type == AVM_ELASTIC) {
+    e2 = e1 * (1.0 - lv_recoil * (1.0 - ct));
+    loss_out = e1 - e2;
+  } else if (type == AVM_EXCITATION) {
+    e2 = fmax(e1 - lv_loss, kEpsFloor);
+    loss_out = e1 - e2;
+  } else {   // ionisation: Opal-Peterson-Beaty sharing (R10)
+    const U4 r2 = philox(seed, id, n_s, 2u);
+    const U4 r3 = philox(seed, id, n_s, 3u);
+    const double u5 = to_unit(r2.w0, r2.w1);
+    ch.u6 = to_unit(r2.w2, r2.w3);
+    ch.u7 = to_unit(r3.w0, r3.w1);
+    const double ea = fmax(e1 - lv_loss, 0.0);
+    const double es = lv_w * tan(u5 * atan(ea / (2.0 * lv_w)));
+    e2 = fmax(ea - es, kEpsFloor);
+    ch.e = fmax(es, kEpsFloor);
+    spawn = true;
+    loss_out = e1 - e2 - ch.e;
+  }
+  deflect(kx, ky, kz, ct, st, cphi, sphi);
+  return e2;
+}
+
+// S8: smallest l with cum[b][l] > x (x < cum[b][L-1] is known).
+__device__ __forceinline__ int select_level(const DevGas& g, int b, double xr) {
+  const double* row = g.cum + (size_t)b * g.L;
+  int l = 0;
+  while (l < g.L - 1 && __ldg(row + l) <= xr) ++l;
+  return l;
+}
+
+}  // namespace avm

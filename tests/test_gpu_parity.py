@@ -1,0 +1,373 @@
+"""GPU parity: the CUDA path (through the C ABI of include/avm.h) against the oracle, element by element.
+
+Tolerance T: continuous outputs agree to 1e-12 relative to
+max(|q_in|, |q_cpu|, q_scale), q_scale = |r' - r| for positions, 1 for direction components, e' for energies;
+discrete outputs (bin, null/real, level, status, child id) are identical.
+"""
+import numpy as np
+import pytest
+from scipy import stats
+
+from paper_2509_15377_b200.gen import fields, gas, primaries
+
+pytestmark = pytest.mark.gpu
+INF = float("inf")
+RTOL = 1e-12
+
+
+@pytest.fixture(scope="module")
+def ctx(avm):
+    return avm.ctx_create(0)
+
+
+def _states(n, rng, e_lo=0.01, e_hi=39.0, box=1e-3, center=(0, 0, 0)):
+    k = rng.normal(size=(3, n)); k /= np.linalg.norm(k, axis=0)
+    st = np.zeros((8, n))
+    st[0:3] = rng.uniform(-box, box, size=(3, n)) + np.array(center)[:, None]
+    st[3] = rng.uniform(0, 5, n)
+    st[4] = np.exp(rng.uniform(np.log(e_lo), np.log(e_hi), n))
+    st[5:8] = k
+    return st
+
+
+def assert_step_parity(cpu, gpu, st_in, what=""):
+    """Tolerance T on one batch of steps.  Returns the number of compared items."""
+    n = st_in.shape[1]
+    assert np.array_equal(cpu.event, gpu.event), f"{what}: events differ at {np.flatnonzero(cpu.event != gpu.event)[:5]}"
+    assert np.array_equal(cpu.status, gpu.status), what
+    assert np.array_equal(cpu.bin, gpu.bin), what
+    assert np.array_equal(cpu.child_id, gpu.child_id), what
+    dr = np.linalg.norm(cpu.state[0:3] - st_in[0:3], axis=0)
+    for c in range(3):
+        scale = np.maximum.reduce([np.abs(st_in[c]), np.abs(cpu.state[c]), dr])
+        err = np.abs(gpu.state[c] - cpu.state[c])
+        assert np.all(err <= RTOL * scale), f"{what}: position {c} rel err {np.max(err / np.maximum(scale, 1e-300)):.3e}"
+    err = np.abs(gpu.state[3] - cpu.state[3])
+    assert np.all(err <= RTOL * np.maximum(np.abs(cpu.state[3]), np.abs(st_in[3]))), what
+    # energies: scale e' (energy after the flight) guards the e' - loss cancellation; e' >= e'' always
+    e_scale = np.maximum.reduce([st_in[4], cpu.state[4]])
+    ion = cpu.child[4] > 0
+    e_scale = np.where(ion, np.maximum(e_scale, cpu.state[4] + cpu.child[4] + 20.0), e_scale)
+    err = np.abs(gpu.state[4] - cpu.state[4])
+    assert np.all(err <= RTOL * e_scale), f"{what}: energy rel err {np.max(err / e_scale):.3e}"
+    for c in range(5, 8):
+        assert np.all(np.abs(gpu.state[c] - cpu.state[c]) <= RTOL), f"{what}: direction {c - 5} err {np.abs(gpu.state[c] - cpu.state[c]).max():.3e}"
+    # children
+    for c in range(3):
+        scale = np.maximum.reduce([np.abs(st_in[c]), np.abs(cpu.child[c]), dr])
+        assert np.all(np.abs(gpu.child[c] - cpu.child[c]) <= RTOL * scale), what
+    assert np.all(np.abs(gpu.child[3] - cpu.child[3]) <= RTOL * np.maximum(np.abs(cpu.child[3]), 1e-300) + 0.0), what
+    assert np.all(np.abs(gpu.child[4] - cpu.child[4]) <= RTOL * e_scale), what
+    for c in range(5, 8):
+        assert np.all(np.abs(gpu.child[c] - cpu.child[c]) <= RTOL), what
+    return n
+
+
+def _random_map(rng, nx=9, ny=11, nz=13, e_scale=4e4):
+    nodes = rng.normal(size=(nz, ny, nx, 4)).astype(np.float32) * e_scale
+    m = (rng.uniform(size=(nz, ny, nx)) > 0.08).astype(np.float32)
+    nodes[..., 3] = m
+    return nodes
+
+
+# --------------------------------------------------------------------------------------------------------
+def test_c1_device_philox_bit_exact(avm, ctx, oracle):
+    """C1 on the device: words and uniforms equal the oracle's (itself pinned to ATen's engine) bit for bit,
+    including block 0xFFFFFFFF (child ids) and n = 0xFFFFFFFE (primaries)."""
+    rng = np.random.default_rng(1)
+    n = 5000
+    ids = rng.integers(0, 2 ** 64, n, dtype=np.uint64)
+    ns = rng.integers(0, 2 ** 32, n, dtype=np.uint64).astype(np.uint32)
+    bl = rng.choice(np.array([0, 1, 2, 3, 0xFFFFFFFF], dtype=np.uint32), n)
+    ns[:5] = [0, 1, 0xFFFFFFFE, 0xFFFFFFF0, 0xFFFFFFFF]
+    ids[:3] = [0, 1, 2 ** 64 - 1]
+    for seed in (0, 1, 0xDEADBEEFCAFEF00D):
+        w, u = avm.philox_batch(ctx, seed, ids, ns, bl)
+        for i in range(0, n, 7):
+            wo = oracle.philox(seed, int(ids[i]), int(ns[i]), int(bl[i]))
+            assert np.array_equal(w[i], wo)
+            ua, ub = oracle.uniform_pair(seed, int(ids[i]), int(ns[i]), int(bl[i]))
+            assert u[i, 0] == ua and u[i, 1] == ub
+        assert np.all((u > 0) & (u < 1))
+
+
+@pytest.mark.parametrize("bc", [(fields.BC_MIRROR, fields.BC_MIRROR), (fields.BC_PERIODIC, fields.BC_NONE),
+                                (fields.BC_NONE, fields.BC_MIRROR)])
+def test_field_eval_parity(avm, ctx, oracle, bc):
+    """S0/R14/R15: slab dispatch, fold and trilinear interpolation, GPU vs oracle on random points that span
+    several periods, the slab boundaries and the outside."""
+    rng = np.random.default_rng(2)
+    nodes = _random_map(rng)
+    h = (1e-4, 1.5e-4, 2e-4)
+    org = (-2e-4, 1e-4, 0.0)
+    Px, Py = 8 * h[0], 10 * h[1]
+    g1 = fields.grid_slab(nodes, org, h, 0.0, 12 * h[2], bc[0], bc[1], Px, Py)
+    u0 = fields.Slab(-5e-4, 0.0, fields.KIND_UNIFORM, (100.0, -200.0, 3000.0))
+    u2 = fields.Slab(12 * h[2], 12 * h[2] + 4e-4, fields.KIND_UNIFORM, (0.0, 0.0, -500.0))
+    fd = fields.FieldDesc([u0, g1, u2], (0, 0, 0), (-40e-4, -50e-4), (40e-4, 50e-4))
+    n = 40000
+    r = np.vstack([rng.uniform(-45e-4, 45e-4, n), rng.uniform(-55e-4, 55e-4, n), rng.uniform(-6e-4, 30e-4, n)])
+    r[2, :50] = [0.0, 12 * h[2], -5e-4, 12 * h[2] + 4e-4, 6 * h[2]] * 10     # exactly on slab faces
+    Ec, mc, sc = oracle.field_eval(fd, r)
+    fg = avm.field_create(ctx, fd)
+    Eg, mg, sg = avm.field_eval(ctx, fg, r)
+    assert np.array_equal(sc, sg)
+    inside = sc >= 0
+    assert inside.sum() > n // 4 and (sc == 1).sum() > n // 8
+    scale = np.abs(nodes[..., :3]).max()
+    assert np.all(np.abs(Eg - Ec)[:, inside] <= 1e-12 * scale)
+    assert np.all(np.abs(mg - mc)[inside] <= 1e-12)
+
+
+@pytest.mark.parametrize("B", [(0.0, 0.0, 0.0), (0.0, 0.5, 0.8660254037844387)])
+@pytest.mark.parametrize("seed", [0, 0x1234567890ABCDEF])
+def test_step_parity_uniform_g0(avm, ctx, oracle, g0, B, seed):
+    """Per-collision parity (north_star level 1) on gas G0, uniform E (configs 1-3), 2.6e5 random states spanning
+    0.01-39 eV, all level types, boundary exits; collision indices up to the reserved range."""
+    rng = np.random.default_rng(3)
+    n = 1 << 18
+    st = _states(n, rng, box=30e-4, center=(0, 0, 30e-4))
+    fd = fields.uniform_gap((0.0, 0.0, -60000.0), 0.0, 60e-4, B)
+    ids = rng.integers(0, 2 ** 64, n, dtype=np.uint64)
+    nidx = rng.integers(0, 2 ** 32 - 64, n, dtype=np.uint64).astype(np.uint32)
+    cpu = oracle.step_batch(g0, fd, seed, st, ids, nidx, t_max=4.9)
+    gg, fg = avm.gas_create(ctx, g0), avm.field_create(ctx, fd)
+    gpu = avm.step_batch(ctx, gg, fg, seed, st, ids, nidx, t_max=4.9)
+    assert_step_parity(cpu, gpu, st, f"B={B}")
+    # the batch really exercises every branch
+    ev = cpu.event
+    assert (ev == -1).sum() > n // 4 and (ev == 0).sum() > 100 and (ev == 1).sum() > 100
+    assert all((ev == l).sum() > 0 for l in range(2, 17)), np.bincount(ev[ev >= 0], minlength=17)
+    assert set(np.unique(cpu.status)) >= {0, 1, 2, 5, 6}
+    # states near the step limit stop with status 7
+    nidx2 = np.full(1000, 0xFFFFFFEF, dtype=np.uint32)
+    c2 = oracle.step_batch(g0, fd, seed, st[:, :1000], ids[:1000], nidx2)
+    g2 = avm.step_batch(ctx, gg, fg, seed, st[:, :1000], ids[:1000], nidx2)
+    assert_step_parity(c2, g2, st[:, :1000])
+    assert (c2.status == 7).sum() > 100
+
+
+def test_step_parity_grid_slabs(avm, ctx, oracle, g0):
+    """Per-collision parity with grid maps: mirror fold, material absorption, slab dispatch, B != 0."""
+    rng = np.random.default_rng(4)
+    nodes = _random_map(rng, 12, 14, 20, e_scale=5e4)
+    h = (1e-4, 1e-4, 1e-4)
+    Px, Py = 10e-4, 12e-4
+    g1 = fields.grid_slab(nodes, (0, 0, 0), h, 0.0, 19e-4, fields.BC_MIRROR, fields.BC_MIRROR, Px, Py)
+    u2 = fields.Slab(19e-4, 40e-4, fields.KIND_UNIFORM, (0.0, 0.0, 3000.0))
+    n = 1 << 17
+    for B in ((0, 0, 0), (0.3, -0.2, 0.9)):
+        fd = fields.FieldDesc([g1, u2], B)
+        st = _states(n, rng, box=20e-4, center=(3e-4, -7e-4, 20e-4))
+        ids = rng.integers(0, 2 ** 64, n, dtype=np.uint64)
+        nidx = rng.integers(0, 1 << 20, n, dtype=np.uint64).astype(np.uint32)
+        cpu = oracle.step_batch(g0, fd, 5, st, ids, nidx)
+        gpu = avm.step_batch(ctx, avm.gas_create(ctx, g0), avm.field_create(ctx, fd), 5, st, ids, nidx)
+        assert_step_parity(cpu, gpu, st, f"grid B={B}")
+        assert (cpu.status == 4).sum() > 100 and (cpu.status == 0).sum() > n // 4
+
+
+def test_step_parity_textbook_gases(avm, ctx, oracle):
+    """The small gases of the pins: every step real (nu_hat = nu), ionisation with threshold 0, attachment only."""
+    rng = np.random.default_rng(5)
+    n = 50000
+    st = _states(n, rng, e_hi=200.0)
+    fd = fields.uniform_gap((1500.0, -700.0, 2500.0), -1.0, 1.0, (0.1, 0.2, -0.4))
+    ids = np.arange(n, dtype=np.uint64)
+    nidx = np.zeros(n, dtype=np.uint32)
+    for g in (gas.constant_elastic(100.0, 0.013), gas.ionisation_only(80.0, w=10.0), gas.attachment_only(2.0, nu_hat=3.0),
+              gas.multi_level_constant([5.0, 0.0, 20.0, 1.0, 14.0],
+                                       [gas.ELASTIC, gas.EXCITATION, gas.EXCITATION, gas.ATTACHMENT, gas.ELASTIC],
+                                       loss=[0, 1.0, 2.5, 0, 0], recoil=[1e-3, 0, 0, 0, 0.5], nu_hat=60.0)):
+        cpu = oracle.step_batch(g, fd, 9, st, ids, nidx)
+        gpu = avm.step_batch(ctx, avm.gas_create(ctx, g), avm.field_create(ctx, fd), 9, st, ids, nidx)
+        assert_step_parity(cpu, gpu, st, g.names[0])
+
+
+# ---- whole avalanches -------------------------------------------------------------------------------------
+def assert_run_same_seed(cpu, gpu, n_levels, min_identical=0.999):
+    """Same seed, same ids: the two runs are the same avalanche electron by electron until rounding flips a
+    discrete decision.  Counts must agree exactly for >= min_identical of the electrons."""
+    c, g = cpu.sorted_by_id(), gpu.sorted_by_id()
+    common, ic, ig = np.intersect1d(c.id, g.id, return_indices=True)
+    assert len(common) >= min_identical * max(c.n, g.n), (c.n, g.n, len(common))
+    same = (c.n_steps[ic] == g.n_steps[ig]) & (c.status[ic] == g.status[ig]) & (c.avalanche[ic] == g.avalanche[ig])
+    assert same.mean() >= min_identical, same.mean()
+    ic, ig = ic[same], ig[same]
+    # identical histories: endpoints agree to accumulated rounding (1e-9 of the path scale is generous)
+    scale = np.maximum(np.abs(c.end[0:3, ic]).max(), 1e-4)
+    assert np.abs(c.end[0:3, ic] - g.end[0:3, ig]).max() <= 1e-9 * scale
+    assert np.all(np.abs(c.end[3, ic] - g.end[3, ig]) <= 1e-9 * np.maximum(c.end[3, ic], 1e-6))
+    assert np.all(np.abs(c.end[4, ic] - g.end[4, ig]) <= 1e-8 * np.maximum(c.end[4, ic], 1.0))
+    assert np.abs(c.birth[:, ic] - g.birth[:, ig]).max() <= 1e-9 * np.maximum(np.abs(c.birth[:, ic]).max(), 1.0)
+    return same.mean(), len(common)
+
+
+def test_config1_same_seed_identical_avalanches(avm, ctx, oracle, g0):
+    """BASELINE config 1 in full, seed 0: same ids, same step counts, same statuses, same tallies."""
+    fd = fields.uniform_gap((0, 0, -30000.0), 0.0, 50e-4)
+    p = primaries.isotropic_primaries(1000, 0)
+    cpu = oracle.run(g0, fd, p, seed=0)
+    gpu = avm.simulate(ctx, avm.gas_create(ctx, g0), avm.field_create(ctx, fd), p, seed=0)
+    frac, n = assert_run_same_seed(cpu, gpu, g0.n_levels)
+    L = g0.n_levels
+    if frac == 1.0 and cpu.n == gpu.n:
+        assert np.array_equal(cpu.tallies_u64, gpu.tallies_u64)
+        assert np.array_equal(cpu.per_avalanche, gpu.per_avalanche)
+    assert abs(int(gpu.tallies_u64[L + 3]) - int(cpu.tallies_u64[L + 3])) <= 1e-3 * int(cpu.tallies_u64[L + 3])
+    assert np.allclose(gpu.tallies_f64, cpu.tallies_f64, rtol=1e-3)
+    # bookkeeping invariants on the GPU result itself (C11)
+    t = gpu.tallies_u64
+    assert gpu.n == 1000 + int(t[14] + t[15]) and (gpu.status == 5).sum() == int(t[16])
+    assert int(gpu.n_steps.sum()) == int(t[L + 3]) and int(t[:L].sum()) == int(t[L + 1])
+    assert np.all(gpu.status != 0) and len(np.unique(gpu.id)) == gpu.n
+    assert np.array_equal(np.bincount(gpu.avalanche, minlength=1000), gpu.per_avalanche[:, 0])
+
+
+def test_config2_reduced_same_seed(avm, ctx, oracle, g0):
+    """BASELINE config 2 (60 kV/cm, 128 um) with 12 primaries: avalanches of 10^3-10^4 exercise append and
+    lane refill; same-seed comparison electron by electron, then drift velocity and alpha within 1 %."""
+    fd = fields.uniform_gap((0, 0, -60000.0), 0.0, 128e-4)
+    p = primaries.isotropic_primaries(12, 0)
+    cpu = oracle.run(g0, fd, p, seed=0, capacity=1 << 18, n_threads=8)
+    gpu = avm.simulate(ctx, avm.gas_create(ctx, g0), avm.field_create(ctx, fd), p, seed=0, capacity=1 << 18)
+    assert cpu.n > 3000
+    assert_run_same_seed(cpu, gpu, g0.n_levels, min_identical=0.99)
+    Wc = cpu.tallies_f64[2] / cpu.tallies_f64[3]; Wg = gpu.tallies_f64[2] / gpu.tallies_f64[3]
+    assert abs(Wg / Wc - 1) < 0.01
+    ac = (float(cpu.tallies_u64[14] + cpu.tallies_u64[15]) - float(cpu.tallies_u64[16])) / cpu.tallies_f64[2]
+    ag = (float(gpu.tallies_u64[14] + gpu.tallies_u64[15]) - float(gpu.tallies_u64[16])) / gpu.tallies_f64[2]
+    assert abs(ag / ac - 1) < 0.01
+
+
+def test_relaunch_guard_gives_same_run(avm, ctx, g0):
+    """a-11: a tiny per-launch iteration guard forces many relaunches (electrons parked in their slots and picked up
+    again through tickets); the avalanche must be the same as in one launch."""
+    fd = fields.uniform_gap((0, 0, -60000.0), 0.0, 60e-4)
+    p = primaries.isotropic_primaries(64, 3)
+    gg, fg = avm.gas_create(ctx, g0), avm.field_create(ctx, fd)
+    one = avm.simulate(ctx, gg, fg, p, seed=3, capacity=1 << 16)
+    _, l1 = avm.run_stats(ctx)
+    many = avm.simulate(ctx, gg, fg, p, seed=3, capacity=1 << 16, max_iters_per_launch=97)
+    _, l2 = avm.run_stats(ctx)
+    assert l1 == 1 and l2 > 10
+    assert_run_same_seed(one, many, g0.n_levels, min_identical=0.99)
+    # one CTA per SM instead of the default: scheduling must not matter either
+    few = avm.simulate(ctx, gg, fg, p, seed=3, capacity=1 << 16, n_ctas_per_sm=1)
+    assert_run_same_seed(one, few, g0.n_levels, min_identical=1.0)
+    assert np.array_equal(one.tallies_u64, few.tallies_u64)
+
+
+def test_run_with_magnetic_field_and_time_cut(avm, ctx, oracle, g0):
+    """Config-3-like: 1 kV/cm, B = 1 T at 30 degrees, time cut so the oracle finishes: same-seed parity."""
+    fd = fields.uniform_gap((0, 0, -1000.0), 0.0, 1.0, (0.0, 0.5, 0.8660254037844387))
+    p = primaries.isotropic_primaries(300, 0, pos=(0, 0, 0.02))
+    cpu = oracle.run(g0, fd, p, seed=0, t_max=2.0, n_threads=8)
+    gpu = avm.simulate(ctx, avm.gas_create(ctx, g0), avm.field_create(ctx, fd), p, seed=0, t_max=2.0)
+    assert_run_same_seed(cpu, gpu, g0.n_levels, min_identical=0.99)
+    assert (gpu.status == 6).sum() > 200
+
+
+def test_run_grid_map_same_seed(avm, ctx, oracle, g0):
+    """Grid slab + uniform slab with mirror fold and material: whole-run parity incl. status 4 endpoints."""
+    rng = np.random.default_rng(6)
+    nz, ny, nx = 40, 13, 11
+    nodes = np.zeros((nz, ny, nx, 4), dtype=np.float32)
+    zz = np.arange(nz)[:, None, None]; yy = np.arange(ny)[None, :, None]; xx = np.arange(nx)[None, None, :]
+    nodes[..., 0] = 8000.0 * np.sin(np.pi * xx / (nx - 1)) * np.cos(0.3 * zz)
+    nodes[..., 1] = 6000.0 * np.sin(np.pi * yy / (ny - 1)) * np.sin(0.2 * zz)
+    nodes[..., 2] = 40000.0 + 15000.0 * np.cos(np.pi * xx / (nx - 1)) * np.cos(np.pi * yy / (ny - 1))
+    nodes[..., 3] = 1.0
+    nodes[15:20, :, :, 3] = ((xx - 5) ** 2 + (yy - 6) ** 2 < 9).astype(np.float32)       # a plate with a hole
+    h = (1e-4, 1e-4, 1e-4)
+    g1 = fields.grid_slab(nodes, (0, 0, 0), h, 0.0, 39e-4, fields.BC_MIRROR, fields.BC_MIRROR, 10e-4, 12e-4)
+    u0 = fields.Slab(-20e-4, 0.0, fields.KIND_UNIFORM, (0.0, 0.0, 30000.0))
+    fd = fields.FieldDesc([u0, g1])
+    p = primaries.isotropic_primaries(400, 7, pos=(0, 0, 38e-4), xy_box=((0, 10e-4), (0, 12e-4)))
+    cpu = oracle.run(g0, fd, p, seed=7, capacity=1 << 17, n_threads=8)
+    gpu = avm.simulate(ctx, avm.gas_create(ctx, g0), avm.field_create(ctx, fd), p, seed=7, capacity=1 << 17)
+    assert_run_same_seed(cpu, gpu, g0.n_levels, min_identical=0.99)
+    assert (cpu.status == 4).sum() > 20 and (cpu.status == 1).sum() > 20
+
+
+def test_statistical_parity_independent_seeds(avm, ctx, oracle, g0):
+    """north_star level 2: GPU seed 1 vs oracle seed 0 on a config-2-like gap (60 kV/cm, 100 um, forward
+    primaries): mean gain within 3 combined SE; KS p > 0.01 on endpoint z... energy and gain distributions."""
+    d = 100e-4
+    fd = fields.uniform_gap((0, 0, -60000.0), 0.0, d)
+    pc = primaries.isotropic_primaries(96, 0, forward=True); pc[:, 2] = 2e-4
+    pg = primaries.isotropic_primaries(96, 1, forward=True); pg[:, 2] = 2e-4
+    cpu = oracle.run(g0, fd, pc, seed=0, capacity=1 << 21, n_threads=8)
+    gpu = avm.simulate(ctx, avm.gas_create(ctx, g0), avm.field_create(ctx, fd), pg, seed=1, capacity=1 << 21)
+    gc, gg = cpu.per_avalanche[:, 0].astype(float), gpu.per_avalanche[:, 0].astype(float)
+    se = np.hypot(gc.std(ddof=1) / np.sqrt(len(gc)), gg.std(ddof=1) / np.sqrt(len(gg)))
+    assert abs(gc.mean() - gg.mean()) < 3 * se, (gc.mean(), gg.mean(), se)
+    assert stats.ks_2samp(gc, gg).pvalue > 0.01
+    anode_c, anode_g = cpu.status == 2, gpu.status == 2
+    assert stats.ks_2samp(cpu.end[4][anode_c][::7], gpu.end[4][anode_g][::7]).pvalue > 0.01      # thinned: electrons of one avalanche are correlated
+    assert stats.ks_2samp(cpu.end[3][anode_c][::97], gpu.end[3][anode_g][::97]).pvalue > 0.01
+    Wc = cpu.tallies_f64[2] / cpu.tallies_f64[3]; Wg = gpu.tallies_f64[2] / gpu.tallies_f64[3]
+    assert abs(Wg / Wc - 1) < 0.01, (Wc, Wg)
+    ac = (float(cpu.tallies_u64[14] + cpu.tallies_u64[15]) - float(cpu.tallies_u64[16])) / cpu.tallies_f64[2]
+    ag = (float(gpu.tallies_u64[14] + gpu.tallies_u64[15]) - float(gpu.tallies_u64[16])) / gpu.tallies_f64[2]
+    assert abs(ag / ac - 1) < 0.02, (ac, ag)
+
+
+def test_c13_yule_furry_on_gpu(avm, ctx):
+    """C13 on the CUDA path: the exact gain distribution through append + tickets + per-avalanche counts."""
+    nu_i, t_max, n_p = 5.0, 0.4, 20000
+    g = gas.ionisation_only(nu_i, nu_hat=12.0)
+    p = primaries.isotropic_primaries(n_p, 43, e_scale=50.0)
+    fd = fields.uniform_gap((0, 0, 0), -1e6, 1e6)
+    r = avm.simulate(ctx, avm.gas_create(ctx, g), avm.field_create(ctx, fd), p, seed=43, t_max=t_max, capacity=1 << 19)
+    size = r.per_avalanche[:, 0].astype(np.int64)
+    nbar = np.exp(nu_i * t_max)
+    assert abs(size.mean() - nbar) < 4 * np.sqrt(nbar * (nbar - 1) / n_p)
+    q = 1 - 1 / nbar
+    edges = np.array([1, 2, 3, 4, 5, 6, 8, 10, 13, 17, 22, 30, 10 ** 9])
+    obs = np.histogram(size, bins=edges)[0]
+    exp = n_p * (q ** (edges[:-1] - 1) - q ** (edges[1:] - 1))
+    assert stats.chisquare(obs, exp * obs.sum() / exp.sum()).pvalue > 1e-3
+    assert np.all(r.status == 6) and r.n == size.sum() and len(np.unique(r.id)) == r.n
+
+
+def test_edge_cases(avm, ctx, oracle, g0):
+    gg = avm.gas_create(ctx, g0)
+    fd = fields.uniform_gap((0, 0, -60000.0), 0.0, 60e-4)
+    fg = avm.field_create(ctx, fd)
+    # empty input
+    r = avm.simulate(ctx, gg, fg, np.zeros((0, 8)), seed=0, capacity=16)
+    assert r.n == 0 and r.tallies_u64.sum() == 0
+    # primaries outside the domain / past the time limit are finished at their birth point
+    p = primaries.fixed_primaries(5, pos=(0, 0, 10e-4), energy=2.0)
+    p[0, 2] = -1e-4; p[1, 2] = 61e-4; p[2, 3] = 9.0; p[3, 0] = np.nan
+    r = avm.simulate(ctx, gg, fg, p, seed=0, t_max=5.0, capacity=1 << 12)
+    c = oracle.run(g0, fd, p, seed=0, t_max=5.0, capacity=1 << 12)
+    rs, cs = r.sorted_by_id(), c.sorted_by_id()
+    assert list(rs.status[:4]) == [1, 2, 6, 3] == list(cs.status[:4])
+    assert np.all(rs.n_steps[:4] == 0) and rs.n == cs.n
+    # capacity overflow: flagged, run terminates, outputs hold `capacity` electrons
+    p = primaries.isotropic_primaries(32, 0, forward=True)
+    bufs = avm.RunBuffers(ctx, 64, 32, gg.n_levels)
+    rc, n = avm.run(ctx, gg, fg, p, bufs, seed=0, allow_overflow=True)
+    assert rc == avm.ERR_CAPACITY and n == 64 and "capacity" in avm.last_error()
+    res = avm.fetch(ctx, bufs, n)
+    assert np.all(res.status != 0)
+    with pytest.raises(avm.AvmError):
+        avm.run(ctx, gg, fg, p, bufs, seed=0)
+    # invalid arguments fail loudly
+    bad = gas.constant_elastic(10.0, 0.0, nu_hat=5.0)
+    with pytest.raises(avm.AvmError):
+        avm.gas_create(ctx, bad)
+    with pytest.raises(avm.AvmError):
+        avm.field_create(ctx, fields.FieldDesc([fields.Slab(1.0, 0.0)]))
+    # device-resident primaries and an id offset: shard [16, 32) of a job equals the same electrons of the whole job
+    import torch
+    p = primaries.isotropic_primaries(32, 5)
+    whole = avm.simulate(ctx, gg, fg, p, seed=5, capacity=1 << 14).sorted_by_id()
+    bufs = avm.RunBuffers(ctx, 1 << 14, 16, gg.n_levels)
+    rc, n = avm.run(ctx, gg, fg, torch.from_numpy(p[16:]).cuda(), bufs, seed=5, id_offset=16)
+    shard = avm.fetch(ctx, bufs, n).sorted_by_id()
+    sel = np.isin(whole.avalanche, np.arange(16, 32))
+    assert np.array_equal(whole.id[sel], shard.id) and np.array_equal(whole.n_steps[sel], shard.n_steps)
+    assert np.array_equal(whole.end[:, sel], shard.end)
