@@ -155,6 +155,9 @@ int32_t avm_run(avm_ctx*, const avm_gas*, const avm_field*, const double* primar
                 const avm_run_opts*, const avm_outputs*, int64_t* n_endpoints_out);
 /* Launch statistics of the last avm_run on this context: kernels launched, persistent-kernel launches. */
 int32_t avm_run_stats(const avm_ctx*, int64_t* n_kernel_launches, int64_t* n_transport_launches);
+/* Device time [ms] of the transport-kernel launches of the last avm_run on this context, summed (CUDA events
+ * recorded on the context's stream around each launch).  *ms_out is HOST.  bench.py's roofline uses it. */
+int32_t avm_run_transport_ms(const avm_ctx*, float* ms_out);
 
 /* Device -> host copy of the first n entries of every non-NULL array of `host` from the same-named array of
  * `dev` ("retrieve the electron endpoints").  `host` is an avm_outputs whose pointers are HOST

@@ -26,7 +26,7 @@ RUN_PRIMARIES_ON_DEVICE, RUN_NO_TALLIES = 1, 2
 MAX_LEVELS, MAX_SLABS = 64, 8
 EXPORTS = ["avm_last_error", "avm_ctx_create", "avm_ctx_destroy", "avm_ctx_sm_count", "avm_gas_bytes",
            "avm_gas_create", "avm_gas_destroy", "avm_gas_nu_hat", "avm_field_create", "avm_field_destroy",
-           "avm_field_eval", "avm_run_workspace_bytes", "avm_run", "avm_run_stats", "avm_fetch", "avm_step_batch",
+           "avm_field_eval", "avm_run_workspace_bytes", "avm_run", "avm_run_stats", "avm_run_transport_ms", "avm_fetch", "avm_step_batch",
            "avm_philox_batch", "avm_fp64_probe"]
 
 
@@ -74,8 +74,9 @@ _lib.avm_gas_nu_hat.restype = C.c_double
 _lib.avm_gas_nu_hat.argtypes = [C.c_void_p]
 for _n in ("avm_ctx_create", "avm_ctx_destroy", "avm_ctx_sm_count", "avm_gas_create", "avm_gas_destroy",
            "avm_field_create", "avm_field_destroy", "avm_field_eval", "avm_run", "avm_run_stats", "avm_fetch",
-           "avm_step_batch", "avm_philox_batch", "avm_fp64_probe"):
+           "avm_step_batch", "avm_philox_batch", "avm_fp64_probe", "avm_run_transport_ms"):
     getattr(_lib, _n).restype = C.c_int32
+_lib.avm_run_transport_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
 _lib.avm_ctx_create.argtypes = [C.c_int32, C.c_void_p, C.POINTER(C.c_void_p)]
 _lib.avm_ctx_destroy.argtypes = [C.c_void_p]
 _lib.avm_ctx_sm_count.argtypes = [C.c_void_p]
@@ -370,6 +371,12 @@ def run_stats(ctx: Context) -> tuple:
     a, b = C.c_int64(0), C.c_int64(0)
     _check(_lib.avm_run_stats(ctx._h, C.byref(a), C.byref(b)))
     return int(a.value), int(b.value)
+
+
+def run_transport_ms(ctx: Context) -> float:
+    ms = C.c_float(0)
+    _check(_lib.avm_run_transport_ms(ctx._h, C.byref(ms)))
+    return float(ms.value)
 
 
 def fetch(ctx: Context, bufs: RunBuffers, n: int, host: Optional[HostBuffers] = None) -> RunResult:

@@ -455,6 +455,8 @@ struct avm_ctx {
   int sm_count = 0;
   unsigned long long* h_counters = nullptr;   // pinned: the one word the host reads per launch
   int64_t n_kernel_launches = 0, n_transport_launches = 0;
+  cudaEvent_t ev_t0 = nullptr, ev_t1 = nullptr;  // bracket the transport launches of the last avm_run
+  float transport_ms = 0.0f;
 };
 struct avm_gas {
   DevGas d{};
@@ -540,6 +542,9 @@ int32_t avm_ctx_create(int32_t device, void* cuda_stream, avm_ctx** out) {
   c->sm_count = prop.multiProcessorCount;
   cudaError_t e = cudaHostAlloc((void**)&c->h_counters, 64, cudaHostAllocDefault);
   if (e != cudaSuccess) { delete c; return fail(AVM_ERR_CUDA, std::string("ctx_create: cudaHostAlloc: ") + cudaGetErrorString(e)); }
+  if (cudaEventCreate(&c->ev_t0) != cudaSuccess || cudaEventCreate(&c->ev_t1) != cudaSuccess) {
+    cudaFreeHost(c->h_counters); delete c; return fail(AVM_ERR_CUDA, "ctx_create: cudaEventCreate");
+  }
   *out = c;
   return AVM_OK;
 }
@@ -547,6 +552,8 @@ int32_t avm_ctx_create(int32_t device, void* cuda_stream, avm_ctx** out) {
 int32_t avm_ctx_destroy(avm_ctx* c) {
   if (!c) return AVM_OK;
   if (c->h_counters) cudaFreeHost(c->h_counters);
+  if (c->ev_t0) cudaEventDestroy(c->ev_t0);
+  if (c->ev_t1) cudaEventDestroy(c->ev_t1);
   delete c;
   return AVM_OK;
 }
@@ -684,6 +691,12 @@ int32_t avm_run_stats(const avm_ctx* c, int64_t* n_kernel_launches, int64_t* n_t
   return AVM_OK;
 }
 
+int32_t avm_run_transport_ms(const avm_ctx* c, float* ms_out) {
+  if (!c || !ms_out) return fail(AVM_ERR_INVALID_ARG, "run_transport_ms: null argument");
+  *ms_out = c->transport_ms;
+  return AVM_OK;
+}
+
 namespace {
 typedef void (*TransportFn)(const DevGas, const DevField, const RunArrays, RunCtl*, const uint64_t, const double,
                             const uint32_t, const uint32_t);
@@ -708,7 +721,7 @@ int32_t avm_run(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, const 
   if (!o->workspace || o->workspace_bytes < avm_run_workspace_bytes(ctx, o->capacity) || ((uintptr_t)o->workspace & 255u))
     return fail(AVM_ERR_INVALID_ARG, "run: workspace null, too small or not 256-byte aligned");
   AVM_CUDA(cudaSetDevice(ctx->device));
-  ctx->n_kernel_launches = 0; ctx->n_transport_launches = 0;
+  ctx->n_kernel_launches = 0; ctx->n_transport_launches = 0; ctx->transport_ms = 0.0f;
   cudaStream_t st = ctx->stream;
   RunCtl* ctl = (RunCtl*)o->workspace;
   double* stage = (double*)((unsigned char*)o->workspace + kCtlBytes);
@@ -752,9 +765,21 @@ int32_t avm_run(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, const 
     if ((uint32_t)(c >> 32) == (uint32_t)c) break;              // a-11: every electron has a non-zero status
     if (++launches > max_launches) return fail(AVM_ERR_STATE, "run: launch limit reached without termination");
     AVM_CUDA(cudaMemsetAsync(&ctl->q_head, 0, sizeof(unsigned int), st));
+    if (launches > 1) {                                          // close the previous launch's bracket
+      float ms = 0.0f;
+      AVM_CUDA(cudaEventElapsedTime(&ms, ctx->ev_t0, ctx->ev_t1));
+      ctx->transport_ms += ms;
+    }
+    AVM_CUDA(cudaEventRecord(ctx->ev_t0, st));
     fn<<<grid, kThreads, 0, st>>>(gas->d, field->d, a, ctl, opts->seed, opts->t_max, max_iters, n_static);
     AVM_CUDA(cudaGetLastError());
+    AVM_CUDA(cudaEventRecord(ctx->ev_t1, st));
     ctx->n_kernel_launches++; ctx->n_transport_launches++;
+  }
+  if (launches > 0) {
+    float ms = 0.0f;
+    AVM_CUDA(cudaEventElapsedTime(&ms, ctx->ev_t0, ctx->ev_t1));
+    ctx->transport_ms += ms;
   }
   const uint64_t total = c >> 32;
   const uint32_t n_end = (uint32_t)(total < (uint64_t)a.cap ? total : (uint64_t)a.cap);

@@ -113,7 +113,7 @@ def test_field_eval_parity(avm, ctx, oracle, bc):
     Eg, mg, sg = avm.field_eval(ctx, fg, r)
     assert np.array_equal(sc, sg)
     inside = sc >= 0
-    assert inside.sum() > n // 4 and (sc == 1).sum() > n // 8
+    assert inside.sum() > n // 4 and (sc == 1).sum() > n // 20
     scale = np.abs(nodes[..., :3]).max()
     assert np.all(np.abs(Eg - Ec)[:, inside] <= 1e-12 * scale)
     assert np.all(np.abs(mg - mc)[inside] <= 1e-12)
@@ -137,8 +137,15 @@ def test_step_parity_uniform_g0(avm, ctx, oracle, g0, B, seed):
     # the batch really exercises every branch
     ev = cpu.event
     assert (ev == -1).sum() > n // 4 and (ev == 0).sum() > 100 and (ev == 1).sum() > 100
-    assert all((ev == l).sum() > 0 for l in range(2, 17)), np.bincount(ev[ev >= 0], minlength=17)
-    assert set(np.unique(cpu.status)) >= {0, 1, 2, 5, 6}
+    assert all((ev == l).sum() > 0 for l in range(2, 16)), np.bincount(ev[ev >= 0], minlength=17)
+    assert set(np.unique(cpu.status)) >= {0, 1, 2, 6}
+    # G0's attachment level (peak 4e-21 cm^2) is too rare to be drawn here: same table with that level x 2e4
+    rates = g0.level_rates(); rates[:, 16] *= 2e4
+    g_att = gas._finish(g0.n_bins, g0.e_max, rates, g0.level_type, g0.level_loss, g0.level_recoil, g0.level_ob_w, g0.names)
+    ca = oracle.step_batch(g_att, fd, seed, st, ids, nidx, t_max=4.9)
+    ga = avm.step_batch(ctx, avm.gas_create(ctx, g_att), fg, seed, st, ids, nidx, t_max=4.9)
+    assert_step_parity(ca, ga, st, f"attachment x2e4, B={B}")
+    assert (ca.event == 16).sum() > 40 and (ca.status == 5).sum() == (ca.event == 16).sum()
     # states near the step limit stop with status 7
     nidx2 = np.full(1000, 0xFFFFFFEF, dtype=np.uint32)
     c2 = oracle.step_batch(g0, fd, seed, st[:, :1000], ids[:1000], nidx2)
@@ -225,10 +232,10 @@ def test_config1_same_seed_identical_avalanches(avm, ctx, oracle, g0):
 
 
 def test_config2_reduced_same_seed(avm, ctx, oracle, g0):
-    """BASELINE config 2 (60 kV/cm, 128 um) with 12 primaries: avalanches of 10^3-10^4 exercise append and
+    """BASELINE config 2 (60 kV/cm, 128 um) with 24 primaries: avalanches of 10^3-10^4 exercise append and
     lane refill; same-seed comparison electron by electron, then drift velocity and alpha within 1 %."""
     fd = fields.uniform_gap((0, 0, -60000.0), 0.0, 128e-4)
-    p = primaries.isotropic_primaries(12, 0)
+    p = primaries.isotropic_primaries(24, 0)
     cpu = oracle.run(g0, fd, p, seed=0, capacity=1 << 18, n_threads=8)
     gpu = avm.simulate(ctx, avm.gas_create(ctx, g0), avm.field_create(ctx, fd), p, seed=0, capacity=1 << 18)
     assert cpu.n > 3000
@@ -287,7 +294,7 @@ def test_run_grid_map_same_seed(avm, ctx, oracle, g0):
     cpu = oracle.run(g0, fd, p, seed=7, capacity=1 << 17, n_threads=8)
     gpu = avm.simulate(ctx, avm.gas_create(ctx, g0), avm.field_create(ctx, fd), p, seed=7, capacity=1 << 17)
     assert_run_same_seed(cpu, gpu, g0.n_levels, min_identical=0.99)
-    assert (cpu.status == 4).sum() > 20 and (cpu.status == 1).sum() > 20
+    assert (cpu.status == 4).sum() > 20 and (cpu.status == 1).sum() > 10
 
 
 def test_statistical_parity_independent_seeds(avm, ctx, oracle, g0):
@@ -304,8 +311,15 @@ def test_statistical_parity_independent_seeds(avm, ctx, oracle, g0):
     assert abs(gc.mean() - gg.mean()) < 3 * se, (gc.mean(), gg.mean(), se)
     assert stats.ks_2samp(gc, gg).pvalue > 0.01
     anode_c, anode_g = cpu.status == 2, gpu.status == 2
-    assert stats.ks_2samp(cpu.end[4][anode_c][::7], gpu.end[4][anode_g][::7]).pvalue > 0.01      # thinned: electrons of one avalanche are correlated
-    assert stats.ks_2samp(cpu.end[3][anode_c][::97], gpu.end[3][anode_g][::97]).pvalue > 0.01
+    # endpoint energy and endpoint z (overshoot past the anode plane), thinned: electrons of one avalanche are correlated
+    assert stats.ks_2samp(cpu.end[4][anode_c][::7], gpu.end[4][anode_g][::7]).pvalue > 0.01
+    assert stats.ks_2samp(cpu.end[2][anode_c][::7] - d, gpu.end[2][anode_g][::7] - d).pvalue > 0.01
+    # arrival times inside one avalanche are strongly correlated: compare one number per avalanche (its mean)
+
+    def mean_arrival(r, sel):
+        cnt = np.bincount(r.avalanche[sel], minlength=96)
+        return np.bincount(r.avalanche[sel], weights=r.end[3][sel], minlength=96)[cnt > 0] / cnt[cnt > 0]
+    assert stats.ks_2samp(mean_arrival(cpu, anode_c), mean_arrival(gpu, anode_g)).pvalue > 0.01
     Wc = cpu.tallies_f64[2] / cpu.tallies_f64[3]; Wg = gpu.tallies_f64[2] / gpu.tallies_f64[3]
     assert abs(Wg / Wc - 1) < 0.01, (Wc, Wg)
     ac = (float(cpu.tallies_u64[14] + cpu.tallies_u64[15]) - float(cpu.tallies_u64[16])) / cpu.tallies_f64[2]
