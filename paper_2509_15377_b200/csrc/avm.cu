@@ -49,7 +49,9 @@ struct RunCtl {
   unsigned long long counters;   // (electrons created << 32) | electrons finished
   unsigned int q_head;           // tickets handed out beyond the static ones
   unsigned int dropped;          // children that did not fit in `capacity`
-  unsigned long long n_null, n_real, n_overflow, n_steps;
+  unsigned long long n_real, n_overflow;
+  unsigned long long n_steps;    // sum over electrons of their collision index n (finalize_kernel)
+  unsigned long long n_term;     // electrons whose last step ended before the null/real decision (status 1-4, 6, 7)
   unsigned long long level[AVM_MAX_LEVELS];
   double sum_loss;
   double sum_d[4];               // sum over electrons of (end - birth): dx, dy, dz, dt
@@ -61,63 +63,15 @@ __device__ __forceinline__ unsigned long long ld_volatile_u64(const unsigned lon
   return *(const volatile unsigned long long*)p;
 }
 
-// ---- one step S0-S9 in velocity form -------------------------------------------------------------------
-struct StepOut {
-  int event;        // -1 null, l >= 0 level, -2 terminated before the decision
-  int bin;
-  int status;       // 0 or the finishing status
-  bool spawn, overflow;
-  Child ch;
-  double e;         // energy after the step (e' for null/terminated, e'' after a collision)
-  double s2;        // |v'|^2 after the flight
-  double kx, ky, kz;  // direction after a real, non-attaching collision (else untouched)
-  double loss;
-};
-
-// In: electron (r, t, v, id, n) with the field (Ex,Ey,Ez) at r.  Out: state after the step; (Ex,Ey,Ez) = the
-// field at the new position (valid when status == 0), which is the next step's S0 (same point, R3).
-template <bool UNIFORM1, bool HASB>
-__device__ __forceinline__ void step_core(const DevGas& g, const DevField& f, const uint8_t* lv_type,
-                                          const double* lv_loss, const double* lv_recoil, const double* lv_w,
-                                          uint64_t seed, double t_max, uint64_t id, uint32_t& n, double& x, double& y,
-                                          double& z, double& t, double& vx, double& vy, double& vz, double& Ex,
-                                          double& Ey, double& Ez, StepOut& o) {
-  o.event = -2; o.bin = -1; o.status = 0; o.spawn = false; o.overflow = false; o.loss = 0.0;
-  const uint32_t n_s = n;                                   // S1
-  const U4 r0 = philox(seed, id, n_s, 0u);
-  const double u1 = to_unit(r0.w0, r0.w1), u2 = to_unit(r0.w2, r0.w3);
-  const double dt = -log(u1) * g.inv_nu_hat;                // S2
-  flight<HASB>(f, Ex, Ey, Ez, dt, x, y, z, vx, vy, vz);     // S3
-  const double s2 = vx * vx + vy * vy + vz * vz;            // S4
-  const double e1 = fmax(s2 * kInvC2Sq, kEpsFloor);
-  t = t + dt;
-  n = n_s + 1u;
-  o.s2 = s2; o.e = e1;
-  double mask;                                              // S5
-  const int si = field_at<UNIFORM1>(f, x, y, z, Ex, Ey, Ez, mask);
-  if (si < 0) { o.status = -si; return; }
-  if (mask < 0.5) { o.status = AVM_MATERIAL; return; }
-  if (t > t_max) { o.status = AVM_TIME_LIMIT; return; }
-  if (n >= kStepLimit) { o.status = AVM_STEP_LIMIT; return; }
-  const double sb = e1 * g.inv_de;                          // S6
-  int b;
-  if (sb >= (double)g.nb) { b = g.nb - 1; o.overflow = true; } else b = (int)sb;
-  o.bin = b;
-  const double xr = u2 * g.nu_hat;                          // S7
-  if (xr >= __ldg(g.nu_tot + b)) { o.event = -1; return; }
-  const int l = select_level(g, b, xr);                     // S8
-  o.event = l;
-  const int type = lv_type[l];
-  if (type == AVM_ATTACHMENT) { o.status = AVM_ATTACHED; return; }   // S9a
-  double kx = 0.0, ky = 0.0, kz = 1.0;
-  if (s2 > 0.0) { const double inv = 1.0 / sqrt(s2); kx = vx * inv; ky = vy * inv; kz = vz * inv; }
-  const double e2 = collide(seed, id, n_s, type, lv_loss[l], lv_recoil[l], lv_w[l], e1, kx, ky, kz, o.spawn, o.ch, o.loss);
-  o.e = e2; o.kx = kx; o.ky = ky; o.kz = kz;
-  const double sp = kC2 * sqrt(e2);
-  vx = sp * kx; vy = sp * ky; vz = sp * kz;
-}
-
 // ---- persistent transport kernel -------------------------------------------------------------------------
+// Loop body of one warp ("iteration"): up to kFlights free flights per lane — a lane stops flying as soon as it
+// draws a real collision or finishes — then ONE collision phase for the lanes with a pending real collision, then the
+// rare warp-uniform branches: append secondaries, retire finished electrons, refill idle lanes.  65 % of the steps
+// of gas G0 are null collisions; with two flights per collision phase 58 % of the lanes enter the collision phase
+// instead of 35 %.
+constexpr int kFlights = 2;
+constexpr uint32_t kRefillEvery = 8;      // idle lanes look for work every 8th iteration (and whenever the warp is empty)
+
 template <bool UNIFORM1, bool HASB, bool TALLY>
 __global__ void __launch_bounds__(kThreads, kMinCtasPerSm)
 transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevField f, const RunArrays a,
@@ -139,81 +93,109 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
   // static tickets, warp-major across the grid: the first electrons fill whole warps, one warp per CTA first
   uint32_t ticket = (warp * gridDim.x + blockIdx.x) * 32u + lane;
   bool have = false;
-  double x = 0, y = 0, z = 0, t = 0, vx = 0, vy = 0, vz = 0, Ex = 0, Ey = 0, Ez = 0;
+  double x = 0, y = 0, z = 0, t = 0, vx = 0, vy = 0, vz = 0, Ex = 0, Ey = 0, Ez = 0, dt = 0, u2 = 0;
   uint64_t id = 0;
-  uint32_t n = 0, slot = 0, aval = 0;
-  uint32_t c_null = 0, c_real = 0, c_steps = 0, c_over = 0;
+  uint32_t n = 0, slot = 0;
+  uint32_t c_real = 0, c_l0 = 0, c_over = 0;      // tallies kept per thread; null counts are derived (finalize_kernel)
   double c_loss = 0.0;
+  uint32_t backoff = 100u;
 
   for (uint32_t it = 0; it < max_iters; ++it) {
-    if (!have) {
+    unsigned act = __ballot_sync(0xFFFFFFFFu, have);
+    // ---- refill idle lanes through their tickets (a-10): rare, warp-uniform branch ----
+    if (act != 0xFFFFFFFFu && (act == 0u || (it % kRefillEvery) == 0u)) {
+      if (!have) {
 #pragma unroll 1
-      for (int tries = 0; tries < 4 && ticket < cap; ++tries) {
-        const int st = ld_volatile_s32(a.status + ticket);
-        if (st == 0) {                              // published and unfinished: this lane runs it
-          __threadfence();
-          slot = ticket;
-          x = __ldcg(a.end + slot); y = __ldcg(a.end + ld + slot); z = __ldcg(a.end + 2 * ld + slot);
-          t = __ldcg(a.end + 3 * ld + slot);
-          const double e = __ldcg(a.end + 4 * ld + slot);
-          const double sp = kC2 * sqrt(e);
-          vx = sp * __ldcg(a.end + 5 * ld + slot); vy = sp * __ldcg(a.end + 6 * ld + slot);
-          vz = sp * __ldcg(a.end + 7 * ld + slot);
-          id = __ldcg(a.id + slot);
-          n = __ldcg(a.nsteps + slot);
-          aval = __ldcg(a.aval + slot);
-          double m;
-          field_at<UNIFORM1>(f, x, y, z, Ex, Ey, Ez, m);     // S0 of its first step here (in-domain by construction)
-          have = true;
-          break;
+        for (int tries = 0; tries < 2 && ticket < cap; ++tries) {
+          const int st = ld_volatile_s32(a.status + ticket);
+          if (st == 0) {                              // published and unfinished: this lane runs it
+            __threadfence();
+            slot = ticket;
+            x = __ldcg(a.end + slot); y = __ldcg(a.end + ld + slot); z = __ldcg(a.end + 2 * ld + slot);
+            t = __ldcg(a.end + 3 * ld + slot);
+            const double e = __ldcg(a.end + 4 * ld + slot);
+            const double sp = kC2 * sqrt(e);
+            vx = sp * __ldcg(a.end + 5 * ld + slot); vy = sp * __ldcg(a.end + 6 * ld + slot);
+            vz = sp * __ldcg(a.end + 7 * ld + slot);
+            id = __ldcg(a.id + slot);
+            n = __ldcg(a.nsteps + slot);
+            double m;
+            field_at<UNIFORM1>(f, x, y, z, Ex, Ey, Ez, m);     // S0 of its first step (in-domain by construction)
+            draw_flight(g, seed, id, n, dt, u2);
+            have = true;
+            break;
+          }
+          if (st < 0) break;                          // not created yet: keep the ticket
+          ticket = n_static_tickets + atomicAdd(&ctl->q_head, 1u);   // finished in an earlier launch: next ticket
         }
-        if (st < 0) break;                          // not created yet: keep the ticket
-        ticket = n_static_tickets + atomicAdd(&ctl->q_head, 1u);   // finished in an earlier launch: next ticket
+      }
+      act = __ballot_sync(0xFFFFFFFFu, have);
+      if (act == 0u) {                                // whole warp idle: poll for termination, back off
+        unsigned long long c = 0ull;
+        if (lane == 0u) c = ld_volatile_u64(&ctl->counters);
+        c = __shfl_sync(0xFFFFFFFFu, c, 0);
+        if ((uint32_t)(c >> 32) == (uint32_t)c) break;
+        __nanosleep(backoff);
+        backoff = min(backoff * 2u, 3200u);
+        continue;
+      }
+      backoff = 100u;
+    }
+
+    // ---- flights ----
+    int fin = 0;                 // finishing status of this lane's electron (0 = still running)
+    bool pend = false;
+    Pending pc;
+    pc.lsel = 0; pc.bin = 0; pc.xr = 0.0;
+#pragma unroll
+    for (int fl = 0; fl < kFlights; ++fl) {
+      if (have && !pend && fin == 0) {
+        bool over = false;
+        const int r = flight_step<UNIFORM1, HASB>(g, f, seed, t_max, id, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt, u2,
+                                                  pc, over);
+        if (r < 0) fin = -r;
+        else if (r > 0) pend = true;
+        if (TALLY && over) ++c_over;
       }
     }
-    const unsigned act = __ballot_sync(0xFFFFFFFFu, have);
-    if (act == 0u) {                                // whole warp idle: poll for termination
-      unsigned long long c = 0ull;
-      if (lane == 0u) c = ld_volatile_u64(&ctl->counters);
-      c = __shfl_sync(0xFFFFFFFFu, c, 0);
-      if ((uint32_t)(c >> 32) == (uint32_t)c) break;
-      __nanosleep(200);
-      continue;
-    }
-    StepOut o;
-    o.status = 0; o.spawn = false;
-    if (have) {
-      step_core<UNIFORM1, HASB>(g, f, s_type, s_loss, s_recoil, s_w, seed, t_max, id, n, x, y, z, t, vx, vy, vz, Ex,
-                                Ey, Ez, o);
+    // ---- collision phase ----
+    bool spawn = false;
+    Child ch;
+    ch.e = 0.0; ch.u6 = 0.5; ch.u7 = 0.0;
+    if (pend) {
+      double loss;
+      int st;
+      const int l = collision_step(g, s_type, s_loss, s_recoil, s_w, seed, id, n, pc, vx, vy, vz, st, spawn, ch, loss);
+      if (st) fin = st;
       if (TALLY) {
-        ++c_steps;
-        if (o.overflow) ++c_over;
-        if (o.event == -1) ++c_null;
-        else if (o.event >= 0) { ++c_real; atomicAdd(&s_hist[o.event], 1u); c_loss += o.loss; }
+        ++c_real;
+        if (l == 0) ++c_l0;
+        else if (l > 1) atomicAdd(&s_hist[l], 1u);
+        c_loss += loss;
       }
     }
     // ---- append secondaries: one atomic per warp (a-9) ----
-    const unsigned sm = __ballot_sync(0xFFFFFFFFu, o.spawn);
+    const unsigned sm = __ballot_sync(0xFFFFFFFFu, spawn);
     if (sm) {
       const int leader = __ffs(sm) - 1;
       unsigned long long old = 0ull;
       if ((int)lane == leader) old = atomicAdd(&ctl->counters, (unsigned long long)__popc(sm) << 32);
       old = __shfl_sync(0xFFFFFFFFu, old, leader);
-      if (o.spawn) {
+      if (spawn) {
         const uint64_t cs = (old >> 32) + (uint64_t)__popc(sm & ((1u << lane) - 1u));
         if (cs < (uint64_t)cap) {
           const uint32_t c = (uint32_t)cs;
           double ckx, cky, ckz;
-          child_direction(o.ch.u6, o.ch.u7, ckx, cky, ckz);
+          child_direction(ch.u6, ch.u7, ckx, cky, ckz);
           __stcg(a.end + c, x); __stcg(a.end + ld + c, y); __stcg(a.end + 2 * ld + c, z); __stcg(a.end + 3 * ld + c, t);
-          __stcg(a.end + 4 * ld + c, o.ch.e);
+          __stcg(a.end + 4 * ld + c, ch.e);
           __stcg(a.end + 5 * ld + c, ckx); __stcg(a.end + 6 * ld + c, cky); __stcg(a.end + 7 * ld + c, ckz);
           __stcg(a.id + c, child_id_of(seed, id, n - 1u));
-          __stcg(a.aval + c, aval);
+          __stcg(a.aval + c, __ldcg(a.aval + slot));
           __stcg(a.nsteps + c, 0u);
           if (a.birth) {
             __stcg(a.birth + c, x); __stcg(a.birth + ld + c, y); __stcg(a.birth + 2 * ld + c, z);
-            __stcg(a.birth + 3 * ld + c, t); __stcg(a.birth + 4 * ld + c, o.ch.e);
+            __stcg(a.birth + 3 * ld + c, t); __stcg(a.birth + 4 * ld + c, ch.e);
           }
           __threadfence();
           *(volatile int*)(a.status + c) = 0;       // publish
@@ -224,27 +206,25 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
       }
     }
     // ---- retire finished electrons: endpoint write, one atomic per warp for `done`, one for new tickets ----
-    const bool fin = have && o.status != 0;
-    const unsigned fm = __ballot_sync(0xFFFFFFFFu, fin);
+    const unsigned fm = __ballot_sync(0xFFFFFFFFu, fin != 0);
     if (fm) {
       const int leader = __ffs(fm) - 1;
       unsigned int base = 0u;
-      if ((int)lane == leader) {
-        base = atomicAdd(&ctl->q_head, (unsigned int)__popc(fm));
-      }
+      if ((int)lane == leader) base = atomicAdd(&ctl->q_head, (unsigned int)__popc(fm));
       base = __shfl_sync(0xFFFFFFFFu, base, leader);
-      if (fin) {
+      if (fin != 0) {
+        const double s2 = vx * vx + vy * vy + vz * vz;
         double kx = 0.0, ky = 0.0, kz = 1.0;
-        if (o.s2 > 0.0) { const double inv = 1.0 / sqrt(o.s2); kx = vx * inv; ky = vy * inv; kz = vz * inv; }
+        if (s2 > 0.0) { const double inv = rsqrt(s2); kx = vx * inv; ky = vy * inv; kz = vz * inv; }
         a.end[slot] = x; a.end[ld + slot] = y; a.end[2 * ld + slot] = z; a.end[3 * ld + slot] = t;
-        a.end[4 * ld + slot] = o.e; a.end[5 * ld + slot] = kx; a.end[6 * ld + slot] = ky; a.end[7 * ld + slot] = kz;
+        a.end[4 * ld + slot] = fmax(s2 * kInvC2Sq, kEpsFloor);
+        a.end[5 * ld + slot] = kx; a.end[6 * ld + slot] = ky; a.end[7 * ld + slot] = kz;
         a.nsteps[slot] = n;
-        a.status[slot] = o.status;
+        a.status[slot] = fin;
         have = false;
         ticket = n_static_tickets + base + (uint32_t)__popc(fm & ((1u << lane) - 1u));
       }
-      __syncwarp();
-      if ((int)lane == leader) { __threadfence(); atomicAdd(&ctl->counters, (unsigned long long)__popc(fm)); }
+      if ((int)lane == leader) atomicAdd(&ctl->counters, (unsigned long long)__popc(fm));
     }
   }
 
@@ -253,31 +233,29 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
   if (have) {
     const double s2 = vx * vx + vy * vy + vz * vz;
     double kx = 0.0, ky = 0.0, kz = 1.0;
-    if (s2 > 0.0) { const double inv = 1.0 / sqrt(s2); kx = vx * inv; ky = vy * inv; kz = vz * inv; }
+    if (s2 > 0.0) { const double inv = rsqrt(s2); kx = vx * inv; ky = vy * inv; kz = vz * inv; }
     a.end[slot] = x; a.end[ld + slot] = y; a.end[2 * ld + slot] = z; a.end[3 * ld + slot] = t;
     a.end[4 * ld + slot] = fmax(s2 * kInvC2Sq, kEpsFloor);
     a.end[5 * ld + slot] = kx; a.end[6 * ld + slot] = ky; a.end[7 * ld + slot] = kz;
     a.nsteps[slot] = n;
   }
   if (TALLY) {
-    // warp reduce the per-thread counters, one atomic per warp; level histogram per CTA
-    unsigned long long v0 = c_null, v1 = c_real, v2 = c_steps, v3 = c_over;
+    // warp reduce the per-thread counters, one atomic per warp; rare-level histogram per CTA
+    unsigned long long v0 = c_real, v1 = c_l0, v3 = c_over;
     double v4 = c_loss;
 #pragma unroll
     for (int o2 = 16; o2 > 0; o2 >>= 1) {
       v0 += __shfl_down_sync(0xFFFFFFFFu, v0, o2); v1 += __shfl_down_sync(0xFFFFFFFFu, v1, o2);
-      v2 += __shfl_down_sync(0xFFFFFFFFu, v2, o2); v3 += __shfl_down_sync(0xFFFFFFFFu, v3, o2);
-      v4 += __shfl_down_sync(0xFFFFFFFFu, v4, o2);
+      v3 += __shfl_down_sync(0xFFFFFFFFu, v3, o2); v4 += __shfl_down_sync(0xFFFFFFFFu, v4, o2);
     }
     if (lane == 0u) {
-      if (v0) atomicAdd(&ctl->n_null, v0);
-      if (v1) atomicAdd(&ctl->n_real, v1);
-      if (v2) atomicAdd(&ctl->n_steps, v2);
+      if (v0) atomicAdd(&ctl->n_real, v0);
+      if (v1) atomicAdd(&ctl->level[0], v1);
       if (v3) atomicAdd(&ctl->n_overflow, v3);
       if (v4 != 0.0) atomicAdd(&ctl->sum_loss, v4);
     }
     __syncthreads();
-    for (int l = threadIdx.x; l < g.L; l += blockDim.x)
+    for (int l = 2 + threadIdx.x; l < g.L; l += blockDim.x)
       if (s_hist[l]) atomicAdd(&ctl->level[l], (unsigned long long)s_hist[l]);
   }
 }
@@ -321,22 +299,39 @@ __global__ void inject_kernel(const __grid_constant__ DevField f, const RunArray
 }
 
 // ---- tallies derived from the endpoints (a-12) -----------------------------------------------------------
+// Per-avalanche counts, flight sums (sum over electrons of end - birth) and the step bookkeeping the hot loop does
+// not count: steps = sum of n; every step is null, real or the electron's last one (ended before the decision), so
+// null = steps - real - #{electrons finished by status 1-4, 6, 7 after at least one step}.
 __global__ void finalize_kernel(const RunArrays a, RunCtl* ctl, const uint32_t n, unsigned long long* per_aval,
                                 const uint32_t n_prim, const bool want_sums) {
   double d[4] = {0.0, 0.0, 0.0, 0.0};
+  unsigned long long steps = 0ull, term = 0ull;
   const size_t ld = a.cap;
   for (uint32_t s = blockIdx.x * blockDim.x + threadIdx.x; s < n; s += gridDim.x * blockDim.x) {
+    const int st = a.status[s];
+    const uint32_t ns = a.nsteps[s];
+    steps += ns;
+    if (ns > 0u && st != AVM_ATTACHED && st != AVM_ACTIVE) ++term;
     if (per_aval) {
       const uint32_t av = a.aval[s];
       if (av < n_prim) {
         atomicAdd(per_aval + 3 * (size_t)av, 1ull);
-        if (a.status[s] == AVM_ATTACHED) atomicAdd(per_aval + 3 * (size_t)av + 2, 1ull);
+        if (st == AVM_ATTACHED) atomicAdd(per_aval + 3 * (size_t)av + 2, 1ull);
       }
     }
     if (want_sums) {
 #pragma unroll
       for (int c = 0; c < 4; ++c) d[c] += a.end[c * ld + s] - a.birth[c * ld + s];
     }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    steps += __shfl_down_sync(0xFFFFFFFFu, steps, o);
+    term += __shfl_down_sync(0xFFFFFFFFu, term, o);
+  }
+  if ((threadIdx.x & 31u) == 0u) {
+    if (steps) atomicAdd(&ctl->n_steps, steps);
+    if (term) atomicAdd(&ctl->n_term, term);
   }
   if (want_sums) {
 #pragma unroll
@@ -358,8 +353,12 @@ __global__ void publish_kernel(const RunCtl* ctl, const int L, unsigned long lon
   }
   if (i == 0u) {
     if (tallies_u64) {
+      unsigned long long others = ctl->level[0];
+      for (int l = 2; l < L; ++l) others += ctl->level[l];
       for (int l = 0; l < L; ++l) tallies_u64[l] = ctl->level[l];
-      tallies_u64[L] = ctl->n_null; tallies_u64[L + 1] = ctl->n_real;
+      if (L > 1) tallies_u64[1] = ctl->n_real - others;           // level 1 is the complement (not counted in the loop)
+      tallies_u64[L] = ctl->n_steps - ctl->n_real - ctl->n_term;  // null collisions
+      tallies_u64[L + 1] = ctl->n_real;
       tallies_u64[L + 2] = ctl->n_overflow; tallies_u64[L + 3] = ctl->n_steps;
     }
     if (tallies_f64) {
@@ -394,20 +393,32 @@ __global__ void step_batch_kernel(const __grid_constant__ DevGas g, const __grid
     return;
   }
   const double sp = kC2 * sqrt(e);
-  double vx = sp * kx, vy = sp * ky, vz = sp * kz;
-  StepOut o;
-  step_core<UNIFORM1, HASB>(g, f, g.type, g.loss, g.recoil, g.w, seed, t_max, id, nn, x, y, z, t, vx, vy, vz, Ex, Ey,
-                            Ez, o);
-  const bool collided = o.event >= 0 && o.status == 0;
-  if (collided) { kx = o.kx; ky = o.ky; kz = o.kz; }
-  else if (o.s2 > 0.0) { const double inv = 1.0 / sqrt(o.s2); kx = vx * inv; ky = vy * inv; kz = vz * inv; }
-  out[i] = x; out[n + i] = y; out[2 * n + i] = z; out[3 * n + i] = t; out[4 * n + i] = o.e;
+  double vx = sp * kx, vy = sp * ky, vz = sp * kz, dt, u2;
+  draw_flight(g, seed, id, nn, dt, u2);
+  Pending pc;
+  pc.lsel = 0; pc.bin = -1; pc.xr = 0.0;
+  bool over = false, spawn = false;
+  Child ch;
+  ch.e = 0.0; ch.u6 = 0.5; ch.u7 = 0.0;
+  int ev = -2, st = 0;
+  const int r = flight_step<UNIFORM1, HASB>(g, f, seed, t_max, id, nn, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt, u2, pc, over);
+  if (r < 0) st = -r;
+  else if (r == 0) ev = -1;
+  else {
+    double loss;
+    ev = collision_step(g, g.type, g.loss, g.recoil, g.w, seed, id, nn, pc, vx, vy, vz, st, spawn, ch, loss);
+  }
+  // state after the step in (energy, direction) form
+  const double s2 = vx * vx + vy * vy + vz * vz;
+  if (s2 > 0.0) { const double inv = rsqrt(s2); kx = vx * inv; ky = vy * inv; kz = vz * inv; }
+  out[i] = x; out[n + i] = y; out[2 * n + i] = z; out[3 * n + i] = t; out[4 * n + i] = fmax(s2 * kInvC2Sq, kEpsFloor);
   out[5 * n + i] = kx; out[6 * n + i] = ky; out[7 * n + i] = kz;
-  event[i] = o.event; status[i] = o.status; bin[i] = o.bin;
-  if (o.spawn) {
+  event[i] = ev; status[i] = st;
+  bin[i] = r < 0 ? -1 : pc.bin;
+  if (spawn) {
     double ckx, cky, ckz;
-    child_direction(o.ch.u6, o.ch.u7, ckx, cky, ckz);
-    child[i] = x; child[n + i] = y; child[2 * n + i] = z; child[3 * n + i] = t; child[4 * n + i] = o.ch.e;
+    child_direction(ch.u6, ch.u7, ckx, cky, ckz);
+    child[i] = x; child[n + i] = y; child[2 * n + i] = z; child[3 * n + i] = t; child[4 * n + i] = ch.e;
     child[5 * n + i] = ckx; child[6 * n + i] = cky; child[7 * n + i] = ckz;
     child_id[i] = child_id_of(seed, id, nn - 1u);
   }
@@ -498,11 +509,12 @@ bool valid_gas(const avm_gas_desc* d, double* max_rate) {
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
-struct GasLayout { size_t nu_tot, cum, loss, recoil, w, type, total; };
+struct GasLayout { size_t nu_tot, head, cum, loss, recoil, w, type, total; };
 GasLayout gas_layout(int nb, int L) {
   GasLayout g;
   size_t off = 0;
   g.nu_tot = off; off = align_up(off + sizeof(double) * nb, 256);
+  g.head = off;   off = align_up(off + 4 * sizeof(double) * (size_t)nb, 256);
   g.cum = off;    off = align_up(off + sizeof(double) * (size_t)nb * L, 256);
   g.loss = off;   off += sizeof(double) * AVM_MAX_LEVELS;
   g.recoil = off; off += sizeof(double) * AVM_MAX_LEVELS;
@@ -575,7 +587,15 @@ int32_t avm_gas_create(avm_ctx* ctx, const avm_gas_desc* d, void* dev_buf, size_
   if (!dev_buf || dev_bytes < lay.total || ((uintptr_t)dev_buf & 255u)) return fail(AVM_ERR_INVALID_ARG, "gas_create: device buffer null, too small or not 256-byte aligned");
   std::vector<unsigned char> h(lay.total, 0);
   double* nu_tot = (double*)(h.data() + lay.nu_tot);
-  for (int b = 0; b < nb; ++b) nu_tot[b] = d->cum_rate[(size_t)b * L + L - 1];
+  double* head = (double*)(h.data() + lay.head);
+  for (int b = 0; b < nb; ++b) {
+    const double* row = d->cum_rate + (size_t)b * L;
+    nu_tot[b] = row[L - 1];
+    head[4 * (size_t)b + 0] = row[L - 1];               // decision record: one 32-byte sector per step
+    head[4 * (size_t)b + 1] = row[0];
+    head[4 * (size_t)b + 2] = row[L > 1 ? 1 : 0];
+    head[4 * (size_t)b + 3] = 0.0;
+  }
   std::memcpy(h.data() + lay.cum, d->cum_rate, sizeof(double) * (size_t)nb * L);
   std::memcpy(h.data() + lay.loss, d->level_loss_eV, sizeof(double) * L);
   std::memcpy(h.data() + lay.recoil, d->level_recoil, sizeof(double) * L);
@@ -593,6 +613,7 @@ int32_t avm_gas_create(avm_ctx* ctx, const avm_gas_desc* d, void* dev_buf, size_
   g->d.nu_hat = g->nu_hat;
   g->d.inv_nu_hat = 1.0 / g->nu_hat;
   g->d.nu_tot = (const double*)(base + lay.nu_tot);
+  g->d.head = (const double2*)(base + lay.head);
   g->d.cum = (const double*)(base + lay.cum);
   g->d.loss = (const double*)(base + lay.loss);
   g->d.recoil = (const double*)(base + lay.recoil);
@@ -785,7 +806,7 @@ int32_t avm_run(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, const 
   const uint32_t n_end = (uint32_t)(total < (uint64_t)a.cap ? total : (uint64_t)a.cap);
   // a-12: tallies from the endpoints
   const bool want_sums = o->tallies_f64 != nullptr;
-  if ((o->per_avalanche || want_sums) && n_end > 0) {
+  if ((o->per_avalanche || want_sums || o->tallies_u64) && n_end > 0) {
     unsigned blocks = (n_end + 255u) / 256u;
     const unsigned maxb = (unsigned)ctx->sm_count * 8u;
     if (blocks > maxb) blocks = maxb;

@@ -24,6 +24,7 @@ struct DevGas {
   int nb, L;
   double inv_de, nu_hat, inv_nu_hat;
   const double* nu_tot;   // [nb]      total real-collision rate per bin (= cum[b][L-1])
+  const double2* head;    // [nb][2]   decision record, 32 B: (nu_tot, cum[b][0]), (cum[b][min(1,L-1)], 0)
   const double* cum;      // [nb][L]   cumulative rates, row-major by bin
   const double* loss;     // [L]
   const double* recoil;   // [L]
@@ -205,7 +206,8 @@ __device__ __forceinline__ void deflect(double& kx, double& ky, double& kz, doub
   const double nx = ct * kx + st * (cphi * b1x + sphi * b2x);
   const double ny = ct * ky + st * (cphi * b1y + sphi * b2y);
   const double nz = ct * kz + st * (cphi * b1z + sphi * b2z);
-  const double inv = 1.0 / sqrt(nx * nx + ny * ny + nz * nz);
+  // |k''|^2 = 1 + d with |d| ~ 1e-15 (unit k, orthonormal basis, ct^2 + st^2 = 1): 1/sqrt(1+d) = 1 - d/2 + O(d^2)
+  const double inv = fma(-0.5, fma(nx, nx, fma(ny, ny, nz * nz)), 1.5);
   kx = nx * inv; ky = ny * inv; kz = nz * inv;
 }
 
@@ -258,11 +260,77 @@ __device__ __forceinline__ double collide(uint64_t seed, uint64_t id, uint32_t n
   return e2;
 }
 
-// S8: smallest l with cum[b][l] > x (x < cum[b][L-1] is known).
-__device__ __forceinline__ int select_level(const DevGas& g, int b, double xr) {
+// S8 for the rare levels: smallest l >= 2 with cum[b][l] > x (x < cum[b][L-1] is known; levels 0 and 1 are
+// decided from the head record).
+__device__ __forceinline__ int select_level_from2(const DevGas& g, int b, double xr) {
   const double* row = g.cum + (size_t)b * g.L;
-  int l = 0;
+  int l = 2;
   while (l < g.L - 1 && __ldg(row + l) <= xr) ++l;
+  return l;
+}
+
+// ---- one step, split at the null/real decision ----------------------------------------------------------------
+// Electron state is kept in velocity form (r, t, v, id, n) plus the draws of its NEXT flight (dt, u2), which are
+// computed one step ahead: the Philox block and the logarithm of step n+1 depend only on (id, n+1) and fill the
+// latency of the decision-record load of step n.
+struct Pending { int lsel, bin; double xr; };   // lsel: 0 / 1 = level decided from the head record, 2 = scan the row
+
+__device__ __forceinline__ void draw_flight(const DevGas& g, uint64_t seed, uint64_t id, uint32_t n, double& dt,
+                                            double& u2) {
+  const U4 r0 = philox(seed, id, n, 0u);                                        // S1
+  dt = -log(to_unit(r0.w0, r0.w1)) * g.inv_nu_hat;                              // S2
+  u2 = to_unit(r0.w2, r0.w3);
+}
+
+// S2-S7 for one electron.  Returns 0 = null collision (continue), 1 = real collision pending (p filled),
+// < 0 = -(finishing status).  (dt, u2) in: this flight's draws; out: the next flight's.  overflow: energy clamped.
+template <bool UNIFORM1, bool HASB>
+__device__ __forceinline__ int flight_step(const DevGas& g, const DevField& f, uint64_t seed, double t_max,
+                                           uint64_t id, uint32_t& n, double& x, double& y, double& z, double& t,
+                                           double& vx, double& vy, double& vz, double& Ex, double& Ey, double& Ez,
+                                           double& dt, double& u2, Pending& p, bool& overflow) {
+  flight<HASB>(f, Ex, Ey, Ez, dt, x, y, z, vx, vy, vz);     // S3
+  const double s2 = vx * vx + vy * vy + vz * vz;            // S4
+  const double e1 = fmax(s2 * kInvC2Sq, kEpsFloor);
+  t = t + dt;
+  n = n + 1u;
+  double mask;                                              // S5
+  const int si = field_at<UNIFORM1>(f, x, y, z, Ex, Ey, Ez, mask);
+  if (si < 0) return si;
+  if (mask < 0.5) return -AVM_MATERIAL;
+  if (t > t_max) return -AVM_TIME_LIMIT;
+  if (n >= kStepLimit) return -AVM_STEP_LIMIT;
+  const double sb = e1 * g.inv_de;                          // S6
+  int b;
+  overflow = sb >= (double)g.nb;
+  b = overflow ? g.nb - 1 : (int)sb;
+  const double2 h0 = __ldg(g.head + 2 * (size_t)b), h1 = __ldg(g.head + 2 * (size_t)b + 1);
+  const double xr = u2 * g.nu_hat;                          // S7 (this flight's u2)
+  draw_flight(g, seed, id, n, dt, u2);                      // next flight's draws: independent of the load above
+  p.bin = b;
+  if (xr >= h0.x) return 0;
+  p.lsel = xr < h0.y ? 0 : (xr < h1.x ? 1 : 2);
+  p.xr = xr;
+  return 1;
+}
+
+// S8-S9 for an electron with a pending real collision (n already incremented by the flight).  Returns the level;
+// status = AVM_ATTACHED for an attachment, else 0 and v is the velocity after the collision.
+__device__ __forceinline__ int collision_step(const DevGas& g, const uint8_t* lv_type, const double* lv_loss,
+                                              const double* lv_recoil, const double* lv_w, uint64_t seed, uint64_t id,
+                                              uint32_t n, const Pending& p, double& vx, double& vy, double& vz,
+                                              int& status, bool& spawn, Child& ch, double& loss) {
+  const int l = p.lsel < 2 ? p.lsel : select_level_from2(g, p.bin, p.xr);     // S8
+  const int type = lv_type[l];
+  status = 0; spawn = false; loss = 0.0;
+  if (type == AVM_ATTACHMENT) { status = AVM_ATTACHED; return l; }             // S9a
+  const double s2 = vx * vx + vy * vy + vz * vz;
+  const double e1 = fmax(s2 * kInvC2Sq, kEpsFloor);
+  double kx = 0.0, ky = 0.0, kz = 1.0;
+  if (s2 > 0.0) { const double inv = rsqrt(s2); kx = vx * inv; ky = vy * inv; kz = vz * inv; }
+  const double e2 = collide(seed, id, n - 1u, type, lv_loss[l], lv_recoil[l], lv_w[l], e1, kx, ky, kz, spawn, ch, loss);
+  const double sp = kC2 * sqrt(e2);
+  vx = sp * kx; vy = sp * ky; vz = sp * kz;
   return l;
 }
 
