@@ -75,6 +75,67 @@ __device__ __forceinline__ double to_unit(uint32_t hi, uint32_t lo) {
   return (one_m - 1.0) + 1.1102230246251565e-16;                            // both steps exact
 }
 
+// ---- elementary functions specialised to this path's argument ranges ------------------------------------------
+// Coefficients live in constant memory so that they enter DFMA as constant-bank operands (an fp64 immediate costs
+// two UMOVs).  Accuracy: a few ulp, far inside the 1e-12 parity tolerance.
+__constant__ double kAtanhC[10] = {1.0 / 3.0, 1.0 / 5.0, 1.0 / 7.0, 1.0 / 9.0, 1.0 / 11.0, 1.0 / 13.0, 1.0 / 15.0,
+                                   1.0 / 17.0, 1.0 / 19.0, 1.0 / 21.0};
+// sin(r pi/2) = r sum_k kSinC[k] r^2k, cos(r pi/2) = sum_k kCosC[k] r^2k (Taylor; |r| <= 1/2: truncation < 5e-17)
+__constant__ double kSinC[8] = {1.5707963267948966, -0.6459640975062463, 0.07969262624616705, -0.004681754135318688,
+                                0.00016044118478735983, -3.598843235212085e-06, 5.692172921967927e-08,
+                                -6.688035109811468e-10};
+__constant__ double kCosC[9] = {1.0, -1.2337005501361697, 0.25366950790104803, -0.02086348076335296,
+                                0.0009192602748394266, -2.5202042373060607e-05, 4.710874778818172e-07,
+                                -6.386603083791852e-09, 6.565963114979473e-11};
+
+// 1/d for normal d well inside the exponent range (MUFU.RCP64H seed, cubic Newton step): ~1 ulp.
+__device__ __forceinline__ double rcp_fast(double d) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(d));
+  double e = fma(-d, r, 1.0);
+  e = fma(e, e, e);
+  return fma(r, e, r);
+}
+
+// log(u) for u strictly inside (0, 1) and normal (the uniforms of to_unit are >= 2^-53): no special cases.
+// u = m 2^e, m in [sqrt(1/2), sqrt(2)); log m = 2 atanh(q), q = (m - 1)/(m + 1), |q| <= 0.1716.
+__device__ __forceinline__ double log_unit(double u) {
+  int hi = __double2hiint(u);
+  const int lo = __double2loint(u);
+  int e = (hi >> 20) - 1023;
+  hi = (hi & 0x000FFFFF) | 0x3FF00000;
+  if (hi >= 0x3FF6A09F) { hi -= 0x00100000; ++e; }
+  const double m = __hiloint2double(hi, lo);
+  const double f = m - 1.0, d = m + 1.0;
+  const double r = rcp_fast(d);
+  double q = f * r;
+  q = fma(fma(-d, q, f), r, q);
+  const double t = q * q;
+  double p = kAtanhC[9];
+#pragma unroll
+  for (int k = 8; k >= 0; --k) p = fma(p, t, kAtanhC[k]);
+  const double lm = 2.0 * fma(q * t, p, q);
+  const double de = (double)e;
+  return fma(de, 0.6931471805599453, fma(de, 2.3190468138462996e-17, lm));
+}
+
+// (sin, cos)(2 pi u) for u in [0, 1]: quadrant q = rint(4u), r = 4u - q in [-1/2, 1/2] (exact).
+__device__ __forceinline__ void sincos_2pi(double u, double& s, double& c) {
+  const double a = 4.0 * u;
+  const int q = __double2int_rn(a);
+  const double r = a - (double)q;
+  const double w = r * r;
+  double ps = kSinC[7], pc = kCosC[8];
+#pragma unroll
+  for (int k = 6; k >= 0; --k) ps = fma(ps, w, kSinC[k]);
+#pragma unroll
+  for (int k = 7; k >= 0; --k) pc = fma(pc, w, kCosC[k]);
+  ps *= r;
+  const double ss = (q & 1) ? pc : ps, cc = (q & 1) ? ps : pc;
+  s = (q & 2) ? -ss : ss;
+  c = ((q + 1) & 2) ? -cc : cc;
+}
+
 // ---- field (S0, R14, R15) -------------------------------------------------------------------------------
 __device__ __forceinline__ double f2d(float v) { return (double)v; }
 
@@ -199,7 +260,7 @@ struct Child { double e, u6, u7; };   // secondary: energy and the two uniforms 
 __device__ __forceinline__ void deflect(double& kx, double& ky, double& kz, double ct, double st, double cphi,
                                         double sphi) {
   const double sg = copysign(1.0, kz);
-  const double A = -1.0 / (sg + kz);
+  const double A = -rcp_fast(sg + kz);
   const double Bq = kx * ky * A;
   const double b1x = 1.0 + sg * kx * kx * A, b1y = sg * Bq, b1z = -sg * kx;
   const double b2x = Bq, b2y = sg + ky * ky * A, b2z = -ky;
@@ -214,7 +275,7 @@ __device__ __forceinline__ void deflect(double& kx, double& ky, double& kz, doub
 __device__ __forceinline__ void child_direction(double u6, double u7, double& kx, double& ky, double& kz) {
   const double sc = 2.0 * sqrt(u6 * (1.0 - u6));
   double s, c;
-  sincospi(2.0 * u7, &s, &c);
+  sincos_2pi(u7, s, c);
   kx = sc * c; ky = sc * s; kz = 1.0 - 2.0 * u6;
 }
 
@@ -234,7 +295,7 @@ __device__ __forceinline__ double collide(uint64_t seed, uint64_t id, uint32_t n
   const double ct = 1.0 - 2.0 * u3;
   const double st = 2.0 * sqrt(u3 * (1.0 - u3));
   double sphi, cphi;
-  sincospi(2.0 * u4, &sphi, &cphi);
+  sincos_2pi(u4, sphi, cphi);
   double e2;
   spawn = false;
   if (type == AVM_ELASTIC) {
@@ -278,7 +339,7 @@ struct Pending { int lsel, bin; double xr; };   // lsel: 0 / 1 = level decided f
 __device__ __forceinline__ void draw_flight(const DevGas& g, uint64_t seed, uint64_t id, uint32_t n, double& dt,
                                             double& u2) {
   const U4 r0 = philox(seed, id, n, 0u);                                        // S1
-  dt = -log(to_unit(r0.w0, r0.w1)) * g.inv_nu_hat;                              // S2
+  dt = -log_unit(to_unit(r0.w0, r0.w1)) * g.inv_nu_hat;                         // S2
   u2 = to_unit(r0.w2, r0.w3);
 }
 
