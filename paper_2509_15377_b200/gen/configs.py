@@ -71,3 +71,47 @@ def replicate(w: Workload, times: int) -> Workload:
         parts.append(q)
     return Workload(f"{w.name}x{times}", w.gas, w.field, np.concatenate(parts, axis=0), w.seed, w.t_max,
                     w.capacity * times, w.note + f"; {times} independent replicas in one batch")
+
+
+# ---- GEM configs (map recipe in gen/gem.py) ------------------------------------
+GEM_Z_HALF_LO, GEM_Z_HALF_HI = -300.0e-4, 299.0e-4        # each map covers -300 ... +299 um about its foil centre
+GEM_STACK_PITCH = 2060.0e-4                               # foil centres 2 mm + 60 um apart (config 5)
+GEM_START_Z = 130.0e-4                                    # 100 um above the top copper surface (z = +30 um)
+
+
+def _gem_slab(e_above: float, e_below: float, z_centre: float, seed: int) -> "fields.Slab":
+    from . import gem
+    nodes = gem.gem_nodes(e_above, e_below, 400.0, seed)
+    return fields.grid_slab(nodes, (0.0, 0.0, z_centre + gem.Z0_UM * gem.UM), (gem.UM, gem.UM, gem.UM),
+                            z_centre + GEM_Z_HALF_LO, z_centre + GEM_Z_HALF_HI,
+                            fields.BC_MIRROR, fields.BC_MIRROR, gem.LX_UM * gem.UM, gem.LY_UM * gem.UM)
+
+
+def _gem_primaries(n: int, seed: int, id_offset: int) -> np.ndarray:
+    from . import gem
+    return primaries.isotropic_primaries(n, seed, pos=(0.0, 0.0, GEM_START_Z), id_offset=id_offset,
+                                         xy_box=((0.0, gem.LX_UM * gem.UM), (0.0, gem.LY_UM * gem.UM)))
+
+
+def config4(n_primaries: int = 1000, seed: int = 0, id_offset: int = 0) -> Workload:
+    """Single GEM: 141 x 245 x 600 fp32 map at 1 um, dV = 400 V, 2 kV/cm drift above, 3 kV/cm induction below,
+    mirror-periodic in x/y; primaries 100 um above the foil, uniform over the cell; electrons move toward -z."""
+    fd = fields.FieldDesc([_gem_slab(2000.0, 3000.0, 0.0, seed)])
+    return Workload("config4", gas.gas_g0(), fd, _gem_primaries(n_primaries, seed, id_offset), seed, INF,
+                    max(256 * n_primaries, 1 << 16),
+                    "single GEM map 141x245x600 (331.6 MB), dV=400 V, 2/3 kV/cm, gas G0, primaries 100 um above the foil")
+
+
+def config5(n_primaries: int = 200, seed: int = 0, id_offset: int = 0) -> Workload:
+    """Triple GEM: three maps (2->3, 3->3, 3->3 kV/cm) whose foil centres are 2.06 mm apart, uniform 3 kV/cm transfer
+    slabs between them; slabs ascend in z, GEM1 (the first the electrons meet) on top at z = 0."""
+    slabs = []
+    for i, (ea, eb) in enumerate(((3000.0, 3000.0), (3000.0, 3000.0), (2000.0, 3000.0))):    # GEM3, GEM2, GEM1
+        zc = -(2 - i) * GEM_STACK_PITCH
+        if slabs:
+            slabs.append(fields.Slab(slabs[-1].z_hi, zc + GEM_Z_HALF_LO, fields.KIND_UNIFORM, (0.0, 0.0, 3000.0)))
+        slabs.append(_gem_slab(ea, eb, zc, seed + (2 - i)))
+    fd = fields.FieldDesc(slabs)
+    return Workload("config5", gas.gas_g0(), fd, _gem_primaries(n_primaries, seed, id_offset), seed, INF,
+                    max(200000 * n_primaries, 1 << 20),
+                    "triple GEM: 3 maps 141x245x600 (995 MB), 3 kV/cm transfer gaps, gas G0, primaries 100 um above GEM1")

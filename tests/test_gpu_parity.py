@@ -385,3 +385,92 @@ def test_edge_cases(avm, ctx, oracle, g0):
     sel = np.isin(whole.avalanche, np.arange(16, 32))
     assert np.array_equal(whole.id[sel], shard.id) and np.array_equal(whole.n_steps[sel], shard.n_steps)
     assert np.array_equal(whole.end[:, sel], shard.end)
+
+
+# ---- BASELINE configs 4 and 5: the full-size GEM maps (331.6 MB each) ------------------------------------------------
+@pytest.fixture(scope="module")
+def cfg4():
+    from paper_2509_15377_b200.gen import configs
+    return configs.config4(n_primaries=24)
+
+
+def _gem_states(n, rng, z_lo, z_hi):
+    st = _states(n, rng, e_lo=0.01, e_hi=39.0)
+    st[0] = rng.uniform(-300e-4, 300e-4, n)            # several mirror periods in x and y
+    st[1] = rng.uniform(-500e-4, 500e-4, n)
+    st[2] = rng.uniform(z_lo, z_hi, n)
+    return st
+
+
+def test_config4_full_map_field_and_step_parity(avm, ctx, oracle, g0, cfg4):
+    """The 141 x 245 x 600 map at full size: field lookups at 2e5 points over several mirror periods, then per-step
+    parity on 2.6e5 states, half of them inside +-45 um of the foil (hole field, material absorption)."""
+    rng = np.random.default_rng(11)
+    fd = cfg4.field
+    fg = avm.field_create(ctx, fd)
+    assert fg.map_bytes == 141 * 245 * 600 * 16
+    n = 200000
+    r = np.vstack([rng.uniform(-700e-4, 700e-4, n), rng.uniform(-900e-4, 900e-4, n), rng.uniform(-305e-4, 304e-4, n)])
+    Ec, mc, sc = oracle.field_eval(fd, r)
+    Eg, mg, sg = avm.field_eval(ctx, fg, r)
+    assert np.array_equal(sc, sg) and (sc == 0).sum() > 0.9 * n
+    ins = sc >= 0
+    assert np.all(np.abs(Eg - Ec)[:, ins] <= 1e-12 * 9e4) and np.all(np.abs(mg - mc)[ins] <= 1e-12)
+    assert ((mc[ins] > 0) & (mc[ins] < 1)).sum() > 100          # points in cells that straddle the material surface
+
+    gg = avm.gas_create(ctx, g0)
+    n = 1 << 17
+    for z_lo, z_hi, what in ((-45e-4, 45e-4, "hole"), (-299e-4, 298e-4, "whole slab")):
+        st = _gem_states(n, rng, z_lo, z_hi)
+        E, m, s = oracle.field_eval(fd, st[0:3])
+        st = st[:, (s == 0) & (m >= 0.5)]                       # a step starts in the gas
+        k = st.shape[1]
+        ids = rng.integers(0, 2 ** 64, k, dtype=np.uint64)
+        nidx = rng.integers(0, 1 << 22, k, dtype=np.uint64).astype(np.uint32)
+        cpu = oracle.step_batch(g0, fd, 21, st, ids, nidx)
+        gpu = avm.step_batch(ctx, gg, fg, 21, st, ids, nidx)
+        assert_step_parity(cpu, gpu, st, f"config4 {what}")
+        assert (cpu.status == 0).sum() > k // 2
+        if what == "hole":
+            assert (cpu.status == 4).sum() > 100 and (cpu.event >= 14).sum() > 10
+
+
+def test_config4_same_seed_run(avm, ctx, oracle, g0, cfg4):
+    """BASELINE config 4 with its first 24 primaries (identical streams to the full run's first 24 avalanches)."""
+    w = cfg4
+    cpu = oracle.run(w.gas, w.field, w.primaries, seed=w.seed, capacity=1 << 15, n_threads=8)
+    gpu = avm.simulate(ctx, avm.gas_create(ctx, g0), avm.field_create(ctx, w.field), w.primaries, seed=w.seed,
+                       capacity=1 << 15)
+    assert cpu.n > 100 and (cpu.status == 4).sum() > 20 and (cpu.status == 1).sum() > 10
+    # ~3e5 steps per electron: a rounding difference can flip one decision in a history; allow a few per cent
+    assert_run_same_seed(cpu, gpu, g0.n_levels, min_identical=0.90)
+    L = g0.n_levels
+    assert abs(int(gpu.tallies_u64[L + 3]) / int(cpu.tallies_u64[L + 3]) - 1) < 0.05
+    t = gpu.tallies_u64
+    assert gpu.n == 24 + int(t[14] + t[15]) and int(gpu.n_steps.sum()) == int(t[L + 3])
+
+
+def test_config5_triple_gem_same_seed_run(avm, ctx, oracle, g0):
+    """BASELINE config 5 layout (three maps, ~1 GB, five slabs) with its first 6 primaries."""
+    from paper_2509_15377_b200.gen import configs
+    w = configs.config5(n_primaries=6)
+    fg = avm.field_create(ctx, w.field)
+    assert fg.map_bytes == 3 * 141 * 245 * 600 * 16
+    rng = np.random.default_rng(12)
+    n = 100000
+    r = np.vstack([rng.uniform(-300e-4, 300e-4, n), rng.uniform(-300e-4, 300e-4, n), rng.uniform(-0.4425, 0.0301, n)])
+    Ec, mc, sc = oracle.field_eval(w.field, r)
+    Eg, mg, sg = avm.field_eval(ctx, fg, r)
+    assert np.array_equal(sc, sg) and all((sc == i).sum() > 1000 for i in range(5))
+    ins = sc >= 0
+    assert np.all(np.abs(Eg - Ec)[:, ins] <= 1e-12 * 9e4) and np.all(np.abs(mg - mc)[ins] <= 1e-12)
+    cpu = oracle.run(w.gas, w.field, w.primaries, seed=w.seed, capacity=1 << 16, n_threads=6)
+    gpu = avm.simulate(ctx, avm.gas_create(ctx, g0), fg, w.primaries, seed=w.seed, capacity=1 << 16)
+    assert cpu.n > 50
+    assert_run_same_seed(cpu, gpu, g0.n_levels, min_identical=0.80)
+    # what is unique regardless of rounding-flipped histories: bookkeeping on the GPU result
+    L = g0.n_levels
+    t = gpu.tallies_u64
+    assert gpu.n == 6 + int(t[14] + t[15]) and int(gpu.n_steps.sum()) == int(t[L + 3])
+    assert np.all(gpu.status != 0) and set(np.unique(gpu.status)) <= {1, 4, 5}
+    assert np.all(gpu.end[2][gpu.status == 1] < w.field.slabs[0].z_lo)
