@@ -30,6 +30,8 @@ UNIT = "collisions/s"
 FP64_PER_NULL = {False: 90.0, True: 170.0}       # free flight + energy + bin + decision; key = B != 0
 FP64_PER_REAL_EXTRA = 110.0                      # deflection angles, basis, rotation, renormalise, speed
 FP64_PER_ION_EXTRA = 80.0                        # Opal-Beaty atan/tan, child direction
+FP64_PER_GRID_EXTRA = 45.0                       # fold + 7 lerps x 4 channels per step in a grid slab
+GATHER_BYTES_PER_GRID_STEP = 128.0               # 8 nodes x 16 B
 FP64_LANES_PER_SM = 64                           # one warp-wide FP64 instruction / 2 clk / scheduler
 
 
@@ -45,15 +47,29 @@ def make_workload(name: str, rank: int = 0):
         w = configs.config3(n_primaries=100000, t_max=20.0, id_offset=rank * 100000)
         w.name = "config3s"
         w.note += "; time cut t_max=20 ns"
+    elif name == "config4":
+        w = configs.config4(id_offset=rank * 1000)
+    elif name.startswith("config4x"):
+        w = configs.replicate(configs.config4(), int(name[len("config4x"):]))
+    elif name == "config5":
+        w = configs.config5(id_offset=rank * 200)
     else:
         raise SystemExit(f"unknown workload {name}")
     return w
 
 
-def alg_fp64(tallies_u64: np.ndarray, L: int, level_type: np.ndarray, has_b: bool) -> float:
+def grid_fraction(field) -> float:
+    """Share of the steps taken inside grid slabs.  Not tallied by the path; estimated as the grid slabs' share of the
+    drift length (exact for one slab: configs 1-4; DESIGN.md §6 for config 5)."""
+    tot = sum(s.z_hi - s.z_lo for s in field.slabs)
+    return sum(s.z_hi - s.z_lo for s in field.slabs if s.kind == 1) / tot
+
+
+def alg_fp64(tallies_u64: np.ndarray, L: int, level_type: np.ndarray, has_b: bool, grid_frac: float = 0.0) -> float:
     n_null, n_real = float(tallies_u64[L]), float(tallies_u64[L + 1])
     n_ion = float(sum(int(tallies_u64[l]) for l in range(L) if level_type[l] == 2))
-    return (n_null + n_real) * FP64_PER_NULL[has_b] + n_real * FP64_PER_REAL_EXTRA + n_ion * FP64_PER_ION_EXTRA
+    return ((n_null + n_real) * (FP64_PER_NULL[has_b] + grid_frac * FP64_PER_GRID_EXTRA) + n_real * FP64_PER_REAL_EXTRA
+            + n_ion * FP64_PER_ION_EXTRA)
 
 
 class ClockSampler:
@@ -239,7 +255,8 @@ def run_ours(args) -> None:
     launches = sum(s["launches"] for s in steps)
     t_launches = sum(s["transport_launches"] for s in steps)
     t_ms = sum(s["transport_ms"] for s in steps)
-    fp64 = sum(alg_fp64(s["tallies"], L, w.gas.level_type, has_b) for s in steps)
+    gfrac = grid_fraction(w.field)
+    fp64 = sum(alg_fp64(s["tallies"], L, w.gas.level_type, has_b, gfrac) for s in steps)
 
     for i in range(min(args.warmup, 2)):
         e2e_step(w.seed + 2000 + i)
@@ -273,6 +290,11 @@ def run_ours(args) -> None:
                 "frac_of_nominal": achieved / peak["nominal"],
                 "alg_fp64_per_collision": fp64 / max(null / world + real / world, 1.0) if world == 1 else None,
                 "launch_ms": t_ms / max(t_launches, 1), "transport_share_of_step": t_ms / max(sum(s["ms"] for s in steps), 1e-9)}
+    if gfrac > 0.0:      # grid maps: the field gather's algorithmic bytes beside the ALU figure
+        gb = gfrac * (null + real) / world * GATHER_BYTES_PER_GRID_STEP
+        roofline["field_gather_GBps"] = gb / (t_ms * 1e-3) / 1e9
+        roofline["field_gather_bytes_per_step"] = GATHER_BYTES_PER_GRID_STEP
+        roofline["grid_step_fraction"] = gfrac
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": tot_ms / max(args.steps, 1), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
