@@ -29,11 +29,27 @@ int32_t fail(int32_t code, const std::string& msg) { g_err = msg; return code; }
     if (e_ != cudaSuccess) return fail(AVM_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); \
   } while (0)
 
-constexpr int kThreads = 256;          // threads per CTA of the transport kernel
-constexpr int kMinCtasPerSm = 2;       // register budget: 65536 / (256 * 2) = 128 registers per thread
+#ifndef AVM_THREADS
+#define AVM_THREADS 512
+#endif
+#ifndef AVM_MIN_CTAS
+#define AVM_MIN_CTAS 1
+#endif
+#ifndef AVM_FLIGHTS
+#define AVM_FLIGHTS 2
+#endif
+#ifndef AVM_COOP_MAX
+#define AVM_COOP_MAX 16
+#endif
+constexpr int kThreads = AVM_THREADS;        // threads per CTA of the transport kernel
+constexpr int kMinCtasPerSm = AVM_MIN_CTAS;  // one 512-thread CTA per SM: 128 registers per thread, <= 227 KB shared
+constexpr int kWarpsPerCta = kThreads / 32;
 constexpr uint32_t kDefaultMaxIters = 1u << 16;
 constexpr int64_t kStageElectrons = 1 << 18;   // primaries staged per H2D chunk (16 MiB)
-constexpr size_t kCtlBytes = 4096;
+constexpr int kMaxGrid = 1024;                 // done flags, one 32-byte sector per CTA
+constexpr size_t kDoneOffset = 4096;
+constexpr size_t kCtlBytes = kDoneOffset + (size_t)kMaxGrid * 32;
+constexpr size_t kMaxDynSmem = 227 * 1024 - 4096;   // static shared memory (level parameters) comes on top
 
 struct RunArrays {
   uint32_t cap;
@@ -46,9 +62,11 @@ struct RunArrays {
 };
 
 struct RunCtl {
-  unsigned long long counters;   // (electrons created << 32) | electrons finished
-  unsigned int q_head;           // tickets handed out beyond the static ones
+  unsigned long long counters;   // (electrons created << 32) | electrons finished; spawn / retire atomics only
+  unsigned char pad0[120];
+  unsigned int q_head;           // tickets handed out beyond the static ones (own 128-byte line)
   unsigned int dropped;          // children that did not fit in `capacity`
+  unsigned char pad1[120];
   unsigned long long n_real, n_overflow;
   unsigned long long n_steps;    // sum over electrons of their collision index n (finalize_kernel)
   unsigned long long n_term;     // electrons whose last step ended before the null/real decision (status 1-4, 6, 7)
@@ -56,27 +74,55 @@ struct RunCtl {
   double sum_loss;
   double sum_d[4];               // sum over electrons of (end - birth): dx, dy, dz, dt
 };
-static_assert(sizeof(RunCtl) <= kCtlBytes, "ctl block");
+static_assert(sizeof(RunCtl) <= kDoneOffset, "ctl block");
 
-__device__ __forceinline__ int ld_volatile_s32(const int* p) { return *(const volatile int*)p; }
-__device__ __forceinline__ unsigned long long ld_volatile_u64(const unsigned long long* p) {
-  return *(const volatile unsigned long long*)p;
+// Per-warp exchange area of the cooperative batches (shared memory): entry j = draws of electron (j mod k') at its
+// step (j div k') of the batch, written by lane j.
+struct WarpBuf {
+  double dt[32], u2[32];
+  double ct[32], st[32], cphi[32], sphi[32];
+  unsigned long long id[32];
+  unsigned int n[32];
+};
+
+__device__ __forceinline__ int ld_relaxed_s32(const int* p) {
+  int v;
+  asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+// Release store: earlier writes of this thread are visible at gpu scope before the flag is.  Unlike __threadfence()
+// this does not invalidate the SM's L1 (no CCTL.IVALL), which the gas-table and field-map loads live in.
+__device__ __forceinline__ void st_release_s32(int* p, int v) {
+  asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ void idle_wait(uint32_t ns) {
+  unsigned long long t0, t1;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+  do {
+    __nanosleep(ns);
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
+  } while (t1 - t0 < (unsigned long long)ns);
 }
 
 // ---- persistent transport kernel -------------------------------------------------------------------------
-// Loop body of one warp ("iteration"): up to kFlights free flights per lane — a lane stops flying as soon as it
-// draws a real collision or finishes — then ONE collision phase for the lanes with a pending real collision, then the
-// rare warp-uniform branches: append secondaries, retire finished electrons, refill idle lanes.  65 % of the steps
-// of gas G0 are null collisions; with two flights per collision phase 58 % of the lanes enter the collision phase
-// instead of 35 %.
-constexpr int kFlights = 2;
-constexpr uint32_t kRefillEvery = 8;      // idle lanes look for work every 8th iteration (and whenever the warp is empty)
+// One warp iteration advances the warp's k electrons (lanes with `have`):
+//  * k <= kCoopMax — cooperative batch: all 32 lanes first prepare the draws (Philox block 0 + logarithm, block 1 +
+//    deflection angles) of the next B = 32 / k' steps of the k electrons (k' = k rounded up to a power of two), lane j
+//    serving electron j mod k' at step j div k', through the warp's WarpBuf; then the owners take up to B steps whose
+//    dependent chain is only flight -> energy -> bin -> threshold record -> branch.  The draws depend on (id, n) alone, so
+//    the result is the same as drawing them in place; draws of steps an electron does not reach are discarded.
+//  * k > kCoopMax — full warp: up to kFlights free flights per lane (a lane stops flying when it draws a real
+//    collision), the draws of a lane's next flight issued behind its threshold-record load, then ONE collision phase.
+// Then the rare warp-uniform branches: append secondaries, retire finished electrons, refill idle lanes.
+constexpr int kFlights = AVM_FLIGHTS;
+constexpr int kCoopMax = AVM_COOP_MAX;
 
-template <bool UNIFORM1, bool HASB, bool TALLY>
+template <bool UNIFORM1, bool HASB, bool TALLY, bool SMEMTAB>
 __global__ void __launch_bounds__(kThreads, kMinCtasPerSm)
 transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevField f, const RunArrays a,
                  RunCtl* __restrict__ ctl, const uint64_t seed, const double t_max, const uint32_t max_iters,
                  const uint32_t n_static_tickets) {
+  extern __shared__ __align__(16) unsigned char s_dyn[];
   __shared__ double s_loss[AVM_MAX_LEVELS], s_recoil[AVM_MAX_LEVELS], s_w[AVM_MAX_LEVELS];
   __shared__ uint8_t s_type[AVM_MAX_LEVELS];
   __shared__ unsigned int s_hist[AVM_MAX_LEVELS];
@@ -85,87 +131,68 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
     s_loss[l] = in ? g.loss[l] : 0.0; s_recoil[l] = in ? g.recoil[l] : 0.0; s_w[l] = in ? g.w[l] : 1.0;
     s_type[l] = in ? g.type[l] : 0; s_hist[l] = 0u;
   }
+  const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+  const ushort4* tab = g.tab;
+  size_t dyn_off = 0;
+  if (SMEMTAB) {                                   // threshold table: 8 bytes per bin, resident in shared memory
+    uint2* dst = reinterpret_cast<uint2*>(s_dyn);
+    const uint2* src = reinterpret_cast<const uint2*>(g.tab);
+    for (int b = threadIdx.x; b < g.nb; b += blockDim.x) dst[b] = __ldg(src + b);
+    tab = reinterpret_cast<const ushort4*>(s_dyn);
+    dyn_off = ((size_t)g.nb * sizeof(ushort4) + 15) & ~(size_t)15;
+  }
+  WarpBuf* const wb = reinterpret_cast<WarpBuf*>(s_dyn + dyn_off) + warp;
+  int* const done = reinterpret_cast<int*>(reinterpret_cast<unsigned char*>(ctl) + kDoneOffset) + 8 * blockIdx.x;
   __syncthreads();
 
-  const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
   const uint32_t cap = a.cap;
   const size_t ld = cap;
-  // static tickets, warp-major across the grid: the first electrons fill whole warps, one warp per CTA first
-  uint32_t ticket = (warp * gridDim.x + blockIdx.x) * 32u + lane;
-  bool have = false;
+  // static tickets, CTA-major then warp then lane: the first electrons go one per warp, spread over all SMs
+  uint32_t ticket = (lane * kWarpsPerCta + warp) * gridDim.x + blockIdx.x;
+  bool have = false, dvalid = false;
   double x = 0, y = 0, z = 0, t = 0, vx = 0, vy = 0, vz = 0, Ex = 0, Ey = 0, Ez = 0, dt = 0, u2 = 0;
   uint64_t id = 0;
   uint32_t n = 0, slot = 0;
   uint32_t c_real = 0, c_l0 = 0, c_over = 0;      // tallies kept per thread; null counts are derived (finalize_kernel)
   double c_loss = 0.0;
-  uint32_t backoff = 100u;
+  uint32_t backoff = 250u;
+  const unsigned lt_mask = (1u << lane) - 1u;
 
-  for (uint32_t it = 0; it < max_iters; ++it) {
-    unsigned act = __ballot_sync(0xFFFFFFFFu, have);
-    // ---- refill idle lanes through their tickets (a-10): rare, warp-uniform branch ----
-    if (act != 0xFFFFFFFFu && (act == 0u || (it % kRefillEvery) == 0u)) {
-      if (!have) {
+  // idle lanes poll their own ticket: pick the electron up when its slot is published (a-10)
+  auto refill = [&]() {
+    if (!have) {
 #pragma unroll 1
-        for (int tries = 0; tries < 2 && ticket < cap; ++tries) {
-          const int st = ld_volatile_s32(a.status + ticket);
-          if (st == 0) {                              // published and unfinished: this lane runs it
-            __threadfence();
-            slot = ticket;
-            x = __ldcg(a.end + slot); y = __ldcg(a.end + ld + slot); z = __ldcg(a.end + 2 * ld + slot);
-            t = __ldcg(a.end + 3 * ld + slot);
-            const double e = __ldcg(a.end + 4 * ld + slot);
-            const double sp = kC2 * sqrt(e);
-            vx = sp * __ldcg(a.end + 5 * ld + slot); vy = sp * __ldcg(a.end + 6 * ld + slot);
-            vz = sp * __ldcg(a.end + 7 * ld + slot);
-            id = __ldcg(a.id + slot);
-            n = __ldcg(a.nsteps + slot);
-            double m;
-            field_at<UNIFORM1>(f, x, y, z, Ex, Ey, Ez, m);     // S0 of its first step (in-domain by construction)
-            draw_flight(g, seed, id, n, dt, u2);
-            have = true;
-            break;
-          }
-          if (st < 0) break;                          // not created yet: keep the ticket
-          ticket = n_static_tickets + atomicAdd(&ctl->q_head, 1u);   // finished in an earlier launch: next ticket
+      for (int tries = 0; tries < 2 && ticket < cap; ++tries) {
+        const int st = ld_relaxed_s32(a.status + ticket);
+        if (st == 0) {                              // published and unfinished: this lane runs it
+          slot = ticket;
+          x = __ldcg(a.end + slot); y = __ldcg(a.end + ld + slot); z = __ldcg(a.end + 2 * ld + slot);
+          t = __ldcg(a.end + 3 * ld + slot);
+          const double e = __ldcg(a.end + 4 * ld + slot);
+          const double sp = kC2 * sqrt(e);
+          vx = sp * __ldcg(a.end + 5 * ld + slot); vy = sp * __ldcg(a.end + 6 * ld + slot);
+          vz = sp * __ldcg(a.end + 7 * ld + slot);
+          id = __ldcg(a.id + slot);
+          n = __ldcg(a.nsteps + slot);
+          double m;
+          field_at<UNIFORM1>(f, x, y, z, Ex, Ey, Ez, m);     // S0 of its first step (in-domain by construction)
+          have = true; dvalid = false;
+          break;
         }
-      }
-      act = __ballot_sync(0xFFFFFFFFu, have);
-      if (act == 0u) {                                // whole warp idle: poll for termination, back off
-        unsigned long long c = 0ull;
-        if (lane == 0u) c = ld_volatile_u64(&ctl->counters);
-        c = __shfl_sync(0xFFFFFFFFu, c, 0);
-        if ((uint32_t)(c >> 32) == (uint32_t)c) break;
-        __nanosleep(backoff);
-        backoff = min(backoff * 2u, 3200u);
-        continue;
-      }
-      backoff = 100u;
-    }
-
-    // ---- flights ----
-    int fin = 0;                 // finishing status of this lane's electron (0 = still running)
-    bool pend = false;
-    Pending pc;
-    pc.lsel = 0; pc.bin = 0; pc.xr = 0.0;
-#pragma unroll
-    for (int fl = 0; fl < kFlights; ++fl) {
-      if (have && !pend && fin == 0) {
-        bool over = false;
-        const int r = flight_step<UNIFORM1, HASB>(g, f, seed, t_max, id, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt, u2,
-                                                  pc, over);
-        if (r < 0) fin = -r;
-        else if (r > 0) pend = true;
-        if (TALLY && over) ++c_over;
+        if (st < 0) break;                          // not created yet: keep the ticket
+        ticket = n_static_tickets + atomicAdd(&ctl->q_head, 1u);   // finished in an earlier launch: next ticket
       }
     }
-    // ---- collision phase ----
+  };
+  // one collision phase for the lanes with a pending real collision, then append their secondaries (a-8, a-9)
+  auto collide_and_append = [&](bool pend, const Pending& pc, bool have_d, const Deflection& dd, int& fin) {
     bool spawn = false;
     Child ch;
     ch.e = 0.0; ch.u6 = 0.5; ch.u7 = 0.0;
     if (pend) {
       double loss;
       int st;
-      const int l = collision_step(g, s_type, s_loss, s_recoil, s_w, seed, id, n, pc, vx, vy, vz, st, spawn, ch, loss);
+      const int l = collision_step(g, s_type, s_loss, s_recoil, s_w, seed, id, n, pc, have_d, dd, vx, vy, vz, st, spawn, ch, loss);
       if (st) fin = st;
       if (TALLY) {
         ++c_real;
@@ -174,15 +201,14 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
         c_loss += loss;
       }
     }
-    // ---- append secondaries: one atomic per warp (a-9) ----
     const unsigned sm = __ballot_sync(0xFFFFFFFFu, spawn);
-    if (sm) {
+    if (sm) {                                       // one atomic per warp
       const int leader = __ffs(sm) - 1;
       unsigned long long old = 0ull;
       if ((int)lane == leader) old = atomicAdd(&ctl->counters, (unsigned long long)__popc(sm) << 32);
       old = __shfl_sync(0xFFFFFFFFu, old, leader);
       if (spawn) {
-        const uint64_t cs = (old >> 32) + (uint64_t)__popc(sm & ((1u << lane) - 1u));
+        const uint64_t cs = (old >> 32) + (uint64_t)__popc(sm & lt_mask);
         if (cs < (uint64_t)cap) {
           const uint32_t c = (uint32_t)cs;
           double ckx, cky, ckz;
@@ -197,15 +223,17 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
             __stcg(a.birth + c, x); __stcg(a.birth + ld + c, y); __stcg(a.birth + 2 * ld + c, z);
             __stcg(a.birth + 3 * ld + c, t); __stcg(a.birth + 4 * ld + c, ch.e);
           }
-          __threadfence();
-          *(volatile int*)(a.status + c) = 0;       // publish
+          st_release_s32(a.status + c, 0);          // publish
         } else {                                    // no room: drop the child, count it as created and finished
           atomicAdd(&ctl->dropped, 1u);
           atomicAdd(&ctl->counters, 1ull);
         }
       }
     }
-    // ---- retire finished electrons: endpoint write, one atomic per warp for `done`, one for new tickets ----
+  };
+  // retire finished electrons: endpoint write, one atomic per warp for `finished`, one for new tickets; the lane that
+  // finishes the last electron raises every CTA's done flag (a-11)
+  auto retire = [&](int fin) {
     const unsigned fm = __ballot_sync(0xFFFFFFFFu, fin != 0);
     if (fm) {
       const int leader = __ffs(fm) - 1;
@@ -222,10 +250,120 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
         a.nsteps[slot] = n;
         a.status[slot] = fin;
         have = false;
-        ticket = n_static_tickets + base + (uint32_t)__popc(fm & ((1u << lane) - 1u));
+        ticket = n_static_tickets + base + (uint32_t)__popc(fm & lt_mask);
       }
-      if ((int)lane == leader) atomicAdd(&ctl->counters, (unsigned long long)__popc(fm));
+      if ((int)lane == leader) {
+        const unsigned long long add = (unsigned long long)__popc(fm);
+        const unsigned long long now = atomicAdd(&ctl->counters, add) + add;
+        if ((uint32_t)(now >> 32) == (uint32_t)now) {          // created == finished: nothing can be created any more
+          int* d0 = reinterpret_cast<int*>(reinterpret_cast<unsigned char*>(ctl) + kDoneOffset);
+          for (unsigned b = 0; b < gridDim.x; ++b) *(volatile int*)(d0 + 8 * b) = 1;
+        }
+      }
     }
+  };
+
+  for (uint32_t it = 0; it < max_iters; ++it) {
+    unsigned act = __ballot_sync(0xFFFFFFFFu, have);
+    // ---- probe the warp's lowest pending ticket (one sector per warp); consumed after the iteration's work ----
+    uint32_t tmin = 0xFFFFFFFFu;
+    int probe = -1;
+    if (act != 0xFFFFFFFFu) {
+      tmin = __reduce_min_sync(0xFFFFFFFFu, have ? 0xFFFFFFFFu : ticket);
+      if (tmin < cap) probe = ld_relaxed_s32(a.status + tmin);
+    }
+    if (act == 0u) {                                // whole warp idle
+      if (probe == -1) {                            // nothing to pick up: check for the end, back off
+        if (ld_relaxed_s32(done) != 0) break;
+        idle_wait(backoff);
+        backoff = min(backoff * 2u, 2000u);
+        continue;
+      }
+      refill();
+      backoff = 250u;
+      act = __ballot_sync(0xFFFFFFFFu, have);
+      if (act == 0u) continue;
+      probe = -1;
+    }
+    const int k = __popc(act);
+
+    if (k <= kCoopMax) {
+      // ---- cooperative batch ----
+      const int lg = 32 - __clz(k - 1);             // k' = 2^lg >= k  (k = 1: __clz(0) = 32)
+      const int kp = 1 << lg, nb_steps = 32 >> lg;
+      const int rank = __popc(act & lt_mask);
+      if (have) { wb->id[rank] = id; wb->n[rank] = n; }
+      __syncwarp();
+      {
+        const int e = (int)lane & (kp - 1), s = (int)lane >> lg;
+        if (e < k) {
+          const uint64_t hid = wb->id[e];
+          const uint32_t hn = wb->n[e] + (uint32_t)s;
+          double ddt, du2;
+          draw_flight(g, seed, hid, hn, ddt, du2);
+          const Deflection d = deflection_draws(seed, hid, hn);
+          wb->dt[lane] = ddt; wb->u2[lane] = du2;
+          wb->ct[lane] = d.ct; wb->st[lane] = d.st; wb->cphi[lane] = d.cphi; wb->sphi[lane] = d.sphi;
+        }
+      }
+      __syncwarp();
+      dvalid = false;
+#pragma unroll 1
+      for (int s = 0; s < nb_steps; ++s) {
+        int fin = 0;
+        bool pend = false;
+        Pending pc;
+        pc.lsel = 0; pc.bin = 0; pc.xr = 0.0;
+        Deflection dd;
+        dd.ct = 1.0; dd.st = 0.0; dd.cphi = 1.0; dd.sphi = 0.0;
+        if (have) {
+          const int idx = s * kp + rank;
+          bool over = false;
+          const int b = advance<UNIFORM1, HASB>(g, f, t_max, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, wb->dt[idx], over);
+          if (b < 0) fin = -b;
+          else {
+            const int r = decide(g, tab[b], b, wb->u2[idx], pc.xr);
+            if (r >= 0) {
+              pend = true; pc.lsel = r; pc.bin = b;
+              dd.ct = wb->ct[idx]; dd.st = wb->st[idx]; dd.cphi = wb->cphi[idx]; dd.sphi = wb->sphi[idx];
+            }
+            if (TALLY && over) ++c_over;
+          }
+        }
+        if (__any_sync(0xFFFFFFFFu, pend)) collide_and_append(pend, pc, true, dd, fin);
+        retire(fin);
+        if (!__any_sync(0xFFFFFFFFu, have)) break;
+      }
+    } else {
+      // ---- full warp ----
+      if (have && !dvalid) { draw_flight(g, seed, id, n, dt, u2); dvalid = true; }
+      int fin = 0;
+      bool pend = false;
+      Pending pc;
+      pc.lsel = 0; pc.bin = 0; pc.xr = 0.0;
+#pragma unroll
+      for (int fl = 0; fl < kFlights; ++fl) {
+        if (have && !pend && fin == 0) {
+          bool over = false;
+          const int b = advance<UNIFORM1, HASB>(g, f, t_max, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt, over);
+          if (b < 0) fin = -b;
+          else {
+            const ushort4 rec = tab[b];
+            const double u2c = u2;
+            draw_flight(g, seed, id, n, dt, u2);    // next flight's draws: independent of the record load
+            const int r = decide(g, rec, b, u2c, pc.xr);
+            if (r >= 0) { pend = true; pc.lsel = r; pc.bin = b; }
+            if (TALLY && over) ++c_over;
+          }
+        }
+      }
+      Deflection dd;
+      dd.ct = 1.0; dd.st = 0.0; dd.cphi = 1.0; dd.sphi = 0.0;
+      collide_and_append(pend, pc, false, dd, fin);
+      retire(fin);
+    }
+    // ---- refill idle lanes when the probed ticket has been published ----
+    if (probe != -1) refill();
   }
 
   // guard expired with the electron still active: park its state in its slot (status stays 0); the next
@@ -401,12 +539,19 @@ __global__ void step_batch_kernel(const __grid_constant__ DevGas g, const __grid
   Child ch;
   ch.e = 0.0; ch.u6 = 0.5; ch.u7 = 0.0;
   int ev = -2, st = 0;
-  const int r = flight_step<UNIFORM1, HASB>(g, f, seed, t_max, id, nn, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt, u2, pc, over);
-  if (r < 0) st = -r;
-  else if (r == 0) ev = -1;
+  const int b = advance<UNIFORM1, HASB>(g, f, t_max, nn, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt, over);
+  if (b < 0) st = -b;
   else {
-    double loss;
-    ev = collision_step(g, g.type, g.loss, g.recoil, g.w, seed, id, nn, pc, vx, vy, vz, st, spawn, ch, loss);
+    pc.bin = b;
+    const int r = decide(g, __ldg(g.tab + b), b, u2, pc.xr);
+    if (r < 0) ev = -1;
+    else {
+      double loss;
+      pc.lsel = r;
+      Deflection dd;
+      dd.ct = 1.0; dd.st = 0.0; dd.cphi = 1.0; dd.sphi = 0.0;
+      ev = collision_step(g, g.type, g.loss, g.recoil, g.w, seed, id, nn, pc, false, dd, vx, vy, vz, st, spawn, ch, loss);
+    }
   }
   // state after the step in (energy, direction) form
   const double s2 = vx * vx + vy * vy + vz * vz;
@@ -414,7 +559,7 @@ __global__ void step_batch_kernel(const __grid_constant__ DevGas g, const __grid
   out[i] = x; out[n + i] = y; out[2 * n + i] = z; out[3 * n + i] = t; out[4 * n + i] = fmax(s2 * kInvC2Sq, kEpsFloor);
   out[5 * n + i] = kx; out[6 * n + i] = ky; out[7 * n + i] = kz;
   event[i] = ev; status[i] = st;
-  bin[i] = r < 0 ? -1 : pc.bin;
+  bin[i] = pc.bin;
   if (spawn) {
     double ckx, cky, ckz;
     child_direction(ch.u6, ch.u7, ckx, cky, ckz);
@@ -509,12 +654,13 @@ bool valid_gas(const avm_gas_desc* d, double* max_rate) {
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
-struct GasLayout { size_t nu_tot, head, cum, loss, recoil, w, type, total; };
+struct GasLayout { size_t nu_tot, head, tab, cum, loss, recoil, w, type, total; };
 GasLayout gas_layout(int nb, int L) {
   GasLayout g;
   size_t off = 0;
   g.nu_tot = off; off = align_up(off + sizeof(double) * nb, 256);
   g.head = off;   off = align_up(off + 4 * sizeof(double) * (size_t)nb, 256);
+  g.tab = off;    off = align_up(off + sizeof(ushort4) * (size_t)nb, 256);
   g.cum = off;    off = align_up(off + sizeof(double) * (size_t)nb * L, 256);
   g.loss = off;   off += sizeof(double) * AVM_MAX_LEVELS;
   g.recoil = off; off += sizeof(double) * AVM_MAX_LEVELS;
@@ -588,6 +734,12 @@ int32_t avm_gas_create(avm_ctx* ctx, const avm_gas_desc* d, void* dev_buf, size_
   std::vector<unsigned char> h(lay.total, 0);
   double* nu_tot = (double*)(h.data() + lay.nu_tot);
   double* head = (double*)(h.data() + lay.head);
+  unsigned short* tab = (unsigned short*)(h.data() + lay.tab);
+  const double nu_hat_r = d->nu_hat > 0.0 ? d->nu_hat : mx;
+  auto q16 = [&](double c) {                       // floor(c / nu_hat * 2^16) clamped to 16 bits (decide())
+    const double v = std::floor(c / nu_hat_r * 65536.0);
+    return (unsigned short)(v < 0.0 ? 0.0 : (v > 65535.0 ? 65535.0 : v));
+  };
   for (int b = 0; b < nb; ++b) {
     const double* row = d->cum_rate + (size_t)b * L;
     nu_tot[b] = row[L - 1];
@@ -595,6 +747,10 @@ int32_t avm_gas_create(avm_ctx* ctx, const avm_gas_desc* d, void* dev_buf, size_
     head[4 * (size_t)b + 1] = row[0];
     head[4 * (size_t)b + 2] = row[L > 1 ? 1 : 0];
     head[4 * (size_t)b + 3] = 0.0;
+    tab[4 * (size_t)b + 0] = q16(row[L - 1]);
+    tab[4 * (size_t)b + 1] = q16(row[0]);
+    tab[4 * (size_t)b + 2] = q16(row[L > 1 ? 1 : 0]);
+    tab[4 * (size_t)b + 3] = 0;
   }
   std::memcpy(h.data() + lay.cum, d->cum_rate, sizeof(double) * (size_t)nb * L);
   std::memcpy(h.data() + lay.loss, d->level_loss_eV, sizeof(double) * L);
@@ -614,6 +770,7 @@ int32_t avm_gas_create(avm_ctx* ctx, const avm_gas_desc* d, void* dev_buf, size_
   g->d.inv_nu_hat = 1.0 / g->nu_hat;
   g->d.nu_tot = (const double*)(base + lay.nu_tot);
   g->d.head = (const double2*)(base + lay.head);
+  g->d.tab = (const ushort4*)(base + lay.tab);
   g->d.cum = (const double*)(base + lay.cum);
   g->d.loss = (const double*)(base + lay.loss);
   g->d.recoil = (const double*)(base + lay.recoil);
@@ -718,18 +875,23 @@ int32_t avm_run_transport_ms(const avm_ctx* c, float* ms_out) {
   return AVM_OK;
 }
 
+}  // extern "C"
+
 namespace {
 typedef void (*TransportFn)(const DevGas, const DevField, const RunArrays, RunCtl*, const uint64_t, const double,
                             const uint32_t, const uint32_t);
-TransportFn pick_transport(bool uniform1, bool has_b, bool tally) {
-  if (uniform1) {
-    if (has_b) return tally ? transport_kernel<true, true, true> : transport_kernel<true, true, false>;
-    return tally ? transport_kernel<true, false, true> : transport_kernel<true, false, false>;
-  }
-  if (has_b) return tally ? transport_kernel<false, true, true> : transport_kernel<false, true, false>;
-  return tally ? transport_kernel<false, false, true> : transport_kernel<false, false, false>;
+template <bool U, bool B>
+TransportFn pick2(bool tally, bool smemtab) {
+  if (tally) return smemtab ? transport_kernel<U, B, true, true> : transport_kernel<U, B, true, false>;
+  return smemtab ? transport_kernel<U, B, false, true> : transport_kernel<U, B, false, false>;
+}
+TransportFn pick_transport(bool uniform1, bool has_b, bool tally, bool smemtab) {
+  if (uniform1) return has_b ? pick2<true, true>(tally, smemtab) : pick2<true, false>(tally, smemtab);
+  return has_b ? pick2<false, true>(tally, smemtab) : pick2<false, false>(tally, smemtab);
 }
 }  // namespace
+
+extern "C" {
 
 int32_t avm_run(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, const double* primaries, int64_t np,
                 const avm_run_opts* opts, const avm_outputs* o, int64_t* n_out) {
@@ -768,12 +930,18 @@ int32_t avm_run(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, const 
     else AVM_CUDA(launch(ctx, inject_kernel<false>, grid, dim3(256), field->d, a, ctl, src, (uint32_t)p0, (uint32_t)cnt, opts->id_offset, opts->t_max));
   }
   // persistent transport (a-2 .. a-11)
-  TransportFn fn = pick_transport(field->uniform1, field->d.has_B != 0, tally);
+  const size_t buf_bytes = sizeof(WarpBuf) * kWarpsPerCta;
+  const size_t tab_bytes = align_up(sizeof(ushort4) * (size_t)gas->d.nb, 16);
+  const bool smemtab = tab_bytes + buf_bytes <= kMaxDynSmem;       // else the threshold table is read through L1
+  const size_t dyn_smem = (smemtab ? tab_bytes : 0) + buf_bytes;
+  TransportFn fn = pick_transport(field->uniform1, field->d.has_B != 0, tally, smemtab);
+  AVM_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn_smem));
   int occ = 0;
-  AVM_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kThreads, 0));
+  AVM_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kThreads, dyn_smem));
   if (occ < 1) return fail(AVM_ERR_CUDA, "run: transport kernel does not fit on an SM");
   if (opts->n_ctas_per_sm > 0 && opts->n_ctas_per_sm < occ) occ = opts->n_ctas_per_sm;
-  const unsigned grid = (unsigned)(ctx->sm_count * occ);
+  unsigned grid = (unsigned)(ctx->sm_count * occ);
+  if (grid > (unsigned)kMaxGrid) grid = kMaxGrid;
   const uint32_t n_static = grid * kThreads;
   const uint32_t max_iters = opts->max_iters_per_launch ? opts->max_iters_per_launch : kDefaultMaxIters;
   unsigned long long c = 0ull;
@@ -792,7 +960,7 @@ int32_t avm_run(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, const 
       ctx->transport_ms += ms;
     }
     AVM_CUDA(cudaEventRecord(ctx->ev_t0, st));
-    fn<<<grid, kThreads, 0, st>>>(gas->d, field->d, a, ctl, opts->seed, opts->t_max, max_iters, n_static);
+    fn<<<grid, kThreads, dyn_smem, st>>>(gas->d, field->d, a, ctl, opts->seed, opts->t_max, max_iters, n_static);
     AVM_CUDA(cudaGetLastError());
     AVM_CUDA(cudaEventRecord(ctx->ev_t1, st));
     ctx->n_kernel_launches++; ctx->n_transport_launches++;

@@ -24,7 +24,8 @@ struct DevGas {
   int nb, L;
   double inv_de, nu_hat, inv_nu_hat;
   const double* nu_tot;   // [nb]      total real-collision rate per bin (= cum[b][L-1])
-  const double2* head;    // [nb][2]   decision record, 32 B: (nu_tot, cum[b][0]), (cum[b][min(1,L-1)], 0)
+  const double2* head;    // [nb][2]   exact decision record, 32 B: (nu_tot, cum[b][0]), (cum[b][min(1,L-1)], 0)
+  const ushort4* tab;     // [nb]      16-bit thresholds floor(c 2^16), c = (nu_tot, cum0, cum1)/nu_hat: the filter of decide()
   const double* cum;      // [nb][L]   cumulative rates, row-major by bin
   const double* loss;     // [L]
   const double* recoil;   // [L]
@@ -284,22 +285,30 @@ __device__ __forceinline__ uint64_t child_id_of(uint64_t seed, uint64_t id, uint
   return (uint64_t)w.w0 | ((uint64_t)w.w1 << 32);
 }
 
-// Real collision of level l at energy e1, direction k (unit).  type/loss/recoil/w are the level's parameters.
-// Returns the new energy; updates k; fills `ch` and returns spawn=true for an ionisation.  *loss_out = energy
-// leaving the electron population (tally).  Attachment is handled by the caller (S9a).
-__device__ __forceinline__ double collide(uint64_t seed, uint64_t id, uint32_t n_s, int type, double lv_loss,
-                                          double lv_recoil, double lv_w, double e1, double& kx, double& ky,
-                                          double& kz, bool& spawn, Child& ch, double& loss_out) {
+// S9b: the deflection draws of step n_s — block 1 -> (cos theta, sin theta, cos phi, sin phi).  They depend on
+// (id, n_s) only, so idle lanes can prepare them ahead of the decision (transport kernel, cooperative batches).
+struct Deflection { double ct, st, cphi, sphi; };
+
+__device__ __forceinline__ Deflection deflection_draws(uint64_t seed, uint64_t id, uint32_t n_s) {
   const U4 r1 = philox(seed, id, n_s, 1u);
   const double u3 = to_unit(r1.w0, r1.w1), u4 = to_unit(r1.w2, r1.w3);
-  const double ct = 1.0 - 2.0 * u3;
-  const double st = 2.0 * sqrt(u3 * (1.0 - u3));
-  double sphi, cphi;
-  sincos_2pi(u4, sphi, cphi);
+  Deflection d;
+  d.ct = 1.0 - 2.0 * u3;
+  d.st = 2.0 * sqrt(u3 * (1.0 - u3));
+  sincos_2pi(u4, d.sphi, d.cphi);
+  return d;
+}
+
+// Real collision of level l at energy e1, direction k (unit), deflection d.  type/loss/recoil/w are the level's
+// parameters.  Returns the new energy; updates k; fills `ch` and returns spawn=true for an ionisation.  *loss_out =
+// energy leaving the electron population (tally).  Attachment is handled by the caller (S9a).
+__device__ __forceinline__ double collide(uint64_t seed, uint64_t id, uint32_t n_s, int type, double lv_loss,
+                                          double lv_recoil, double lv_w, double e1, const Deflection& d, double& kx,
+                                          double& ky, double& kz, bool& spawn, Child& ch, double& loss_out) {
   double e2;
   spawn = false;
   if (type == AVM_ELASTIC) {
-    e2 = e1 * (1.0 - lv_recoil * (1.0 - ct));
+    e2 = e1 * (1.0 - lv_recoil * (1.0 - d.ct));
     loss_out = e1 - e2;
   } else if (type == AVM_EXCITATION) {
     e2 = fmax(e1 - lv_loss, kEpsFloor);
@@ -317,7 +326,7 @@ __device__ __forceinline__ double collide(uint64_t seed, uint64_t id, uint32_t n
     spawn = true;
     loss_out = e1 - e2 - ch.e;
   }
-  deflect(kx, ky, kz, ct, st, cphi, sphi);
+  deflect(kx, ky, kz, d.ct, d.st, d.cphi, d.sphi);
   return e2;
 }
 
@@ -331,9 +340,9 @@ __device__ __forceinline__ int select_level_from2(const DevGas& g, int b, double
 }
 
 // ---- one step, split at the null/real decision ----------------------------------------------------------------
-// Electron state is kept in velocity form (r, t, v, id, n) plus the draws of its NEXT flight (dt, u2), which are
-// computed one step ahead: the Philox block and the logarithm of step n+1 depend only on (id, n+1) and fill the
-// latency of the decision-record load of step n.
+// Electron state is kept in velocity form (r, t, v, id, n).  The draws of a flight (dt, u2) depend on (id, n) only and
+// are prepared ahead of the flight that uses them — by the lane itself one step ahead, or by the idle lanes of its warp
+// a whole batch ahead (transport kernel).
 struct Pending { int lsel, bin; double xr; };   // lsel: 0 / 1 = level decided from the head record, 2 = scan the row
 
 __device__ __forceinline__ void draw_flight(const DevGas& g, uint64_t seed, uint64_t id, uint32_t n, double& dt,
@@ -343,13 +352,29 @@ __device__ __forceinline__ void draw_flight(const DevGas& g, uint64_t seed, uint
   u2 = to_unit(r0.w2, r0.w3);
 }
 
-// S2-S7 for one electron.  Returns 0 = null collision (continue), 1 = real collision pending (p filled),
-// < 0 = -(finishing status).  (dt, u2) in: this flight's draws; out: the next flight's.  overflow: energy clamped.
+// S7 + the common part of S8 for bin b and uniform u2: -1 = null collision, 0 / 1 = level 0 / 1, 2 = a level >= 2
+// (p.xr is then needed for the row scan).  `rec` = tab[b] holds q = floor(c 2^16) for c = (nu_tot, cum0, cum1)/nu_hat;
+// with h = floor(u2 2^16): h >= q + 2 implies u2 nu_hat >= cum and h <= q - 2 implies u2 nu_hat < cum with a margin of
+// nu_hat 2^-16, far above the rounding of the fp64 product — so the 16-bit filter takes the oracle's decision exactly,
+// and the 2e-4 of the steps that fall inside a band are decided from the exact fp64 record.
+__device__ __forceinline__ int decide(const DevGas& g, const ushort4 rec, int b, double u2, double& xr) {
+  const uint32_t h = (uint32_t)__double2int_rz(u2 * 65536.0);     // exact: top 16 bits of the uniform
+  const uint32_t qt = rec.x, q0 = rec.y, q1 = rec.z;
+  xr = u2 * g.nu_hat;
+  if (h >= qt + 2u) return -1;
+  if (h + 2u <= q0) return 0;
+  if (h >= q0 + 2u && h + 2u <= q1) return 1;
+  if (h >= q1 + 2u && h + 2u <= qt) return 2;
+  const double2 h0 = __ldg(g.head + 2 * (size_t)b), h1 = __ldg(g.head + 2 * (size_t)b + 1);
+  if (xr >= h0.x) return -1;
+  return xr < h0.y ? 0 : (xr < h1.x ? 1 : 2);
+}
+
+// S3-S6 for one electron with this flight's dt.  Returns the energy bin (>= 0) or -(finishing status).
 template <bool UNIFORM1, bool HASB>
-__device__ __forceinline__ int flight_step(const DevGas& g, const DevField& f, uint64_t seed, double t_max,
-                                           uint64_t id, uint32_t& n, double& x, double& y, double& z, double& t,
-                                           double& vx, double& vy, double& vz, double& Ex, double& Ey, double& Ez,
-                                           double& dt, double& u2, Pending& p, bool& overflow) {
+__device__ __forceinline__ int advance(const DevGas& g, const DevField& f, double t_max, uint32_t& n, double& x,
+                                       double& y, double& z, double& t, double& vx, double& vy, double& vz, double& Ex,
+                                       double& Ey, double& Ez, double dt, bool& overflow) {
   flight<HASB>(f, Ex, Ey, Ez, dt, x, y, z, vx, vy, vz);     // S3
   const double s2 = vx * vx + vy * vy + vz * vz;            // S4
   const double e1 = fmax(s2 * kInvC2Sq, kEpsFloor);
@@ -362,34 +387,27 @@ __device__ __forceinline__ int flight_step(const DevGas& g, const DevField& f, u
   if (t > t_max) return -AVM_TIME_LIMIT;
   if (n >= kStepLimit) return -AVM_STEP_LIMIT;
   const double sb = e1 * g.inv_de;                          // S6
-  int b;
   overflow = sb >= (double)g.nb;
-  b = overflow ? g.nb - 1 : (int)sb;
-  const double2 h0 = __ldg(g.head + 2 * (size_t)b), h1 = __ldg(g.head + 2 * (size_t)b + 1);
-  const double xr = u2 * g.nu_hat;                          // S7 (this flight's u2)
-  draw_flight(g, seed, id, n, dt, u2);                      // next flight's draws: independent of the load above
-  p.bin = b;
-  if (xr >= h0.x) return 0;
-  p.lsel = xr < h0.y ? 0 : (xr < h1.x ? 1 : 2);
-  p.xr = xr;
-  return 1;
+  return overflow ? g.nb - 1 : (int)sb;
 }
 
 // S8-S9 for an electron with a pending real collision (n already incremented by the flight).  Returns the level;
-// status = AVM_ATTACHED for an attachment, else 0 and v is the velocity after the collision.
+// status = AVM_ATTACHED for an attachment, else 0 and v is the velocity after the collision.  d = deflection_draws of
+// step n - 1 when `have_d`, else drawn here.
 __device__ __forceinline__ int collision_step(const DevGas& g, const uint8_t* lv_type, const double* lv_loss,
                                               const double* lv_recoil, const double* lv_w, uint64_t seed, uint64_t id,
-                                              uint32_t n, const Pending& p, double& vx, double& vy, double& vz,
-                                              int& status, bool& spawn, Child& ch, double& loss) {
+                                              uint32_t n, const Pending& p, bool have_d, Deflection d, double& vx,
+                                              double& vy, double& vz, int& status, bool& spawn, Child& ch, double& loss) {
   const int l = p.lsel < 2 ? p.lsel : select_level_from2(g, p.bin, p.xr);     // S8
   const int type = lv_type[l];
   status = 0; spawn = false; loss = 0.0;
   if (type == AVM_ATTACHMENT) { status = AVM_ATTACHED; return l; }             // S9a
+  if (!have_d) d = deflection_draws(seed, id, n - 1u);                         // S9b
   const double s2 = vx * vx + vy * vy + vz * vz;
   const double e1 = fmax(s2 * kInvC2Sq, kEpsFloor);
   double kx = 0.0, ky = 0.0, kz = 1.0;
   if (s2 > 0.0) { const double inv = rsqrt(s2); kx = vx * inv; ky = vy * inv; kz = vz * inv; }
-  const double e2 = collide(seed, id, n - 1u, type, lv_loss[l], lv_recoil[l], lv_w[l], e1, kx, ky, kz, spawn, ch, loss);
+  const double e2 = collide(seed, id, n - 1u, type, lv_loss[l], lv_recoil[l], lv_w[l], e1, d, kx, ky, kz, spawn, ch, loss);
   const double sp = kC2 * sqrt(e2);
   vx = sp * kx; vy = sp * ky; vz = sp * kz;
   return l;
