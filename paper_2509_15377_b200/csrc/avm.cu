@@ -83,6 +83,10 @@ struct WarpBuf {
   double ct[32], st[32], cphi[32], sphi[32];
   unsigned long long id[32];
   unsigned int n[32];
+  // time-parallel batches: base state of electron e (entry e), written by its owner lane / its group's first lane
+  double bs[7][16];
+  unsigned int bslot[16];
+  int bfin[16];
 };
 
 __device__ __forceinline__ int ld_relaxed_s32(const int* p) {
@@ -287,7 +291,107 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
     }
     const int k = __popc(act);
 
-    if (k <= kCoopMax) {
+    if (UNIFORM1 && k <= kCoopMax) {
+      // ---- time-parallel batch (uniform E, optional B): g = 32 / k' lanes per electron ----
+      // In a constant field, consecutive null flights compose exactly: the state after flights dt_1 .. dt_j is the
+      // ballistic / helical flight of duration T_j = dt_1 + .. + dt_j from the base state.  Lane s of electron e's group
+      // evaluates the END of step s (position, energy, bounds, bin, null/real decision with its own u2) in parallel; the
+      // first lane whose step is not null (real collision or termination) is the electron's next event, every step
+      // before it was null, and the draws after it stay valid for the next pass from the new base state.  The draws
+      // depend on (id, n) only, so this is the sequence of steps S0-S9 the oracle takes, evaluated out of order.
+      const int lg = 32 - __clz(k - 1);             // k' = 2^lg >= k  (k = 1: __clz(0) = 32)
+      const int kp = 1 << lg, gl = 32 >> lg;        // gl = lanes (steps per batch) of one electron
+      const int rank = __popc(act & lt_mask);
+      const int e = (int)lane & (kp - 1), sidx = (int)lane >> lg;
+      if (have) {
+        wb->bs[0][rank] = x; wb->bs[1][rank] = y; wb->bs[2][rank] = z; wb->bs[3][rank] = t;
+        wb->bs[4][rank] = vx; wb->bs[5][rank] = vy; wb->bs[6][rank] = vz;
+        wb->id[rank] = id; wb->n[rank] = n; wb->bslot[rank] = slot;
+      }
+      __syncwarp();
+      bool alive = e < k;
+      double bx = 0, by = 0, bz = 0, bt = 0, bvx = 0, bvy = 0, bvz = 0;
+      uint32_t bn = 0;
+      if (alive) {
+        bx = wb->bs[0][e]; by = wb->bs[1][e]; bz = wb->bs[2][e]; bt = wb->bs[3][e];
+        bvx = wb->bs[4][e]; bvy = wb->bs[5][e]; bvz = wb->bs[6][e];
+        id = wb->id[e]; bn = wb->n[e]; slot = wb->bslot[e];
+      }
+      __syncwarp();
+      // draws of step bn + sidx, and the inclusive sums P of dt over the group's steps 0 .. sidx
+      double P = 0.0, u2j = 0.0;
+      Deflection dj;
+      dj.ct = 1.0; dj.st = 0.0; dj.cphi = 1.0; dj.sphi = 0.0;
+      if (alive) {
+        draw_flight(g, seed, id, bn + (uint32_t)sidx, P, u2j);
+        dj = deflection_draws(seed, id, bn + (uint32_t)sidx);
+      }
+      for (int d = kp; d < 32; d <<= 1) {
+        const double up = __shfl_up_sync(0xFFFFFFFFu, P, d);
+        if ((int)lane >= d) P += up;
+      }
+      const unsigned gmask = (lg == 0 ? 0xFFFFFFFFu : lg == 1 ? 0x55555555u : lg == 2 ? 0x11111111u
+                              : lg == 3 ? 0x01010101u : 0x00010001u) << e;
+      const int last = ((gl - 1) << lg) | e;
+      double Pb = 0.0;
+      int cur = 0, gfin = 0;
+      Ex = f.slab[0].E[0]; Ey = f.slab[0].E[1]; Ez = f.slab[0].E[2];
+#pragma unroll 1
+      for (;;) {
+        const bool valid = alive && sidx >= cur;
+        x = bx; y = by; z = bz; t = bt; vx = bvx; vy = bvy; vz = bvz;
+        n = bn + (uint32_t)(sidx - cur);
+        bool over = false, ev = false;
+        int b = 0, r = -1;
+        Pending pc;
+        pc.lsel = 0; pc.bin = 0; pc.xr = 0.0;
+        if (valid) {
+          b = advance<UNIFORM1, HASB>(g, f, t_max, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, P - Pb, over);
+          if (b < 0) ev = true;
+          else { r = decide(g, tab[b], b, u2j, pc.xr); ev = r >= 0; }
+        }
+        const unsigned evm = __ballot_sync(0xFFFFFFFFu, ev) & gmask;
+        const int fl = __ffs(evm) - 1;                       // the group's first step that is not null, or -1
+        if (TALLY && valid && over && (fl < 0 || (int)lane <= fl)) ++c_over;
+        int fin = 0;
+        bool pend = false;
+        if ((int)lane == fl) {
+          if (b < 0) fin = -b;
+          else { pend = true; pc.lsel = r; pc.bin = b; }
+        }
+        if (__any_sync(0xFFFFFFFFu, pend)) collide_and_append(pend, pc, true, dj, fin);
+        // the group's new base: the state after its first event, or after its last step when all were null
+        const int src = fl >= 0 ? fl : last;
+        const double nx_ = __shfl_sync(0xFFFFFFFFu, x, src), ny_ = __shfl_sync(0xFFFFFFFFu, y, src);
+        const double nz_ = __shfl_sync(0xFFFFFFFFu, z, src), nt_ = __shfl_sync(0xFFFFFFFFu, t, src);
+        const double nvx = __shfl_sync(0xFFFFFFFFu, vx, src), nvy = __shfl_sync(0xFFFFFFFFu, vy, src);
+        const double nvz = __shfl_sync(0xFFFFFFFFu, vz, src), nP = __shfl_sync(0xFFFFFFFFu, P, src);
+        const uint32_t nn = __shfl_sync(0xFFFFFFFFu, n, src);
+        const int nfin = __shfl_sync(0xFFFFFFFFu, fin, src);
+        if (alive) {
+          bx = nx_; by = ny_; bz = nz_; bt = nt_; bvx = nvx; bvy = nvy; bvz = nvz; Pb = nP; bn = nn; gfin = nfin;
+          cur = (src >> lg) + 1;
+          if (gfin != 0 || cur >= gl) alive = false;
+        }
+        if (!__any_sync(0xFFFFFFFFu, alive)) break;
+      }
+      // hand the electrons back to their owner lanes
+      if (sidx == 0 && e < k) {
+        wb->bs[0][e] = bx; wb->bs[1][e] = by; wb->bs[2][e] = bz; wb->bs[3][e] = bt;
+        wb->bs[4][e] = bvx; wb->bs[5][e] = bvy; wb->bs[6][e] = bvz;
+        wb->n[e] = bn; wb->bfin[e] = gfin;
+      }
+      __syncwarp();
+      int fin = 0;
+      if (have) {
+        x = wb->bs[0][rank]; y = wb->bs[1][rank]; z = wb->bs[2][rank]; t = wb->bs[3][rank];
+        vx = wb->bs[4][rank]; vy = wb->bs[5][rank]; vz = wb->bs[6][rank];
+        id = wb->id[rank]; n = wb->n[rank]; slot = wb->bslot[rank]; fin = wb->bfin[rank];
+      }
+      __syncwarp();
+      dvalid = false;
+      retire(fin);
+    } else if (k <= kCoopMax) {
       // ---- cooperative batch ----
       const int lg = 32 - __clz(k - 1);             // k' = 2^lg >= k  (k = 1: __clz(0) = 32)
       const int kp = 1 << lg, nb_steps = 32 >> lg;
