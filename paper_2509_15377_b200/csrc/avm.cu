@@ -79,7 +79,8 @@ static_assert(sizeof(RunCtl) <= kDoneOffset, "ctl block");
 // Per-warp exchange area of the cooperative batches (shared memory): entry j = draws of electron (j mod k') at its
 // step (j div k') of the batch, written by lane j.
 struct WarpBuf {
-  double dt[32], u2[32];
+  double dt[32];
+  uint2 u2w[32];
   double ct[32], st[32], cphi[32], sphi[32];
   unsigned long long id[32];
   unsigned int n[32];
@@ -124,17 +125,16 @@ constexpr int kCoopMax = AVM_COOP_MAX;
 template <bool UNIFORM1, bool HASB, bool TALLY, bool SMEMTAB>
 __global__ void __launch_bounds__(kThreads, kMinCtasPerSm)
 transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevField f, const RunArrays a,
-                 RunCtl* __restrict__ ctl, const uint64_t seed, const double t_max, const uint32_t max_iters,
-                 const uint32_t n_static_tickets) {
+                 RunCtl* __restrict__ ctl, const __grid_constant__ PhiloxKeys K, const double t_max,
+                 const uint32_t max_iters, const uint32_t n_static_tickets) {
   extern __shared__ __align__(16) unsigned char s_dyn[];
-  __shared__ double s_loss[AVM_MAX_LEVELS], s_recoil[AVM_MAX_LEVELS], s_w[AVM_MAX_LEVELS];
-  __shared__ uint8_t s_type[AVM_MAX_LEVELS];
+  __shared__ LevelPar s_lv[AVM_MAX_LEVELS];
+  __shared__ double2 s_logtab[128];
   __shared__ unsigned int s_hist[AVM_MAX_LEVELS];
-  for (int l = threadIdx.x; l < AVM_MAX_LEVELS; l += blockDim.x) {
-    const bool in = l < g.L;
-    s_loss[l] = in ? g.loss[l] : 0.0; s_recoil[l] = in ? g.recoil[l] : 0.0; s_w[l] = in ? g.w[l] : 1.0;
-    s_type[l] = in ? g.type[l] : 0; s_hist[l] = 0u;
-  }
+  stage_levels(g, s_lv);
+  for (int l = threadIdx.x; l < AVM_MAX_LEVELS; l += blockDim.x) s_hist[l] = 0u;
+  for (int i = threadIdx.x; i < 128; i += blockDim.x)
+    s_logtab[i] = make_double2(__longlong_as_double((long long)kLogTab[i].rc), __longlong_as_double((long long)kLogTab[i].L));
   const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
   const ushort4* tab = g.tab;
   size_t dyn_off = 0;
@@ -154,7 +154,8 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
   // static tickets, CTA-major then warp then lane: the first electrons go one per warp, spread over all SMs
   uint32_t ticket = (lane * kWarpsPerCta + warp) * gridDim.x + blockIdx.x;
   bool have = false, dvalid = false;
-  double x = 0, y = 0, z = 0, t = 0, vx = 0, vy = 0, vz = 0, Ex = 0, Ey = 0, Ez = 0, dt = 0, u2 = 0;
+  double x = 0, y = 0, z = 0, t = 0, vx = 0, vy = 0, vz = 0, Ex = 0, Ey = 0, Ez = 0, dt = 0;
+  uint2 u2w = make_uint2(0u, 0u);
   uint64_t id = 0;
   uint32_t n = 0, slot = 0;
   uint32_t c_real = 0, c_l0 = 0, c_over = 0;      // tallies kept per thread; null counts are derived (finalize_kernel)
@@ -196,7 +197,7 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
     if (pend) {
       double loss;
       int st;
-      const int l = collision_step(g, s_type, s_loss, s_recoil, s_w, seed, id, n, pc, have_d, dd, vx, vy, vz, st, spawn, ch, loss);
+      const int l = collision_step(g, s_lv, K, id, n, pc, have_d, dd, vx, vy, vz, st, spawn, ch, loss);
       if (st) fin = st;
       if (TALLY) {
         ++c_real;
@@ -220,7 +221,7 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
           __stcg(a.end + c, x); __stcg(a.end + ld + c, y); __stcg(a.end + 2 * ld + c, z); __stcg(a.end + 3 * ld + c, t);
           __stcg(a.end + 4 * ld + c, ch.e);
           __stcg(a.end + 5 * ld + c, ckx); __stcg(a.end + 6 * ld + c, cky); __stcg(a.end + 7 * ld + c, ckz);
-          __stcg(a.id + c, child_id_of(seed, id, n - 1u));
+          __stcg(a.id + c, child_id_of(K, id, n - 1u));
           __stcg(a.aval + c, __ldcg(a.aval + slot));
           __stcg(a.nsteps + c, 0u);
           if (a.birth) {
@@ -319,12 +320,13 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
       }
       __syncwarp();
       // draws of step bn + sidx, and the inclusive sums P of dt over the group's steps 0 .. sidx
-      double P = 0.0, u2j = 0.0;
+      double P = 0.0;
+      uint2 u2j = make_uint2(0u, 0u);
       Deflection dj;
       dj.ct = 1.0; dj.st = 0.0; dj.cphi = 1.0; dj.sphi = 0.0;
       if (alive) {
-        draw_flight(g, seed, id, bn + (uint32_t)sidx, P, u2j);
-        dj = deflection_draws(seed, id, bn + (uint32_t)sidx);
+        draw_flight(g, K, s_logtab, id, bn + (uint32_t)sidx, P, u2j);
+        dj = deflection_draws(K, id, bn + (uint32_t)sidx);
       }
       for (int d = kp; d < 32; d <<= 1) {
         const double up = __shfl_up_sync(0xFFFFFFFFu, P, d);
@@ -335,7 +337,6 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
       const int last = ((gl - 1) << lg) | e;
       double Pb = 0.0;
       int cur = 0, gfin = 0;
-      Ex = f.slab[0].E[0]; Ey = f.slab[0].E[1]; Ez = f.slab[0].E[2];
 #pragma unroll 1
       for (;;) {
         const bool valid = alive && sidx >= cur;
@@ -403,10 +404,11 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
         if (e < k) {
           const uint64_t hid = wb->id[e];
           const uint32_t hn = wb->n[e] + (uint32_t)s;
-          double ddt, du2;
-          draw_flight(g, seed, hid, hn, ddt, du2);
-          const Deflection d = deflection_draws(seed, hid, hn);
-          wb->dt[lane] = ddt; wb->u2[lane] = du2;
+          double ddt;
+          uint2 du2;
+          draw_flight(g, K, s_logtab, hid, hn, ddt, du2);
+          const Deflection d = deflection_draws(K, hid, hn);
+          wb->dt[lane] = ddt; wb->u2w[lane] = du2;
           wb->ct[lane] = d.ct; wb->st[lane] = d.st; wb->cphi[lane] = d.cphi; wb->sphi[lane] = d.sphi;
         }
       }
@@ -426,7 +428,7 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
           const int b = advance<UNIFORM1, HASB>(g, f, t_max, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, wb->dt[idx], over);
           if (b < 0) fin = -b;
           else {
-            const int r = decide(g, tab[b], b, wb->u2[idx], pc.xr);
+            const int r = decide(g, tab[b], b, wb->u2w[idx], pc.xr);
             if (r >= 0) {
               pend = true; pc.lsel = r; pc.bin = b;
               dd.ct = wb->ct[idx]; dd.st = wb->st[idx]; dd.cphi = wb->cphi[idx]; dd.sphi = wb->sphi[idx];
@@ -440,7 +442,7 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
       }
     } else {
       // ---- full warp ----
-      if (have && !dvalid) { draw_flight(g, seed, id, n, dt, u2); dvalid = true; }
+      if (have && !dvalid) { draw_flight(g, K, s_logtab, id, n, dt, u2w); dvalid = true; }
       int fin = 0;
       bool pend = false;
       Pending pc;
@@ -453,8 +455,8 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
           if (b < 0) fin = -b;
           else {
             const ushort4 rec = tab[b];
-            const double u2c = u2;
-            draw_flight(g, seed, id, n, dt, u2);    // next flight's draws: independent of the record load
+            const uint2 u2c = u2w;
+            draw_flight(g, K, s_logtab, id, n, dt, u2w);    // next flight's draws: independent of the record load
             const int r = decide(g, rec, b, u2c, pc.xr);
             if (r >= 0) { pend = true; pc.lsel = r; pc.bin = b; }
             if (TALLY && over) ++c_over;
@@ -618,6 +620,13 @@ __global__ void step_batch_kernel(const __grid_constant__ DevGas g, const __grid
                                   const uint32_t* __restrict__ n_idx, double* __restrict__ out,
                                   int32_t* __restrict__ event, int32_t* __restrict__ status, int32_t* __restrict__ bin,
                                   double* __restrict__ child, uint64_t* __restrict__ child_id) {
+  __shared__ LevelPar s_lv[AVM_MAX_LEVELS];
+  __shared__ double2 s_logtab[128];
+  stage_levels(g, s_lv);
+  for (int j = threadIdx.x; j < 128; j += blockDim.x)
+    s_logtab[j] = make_double2(__longlong_as_double((long long)kLogTab[j].rc), __longlong_as_double((long long)kLogTab[j].L));
+  __syncthreads();
+  const PhiloxKeys K = philox_keys(seed);
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   double x = in[i], y = in[n + i], z = in[2 * n + i], t = in[3 * n + i];
@@ -635,8 +644,9 @@ __global__ void step_batch_kernel(const __grid_constant__ DevGas g, const __grid
     return;
   }
   const double sp = kC2 * sqrt(e);
-  double vx = sp * kx, vy = sp * ky, vz = sp * kz, dt, u2;
-  draw_flight(g, seed, id, nn, dt, u2);
+  double vx = sp * kx, vy = sp * ky, vz = sp * kz, dt;
+  uint2 u2;
+  draw_flight(g, K, s_logtab, id, nn, dt, u2);
   Pending pc;
   pc.lsel = 0; pc.bin = -1; pc.xr = 0.0;
   bool over = false, spawn = false;
@@ -654,7 +664,7 @@ __global__ void step_batch_kernel(const __grid_constant__ DevGas g, const __grid
       pc.lsel = r;
       Deflection dd;
       dd.ct = 1.0; dd.st = 0.0; dd.cphi = 1.0; dd.sphi = 0.0;
-      ev = collision_step(g, g.type, g.loss, g.recoil, g.w, seed, id, nn, pc, false, dd, vx, vy, vz, st, spawn, ch, loss);
+      ev = collision_step(g, s_lv, K, id, nn, pc, false, dd, vx, vy, vz, st, spawn, ch, loss);
     }
   }
   // state after the step in (energy, direction) form
@@ -669,7 +679,7 @@ __global__ void step_batch_kernel(const __grid_constant__ DevGas g, const __grid
     child_direction(ch.u6, ch.u7, ckx, cky, ckz);
     child[i] = x; child[n + i] = y; child[2 * n + i] = z; child[3 * n + i] = t; child[4 * n + i] = ch.e;
     child[5 * n + i] = ckx; child[6 * n + i] = cky; child[7 * n + i] = ckz;
-    child_id[i] = child_id_of(seed, id, nn - 1u);
+    child_id[i] = child_id_of(K, id, nn - 1u);
   }
 }
 
@@ -687,7 +697,7 @@ __global__ void philox_batch_kernel(const uint64_t seed, const int64_t n, const 
                                     uint32_t* __restrict__ words, double* __restrict__ u) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
-  const U4 w = philox(seed, id[i], n_idx[i], block[i]);
+  const U4 w = philox(philox_keys(seed), id[i], n_idx[i], block[i]);
   words[4 * i] = w.w0; words[4 * i + 1] = w.w1; words[4 * i + 2] = w.w2; words[4 * i + 3] = w.w3;
   u[2 * i] = to_unit(w.w0, w.w1); u[2 * i + 1] = to_unit(w.w2, w.w3);
 }
@@ -870,6 +880,10 @@ int32_t avm_gas_create(avm_ctx* ctx, const avm_gas_desc* d, void* dev_buf, size_
   g->nu_hat = d->nu_hat > 0.0 ? d->nu_hat : mx;
   g->d.nb = nb; g->d.L = L;
   g->d.inv_de = (double)nb / d->e_max_eV;
+  {
+    const double fb = kEpsFloor * g->d.inv_de;
+    g->d.bin_floor = fb >= (double)(nb - 1) ? nb - 1 : (int)fb;
+  }
   g->d.nu_hat = g->nu_hat;
   g->d.inv_nu_hat = 1.0 / g->nu_hat;
   g->d.nu_tot = (const double*)(base + lay.nu_tot);
@@ -946,6 +960,22 @@ int32_t avm_field_create(avm_ctx* ctx, const avm_field_desc* d, avm_field** out)
     F.inv_omega = 1.0 / F.omega;
   }
   f->uniform1 = d->n_slabs == 1 && d->slabs[0].kind == 0;
+  F.xy_bounded = 0;
+  for (int a = 0; a < 2; ++a)
+    if (std::isfinite(F.xy_lo[a]) || std::isfinite(F.xy_hi[a]) || F.xy_lo[a] != F.xy_lo[a] || F.xy_hi[a] != F.xy_hi[a]) F.xy_bounded = 1;
+  {
+    // constants of the flight in slab 0 (used when the field is one uniform slab), same formulas as flight<>
+    const double* E = F.slab[0].E;
+    for (int a = 0; a < 3; ++a) { F.ua[a] = -kKappa * E[a]; F.uvd[a] = 0.0; F.uap[a] = 0.0; }
+    if (F.has_B) {
+      const double a_b = F.ua[0] * F.bh[0] + F.ua[1] * F.bh[1] + F.ua[2] * F.bh[2];
+      const double sc = kExBUnit / F.Bn2;
+      F.uvd[0] = sc * (E[1] * F.B[2] - E[2] * F.B[1]);
+      F.uvd[1] = sc * (E[2] * F.B[0] - E[0] * F.B[2]);
+      F.uvd[2] = sc * (E[0] * F.B[1] - E[1] * F.B[0]);
+      for (int a = 0; a < 3; ++a) F.uap[a] = a_b * F.bh[a];
+    }
+  }
   *out = f;
   return AVM_OK;
 }
@@ -982,7 +1012,7 @@ int32_t avm_run_transport_ms(const avm_ctx* c, float* ms_out) {
 }  // extern "C"
 
 namespace {
-typedef void (*TransportFn)(const DevGas, const DevField, const RunArrays, RunCtl*, const uint64_t, const double,
+typedef void (*TransportFn)(const DevGas, const DevField, const RunArrays, RunCtl*, const PhiloxKeys, const double,
                             const uint32_t, const uint32_t);
 template <bool U, bool B>
 TransportFn pick2(bool tally, bool smemtab) {
@@ -1064,7 +1094,7 @@ int32_t avm_run(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, const 
       ctx->transport_ms += ms;
     }
     AVM_CUDA(cudaEventRecord(ctx->ev_t0, st));
-    fn<<<grid, kThreads, dyn_smem, st>>>(gas->d, field->d, a, ctl, opts->seed, opts->t_max, max_iters, n_static);
+    fn<<<grid, kThreads, dyn_smem, st>>>(gas->d, field->d, a, ctl, philox_keys(opts->seed), opts->t_max, max_iters, n_static);
     AVM_CUDA(cudaGetLastError());
     AVM_CUDA(cudaEventRecord(ctx->ev_t1, st));
     ctx->n_kernel_launches++; ctx->n_transport_launches++;

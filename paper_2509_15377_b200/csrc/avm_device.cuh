@@ -22,6 +22,7 @@ constexpr uint32_t kStepLimit = 0xFFFFFFF0u;
 // ---- device-resident descriptions (passed by value as __grid_constant__ kernel parameters) -------------
 struct DevGas {
   int nb, L;
+  int bin_floor;          // (int)(eps_floor * inv_de): the bin of the energy floor (0 for any sensible table)
   double inv_de, nu_hat, inv_nu_hat;
   const double* nu_tot;   // [nb]      total real-collision rate per bin (= cum[b][L-1])
   const double2* head;    // [nb][2]   exact decision record, 32 B: (nu_tot, cum[b][0]), (cum[b][min(1,L-1)], 0)
@@ -50,37 +51,57 @@ struct DevField {
   double z_lo, z_hi;
   double xy_lo[2], xy_hi[2];
   double B[3], bh[3], Bn2, omega, inv_omega;
+  // one uniform slab (configs 1-3): constants of the flight, computed once by avm_field_create
+  double ua[3];     // a = -kappa E
+  double uvd[3];    // E x B drift velocity
+  double uap[3];    // (a . b) b
+  int xy_bounded;   // any of xy_lo / xy_hi finite
 };
+
+// Philox round keys of the run's seed: k0 + r 0x9E3779B9, k1 + r 0xBB67AE85, r = 0..9.  Passed as a kernel parameter so
+// that they enter the rounds' LOP3 as constant-bank operands.
+struct PhiloxKeys { uint32_t k0[10], k1[10]; };
+
+__host__ __device__ inline PhiloxKeys philox_keys(uint64_t seed) {
+  PhiloxKeys K;
+  uint32_t a = (uint32_t)seed, b = (uint32_t)(seed >> 32);
+  for (int r = 0; r < 10; ++r) { K.k0[r] = a; K.k1[r] = b; a += 0x9E3779B9u; b += 0xBB67AE85u; }
+  return K;
+}
 
 // ---- Philox4x32-10 (Salmon et al., SC'11) — DESIGN.md §3 "Uniforms" --------------------------------------
 struct U4 { uint32_t w0, w1, w2, w3; };
 
-__device__ __forceinline__ U4 philox(uint64_t seed, uint64_t id, uint32_t n, uint32_t block) {
+__device__ __forceinline__ U4 philox(const PhiloxKeys& K, uint64_t id, uint32_t n, uint32_t block) {
   uint32_t c0 = n, c1 = block, c2 = (uint32_t)id, c3 = (uint32_t)(id >> 32);
-  uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
 #pragma unroll
   for (int r = 0; r < 10; ++r) {
     const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
     const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
-    c0 = hi1 ^ c1 ^ k0; c1 = lo1; c2 = hi0 ^ c3 ^ k1; c3 = lo0;
-    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    c0 = hi1 ^ c1 ^ K.k0[r]; c1 = lo1; c2 = hi0 ^ c3 ^ K.k1[r]; c3 = lo0;
   }
   return U4{c0, c1, c2, c3};
 }
 
 // u = ((x >> 12) + 0.5) * 2^-52 with x = hi:lo — strictly inside (0,1), exactly representable.
 __device__ __forceinline__ double to_unit(uint32_t hi, uint32_t lo) {
-  // Build the double 1.m directly: mantissa = top 52 bits of x, value in [1,2); subtract 1 and add 2^-53.
+  // Build the double 1.m directly: mantissa = top 52 bits of x, value 1 + k 2^-52 in [1,2); subtracting 1 - 2^-53
+  // gives (2k + 1) 2^-53, which has at most 53 significant bits: the subtraction is exact.
   const uint32_t mh = hi >> 12, ml = (hi << 20) | (lo >> 12);
-  const double one_m = __hiloint2double((int)(0x3FF00000u | mh), (int)ml);   // 1 + (x>>12) 2^-52, exact
-  return (one_m - 1.0) + 1.1102230246251565e-16;                            // both steps exact
+  const double one_m = __hiloint2double((int)(0x3FF00000u | mh), (int)ml);
+  return one_m - 0.99999999999999988898;                                     // 1 - 2^-53
 }
 
 // ---- elementary functions specialised to this path's argument ranges ------------------------------------------
 // Coefficients live in constant memory so that they enter DFMA as constant-bank operands (an fp64 immediate costs
 // two UMOVs).  Accuracy: a few ulp, far inside the 1e-12 parity tolerance.
-__constant__ double kAtanhC[10] = {1.0 / 3.0, 1.0 / 5.0, 1.0 / 7.0, 1.0 / 9.0, 1.0 / 11.0, 1.0 / 13.0, 1.0 / 15.0,
-                                   1.0 / 17.0, 1.0 / 19.0, 1.0 / 21.0};
+// log1p(r) = r + r^2 (kLog1pC[0] + kLog1pC[1] r + ...), |r| < 2^-7: the first dropped term is r^9/9 < 2e-18 |r|
+__constant__ double kLog1pC[7] = {-1.0 / 2.0, 1.0 / 3.0, -1.0 / 4.0, 1.0 / 5.0, -1.0 / 6.0, 1.0 / 7.0, -1.0 / 8.0};
+// (rc, L) per 1/128 of the mantissa range — see gen_logtab.py.  Kernels stage it in shared memory.
+struct LogEntry { unsigned long long rc, L; };
+__device__ const LogEntry kLogTab[128] = {
+#include "avm_logtab.inc"
+};
 // sin(r pi/2) = r sum_k kSinC[k] r^2k, cos(r pi/2) = sum_k kCosC[k] r^2k (Taylor; |r| <= 1/2: truncation < 5e-17)
 __constant__ double kSinC[8] = {1.5707963267948966, -0.6459640975062463, 0.07969262624616705, -0.004681754135318688,
                                 0.00016044118478735983, -3.598843235212085e-06, 5.692172921967927e-08,
@@ -99,25 +120,21 @@ __device__ __forceinline__ double rcp_fast(double d) {
 }
 
 // log(u) for u strictly inside (0, 1) and normal (the uniforms of to_unit are >= 2^-53): no special cases.
-// u = m 2^e, m in [sqrt(1/2), sqrt(2)); log m = 2 atanh(q), q = (m - 1)/(m + 1), |q| <= 0.1716.
-__device__ __forceinline__ double log_unit(double u) {
-  int hi = __double2hiint(u);
-  const int lo = __double2loint(u);
-  int e = (hi >> 20) - 1023;
-  hi = (hi & 0x000FFFFF) | 0x3FF00000;
-  if (hi >= 0x3FF6A09F) { hi -= 0x00100000; ++e; }
-  const double m = __hiloint2double(hi, lo);
-  const double f = m - 1.0, d = m + 1.0;
-  const double r = rcp_fast(d);
-  double q = f * r;
-  q = fma(fma(-d, q, f), r, q);
-  const double t = q * q;
-  double p = kAtanhC[9];
+// u = m 2^e, m in [1,2); i = top 7 mantissa bits; reduced argument m' = m (i < 53) or m/2 (e bumped) in [0.707, 1.414);
+// r = m' rc' - 1 by one fma (|r| < 2^-7); log u = e' ln2 + L_i + log1p(r).  ~1 ulp, full relative accuracy as u -> 1.
+// `tab` = kLogTab or its shared-memory copy.
+__device__ __forceinline__ double log_unit(double u, const double2* __restrict__ tab) {
+  const int hi = __double2hiint(u), lo = __double2loint(u);
+  const int e = ((hi + 0x96000) >> 20) - 1023;          // mantissa >= 53/128 carries into the exponent
+  const double m = __hiloint2double((hi & 0x000FFFFF) | 0x3FF00000, lo);
+  const double2 en = tab[(hi >> 13) & 127];
+  const double r = fma(m, en.x, -1.0);
+  double p = kLog1pC[6];
 #pragma unroll
-  for (int k = 8; k >= 0; --k) p = fma(p, t, kAtanhC[k]);
-  const double lm = 2.0 * fma(q * t, p, q);
+  for (int k = 5; k >= 0; --k) p = fma(p, r, kLog1pC[k]);
   const double de = (double)e;
-  return fma(de, 0.6931471805599453, fma(de, 2.3190468138462996e-17, lm));
+  const double l1 = fma(r * r, p, r);
+  return fma(de, 0.693147180369123816490, fma(de, 1.90821492927058770002e-10, en.y + l1));
 }
 
 // (sin, cos)(2 pi u) for u in [0, 1]: quadrant q = rint(4u), r = 4u - q in [-1/2, 1/2] (exact).
@@ -200,13 +217,21 @@ __device__ __forceinline__ bool grid_at(const DevSlab& s, double x, double y, do
 
 // Field and mask at r.  Returns the slab index (>= 0) or -status when r is outside the domain.
 // UNIFORM1 = the field is one uniform slab (configs 1-3): no dispatch, no loads.
+// Slow path of the bounds test: which face was crossed (S5 order: z_lo, z_hi, then x/y; NaN coordinates -> 3).
+__device__ __forceinline__ int outside_status(const DevField& f, double x, double y, double z) {
+  if (z < f.z_lo) return -AVM_LEFT_ZLO;
+  if (z > f.z_hi) return -AVM_LEFT_ZHI;
+  return -AVM_LEFT_XY;
+}
+
 template <bool UNIFORM1>
 __device__ __forceinline__ int field_at(const DevField& f, double x, double y, double z, double& Ex, double& Ey,
                                         double& Ez, double& mask) {
-  if (z < f.z_lo) return -AVM_LEFT_ZLO;
-  if (z > f.z_hi) return -AVM_LEFT_ZHI;
-  // written so that NaN coordinates fail the test (status 3), like the oracle
-  if (!(x >= f.xy_lo[0] && x <= f.xy_hi[0] && y >= f.xy_lo[1] && y <= f.xy_hi[1] && z == z)) return -AVM_LEFT_XY;
+  // written so that NaN coordinates fail the test, like the oracle
+  bool in = (z >= f.z_lo) & (z <= f.z_hi);
+  if (f.xy_bounded) in = in & (x >= f.xy_lo[0]) & (x <= f.xy_hi[0]) & (y >= f.xy_lo[1]) & (y <= f.xy_hi[1]);
+  else in = in & ((x + y) == (x + y));
+  if (!in) return outside_status(f, x, y, z);
   if (UNIFORM1) {
     Ex = f.slab[0].E[0]; Ey = f.slab[0].E[1]; Ez = f.slab[0].E[2]; mask = 1.0;
     return 0;
@@ -220,24 +245,32 @@ __device__ __forceinline__ int field_at(const DevField& f, double x, double y, d
 }
 
 // ---- S2-S3: free flight of duration dt in constant E (and B) from (r, v) ---------------------------------
-template <bool HASB>
+// UNIFORM1: E is the run constant of slab 0 and the arguments Ex, Ey, Ez are ignored (a, E x B drift and a-parallel
+// come precomputed from DevField).
+template <bool UNIFORM1, bool HASB>
 __device__ __forceinline__ void flight(const DevField& f, double Ex, double Ey, double Ez, double dt, double& x,
                                        double& y, double& z, double& vx, double& vy, double& vz) {
-  const double ax = -kKappa * Ex, ay = -kKappa * Ey, az = -kKappa * Ez;
+  const double ax = UNIFORM1 ? f.ua[0] : -kKappa * Ex, ay = UNIFORM1 ? f.ua[1] : -kKappa * Ey,
+               az = UNIFORM1 ? f.ua[2] : -kKappa * Ez;
   if (!HASB) {
     const double h = 0.5 * dt * dt;
     x = (x + vx * dt) + ax * h; y = (y + vy * dt) + ay * h; z = (z + vz * dt) + az * h;
     vx = vx + ax * dt; vy = vy + ay * dt; vz = vz + az * dt;
   } else {
     const double bx = f.bh[0], by = f.bh[1], bz = f.bh[2];
-    const double a_b = ax * bx + ay * by + az * bz;
     const double v_b = vx * bx + vy * by + vz * bz;
-    const double sc = kExBUnit / f.Bn2;
-    const double dx_ = sc * (Ey * f.B[2] - Ez * f.B[1]);      // E x B drift velocity
-    const double dy_ = sc * (Ez * f.B[0] - Ex * f.B[2]);
-    const double dz_ = sc * (Ex * f.B[1] - Ey * f.B[0]);
+    double dx_, dy_, dz_, qx, qy, qz;
+    if (UNIFORM1) {
+      dx_ = f.uvd[0]; dy_ = f.uvd[1]; dz_ = f.uvd[2]; qx = f.uap[0]; qy = f.uap[1]; qz = f.uap[2];
+    } else {
+      const double a_b = ax * bx + ay * by + az * bz;
+      const double sc = kExBUnit / f.Bn2;
+      dx_ = sc * (Ey * f.B[2] - Ez * f.B[1]);                  // E x B drift velocity
+      dy_ = sc * (Ez * f.B[0] - Ex * f.B[2]);
+      dz_ = sc * (Ex * f.B[1] - Ey * f.B[0]);
+      qx = a_b * bx; qy = a_b * by; qz = a_b * bz;             // a parallel
+    }
     const double px = v_b * bx, py = v_b * by, pz = v_b * bz;  // v parallel
-    const double qx = a_b * bx, qy = a_b * by, qz = a_b * bz;  // a parallel
     const double wx = vx - px - dx_, wy = vy - py - dy_, wz = vz - pz - dz_;
     const double cx = by * wz - bz * wy, cy = bz * wx - bx * wz, cz = bx * wy - by * wx;   // b x w0
     const double th = f.omega * dt;
@@ -257,113 +290,101 @@ __device__ __forceinline__ void flight(const DevField& f, double Ex, double Ey, 
 // ---- S9: collision outcome ------------------------------------------------------------------------------
 struct Child { double e, u6, u7; };   // secondary: energy and the two uniforms of its isotropic direction
 
-// S9d: rotate unit vector k by polar (ct, st) and azimuth (cphi, sphi) about itself (Duff et al. 2017 basis).
-__device__ __forceinline__ void deflect(double& kx, double& ky, double& kz, double ct, double st, double cphi,
-                                        double sphi) {
-  const double sg = copysign(1.0, kz);
-  const double A = -rcp_fast(sg + kz);
-  const double Bq = kx * ky * A;
-  const double b1x = 1.0 + sg * kx * kx * A, b1y = sg * Bq, b1z = -sg * kx;
-  const double b2x = Bq, b2y = sg + ky * ky * A, b2z = -ky;
-  const double nx = ct * kx + st * (cphi * b1x + sphi * b2x);
-  const double ny = ct * ky + st * (cphi * b1y + sphi * b2y);
-  const double nz = ct * kz + st * (cphi * b1z + sphi * b2z);
-  // |k''|^2 = 1 + d with |d| ~ 1e-15 (unit k, orthonormal basis, ct^2 + st^2 = 1): 1/sqrt(1+d) = 1 - d/2 + O(d^2)
-  const double inv = fma(-0.5, fma(nx, nx, fma(ny, ny, nz * nz)), 1.5);
-  kx = nx * inv; ky = ny * inv; kz = nz * inv;
+// Level parameters as the kernels keep them in shared memory: two 16-byte loads per collision.
+struct __align__(16) LevelPar { double loss, recoil, w; int type, pad; };
+
+__device__ __forceinline__ void stage_levels(const DevGas& g, LevelPar* s_lv) {
+  for (int l = threadIdx.x; l < AVM_MAX_LEVELS; l += blockDim.x) {
+    const bool in = l < g.L;
+    LevelPar p;
+    p.loss = in ? g.loss[l] : 0.0; p.recoil = in ? g.recoil[l] : 0.0; p.w = in ? g.w[l] : 1.0;
+    p.type = in ? g.type[l] : 0; p.pad = 0;
+    s_lv[l] = p;
+  }
+}
+
+// 1/sqrt(a) for normal a > 0 (MUFU.RSQ64H seed, one third-order step): ~1 ulp.
+__device__ __forceinline__ double rsqrt_fast(double a) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
+  const double e = fma(-a, y * y, 1.0);
+  return fma(fma(e, 0.375, 0.5), y * e, y);
+}
+// sqrt(a) for normal a > 0: a / sqrt(a) with one correction step.
+__device__ __forceinline__ double sqrt_fast(double a) {
+  const double y = rsqrt_fast(a);
+  const double r = a * y;
+  return fma(fma(-r, r, a), 0.5 * y, r);
+}
+// x with its sign flipped when sbit = 0x80000000 (sbit = 0: unchanged): the product x * (+-1) on the integer pipe.
+__device__ __forceinline__ double xor_sign(double x, int sbit) {
+  return __hiloint2double(__double2hiint(x) ^ sbit, __double2loint(x));
 }
 
 __device__ __forceinline__ void child_direction(double u6, double u7, double& kx, double& ky, double& kz) {
-  const double sc = 2.0 * sqrt(u6 * (1.0 - u6));
+  const double sc = 2.0 * sqrt_fast(u6 * (1.0 - u6));
   double s, c;
   sincos_2pi(u7, s, c);
   kx = sc * c; ky = sc * s; kz = 1.0 - 2.0 * u6;
 }
 
-__device__ __forceinline__ uint64_t child_id_of(uint64_t seed, uint64_t id, uint32_t n_s) {
-  const U4 w = philox(seed, id, n_s, kBlockChildId);
+__device__ __forceinline__ uint64_t child_id_of(const PhiloxKeys& K, uint64_t id, uint32_t n_s) {
+  const U4 w = philox(K, id, n_s, kBlockChildId);
   return (uint64_t)w.w0 | ((uint64_t)w.w1 << 32);
 }
 
 // S9b: the deflection draws of step n_s — block 1 -> (cos theta, sin theta, cos phi, sin phi).  They depend on
-// (id, n_s) only, so idle lanes can prepare them ahead of the decision (transport kernel, cooperative batches).
+// (id, n_s) only, so idle lanes can prepare them ahead of the decision (transport kernel, batches).
 struct Deflection { double ct, st, cphi, sphi; };
 
-__device__ __forceinline__ Deflection deflection_draws(uint64_t seed, uint64_t id, uint32_t n_s) {
-  const U4 r1 = philox(seed, id, n_s, 1u);
+__device__ __forceinline__ Deflection deflection_draws(const PhiloxKeys& K, uint64_t id, uint32_t n_s) {
+  const U4 r1 = philox(K, id, n_s, 1u);
   const double u3 = to_unit(r1.w0, r1.w1), u4 = to_unit(r1.w2, r1.w3);
   Deflection d;
   d.ct = 1.0 - 2.0 * u3;
-  d.st = 2.0 * sqrt(u3 * (1.0 - u3));
+  d.st = 2.0 * sqrt_fast(u3 * (1.0 - u3));        // u3 (1 - u3) >= 2^-54: normal
   sincos_2pi(u4, d.sphi, d.cphi);
   return d;
 }
 
-// Real collision of level l at energy e1, direction k (unit), deflection d.  type/loss/recoil/w are the level's
-// parameters.  Returns the new energy; updates k; fills `ch` and returns spawn=true for an ionisation.  *loss_out =
-// energy leaving the electron population (tally).  Attachment is handled by the caller (S9a).
-__device__ __forceinline__ double collide(uint64_t seed, uint64_t id, uint32_t n_s, int type, double lv_loss,
-                                          double lv_recoil, double lv_w, double e1, const Deflection& d, double& kx,
-                                          double& ky, double& kz, bool& spawn, Child& ch, double& loss_out) {
-  double e2;
-  spawn = false;
-  if (type == AVM_ELASTIC) {
-    e2 = e1 * (1.0 - lv_recoil * (1.0 - d.ct));
-    loss_out = e1 - e2;
-  } else if (type == AVM_EXCITATION) {
-    e2 = fmax(e1 - lv_loss, kEpsFloor);
-    loss_out = e1 - e2;
-  } else {   // ionisation: Opal-Peterson-Beaty sharing (R10)
-    const U4 r2 = philox(seed, id, n_s, 2u);
-    const U4 r3 = philox(seed, id, n_s, 3u);
-    const double u5 = to_unit(r2.w0, r2.w1);
-    ch.u6 = to_unit(r2.w2, r2.w3);
-    ch.u7 = to_unit(r3.w0, r3.w1);
-    const double ea = fmax(e1 - lv_loss, 0.0);
-    const double es = lv_w * tan(u5 * atan(ea / (2.0 * lv_w)));
-    e2 = fmax(ea - es, kEpsFloor);
-    ch.e = fmax(es, kEpsFloor);
-    spawn = true;
-    loss_out = e1 - e2 - ch.e;
-  }
-  deflect(kx, ky, kz, d.ct, d.st, d.cphi, d.sphi);
-  return e2;
-}
-
-// S8 for the rare levels: smallest l >= 2 with cum[b][l] > x (x < cum[b][L-1] is known; levels 0 and 1 are
-// decided from the head record).
+// S8 for the rare levels: smallest l >= 2 with cum[b][l] > x (x < cum[b][L-1] is known; levels 0 and 1 are decided
+// from the head record).  The row is non-decreasing, so l = 2 + #{2 <= j < L-1 : cum[b][j] <= x}: independent loads,
+// one memory round trip instead of a dependent scan.
 __device__ __forceinline__ int select_level_from2(const DevGas& g, int b, double xr) {
   const double* row = g.cum + (size_t)b * g.L;
   int l = 2;
-  while (l < g.L - 1 && __ldg(row + l) <= xr) ++l;
+#pragma unroll 8
+  for (int j = 2; j < g.L - 1; ++j) l += (__ldg(row + j) <= xr) ? 1 : 0;
   return l;
 }
 
 // ---- one step, split at the null/real decision ----------------------------------------------------------------
-// Electron state is kept in velocity form (r, t, v, id, n).  The draws of a flight (dt, u2) depend on (id, n) only and
-// are prepared ahead of the flight that uses them — by the lane itself one step ahead, or by the idle lanes of its warp
-// a whole batch ahead (transport kernel).
+// Electron state is kept in velocity form (r, t, v, id, n).  The draws of a flight depend on (id, n) only and are
+// prepared ahead of the flight that uses them — by the lane itself one step ahead, or by the idle lanes of its warp a
+// whole batch ahead (transport kernel).  u2 travels as its raw Philox words (w2, w3): the decision needs only their
+// top 16 bits, the double is built in the rare exact path.
 struct Pending { int lsel, bin; double xr; };   // lsel: 0 / 1 = level decided from the head record, 2 = scan the row
 
-__device__ __forceinline__ void draw_flight(const DevGas& g, uint64_t seed, uint64_t id, uint32_t n, double& dt,
-                                            double& u2) {
-  const U4 r0 = philox(seed, id, n, 0u);                                        // S1
-  dt = -log_unit(to_unit(r0.w0, r0.w1)) * g.inv_nu_hat;                         // S2
-  u2 = to_unit(r0.w2, r0.w3);
+__device__ __forceinline__ void draw_flight(const DevGas& g, const PhiloxKeys& K, const double2* __restrict__ logtab,
+                                            uint64_t id, uint32_t n, double& dt, uint2& u2w) {
+  const U4 r0 = philox(K, id, n, 0u);                                           // S1
+  dt = -log_unit(to_unit(r0.w0, r0.w1), logtab) * g.inv_nu_hat;                 // S2
+  u2w = make_uint2(r0.w2, r0.w3);
 }
 
-// S7 + the common part of S8 for bin b and uniform u2: -1 = null collision, 0 / 1 = level 0 / 1, 2 = a level >= 2
-// (p.xr is then needed for the row scan).  `rec` = tab[b] holds q = floor(c 2^16) for c = (nu_tot, cum0, cum1)/nu_hat;
-// with h = floor(u2 2^16): h >= q + 2 implies u2 nu_hat >= cum and h <= q - 2 implies u2 nu_hat < cum with a margin of
-// nu_hat 2^-16, far above the rounding of the fp64 product — so the 16-bit filter takes the oracle's decision exactly,
-// and the 2e-4 of the steps that fall inside a band are decided from the exact fp64 record.
-__device__ __forceinline__ int decide(const DevGas& g, const ushort4 rec, int b, double u2, double& xr) {
-  const uint32_t h = (uint32_t)__double2int_rz(u2 * 65536.0);     // exact: top 16 bits of the uniform
+// S7 + the common part of S8 for bin b and uniform u2 = to_unit(u2w): -1 = null collision, 0 / 1 = level 0 / 1, 2 = a
+// level >= 2 (xr = u2 nu_hat is then set for the row scan).  `rec` = tab[b] holds q = floor(c 2^16) for c = (nu_tot,
+// cum0, cum1)/nu_hat; h = floor(u2 2^16) = w2 >> 16 exactly (u2 = ((x >> 12) + 1/2) 2^-52, x = w2:w3).  h >= q + 2 implies
+// u2 nu_hat >= cum and h <= q - 2 implies u2 nu_hat < cum with a margin of nu_hat 2^-16, far above the rounding of the
+// fp64 product — so the 16-bit filter takes the oracle's decision exactly, and the 2e-4 of the steps that fall inside a
+// band are decided from the exact fp64 record.
+__device__ __forceinline__ int decide(const DevGas& g, const ushort4 rec, int b, uint2 u2w, double& xr) {
+  const uint32_t h = u2w.x >> 16;
   const uint32_t qt = rec.x, q0 = rec.y, q1 = rec.z;
-  xr = u2 * g.nu_hat;
   if (h >= qt + 2u) return -1;
   if (h + 2u <= q0) return 0;
   if (h >= q0 + 2u && h + 2u <= q1) return 1;
+  xr = to_unit(u2w.x, u2w.y) * g.nu_hat;
   if (h >= q1 + 2u && h + 2u <= qt) return 2;
   const double2 h0 = __ldg(g.head + 2 * (size_t)b), h1 = __ldg(g.head + 2 * (size_t)b + 1);
   if (xr >= h0.x) return -1;
@@ -375,41 +396,89 @@ template <bool UNIFORM1, bool HASB>
 __device__ __forceinline__ int advance(const DevGas& g, const DevField& f, double t_max, uint32_t& n, double& x,
                                        double& y, double& z, double& t, double& vx, double& vy, double& vz, double& Ex,
                                        double& Ey, double& Ez, double dt, bool& overflow) {
-  flight<HASB>(f, Ex, Ey, Ez, dt, x, y, z, vx, vy, vz);     // S3
-  const double s2 = vx * vx + vy * vy + vz * vz;            // S4
-  const double e1 = fmax(s2 * kInvC2Sq, kEpsFloor);
+  flight<UNIFORM1, HASB>(f, Ex, Ey, Ez, dt, x, y, z, vx, vy, vz);     // S3
+  const double s2 = vx * vx + vy * vy + vz * vz;                      // S4
   t = t + dt;
   n = n + 1u;
-  double mask;                                              // S5
-  const int si = field_at<UNIFORM1>(f, x, y, z, Ex, Ey, Ez, mask);
-  if (si < 0) return si;
-  if (mask < 0.5) return -AVM_MATERIAL;
-  if (t > t_max) return -AVM_TIME_LIMIT;
-  if (n >= kStepLimit) return -AVM_STEP_LIMIT;
-  const double sb = e1 * g.inv_de;                          // S6
-  overflow = sb >= (double)g.nb;
-  return overflow ? g.nb - 1 : (int)sb;
+  if (UNIFORM1) {                                                     // S5: one test on the common path
+    bool ok = (z >= f.z_lo) & (z <= f.z_hi) & (t <= t_max) & (n < kStepLimit);
+    if (f.xy_bounded) ok = ok & (x >= f.xy_lo[0]) & (x <= f.xy_hi[0]) & (y >= f.xy_lo[1]) & (y <= f.xy_hi[1]);
+    else ok = ok & ((x + y) == (x + y));
+    if (!ok) {
+      const bool in = (z >= f.z_lo) & (z <= f.z_hi) & (x >= f.xy_lo[0]) & (x <= f.xy_hi[0]) & (y >= f.xy_lo[1]) &
+                      (y <= f.xy_hi[1]);
+      if (!in) return outside_status(f, x, y, z);
+      return t > t_max ? -AVM_TIME_LIMIT : -AVM_STEP_LIMIT;
+    }
+  } else {
+    double mask;
+    const int si = field_at<UNIFORM1>(f, x, y, z, Ex, Ey, Ez, mask);
+    if (si < 0) return si;
+    if (mask < 0.5) return -AVM_MATERIAL;
+    if (t > t_max) return -AVM_TIME_LIMIT;
+    if (n >= kStepLimit) return -AVM_STEP_LIMIT;
+  }
+  // S6.  eps' = max(s2 inv_c2sq, eps_floor) and b = min(nb - 1, (int)(eps' inv_de)); the floor is applied to the bin
+  // (monotone: (int)(max(e, fl) c) = max((int)(e c), (int)(fl c))), the clamp after a saturating conversion.
+  const int braw = __double2int_rz((s2 * kInvC2Sq) * g.inv_de);
+  overflow = braw >= g.nb;
+  return max(min(braw, g.nb - 1), g.bin_floor);
 }
 
 // S8-S9 for an electron with a pending real collision (n already incremented by the flight).  Returns the level;
 // status = AVM_ATTACHED for an attachment, else 0 and v is the velocity after the collision.  d = deflection_draws of
 // step n - 1 when `have_d`, else drawn here.
-__device__ __forceinline__ int collision_step(const DevGas& g, const uint8_t* lv_type, const double* lv_loss,
-                                              const double* lv_recoil, const double* lv_w, uint64_t seed, uint64_t id,
-                                              uint32_t n, const Pending& p, bool have_d, Deflection d, double& vx,
-                                              double& vy, double& vz, int& status, bool& spawn, Child& ch, double& loss) {
+// S9d in velocity form: with s = |v'|, sg = sign(v'z), A = -1/(sg s + v'z), the Duff et al. basis about k' = v'/s scaled
+// by s is  s e1 = (s + sg v'x^2 A, sg v'x v'y A, -sg v'x),  s e2 = (v'x v'y A, sg s + v'y^2 A, -v'y),  so that
+// v'' = (speed''/s) [cos(theta) v' + sin(theta) (cos(phi) s e1 + sin(phi) s e2)] without normalising k' first.
+__device__ __forceinline__ int collision_step(const DevGas& g, const LevelPar* __restrict__ lv, const PhiloxKeys& K,
+                                              uint64_t id, uint32_t n, const Pending& p, bool have_d, Deflection d,
+                                              double& vx, double& vy, double& vz, int& status, bool& spawn, Child& ch,
+                                              double& loss) {
   const int l = p.lsel < 2 ? p.lsel : select_level_from2(g, p.bin, p.xr);     // S8
-  const int type = lv_type[l];
+  const LevelPar par = lv[l];
   status = 0; spawn = false; loss = 0.0;
-  if (type == AVM_ATTACHMENT) { status = AVM_ATTACHED; return l; }             // S9a
-  if (!have_d) d = deflection_draws(seed, id, n - 1u);                         // S9b
-  const double s2 = vx * vx + vy * vy + vz * vz;
-  const double e1 = fmax(s2 * kInvC2Sq, kEpsFloor);
-  double kx = 0.0, ky = 0.0, kz = 1.0;
-  if (s2 > 0.0) { const double inv = rsqrt(s2); kx = vx * inv; ky = vy * inv; kz = vz * inv; }
-  const double e2 = collide(seed, id, n - 1u, type, lv_loss[l], lv_recoil[l], lv_w[l], e1, d, kx, ky, kz, spawn, ch, loss);
-  const double sp = kC2 * sqrt(e2);
-  vx = sp * kx; vy = sp * ky; vz = sp * kz;
+  if (par.type == AVM_ATTACHMENT) { status = AVM_ATTACHED; return l; }         // S9a
+  if (!have_d) d = deflection_draws(K, id, n - 1u);                            // S9b
+  double s2 = vx * vx + vy * vy + vz * vz;
+  if (!(s2 >= 1e-280)) {                          // v' = 0 (never in practice): direction +z, energy at the floor
+    vx = 0.0; vy = 0.0; vz = kC2 * 1e-5; s2 = vz * vz;
+  }
+  double e1 = s2 * kInvC2Sq;
+  if (e1 < kEpsFloor) e1 = kEpsFloor;
+  double e2;                                                                    // S9c
+  if (par.type == AVM_ELASTIC) {
+    e2 = e1 * (1.0 - par.recoil * (1.0 - d.ct));
+    loss = e1 - e2;
+  } else if (par.type == AVM_EXCITATION) {
+    e2 = e1 - par.loss;
+    if (!(e2 > kEpsFloor)) e2 = kEpsFloor;
+    loss = e1 - e2;
+  } else {   // ionisation: Opal-Peterson-Beaty sharing (R10)
+    const U4 r2 = philox(K, id, n - 1u, 2u);
+    const U4 r3 = philox(K, id, n - 1u, 3u);
+    const double u5 = to_unit(r2.w0, r2.w1);
+    ch.u6 = to_unit(r2.w2, r2.w3);
+    ch.u7 = to_unit(r3.w0, r3.w1);
+    const double ea = fmax(e1 - par.loss, 0.0);
+    const double es = par.w * tan(u5 * atan(ea / (2.0 * par.w)));
+    e2 = fmax(ea - es, kEpsFloor);
+    ch.e = fmax(es, kEpsFloor);
+    spawn = true;
+    loss = e1 - e2 - ch.e;
+  }
+  const double rs = rsqrt_fast(s2), s = s2 * rs;                               // S9d
+  const int sb = __double2hiint(vz) & 0x80000000;                              // sg = copysign(1, v'z)
+  const double sgs = xor_sign(s, sb);
+  const double A = -rcp_fast(sgs + vz);
+  const double Bq = vx * vy * A;
+  const double b1x = fma(xor_sign(vx * vx, sb), A, s), b1y = xor_sign(Bq, sb), b1z = xor_sign(vx, sb ^ 0x80000000);
+  const double b2x = Bq, b2y = fma(vy * vy, A, sgs), b2z = -vy;
+  const double rx = fma(d.ct, vx, d.st * fma(d.cphi, b1x, d.sphi * b2x));
+  const double ry = fma(d.ct, vy, d.st * fma(d.cphi, b1y, d.sphi * b2y));
+  const double rz = fma(d.ct, vz, d.st * fma(d.cphi, b1z, d.sphi * b2z));
+  const double ratio = (kC2 * sqrt_fast(e2)) * rs;                             // speed'' / s
+  vx = rx * ratio; vy = ry * ratio; vz = rz * ratio;
   return l;
 }
 
