@@ -39,7 +39,7 @@ int32_t fail(int32_t code, const std::string& msg) { g_err = msg; return code; }
 #define AVM_FLIGHTS 2
 #endif
 #ifndef AVM_COOP_MAX
-#define AVM_COOP_MAX 16
+#define AVM_COOP_MAX 8
 #endif
 constexpr int kThreads = AVM_THREADS;        // threads per CTA of the transport kernel
 constexpr int kMinCtasPerSm = AVM_MIN_CTAS;  // one 512-thread CTA per SM: 128 registers per thread, <= 227 KB shared
@@ -769,13 +769,15 @@ bool valid_gas(const avm_gas_desc* d, double* max_rate) {
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct GasLayout { size_t nu_tot, head, tab, cum, loss, recoil, w, type, total; };
+int padded_levels(int L) { return (L + 1) & ~1; }
 GasLayout gas_layout(int nb, int L) {
   GasLayout g;
+  const int Lp = padded_levels(L);
   size_t off = 0;
   g.nu_tot = off; off = align_up(off + sizeof(double) * nb, 256);
   g.head = off;   off = align_up(off + 4 * sizeof(double) * (size_t)nb, 256);
   g.tab = off;    off = align_up(off + sizeof(ushort4) * (size_t)nb, 256);
-  g.cum = off;    off = align_up(off + sizeof(double) * (size_t)nb * L, 256);
+  g.cum = off;    off = align_up(off + sizeof(double) * (size_t)nb * Lp, 256);
   g.loss = off;   off += sizeof(double) * AVM_MAX_LEVELS;
   g.recoil = off; off += sizeof(double) * AVM_MAX_LEVELS;
   g.w = off;      off += sizeof(double) * AVM_MAX_LEVELS;
@@ -866,7 +868,14 @@ int32_t avm_gas_create(avm_ctx* ctx, const avm_gas_desc* d, void* dev_buf, size_
     tab[4 * (size_t)b + 2] = q16(row[L > 1 ? 1 : 0]);
     tab[4 * (size_t)b + 3] = 0;
   }
-  std::memcpy(h.data() + lay.cum, d->cum_rate, sizeof(double) * (size_t)nb * L);
+  {
+    const int Lp = padded_levels(L);
+    double* cum = (double*)(h.data() + lay.cum);
+    for (int b = 0; b < nb; ++b) {
+      for (int l = 0; l < L; ++l) cum[(size_t)b * Lp + l] = d->cum_rate[(size_t)b * L + l];
+      for (int l = L; l < Lp; ++l) cum[(size_t)b * Lp + l] = std::numeric_limits<double>::infinity();
+    }
+  }
   std::memcpy(h.data() + lay.loss, d->level_loss_eV, sizeof(double) * L);
   std::memcpy(h.data() + lay.recoil, d->level_recoil, sizeof(double) * L);
   std::memcpy(h.data() + lay.w, d->level_ob_w_eV, sizeof(double) * L);
@@ -878,7 +887,7 @@ int32_t avm_gas_create(avm_ctx* ctx, const avm_gas_desc* d, void* dev_buf, size_
   if (!g) return fail(AVM_ERR_STATE, "gas_create: out of host memory");
   unsigned char* base = (unsigned char*)dev_buf;
   g->nu_hat = d->nu_hat > 0.0 ? d->nu_hat : mx;
-  g->d.nb = nb; g->d.L = L;
+  g->d.nb = nb; g->d.L = L; g->d.Lp = padded_levels(L);
   g->d.inv_de = (double)nb / d->e_max_eV;
   {
     const double fb = kEpsFloor * g->d.inv_de;

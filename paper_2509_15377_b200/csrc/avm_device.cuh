@@ -22,12 +22,13 @@ constexpr uint32_t kStepLimit = 0xFFFFFFF0u;
 // ---- device-resident descriptions (passed by value as __grid_constant__ kernel parameters) -------------
 struct DevGas {
   int nb, L;
+  int Lp;                 // row stride of `cum`: L rounded up to an even count, pad entries = +inf
   int bin_floor;          // (int)(eps_floor * inv_de): the bin of the energy floor (0 for any sensible table)
   double inv_de, nu_hat, inv_nu_hat;
   const double* nu_tot;   // [nb]      total real-collision rate per bin (= cum[b][L-1])
   const double2* head;    // [nb][2]   exact decision record, 32 B: (nu_tot, cum[b][0]), (cum[b][min(1,L-1)], 0)
   const ushort4* tab;     // [nb]      16-bit thresholds floor(c 2^16), c = (nu_tot, cum0, cum1)/nu_hat: the filter of decide()
-  const double* cum;      // [nb][L]   cumulative rates, row-major by bin
+  const double* cum;      // [nb][Lp]  cumulative rates, row-major by bin, rows 16-byte aligned
   const double* loss;     // [L]
   const double* recoil;   // [L]
   const double* w;        // [L]
@@ -154,6 +155,23 @@ __device__ __forceinline__ void sincos_2pi(double u, double& s, double& c) {
   c = ((q + 1) & 2) ? -cc : cc;
 }
 
+// (sin, cos)(a) for the half rotation angle of a helical flight: |a| <= pi/4 (the common case: omega dt / 2 ~ 1e-2)
+// through the same polynomials, anything larger through the library routine.
+__device__ __forceinline__ void sincos_half_angle(double a, double& s, double& c) {
+  const double r = a * 0.63661977236758134308;      // a / (pi/2)
+  if (fabs(r) <= 0.5) {
+    const double w = r * r;
+    double ps = kSinC[7], pc = kCosC[8];
+#pragma unroll
+    for (int k = 6; k >= 0; --k) ps = fma(ps, w, kSinC[k]);
+#pragma unroll
+    for (int k = 7; k >= 0; --k) pc = fma(pc, w, kCosC[k]);
+    s = ps * r; c = pc;
+  } else {
+    sincos(a, &s, &c);
+  }
+}
+
 // ---- field (S0, R14, R15) -------------------------------------------------------------------------------
 __device__ __forceinline__ double f2d(float v) { return (double)v; }
 
@@ -275,7 +293,7 @@ __device__ __forceinline__ void flight(const DevField& f, double Ex, double Ey, 
     const double cx = by * wz - bz * wy, cy = bz * wx - bx * wz, cz = bx * wy - by * wx;   // b x w0
     const double th = f.omega * dt;
     double sh, ch;
-    sincos(0.5 * th, &sh, &ch);
+    sincos_half_angle(0.5 * th, sh, ch);
     const double sn = 2.0 * sh * ch, vers = 2.0 * sh * sh, cs = 1.0 - vers;
     const double h = 0.5 * dt * dt, io = f.inv_omega;
     x = x + px * dt + qx * h + dx_ * dt + (wx * sn + cx * vers) * io;
@@ -349,13 +367,23 @@ __device__ __forceinline__ Deflection deflection_draws(const PhiloxKeys& K, uint
 
 // S8 for the rare levels: smallest l >= 2 with cum[b][l] > x (x < cum[b][L-1] is known; levels 0 and 1 are decided
 // from the head record).  The row is non-decreasing, so l = 2 + #{2 <= j < L-1 : cum[b][j] <= x}: independent loads,
-// one memory round trip instead of a dependent scan.
+// one memory round trip instead of a dependent scan (rows padded with +inf to an even count: 16-byte loads).
 __device__ __forceinline__ int select_level_from2(const DevGas& g, int b, double xr) {
-  const double* row = g.cum + (size_t)b * g.L;
+  const double2* row = reinterpret_cast<const double2*>(g.cum + (size_t)b * g.Lp) + 1;   // entries 2, 3, ...
+  const int np = (g.Lp - 2) >> 1;
   int l = 2;
-#pragma unroll 8
-  for (int j = 2; j < g.L - 1; ++j) l += (__ldg(row + j) <= xr) ? 1 : 0;
+#pragma unroll 4
+  for (int j = 0; j < np; ++j) {
+    const double2 v = __ldg(row + j);
+    l += ((v.x <= xr) ? 1 : 0) + ((v.y <= xr) ? 1 : 0);
+  }
   return l;
+}
+// Issued when the decision record says "a level >= 2": the row is in L1 by the time the collision phase scans it.
+__device__ __forceinline__ void prefetch_row(const DevGas& g, int b) {
+  const char* row = reinterpret_cast<const char*>(g.cum + (size_t)b * g.Lp);
+  asm volatile("prefetch.global.L1 [%0];" ::"l"(row + 16));
+  asm volatile("prefetch.global.L1 [%0];" ::"l"(row + (size_t)g.Lp * 8 - 8));
 }
 
 // ---- one step, split at the null/real decision ----------------------------------------------------------------
@@ -385,10 +413,13 @@ __device__ __forceinline__ int decide(const DevGas& g, const ushort4 rec, int b,
   if (h + 2u <= q0) return 0;
   if (h >= q0 + 2u && h + 2u <= q1) return 1;
   xr = to_unit(u2w.x, u2w.y) * g.nu_hat;
-  if (h >= q1 + 2u && h + 2u <= qt) return 2;
+  if (h >= q1 + 2u && h + 2u <= qt) { prefetch_row(g, b); return 2; }
   const double2 h0 = __ldg(g.head + 2 * (size_t)b), h1 = __ldg(g.head + 2 * (size_t)b + 1);
   if (xr >= h0.x) return -1;
-  return xr < h0.y ? 0 : (xr < h1.x ? 1 : 2);
+  if (xr < h0.y) return 0;
+  if (xr < h1.x) return 1;
+  prefetch_row(g, b);
+  return 2;
 }
 
 // S3-S6 for one electron with this flight's dt.  Returns the energy bin (>= 0) or -(finishing status).
