@@ -332,7 +332,7 @@ struct Record { Electron el; };
 // The avalanche driver: transport until status != 0, push newly created electrons, repeat.
 // Serial: one electron at a time from a stack.  Order is irrelevant because draws are keyed by (id, n).
 void run_range(const Gas& g, const avmo_field_desc* f, const double* prim, int64_t p0, int64_t p1, uint64_t seed,
-               double t_max, std::vector<Electron>& done, Tally& tl) {
+               uint64_t id_offset, double t_max, std::vector<Electron>& done, Tally& tl) {
   std::vector<Electron> stack;
   StepOut so;
   for (int64_t p = p0; p < p1; ++p) {
@@ -341,7 +341,7 @@ void run_range(const Gas& g, const avmo_field_desc* f, const double* prim, int64
     el.x = q[0]; el.y = q[1]; el.z = q[2]; el.t = q[3]; el.e = std::max(q[4], EPS_FLOOR);
     double nk = std::sqrt(q[5] * q[5] + q[6] * q[6] + q[7] * q[7]);
     if (!(nk > 0)) { el.kx = 0; el.ky = 0; el.kz = 1; } else { el.kx = q[5] / nk; el.ky = q[6] / nk; el.kz = q[7] / nk; }
-    el.id = (uint64_t)p; el.n = 0; el.aval = (uint32_t)p; el.status = AVMO_ACTIVE;
+    el.id = id_offset + (uint64_t)p; el.n = 0; el.aval = (uint32_t)p; el.status = AVMO_ACTIVE;
     el.birth[0] = el.x; el.birth[1] = el.y; el.birth[2] = el.z; el.birth[3] = el.t; el.birth[4] = el.e;
     // a-1: reject out-of-domain primaries (status set, endpoint = birth point)
     double E[3], m;
@@ -424,12 +424,12 @@ int32_t avmo_run(const avmo_gas_desc* gd, const avmo_field_desc* f, const double
   std::vector<Tally> tl(nt);
   for (auto& t : tl) t.level.assign(g.L, 0);
   if (nt == 1) {
-    run_range(g, f, prim, 0, np, opts->seed, opts->t_max, done[0], tl[0]);
+    run_range(g, f, prim, 0, np, opts->seed, opts->id_offset, opts->t_max, done[0], tl[0]);
   } else {                       // timed multi-core baseline only: disjoint primary ranges, identical results
     std::vector<std::thread> th;
     for (int t = 0; t < nt; ++t) {
       int64_t p0 = np * t / nt, p1 = np * (t + 1) / nt;
-      th.emplace_back([&, t, p0, p1] { run_range(g, f, prim, p0, p1, opts->seed, opts->t_max, done[t], tl[t]); });
+      th.emplace_back([&, t, p0, p1] { run_range(g, f, prim, p0, p1, opts->seed, opts->id_offset, opts->t_max, done[t], tl[t]); });
     }
     for (auto& x : th) x.join();
   }

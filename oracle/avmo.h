@@ -51,7 +51,8 @@ typedef struct {
 
 typedef struct { const avmo_slab* slabs; int32_t n_slabs; double B[3]; double xy_lo[2], xy_hi[2]; } avmo_field_desc;
 
-typedef struct { uint64_t seed; double t_max; int32_t n_threads; } avmo_run_opts;
+/* id_offset: primary p gets electron id id_offset + p (shards of one job use disjoint id ranges); avalanche stays p. */
+typedef struct { uint64_t seed; double t_max; int32_t n_threads; uint64_t id_offset; } avmo_run_opts;
 
 typedef struct {
   int64_t capacity;

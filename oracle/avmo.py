@@ -47,7 +47,7 @@ class FieldDescC(C.Structure):
 
 
 class RunOpts(C.Structure):
-    _fields_ = [("seed", C.c_uint64), ("t_max", C.c_double), ("n_threads", C.c_int32)]
+    _fields_ = [("seed", C.c_uint64), ("t_max", C.c_double), ("n_threads", C.c_int32), ("id_offset", C.c_uint64)]
 
 
 class Outputs(C.Structure):
@@ -183,7 +183,8 @@ class RunResult:
                          self.end[:, o], self.per_avalanche, self.tallies_u64, self.tallies_f64, self.rc)
 
 
-def run(gas, field, primaries, seed=0, t_max=float("inf"), capacity=None, n_threads=1, allow_overflow=False) -> RunResult:
+def run(gas, field, primaries, seed=0, t_max=float("inf"), capacity=None, n_threads=1, allow_overflow=False,
+        id_offset=0) -> RunResult:
     prim = np.ascontiguousarray(primaries, dtype=np.float64)
     np_ = prim.shape[0]
     cap = int(capacity if capacity is not None else max(4 * np_, 1 << 16))
@@ -194,7 +195,7 @@ def run(gas, field, primaries, seed=0, t_max=float("inf"), capacity=None, n_thre
     gd, _kg = gas_desc(gas)
     fd, _kf = field_desc(field)
     o = Outputs(cap, _p(ident), _p(av), _p(st), _p(ns), _p(birth), _p(end), _p(pa), _p(tu), _p(tf))
-    opts = RunOpts(int(seed), float(t_max), int(n_threads))
+    opts = RunOpts(int(seed), float(t_max), int(n_threads), int(id_offset))
     n_out = C.c_int64(0)
     rc = lib().avmo_run(C.byref(gd), C.byref(fd), _p(prim), C.c_int64(np_), C.byref(opts), C.byref(o), C.byref(n_out))
     if rc == -2 and not allow_overflow:
