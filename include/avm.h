@@ -117,7 +117,14 @@ int32_t avm_field_eval(avm_ctx*, const avm_field*, int64_t n, const double* r, d
  * Primary p gets id = p + id_offset and avalanche index p; secondaries get id = Philox(n_s, 0xFFFFFFFF, parent
  * id) (R16) and inherit the avalanche index.  A primary outside the domain / inside material is finished at
  * its birth point with the corresponding status. */
-enum { AVM_RUN_PRIMARIES_ON_DEVICE = 1u, AVM_RUN_NO_TALLIES = 2u };
+enum {
+  AVM_RUN_PRIMARIES_ON_DEVICE = 1u,
+  AVM_RUN_NO_TALLIES = 2u,
+  /* Launch shape of the transport kernel.  Default: chosen from n_primaries (wide when the primaries alone outnumber
+   * the lanes of the latency shape).  Results do not depend on the shape. */
+  AVM_RUN_SHAPE_WIDE = 4u,        /* 768 threads per SM: most lanes, for runs that keep them busy */
+  AVM_RUN_SHAPE_LATENCY = 8u      /* 512 threads per SM with time-parallel batches: fewest cycles per step */
+};
 typedef struct {
   uint64_t seed;
   double t_max;                   /* ns; electrons with t > t_max stop with status 6 (+inf: none) */

@@ -32,8 +32,8 @@ int32_t fail(int32_t code, const std::string& msg) { g_err = msg; return code; }
 #ifndef AVM_THREADS
 #define AVM_THREADS 512
 #endif
-#ifndef AVM_MIN_CTAS
-#define AVM_MIN_CTAS 1
+#ifndef AVM_THREADS_WIDE
+#define AVM_THREADS_WIDE 768
 #endif
 #ifndef AVM_FLIGHTS
 #define AVM_FLIGHTS 2
@@ -41,9 +41,12 @@ int32_t fail(int32_t code, const std::string& msg) { g_err = msg; return code; }
 #ifndef AVM_COOP_MAX
 #define AVM_COOP_MAX 8
 #endif
-constexpr int kThreads = AVM_THREADS;        // threads per CTA of the transport kernel
-constexpr int kMinCtasPerSm = AVM_MIN_CTAS;  // one 512-thread CTA per SM: 128 registers per thread, <= 227 KB shared
-constexpr int kWarpsPerCta = kThreads / 32;
+// Two launch shapes of the transport kernel, one CTA per SM either way (the threshold table takes 160 KB of shared
+// memory).  Latency shape: 512 threads, up to 128 registers, with the time-parallel batches — for runs whose electrons
+// are fewer than the lanes for most of their duration.  Wide shape: 768 threads, 80 registers, cooperative batches only —
+// chosen when the primaries alone outnumber the lanes of the latency shape (or by flag).
+constexpr int kThreads = AVM_THREADS;
+constexpr int kThreadsWide = AVM_THREADS_WIDE;
 constexpr uint32_t kDefaultMaxIters = 1u << 16;
 constexpr int64_t kStageElectrons = 1 << 18;   // primaries staged per H2D chunk (16 MiB)
 constexpr int kMaxGrid = 1024;                 // done flags, one 32-byte sector per CTA
@@ -79,16 +82,22 @@ static_assert(sizeof(RunCtl) <= kDoneOffset, "ctl block");
 // Per-warp exchange area of the cooperative batches (shared memory): entry j = draws of electron (j mod k') at its
 // step (j div k') of the batch, written by lane j.
 struct WarpBuf {
-  double dt[32];
-  uint2 u2w[32];
-  double ct[32], st[32], cphi[32], sphi[32];
+  union {
+    struct {                       // cooperative batches: draws of entry j
+      double dt[32];
+      uint2 u2w[32];
+      double ct[32], st[32], cphi[32], sphi[32];
+    };
+    struct {                       // time-parallel batches: base state of electron e, owner lane <-> group
+      double bs[7][16];
+      unsigned int bslot[16];
+      int bfin[16];
+    };
+  };
   unsigned long long id[32];
   unsigned int n[32];
-  // time-parallel batches: base state of electron e (entry e), written by its owner lane / its group's first lane
-  double bs[7][16];
-  unsigned int bslot[16];
-  int bfin[16];
 };
+static_assert(sizeof(WarpBuf) == 1920, "WarpBuf");
 
 __device__ __forceinline__ int ld_relaxed_s32(const int* p) {
   int v;
@@ -122,8 +131,8 @@ __device__ __forceinline__ void idle_wait(uint32_t ns) {
 constexpr int kFlights = AVM_FLIGHTS;
 constexpr int kCoopMax = AVM_COOP_MAX;
 
-template <bool UNIFORM1, bool HASB, bool TALLY, bool SMEMTAB>
-__global__ void __launch_bounds__(kThreads, kMinCtasPerSm)
+template <bool UNIFORM1, bool HASB, bool TALLY, bool SMEMTAB, int THREADS, bool TPB>
+__global__ void __launch_bounds__(THREADS, 1)
 transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevField f, const RunArrays a,
                  RunCtl* __restrict__ ctl, const __grid_constant__ PhiloxKeys K, const double t_max,
                  const uint32_t max_iters, const uint32_t n_static_tickets) {
@@ -152,6 +161,7 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
   const uint32_t cap = a.cap;
   const size_t ld = cap;
   // static tickets, CTA-major then warp then lane: the first electrons go one per warp, spread over all SMs
+  constexpr int kWarpsPerCta = THREADS / 32;
   uint32_t ticket = (lane * kWarpsPerCta + warp) * gridDim.x + blockIdx.x;
   bool have = false, dvalid = false;
   double x = 0, y = 0, z = 0, t = 0, vx = 0, vy = 0, vz = 0, Ex = 0, Ey = 0, Ez = 0, dt = 0;
@@ -292,7 +302,7 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
     }
     const int k = __popc(act);
 
-    if (UNIFORM1 && k <= kCoopMax) {
+    if (TPB && UNIFORM1 && k <= kCoopMax) {
       // ---- time-parallel batch (uniform E, optional B): g = 32 / k' lanes per electron ----
       // In a constant field, consecutive null flights compose exactly: the state after flights dt_1 .. dt_j is the
       // ballistic / helical flight of duration T_j = dt_1 + .. + dt_j from the base state.  Lane s of electron e's group
@@ -1023,14 +1033,18 @@ int32_t avm_run_transport_ms(const avm_ctx* c, float* ms_out) {
 namespace {
 typedef void (*TransportFn)(const DevGas, const DevField, const RunArrays, RunCtl*, const PhiloxKeys, const double,
                             const uint32_t, const uint32_t);
-template <bool U, bool B>
-TransportFn pick2(bool tally, bool smemtab) {
-  if (tally) return smemtab ? transport_kernel<U, B, true, true> : transport_kernel<U, B, true, false>;
-  return smemtab ? transport_kernel<U, B, false, true> : transport_kernel<U, B, false, false>;
+template <bool U, bool B, int T, bool TPB>
+TransportFn pick3(bool tally, bool smemtab) {
+  if (tally) return smemtab ? transport_kernel<U, B, true, true, T, TPB> : transport_kernel<U, B, true, false, T, TPB>;
+  return smemtab ? transport_kernel<U, B, false, true, T, TPB> : transport_kernel<U, B, false, false, T, TPB>;
 }
-TransportFn pick_transport(bool uniform1, bool has_b, bool tally, bool smemtab) {
-  if (uniform1) return has_b ? pick2<true, true>(tally, smemtab) : pick2<true, false>(tally, smemtab);
-  return has_b ? pick2<false, true>(tally, smemtab) : pick2<false, false>(tally, smemtab);
+template <bool U, bool B>
+TransportFn pick2(bool tally, bool smemtab, bool wide) {
+  return wide ? pick3<U, B, kThreadsWide, false>(tally, smemtab) : pick3<U, B, kThreads, true>(tally, smemtab);
+}
+TransportFn pick_transport(bool uniform1, bool has_b, bool tally, bool smemtab, bool wide) {
+  if (uniform1) return has_b ? pick2<true, true>(tally, smemtab, wide) : pick2<true, false>(tally, smemtab, wide);
+  return has_b ? pick2<false, true>(tally, smemtab, wide) : pick2<false, false>(tally, smemtab, wide);
 }
 }  // namespace
 
@@ -1073,19 +1087,23 @@ int32_t avm_run(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, const 
     else AVM_CUDA(launch(ctx, inject_kernel<false>, grid, dim3(256), field->d, a, ctl, src, (uint32_t)p0, (uint32_t)cnt, opts->id_offset, opts->t_max));
   }
   // persistent transport (a-2 .. a-11)
-  const size_t buf_bytes = sizeof(WarpBuf) * kWarpsPerCta;
+  bool wide = np > (int64_t)ctx->sm_count * kThreads;            // the primaries alone outnumber the latency shape's lanes
+  if (opts->flags & AVM_RUN_SHAPE_WIDE) wide = true;
+  if (opts->flags & AVM_RUN_SHAPE_LATENCY) wide = false;
+  const int threads = wide ? kThreadsWide : kThreads;
+  const size_t buf_bytes = sizeof(WarpBuf) * (size_t)(threads / 32);
   const size_t tab_bytes = align_up(sizeof(ushort4) * (size_t)gas->d.nb, 16);
   const bool smemtab = tab_bytes + buf_bytes <= kMaxDynSmem;       // else the threshold table is read through L1
   const size_t dyn_smem = (smemtab ? tab_bytes : 0) + buf_bytes;
-  TransportFn fn = pick_transport(field->uniform1, field->d.has_B != 0, tally, smemtab);
+  TransportFn fn = pick_transport(field->uniform1, field->d.has_B != 0, tally, smemtab, wide);
   AVM_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn_smem));
   int occ = 0;
-  AVM_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kThreads, dyn_smem));
+  AVM_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, threads, dyn_smem));
   if (occ < 1) return fail(AVM_ERR_CUDA, "run: transport kernel does not fit on an SM");
   if (opts->n_ctas_per_sm > 0 && opts->n_ctas_per_sm < occ) occ = opts->n_ctas_per_sm;
   unsigned grid = (unsigned)(ctx->sm_count * occ);
   if (grid > (unsigned)kMaxGrid) grid = kMaxGrid;
-  const uint32_t n_static = grid * kThreads;
+  const uint32_t n_static = grid * (uint32_t)threads;
   const uint32_t max_iters = opts->max_iters_per_launch ? opts->max_iters_per_launch : kDefaultMaxIters;
   unsigned long long c = 0ull;
   const int64_t max_launches = 1ll << 20;
@@ -1103,7 +1121,7 @@ int32_t avm_run(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, const 
       ctx->transport_ms += ms;
     }
     AVM_CUDA(cudaEventRecord(ctx->ev_t0, st));
-    fn<<<grid, kThreads, dyn_smem, st>>>(gas->d, field->d, a, ctl, philox_keys(opts->seed), opts->t_max, max_iters, n_static);
+    fn<<<grid, threads, dyn_smem, st>>>(gas->d, field->d, a, ctl, philox_keys(opts->seed), opts->t_max, max_iters, n_static);
     AVM_CUDA(cudaGetLastError());
     AVM_CUDA(cudaEventRecord(ctx->ev_t1, st));
     ctx->n_kernel_launches++; ctx->n_transport_launches++;

@@ -277,6 +277,22 @@ def test_relaunch_guard_gives_same_run(avm, ctx, g0):
     assert np.array_equal(one.tallies_u64, few.tallies_u64)
 
 
+def test_launch_shape_does_not_change_the_run(avm, ctx, oracle, g0):
+    """The two launch shapes of the transport kernel (512 threads with time-parallel batches / 768 threads with
+    cooperative batches only) evaluate the same steps: same-seed runs agree with each other and with the oracle, with
+    and without B."""
+    for B, E0, gap, tmax in (((0.0, 0.0, 0.0), -60000.0, 60e-4, float("inf")), ((0.0, 0.5, 0.8660254037844387), -1000.0, 1.0, 1.0)):
+        fd = fields.uniform_gap((0, 0, E0), 0.0, gap, B)
+        p = primaries.isotropic_primaries(96, 5, pos=(0, 0, 0.3 * gap))
+        gg, fg = avm.gas_create(ctx, g0), avm.field_create(ctx, fd)
+        cpu = oracle.run(g0, fd, p, seed=5, t_max=tmax, n_threads=8)
+        lat = avm.simulate(ctx, gg, fg, p, seed=5, t_max=tmax, capacity=1 << 17, flags=avm.RUN_SHAPE_LATENCY)
+        wide = avm.simulate(ctx, gg, fg, p, seed=5, t_max=tmax, capacity=1 << 17, flags=avm.RUN_SHAPE_WIDE)
+        assert_run_same_seed(cpu, lat, g0.n_levels, min_identical=0.99)
+        assert_run_same_seed(cpu, wide, g0.n_levels, min_identical=0.99)
+        assert_run_same_seed(lat, wide, g0.n_levels, min_identical=0.99)
+
+
 def test_run_with_magnetic_field_and_time_cut(avm, ctx, oracle, g0):
     """Config-3-like: 1 kV/cm, B = 1 T at 30 degrees, time cut so the oracle finishes: same-seed parity."""
     fd = fields.uniform_gap((0, 0, -1000.0), 0.0, 1.0, (0.0, 0.5, 0.8660254037844387))
