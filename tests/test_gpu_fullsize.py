@@ -1,0 +1,105 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (primaries resident on the
+device, the workload's capacity, default launch shape).
+
+Configs 1, 2 and 4 are small enough for the oracle in full: the whole run is compared electron by electron.  Configs 3
+(with bench's time cut) and 5 are not: the GPU runs them in full, properties that hold at any size are checked on every
+electron (charge conservation, the step bookkeeping of the tallies, status validity, per-avalanche counts), and the
+first avalanches — identical Philox streams to the oracle's run of the same primaries — are compared one by one.
+"""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from paper_2509_15377_b200.gen import configs
+from test_gpu_parity import assert_run_same_seed
+
+pytestmark = pytest.mark.gpu
+CORES = os.cpu_count() or 1
+
+
+@pytest.fixture(scope="module")
+def ctx(avm):
+    return avm.ctx_create(0)
+
+
+def run_as_bench(avm, ctx, w, t_max=None):
+    """avm_run the way bench.py's device_step does, then fetch."""
+    gg, fg = avm.gas_create(ctx, w.gas), avm.field_create(ctx, w.field)
+    bufs = avm.RunBuffers(ctx, w.capacity, w.n_primaries, w.gas.n_levels)
+    prim_dev = torch.from_numpy(w.primaries.copy()).to(ctx.device)
+    _, n = avm.run(ctx, gg, fg, prim_dev, bufs, seed=w.seed, t_max=w.t_max if t_max is None else t_max)
+    return avm.fetch(ctx, bufs, n)
+
+
+def check_invariants(r, w):
+    """Properties of any correct run, whatever its size (D3)."""
+    L = w.gas.n_levels
+    t = r.tallies_u64
+    ion = sum(int(t[l]) for l in range(L) if w.gas.level_type[l] == 2)
+    att = sum(int(t[l]) for l in range(L) if w.gas.level_type[l] == 3)
+    assert r.n == w.n_primaries + ion                                  # electrons = primaries + ionisations
+    assert int((r.status == 5).sum()) == att                           # attached electrons = attachment collisions
+    assert np.all((r.status >= 1) & (r.status <= 7))                   # every electron has a non-zero status
+    assert sum(int(t[l]) for l in range(L)) == int(t[L + 1])           # level counts sum to the real collisions
+    assert int(r.n_steps.astype(np.int64).sum()) == int(t[L + 3])      # steps
+    ended_before_decision = int(((r.status != 5) & (r.n_steps > 0)).sum())
+    assert int(t[L]) + int(t[L + 1]) + ended_before_decision == int(t[L + 3])   # null + real + last flights = steps
+    pa = r.per_avalanche
+    assert int(pa[:, 0].sum()) == r.n and np.array_equal(pa[:, 1], pa[:, 0] - 1) and int(pa[:, 2].sum()) == att
+    assert np.array_equal(np.bincount(r.avalanche.astype(np.int64), minlength=w.n_primaries), pa[:, 0].astype(np.int64))
+    assert len(np.unique(r.id)) == r.n                                 # hashed child ids do not collide (R16)
+    assert np.all(r.end[3] >= r.birth[3])
+
+
+def first_avalanches(r, m):
+    """The electrons of avalanches 0 .. m-1 as a run result of their own."""
+    sel = r.avalanche < m
+    return type(r)(int(sel.sum()), r.id[sel], r.avalanche[sel], r.status[sel], r.n_steps[sel], r.birth[:, sel],
+                   r.end[:, sel], r.per_avalanche[:m], r.tallies_u64, r.tallies_f64)
+
+
+def test_config2_full_size(avm, ctx, oracle):
+    w = configs.config2()
+    gpu = run_as_bench(avm, ctx, w)
+    check_invariants(gpu, w)
+    cpu = oracle.run(w.gas, w.field, w.primaries, seed=w.seed, capacity=w.capacity, n_threads=CORES)
+    assert cpu.n > 100000
+    assert_run_same_seed(cpu, gpu, w.gas.n_levels, min_identical=0.999)
+    L = w.gas.n_levels
+    assert abs(int(gpu.tallies_u64[L + 3]) / int(cpu.tallies_u64[L + 3]) - 1) < 1e-3
+    assert abs(gpu.n / cpu.n - 1) < 1e-3
+    Wc = cpu.tallies_f64[2] / cpu.tallies_f64[3]; Wg = gpu.tallies_f64[2] / gpu.tallies_f64[3]
+    assert abs(Wg / Wc - 1) < 1e-3
+
+
+def test_config3_time_cut_full_size(avm, ctx, oracle):
+    """bench's config3s: 1e5 primaries with B, t_max = 20 ns (the wide launch shape is chosen from the primary count)."""
+    w = configs.config3(n_primaries=100000, t_max=20.0)
+    gpu = run_as_bench(avm, ctx, w)
+    check_invariants(gpu, w)
+    assert (gpu.status == 6).sum() > 0.9 * w.n_primaries               # almost all reach the time cut
+    m = 96
+    cpu = oracle.run(w.gas, w.field, w.primaries[:m], seed=w.seed, t_max=20.0, n_threads=CORES)
+    assert_run_same_seed(cpu, first_avalanches(gpu, m), w.gas.n_levels, min_identical=0.97, end_rtol=1e-7)
+
+
+def test_config4_full_size(avm, ctx, oracle):
+    w = configs.config4()
+    gpu = run_as_bench(avm, ctx, w)
+    check_invariants(gpu, w)
+    cpu = oracle.run(w.gas, w.field, w.primaries, seed=w.seed, capacity=w.capacity, n_threads=CORES)
+    assert cpu.n > 5000
+    assert_run_same_seed(cpu, gpu, w.gas.n_levels, min_identical=0.90, end_rtol=1e-6, tail=0.05)
+    L = w.gas.n_levels
+    assert abs(int(gpu.tallies_u64[L + 3]) / int(cpu.tallies_u64[L + 3]) - 1) < 0.02
+
+
+def test_config5_full_size(avm, ctx, oracle):
+    w = configs.config5()
+    gpu = run_as_bench(avm, ctx, w)
+    check_invariants(gpu, w)
+    m = 4
+    cpu = oracle.run(w.gas, w.field, w.primaries[:m], seed=w.seed, capacity=1 << 16, n_threads=m)
+    assert_run_same_seed(cpu, first_avalanches(gpu, m), w.gas.n_levels, min_identical=0.80, end_rtol=1e-6, tail=0.05)
