@@ -129,7 +129,8 @@ typedef struct {
   uint64_t seed;
   double t_max;                   /* ns; electrons with t > t_max stop with status 6 (+inf: none) */
   uint32_t flags;
-  uint32_t max_iters_per_launch;  /* guard on the persistent kernel's loop (0 = default); the host relaunches */
+  uint32_t max_iters_per_launch;  /* guard: working iterations per warp and launch (0 = default 2^22); the warp that
+                                   * reaches it stops the launch, live electrons are parked, the host relaunches */
   uint64_t id_offset;             /* id of primary 0 (replicas / shards of one job use disjoint ranges) */
   int32_t n_ctas_per_sm;          /* 0 = default */
 } avm_run_opts;

@@ -32,6 +32,9 @@ int32_t fail(int32_t code, const std::string& msg) { g_err = msg; return code; }
 #ifndef AVM_THREADS
 #define AVM_THREADS 512
 #endif
+#ifndef AVM_BACKOFF_MAX
+#define AVM_BACKOFF_MAX 2000
+#endif
 #ifndef AVM_THREADS_WIDE
 #define AVM_THREADS_WIDE 768
 #endif
@@ -47,7 +50,8 @@ int32_t fail(int32_t code, const std::string& msg) { g_err = msg; return code; }
 // chosen when the primaries alone outnumber the lanes of the latency shape (or by flag).
 constexpr int kThreads = AVM_THREADS;
 constexpr int kThreadsWide = AVM_THREADS_WIDE;
-constexpr uint32_t kDefaultMaxIters = 1u << 16;
+constexpr uint32_t kMaxIdlePolls = 1u << 23;
+constexpr uint32_t kDefaultMaxIters = 1u << 22;   // working iterations per warp and launch (seconds of work): a safety net
 constexpr int64_t kStageElectrons = 1 << 18;   // primaries staged per H2D chunk (16 MiB)
 constexpr int kMaxGrid = 1024;                 // done flags, one 32-byte sector per CTA
 constexpr size_t kDoneOffset = 4096;
@@ -278,7 +282,13 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
     }
   };
 
-  for (uint32_t it = 0; it < max_iters; ++it) {
+  // `it` counts the iterations in which the warp advanced electrons; idle polling does not use up the guard (an idle
+  // warp that left early would strand the electrons later published to its tickets until the next launch).  The warp
+  // whose guard expires raises the stop flag (done = 2) of every CTA: idle warps leave, working warps park their
+  // electrons at their next check, and the host relaunches.
+  uint32_t it = 0, idle_polls = 0;
+  bool stopped = false;
+  while (it < max_iters) {
     unsigned act = __ballot_sync(0xFFFFFFFFu, have);
     // ---- probe the warp's lowest pending ticket (one sector per warp); consumed after the iteration's work ----
     uint32_t tmin = 0xFFFFFFFFu;
@@ -289,17 +299,21 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
     }
     if (act == 0u) {                                // whole warp idle
       if (probe == -1) {                            // nothing to pick up: check for the end, back off
-        if (ld_relaxed_s32(done) != 0) break;
+        if (ld_relaxed_s32(done) != 0) { stopped = true; break; }
+        if (++idle_polls >= kMaxIdlePolls) { it = max_iters; break; }   // safety net: ~15 s without work ends the launch
         idle_wait(backoff);
-        backoff = min(backoff * 2u, 2000u);
+        backoff = min(backoff * 2u, (uint32_t)AVM_BACKOFF_MAX);
         continue;
       }
       refill();
       backoff = 250u;
+      idle_polls = 0;
       act = __ballot_sync(0xFFFFFFFFu, have);
       if (act == 0u) continue;
       probe = -1;
     }
+    ++it;
+    if ((it & 15u) == 0u && ld_relaxed_s32(done) == 2) { stopped = true; break; }
     const int k = __popc(act);
 
     if (TPB && UNIFORM1 && k <= kCoopMax) {
@@ -482,8 +496,13 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
     if (probe != -1) refill();
   }
 
-  // guard expired with the electron still active: park its state in its slot (status stays 0); the next
-  // launch picks it up through the tickets.
+  if (it >= max_iters && !stopped) {                // guard expired here: stop the launch everywhere
+    int* d0 = reinterpret_cast<int*>(reinterpret_cast<unsigned char*>(ctl) + kDoneOffset);
+    for (unsigned b = lane; b < gridDim.x; b += 32u)
+      if (ld_relaxed_s32(d0 + 8 * b) == 0) *(volatile int*)(d0 + 8 * b) = 2;
+  }
+  // guard expired or launch stopped with the electron still active: park its state in its slot (status stays 0);
+  // the next launch picks it up through the tickets.
   if (have) {
     const double s2 = vx * vx + vy * vy + vz * vz;
     double kx = 0.0, ky = 0.0, kz = 1.0;
@@ -1115,6 +1134,7 @@ int32_t avm_run(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, const 
     if ((uint32_t)(c >> 32) == (uint32_t)c) break;              // a-11: every electron has a non-zero status
     if (++launches > max_launches) return fail(AVM_ERR_STATE, "run: launch limit reached without termination");
     AVM_CUDA(cudaMemsetAsync(&ctl->q_head, 0, sizeof(unsigned int), st));
+    if (launches > 1) AVM_CUDA(cudaMemsetAsync((unsigned char*)ctl + kDoneOffset, 0, (size_t)kMaxGrid * 32, st));   // stop flags
     if (launches > 1) {                                          // close the previous launch's bracket
       float ms = 0.0f;
       AVM_CUDA(cudaEventElapsedTime(&ms, ctx->ev_t0, ctx->ev_t1));

@@ -267,9 +267,9 @@ def test_relaunch_guard_gives_same_run(avm, ctx, g0):
     gg, fg = avm.gas_create(ctx, g0), avm.field_create(ctx, fd)
     one = avm.simulate(ctx, gg, fg, p, seed=3, capacity=1 << 16)
     _, l1 = avm.run_stats(ctx)
-    many = avm.simulate(ctx, gg, fg, p, seed=3, capacity=1 << 16, max_iters_per_launch=11)
+    many = avm.simulate(ctx, gg, fg, p, seed=3, capacity=1 << 16, max_iters_per_launch=5)
     _, l2 = avm.run_stats(ctx)
-    assert l1 == 1 and l2 > 10
+    assert l1 == 1 and l2 > 10, (l1, l2)
     assert_run_same_seed(one, many, g0.n_levels, min_identical=0.99)
     # one CTA per SM instead of the default: scheduling must not matter either
     few = avm.simulate(ctx, gg, fg, p, seed=3, capacity=1 << 16, n_ctas_per_sm=1)
