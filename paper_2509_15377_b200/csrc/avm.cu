@@ -976,9 +976,11 @@ int32_t avm_field_create(avm_ctx* ctx, const avm_field_desc* d, avm_field** out)
       for (int a = 0; a < 3; ++a) { S.org[a] = s.origin[a]; S.inv_h[a] = 1.0 / s.spacing[a]; }
       for (int a = 0; a < 2; ++a) {
         S.bc[a] = bc[a];
-        S.span[a] = (nn[a] - 1) * s.spacing[a];
-        S.P[a] = bc[a] == 2 ? 2.0 * per[a] : per[a];
+        S.span[a] = bc[a] ? inf : (nn[a] - 1) * s.spacing[a];
+        S.P[a] = bc[a] == 2 ? 2.0 * per[a] : (bc[a] == 1 ? per[a] : 1.0);
         S.inv_P[a] = bc[a] ? 1.0 / S.P[a] : 0.0;
+        S.Pc[a] = bc[a] ? S.P[a] : inf;
+        S.lo[a] = bc[a] ? 0.0 : -inf;
         S.half[a] = bc[a] == 2 ? per[a] : inf;
       }
     }

@@ -38,8 +38,10 @@ struct DevGas {
 struct DevSlab {
   double z_lo, z_hi;
   double E[3];
-  double org[3], inv_h[3], span[2];   // span = (n-1)*h in x, y (bc none)
-  double P[2], inv_P[2];              // fold period per axis (periodic: P; mirror: 2P) and its inverse
+  double org[3], inv_h[3], span[2];   // span = (n-1)*h in x, y for bc none, +inf otherwise
+  // fold per axis, one branch-free formula for the three boundary conditions (fold_axis):
+  double P[2], inv_P[2];              // fold period (periodic: P; mirror: 2P; none: 1) and its inverse (none: 0)
+  double Pc[2], lo[2];                // rounding guard q >= Pc || q < lo -> 0 (none: +inf, -inf; else P, 0)
   double half[2];                     // mirror: P (reflect when q > half); else +inf
   const float4* nodes;
   int kind, nx, ny, nz, bc[2];
@@ -175,17 +177,17 @@ __device__ __forceinline__ void sincos_half_angle(double a, double& s, double& c
 // ---- field (S0, R14, R15) -------------------------------------------------------------------------------
 __device__ __forceinline__ double f2d(float v) { return (double)v; }
 
-// Fold coordinate `q = x - org` of axis ax into the stored cell.  Returns false when outside with bc none.
+// Fold coordinate `q = x - org` of axis ax into the stored cell (R15).  Returns false when outside with bc none.
+// Branch-free: the three boundary conditions differ only in the slab's constants (none: P = 1, inv_P = 0, no guard, no
+// reflection, span = grid extent; periodic / mirror: span = +inf).
 __device__ __forceinline__ bool fold_axis(const DevSlab& s, int ax, double x, double& q, bool& flip) {
-  flip = false;
-  q = x - s.org[ax];
-  const int bc = s.bc[ax];
-  if (bc == 0) return q >= 0.0 && q <= s.span[ax];
+  const double q0 = x - s.org[ax];
   const double P = s.P[ax];
-  q = q - P * floor(q * s.inv_P[ax]);
-  if (q >= P || q < 0.0) q = 0.0;
-  if (q > s.half[ax]) { q = P - q; flip = true; }
-  return true;
+  double qq = q0 - P * floor(q0 * s.inv_P[ax]);
+  qq = (qq >= s.Pc[ax] || qq < s.lo[ax]) ? 0.0 : qq;
+  flip = qq > s.half[ax];
+  q = flip ? P - qq : qq;
+  return (q >= 0.0) & (q <= s.span[ax]);
 }
 
 __device__ __forceinline__ void cell_of(double s, int n, int& i, double& w) {
@@ -211,8 +213,8 @@ __device__ __forceinline__ bool grid_at(const DevSlab& s, double x, double y, do
                                         double& Ez, double& mask) {
   double qx, qy;
   bool fx, fy;
-  if (!fold_axis(s, 0, x, qx, fx)) return false;
-  if (!fold_axis(s, 1, y, qy, fy)) return false;
+  const bool okx = fold_axis(s, 0, x, qx, fx);
+  const bool oky = fold_axis(s, 1, y, qy, fy);      // outside a bc-none grid: the cell index is clamped, the result unused
   int i, j, k;
   double wx, wy, wz;
   cell_of(qx * s.inv_h[0], s.nx, i, wx);
@@ -230,7 +232,7 @@ __device__ __forceinline__ bool grid_at(const DevSlab& s, double x, double y, do
   mask = lerp3(f2d(n000.w), f2d(n100.w), f2d(n010.w), f2d(n110.w), f2d(n001.w), f2d(n101.w), f2d(n011.w), f2d(n111.w), wx, wy, wz);
   Ex = fx ? -ex : ex;
   Ey = fy ? -ey : ey;
-  return true;
+  return okx & oky;
 }
 
 // Field and mask at r.  Returns the slab index (>= 0) or -status when r is outside the domain.
@@ -442,12 +444,26 @@ __device__ __forceinline__ int advance(const DevGas& g, const DevField& f, doubl
       return t > t_max ? -AVM_TIME_LIMIT : -AVM_STEP_LIMIT;
     }
   } else {
-    double mask;
-    const int si = field_at<UNIFORM1>(f, x, y, z, Ex, Ey, Ez, mask);
-    if (si < 0) return si;
-    if (mask < 0.5) return -AVM_MATERIAL;
-    if (t > t_max) return -AVM_TIME_LIMIT;
-    if (n >= kStepLimit) return -AVM_STEP_LIMIT;
+    // the lookup runs unconditionally (indices are clamped, so any r' is safe to look up) and every S5 condition
+    // joins one predicate; the status is decoded, in S5's order, only when it fails
+    bool inb = (z >= f.z_lo) & (z <= f.z_hi);
+    if (f.xy_bounded) inb = inb & (x >= f.xy_lo[0]) & (x <= f.xy_hi[0]) & (y >= f.xy_lo[1]) & (y <= f.xy_hi[1]);
+    else inb = inb & ((x + y) == (x + y));
+    int si = f.n_slabs - 1;
+    for (int i = f.n_slabs - 2; i >= 0; --i) if (z < f.slab[i].z_hi) si = i;
+    const DevSlab& s = f.slab[si];
+    double nEx, nEy, nEz, mask = 1.0;
+    bool fold_ok = true;
+    if (s.kind == 0) { nEx = s.E[0]; nEy = s.E[1]; nEz = s.E[2]; }
+    else fold_ok = grid_at(s, x, y, z, nEx, nEy, nEz, mask);
+    const bool ok = inb & fold_ok & !(mask < 0.5) & !(t > t_max) & (n < kStepLimit);
+    if (!ok) {
+      if (!inb) return outside_status(f, x, y, z);
+      if (!fold_ok) return -AVM_LEFT_XY;
+      if (mask < 0.5) return -AVM_MATERIAL;
+      return t > t_max ? -AVM_TIME_LIMIT : -AVM_STEP_LIMIT;
+    }
+    Ex = nEx; Ey = nEy; Ez = nEz;
   }
   // S6.  eps' = max(s2 inv_c2sq, eps_floor) and b = min(nb - 1, (int)(eps' inv_de)); the floor is applied to the bin
   // (monotone: (int)(max(e, fl) c) = max((int)(e c), (int)(fl c))), the clamp after a saturating conversion.
