@@ -132,7 +132,7 @@ typedef struct {
   uint32_t max_iters_per_launch;  /* guard: working iterations per warp and launch (0 = default 2^22); the warp that
                                    * reaches it stops the launch, live electrons are parked, the host relaunches */
   uint64_t id_offset;             /* id of primary 0 (replicas / shards of one job use disjoint ranges) */
-  int32_t n_ctas_per_sm;          /* 0 = default */
+  int32_t max_ctas;               /* 0 = one CTA per SM; else at most this many CTAs (results do not depend on it) */
 } avm_run_opts;
 
 /* Caller-provided DEVICE buffers; `capacity` = maximum number of electrons ever created (primaries +

@@ -56,7 +56,7 @@ class _FieldDesc(C.Structure):
 
 class _RunOpts(C.Structure):
     _fields_ = [("seed", C.c_uint64), ("t_max", C.c_double), ("flags", C.c_uint32),
-                ("max_iters_per_launch", C.c_uint32), ("id_offset", C.c_uint64), ("n_ctas_per_sm", C.c_int32)]
+                ("max_iters_per_launch", C.c_uint32), ("id_offset", C.c_uint64), ("max_ctas", C.c_int32)]
 
 
 class _Outputs(C.Structure):
@@ -344,7 +344,7 @@ class RunResult:
 
 
 def run(ctx: Context, gas: Gas, field: Field, primaries, bufs: RunBuffers, seed=0, t_max=float("inf"), flags=0,
-        max_iters_per_launch=0, id_offset=0, n_ctas_per_sm=0, allow_overflow=False) -> tuple:
+        max_iters_per_launch=0, id_offset=0, max_ctas=0, allow_overflow=False) -> tuple:
     """avm_run.  primaries: numpy/CPU tensor [Np, 8] (H2D inside the call) or a CUDA tensor (flag set here).
     Returns (rc, n_endpoints); outputs stay in `bufs` on the device."""
     if isinstance(primaries, torch.Tensor) and primaries.is_cuda:
@@ -359,7 +359,7 @@ def run(ctx: Context, gas: Gas, field: Field, primaries, bufs: RunBuffers, seed=
     else:
         p = np.ascontiguousarray(primaries, dtype=np.float64)
         ptr, np_ = _hp(p), p.shape[0]
-    opts = _RunOpts(int(seed), float(t_max), int(flags), int(max_iters_per_launch), int(id_offset), int(n_ctas_per_sm))
+    opts = _RunOpts(int(seed), float(t_max), int(flags), int(max_iters_per_launch), int(id_offset), int(max_ctas))
     o = bufs.c_struct()
     n_out = C.c_int64(0)
     rc = _lib.avm_run(ctx._h, gas._h, field._h, ptr, np_, C.byref(opts), C.byref(o), C.byref(n_out))

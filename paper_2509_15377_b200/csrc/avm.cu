@@ -1121,9 +1121,9 @@ int32_t avm_run(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, const 
   int occ = 0;
   AVM_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, threads, dyn_smem));
   if (occ < 1) return fail(AVM_ERR_CUDA, "run: transport kernel does not fit on an SM");
-  if (opts->n_ctas_per_sm > 0 && opts->n_ctas_per_sm < occ) occ = opts->n_ctas_per_sm;
   unsigned grid = (unsigned)(ctx->sm_count * occ);
   if (grid > (unsigned)kMaxGrid) grid = kMaxGrid;
+  if (opts->max_ctas > 0 && (unsigned)opts->max_ctas < grid) grid = (unsigned)opts->max_ctas;
   const uint32_t n_static = grid * (uint32_t)threads;
   const uint32_t max_iters = opts->max_iters_per_launch ? opts->max_iters_per_launch : kDefaultMaxIters;
   unsigned long long c = 0ull;

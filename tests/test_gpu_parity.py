@@ -271,8 +271,8 @@ def test_relaunch_guard_gives_same_run(avm, ctx, g0):
     _, l2 = avm.run_stats(ctx)
     assert l1 == 1 and l2 > 10, (l1, l2)
     assert_run_same_seed(one, many, g0.n_levels, min_identical=0.99)
-    # one CTA per SM instead of the default: scheduling must not matter either
-    few = avm.simulate(ctx, gg, fg, p, seed=3, capacity=1 << 16, n_ctas_per_sm=1)
+    # 5 CTAs instead of one per SM (electrons queue for lanes): scheduling must not matter either
+    few = avm.simulate(ctx, gg, fg, p, seed=3, capacity=1 << 16, max_ctas=5)
     assert_run_same_seed(one, few, g0.n_levels, min_identical=1.0)
     assert np.array_equal(one.tallies_u64, few.tallies_u64)
 
