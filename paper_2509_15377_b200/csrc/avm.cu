@@ -366,14 +366,35 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
         const bool valid = alive && sidx >= cur;
         x = bx; y = by; z = bz; t = bt; vx = bvx; vy = bvy; vz = bvz;
         n = bn + (uint32_t)(sidx - cur);
-        bool over = false, ev = false;
+        bool over = false, ev = false, fast = false;
         int b = 0, r = -1;
         Pending pc;
         pc.lsel = 0; pc.bin = 0; pc.xr = 0.0;
+        double fvx = 0.0, fvy = 0.0, fvz = 0.0, floss = 0.0;
         if (valid) {
-          b = advance<UNIFORM1, HASB>(g, f, t_max, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, P - Pb, over);
-          if (b < 0) ev = true;
-          else { r = decide(g, tab[b], b, u2j, pc.xr); ev = r >= 0; }
+          // One straight-line block, so that the independent chains overlap: the flight (S3-S4), the S5 predicate, the bin,
+          // the threshold record and its 16-bit decision — and the ELASTIC collision this step would be, evaluated ahead
+          // of the decision from the post-flight velocity (levels 0 / 1 are 97 % of the real collisions).  The rare
+          // outcomes (termination, a band of the filter, another level or type) are decoded after the block.
+          flight<UNIFORM1, HASB>(f, 0.0, 0.0, 0.0, P - Pb, x, y, z, vx, vy, vz);
+          const double s2 = vx * vx + vy * vy + vz * vz;
+          t = t + (P - Pb);
+          n = n + 1u;
+          const bool ok = uniform_continues(f, t_max, n, x, y, z, t);
+          b = energy_bin(g, s2, over);
+          r = decide_filter(tab[b], u2j);
+          const LevelPar par = s_lv[r == 1 ? 1 : 0];
+          fvx = vx; fvy = vy; fvz = vz;
+          floss = elastic_collision(par.recoil, dj, s2, fvx, fvy, fvz);
+          fast = ok & ((r == 0) | (r == 1)) & (par.type == AVM_ELASTIC) & (s2 >= 1e-280);
+          if (!ok) {
+            b = uniform_exit_status(f, t_max, x, y, z, t);
+          } else if (r == -2 || r == 2) {
+            pc.xr = to_unit(u2j.x, u2j.y) * g.nu_hat;
+            if (r == -2) r = decide_exact(g, b, pc.xr);
+            if (r == 2) prefetch_row(g, b);
+          }
+          ev = b < 0 || r >= 0;
         }
         const unsigned evm = __ballot_sync(0xFFFFFFFFu, ev) & gmask;
         const int fl = __ffs(evm) - 1;                       // the group's first step that is not null, or -1
@@ -382,7 +403,10 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
         bool pend = false;
         if ((int)lane == fl) {
           if (b < 0) fin = -b;
-          else { pend = true; pc.lsel = r; pc.bin = b; }
+          else if (fast) {                                   // the collision is already there
+            vx = fvx; vy = fvy; vz = fvz;
+            if (TALLY) { ++c_real; if (r == 0) ++c_l0; c_loss += floss; }
+          } else { pend = true; pc.lsel = r; pc.bin = b; }
         }
         if (__any_sync(0xFFFFFFFFu, pend)) collide_and_append(pend, pc, true, dj, fin);
         // the group's new base: the state after its first event, or after its last step when all were null

@@ -408,6 +408,21 @@ __device__ __forceinline__ void draw_flight(const DevGas& g, const PhiloxKeys& K
 // u2 nu_hat >= cum and h <= q - 2 implies u2 nu_hat < cum with a margin of nu_hat 2^-16, far above the rounding of the
 // fp64 product — so the 16-bit filter takes the oracle's decision exactly, and the 2e-4 of the steps that fall inside a
 // band are decided from the exact fp64 record.
+// The 16-bit filter alone, branch-free: -1 / 0 / 1 / 2 as decide(), or -2 when h lies in a band (exact record needed).
+__device__ __forceinline__ int decide_filter(const ushort4 rec, uint2 u2w) {
+  const uint32_t h = u2w.x >> 16;
+  const uint32_t qt = rec.x, q0 = rec.y, q1 = rec.z;
+  const bool null = h >= qt + 2u, l0 = h + 2u <= q0;
+  const bool l1 = (h >= q0 + 2u) & (h + 2u <= q1), l2 = (h >= q1 + 2u) & (h + 2u <= qt);
+  return null ? -1 : (l0 ? 0 : (l1 ? 1 : (l2 ? 2 : -2)));
+}
+// The exact decision from the fp64 record (inside a band of the filter).
+__device__ __forceinline__ int decide_exact(const DevGas& g, int b, double xr) {
+  const double2 h0 = __ldg(g.head + 2 * (size_t)b), h1 = __ldg(g.head + 2 * (size_t)b + 1);
+  if (xr >= h0.x) return -1;
+  if (xr < h0.y) return 0;
+  return xr < h1.x ? 1 : 2;
+}
 __device__ __forceinline__ int decide(const DevGas& g, const ushort4 rec, int b, uint2 u2w, double& xr) {
   const uint32_t h = u2w.x >> 16;
   const uint32_t qt = rec.x, q0 = rec.y, q1 = rec.z;
@@ -415,13 +430,35 @@ __device__ __forceinline__ int decide(const DevGas& g, const ushort4 rec, int b,
   if (h + 2u <= q0) return 0;
   if (h >= q0 + 2u && h + 2u <= q1) return 1;
   xr = to_unit(u2w.x, u2w.y) * g.nu_hat;
-  if (h >= q1 + 2u && h + 2u <= qt) { prefetch_row(g, b); return 2; }
-  const double2 h0 = __ldg(g.head + 2 * (size_t)b), h1 = __ldg(g.head + 2 * (size_t)b + 1);
-  if (xr >= h0.x) return -1;
-  if (xr < h0.y) return 0;
-  if (xr < h1.x) return 1;
-  prefetch_row(g, b);
-  return 2;
+  int r = 2;
+  if (!(h >= q1 + 2u && h + 2u <= qt)) r = decide_exact(g, b, xr);
+  if (r == 2) prefetch_row(g, b);
+  return r;
+}
+
+// S6.  eps' = max(s2 inv_c2sq, eps_floor) and b = min(nb - 1, (int)(eps' inv_de)); the floor is applied to the bin
+// (monotone: (int)(max(e, fl) c) = max((int)(e c), (int)(fl c))), the clamp after a saturating conversion.
+__device__ __forceinline__ int energy_bin(const DevGas& g, double s2, bool& overflow) {
+  const int braw = __double2int_rz((s2 * kInvC2Sq) * g.inv_de);
+  overflow = braw >= g.nb;
+  return max(min(braw, g.nb - 1), g.bin_floor);
+}
+
+// S5 in one uniform slab: every condition under which the electron goes on, as one predicate; and, when it fails, the
+// status in S5's order (z faces, x/y bounds or NaN, time limit, step limit), negated.
+__device__ __forceinline__ bool uniform_continues(const DevField& f, double t_max, uint32_t n, double x, double y,
+                                                  double z, double t) {
+  bool ok = (z >= f.z_lo) & (z <= f.z_hi) & (t <= t_max) & (n < kStepLimit);
+  if (f.xy_bounded) ok = ok & (x >= f.xy_lo[0]) & (x <= f.xy_hi[0]) & (y >= f.xy_lo[1]) & (y <= f.xy_hi[1]);
+  else ok = ok & ((x + y) == (x + y));
+  return ok;
+}
+__device__ __forceinline__ int uniform_exit_status(const DevField& f, double t_max, double x, double y, double z,
+                                                   double t) {
+  const bool in = (z >= f.z_lo) & (z <= f.z_hi) & (x >= f.xy_lo[0]) & (x <= f.xy_hi[0]) & (y >= f.xy_lo[1]) &
+                  (y <= f.xy_hi[1]);
+  if (!in) return outside_status(f, x, y, z);
+  return t > t_max ? -AVM_TIME_LIMIT : -AVM_STEP_LIMIT;
 }
 
 // S3-S6 for one electron with this flight's dt.  Returns the energy bin (>= 0) or -(finishing status).
@@ -434,15 +471,7 @@ __device__ __forceinline__ int advance(const DevGas& g, const DevField& f, doubl
   t = t + dt;
   n = n + 1u;
   if (UNIFORM1) {                                                     // S5: one test on the common path
-    bool ok = (z >= f.z_lo) & (z <= f.z_hi) & (t <= t_max) & (n < kStepLimit);
-    if (f.xy_bounded) ok = ok & (x >= f.xy_lo[0]) & (x <= f.xy_hi[0]) & (y >= f.xy_lo[1]) & (y <= f.xy_hi[1]);
-    else ok = ok & ((x + y) == (x + y));
-    if (!ok) {
-      const bool in = (z >= f.z_lo) & (z <= f.z_hi) & (x >= f.xy_lo[0]) & (x <= f.xy_hi[0]) & (y >= f.xy_lo[1]) &
-                      (y <= f.xy_hi[1]);
-      if (!in) return outside_status(f, x, y, z);
-      return t > t_max ? -AVM_TIME_LIMIT : -AVM_STEP_LIMIT;
-    }
+    if (!uniform_continues(f, t_max, n, x, y, z, t)) return uniform_exit_status(f, t_max, x, y, z, t);
   } else {
     // the lookup runs unconditionally (indices are clamped, so any r' is safe to look up) and every S5 condition
     // joins one predicate; the status is decoded, in S5's order, only when it fails
@@ -465,11 +494,35 @@ __device__ __forceinline__ int advance(const DevGas& g, const DevField& f, doubl
     }
     Ex = nEx; Ey = nEy; Ez = nEz;
   }
-  // S6.  eps' = max(s2 inv_c2sq, eps_floor) and b = min(nb - 1, (int)(eps' inv_de)); the floor is applied to the bin
-  // (monotone: (int)(max(e, fl) c) = max((int)(e c), (int)(fl c))), the clamp after a saturating conversion.
-  const int braw = __double2int_rz((s2 * kInvC2Sq) * g.inv_de);
-  overflow = braw >= g.nb;
-  return max(min(braw, g.nb - 1), g.bin_floor);
+  return energy_bin(g, s2, overflow);
+}
+
+// S9d in velocity form (see collision_step): v'' = (c2 sqrt(e2) / s) R(v') for |v'|^2 = s2 >= 1e-280.
+__device__ __forceinline__ void rotate_scale(const Deflection& d, double s2, double e2, double& vx, double& vy,
+                                             double& vz) {
+  const double rs = rsqrt_fast(s2), s = s2 * rs;
+  const int sb = __double2hiint(vz) & 0x80000000;                              // sg = copysign(1, v'z)
+  const double sgs = xor_sign(s, sb);
+  const double A = -rcp_fast(sgs + vz);
+  const double Bq = vx * vy * A;
+  const double b1x = fma(xor_sign(vx * vx, sb), A, s), b1y = xor_sign(Bq, sb), b1z = xor_sign(vx, sb ^ 0x80000000);
+  const double b2x = Bq, b2y = fma(vy * vy, A, sgs), b2z = -vy;
+  const double rx = fma(d.ct, vx, d.st * fma(d.cphi, b1x, d.sphi * b2x));
+  const double ry = fma(d.ct, vy, d.st * fma(d.cphi, b1y, d.sphi * b2y));
+  const double rz = fma(d.ct, vz, d.st * fma(d.cphi, b1z, d.sphi * b2z));
+  const double ratio = (kC2 * sqrt_fast(e2)) * rs;                             // speed'' / s
+  vx = rx * ratio; vy = ry * ratio; vz = rz * ratio;
+}
+
+// S9c + S9d of an ELASTIC collision with recoil factor r_l from the post-flight velocity (s2 = |v'|^2 >= 1e-280).
+// Returns the energy loss.  Branch-free: the time-parallel batches evaluate it for every step ahead of the decision.
+__device__ __forceinline__ double elastic_collision(double recoil, const Deflection& d, double s2, double& vx, double& vy,
+                                                    double& vz) {
+  double e1 = s2 * kInvC2Sq;
+  e1 = e1 < kEpsFloor ? kEpsFloor : e1;
+  const double e2 = e1 * (1.0 - recoil * (1.0 - d.ct));
+  rotate_scale(d, s2, e2, vx, vy, vz);
+  return e1 - e2;
 }
 
 // S8-S9 for an electron with a pending real collision (n already incremented by the flight).  Returns the level;
@@ -514,18 +567,7 @@ __device__ __forceinline__ int collision_step(const DevGas& g, const LevelPar* _
     spawn = true;
     loss = e1 - e2 - ch.e;
   }
-  const double rs = rsqrt_fast(s2), s = s2 * rs;                               // S9d
-  const int sb = __double2hiint(vz) & 0x80000000;                              // sg = copysign(1, v'z)
-  const double sgs = xor_sign(s, sb);
-  const double A = -rcp_fast(sgs + vz);
-  const double Bq = vx * vy * A;
-  const double b1x = fma(xor_sign(vx * vx, sb), A, s), b1y = xor_sign(Bq, sb), b1z = xor_sign(vx, sb ^ 0x80000000);
-  const double b2x = Bq, b2y = fma(vy * vy, A, sgs), b2z = -vy;
-  const double rx = fma(d.ct, vx, d.st * fma(d.cphi, b1x, d.sphi * b2x));
-  const double ry = fma(d.ct, vy, d.st * fma(d.cphi, b1y, d.sphi * b2y));
-  const double rz = fma(d.ct, vz, d.st * fma(d.cphi, b1z, d.sphi * b2z));
-  const double ratio = (kC2 * sqrt_fast(e2)) * rs;                             // speed'' / s
-  vx = rx * ratio; vy = ry * ratio; vz = rz * ratio;
+  rotate_scale(d, s2, e2, vx, vy, vz);                                         // S9d
   return l;
 }
 
