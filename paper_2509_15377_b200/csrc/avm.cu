@@ -93,9 +93,9 @@ struct WarpBuf {
       double ct[32], st[32], cphi[32], sphi[32];
     };
     struct {                       // time-parallel batches: base state of electron e, owner lane <-> group
-      double bs[7][16];
+      double2 bsv[16][4];          // (x, y), (z, t), (vx, vy), (vz, sum of dt up to the base)
+      uint2 bnf[16];               // (n, finishing status)
       unsigned int bslot[16];
-      int bfin[16];
     };
   };
   unsigned long long id[32];
@@ -329,18 +329,18 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
       const int rank = __popc(act & lt_mask);
       const int e = (int)lane & (kp - 1), sidx = (int)lane >> lg;
       if (have) {
-        wb->bs[0][rank] = x; wb->bs[1][rank] = y; wb->bs[2][rank] = z; wb->bs[3][rank] = t;
-        wb->bs[4][rank] = vx; wb->bs[5][rank] = vy; wb->bs[6][rank] = vz;
-        wb->id[rank] = id; wb->n[rank] = n; wb->bslot[rank] = slot;
+        wb->bsv[rank][0] = make_double2(x, y); wb->bsv[rank][1] = make_double2(z, t);
+        wb->bsv[rank][2] = make_double2(vx, vy); wb->bsv[rank][3] = make_double2(vz, 0.0);
+        wb->id[rank] = id; wb->bnf[rank] = make_uint2(n, 0u); wb->bslot[rank] = slot;
       }
       __syncwarp();
       bool alive = e < k;
       double bx = 0, by = 0, bz = 0, bt = 0, bvx = 0, bvy = 0, bvz = 0;
       uint32_t bn = 0;
       if (alive) {
-        bx = wb->bs[0][e]; by = wb->bs[1][e]; bz = wb->bs[2][e]; bt = wb->bs[3][e];
-        bvx = wb->bs[4][e]; bvy = wb->bs[5][e]; bvz = wb->bs[6][e];
-        id = wb->id[e]; bn = wb->n[e]; slot = wb->bslot[e];
+        const double2 q0 = wb->bsv[e][0], q1 = wb->bsv[e][1], q2 = wb->bsv[e][2], q3 = wb->bsv[e][3];
+        bx = q0.x; by = q0.y; bz = q1.x; bt = q1.y; bvx = q2.x; bvy = q2.y; bvz = q3.x;
+        id = wb->id[e]; bn = wb->bnf[e].x; slot = wb->bslot[e];
       }
       __syncwarp();
       // draws of step bn + sidx, and the inclusive sums P of dt over the group's steps 0 .. sidx
@@ -410,32 +410,32 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
         }
         if (__any_sync(0xFFFFFFFFu, pend)) collide_and_append(pend, pc, true, dj, fin);
         // the group's new base: the state after its first event, or after its last step when all were null
+        // (through the warp's exchange area: four 16-byte stores by one lane, four broadcast loads by its group)
         const int src = fl >= 0 ? fl : last;
-        const double nx_ = __shfl_sync(0xFFFFFFFFu, x, src), ny_ = __shfl_sync(0xFFFFFFFFu, y, src);
-        const double nz_ = __shfl_sync(0xFFFFFFFFu, z, src), nt_ = __shfl_sync(0xFFFFFFFFu, t, src);
-        const double nvx = __shfl_sync(0xFFFFFFFFu, vx, src), nvy = __shfl_sync(0xFFFFFFFFu, vy, src);
-        const double nvz = __shfl_sync(0xFFFFFFFFu, vz, src), nP = __shfl_sync(0xFFFFFFFFu, P, src);
-        const uint32_t nn = __shfl_sync(0xFFFFFFFFu, n, src);
-        const int nfin = __shfl_sync(0xFFFFFFFFu, fin, src);
+        if (alive && (int)lane == src) {
+          wb->bsv[e][0] = make_double2(x, y); wb->bsv[e][1] = make_double2(z, t);
+          wb->bsv[e][2] = make_double2(vx, vy); wb->bsv[e][3] = make_double2(vz, P);
+          wb->bnf[e] = make_uint2(n, (unsigned)fin);
+        }
+        __syncwarp();
         if (alive) {
-          bx = nx_; by = ny_; bz = nz_; bt = nt_; bvx = nvx; bvy = nvy; bvz = nvz; Pb = nP; bn = nn; gfin = nfin;
+          const double2 q0 = wb->bsv[e][0], q1 = wb->bsv[e][1], q2 = wb->bsv[e][2], q3 = wb->bsv[e][3];
+          const uint2 nf = wb->bnf[e];
+          bx = q0.x; by = q0.y; bz = q1.x; bt = q1.y; bvx = q2.x; bvy = q2.y; bvz = q3.x; Pb = q3.y;
+          bn = nf.x; gfin = (int)nf.y;
           cur = (src >> lg) + 1;
           if (gfin != 0 || cur >= gl) alive = false;
         }
+        __syncwarp();
         if (!__any_sync(0xFFFFFFFFu, alive)) break;
       }
-      // hand the electrons back to their owner lanes
-      if (sidx == 0 && e < k) {
-        wb->bs[0][e] = bx; wb->bs[1][e] = by; wb->bs[2][e] = bz; wb->bs[3][e] = bt;
-        wb->bs[4][e] = bvx; wb->bs[5][e] = bvy; wb->bs[6][e] = bvz;
-        wb->n[e] = bn; wb->bfin[e] = gfin;
-      }
-      __syncwarp();
+      // the electrons go back to their owner lanes: the exchange area holds each group's final base state
       int fin = 0;
       if (have) {
-        x = wb->bs[0][rank]; y = wb->bs[1][rank]; z = wb->bs[2][rank]; t = wb->bs[3][rank];
-        vx = wb->bs[4][rank]; vy = wb->bs[5][rank]; vz = wb->bs[6][rank];
-        id = wb->id[rank]; n = wb->n[rank]; slot = wb->bslot[rank]; fin = wb->bfin[rank];
+        const double2 q0 = wb->bsv[rank][0], q1 = wb->bsv[rank][1], q2 = wb->bsv[rank][2], q3 = wb->bsv[rank][3];
+        const uint2 nf = wb->bnf[rank];
+        x = q0.x; y = q0.y; z = q1.x; t = q1.y; vx = q2.x; vy = q2.y; vz = q3.x;
+        id = wb->id[rank]; n = nf.x; slot = wb->bslot[rank]; fin = (int)nf.y;
       }
       __syncwarp();
       dvalid = false;
