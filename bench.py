@@ -33,10 +33,10 @@ FP64_PER_ION_EXTRA = 80.0                        # Opal-Beaty atan/tan, child di
 FP64_PER_GRID_EXTRA = 45.0                       # fold + 7 lerps x 4 channels per step in a grid slab
 GATHER_BYTES_PER_GRID_STEP = 128.0               # 8 nodes x 16 B
 FP64_LANES_PER_SM = 64                           # one warp-wide FP64 instruction / 2 clk / scheduler
-# From the committed ncu captures of the transport kernel (profiles/r1c_transport_ncu.md), per launch of the workload:
+# From the committed ncu captures of the transport kernel (profiles/r1d_transport_ncu.md), per launch of the workload:
 # DRAM bytes read + written, DFMA + DMUL + DADD thread-instructions per collision, FP64 pipe active %.
-NCU_R1C = {"config2": {"traffic": 3964672 + 102144, "sass_fp64_per_collision": 73.8, "fp64_pipe_active_pct": 21.4},
-           "config2x16": {"traffic": 91168256 + 419136256, "sass_fp64_per_collision": 63.3, "fp64_pipe_active_pct": 27.3}}
+NCU_CAPTURE = {"config2": {"traffic": 3897344 + 48640, "sass_fp64_per_collision": 92.4, "fp64_pipe_active_pct": 22.9},
+               "config2x16": {"traffic": 92790528 + 419887104, "sass_fp64_per_collision": 64.4, "fp64_pipe_active_pct": 27.3}}
 
 
 def make_workload(name: str, rank: int = 0):
@@ -289,11 +289,11 @@ def run_ours(args) -> None:
     achieved = (fp64 / max(t_launches, 1)) / ((t_ms / max(t_launches, 1)) * 1e-3)
     roofline = {"bound": "alu", "kernel": "transport_kernel", "achieved": achieved / 1e12, "peak": peak["measured"] / 1e12,
                 "unit": "T FP64 thread-instr/s", "frac": achieved / peak["measured"],
-                "traffic": NCU_R1C.get(w.name, {}).get("traffic"),
-                "traffic_source": "profiles/r1c_transport_ncu.md (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum, one launch)"
-                                  if w.name in NCU_R1C else None,
-                "sass_fp64_per_collision_ncu": NCU_R1C.get(w.name, {}).get("sass_fp64_per_collision"),
-                "fp64_pipe_active_pct_ncu": NCU_R1C.get(w.name, {}).get("fp64_pipe_active_pct"),
+                "traffic": NCU_CAPTURE.get(w.name, {}).get("traffic"),
+                "traffic_source": "profiles/r1d_transport_ncu.md (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum, one launch)"
+                                  if w.name in NCU_CAPTURE else None,
+                "sass_fp64_per_collision_ncu": NCU_CAPTURE.get(w.name, {}).get("sass_fp64_per_collision"),
+                "fp64_pipe_active_pct_ncu": NCU_CAPTURE.get(w.name, {}).get("fp64_pipe_active_pct"),
                 "peak_source": "measured: avm_fp64_probe DFMA rate on this GPU in this run",
                 "peak_nominal": peak["nominal"] / 1e12,
                 "frac_of_nominal": achieved / peak["nominal"],
