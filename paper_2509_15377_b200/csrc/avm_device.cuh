@@ -461,40 +461,58 @@ __device__ __forceinline__ int uniform_exit_status(const DevField& f, double t_m
   return t > t_max ? -AVM_TIME_LIMIT : -AVM_STEP_LIMIT;
 }
 
+// S5 at r' (and S0 of the next step: the field there): 0 when the electron goes on — Ex, Ey, Ez then hold the field at
+// r' — or -(finishing status).  One uniform slab: one predicate.  Maps: the lookup runs unconditionally (indices are
+// clamped, so any r' is safe to look up), every condition joins one predicate, and the status is decoded, in S5's
+// order, only when it fails.
+template <bool UNIFORM1>
+__device__ __forceinline__ int s5_status(const DevField& f, double t_max, uint32_t n, double x, double y, double z,
+                                         double t, double& Ex, double& Ey, double& Ez) {
+  if (UNIFORM1) {
+    if (!uniform_continues(f, t_max, n, x, y, z, t)) return uniform_exit_status(f, t_max, x, y, z, t);
+    return 0;
+  }
+  bool inb = (z >= f.z_lo) & (z <= f.z_hi);
+  if (f.xy_bounded) inb = inb & (x >= f.xy_lo[0]) & (x <= f.xy_hi[0]) & (y >= f.xy_lo[1]) & (y <= f.xy_hi[1]);
+  else inb = inb & ((x + y) == (x + y));
+  int si = f.n_slabs - 1;
+  for (int i = f.n_slabs - 2; i >= 0; --i) if (z < f.slab[i].z_hi) si = i;
+  const DevSlab& s = f.slab[si];
+  double nEx, nEy, nEz, mask = 1.0;
+  bool fold_ok = true;
+  if (s.kind == 0) { nEx = s.E[0]; nEy = s.E[1]; nEz = s.E[2]; }
+  else fold_ok = grid_at(s, x, y, z, nEx, nEy, nEz, mask);
+  const bool ok = inb & fold_ok & !(mask < 0.5) & !(t > t_max) & (n < kStepLimit);
+  if (!ok) {
+    if (!inb) return outside_status(f, x, y, z);
+    if (!fold_ok) return -AVM_LEFT_XY;
+    if (mask < 0.5) return -AVM_MATERIAL;
+    return t > t_max ? -AVM_TIME_LIMIT : -AVM_STEP_LIMIT;
+  }
+  Ex = nEx; Ey = nEy; Ez = nEz;
+  return 0;
+}
+
+// S3-S4: the flight itself; t and n advance.  Returns |v'|^2.
+template <bool UNIFORM1, bool HASB>
+__device__ __forceinline__ double advance_move(const DevField& f, uint32_t& n, double& x, double& y, double& z, double& t,
+                                               double& vx, double& vy, double& vz, double Ex, double Ey, double Ez,
+                                               double dt) {
+  flight<UNIFORM1, HASB>(f, Ex, Ey, Ez, dt, x, y, z, vx, vy, vz);
+  t = t + dt;
+  n = n + 1u;
+  return vx * vx + vy * vy + vz * vz;
+}
+
 // S3-S6 for one electron with this flight's dt.  Returns the energy bin (>= 0) or -(finishing status).
 template <bool UNIFORM1, bool HASB>
 __device__ __forceinline__ int advance(const DevGas& g, const DevField& f, double t_max, uint32_t& n, double& x,
                                        double& y, double& z, double& t, double& vx, double& vy, double& vz, double& Ex,
                                        double& Ey, double& Ez, double dt, bool& overflow) {
-  flight<UNIFORM1, HASB>(f, Ex, Ey, Ez, dt, x, y, z, vx, vy, vz);     // S3
-  const double s2 = vx * vx + vy * vy + vz * vz;                      // S4
-  t = t + dt;
-  n = n + 1u;
-  if (UNIFORM1) {                                                     // S5: one test on the common path
-    if (!uniform_continues(f, t_max, n, x, y, z, t)) return uniform_exit_status(f, t_max, x, y, z, t);
-  } else {
-    // the lookup runs unconditionally (indices are clamped, so any r' is safe to look up) and every S5 condition
-    // joins one predicate; the status is decoded, in S5's order, only when it fails
-    bool inb = (z >= f.z_lo) & (z <= f.z_hi);
-    if (f.xy_bounded) inb = inb & (x >= f.xy_lo[0]) & (x <= f.xy_hi[0]) & (y >= f.xy_lo[1]) & (y <= f.xy_hi[1]);
-    else inb = inb & ((x + y) == (x + y));
-    int si = f.n_slabs - 1;
-    for (int i = f.n_slabs - 2; i >= 0; --i) if (z < f.slab[i].z_hi) si = i;
-    const DevSlab& s = f.slab[si];
-    double nEx, nEy, nEz, mask = 1.0;
-    bool fold_ok = true;
-    if (s.kind == 0) { nEx = s.E[0]; nEy = s.E[1]; nEz = s.E[2]; }
-    else fold_ok = grid_at(s, x, y, z, nEx, nEy, nEz, mask);
-    const bool ok = inb & fold_ok & !(mask < 0.5) & !(t > t_max) & (n < kStepLimit);
-    if (!ok) {
-      if (!inb) return outside_status(f, x, y, z);
-      if (!fold_ok) return -AVM_LEFT_XY;
-      if (mask < 0.5) return -AVM_MATERIAL;
-      return t > t_max ? -AVM_TIME_LIMIT : -AVM_STEP_LIMIT;
-    }
-    Ex = nEx; Ey = nEy; Ez = nEz;
-  }
-  return energy_bin(g, s2, overflow);
+  const double s2 = advance_move<UNIFORM1, HASB>(f, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt);   // S3, S4
+  const int st = s5_status<UNIFORM1>(f, t_max, n, x, y, z, t, Ex, Ey, Ez);                        // S5
+  if (st < 0) return st;
+  return energy_bin(g, s2, overflow);                                                            // S6
 }
 
 // S9d in velocity form (see collision_step): v'' = (c2 sqrt(e2) / s) R(v') for |v'|^2 = s2 >= 1e-280.
