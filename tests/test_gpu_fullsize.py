@@ -103,3 +103,39 @@ def test_config5_full_size(avm, ctx, oracle):
     m = 4
     cpu = oracle.run(w.gas, w.field, w.primaries[:m], seed=w.seed, capacity=1 << 16, n_threads=m)
     assert_run_same_seed(cpu, first_avalanches(gpu, m), w.gas.n_levels, min_identical=0.80, end_rtol=1e-6, tail=0.05)
+
+
+def test_config3_drift_lorentz_angle_and_diffusion(avm, ctx, oracle):
+    """What config 3 is for (BASELINE.json): drift velocity vector, Lorentz angle and diffusion in E = 1 kV/cm with
+    B = 1 T at 30 degrees, from the endpoints of the full-size GPU run (time cut 20 ns, 1e5 electrons) against the oracle's
+    run of 6000 other primaries (independent streams: seed 1): components within 3 combined standard errors and 1.5 %."""
+    w = configs.config3(n_primaries=100000, t_max=20.0)
+    gpu = run_as_bench(avm, ctx, w)
+    wo = configs.config3(n_primaries=6000, seed=1, t_max=20.0)
+    cpu = oracle.run(wo.gas, wo.field, wo.primaries, seed=1, t_max=20.0, n_threads=CORES)
+
+    def transport(r):
+        sel = r.status == 6                                            # reached the time cut: same flight time for all
+        d = r.end[0:3, sel] - r.birth[0:3, sel]
+        T = (r.end[3, sel] - r.birth[3, sel]).mean()
+        n = sel.sum()
+        W = d.mean(axis=1) / T
+        W_se = d.std(axis=1, ddof=1) / np.sqrt(n) / T
+        D = d.var(axis=1, ddof=1) / (2 * T)                            # diffusion coefficients along x, y, z
+        D_se = D * np.sqrt(2.0 / (n - 1))
+        return W, W_se, D, D_se, n
+
+    Wg, Wg_se, Dg, Dg_se, ng = transport(gpu)
+    Wc, Wc_se, Dc, Dc_se, nc = transport(cpu)
+    assert ng > 90000 and nc > 5400
+    for a in range(3):
+        se = np.hypot(Wg_se[a], Wc_se[a])
+        assert abs(Wg[a] - Wc[a]) <= 3 * se + 0.015 * np.linalg.norm(Wc), (a, Wg, Wc, se)
+        assert abs(Dg[a] - Dc[a]) <= 3 * np.hypot(Dg_se[a], Dc_se[a]) + 0.015 * Dc[a], (a, Dg, Dc)
+    # Lorentz angle: between the drift velocity and the force direction (+z, reading R1); its standard error from the
+    # transverse components' (the oracle's 6000 electrons dominate it)
+    ang = lambda W: np.degrees(np.arccos(W[2] / np.linalg.norm(W)))
+    ang_se = lambda W, se: np.degrees(np.hypot(se[0], se[1]) / W[2])
+    assert Wg[2] > 0 and abs(Wg[0]) > 3 * Wg_se[0]                     # E x B drift along x is resolved
+    assert abs(ang(Wg) - ang(Wc)) <= 3 * np.hypot(ang_se(Wg, Wg_se), ang_se(Wc, Wc_se)) + 0.1, (ang(Wg), ang(Wc))
+    assert 1.0 < ang(Wg) < 6.0
