@@ -505,7 +505,12 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
             const ushort4 rec = tab[b];
             const uint2 u2c = u2w;
             draw_flight(g, K, s_logtab, id, n, dt, u2w);    // next flight's draws: independent of the record load
-            const int r = decide(g, rec, b, u2c, pc.xr);
+            int r = decide_filter(rec, u2c);                // branch-free; the rare outcomes below
+            if (r == -2 || r == 2) {
+              pc.xr = to_unit(u2c.x, u2c.y) * g.nu_hat;
+              if (r == -2) r = decide_exact(g, b, pc.xr);
+              if (r == 2) prefetch_row(g, b);
+            }
             if (r >= 0) { pend = true; pc.lsel = r; pc.bin = b; }
             if (TALLY && over) ++c_over;
           }
