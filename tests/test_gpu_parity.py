@@ -502,3 +502,27 @@ def test_config5_triple_gem_same_seed_run(avm, ctx, oracle, g0):
     assert gpu.n == 6 + int(t[14] + t[15]) and int(gpu.n_steps.sum()) == int(t[L + 3])
     assert np.all(gpu.status != 0) and set(np.unique(gpu.status)) <= {1, 4, 5}
     assert np.all(gpu.end[2][gpu.status == 1] < w.field.slabs[0].z_lo)
+
+
+def test_c3_nu_hat_invariance_on_gpu(avm, ctx, oracle, g0):
+    """C3 on the device: nu_hat = 1.7 x the maximum rate rescales the 16-bit threshold table and the flight times; the
+    run stays the same avalanche as the oracle's with the same nu_hat (same seed), and its statistics agree with the
+    default-nu_hat oracle run (independent streams)."""
+    import dataclasses
+    fd = fields.uniform_gap((0, 0, -45000.0), 0.0, 80e-4)
+    p = primaries.isotropic_primaries(600, 71, forward=True)
+    p[:, 2] = 2e-4
+    g2 = dataclasses.replace(g0, nu_hat=1.7 * g0.resolved_nu_hat())
+    fg = avm.field_create(ctx, fd)
+    gpu = avm.simulate(ctx, avm.gas_create(ctx, g2), fg, p, seed=71, capacity=1 << 20)
+    cpu2 = oracle.run(g2, fd, p, seed=71, capacity=1 << 20, n_threads=8)
+    assert_run_same_seed(cpu2, gpu, g0.n_levels, min_identical=0.999)
+    cpu1 = oracle.run(g0, fd, p, seed=72, capacity=1 << 20, n_threads=8)
+    L = g0.n_levels
+    g_gpu, g_cpu = gpu.per_avalanche[:, 0].astype(float), cpu1.per_avalanche[:, 0].astype(float)
+    se = np.hypot(g_gpu.std(ddof=1), g_cpu.std(ddof=1)) / np.sqrt(len(g_gpu))
+    assert abs(g_gpu.mean() - g_cpu.mean()) < 3.5 * se
+    Wg, Wc = gpu.tallies_f64[2] / gpu.tallies_f64[3], cpu1.tallies_f64[2] / cpu1.tallies_f64[3]
+    assert abs(Wg / Wc - 1) < 0.015
+    rg = float(gpu.tallies_u64[L + 1]) / gpu.tallies_f64[3]; rc = float(cpu1.tallies_u64[L + 1]) / cpu1.tallies_f64[3]
+    assert abs(rg / rc - 1) < 0.015                                    # real collisions per ns of flight

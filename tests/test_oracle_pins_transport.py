@@ -310,3 +310,36 @@ def test_c14_gain_vs_townsend_alpha(oracle, g0):
     assert len(fw) >= 12
     a_gain = np.log(fw.mean()) / (d - 2e-4)
     assert abs(a_gain - alpha) < 0.10 * alpha, (a_gain, alpha)
+
+
+def _transport_stats(r, n_levels):
+    """Per-primary gain (mean, SE), drift velocity along the force, ionisations per cm of drift, real collisions per ns."""
+    gain = r.per_avalanche[:, 0].astype(float)
+    t = r.tallies_u64
+    W = r.tallies_f64[2] / r.tallies_f64[3]
+    alpha = (float(t[14] + t[15]) - float(t[16])) / r.tallies_f64[2]
+    nu_real = float(t[n_levels + 1]) / r.tallies_f64[3]
+    return gain.mean(), gain.std(ddof=1) / np.sqrt(len(gain)), W, alpha, nu_real
+
+
+def test_c3_null_collision_invariance_g0(oracle, g0):
+    """C3: the null-collision method is exact for ANY nu_hat >= max total rate — doubling nu_hat doubles the null steps
+    and must leave every statistic alone: gain, drift velocity, Townsend alpha and the real-collision rate of gas G0 at
+    45 kV/cm (independent streams, so within sampling errors)."""
+    import dataclasses
+    f = fields.uniform_gap((0, 0, -45000.0), 0.0, 80e-4)
+    p = primaries.isotropic_primaries(1500, 61, forward=True)
+    p[:, 2] = 2e-4
+    g2 = dataclasses.replace(g0, nu_hat=2.0 * g0.resolved_nu_hat())
+    a = oracle.run(g0, f, p, seed=61, capacity=1 << 20, n_threads=8)
+    b = oracle.run(g2, f, p, seed=62, capacity=1 << 20, n_threads=8)
+    L = g0.n_levels
+    # the null steps double (real collisions do not)
+    null_a, null_b = float(a.tallies_u64[L]), float(b.tallies_u64[L])
+    real_a, real_b = float(a.tallies_u64[L + 1]), float(b.tallies_u64[L + 1])
+    assert abs((null_b + real_b) / (null_a + real_a) / 2.0 - 1.0) < 0.05
+    ga, sa, Wa, aa, na = _transport_stats(a, L)
+    gb, sb, Wb, ab, nb = _transport_stats(b, L)
+    assert abs(ga - gb) < 3.5 * np.hypot(sa, sb), (ga, gb, sa, sb)
+    assert abs(Wb / Wa - 1) < 0.01 and abs(nb / na - 1) < 0.01, (Wa, Wb, na, nb)
+    assert abs(ab / aa - 1) < 0.04, (aa, ab)
