@@ -241,7 +241,7 @@ def run_ours(args) -> None:
         res = avm.fetch(ctx, bufs, n, host)
         dt = time.perf_counter() - t0
         d2h = n * (8 + 4 + 4 + 4 + 5 * 8 + 8 * 8) + w.n_primaries * 24 + (L + 4) * 8 + 40
-        return {"s": dt, "n": n, "tallies": res.tallies_u64, "d2h": d2h}
+        return {"s": dt, "n": n, "tallies": res.tallies_u64.copy(), "d2h": d2h}
 
     for i in range(args.warmup):
         device_step(w.seed + 1000 + i)

@@ -380,16 +380,16 @@ def run_transport_ms(ctx: Context) -> float:
 
 
 def fetch(ctx: Context, bufs: RunBuffers, n: int, host: Optional[HostBuffers] = None) -> RunResult:
-    """avm_fetch: device -> host copy of the first n endpoints and the tallies."""
+    """avm_fetch: device -> host copy of the first n endpoints and the tallies.  With caller-provided `host` buffers the
+    result holds VIEWS into them (valid until they are reused: no second copy on the host); without, views into buffers
+    of its own."""
     host = host or HostBuffers(max(n, 1), bufs.n_primaries, bufs.n_levels, pinned=False)
     d, h = bufs.c_struct(), host.c_struct()
     _check(_lib.avm_fetch(ctx._h, C.byref(d), n, bufs.n_primaries, bufs.n_levels, C.byref(h)))
-    u64 = lambda t: t.numpy().view(np.uint64)
-    return RunResult(n, u64(host.id)[:n].copy(), host.avalanche.numpy().view(np.uint32)[:n].copy(),
-                     host.status.numpy()[:n].copy(), host.n_steps.numpy().view(np.uint32)[:n].copy(),
-                     host.birth.numpy()[:, :n].copy(), host.end.numpy()[:, :n].copy(),
-                     u64(host.per_avalanche)[:bufs.n_primaries].copy(), u64(host.tallies_u64).copy(),
-                     host.tallies_f64.numpy().copy())
+    u64 = lambda t: t.numpy().view(np.uint64)      # numpy views keep their torch storage alive
+    return RunResult(n, u64(host.id)[:n], host.avalanche.numpy().view(np.uint32)[:n], host.status.numpy()[:n],
+                     host.n_steps.numpy().view(np.uint32)[:n], host.birth.numpy()[:, :n], host.end.numpy()[:, :n],
+                     u64(host.per_avalanche)[:bufs.n_primaries], u64(host.tallies_u64), host.tallies_f64.numpy())
 
 
 def simulate(ctx: Context, gas: Gas, field: Field, primaries, seed=0, t_max=float("inf"), capacity=None, **kw) -> RunResult:
