@@ -984,6 +984,7 @@ int32_t avm_field_create(avm_ctx* ctx, const avm_field_desc* d, avm_field** out)
     if (!(s.z_hi > s.z_lo)) bad = "field: slab z_hi <= z_lo";
     else if (i > 0 && s.z_lo != d->slabs[i - 1].z_hi) bad = "field: slabs not contiguous/ascending";
     else if (s.kind != 0 && s.kind != 1) bad = "field: kind";
+    if (!bad && s.kind == 0 && !(std::isfinite(s.E[0]) && std::isfinite(s.E[1]) && std::isfinite(s.E[2]))) bad = "field: uniform E is not finite";
     S.z_lo = s.z_lo; S.z_hi = s.z_hi; S.kind = s.kind;
     for (int a = 0; a < 3; ++a) S.E[a] = s.E[a];
     if (!bad && s.kind == 1) {
@@ -1018,6 +1019,7 @@ int32_t avm_field_create(avm_ctx* ctx, const avm_field_desc* d, avm_field** out)
   F.z_lo = d->slabs[0].z_lo;
   F.z_hi = d->slabs[d->n_slabs - 1].z_hi;
   for (int a = 0; a < 2; ++a) { F.xy_lo[a] = d->xy_lo[a]; F.xy_hi[a] = d->xy_hi[a]; }
+  if (!(std::isfinite(d->B[0]) && std::isfinite(d->B[1]) && std::isfinite(d->B[2]))) { delete f; return fail(AVM_ERR_INVALID_ARG, "field: B is not finite"); }
   const double Bn2 = d->B[0] * d->B[0] + d->B[1] * d->B[1] + d->B[2] * d->B[2];
   F.has_B = Bn2 != 0.0;
   F.Bn2 = Bn2;

@@ -403,6 +403,10 @@ def test_edge_cases(avm, ctx, oracle, g0):
         avm.gas_create(ctx, bad)
     with pytest.raises(avm.AvmError):
         avm.field_create(ctx, fields.FieldDesc([fields.Slab(1.0, 0.0)]))
+    with pytest.raises(avm.AvmError):
+        avm.field_create(ctx, fields.uniform_gap((0.0, float("nan"), -1000.0), 0.0, 1.0))
+    with pytest.raises(avm.AvmError):
+        avm.field_create(ctx, fields.uniform_gap((0.0, 0.0, -1000.0), 0.0, 1.0, (0.0, float("inf"), 0.0)))
     # device-resident primaries and an id offset: shard [16, 32) of a job equals the same electrons of the whole job
     import torch
     p = primaries.isotropic_primaries(32, 5)
