@@ -123,12 +123,16 @@ __device__ __forceinline__ void idle_wait(uint32_t ns) {
 }
 
 // ---- persistent transport kernel -------------------------------------------------------------------------
-// One warp iteration advances the warp's k electrons (lanes with `have`):
-//  * k <= kCoopMax — cooperative batch: all 32 lanes first prepare the draws (Philox block 0 + logarithm, block 1 +
-//    deflection angles) of the next B = 32 / k' steps of the k electrons (k' = k rounded up to a power of two), lane j
-//    serving electron j mod k' at step j div k', through the warp's WarpBuf; then the owners take up to B steps whose
-//    dependent chain is only flight -> energy -> bin -> threshold record -> branch.  The draws depend on (id, n) alone, so
-//    the result is the same as drawing them in place; draws of steps an electron does not reach are discarded.
+// One warp iteration advances the warp's k electrons (lanes with `have`) in one of three forms:
+//  * k <= kCoopMax, one uniform slab, latency shape (TPB) — time-parallel batch: consecutive null flights in a constant
+//    field compose exactly, so the 32 / k' lanes of an electron (k' = k rounded up to a power of two) evaluate its next
+//    32 / k' steps at once from pre-drawn flight times; the first step that is not null is the electron's event.
+//  * k <= kCoopMax otherwise (grid maps, wide shape) — cooperative batch: all 32 lanes first prepare the draws (Philox
+//    block 0 + logarithm, block 1 + deflection angles) of the next B = 32 / k' steps of the k electrons, lane j serving
+//    electron j mod k' at step j div k', through the warp's WarpBuf; then the owners take up to B steps whose dependent
+//    chain is only flight -> field -> energy -> bin -> threshold record -> branch.
+//    In both, the draws depend on (id, n) alone, so the result is the same as drawing them in place; draws of steps an
+//    electron does not reach are discarded.
 //  * k > kCoopMax — full warp: up to kFlights free flights per lane (a lane stops flying when it draws a real
 //    collision), the draws of a lane's next flight issued behind its threshold-record load, then ONE collision phase.
 // Then the rare warp-uniform branches: append secondaries, retire finished electrons, refill idle lanes.
