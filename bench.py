@@ -197,6 +197,11 @@ def run_ours(args) -> None:
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    from paper_2509_15377_b200 import build as _build
+    if rank == 0:
+        _build.build()                               # no-op when libavm.so is newer than its sources
+    if dist is not None:
+        dist.barrier()
     from paper_2509_15377_b200 import avm            # raises when libavm.so is missing
 
     # weak scaling: every rank runs the whole workload on its own id range — avalanches are

@@ -31,5 +31,7 @@ def avm():
     import torch
     if not torch.cuda.is_available():
         pytest.fail("gpu test selected but no CUDA device is visible")
+    from paper_2509_15377_b200 import build
+    build.build()                         # no-op when libavm.so is newer than its sources (nvcc is on the GPU box too)
     from paper_2509_15377_b200 import avm as _avm
     return _avm
