@@ -182,6 +182,23 @@ int32_t avm_step_batch(avm_ctx*, const avm_gas*, const avm_field*, uint64_t seed
                        const double* state_in, const uint64_t* id, const uint32_t* n_idx, double* state_out,
                        int32_t* event, int32_t* status, int32_t* bin, double* child_out, uint64_t* child_id);
 
+/* The same hook through the step FORMS the persistent kernel runs (the device functions of
+ * csrc/avm_forms.cuh, shared by the kernel and this hook) — north_star "per-collision steps ... relative 1e-12" on the
+ * instruction sequences that earn the bench number (PAPER.md:65-69 for what a step is).
+ *  form 0: the general sequence (= avm_step_batch).  Arrays of length n.
+ *  form 1: the full-warp form: 16-bit threshold filter + exact record inside a band, the next flight's draws hoisted
+ *          behind the record load, deflection drawn in the collision phase.  Arrays of length n.
+ *  form 2: one time-parallel batch per warp (one uniform slab only): k electrons per warp (1..16, n a multiple of k) on
+ *          scattered lanes, gl = 32 / 2^ceil(log2 k) consecutive steps of each, evaluated as composed flights.  Output
+ *          arrays have n * gl entries ([8][n * gl] for states): entry i * gl + s = the result of step s of electron i,
+ *          in the sense of avm_step_batch (state after the step, event, status, bin, child).  Entries of steps the
+ *          electron does not reach (it finished earlier in the batch) are left untouched: pre-fill event with -3.
+ * k is ignored for forms 0 and 1. */
+int32_t avm_step_batch_form(avm_ctx*, const avm_gas*, const avm_field*, uint64_t seed, double t_max, int32_t form,
+                            int32_t k, int64_t n, const double* state_in, const uint64_t* id, const uint32_t* n_idx,
+                            double* state_out, int32_t* event, int32_t* status, int32_t* bin, double* child_out,
+                            uint64_t* child_id);
+
 /* Philox block (seed, id, n, block) -> words[4] and two uniforms, for n_items items.  All arrays DEVICE.
  * Pin C1: lets the tests compare the device generator bit for bit. */
 int32_t avm_philox_batch(avm_ctx*, uint64_t seed, int64_t n_items, const uint64_t* id, const uint32_t* n_idx,
@@ -189,7 +206,7 @@ int32_t avm_philox_batch(avm_ctx*, uint64_t seed, int64_t n_items, const uint64_
 
 /* FP64 issue-rate probe: runs a chain of dependent-free DFMA streams (n_threads threads, iters iterations of
  * 8 independent FMAs each) and writes the elapsed milliseconds; used by bench.py to measure the ALU roofline
- * denominator on the box it runs on.  sink: DEVICE [n_threads] doubles. */
+ * denominator on the box it runs on.  sink: DEVICE [n_blocks * n_threads_per_block] doubles. */
 int32_t avm_fp64_probe(avm_ctx*, int32_t n_blocks, int32_t n_threads_per_block, int64_t iters, double* sink,
                        float* ms_out /*host*/);
 

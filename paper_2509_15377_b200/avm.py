@@ -26,7 +26,7 @@ RUN_PRIMARIES_ON_DEVICE, RUN_NO_TALLIES, RUN_SHAPE_WIDE, RUN_SHAPE_LATENCY = 1, 
 MAX_LEVELS, MAX_SLABS = 64, 8
 EXPORTS = ["avm_last_error", "avm_ctx_create", "avm_ctx_destroy", "avm_ctx_sm_count", "avm_gas_bytes",
            "avm_gas_create", "avm_gas_destroy", "avm_gas_nu_hat", "avm_field_create", "avm_field_destroy",
-           "avm_field_eval", "avm_run_workspace_bytes", "avm_run", "avm_run_stats", "avm_run_transport_ms", "avm_fetch", "avm_step_batch",
+           "avm_field_eval", "avm_run_workspace_bytes", "avm_run", "avm_run_stats", "avm_run_transport_ms", "avm_fetch", "avm_step_batch", "avm_step_batch_form",
            "avm_philox_batch", "avm_fp64_probe"]
 
 
@@ -74,7 +74,7 @@ _lib.avm_gas_nu_hat.restype = C.c_double
 _lib.avm_gas_nu_hat.argtypes = [C.c_void_p]
 for _n in ("avm_ctx_create", "avm_ctx_destroy", "avm_ctx_sm_count", "avm_gas_create", "avm_gas_destroy",
            "avm_field_create", "avm_field_destroy", "avm_field_eval", "avm_run", "avm_run_stats", "avm_fetch",
-           "avm_step_batch", "avm_philox_batch", "avm_fp64_probe", "avm_run_transport_ms"):
+           "avm_step_batch", "avm_step_batch_form", "avm_philox_batch", "avm_fp64_probe", "avm_run_transport_ms"):
     getattr(_lib, _n).restype = C.c_int32
 _lib.avm_run_transport_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
 _lib.avm_ctx_create.argtypes = [C.c_int32, C.c_void_p, C.POINTER(C.c_void_p)]
@@ -90,6 +90,7 @@ _lib.avm_run.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int
 _lib.avm_run_stats.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
 _lib.avm_fetch.argtypes = [C.c_void_p, C.POINTER(_Outputs), C.c_int64, C.c_int64, C.c_int32, C.POINTER(_Outputs)]
 _lib.avm_step_batch.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint64, C.c_double, C.c_int64] + [C.c_void_p] * 9
+_lib.avm_step_batch_form.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint64, C.c_double, C.c_int32, C.c_int32, C.c_int64] + [C.c_void_p] * 9
 _lib.avm_philox_batch.argtypes = [C.c_void_p, C.c_uint64, C.c_int64] + [C.c_void_p] * 5
 _lib.avm_fp64_probe.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int64, C.c_void_p, C.POINTER(C.c_float)]
 
@@ -257,6 +258,37 @@ def step_batch(ctx: Context, gas: Gas, field: Field, seed, state, ids, n_idx, t_
                                _dev(out), _dev(ev), _dev(stt), _dev(bn), _dev(ch), _dev(cid)))
     return StepResult(out.cpu().numpy(), ev.cpu().numpy(), stt.cpu().numpy(), bn.cpu().numpy(), ch.cpu().numpy(),
                       cid.cpu().numpy().view(np.uint64))
+
+
+def step_form_lanes(k: int) -> int:
+    """Steps per time-parallel batch when a warp holds k electrons: 32 / 2^ceil(log2 k)."""
+    return 32 >> max(int(k) - 1, 0).bit_length()
+
+
+def step_batch_form(ctx: Context, gas: Gas, field: Field, seed, state, ids, n_idx, form: int, k: int = 1,
+                    t_max=float("inf")) -> StepResult:
+    """avm_step_batch_form.  Forms 0 / 1: as step_batch.  Form 2: arrays get a trailing axis of gl = step_form_lanes(k)
+    steps per electron ([8, n, gl], [n, gl]); steps the batch did not reach have event == -3."""
+    st = torch.from_numpy(np.ascontiguousarray(state, dtype=np.float64)).to(ctx.device)
+    n = st.shape[1]
+    gl = step_form_lanes(k) if form == 2 else 1
+    m = n * gl
+    idt = torch.from_numpy(np.ascontiguousarray(ids, dtype=np.uint64).view(np.int64)).to(ctx.device)
+    nt = torch.from_numpy(np.ascontiguousarray(n_idx, dtype=np.uint32).view(np.int32)).to(ctx.device)
+    out = torch.zeros((8, m), dtype=torch.float64, device=ctx.device)
+    ev = torch.full((m,), -3, dtype=torch.int32, device=ctx.device)
+    stt = torch.zeros(m, dtype=torch.int32, device=ctx.device)
+    bn = torch.full((m,), -1, dtype=torch.int32, device=ctx.device)
+    ch = torch.zeros((8, m), dtype=torch.float64, device=ctx.device)
+    cid = torch.zeros(m, dtype=torch.int64, device=ctx.device)
+    _check(_lib.avm_step_batch_form(ctx._h, gas._h, field._h, int(seed), float(t_max), int(form), int(k), n, _dev(st),
+                                    _dev(idt), _dev(nt), _dev(out), _dev(ev), _dev(stt), _dev(bn), _dev(ch), _dev(cid)))
+    r = StepResult(out.cpu().numpy(), ev.cpu().numpy(), stt.cpu().numpy(), bn.cpu().numpy(), ch.cpu().numpy(),
+                   cid.cpu().numpy().view(np.uint64))
+    if form == 2:
+        r = StepResult(r.state.reshape(8, n, gl), r.event.reshape(n, gl), r.status.reshape(n, gl), r.bin.reshape(n, gl),
+                       r.child.reshape(8, n, gl), r.child_id.reshape(n, gl))
+    return r
 
 
 def philox_batch(ctx: Context, seed, ids, n_idx, block):

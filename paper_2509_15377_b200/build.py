@@ -4,6 +4,7 @@ nvcc cross-compiles without a GPU.  The .so is git-ignored but travels to the GP
 """
 from __future__ import annotations
 
+import glob
 import os
 import shutil
 import subprocess
@@ -12,7 +13,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(_HERE)
 SO = os.path.join(_HERE, "libavm.so")
 SOURCES = [os.path.join(_HERE, "csrc", "avm.cu")]
-DEPS = SOURCES + [os.path.join(_HERE, "csrc", "avm_device.cuh"), os.path.join(ROOT, "include", "avm.h")]
+DEPS = sorted(glob.glob(os.path.join(_HERE, "csrc", "*"))) + [os.path.join(ROOT, "include", "avm.h")]   # every file the build reads
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC"]
 

@@ -14,7 +14,7 @@
 #include <string>
 #include <vector>
 
-#include "avm_device.cuh"
+#include "avm_forms.cuh"
 
 using namespace avm;
 
@@ -83,29 +83,17 @@ struct RunCtl {
 };
 static_assert(sizeof(RunCtl) <= kDoneOffset, "ctl block");
 
-// Per-warp exchange area of the cooperative batches (shared memory): entry j = draws of electron (j mod k') at its
-// step (j div k') of the batch, written by lane j.
-struct WarpBuf {
-  union {
-    struct {                       // cooperative batches: draws of entry j
-      double dt[32];
-      uint2 u2w[32];
-      double ct[32], st[32], cphi[32], sphi[32];
-    };
-    struct {                       // time-parallel batches: base state of electron e, owner lane <-> group
-      double2 bsv[16][4];          // (x, y), (z, t), (vx, vy), (vz, sum of dt up to the base)
-      uint2 bnf[16];               // (n, finishing status)
-      unsigned int bslot[16];
-    };
-  };
-  unsigned long long id[32];
-  unsigned int n[32];
-};
-static_assert(sizeof(WarpBuf) == 1920, "WarpBuf");
-
 __device__ __forceinline__ int ld_relaxed_s32(const int* p) {
   int v;
   asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+// Acquire load: pairs with st_release_s32 of the producer, so that the slot's payload, read after it, is the published
+// one under the PTX memory model (not only by in-order issue behind the branch).  Costs one CCTL.IVALL: used once per
+// electron pick-up, never for polling.
+__device__ __forceinline__ int ld_acquire_s32(const int* p) {
+  int v;
+  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
 }
 // Release store: earlier writes of this thread are visible at gpu scope before the flag is.  Unlike __threadfence()
@@ -176,8 +164,7 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
   uint2 u2w = make_uint2(0u, 0u);
   uint64_t id = 0;
   uint32_t n = 0, slot = 0;
-  uint32_t c_real = 0, c_l0 = 0, c_over = 0;      // tallies kept per thread; null counts are derived (finalize_kernel)
-  double c_loss = 0.0;
+  Tally tl;                                       // tallies kept per thread; null counts are derived (finalize_kernel)
   uint32_t backoff = 250u;
   const unsigned lt_mask = (1u << lane) - 1u;
 
@@ -186,7 +173,8 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
     if (!have) {
 #pragma unroll 1
       for (int tries = 0; tries < 2 && ticket < cap; ++tries) {
-        const int st = ld_relaxed_s32(a.status + ticket);
+        int st = ld_relaxed_s32(a.status + ticket);  // polling probe
+        if (st == 0) st = ld_acquire_s32(a.status + ticket);   // consumed: order the payload loads after the flag
         if (st == 0) {                              // published and unfinished: this lane runs it
           slot = ticket;
           x = __ldcg(a.end + slot); y = __ldcg(a.end + ld + slot); z = __ldcg(a.end + 2 * ld + slot);
@@ -208,20 +196,21 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
     }
   };
   // one collision phase for the lanes with a pending real collision, then append their secondaries (a-8, a-9)
-  auto collide_and_append = [&](bool pend, const Pending& pc, bool have_d, const Deflection& dd, int& fin) {
+  auto collide_and_append = [&](bool pend, const Pending& pc, bool have_d, const Deflection& dd, int& fin) -> int {
     bool spawn = false;
     Child ch;
     ch.e = 0.0; ch.u6 = 0.5; ch.u7 = 0.0;
+    int l = -1;
     if (pend) {
       double loss;
       int st;
-      const int l = collision_step(g, s_lv, K, id, n, pc, have_d, dd, vx, vy, vz, st, spawn, ch, loss);
+      l = collision_step(g, s_lv, K, id, n, pc, have_d, dd, vx, vy, vz, st, spawn, ch, loss);
       if (st) fin = st;
       if (TALLY) {
-        ++c_real;
-        if (l == 0) ++c_l0;
+        ++tl.real;
+        if (l == 0) ++tl.l0;
         else if (l > 1) atomicAdd(&s_hist[l], 1u);
-        c_loss += loss;
+        tl.loss += loss;
       }
     }
     const unsigned sm = __ballot_sync(0xFFFFFFFFu, spawn);
@@ -253,6 +242,7 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
         }
       }
     }
+    return l;
   };
   // retire finished electrons: endpoint write, one atomic per warp for `finished`, one for new tickets; the lane that
   // finishes the last electron raises every CTA's done flag (a-11)
@@ -321,127 +311,10 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
     const int k = __popc(act);
 
     if (TPB && UNIFORM1 && k <= kCoopMax) {
-      // ---- time-parallel batch (uniform E, optional B): g = 32 / k' lanes per electron ----
-      // In a constant field, consecutive null flights compose exactly: the state after flights dt_1 .. dt_j is the
-      // ballistic / helical flight of duration T_j = dt_1 + .. + dt_j from the base state.  Lane s of electron e's group
-      // evaluates the END of step s (position, energy, bounds, bin, null/real decision with its own u2) in parallel; the
-      // first lane whose step is not null (real collision or termination) is the electron's next event, every step
-      // before it was null, and the draws after it stay valid for the next pass from the new base state.  The draws
-      // depend on (id, n) only, so this is the sequence of steps S0-S9 the oracle takes, evaluated out of order.
-      const int lg = 32 - __clz(k - 1);             // k' = 2^lg >= k  (k = 1: __clz(0) = 32)
-      const int kp = 1 << lg, gl = 32 >> lg;        // gl = lanes (steps per batch) of one electron
-      const int rank = __popc(act & lt_mask);
-      const int e = (int)lane & (kp - 1), sidx = (int)lane >> lg;
-      if (have) {
-        wb->bsv[rank][0] = make_double2(x, y); wb->bsv[rank][1] = make_double2(z, t);
-        wb->bsv[rank][2] = make_double2(vx, vy); wb->bsv[rank][3] = make_double2(vz, 0.0);
-        wb->id[rank] = id; wb->bnf[rank] = make_uint2(n, 0u); wb->bslot[rank] = slot;
-      }
-      __syncwarp();
-      bool alive = e < k;
-      double bx = 0, by = 0, bz = 0, bt = 0, bvx = 0, bvy = 0, bvz = 0;
-      uint32_t bn = 0;
-      if (alive) {
-        const double2 q0 = wb->bsv[e][0], q1 = wb->bsv[e][1], q2 = wb->bsv[e][2], q3 = wb->bsv[e][3];
-        bx = q0.x; by = q0.y; bz = q1.x; bt = q1.y; bvx = q2.x; bvy = q2.y; bvz = q3.x;
-        id = wb->id[e]; bn = wb->bnf[e].x; slot = wb->bslot[e];
-      }
-      __syncwarp();
-      // draws of step bn + sidx, and the inclusive sums P of dt over the group's steps 0 .. sidx
-      double P = 0.0;
-      uint2 u2j = make_uint2(0u, 0u);
-      Deflection dj;
-      dj.ct = 1.0; dj.st = 0.0; dj.cphi = 1.0; dj.sphi = 0.0;
-      if (alive) {
-        draw_flight(g, K, s_logtab, id, bn + (uint32_t)sidx, P, u2j);
-        dj = deflection_draws(K, id, bn + (uint32_t)sidx);
-      }
-      for (int d = kp; d < 32; d <<= 1) {
-        const double up = __shfl_up_sync(0xFFFFFFFFu, P, d);
-        if ((int)lane >= d) P += up;
-      }
-      const unsigned gmask = (lg == 0 ? 0xFFFFFFFFu : lg == 1 ? 0x55555555u : lg == 2 ? 0x11111111u
-                              : lg == 3 ? 0x01010101u : 0x00010001u) << e;
-      const int last = ((gl - 1) << lg) | e;
-      double Pb = 0.0;
-      int cur = 0, gfin = 0;
-#pragma unroll 1
-      for (;;) {
-        const bool valid = alive && sidx >= cur;
-        x = bx; y = by; z = bz; t = bt; vx = bvx; vy = bvy; vz = bvz;
-        n = bn + (uint32_t)(sidx - cur);
-        bool over = false, ev = false, fast = false;
-        int b = 0, r = -1;
-        Pending pc;
-        pc.lsel = 0; pc.bin = 0; pc.xr = 0.0;
-        double fvx = 0.0, fvy = 0.0, fvz = 0.0, floss = 0.0;
-        if (valid) {
-          // One straight-line block, so that the independent chains overlap: the flight (S3-S4), the S5 predicate, the bin,
-          // the threshold record and its 16-bit decision — and the ELASTIC collision this step would be, evaluated ahead
-          // of the decision from the post-flight velocity (levels 0 / 1 are 97 % of the real collisions).  The rare
-          // outcomes (termination, a band of the filter, another level or type) are decoded after the block.
-          flight<UNIFORM1, HASB>(f, 0.0, 0.0, 0.0, P - Pb, x, y, z, vx, vy, vz);
-          const double s2 = vx * vx + vy * vy + vz * vz;
-          t = t + (P - Pb);
-          n = n + 1u;
-          const bool ok = uniform_continues(f, t_max, n, x, y, z, t);
-          b = energy_bin(g, s2, over);
-          r = decide_filter(tab[b], u2j);
-          const LevelPar par = s_lv[r == 1 ? 1 : 0];
-          fvx = vx; fvy = vy; fvz = vz;
-          floss = elastic_collision(par.recoil, dj, s2, fvx, fvy, fvz);
-          fast = ok & ((r == 0) | (r == 1)) & (par.type == AVM_ELASTIC) & (s2 >= 1e-280);
-          if (!ok) {
-            b = uniform_exit_status(f, t_max, x, y, z, t);
-          } else if (r == -2 || r == 2) {
-            pc.xr = to_unit(u2j.x, u2j.y) * g.nu_hat;
-            if (r == -2) r = decide_exact(g, b, pc.xr);
-            if (r == 2) prefetch_row(g, b);
-          }
-          ev = b < 0 || r >= 0;
-        }
-        const unsigned evm = __ballot_sync(0xFFFFFFFFu, ev) & gmask;
-        const int fl = __ffs(evm) - 1;                       // the group's first step that is not null, or -1
-        if (TALLY && valid && over && (fl < 0 || (int)lane <= fl)) ++c_over;
-        int fin = 0;
-        bool pend = false;
-        if ((int)lane == fl) {
-          if (b < 0) fin = -b;
-          else if (fast) {                                   // the collision is already there
-            vx = fvx; vy = fvy; vz = fvz;
-            if (TALLY) { ++c_real; if (r == 0) ++c_l0; c_loss += floss; }
-          } else { pend = true; pc.lsel = r; pc.bin = b; }
-        }
-        if (__any_sync(0xFFFFFFFFu, pend)) collide_and_append(pend, pc, true, dj, fin);
-        // the group's new base: the state after its first event, or after its last step when all were null
-        // (through the warp's exchange area: four 16-byte stores by one lane, four broadcast loads by its group)
-        const int src = fl >= 0 ? fl : last;
-        if (alive && (int)lane == src) {
-          wb->bsv[e][0] = make_double2(x, y); wb->bsv[e][1] = make_double2(z, t);
-          wb->bsv[e][2] = make_double2(vx, vy); wb->bsv[e][3] = make_double2(vz, P);
-          wb->bnf[e] = make_uint2(n, (unsigned)fin);
-        }
-        __syncwarp();
-        if (alive) {
-          const double2 q0 = wb->bsv[e][0], q1 = wb->bsv[e][1], q2 = wb->bsv[e][2], q3 = wb->bsv[e][3];
-          const uint2 nf = wb->bnf[e];
-          bx = q0.x; by = q0.y; bz = q1.x; bt = q1.y; bvx = q2.x; bvy = q2.y; bvz = q3.x; Pb = q3.y;
-          bn = nf.x; gfin = (int)nf.y;
-          cur = (src >> lg) + 1;
-          if (gfin != 0 || cur >= gl) alive = false;
-        }
-        __syncwarp();
-        if (!__any_sync(0xFFFFFFFFu, alive)) break;
-      }
-      // the electrons go back to their owner lanes: the exchange area holds each group's final base state
-      int fin = 0;
-      if (have) {
-        const double2 q0 = wb->bsv[rank][0], q1 = wb->bsv[rank][1], q2 = wb->bsv[rank][2], q3 = wb->bsv[rank][3];
-        const uint2 nf = wb->bnf[rank];
-        x = q0.x; y = q0.y; z = q1.x; t = q1.y; vx = q2.x; vy = q2.y; vz = q3.x;
-        id = wb->id[rank]; n = nf.x; slot = wb->bslot[rank]; fin = (int)nf.y;
-      }
-      __syncwarp();
+      // ---- time-parallel batch (uniform E, optional B): g = 32 / k' lanes per electron (avm_forms.cuh) ----
+      const int fin = tp_batch<UNIFORM1, HASB, TALLY>(g, f, K, tab, s_lv, s_logtab, wb, t_max, lane, act, have, x, y, z, t, vx,
+                                                      vy, vz, id, n, slot, tl, collide_and_append,
+                                                      [](bool, int, int, int, int, int) {});
       dvalid = false;
       retire(fin);
     } else if (k <= kCoopMax) {
@@ -485,7 +358,7 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
               pend = true; pc.lsel = r; pc.bin = b;
               dd.ct = wb->ct[idx]; dd.st = wb->st[idx]; dd.cphi = wb->cphi[idx]; dd.sphi = wb->sphi[idx];
             }
-            if (TALLY && over) ++c_over;
+            if (TALLY && over) ++tl.over;
           }
         }
         if (__any_sync(0xFFFFFFFFu, pend)) collide_and_append(pend, pc, true, dd, fin);
@@ -501,24 +374,9 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
       pc.lsel = 0; pc.bin = 0; pc.xr = 0.0;
 #pragma unroll
       for (int fl = 0; fl < kFlights; ++fl) {
-        if (have && !pend && fin == 0) {
-          bool over = false;
-          const int b = advance<UNIFORM1, HASB>(g, f, t_max, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt, over);
-          if (b < 0) fin = -b;
-          else {
-            const ushort4 rec = tab[b];
-            const uint2 u2c = u2w;
-            draw_flight(g, K, s_logtab, id, n, dt, u2w);    // next flight's draws: independent of the record load
-            int r = decide_filter(rec, u2c);                // branch-free; the rare outcomes below
-            if (r == -2 || r == 2) {
-              pc.xr = to_unit(u2c.x, u2c.y) * g.nu_hat;
-              if (r == -2) r = decide_exact(g, b, pc.xr);
-              if (r == 2) prefetch_row(g, b);
-            }
-            if (r >= 0) { pend = true; pc.lsel = r; pc.bin = b; }
-            if (TALLY && over) ++c_over;
-          }
-        }
+        if (have && !pend && fin == 0)
+          fw_flight<UNIFORM1, HASB, TALLY>(g, f, K, tab, s_logtab, t_max, id, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt, u2w, fin,
+                                           pend, pc, tl);
       }
       Deflection dd;
       dd.ct = 1.0; dd.st = 0.0; dd.cphi = 1.0; dd.sphi = 0.0;
@@ -547,8 +405,8 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
   }
   if (TALLY) {
     // warp reduce the per-thread counters, one atomic per warp; rare-level histogram per CTA
-    unsigned long long v0 = c_real, v1 = c_l0, v3 = c_over;
-    double v4 = c_loss;
+    unsigned long long v0 = tl.real, v1 = tl.l0, v3 = tl.over;
+    double v4 = tl.loss;
 #pragma unroll
     for (int o2 = 16; o2 > 0; o2 >>= 1) {
       v0 += __shfl_down_sync(0xFFFFFFFFu, v0, o2); v1 += __shfl_down_sync(0xFFFFFFFFu, v1, o2);
@@ -675,7 +533,10 @@ __global__ void publish_kernel(const RunCtl* ctl, const int L, unsigned long lon
 }
 
 // ---- parity hooks ----------------------------------------------------------------------------------------
-template <bool UNIFORM1, bool HASB>
+// FORM 0: the general sequence draw_flight -> advance -> decide -> collision_step.  FORM 1: the full-warp form of the
+// transport kernel — fw_flight (avm_forms.cuh: advance, decide_filter / decide_exact, the next flight's draws hoisted
+// behind the record load) and the collision phase with the deflection drawn there.
+template <bool UNIFORM1, bool HASB, int FORM>
 __global__ void step_batch_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevField f,
                                   const uint64_t seed, const double t_max, const int64_t n,
                                   const double* __restrict__ in, const uint64_t* __restrict__ ids,
@@ -715,18 +576,36 @@ __global__ void step_batch_kernel(const __grid_constant__ DevGas g, const __grid
   Child ch;
   ch.e = 0.0; ch.u6 = 0.5; ch.u7 = 0.0;
   int ev = -2, st = 0;
-  const int b = advance<UNIFORM1, HASB>(g, f, t_max, nn, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt, over);
-  if (b < 0) st = -b;
-  else {
-    pc.bin = b;
-    const int r = decide(g, __ldg(g.tab + b), b, u2, pc.xr);
-    if (r < 0) ev = -1;
+  Deflection dd;
+  dd.ct = 1.0; dd.st = 0.0; dd.cphi = 1.0; dd.sphi = 0.0;
+  if (FORM == 1) {
+    bool pend = false;
+    Tally tl;
+    fw_flight<UNIFORM1, HASB, true>(g, f, K, g.tab, s_logtab, t_max, id, nn, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt, u2, st, pend,
+                                    pc, tl);
+    over = tl.over != 0u;
+    if (st == 0) {
+      ev = -1;
+      if (pend) {
+        double loss;
+        ev = collision_step(g, s_lv, K, id, nn, pc, false, dd, vx, vy, vz, st, spawn, ch, loss);
+      } else {
+        bool o2;
+        pc.bin = energy_bin(g, vx * vx + vy * vy + vz * vz, o2);     // a null step leaves the velocity alone: its bin, for the report
+      }
+    }
+  } else {
+    const int b = advance<UNIFORM1, HASB>(g, f, t_max, nn, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt, over);
+    if (b < 0) st = -b;
     else {
-      double loss;
-      pc.lsel = r;
-      Deflection dd;
-      dd.ct = 1.0; dd.st = 0.0; dd.cphi = 1.0; dd.sphi = 0.0;
-      ev = collision_step(g, s_lv, K, id, nn, pc, false, dd, vx, vy, vz, st, spawn, ch, loss);
+      pc.bin = b;
+      const int r = decide(g, __ldg(g.tab + b), b, u2, pc.xr);
+      if (r < 0) ev = -1;
+      else {
+        double loss;
+        pc.lsel = r;
+        ev = collision_step(g, s_lv, K, id, nn, pc, false, dd, vx, vy, vz, st, spawn, ch, loss);
+      }
     }
   }
   // state after the step in (energy, direction) form
@@ -743,6 +622,82 @@ __global__ void step_batch_kernel(const __grid_constant__ DevGas g, const __grid
     child[5 * n + i] = ckx; child[6 * n + i] = cky; child[7 * n + i] = ckz;
     child_id[i] = child_id_of(K, id, nn - 1u);
   }
+}
+
+// FORM 2: one time-parallel batch (tp_batch, avm_forms.cuh) per warp, k electrons per warp on scattered lanes.  Entry
+// i * gl + s of the outputs = step s of electron i, gl = 32 / k' steps per batch; entries the batch does not reach (the
+// electron finished earlier) keep what the caller put there.
+template <bool HASB>
+__global__ void __launch_bounds__(128)
+step_form_tp_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevField f, const uint64_t seed, const double t_max,
+                    const int64_t n, const int k, const double* __restrict__ in, const uint64_t* __restrict__ ids,
+                    const uint32_t* __restrict__ n_idx, double* __restrict__ out, int32_t* __restrict__ event,
+                    int32_t* __restrict__ status, int32_t* __restrict__ bin, double* __restrict__ child,
+                    uint64_t* __restrict__ child_id) {
+  __shared__ LevelPar s_lv[AVM_MAX_LEVELS];
+  __shared__ double2 s_logtab[128];
+  __shared__ WarpBuf s_wb[4];
+  __shared__ long long s_gidx[4][16];
+  stage_levels(g, s_lv);
+  for (int j = threadIdx.x; j < 128; j += blockDim.x)
+    s_logtab[j] = make_double2(__longlong_as_double((long long)kLogTab[j].rc), __longlong_as_double((long long)kLogTab[j].L));
+  __syncthreads();
+  const PhiloxKeys K = philox_keys(seed);
+  const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+  const int64_t w = (int64_t)blockIdx.x * 4 + warp;
+  int j = -1;
+  for (int q = 0; q < k; ++q) if ((unsigned)((37 * q + 5) & 31) == lane) j = q;   // electron q of the warp sits on lane (37 q + 5) mod 32
+  const int64_t i = w * k + j;
+  const bool have = j >= 0 && i < n;
+  double x = 0, y = 0, z = 0, t = 0, vx = 0, vy = 0, vz = 0;
+  uint64_t id = 0;
+  uint32_t nn = 0, slot = 0;
+  if (have) {
+    x = in[i]; y = in[n + i]; z = in[2 * n + i]; t = in[3 * n + i];
+    const double sp = kC2 * sqrt(in[4 * n + i]);
+    vx = sp * in[5 * n + i]; vy = sp * in[6 * n + i]; vz = sp * in[7 * n + i];
+    id = ids[i]; nn = n_idx[i];
+  }
+  const unsigned act = __ballot_sync(0xFFFFFFFFu, have);
+  if (act == 0u) return;
+  const int lg = 32 - __clz(__popc(act) - 1), gl = 32 >> lg;
+  const int64_t N = n * gl;
+  if (have) s_gidx[warp][__popc(act & ((1u << lane) - 1u))] = i;
+  __syncwarp();
+  Tally tl;
+  auto collide = [&](bool pend, const Pending& pc, bool have_d, const Deflection& dd, int& fin) -> int {
+    int l = -1;
+    if (pend) {
+      double loss;
+      int st;
+      bool spawn;
+      Child ch;
+      ch.e = 0.0; ch.u6 = 0.5; ch.u7 = 0.0;
+      l = collision_step(g, s_lv, K, id, nn, pc, have_d, dd, vx, vy, vz, st, spawn, ch, loss);
+      if (st) fin = st;
+      if (spawn) {
+        const int64_t o = s_gidx[warp][lane & ((1u << lg) - 1u)] * gl + (lane >> lg);
+        double ckx, cky, ckz;
+        child_direction(ch.u6, ch.u7, ckx, cky, ckz);
+        child[o] = x; child[N + o] = y; child[2 * N + o] = z; child[3 * N + o] = t; child[4 * N + o] = ch.e;
+        child[5 * N + o] = ckx; child[6 * N + o] = cky; child[7 * N + o] = ckz;
+        child_id[o] = child_id_of(K, id, nn - 1u);
+      }
+    }
+    return l;
+  };
+  auto commit = [&](bool on, int e, int sidx, int ev, int b, int fin) {
+    if (!on) return;
+    const int64_t o = s_gidx[warp][e] * gl + sidx;
+    const double s2 = vx * vx + vy * vy + vz * vz;
+    double kx = 0.0, ky = 0.0, kz = 1.0;
+    if (s2 > 0.0) { const double inv = rsqrt(s2); kx = vx * inv; ky = vy * inv; kz = vz * inv; }
+    out[o] = x; out[N + o] = y; out[2 * N + o] = z; out[3 * N + o] = t; out[4 * N + o] = fmax(s2 * kInvC2Sq, kEpsFloor);
+    out[5 * N + o] = kx; out[6 * N + o] = ky; out[7 * N + o] = kz;
+    event[o] = ev; status[o] = fin; bin[o] = b < 0 ? -1 : b;
+  };
+  tp_batch<true, HASB, true>(g, f, K, g.tab, s_lv, s_logtab, &s_wb[warp], t_max, lane, act, have, x, y, z, t, vx, vy, vz, id, nn,
+                             slot, tl, collide, commit);
 }
 
 __global__ void field_eval_kernel(const __grid_constant__ DevField f, const int64_t n, const double* __restrict__ r,
@@ -1235,19 +1190,37 @@ int32_t avm_fetch(avm_ctx* ctx, const avm_outputs* dev, int64_t n, int64_t np, i
   return AVM_OK;
 }
 
-int32_t avm_step_batch(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, uint64_t seed, double t_max, int64_t n,
-                       const double* in, const uint64_t* id, const uint32_t* n_idx, double* out, int32_t* event,
-                       int32_t* status, int32_t* bin, double* child, uint64_t* child_id) {
+int32_t avm_step_batch_form(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, uint64_t seed, double t_max, int32_t form,
+                            int32_t k, int64_t n, const double* in, const uint64_t* id, const uint32_t* n_idx, double* out,
+                            int32_t* event, int32_t* status, int32_t* bin, double* child, uint64_t* child_id) {
   if (!ctx || !gas || !field || n < 0) return fail(AVM_ERR_INVALID_ARG, "step_batch: null argument");
+  if (form < 0 || form > 2) return fail(AVM_ERR_INVALID_ARG, "step_batch: form must be 0, 1 or 2");
+  if (form == 2 && (k < 1 || k > 16 || n % k != 0)) return fail(AVM_ERR_INVALID_ARG, "step_batch: form 2 needs 1 <= k <= 16 electrons per warp and n a multiple of k");
+  if (form == 2 && !field->uniform1) return fail(AVM_ERR_INVALID_ARG, "step_batch: form 2 (time-parallel batch) needs a field of one uniform slab");
   if (n == 0) return AVM_OK;
   if (!in || !id || !n_idx || !out || !event || !status || !bin || !child || !child_id) return fail(AVM_ERR_INVALID_ARG, "step_batch: null array");
   AVM_CUDA(cudaSetDevice(ctx->device));
-  const dim3 grid((unsigned)((n + 127) / 128)), block(128);
   const bool u = field->uniform1, b = field->d.has_B != 0;
-#define AVM_SB(U, B) AVM_CUDA(launch(ctx, step_batch_kernel<U, B>, grid, block, gas->d, field->d, seed, t_max, n, in, id, n_idx, out, event, status, bin, child, child_id))
-  if (u && b) AVM_SB(true, true); else if (u) AVM_SB(true, false); else if (b) AVM_SB(false, true); else AVM_SB(false, false);
+  if (form == 2) {
+    const int64_t warps = n / k;
+    const dim3 grid((unsigned)((warps + 3) / 4)), block(128);
+    if (b) AVM_CUDA(launch(ctx, step_form_tp_kernel<true>, grid, block, gas->d, field->d, seed, t_max, n, (int)k, in, id, n_idx, out, event, status, bin, child, child_id));
+    else AVM_CUDA(launch(ctx, step_form_tp_kernel<false>, grid, block, gas->d, field->d, seed, t_max, n, (int)k, in, id, n_idx, out, event, status, bin, child, child_id));
+    return AVM_OK;
+  }
+  const dim3 grid((unsigned)((n + 127) / 128)), block(128);
+#define AVM_SB(U, B, F) AVM_CUDA(launch(ctx, step_batch_kernel<U, B, F>, grid, block, gas->d, field->d, seed, t_max, n, in, id, n_idx, out, event, status, bin, child, child_id))
+#define AVM_SBF(U, B) do { if (form == 1) AVM_SB(U, B, 1); else AVM_SB(U, B, 0); } while (0)
+  if (u && b) AVM_SBF(true, true); else if (u) AVM_SBF(true, false); else if (b) AVM_SBF(false, true); else AVM_SBF(false, false);
+#undef AVM_SBF
 #undef AVM_SB
   return AVM_OK;
+}
+
+int32_t avm_step_batch(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, uint64_t seed, double t_max, int64_t n,
+                       const double* in, const uint64_t* id, const uint32_t* n_idx, double* out, int32_t* event,
+                       int32_t* status, int32_t* bin, double* child, uint64_t* child_id) {
+  return avm_step_batch_form(ctx, gas, field, seed, t_max, 0, 1, n, in, id, n_idx, out, event, status, bin, child, child_id);
 }
 
 int32_t avm_philox_batch(avm_ctx* ctx, uint64_t seed, int64_t n, const uint64_t* id, const uint32_t* n_idx,
