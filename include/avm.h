@@ -86,7 +86,7 @@ double avm_gas_nu_hat(const avm_gas*);
  * laid out [nz][ny][nx][4], trilinear interpolation (x, then y, then z); mask < 0.5 = solid material, the
  * electron is absorbed (R14).  bc 0: leaving the grid in x/y ends the electron (status 3); 1: periodic with
  * the given period; 2: mirror-periodic — fold into [0, period], the field component normal to the mirror
- * changes sign (R15).  B is one constant vector for the whole run (exact helical flight when non-zero).
+ * changes sign (R15).  The map is fp32 storage; all arithmetic on it is fp64.  B is one constant vector for the whole run (exact helical flight when non-zero).
  * xy_lo/xy_hi: absorbing bounds in x and y (+-inf allowed). */
 typedef struct {
   double z_lo, z_hi;
@@ -97,6 +97,10 @@ typedef struct {
   double origin[3], spacing[3];
   int32_t bc_x, bc_y;
   double period_x, period_y;
+  double* nodes_f64_dev;          /* DEVICE scratch or NULL: [nz][ny][nx][4] doubles, 16-byte aligned, borrowed until
+                                   * avm_field_destroy.  When given, avm_field_create widens the fp32 map into it once
+                                   * (same values) and lookups read it: no float-to-double conversion per step, twice
+                                   * the bytes.  Results are identical either way. */
 } avm_slab;
 typedef struct {
   const avm_slab* slabs;          /* host [n_slabs], 1..AVM_MAX_SLABS */
@@ -119,7 +123,7 @@ int32_t avm_field_eval(avm_ctx*, const avm_field*, int64_t n, const double* r, d
  * its birth point with the corresponding status. */
 enum {
   AVM_RUN_PRIMARIES_ON_DEVICE = 1u,
-  AVM_RUN_NO_TALLIES = 2u,
+  AVM_RUN_NO_TALLIES = 2u,        /* accepted for compatibility: the hot loop's tallies are three per-thread counters */
   /* Launch shape of the transport kernel.  Default: chosen from n_primaries (wide when the primaries alone outnumber
    * the lanes of the latency shape).  Results do not depend on the shape. */
   AVM_RUN_SHAPE_WIDE = 4u,        /* 768 threads per SM: most lanes, for runs that keep them busy */
@@ -189,8 +193,10 @@ int32_t avm_step_batch(avm_ctx*, const avm_gas*, const avm_field*, uint64_t seed
  *  form 1: the full-warp form: 16-bit threshold filter + exact record inside a band, the next flight's draws hoisted
  *          behind the record load, deflection drawn in the collision phase.  Arrays of length n.
  *  form 2: one time-parallel batch per warp (one uniform slab only): k electrons per warp (1..16, n a multiple of k) on
- *          scattered lanes, gl = 32 / 2^ceil(log2 k) consecutive steps of each, evaluated as composed flights.  Output
- *          arrays have n * gl entries ([8][n * gl] for states): entry i * gl + s = the result of step s of electron i,
+ *          scattered lanes, gl = 32 / 2^ceil(log2 k) consecutive steps of each, evaluated as composed flights.
+ *  form 3: one serial batch per warp (any field): cooperative draws through shared memory, then every owner lane takes
+ *          its electron's gl steps one after the other in straight-line code.  Same k, gl and layout as form 2.
+ *          For forms 2 and 3 the output arrays have n * gl entries ([8][n * gl] for states): entry i * gl + s = the result of step s of electron i,
  *          in the sense of avm_step_batch (state after the step, event, status, bin, child).  Entries of steps the
  *          electron does not reach (it finished earlier in the batch) are left untouched: pre-fill event with -3.
  * k is ignored for forms 0 and 1. */

@@ -46,7 +46,7 @@ class _Slab(C.Structure):
     _fields_ = [("z_lo", C.c_double), ("z_hi", C.c_double), ("kind", C.c_int32), ("E", C.c_double * 3),
                 ("nodes_dev", C.c_void_p), ("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
                 ("origin", C.c_double * 3), ("spacing", C.c_double * 3), ("bc_x", C.c_int32), ("bc_y", C.c_int32),
-                ("period_x", C.c_double), ("period_y", C.c_double)]
+                ("period_x", C.c_double), ("period_y", C.c_double), ("nodes_f64_dev", C.c_void_p)]
 
 
 class _FieldDesc(C.Structure):
@@ -190,11 +190,14 @@ class Field:
     """avm_field: slab descriptors; grid nodes are uploaded once into torch device tensors kept alive here
     (the one-off field-map transfer the paper excludes from its timings)."""
 
-    def __init__(self, ctx: Context, desc):
+    def __init__(self, ctx: Context, desc, widen: bool = True):
+        """widen: also give the library an fp64 scratch copy of every grid map (avm_slab.nodes_f64_dev): twice the
+        bytes, no float-to-double conversions in the lookup; results are identical."""
         self.ctx = ctx
         n = len(desc.slabs)
         arr = (_Slab * max(n, 1))()
         self.nodes = []
+        self.wide = []
         self.map_bytes = 0
         for i, s in enumerate(desc.slabs):
             a = arr[i]
@@ -209,6 +212,10 @@ class Field:
                 self.map_bytes += t.numel() * 4
                 a.nodes_dev = t.data_ptr()
                 a.nz, a.ny, a.nx = t.shape[:3]
+                if widen:
+                    wd = torch.empty(t.numel(), dtype=torch.float64, device=ctx.device)
+                    self.wide.append(wd)
+                    a.nodes_f64_dev = wd.data_ptr()
             a.origin[:] = s.origin
             a.spacing[:] = s.spacing
             a.bc_x, a.bc_y, a.period_x, a.period_y = s.bc_x, s.bc_y, s.period_x, s.period_y
@@ -224,8 +231,8 @@ class Field:
             pass
 
 
-def field_create(ctx, desc) -> Field:
-    return Field(ctx, desc)
+def field_create(ctx, desc, widen: bool = True) -> Field:
+    return Field(ctx, desc, widen)
 
 
 def field_eval(ctx: Context, field: Field, r):
@@ -267,11 +274,11 @@ def step_form_lanes(k: int) -> int:
 
 def step_batch_form(ctx: Context, gas: Gas, field: Field, seed, state, ids, n_idx, form: int, k: int = 1,
                     t_max=float("inf")) -> StepResult:
-    """avm_step_batch_form.  Forms 0 / 1: as step_batch.  Form 2: arrays get a trailing axis of gl = step_form_lanes(k)
-    steps per electron ([8, n, gl], [n, gl]); steps the batch did not reach have event == -3."""
+    """avm_step_batch_form.  Forms 0 / 1: as step_batch.  Forms 2 / 3: arrays get a trailing axis of gl =
+    step_form_lanes(k) steps per electron ([8, n, gl], [n, gl]); steps the batch did not reach have event == -3."""
     st = torch.from_numpy(np.ascontiguousarray(state, dtype=np.float64)).to(ctx.device)
     n = st.shape[1]
-    gl = step_form_lanes(k) if form == 2 else 1
+    gl = step_form_lanes(k) if form >= 2 else 1
     m = n * gl
     idt = torch.from_numpy(np.ascontiguousarray(ids, dtype=np.uint64).view(np.int64)).to(ctx.device)
     nt = torch.from_numpy(np.ascontiguousarray(n_idx, dtype=np.uint32).view(np.int32)).to(ctx.device)
@@ -285,7 +292,7 @@ def step_batch_form(ctx: Context, gas: Gas, field: Field, seed, state, ids, n_id
                                     _dev(idt), _dev(nt), _dev(out), _dev(ev), _dev(stt), _dev(bn), _dev(ch), _dev(cid)))
     r = StepResult(out.cpu().numpy(), ev.cpu().numpy(), stt.cpu().numpy(), bn.cpu().numpy(), ch.cpu().numpy(),
                    cid.cpu().numpy().view(np.uint64))
-    if form == 2:
+    if form >= 2:
         r = StepResult(r.state.reshape(8, n, gl), r.event.reshape(n, gl), r.status.reshape(n, gl), r.bin.reshape(n, gl),
                        r.child.reshape(8, n, gl), r.child_id.reshape(n, gl))
     return r

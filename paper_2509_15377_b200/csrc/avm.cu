@@ -127,7 +127,10 @@ __device__ __forceinline__ void idle_wait(uint32_t ns) {
 constexpr int kFlights = AVM_FLIGHTS;
 constexpr int kCoopMax = AVM_COOP_MAX;
 
-template <bool UNIFORM1, bool HASB, bool TALLY, bool SMEMTAB, int THREADS, bool TPB>
+#ifndef AVM_SB_UNIFORM
+#define AVM_SB_UNIFORM 0     // 1: serial batches instead of time-parallel ones in one uniform slab without B
+#endif
+template <int FK, bool HASB, bool TALLY, bool SMEMTAB, int THREADS, bool TPB>
 __global__ void __launch_bounds__(THREADS, 1)
 transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevField f, const RunArrays a,
                  RunCtl* __restrict__ ctl, const __grid_constant__ PhiloxKeys K, const double t_max,
@@ -186,7 +189,7 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
           id = __ldcg(a.id + slot);
           n = __ldcg(a.nsteps + slot);
           double m;
-          field_at<UNIFORM1>(f, x, y, z, Ex, Ey, Ez, m);     // S0 of its first step (in-domain by construction)
+          field_at<FK>(f, x, y, z, Ex, Ey, Ez, m);           // S0 of its first step (in-domain by construction)
           have = true; dvalid = false;
           break;
         }
@@ -310,61 +313,19 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
     if ((it & 15u) == 0u && ld_relaxed_s32(done) == 2) { stopped = true; break; }
     const int k = __popc(act);
 
-    if (TPB && UNIFORM1 && k <= kCoopMax) {
+    if (TPB && FK == 1 && (HASB || !AVM_SB_UNIFORM) && k <= kCoopMax) {
       // ---- time-parallel batch (uniform E, optional B): g = 32 / k' lanes per electron (avm_forms.cuh) ----
-      const int fin = tp_batch<UNIFORM1, HASB, TALLY>(g, f, K, tab, s_lv, s_logtab, wb, t_max, lane, act, have, x, y, z, t, vx,
-                                                      vy, vz, id, n, slot, tl, collide_and_append,
-                                                      [](bool, int, int, int, int, int) {});
-      dvalid = false;
-      retire(fin);
-    } else if (k <= kCoopMax) {
-      // ---- cooperative batch ----
-      const int lg = 32 - __clz(k - 1);             // k' = 2^lg >= k  (k = 1: __clz(0) = 32)
-      const int kp = 1 << lg, nb_steps = 32 >> lg;
-      const int rank = __popc(act & lt_mask);
-      if (have) { wb->id[rank] = id; wb->n[rank] = n; }
-      __syncwarp();
-      {
-        const int e = (int)lane & (kp - 1), s = (int)lane >> lg;
-        if (e < k) {
-          const uint64_t hid = wb->id[e];
-          const uint32_t hn = wb->n[e] + (uint32_t)s;
-          double ddt;
-          uint2 du2;
-          draw_flight(g, K, s_logtab, hid, hn, ddt, du2);
-          const Deflection d = deflection_draws(K, hid, hn);
-          wb->dt[lane] = ddt; wb->u2w[lane] = du2;
-          wb->ct[lane] = d.ct; wb->st[lane] = d.st; wb->cphi[lane] = d.cphi; wb->sphi[lane] = d.sphi;
-        }
-      }
-      __syncwarp();
-      dvalid = false;
-#pragma unroll 1
-      for (int s = 0; s < nb_steps; ++s) {
-        int fin = 0;
-        bool pend = false;
-        Pending pc;
-        pc.lsel = 0; pc.bin = 0; pc.xr = 0.0;
-        Deflection dd;
-        dd.ct = 1.0; dd.st = 0.0; dd.cphi = 1.0; dd.sphi = 0.0;
-        if (have) {
-          const int idx = s * kp + rank;
-          bool over = false;
-          const int b = advance<UNIFORM1, HASB>(g, f, t_max, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, wb->dt[idx], over);
-          if (b < 0) fin = -b;
-          else {
-            const int r = decide(g, tab[b], b, wb->u2w[idx], pc.xr);
-            if (r >= 0) {
-              pend = true; pc.lsel = r; pc.bin = b;
-              dd.ct = wb->ct[idx]; dd.st = wb->st[idx]; dd.cphi = wb->cphi[idx]; dd.sphi = wb->sphi[idx];
-            }
-            if (TALLY && over) ++tl.over;
-          }
-        }
-        if (__any_sync(0xFFFFFFFFu, pend)) collide_and_append(pend, pc, true, dd, fin);
+      if constexpr (FK == 1) {
+        const int fin = tp_batch<FK, HASB, TALLY>(g, f, K, tab, s_lv, s_logtab, wb, t_max, lane, act, have, x, y, z, t, vx, vy, vz,
+                                                  id, n, slot, tl, collide_and_append, [](bool, int, int, int, int, int) {});
+        dvalid = false;
         retire(fin);
-        if (!__any_sync(0xFFFFFFFFu, have)) break;
       }
+    } else if (k <= kCoopMax) {
+      // ---- serial batch: cooperative draws, then every owner lane walks its electron's steps alone (avm_forms.cuh) ----
+      sb_batch<FK, HASB, TALLY>(g, f, K, tab, s_logtab, wb, t_max, lane, act, have, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, id, n, tl,
+                                collide_and_append, retire, [](int, int, int, int, int) {});
+      dvalid = false;
     } else {
       // ---- full warp ----
       if (have && !dvalid) { draw_flight(g, K, s_logtab, id, n, dt, u2w); dvalid = true; }
@@ -375,7 +336,7 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
 #pragma unroll
       for (int fl = 0; fl < kFlights; ++fl) {
         if (have && !pend && fin == 0)
-          fw_flight<UNIFORM1, HASB, TALLY>(g, f, K, tab, s_logtab, t_max, id, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt, u2w, fin,
+          fw_flight<FK, HASB, TALLY>(g, f, K, tab, s_logtab, t_max, id, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt, u2w, fin,
                                            pend, pc, tl);
       }
       Deflection dd;
@@ -425,7 +386,7 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
 }
 
 // ---- primary injection (a-1) -----------------------------------------------------------------------------
-template <bool UNIFORM1>
+template <int FK>
 __global__ void inject_kernel(const __grid_constant__ DevField f, const RunArrays a, RunCtl* ctl,
                               const double* __restrict__ prim, const uint32_t p0, const uint32_t count,
                               const uint64_t id_offset, const double t_max) {
@@ -440,7 +401,7 @@ __global__ void inject_kernel(const __grid_constant__ DevField f, const RunArray
     const double nk = sqrt(kx * kx + ky * ky + kz * kz);
     if (!(nk > 0.0)) { kx = 0.0; ky = 0.0; kz = 1.0; } else { kx /= nk; ky /= nk; kz /= nk; }
     double Ex, Ey, Ez, m = 1.0;
-    const int si = field_at<UNIFORM1>(f, x, y, z, Ex, Ey, Ez, m);
+    const int si = field_at<FK>(f, x, y, z, Ex, Ey, Ez, m);
     int st = 0;
     if (si < 0) st = -si;
     else if (m < 0.5) st = AVM_MATERIAL;
@@ -536,7 +497,7 @@ __global__ void publish_kernel(const RunCtl* ctl, const int L, unsigned long lon
 // FORM 0: the general sequence draw_flight -> advance -> decide -> collision_step.  FORM 1: the full-warp form of the
 // transport kernel — fw_flight (avm_forms.cuh: advance, decide_filter / decide_exact, the next flight's draws hoisted
 // behind the record load) and the collision phase with the deflection drawn there.
-template <bool UNIFORM1, bool HASB, int FORM>
+template <int FK, bool HASB, int FORM>
 __global__ void step_batch_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevField f,
                                   const uint64_t seed, const double t_max, const int64_t n,
                                   const double* __restrict__ in, const uint64_t* __restrict__ ids,
@@ -560,7 +521,7 @@ __global__ void step_batch_kernel(const __grid_constant__ DevGas g, const __grid
   for (int c = 0; c < 8; ++c) child[c * n + i] = 0.0;
   child_id[i] = 0ull;
   double Ex, Ey, Ez, m;
-  const int si = field_at<UNIFORM1>(f, x, y, z, Ex, Ey, Ez, m);     // S0
+  const int si = field_at<FK>(f, x, y, z, Ex, Ey, Ez, m);     // S0
   if (si < 0) {                                                     // caller error: reported as a status
     for (int c = 0; c < 8; ++c) out[c * n + i] = in[c * n + i];
     event[i] = -2; status[i] = -si; bin[i] = -1;
@@ -581,7 +542,7 @@ __global__ void step_batch_kernel(const __grid_constant__ DevGas g, const __grid
   if (FORM == 1) {
     bool pend = false;
     Tally tl;
-    fw_flight<UNIFORM1, HASB, true>(g, f, K, g.tab, s_logtab, t_max, id, nn, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt, u2, st, pend,
+    fw_flight<FK, HASB, true>(g, f, K, g.tab, s_logtab, t_max, id, nn, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt, u2, st, pend,
                                     pc, tl);
     over = tl.over != 0u;
     if (st == 0) {
@@ -595,7 +556,7 @@ __global__ void step_batch_kernel(const __grid_constant__ DevGas g, const __grid
       }
     }
   } else {
-    const int b = advance<UNIFORM1, HASB>(g, f, t_max, nn, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt, over);
+    const int b = advance<FK, HASB>(g, f, t_max, nn, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt, over);
     if (b < 0) st = -b;
     else {
       pc.bin = b;
@@ -624,16 +585,16 @@ __global__ void step_batch_kernel(const __grid_constant__ DevGas g, const __grid
   }
 }
 
-// FORM 2: one time-parallel batch (tp_batch, avm_forms.cuh) per warp, k electrons per warp on scattered lanes.  Entry
-// i * gl + s of the outputs = step s of electron i, gl = 32 / k' steps per batch; entries the batch does not reach (the
-// electron finished earlier) keep what the caller put there.
-template <bool HASB>
+// FORMS 2 and 3: one batch per warp — a time-parallel batch (tp_batch) or a serial batch (sb_batch) of avm_forms.cuh — with
+// k electrons per warp on scattered lanes.  Entry i * gl + s of the outputs = step s of electron i, gl = 32 / k' steps per
+// batch; entries the batch does not reach (the electron finished earlier) keep what the caller put there.
+template <int FK, bool HASB, int FORM>
 __global__ void __launch_bounds__(128)
-step_form_tp_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevField f, const uint64_t seed, const double t_max,
-                    const int64_t n, const int k, const double* __restrict__ in, const uint64_t* __restrict__ ids,
-                    const uint32_t* __restrict__ n_idx, double* __restrict__ out, int32_t* __restrict__ event,
-                    int32_t* __restrict__ status, int32_t* __restrict__ bin, double* __restrict__ child,
-                    uint64_t* __restrict__ child_id) {
+step_form_batch_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevField f, const uint64_t seed,
+                       const double t_max, const int64_t n, const int k, const double* __restrict__ in,
+                       const uint64_t* __restrict__ ids, const uint32_t* __restrict__ n_idx, double* __restrict__ out,
+                       int32_t* __restrict__ event, int32_t* __restrict__ status, int32_t* __restrict__ bin,
+                       double* __restrict__ child, uint64_t* __restrict__ child_id) {
   __shared__ LevelPar s_lv[AVM_MAX_LEVELS];
   __shared__ double2 s_logtab[128];
   __shared__ WarpBuf s_wb[4];
@@ -648,8 +609,8 @@ step_form_tp_kernel(const __grid_constant__ DevGas g, const __grid_constant__ De
   int j = -1;
   for (int q = 0; q < k; ++q) if ((unsigned)((37 * q + 5) & 31) == lane) j = q;   // electron q of the warp sits on lane (37 q + 5) mod 32
   const int64_t i = w * k + j;
-  const bool have = j >= 0 && i < n;
-  double x = 0, y = 0, z = 0, t = 0, vx = 0, vy = 0, vz = 0;
+  bool have = j >= 0 && i < n;
+  double x = 0, y = 0, z = 0, t = 0, vx = 0, vy = 0, vz = 0, Ex = 0, Ey = 0, Ez = 0;
   uint64_t id = 0;
   uint32_t nn = 0, slot = 0;
   if (have) {
@@ -657,14 +618,19 @@ step_form_tp_kernel(const __grid_constant__ DevGas g, const __grid_constant__ De
     const double sp = kC2 * sqrt(in[4 * n + i]);
     vx = sp * in[5 * n + i]; vy = sp * in[6 * n + i]; vz = sp * in[7 * n + i];
     id = ids[i]; nn = n_idx[i];
+    double m;
+    field_at<FK>(f, x, y, z, Ex, Ey, Ez, m);                                       // S0 of the first step (in-domain: caller's duty)
   }
   const unsigned act = __ballot_sync(0xFFFFFFFFu, have);
   if (act == 0u) return;
   const int lg = 32 - __clz(__popc(act) - 1), gl = 32 >> lg;
   const int64_t N = n * gl;
-  if (have) s_gidx[warp][__popc(act & ((1u << lane) - 1u))] = i;
+  const int rank = __popc(act & ((1u << lane) - 1u));
+  if (have) s_gidx[warp][rank] = i;
   __syncwarp();
   Tally tl;
+  // the output entry a lane is working on: tp_batch gives lane (e, sidx) one step; sb_batch gives the owner lane all steps
+  int64_t o_cur = 0;
   auto collide = [&](bool pend, const Pending& pc, bool have_d, const Deflection& dd, int& fin) -> int {
     int l = -1;
     if (pend) {
@@ -676,7 +642,7 @@ step_form_tp_kernel(const __grid_constant__ DevGas g, const __grid_constant__ De
       l = collision_step(g, s_lv, K, id, nn, pc, have_d, dd, vx, vy, vz, st, spawn, ch, loss);
       if (st) fin = st;
       if (spawn) {
-        const int64_t o = s_gidx[warp][lane & ((1u << lg) - 1u)] * gl + (lane >> lg);
+        const int64_t o = FORM == 2 ? s_gidx[warp][lane & ((1u << lg) - 1u)] * gl + (lane >> lg) : o_cur;
         double ckx, cky, ckz;
         child_direction(ch.u6, ch.u7, ckx, cky, ckz);
         child[o] = x; child[N + o] = y; child[2 * N + o] = z; child[3 * N + o] = t; child[4 * N + o] = ch.e;
@@ -686,8 +652,7 @@ step_form_tp_kernel(const __grid_constant__ DevGas g, const __grid_constant__ De
     }
     return l;
   };
-  auto commit = [&](bool on, int e, int sidx, int ev, int b, int fin) {
-    if (!on) return;
+  auto record = [&](int e, int sidx, int ev, int b, int fin) {
     const int64_t o = s_gidx[warp][e] * gl + sidx;
     const double s2 = vx * vx + vy * vy + vz * vz;
     double kx = 0.0, ky = 0.0, kz = 1.0;
@@ -696,8 +661,26 @@ step_form_tp_kernel(const __grid_constant__ DevGas g, const __grid_constant__ De
     out[5 * N + o] = kx; out[6 * N + o] = ky; out[7 * N + o] = kz;
     event[o] = ev; status[o] = fin; bin[o] = b < 0 ? -1 : b;
   };
-  tp_batch<true, HASB, true>(g, f, K, g.tab, s_lv, s_logtab, &s_wb[warp], t_max, lane, act, have, x, y, z, t, vx, vy, vz, id, nn,
-                             slot, tl, collide, commit);
+  if constexpr (FORM == 2) {
+    tp_batch<FK, HASB, true>(g, f, K, g.tab, s_lv, s_logtab, &s_wb[warp], t_max, lane, act, have, x, y, z, t, vx, vy, vz, id, nn,
+                             slot, tl, collide, [&](bool on, int e, int sidx, int ev, int b, int fin) { if (on) record(e, sidx, ev, b, fin); });
+  } else {
+    // sb_batch calls commit AFTER a step; the child of a collision is recorded inside collide, before the commit of the
+    // same step: o_cur is kept one step ahead (the owner lane's next output entry)
+    o_cur = have ? i * gl : 0;
+    sb_batch<FK, HASB, true>(g, f, K, g.tab, s_logtab, &s_wb[warp], t_max, lane, act, have, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, id,
+                             nn, tl, collide, [&](int fin) { if (fin != 0) have = false; },
+                             [&](int e, int sidx, int ev, int b, int fin) { record(e, sidx, ev, b, fin); o_cur = s_gidx[warp][e] * gl + sidx + 1; });
+  }
+}
+
+// Widened copy of a grid map: node i's float4 (Ex, Ey, Ez, mask) -> four doubles, exactly (avm_slab.nodes_f64_dev).
+__global__ void widen_map_kernel(const float4* __restrict__ in, double2* __restrict__ out, const size_t n_nodes) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_nodes; i += (size_t)gridDim.x * blockDim.x) {
+    const float4 v = __ldg(in + i);
+    out[2 * i] = make_double2((double)v.x, (double)v.y);
+    out[2 * i + 1] = make_double2((double)v.z, (double)v.w);
+  }
 }
 
 __global__ void field_eval_kernel(const __grid_constant__ DevField f, const int64_t n, const double* __restrict__ r,
@@ -751,6 +734,7 @@ struct avm_gas {
 };
 struct avm_field {
   DevField d{};
+  int fk = 0;                 // 1 = one uniform slab, 2 = one grid slab, 0 = any other stack (template parameter FK)
   bool uniform1 = false;
 };
 
@@ -958,6 +942,8 @@ int32_t avm_field_create(avm_ctx* ctx, const avm_field_desc* d, avm_field** out)
         if (s.bc_y && !(s.period_y > 0 && s.period_y <= (s.ny - 1) * s.spacing[1] * (1 + 1e-12))) bad = "field: period_y";
       }
       S.nodes = (const float4*)s.nodes_dev;
+      S.nodes64 = s.nodes_f64_dev;
+      if (!bad && s.nodes_f64_dev && ((uintptr_t)s.nodes_f64_dev & 15u)) bad = "field: nodes_f64_dev not 16-byte aligned";
       S.nx = s.nx; S.ny = s.ny; S.nz = s.nz;
       const int bc[2] = {s.bc_x, s.bc_y};
       const double per[2] = {s.period_x, s.period_y};
@@ -989,7 +975,20 @@ int32_t avm_field_create(avm_ctx* ctx, const avm_field_desc* d, avm_field** out)
     F.omega = kOmega1 * Bn;
     F.inv_omega = 1.0 / F.omega;
   }
+  for (int i = 0; i < d->n_slabs; ++i) {           // widen the grid maps once (the one-off field transfer)
+    const DevSlab& S = F.slab[i];
+    if (S.kind != 1 || !S.nodes64) continue;
+    const size_t nn = (size_t)S.nx * S.ny * S.nz;
+    cudaError_t e = cudaSetDevice(ctx->device);
+    if (e == cudaSuccess) {
+      widen_map_kernel<<<(unsigned)ctx->sm_count * 8u, 256, 0, ctx->stream>>>(S.nodes, (double2*)S.nodes64, nn);
+      e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) { delete f; return fail(AVM_ERR_CUDA, std::string("field_create: widening the map: ") + cudaGetErrorString(e)); }
+  }
   f->uniform1 = d->n_slabs == 1 && d->slabs[0].kind == 0;
+  f->fk = f->uniform1 ? 1 : (d->n_slabs == 1 ? 2 : 0);
   F.xy_bounded = 0;
   for (int a = 0; a < 2; ++a)
     if (std::isfinite(F.xy_lo[a]) || std::isfinite(F.xy_hi[a]) || F.xy_lo[a] != F.xy_lo[a] || F.xy_hi[a] != F.xy_hi[a]) F.xy_bounded = 1;
@@ -1044,18 +1043,19 @@ int32_t avm_run_transport_ms(const avm_ctx* c, float* ms_out) {
 namespace {
 typedef void (*TransportFn)(const DevGas, const DevField, const RunArrays, RunCtl*, const PhiloxKeys, const double,
                             const uint32_t, const uint32_t);
-template <bool U, bool B, int T, bool TPB>
-TransportFn pick3(bool tally, bool smemtab) {
-  if (tally) return smemtab ? transport_kernel<U, B, true, true, T, TPB> : transport_kernel<U, B, true, false, T, TPB>;
-  return smemtab ? transport_kernel<U, B, false, true, T, TPB> : transport_kernel<U, B, false, false, T, TPB>;
+// Tallies are always kept in the hot loop (three per-thread counters); AVM_RUN_NO_TALLIES only skips their publication.
+template <int FK, bool B, int T, bool TPB>
+TransportFn pick3(bool smemtab) {
+  return smemtab ? transport_kernel<FK, B, true, true, T, TPB> : transport_kernel<FK, B, true, false, T, TPB>;
 }
-template <bool U, bool B>
-TransportFn pick2(bool tally, bool smemtab, bool wide) {
-  return wide ? pick3<U, B, kThreadsWide, false>(tally, smemtab) : pick3<U, B, kThreads, true>(tally, smemtab);
+template <int FK, bool B>
+TransportFn pick2(bool smemtab, bool wide) {
+  return wide ? pick3<FK, B, kThreadsWide, false>(smemtab) : pick3<FK, B, kThreads, true>(smemtab);
 }
-TransportFn pick_transport(bool uniform1, bool has_b, bool tally, bool smemtab, bool wide) {
-  if (uniform1) return has_b ? pick2<true, true>(tally, smemtab, wide) : pick2<true, false>(tally, smemtab, wide);
-  return has_b ? pick2<false, true>(tally, smemtab, wide) : pick2<false, false>(tally, smemtab, wide);
+TransportFn pick_transport(int fk, bool has_b, bool smemtab, bool wide) {
+  if (fk == 1) return has_b ? pick2<1, true>(smemtab, wide) : pick2<1, false>(smemtab, wide);
+  if (fk == 2) return has_b ? pick2<2, true>(smemtab, wide) : pick2<2, false>(smemtab, wide);
+  return has_b ? pick2<0, true>(smemtab, wide) : pick2<0, false>(smemtab, wide);
 }
 }  // namespace
 
@@ -1079,7 +1079,6 @@ int32_t avm_run(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, const 
   RunArrays a;
   a.cap = (uint32_t)o->capacity; a.id = o->id; a.aval = o->avalanche; a.status = o->status; a.nsteps = o->n_steps;
   a.birth = o->birth; a.end = o->end;
-  const bool tally = !(opts->flags & AVM_RUN_NO_TALLIES);
   const bool on_dev = opts->flags & AVM_RUN_PRIMARIES_ON_DEVICE;
 
   AVM_CUDA(cudaMemsetAsync(ctl, 0, kCtlBytes, st));
@@ -1094,8 +1093,8 @@ int32_t avm_run(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, const 
       src = stage;
     }
     const dim3 grid((unsigned)((cnt + 255) / 256));
-    if (field->uniform1) AVM_CUDA(launch(ctx, inject_kernel<true>, grid, dim3(256), field->d, a, ctl, src, (uint32_t)p0, (uint32_t)cnt, opts->id_offset, opts->t_max));
-    else AVM_CUDA(launch(ctx, inject_kernel<false>, grid, dim3(256), field->d, a, ctl, src, (uint32_t)p0, (uint32_t)cnt, opts->id_offset, opts->t_max));
+    if (field->uniform1) AVM_CUDA(launch(ctx, inject_kernel<1>, grid, dim3(256), field->d, a, ctl, src, (uint32_t)p0, (uint32_t)cnt, opts->id_offset, opts->t_max));
+    else AVM_CUDA(launch(ctx, inject_kernel<0>, grid, dim3(256), field->d, a, ctl, src, (uint32_t)p0, (uint32_t)cnt, opts->id_offset, opts->t_max));
   }
   // persistent transport (a-2 .. a-11)
   bool wide = np > (int64_t)ctx->sm_count * kThreads;            // the primaries alone outnumber the latency shape's lanes
@@ -1106,7 +1105,7 @@ int32_t avm_run(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, const 
   const size_t tab_bytes = align_up(sizeof(ushort4) * (size_t)gas->d.nb, 16);
   const bool smemtab = tab_bytes + buf_bytes <= kMaxDynSmem;       // else the threshold table is read through L1
   const size_t dyn_smem = (smemtab ? tab_bytes : 0) + buf_bytes;
-  TransportFn fn = pick_transport(field->uniform1, field->d.has_B != 0, tally, smemtab, wide);
+  TransportFn fn = pick_transport(field->fk, field->d.has_B != 0, smemtab, wide);
   AVM_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn_smem));
   int occ = 0;
   AVM_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, threads, dyn_smem));
@@ -1194,26 +1193,37 @@ int32_t avm_step_batch_form(avm_ctx* ctx, const avm_gas* gas, const avm_field* f
                             int32_t k, int64_t n, const double* in, const uint64_t* id, const uint32_t* n_idx, double* out,
                             int32_t* event, int32_t* status, int32_t* bin, double* child, uint64_t* child_id) {
   if (!ctx || !gas || !field || n < 0) return fail(AVM_ERR_INVALID_ARG, "step_batch: null argument");
-  if (form < 0 || form > 2) return fail(AVM_ERR_INVALID_ARG, "step_batch: form must be 0, 1 or 2");
-  if (form == 2 && (k < 1 || k > 16 || n % k != 0)) return fail(AVM_ERR_INVALID_ARG, "step_batch: form 2 needs 1 <= k <= 16 electrons per warp and n a multiple of k");
+  if (form < 0 || form > 3) return fail(AVM_ERR_INVALID_ARG, "step_batch: form must be 0, 1, 2 or 3");
+  if (form >= 2 && (k < 1 || k > 16 || n % k != 0)) return fail(AVM_ERR_INVALID_ARG, "step_batch: forms 2 and 3 need 1 <= k <= 16 electrons per warp and n a multiple of k");
   if (form == 2 && !field->uniform1) return fail(AVM_ERR_INVALID_ARG, "step_batch: form 2 (time-parallel batch) needs a field of one uniform slab");
   if (n == 0) return AVM_OK;
   if (!in || !id || !n_idx || !out || !event || !status || !bin || !child || !child_id) return fail(AVM_ERR_INVALID_ARG, "step_batch: null array");
   AVM_CUDA(cudaSetDevice(ctx->device));
-  const bool u = field->uniform1, b = field->d.has_B != 0;
+  const int fk = field->fk;
+  const bool b = field->d.has_B != 0;
+#define AVM_ARGS gas->d, field->d, seed, t_max, n, in, id, n_idx, out, event, status, bin, child, child_id
+#define AVM_BARGS gas->d, field->d, seed, t_max, n, (int)k, in, id, n_idx, out, event, status, bin, child, child_id
   if (form == 2) {
-    const int64_t warps = n / k;
-    const dim3 grid((unsigned)((warps + 3) / 4)), block(128);
-    if (b) AVM_CUDA(launch(ctx, step_form_tp_kernel<true>, grid, block, gas->d, field->d, seed, t_max, n, (int)k, in, id, n_idx, out, event, status, bin, child, child_id));
-    else AVM_CUDA(launch(ctx, step_form_tp_kernel<false>, grid, block, gas->d, field->d, seed, t_max, n, (int)k, in, id, n_idx, out, event, status, bin, child, child_id));
-    return AVM_OK;
-  }
-  const dim3 grid((unsigned)((n + 127) / 128)), block(128);
-#define AVM_SB(U, B, F) AVM_CUDA(launch(ctx, step_batch_kernel<U, B, F>, grid, block, gas->d, field->d, seed, t_max, n, in, id, n_idx, out, event, status, bin, child, child_id))
-#define AVM_SBF(U, B) do { if (form == 1) AVM_SB(U, B, 1); else AVM_SB(U, B, 0); } while (0)
-  if (u && b) AVM_SBF(true, true); else if (u) AVM_SBF(true, false); else if (b) AVM_SBF(false, true); else AVM_SBF(false, false);
-#undef AVM_SBF
+    const dim3 grid((unsigned)((n / k + 3) / 4)), block(128);
+    if (b) AVM_CUDA(launch(ctx, step_form_batch_kernel<1, true, 2>, grid, block, AVM_BARGS));
+    else AVM_CUDA(launch(ctx, step_form_batch_kernel<1, false, 2>, grid, block, AVM_BARGS));
+  } else if (form == 3) {
+    const dim3 grid((unsigned)((n / k + 3) / 4)), block(128);
+#define AVM_F3(FK) do { if (b) AVM_CUDA(launch(ctx, step_form_batch_kernel<FK, true, 3>, grid, block, AVM_BARGS)); \
+                        else AVM_CUDA(launch(ctx, step_form_batch_kernel<FK, false, 3>, grid, block, AVM_BARGS)); } while (0)
+    if (fk == 1) AVM_F3(1); else if (fk == 2) AVM_F3(2); else AVM_F3(0);
+#undef AVM_F3
+  } else {
+    const dim3 grid((unsigned)((n + 127) / 128)), block(128);
+#define AVM_SB(FK, B) do { if (form == 1) AVM_CUDA(launch(ctx, step_batch_kernel<FK, B, 1>, grid, block, AVM_ARGS)); \
+                           else AVM_CUDA(launch(ctx, step_batch_kernel<FK, B, 0>, grid, block, AVM_ARGS)); } while (0)
+#define AVM_SBK(FK) do { if (b) AVM_SB(FK, true); else AVM_SB(FK, false); } while (0)
+    if (fk == 1) AVM_SBK(1); else if (fk == 2) AVM_SBK(2); else AVM_SBK(0);
+#undef AVM_SBK
 #undef AVM_SB
+  }
+#undef AVM_ARGS
+#undef AVM_BARGS
   return AVM_OK;
 }
 

@@ -44,6 +44,7 @@ struct DevSlab {
   double Pc[2], lo[2];                // rounding guard q >= Pc || q < lo -> 0 (none: +inf, -inf; else P, 0)
   double half[2];                     // mirror: P (reflect when q > half); else +inf
   const float4* nodes;
+  const double* nodes64;              // optional widened copy [nz][ny][nx][4] (same values as doubles): no conversions per lookup
   int kind, nx, ny, nz, bc[2];
 };
 
@@ -209,6 +210,9 @@ __device__ __forceinline__ double lerp3(double c000, double c100, double c010, d
 }
 
 // Grid lookup inside slab s (z already known to lie in the slab).  Returns false when x/y leave a bc-none grid.
+// Nodes come from the widened fp64 copy of the map when the caller gave one (avm_slab.nodes_f64_dev): two 16-byte loads
+// per node and no float-to-double conversions (32 per lookup otherwise, 8 cycles of the conversion pipe each); the values
+// are the same doubles either way.
 __device__ __forceinline__ bool grid_at(const DevSlab& s, double x, double y, double z, double& Ex, double& Ey,
                                         double& Ez, double& mask) {
   double qx, qy;
@@ -220,23 +224,40 @@ __device__ __forceinline__ bool grid_at(const DevSlab& s, double x, double y, do
   cell_of(qx * s.inv_h[0], s.nx, i, wx);
   cell_of(qy * s.inv_h[1], s.ny, j, wy);
   cell_of((z - s.org[2]) * s.inv_h[2], s.nz, k, wz);
-  const float4* p = s.nodes + ((size_t)k * s.ny + j) * s.nx + i;
   const size_t sy = (size_t)s.nx, sz = (size_t)s.nx * s.ny;
-  const float4 n000 = __ldg(p), n100 = __ldg(p + 1);
-  const float4 n010 = __ldg(p + sy), n110 = __ldg(p + sy + 1);
-  const float4 n001 = __ldg(p + sz), n101 = __ldg(p + sz + 1);
-  const float4 n011 = __ldg(p + sz + sy), n111 = __ldg(p + sz + sy + 1);
-  const double ex = lerp3(f2d(n000.x), f2d(n100.x), f2d(n010.x), f2d(n110.x), f2d(n001.x), f2d(n101.x), f2d(n011.x), f2d(n111.x), wx, wy, wz);
-  const double ey = lerp3(f2d(n000.y), f2d(n100.y), f2d(n010.y), f2d(n110.y), f2d(n001.y), f2d(n101.y), f2d(n011.y), f2d(n111.y), wx, wy, wz);
-  Ez = lerp3(f2d(n000.z), f2d(n100.z), f2d(n010.z), f2d(n110.z), f2d(n001.z), f2d(n101.z), f2d(n011.z), f2d(n111.z), wx, wy, wz);
-  mask = lerp3(f2d(n000.w), f2d(n100.w), f2d(n010.w), f2d(n110.w), f2d(n001.w), f2d(n101.w), f2d(n011.w), f2d(n111.w), wx, wy, wz);
+  const size_t o = ((size_t)k * s.ny + j) * s.nx + i;
+  double ex, ey;
+  if (s.nodes64) {
+    const double2* p = reinterpret_cast<const double2*>(s.nodes64) + 2 * o;
+    const double2 a000 = __ldg(p), b000 = __ldg(p + 1), a100 = __ldg(p + 2), b100 = __ldg(p + 3);
+    const double2 a010 = __ldg(p + 2 * sy), b010 = __ldg(p + 2 * sy + 1), a110 = __ldg(p + 2 * sy + 2), b110 = __ldg(p + 2 * sy + 3);
+    const double2 a001 = __ldg(p + 2 * sz), b001 = __ldg(p + 2 * sz + 1), a101 = __ldg(p + 2 * sz + 2), b101 = __ldg(p + 2 * sz + 3);
+    const double2 a011 = __ldg(p + 2 * (sz + sy)), b011 = __ldg(p + 2 * (sz + sy) + 1), a111 = __ldg(p + 2 * (sz + sy) + 2),
+                  b111 = __ldg(p + 2 * (sz + sy) + 3);
+    ex = lerp3(a000.x, a100.x, a010.x, a110.x, a001.x, a101.x, a011.x, a111.x, wx, wy, wz);
+    ey = lerp3(a000.y, a100.y, a010.y, a110.y, a001.y, a101.y, a011.y, a111.y, wx, wy, wz);
+    Ez = lerp3(b000.x, b100.x, b010.x, b110.x, b001.x, b101.x, b011.x, b111.x, wx, wy, wz);
+    mask = lerp3(b000.y, b100.y, b010.y, b110.y, b001.y, b101.y, b011.y, b111.y, wx, wy, wz);
+  } else {
+    const float4* p = s.nodes + o;
+    const float4 n000 = __ldg(p), n100 = __ldg(p + 1);
+    const float4 n010 = __ldg(p + sy), n110 = __ldg(p + sy + 1);
+    const float4 n001 = __ldg(p + sz), n101 = __ldg(p + sz + 1);
+    const float4 n011 = __ldg(p + sz + sy), n111 = __ldg(p + sz + sy + 1);
+    ex = lerp3(f2d(n000.x), f2d(n100.x), f2d(n010.x), f2d(n110.x), f2d(n001.x), f2d(n101.x), f2d(n011.x), f2d(n111.x), wx, wy, wz);
+    ey = lerp3(f2d(n000.y), f2d(n100.y), f2d(n010.y), f2d(n110.y), f2d(n001.y), f2d(n101.y), f2d(n011.y), f2d(n111.y), wx, wy, wz);
+    Ez = lerp3(f2d(n000.z), f2d(n100.z), f2d(n010.z), f2d(n110.z), f2d(n001.z), f2d(n101.z), f2d(n011.z), f2d(n111.z), wx, wy, wz);
+    mask = lerp3(f2d(n000.w), f2d(n100.w), f2d(n010.w), f2d(n110.w), f2d(n001.w), f2d(n101.w), f2d(n011.w), f2d(n111.w), wx, wy, wz);
+  }
   Ex = fx ? -ex : ex;
   Ey = fy ? -ey : ey;
   return okx & oky;
 }
 
 // Field and mask at r.  Returns the slab index (>= 0) or -status when r is outside the domain.
-// UNIFORM1 = the field is one uniform slab (configs 1-3): no dispatch, no loads.
+// FK = field kind the kernel is compiled for: 1 = the field is one uniform slab (configs 1-3: no dispatch, no loads), 2 = one
+// grid slab (config 4: the slab's constants are read at fixed constant-bank offsets instead of through a dynamic slab
+// index), 0 = any slab stack (config 5).
 // Slow path of the bounds test: which face was crossed (S5 order: z_lo, z_hi, then x/y; NaN coordinates -> 3).
 __device__ __forceinline__ int outside_status(const DevField& f, double x, double y, double z) {
   if (z < f.z_lo) return -AVM_LEFT_ZLO;
@@ -244,7 +265,7 @@ __device__ __forceinline__ int outside_status(const DevField& f, double x, doubl
   return -AVM_LEFT_XY;
 }
 
-template <bool UNIFORM1>
+template <int FK>
 __device__ __forceinline__ int field_at(const DevField& f, double x, double y, double z, double& Ex, double& Ey,
                                         double& Ez, double& mask) {
   // written so that NaN coordinates fail the test, like the oracle
@@ -252,14 +273,17 @@ __device__ __forceinline__ int field_at(const DevField& f, double x, double y, d
   if (f.xy_bounded) in = in & (x >= f.xy_lo[0]) & (x <= f.xy_hi[0]) & (y >= f.xy_lo[1]) & (y <= f.xy_hi[1]);
   else in = in & ((x + y) == (x + y));
   if (!in) return outside_status(f, x, y, z);
-  if (UNIFORM1) {
+  if (FK == 1) {
     Ex = f.slab[0].E[0]; Ey = f.slab[0].E[1]; Ez = f.slab[0].E[2]; mask = 1.0;
     return 0;
   }
-  int si = f.n_slabs - 1;
-  for (int i = f.n_slabs - 2; i >= 0; --i) if (z < f.slab[i].z_hi) si = i;
+  int si = 0;
+  if (FK == 0) {
+    si = f.n_slabs - 1;
+    for (int i = f.n_slabs - 2; i >= 0; --i) if (z < f.slab[i].z_hi) si = i;
+  }
   const DevSlab& s = f.slab[si];
-  if (s.kind == 0) { Ex = s.E[0]; Ey = s.E[1]; Ez = s.E[2]; mask = 1.0; return si; }
+  if (FK == 0 && s.kind == 0) { Ex = s.E[0]; Ey = s.E[1]; Ez = s.E[2]; mask = 1.0; return si; }
   if (!grid_at(s, x, y, z, Ex, Ey, Ez, mask)) return -AVM_LEFT_XY;
   return si;
 }
@@ -267,9 +291,10 @@ __device__ __forceinline__ int field_at(const DevField& f, double x, double y, d
 // ---- S2-S3: free flight of duration dt in constant E (and B) from (r, v) ---------------------------------
 // UNIFORM1: E is the run constant of slab 0 and the arguments Ex, Ey, Ez are ignored (a, E x B drift and a-parallel
 // come precomputed from DevField).
-template <bool UNIFORM1, bool HASB>
+template <int FK, bool HASB>
 __device__ __forceinline__ void flight(const DevField& f, double Ex, double Ey, double Ez, double dt, double& x,
                                        double& y, double& z, double& vx, double& vy, double& vz) {
+  constexpr bool UNIFORM1 = FK == 1;
   const double ax = UNIFORM1 ? f.ua[0] : -kKappa * Ex, ay = UNIFORM1 ? f.ua[1] : -kKappa * Ey,
                az = UNIFORM1 ? f.ua[2] : -kKappa * Ez;
   if (!HASB) {
@@ -465,22 +490,25 @@ __device__ __forceinline__ int uniform_exit_status(const DevField& f, double t_m
 // r' — or -(finishing status).  One uniform slab: one predicate.  Maps: the lookup runs unconditionally (indices are
 // clamped, so any r' is safe to look up), every condition joins one predicate, and the status is decoded, in S5's
 // order, only when it fails.
-template <bool UNIFORM1>
+template <int FK>
 __device__ __forceinline__ int s5_status(const DevField& f, double t_max, uint32_t n, double x, double y, double z,
                                          double t, double& Ex, double& Ey, double& Ez) {
-  if (UNIFORM1) {
+  if (FK == 1) {
     if (!uniform_continues(f, t_max, n, x, y, z, t)) return uniform_exit_status(f, t_max, x, y, z, t);
     return 0;
   }
   bool inb = (z >= f.z_lo) & (z <= f.z_hi);
   if (f.xy_bounded) inb = inb & (x >= f.xy_lo[0]) & (x <= f.xy_hi[0]) & (y >= f.xy_lo[1]) & (y <= f.xy_hi[1]);
   else inb = inb & ((x + y) == (x + y));
-  int si = f.n_slabs - 1;
-  for (int i = f.n_slabs - 2; i >= 0; --i) if (z < f.slab[i].z_hi) si = i;
+  int si = 0;
+  if (FK == 0) {
+    si = f.n_slabs - 1;
+    for (int i = f.n_slabs - 2; i >= 0; --i) if (z < f.slab[i].z_hi) si = i;
+  }
   const DevSlab& s = f.slab[si];
   double nEx, nEy, nEz, mask = 1.0;
   bool fold_ok = true;
-  if (s.kind == 0) { nEx = s.E[0]; nEy = s.E[1]; nEz = s.E[2]; }
+  if (FK == 0 && s.kind == 0) { nEx = s.E[0]; nEy = s.E[1]; nEz = s.E[2]; }
   else fold_ok = grid_at(s, x, y, z, nEx, nEy, nEz, mask);
   const bool ok = inb & fold_ok & !(mask < 0.5) & !(t > t_max) & (n < kStepLimit);
   if (!ok) {
@@ -494,23 +522,23 @@ __device__ __forceinline__ int s5_status(const DevField& f, double t_max, uint32
 }
 
 // S3-S4: the flight itself; t and n advance.  Returns |v'|^2.
-template <bool UNIFORM1, bool HASB>
+template <int FK, bool HASB>
 __device__ __forceinline__ double advance_move(const DevField& f, uint32_t& n, double& x, double& y, double& z, double& t,
                                                double& vx, double& vy, double& vz, double Ex, double Ey, double Ez,
                                                double dt) {
-  flight<UNIFORM1, HASB>(f, Ex, Ey, Ez, dt, x, y, z, vx, vy, vz);
+  flight<FK, HASB>(f, Ex, Ey, Ez, dt, x, y, z, vx, vy, vz);
   t = t + dt;
   n = n + 1u;
   return vx * vx + vy * vy + vz * vz;
 }
 
 // S3-S6 for one electron with this flight's dt.  Returns the energy bin (>= 0) or -(finishing status).
-template <bool UNIFORM1, bool HASB>
+template <int FK, bool HASB>
 __device__ __forceinline__ int advance(const DevGas& g, const DevField& f, double t_max, uint32_t& n, double& x,
                                        double& y, double& z, double& t, double& vx, double& vy, double& vz, double& Ex,
                                        double& Ey, double& Ez, double dt, bool& overflow) {
-  const double s2 = advance_move<UNIFORM1, HASB>(f, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt);   // S3, S4
-  const int st = s5_status<UNIFORM1>(f, t_max, n, x, y, z, t, Ex, Ey, Ez);                        // S5
+  const double s2 = advance_move<FK, HASB>(f, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt);   // S3, S4
+  const int st = s5_status<FK>(f, t_max, n, x, y, z, t, Ex, Ey, Ez);                        // S5
   if (st < 0) return st;
   return energy_bin(g, s2, overflow);                                                            // S6
 }

@@ -37,14 +37,14 @@ static_assert(sizeof(WarpBuf) == 1920, "WarpBuf");
 // S3-S7 with this flight's pre-drawn (dt, u2w); the draws of the lane's NEXT flight are issued behind the threshold-record
 // load.  On return: fin = finishing status (or 0), pend / pc = a real collision is pending (collision_step follows, in
 // the warp's one collision phase), (dt, u2w) = the next flight's draws.
-template <bool UNIFORM1, bool HASB, bool TALLY>
+template <int FK, bool HASB, bool TALLY>
 __device__ __forceinline__ void fw_flight(const DevGas& g, const DevField& f, const PhiloxKeys& K,
                                           const ushort4* __restrict__ tab, const double2* __restrict__ logtab,
                                           const double t_max, const uint64_t id, uint32_t& n, double& x, double& y,
                                           double& z, double& t, double& vx, double& vy, double& vz, double& Ex, double& Ey,
                                           double& Ez, double& dt, uint2& u2w, int& fin, bool& pend, Pending& pc, Tally& tl) {
   bool over = false;
-  const int b = advance<UNIFORM1, HASB>(g, f, t_max, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt, over);
+  const int b = advance<FK, HASB>(g, f, t_max, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt, over);
   if (b < 0) { fin = -b; return; }
   const ushort4 rec = tab[b];
   const uint2 u2c = u2w;
@@ -73,13 +73,14 @@ __device__ __forceinline__ void fw_flight(const DevGas& g, const DevField& f, co
 // commit(on, e, sidx, ev, bin, fin): called once per pass by every lane; on = this lane's step was taken in this pass,
 //   its result is in x .. vz, n; ev = -1 null, level, or -2 ended before the decision.
 // Returns the finishing status of the lane's own electron (0 = still active); its state is back in x .. vz, id, n, slot.
-template <bool UNIFORM1, bool HASB, bool TALLY, class Collide, class Commit>
+template <int FK, bool HASB, bool TALLY, class Collide, class Commit>
 __device__ __forceinline__ int tp_batch(const DevGas& g, const DevField& f, const PhiloxKeys& K,
                                         const ushort4* __restrict__ tab, const LevelPar* __restrict__ s_lv,
                                         const double2* __restrict__ s_logtab, WarpBuf* __restrict__ wb, const double t_max,
                                         const unsigned lane, const unsigned act, const bool have, double& x, double& y,
                                         double& z, double& t, double& vx, double& vy, double& vz, uint64_t& id, uint32_t& n,
                                         uint32_t& slot, Tally& tl, Collide&& collide, Commit&& commit) {
+  static_assert(FK == 1, "time-parallel batches need a constant field: one uniform slab");
   const unsigned lt_mask = (1u << lane) - 1u;
   const int k = __popc(act);
   const int lg = 32 - __clz(k - 1);             // k' = 2^lg >= k  (k = 1: __clz(0) = 32)
@@ -134,7 +135,7 @@ __device__ __forceinline__ int tp_batch(const DevGas& g, const DevField& f, cons
       // the threshold record and its 16-bit decision — and the ELASTIC collision this step would be, evaluated ahead
       // of the decision from the post-flight velocity (levels 0 / 1 are 97 % of the real collisions).  The rare
       // outcomes (termination, a band of the filter, another level or type) are decoded after the block.
-      flight<UNIFORM1, HASB>(f, 0.0, 0.0, 0.0, P - Pb, x, y, z, vx, vy, vz);
+      flight<FK, HASB>(f, 0.0, 0.0, 0.0, P - Pb, x, y, z, vx, vy, vz);
       const double s2 = vx * vx + vy * vy + vz * vz;
       t = t + (P - Pb);
       n = n + 1u;
@@ -204,6 +205,94 @@ __device__ __forceinline__ int tp_batch(const DevGas& g, const DevField& f, cons
   }
   __syncwarp();
   return fin;
+}
+
+// ---- serial batch (any field) ----------------------------------------------------------------------------------------
+// For a warp that holds k <= 16 electrons.  All 32 lanes first prepare the draws (Philox block 0 + logarithm, block 1 +
+// deflection angles) of the next B = 32 / k' steps of the k electrons, lane j serving electron j mod k' at step j div k',
+// through the warp's WarpBuf — the draws depend on (id, n) alone, so this is the same as drawing them in place, and draws
+// of steps an electron does not reach are discarded.  Then every owner lane walks through ITS electron's steps on its own:
+// one straight-line block per step — flight (S3-S4), energy bin and threshold record (S6, S7), the S5 predicate with the
+// field lookup at the new position (= S0 of the next step) — and goes straight on when the step was a null collision, with
+// no warp vote, ballot or shuffle in between.  A lane leaves its loop at an event (a real collision pending, or the
+// electron finished); the warp then runs one collision / append / retire phase for the lanes with events, and the loops
+// resume until every electron has used its B steps.
+//
+// collide(pend, pc, have_d, d, fin) -> level; retire(fin): warp-wide, frees the lanes whose electron finished (clears
+// `have`); commit(e, s, ev, bin, fin): step s of the batch of the warp's e-th electron is done, its result is in x .. vz, n.
+template <int FK, bool HASB, bool TALLY, class Collide, class Retire, class Commit>
+__device__ __forceinline__ void sb_batch(const DevGas& g, const DevField& f, const PhiloxKeys& K,
+                                         const ushort4* __restrict__ tab, const double2* __restrict__ s_logtab,
+                                         WarpBuf* __restrict__ wb, const double t_max, const unsigned lane, const unsigned act,
+                                         bool& have, double& x, double& y, double& z, double& t, double& vx, double& vy,
+                                         double& vz, double& Ex, double& Ey, double& Ez, const uint64_t& id, uint32_t& n,
+                                         Tally& tl, Collide&& collide, Retire&& retire, Commit&& commit) {
+  const unsigned lt_mask = (1u << lane) - 1u;
+  const int k = __popc(act);
+  const int lg = 32 - __clz(k - 1);             // k' = 2^lg >= k  (k = 1: __clz(0) = 32)
+  const int kp = 1 << lg, nb_steps = 32 >> lg;
+  const int rank = __popc(act & lt_mask);
+  if (have) { wb->id[rank] = id; wb->n[rank] = n; }
+  __syncwarp();
+  {
+    const int e = (int)lane & (kp - 1), s = (int)lane >> lg;
+    if (e < k) {
+      const uint64_t hid = wb->id[e];
+      const uint32_t hn = wb->n[e] + (uint32_t)s;
+      double ddt;
+      uint2 du2;
+      draw_flight(g, K, s_logtab, hid, hn, ddt, du2);
+      const Deflection d = deflection_draws(K, hid, hn);
+      wb->dt[lane] = ddt; wb->u2w[lane] = du2;
+      wb->ct[lane] = d.ct; wb->st[lane] = d.st; wb->cphi[lane] = d.cphi; wb->sphi[lane] = d.sphi;
+    }
+  }
+  __syncwarp();
+  int s = 0;                                    // this lane's next step of the batch
+#pragma unroll 1
+  for (;;) {
+    int fin = 0, sc = 0;
+    bool pend = false;
+    Pending pc;
+    pc.lsel = 0; pc.bin = -1; pc.xr = 0.0;
+    Deflection dd;
+    dd.ct = 1.0; dd.st = 0.0; dd.cphi = 1.0; dd.sphi = 0.0;
+    if (have) {
+#pragma unroll 1
+      while (s < nb_steps) {
+        const int idx = s * kp + rank;
+        const double dtj = wb->dt[idx];
+        const uint2 u2 = wb->u2w[idx];
+        sc = s; ++s;
+        const double s2 = advance_move<FK, HASB>(f, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dtj);   // S3, S4
+        bool over;
+        const int b = energy_bin(g, s2, over);                                                     // S6 (counts only when S5 passes)
+        int r = decide_filter(tab[b], u2);                                                         // S7 and the head of S8
+        const int st = s5_status<FK>(f, t_max, n, x, y, z, t, Ex, Ey, Ez);                         // S5; the field at r' = S0 of the next step
+        if (st == 0 && r == -1) {                                                                  // null collision: straight on
+          if (TALLY && over) ++tl.over;
+          commit(rank, sc, -1, b, 0);
+          continue;
+        }
+        if (st < 0) { fin = -st; break; }
+        if (TALLY && over) ++tl.over;
+        if (r == -2 || r == 2) {
+          pc.xr = to_unit(u2.x, u2.y) * g.nu_hat;
+          if (r == -2) r = decide_exact(g, b, pc.xr);
+          if (r == 2) prefetch_row(g, b);
+        }
+        if (r < 0) { commit(rank, sc, -1, b, 0); continue; }
+        pend = true; pc.lsel = r; pc.bin = b;
+        dd.ct = wb->ct[idx]; dd.st = wb->st[idx]; dd.cphi = wb->cphi[idx]; dd.sphi = wb->sphi[idx];
+        break;
+      }
+    }
+    int lvl = -1;
+    if (__any_sync(0xFFFFFFFFu, pend)) lvl = collide(pend, pc, true, dd, fin);
+    if (have && (pend || fin != 0)) commit(rank, sc, pend ? lvl : -2, pc.bin, fin);
+    retire(fin);
+    if (!__any_sync(0xFFFFFFFFu, have && s < nb_steps)) break;
+  }
 }
 
 }  // namespace avm

@@ -138,16 +138,21 @@ def oracle_sequence(oracle, g, fd, seed, st, ids, n0, gl, t_max):
     return out, st_in
 
 
-def assert_form2_parity(avm, cpu, st_in, gpu, gl, what):
+def assert_form2_parity(avm, cpu, st_in, gpu, gl, what, composed=False):
+    """composed (form 2): a step's position is the composed flight from the batch's base state, so its rounding is relative
+    to the coordinate's largest magnitude since the batch began (the oracle's sequential sum carries the same absolute
+    rounding); form 3 steps sequentially and needs no such allowance."""
     assert np.array_equal(cpu.event == -3, gpu.event == -3), f"{what}: the batches reach different steps"
     total = 0
+    run_max = np.zeros((3, st_in.shape[1]))
     for s in range(gl):
+        run_max = np.maximum(run_max, np.abs(st_in[0:3, :, s]))
         sel = cpu.event[:, s] != -3
         if not sel.any():
             continue
         c = type(cpu)(cpu.state[:, sel, s], cpu.event[sel, s], cpu.status[sel, s], cpu.bin[sel, s], cpu.child[:, sel, s], cpu.child_id[sel, s])
         g = type(cpu)(gpu.state[:, sel, s], gpu.event[sel, s], gpu.status[sel, s], gpu.bin[sel, s], gpu.child[:, sel, s], gpu.child_id[sel, s])
-        total += assert_step_parity(c, g, st_in[:, sel, s], f"{what} step {s}")
+        total += assert_step_parity(c, g, st_in[:, sel, s], f"{what} step {s}", pos_floor=run_max[:, sel] if composed else None)
     return total
 
 
@@ -170,7 +175,7 @@ def test_form2_time_parallel_batch(avm, ctx, oracle, g0, B, k):
     st[3, 50:400] = t_max - rng.uniform(0.0, 20.0, 350) / g0.resolved_nu_hat()    # some run into the time limit inside the batch
     cpu, st_in = oracle_sequence(oracle, g0, fd, 3, st, ids, n0, gl, t_max)
     gpu = avm.step_batch_form(ctx, gg, fg, 3, st, ids, n0, form=2, k=k, t_max=t_max)
-    total = assert_form2_parity(avm, cpu, st_in, gpu, gl, f"form 2 k={k} B={B}")
+    total = assert_form2_parity(avm, cpu, st_in, gpu, gl, f"form 2 k={k} B={B}", composed=True)
     assert total > n * min(gl, 3) * 0.7
     ev = cpu.event[cpu.event != -3]
     assert (ev == -1).sum() > n and (ev == 0).sum() > 50 and (ev == 1).sum() > 50 and (ev >= 2).sum() > 10
@@ -192,7 +197,7 @@ def test_form2_composed_flight_time_and_filter_bands(avm, ctx, oracle, g0, B):
         st, ids, n0, s_t, which = in_band_states(g0, seed, 400 * k, gl, rng)
         cpu, st_in = oracle_sequence(oracle, g0, fd, seed, st, ids, n0, gl, float("inf"))
         gpu = avm.step_batch_form(ctx, gg, fg, seed, st, ids, n0, form=2, k=k)
-        assert_form2_parity(avm, cpu, st_in, gpu, gl, f"form 2 in-band k={k} B={B}")
+        assert_form2_parity(avm, cpu, st_in, gpu, gl, f"form 2 in-band k={k} B={B}", composed=True)
         reached = cpu.event != -3
         tc, tg = cpu.state[3][reached], gpu.state[3][reached]
         assert np.all(np.abs(tg - tc) <= 32 * 2.0 ** -52 * tc), np.max(np.abs(tg - tc) / tc) / 2.0 ** -52
@@ -218,3 +223,65 @@ def test_overflow_tally_in_every_form(avm, ctx, oracle):
         assert (cpu.end[4] > 5.0).mean() > 0.5 and int(cpu.tallies_u64[3]) > 5 * n_p
         assert np.array_equal(np.sort(cpu.n_steps), np.sort(gpu.n_steps)), what
         assert np.array_equal(cpu.tallies_u64, gpu.tallies_u64), (what, cpu.tallies_u64, gpu.tallies_u64)
+
+
+def _form3_case(avm, ctx, oracle, g, fd, fg, k, rng, center, box, what, t_max=5.0):
+    gl = avm.step_form_lanes(k)
+    n = k * 1200
+    st = _states(n, rng, box=box, center=center)
+    E, m, sl = oracle.field_eval(fd, st[0:3])
+    ok = (sl >= 0) & (m >= 0.5)
+    st[:, ~ok] = st[:, np.flatnonzero(ok)[0]][:, None]                 # a step starts in the gas
+    st[3, 50:400] = t_max - rng.uniform(0.0, 20.0, 350) / g.resolved_nu_hat()
+    ids = rng.integers(0, 2 ** 64, n, dtype=np.uint64)
+    n0 = rng.integers(0, 2 ** 32 - 64, n, dtype=np.uint64).astype(np.uint32)
+    n0[:50] = 0xFFFFFFEF - rng.integers(0, 6, 50)
+    cpu, st_in = oracle_sequence(oracle, g, fd, 3, st, ids, n0, gl, t_max)
+    gpu = avm.step_batch_form(ctx, avm.gas_create(ctx, g), fg, 3, st, ids, n0, form=3, k=k, t_max=t_max)
+    total = assert_form2_parity(avm, cpu, st_in, gpu, gl, what)
+    assert total > n * min(gl, 3) * 0.5
+    return cpu
+
+
+@pytest.mark.parametrize("B", [(0.0, 0.0, 0.0), B30])
+@pytest.mark.parametrize("k", [1, 3, 8, 16])
+def test_form3_serial_batch_uniform(avm, ctx, oracle, g0, B, k):
+    """Form 3 (serial batch) in one uniform slab: gl sequential oracle steps per electron, every output of every step."""
+    rng = np.random.default_rng(60 + k)
+    fd = fields.uniform_gap((0.0, 0.0, -60000.0), 0.0, 60e-4, B)
+    cpu = _form3_case(avm, ctx, oracle, g0, fd, avm.field_create(ctx, fd), k, rng, (0, 0, 30e-4), 30e-4, f"form 3 uniform k={k} B={B}")
+    ev = cpu.event[cpu.event != -3]
+    assert (ev == -1).sum() > 1000 and (ev == 0).sum() > 50 and (ev == 1).sum() > 50 and (ev >= 2).sum() > 10
+    assert set(np.unique(cpu.status)) >= {0, 1, 2, 6, 7}
+
+
+@pytest.mark.parametrize("widen", [True, False])
+@pytest.mark.parametrize("B", [(0.0, 0.0, 0.0), (0.3, -0.2, 0.9)])
+def test_form3_serial_batch_grid(avm, ctx, oracle, g0, B, widen):
+    """Form 3 on maps: ONE grid slab (the kernel specialisation of config 4: mirror fold, material) and a stack of a grid
+    and a uniform slab (the generic one of config 5), from the fp32 nodes and from their widened fp64 copy."""
+    rng = np.random.default_rng(70)
+    nodes = _random_map(rng, 12, 14, 40, e_scale=5e4)
+    nodes[..., 2] -= 4e4
+    h = (1e-4, 1e-4, 1e-4)
+    one = fields.FieldDesc([fields.grid_slab(nodes, (0, 0, 0), h, 0.0, 39e-4, fields.BC_MIRROR, fields.BC_MIRROR, 10e-4, 12e-4)], B)
+    two = fields.FieldDesc([fields.grid_slab(nodes, (0, 0, 0), h, 0.0, 39e-4, fields.BC_MIRROR, fields.BC_PERIODIC, 10e-4, 12e-4),
+                            fields.Slab(39e-4, 60e-4, fields.KIND_UNIFORM, (0.0, 0.0, -30000.0))], B, (-40e-4, -50e-4), (40e-4, 50e-4))
+    for fd, zc, zb, what in ((one, 20e-4, 19e-4, "one grid slab"), (two, 30e-4, 29e-4, "grid + uniform")):
+        fg = avm.field_create(ctx, fd, widen=widen)
+        for k in (1, 2, 5):
+            cpu = _form3_case(avm, ctx, oracle, g0, fd, fg, k, rng, (3e-4, -7e-4, zc), zb, f"form 3 {what} k={k} B={B} widen={widen}")
+            assert (cpu.status == 4).sum() > 20 and (cpu.status == 0).sum() > 1000
+
+
+def test_form3_states_inside_the_filter_bands(avm, ctx, oracle, g0):
+    rng = np.random.default_rng(80)
+    seed = 9
+    fd = fields.uniform_gap((0.0, 0.0, 0.0), -1.0, 1.0)
+    gg, fg = avm.gas_create(ctx, g0), avm.field_create(ctx, fd)
+    for k in (1, 4):
+        gl = avm.step_form_lanes(k)
+        st, ids, n0, s_t, which = in_band_states(g0, seed, 400 * k, gl, rng)
+        cpu, st_in = oracle_sequence(oracle, g0, fd, seed, st, ids, n0, gl, float("inf"))
+        gpu = avm.step_batch_form(ctx, gg, fg, seed, st, ids, n0, form=3, k=k)
+        assert_form2_parity(avm, cpu, st_in, gpu, gl, f"form 3 in-band k={k}")
