@@ -1,16 +1,21 @@
 #!/usr/bin/env python
-"""bench.py — electron-collisions/s (real + null) of the avalanche hot path on B200, with its ALU roofline.
+"""bench.py — electron-collisions/s (real + null) of the avalanche hot path on B200, with its roofline.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config2|config2x64|config1|config3s]
-  python bench.py --impl reference ...     # the oracle on the host cores (DESIGN.md §7)
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload all|config1|config2|config3s|config4|config5|...]
+  python bench.py --impl reference ...     # the oracle on the host cores (DESIGN.md §9)
 
-A "step" is one pass of the whole hot path (avm_run: primary injection, persistent transport kernel with
-secondary append and lane refill, tallies) over one batch of primaries of the workload.  Prints ONE JSON line.
-Nothing here reads /root/reference.
+A "step" is one pass of the whole hot path (avm_run: primary injection, persistent transport kernel with secondary
+append and lane refill, tallies) over one batch of primaries of a workload.  The default run (`--workload all`) times
+ALL FIVE BASELINE.json configs: the headline (`value`, `config.workload`, `roofline`, `e2e`, `cpu_baseline`) is config 3
+with its time cut — the largest one by collisions per step that fits the bench budget — timed for
+exactly K steps after W warm-ups; the other four are in `per_config`, each with its own steps / warm-ups stated there.
+Prints ONE JSON line.  Nothing here reads /root/reference.
 """
 from __future__ import annotations
 
 import argparse
+import glob
+import hashlib
 import json
 import os
 import subprocess
@@ -26,17 +31,49 @@ if ROOT not in sys.path:
 
 METRIC = "electron-collisions/s (real+null)"
 UNIT = "collisions/s"
-# Algorithmic FP64 thread-instructions per unit: what the method must do.
+HEADLINE = "config3s"
+# workload -> (multiplier of --steps, oracle sample = first n primaries; 0 = all).  Oracle samples follow SURVEY.md §8(d)
+# "Oracle timing" (config 3: first primaries only, config 5: first 8), sized for ~1-10 s each on the box's cores.
+ALL = {"config1": (4, 0), "config2": (2, 0), "config3s": (1, 2048), "config4": (1, 0), "config5": (0.5, 8)}
+# Algorithmic FP64 thread-instructions per unit: what the method must do — NOT what
+# the kernel executes (the executed count and the FP64 pipe's busy share come from the ncu capture, when it is current).
 FP64_PER_NULL = {False: 90.0, True: 170.0}       # free flight + energy + bin + decision; key = B != 0
 FP64_PER_REAL_EXTRA = 110.0                      # deflection angles, basis, rotation, renormalise, speed
 FP64_PER_ION_EXTRA = 80.0                        # Opal-Beaty atan/tan, child direction
 FP64_PER_GRID_EXTRA = 45.0                       # fold + 7 lerps x 4 channels per step in a grid slab
-GATHER_BYTES_PER_GRID_STEP = 128.0               # 8 nodes x 16 B
+GATHER_BYTES_PER_GRID_STEP = 128.0               # 8 nodes x 16 B of the fp32 map; the widened copy moves 256
 FP64_LANES_PER_SM = 64                           # one warp-wide FP64 instruction / 2 clk / scheduler
-# From the committed ncu captures of the transport kernel (profiles/r1d_transport_ncu.md), per launch of the workload:
-# DRAM bytes read + written, DFMA + DMUL + DADD thread-instructions per collision, FP64 pipe active %.
-NCU_CAPTURE = {"config2": {"traffic": 3897344 + 48640, "sass_fp64_per_collision": 92.4, "fp64_pipe_active_pct": 22.9},
-               "config2x16": {"traffic": 92790528 + 419887104, "sass_fp64_per_collision": 64.4, "fp64_pipe_active_pct": 27.3}}
+NCU_CAPTURE_FILE = os.path.join(ROOT, "profiles", "ncu_capture.json.txt")
+
+
+def kernel_source_hash() -> str:
+    """sha256 over the kernel sources: an ncu capture describes the kernels only while this is unchanged."""
+    h = hashlib.sha256()
+    for p in sorted(glob.glob(os.path.join(ROOT, "paper_2509_15377_b200", "csrc", "*"))):
+        if p.endswith((".cu", ".cuh", ".inc")):
+            h.update(os.path.basename(p).encode())
+            h.update(open(p, "rb").read())
+    return h.hexdigest()[:16]
+
+
+def ncu_capture(workload: str) -> dict:
+    """Figures of the committed `ncu --set full` capture of the transport kernel on this workload (profiles/), or nulls
+    when there is none or the kernels have changed since (never a stale number)."""
+    out = {"traffic": None, "sass_fp64_per_collision_ncu": None, "fp64_pipe_active_pct_ncu": None, "ncu_source": None}
+    try:
+        d = json.load(open(NCU_CAPTURE_FILE))
+    except Exception:
+        return out
+    e = d.get("workloads", {}).get(workload)
+    if e is None:
+        return out
+    if d.get("kernel_source_hash") != kernel_source_hash():
+        out["ncu_source"] = f"{e.get('profile')}: stale (kernels changed since the capture), figures withheld"
+        return out
+    out.update(traffic=e.get("dram_bytes_per_launch"), sass_fp64_per_collision_ncu=e.get("sass_fp64_per_collision"),
+               fp64_pipe_active_pct_ncu=e.get("fp64_pipe_active_pct"),
+               ncu_source=f"{e.get('profile')} (ncu --set full, one launch; dram__bytes_read.sum + dram__bytes_write.sum)")
+    return out
 
 
 def make_workload(name: str, rank: int = 0):
@@ -57,9 +94,19 @@ def make_workload(name: str, rank: int = 0):
         w = configs.replicate(configs.config4(), int(name[len("config4x"):]))
     elif name == "config5":
         w = configs.config5(id_offset=rank * 200)
+    elif name == "config5hg":
+        w = configs.config5hg(id_offset=rank * 8)
     else:
         raise SystemExit(f"unknown workload {name}")
     return w
+
+
+def config_dict(w, world: int) -> dict:
+    """What defines the workload — identical in both arms (`--impl ours` / `--impl reference`)."""
+    return {"workload": w.name, "note": w.note, "n_primaries_per_gpu": w.n_primaries, "seed": "workload seed + step index",
+            "t_max_ns": None if not np.isfinite(w.t_max) else w.t_max,
+            "l2": "GPU arm: 256 MiB buffer written between timed iterations",
+            "parallelism": f"replicas over primaries x{world}, no collective"}
 
 
 def grid_fraction(field) -> float:
@@ -127,20 +174,25 @@ class ClockSampler:
         return out
 
 
-def fp64_peak(avm, ctx) -> dict:
-    """The ALU roofline denominator: FP64 thread-instructions per second.  Nominal = SMs x 64 FP64
-    lanes x max SM clock; measured = the library's DFMA probe (8 independent chains per thread, 8 CTAs per SM)."""
-    sm_max_mhz = 1965.0
+def measured_peaks(avm, ctx) -> dict:
+    """The roofline denominators, measured on this GPU in this run: FP64 thread-instructions per second (the
+    library's DFMA probe; nominal = SMs x 64 FP64 lanes x max SM clock), random 32-byte-sector gather bandwidth with the
+    working set in L2 (2.7 MB = the gas table, 64 MB) and in HBM (1 GiB), shared-memory random 8-byte loads per second."""
+    sm_max_mhz, hbm = 1965.0, None
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
-            sm_max_mhz = float(json.load(f).get("sm_max_mhz", sm_max_mhz))
+            mp = json.load(f)
+            sm_max_mhz = float(mp.get("sm_max_mhz", sm_max_mhz)); hbm = mp.get("hbm_gbs")
     except Exception:
         pass
     nominal = ctx.sm_count * FP64_LANES_PER_SM * sm_max_mhz * 1e6
-    best = 0.0
-    for _ in range(3):
-        best = max(best, avm.fp64_probe(ctx, iters=1 << 15)["dfma_per_s"])
-    return {"nominal": nominal, "measured": best, "sm_max_mhz": sm_max_mhz}
+    best = max(avm.fp64_probe(ctx, iters=1 << 15)["dfma_per_s"] for _ in range(3))
+    g = {}
+    for label, nbytes, iters in (("l2_2p7MB", 2_700_000 // 32 * 32, 4096), ("l2_64MB", 64 << 20, 4096), ("hbm_1GiB", 1 << 30, 1024)):
+        g[label] = max(avm.gather_probe(ctx, nbytes, iters=iters)["GBps"] for _ in range(2))
+    sm = max(avm.smem_probe(ctx)["loads_per_s"] for _ in range(2))
+    return {"fp64_nominal": nominal, "fp64_measured": best, "sm_max_mhz": sm_max_mhz, "gather_GBps": g,
+            "smem_random_8B_loads_per_s": sm, "hbm_copy_GBps_MEASURED_PEAKS": hbm}
 
 
 def oracle_leg(w, n_prim: int, threads: int) -> dict:
@@ -156,31 +208,169 @@ def oracle_leg(w, n_prim: int, threads: int) -> dict:
             "electrons": int(r.n), "primaries": int(n_prim)}
 
 
+def cpu_baseline_entry(w, sample: int, cores: int) -> dict:
+    n_prim = min(w.n_primaries, sample) if sample > 0 else w.n_primaries
+    o = oracle_leg(w, n_prim, cores)
+    return {"value": o["collisions"] / o["seconds"], "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"first {n_prim} of {w.n_primaries} primaries of {w.name}, seed {w.seed}, {cores} threads over disjoint "
+                      f"primary ranges, {o['collisions']} collisions in {o['seconds']:.2f} s",
+            "avalanches_per_s": n_prim / o["seconds"], "null_per_s": o["null"] / o["seconds"], "real_per_s": o["real"] / o["seconds"]}
+
+
+def workload_list(args):
+    if args.workload == "all":
+        return [(nm, max(1, int(round(args.steps * mult))), smp) for nm, (mult, smp) in ALL.items()]
+    smp = args.ref_primaries if args.ref_primaries > 0 else ALL.get(args.workload, (1, 0))[1]
+    return [(args.workload, args.steps, smp)]
+
+
 def run_reference(args) -> None:
-    """--impl reference: the oracle on the host cores (rank 0 only), same metric/unit/config as our arm."""
+    """--impl reference: the oracle on the host cores (rank 0 only), same metric/unit/config as our arm.  The headline is
+    timed for K steps after W warm-ups on a bounded sample; the other configs get one bounded run each in per_config."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    w = make_workload(args.workload)
     cores = os.cpu_count() or 1
-    n_prim = min(w.n_primaries, args.ref_primaries) if args.ref_primaries > 0 else w.n_primaries
-    for _ in range(args.warmup):
-        oracle_leg(w, n_prim, cores)
-    tot_c, tot_s, tot_p, last = 0, 0.0, 0, None
-    for _ in range(args.steps):
-        last = oracle_leg(w, n_prim, cores)
-        tot_c += last["collisions"]; tot_s += last["seconds"]; tot_p += n_prim
-    v = tot_c / tot_s
-    sample = f"first {n_prim} of {w.n_primaries} primaries of {w.name} per step, {cores} threads over disjoint primary ranges"
-    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": 1e3 * tot_s / max(args.steps, 1), "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": w.name, "note": w.note, "n_primaries_per_step": n_prim},
-            "avalanches_per_s": tot_p / tot_s,
-            "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
-            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-            "gpu_launches": 0}
+    wl = workload_list(args)
+    head = HEADLINE if args.workload == "all" else args.workload
+    per, line = [], None
+    for name, _, sample in wl:
+        w = make_workload(name)
+        if args.ref_primaries > 0:
+            sample = args.ref_primaries
+        if name == head:
+            n_prim = min(w.n_primaries, sample) if sample > 0 else w.n_primaries
+            for _ in range(args.warmup):
+                oracle_leg(w, n_prim, cores)
+            tot_c = tot_s = tot_n = tot_r = 0.0
+            for _ in range(args.steps):
+                o = oracle_leg(w, n_prim, cores)
+                tot_c += o["collisions"]; tot_s += o["seconds"]; tot_n += o["null"]; tot_r += o["real"]
+            v = tot_c / tot_s
+            smp = f"first {n_prim} of {w.n_primaries} primaries of {w.name} per step, {cores} threads over disjoint primary ranges"
+            cb = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": smp}
+            line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+                    "warmup": args.warmup, "ms_per_step": 1e3 * tot_s / max(args.steps, 1), "higher_is_better": True,
+                    "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                    "config": config_dict(w, args.gpus), "null_per_s": tot_n / tot_s, "real_per_s": tot_r / tot_s,
+                    "avalanches_per_s": n_prim * args.steps / tot_s, "cpu_baseline": cb,
+                    "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+            per.append({"workload": name, "value": v, "unit": UNIT, "ms_per_step": line["ms_per_step"], "steps": args.steps,
+                        "null_per_s": line["null_per_s"], "real_per_s": line["real_per_s"],
+                        "avalanches_per_s": line["avalanches_per_s"], "cpu_baseline": cb})
+        else:
+            cb = cpu_baseline_entry(w, sample, cores)
+            per.append({"workload": name, "value": cb["value"], "unit": UNIT, "steps": 1, "null_per_s": cb["null_per_s"],
+                        "real_per_s": cb["real_per_s"], "avalanches_per_s": cb["avalanches_per_s"], "cpu_baseline": cb})
+    line["per_config"] = per
     print(json.dumps(line), flush=True)
+
+
+def bench_workload(avm, ctx, torch, dist, name, steps, warmup, sample, rank, world, peaks, flush, with_cpu, cores):
+    """W warm-ups + exactly `steps` timed steps of one workload (device-timed, inputs resident) and the same through the
+    user's call with host buffers (e2e); returns its per_config entry (rank 0) and the clock samples of the timed region."""
+    w = make_workload(name, rank)
+    id_offset = rank * w.n_primaries
+    gg, fg = avm.gas_create(ctx, w.gas), avm.field_create(ctx, w.field)
+    L = w.gas.n_levels
+    has_b = any(v != 0.0 for v in w.field.B)
+    bufs = avm.RunBuffers(ctx, w.capacity, w.n_primaries, L)
+    prim_host = torch.from_numpy(w.primaries.copy()).pin_memory()
+    prim_dev = prim_host.to(ctx.device)
+    host = avm.HostBuffers(w.capacity, w.n_primaries, L, pinned=True)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def device_step(seed):
+        flush.zero_()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        _, n = avm.run(ctx, gg, fg, prim_dev, bufs, seed=seed, t_max=w.t_max, id_offset=id_offset)
+        e1.record()
+        e1.synchronize()
+        t = bufs.tallies_u64.cpu().numpy().view(np.uint64)
+        k, kt = avm.run_stats(ctx)
+        return {"ms": e0.elapsed_time(e1), "n": n, "tallies": t, "launches": k, "transport_launches": kt,
+                "transport_ms": avm.run_transport_ms(ctx)}
+
+    def e2e_step(seed):
+        """The user's call: host primaries in (H2D inside avm_run), endpoints and tallies back to pinned host."""
+        flush.zero_()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        _, n = avm.run(ctx, gg, fg, prim_host, bufs, seed=seed, t_max=w.t_max, id_offset=id_offset)
+        res = avm.fetch(ctx, bufs, n, host)
+        dt = time.perf_counter() - t0
+        per_el = sum(getattr(host, a).element_size() * (getattr(host, a).numel() // host.capacity) for a in ("id", "avalanche", "status", "n_steps", "birth", "end"))
+        d2h = n * per_el + host.per_avalanche.numel() * 8 + host.tallies_u64.numel() * 8 + host.tallies_f64.numel() * 8
+        return {"s": dt, "n": n, "tallies": res.tallies_u64.copy(), "d2h": d2h}
+
+    for i in range(warmup):
+        device_step(w.seed + 1000 + i)
+    sampler = ClockSampler(ctx.device.index or 0)
+    barrier()
+    sampler.start()
+    st = [device_step(w.seed + i) for i in range(steps)]
+    barrier()
+    clocks = sampler.stop()
+    for i in range(min(warmup, 2)):
+        e2e_step(w.seed + 2000 + i)
+    barrier()
+    e2e = [e2e_step(w.seed + i) for i in range(steps)]
+    barrier()
+
+    gfrac = grid_fraction(w.field)
+    tot_ms = sum(s["ms"] for s in st)
+    t_ms = sum(s["transport_ms"] for s in st)
+    sums = [sum(int(s["tallies"][L]) for s in st), sum(int(s["tallies"][L + 1]) for s in st), sum(int(s["n"]) for s in st),
+            sum(s["launches"] for s in st), sum(int(s["tallies"][L]) + int(s["tallies"][L + 1]) for s in e2e),
+            sum(alg_fp64(s["tallies"], L, w.gas.level_type, has_b, gfrac) for s in st), sum(s["transport_launches"] for s in st)]
+    e2e_s = sum(s["s"] for s in e2e)
+    vals = torch.tensor([tot_ms, e2e_s, t_ms], dtype=torch.float64, device=ctx.device)
+    sums_t = torch.tensor(sums, dtype=torch.float64, device=ctx.device)
+    if dist is not None:
+        dist.all_reduce(vals, op=dist.ReduceOp.MAX)          # reporting only: max time over ranks, job totals
+        dist.all_reduce(sums_t, op=dist.ReduceOp.SUM)
+    tot_ms_max, e2e_s_max, _ = (float(x) for x in vals.cpu())
+    null, real, electrons, launches, e2e_coll, _, _ = (float(x) for x in sums_t.cpu())
+    if rank != 0:
+        return None, clocks
+    # roofline of the dominant kernel (transport_kernel), this rank: algorithmic units per launch / its average launch
+    # duration (CUDA events recorded inside avm_run around each launch, on the ctx stream)
+    n_launch = max(sums[6], 1)
+    achieved = (sums[5] / n_launch) / ((t_ms / n_launch) * 1e-3)
+    cap = ncu_capture(w.name)
+    roofline = {"bound": "alu", "kernel": "transport_kernel", "achieved": achieved / 1e12, "peak": peaks["fp64_measured"] / 1e12,
+                "unit": "T FP64 thread-instr/s", "frac": achieved / peaks["fp64_measured"],
+                "frac_kind": "ALGORITHMIC FP64 thread-instructions of SURVEY §8(d) (null 90/170, real +110, ionisation +80, grid +45), "
+                             "held fixed, / DFMA rate measured in this run; the kernel executes fewer (sass_fp64_per_collision_ncu)",
+                "traffic": cap["traffic"], "sass_fp64_per_collision_ncu": cap["sass_fp64_per_collision_ncu"],
+                "fp64_pipe_active_pct_ncu": cap["fp64_pipe_active_pct_ncu"], "ncu_source": cap["ncu_source"],
+                "peak_source": "measured: avm_fp64_probe DFMA rate on this GPU in this run", "peak_nominal": peaks["fp64_nominal"] / 1e12,
+                "alg_fp64_per_collision": sums[5] / max(sums[0] + sums[1], 1.0),
+                "launch_ms": t_ms / n_launch, "transport_share_of_step": t_ms / max(tot_ms, 1e-9)}
+    if gfrac > 0.0:      # maps: the field gather against the MEASURED random-sector bandwidth (SURVEY §8(d)); report the lower fraction's bound
+        gb = gfrac * (sums[0] + sums[1]) * GATHER_BYTES_PER_GRID_STEP
+        ws = sum(s.nodes.nbytes for s in w.field.slabs if s.kind == 1)
+        key = "hbm_1GiB" if ws > (100 << 20) else "l2_64MB"
+        roofline["gather"] = {"achieved_GBps": gb / (t_ms * 1e-3) / 1e9, "peak_GBps": peaks["gather_GBps"][key],
+                              "peak_kind": f"measured random 32-byte-sector gather, working set {key} (map {ws / 1e6:.0f} MB)",
+                              "frac": gb / (t_ms * 1e-3) / 1e9 / peaks["gather_GBps"][key],
+                              "bytes_per_grid_step": GATHER_BYTES_PER_GRID_STEP, "grid_step_fraction": gfrac}
+    wall = tot_ms_max * 1e-3
+    entry = {"workload": w.name, "value": (null + real) / wall, "unit": UNIT, "steps": steps, "warmup": warmup,
+             "ms_per_step": tot_ms_max / max(steps, 1), "null_per_s": null / wall, "real_per_s": real / wall,
+             "avalanches_per_s": world * w.n_primaries * steps / wall, "electrons_per_step": electrons / max(steps, 1) / world,
+             "collisions_per_step": (null + real) / max(steps, 1) / world, "roofline": roofline,
+             "e2e": {"value": e2e_coll / e2e_s_max, "unit": UNIT, "h2d_bytes_per_step": int(w.n_primaries * 64),
+                     "d2h_bytes_per_step": int(sum(s["d2h"] for s in e2e) / max(len(e2e), 1)), "ms_per_step": 1e3 * e2e_s_max / max(steps, 1)},
+             "gpu_launches": int(launches), "config": config_dict(w, world), "capacity": w.capacity, "clocks": clocks}
+    if with_cpu:
+        entry["cpu_baseline"] = cpu_baseline_entry(w, sample, cores)
+    return entry, clocks
 
 
 def run_ours(args) -> None:
@@ -206,131 +396,36 @@ def run_ours(args) -> None:
 
     # weak scaling: every rank runs the whole workload on its own id range — avalanches are
     # independent, gas table and field are replicated, no data-path collective.
-    w = make_workload(args.workload, rank)
-    id_offset = rank * w.n_primaries
     ctx = avm.ctx_create(local_rank)
-    gg, fg = avm.gas_create(ctx, w.gas), avm.field_create(ctx, w.field)
-    L = w.gas.n_levels
-    has_b = any(v != 0.0 for v in w.field.B)
-    bufs = avm.RunBuffers(ctx, w.capacity, w.n_primaries, L)
-    prim_host = torch.from_numpy(w.primaries.copy()).pin_memory()
-    prim_dev = prim_host.to(ctx.device)
-    host = avm.HostBuffers(w.capacity, w.n_primaries, L, pinned=True)
+    peaks = measured_peaks(avm, ctx)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=ctx.device)       # > 126 MB L2
-    peak = fp64_peak(avm, ctx)
-
-    def barrier():
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    def device_step(seed):
-        """One pass of the hot path, primaries resident in HBM; device time by CUDA events on the ctx stream."""
-        flush.zero_()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        _, n = avm.run(ctx, gg, fg, prim_dev, bufs, seed=seed, t_max=w.t_max, id_offset=id_offset)
-        e1.record()
-        e1.synchronize()
-        t = bufs.tallies_u64.cpu().numpy().view(np.uint64)
-        k, kt = avm.run_stats(ctx)
-        return {"ms": e0.elapsed_time(e1), "n": n, "tallies": t, "launches": k, "transport_launches": kt,
-                "transport_ms": avm.run_transport_ms(ctx)}
-
-    def e2e_step(seed):
-        """The user's call: host primaries in (H2D inside avm_run), endpoints and tallies back to pinned host."""
-        flush.zero_()
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        _, n = avm.run(ctx, gg, fg, prim_host, bufs, seed=seed, t_max=w.t_max, id_offset=id_offset)
-        res = avm.fetch(ctx, bufs, n, host)
-        dt = time.perf_counter() - t0
-        d2h = n * (8 + 4 + 4 + 4 + 5 * 8 + 8 * 8) + w.n_primaries * 24 + (L + 4) * 8 + 40
-        return {"s": dt, "n": n, "tallies": res.tallies_u64.copy(), "d2h": d2h}
-
-    for i in range(args.warmup):
-        device_step(w.seed + 1000 + i)
-    sampler = ClockSampler(local_rank)
-    barrier()
-    sampler.start()
-    steps = [device_step(w.seed + i) for i in range(args.steps)]
-    barrier()
-    clocks = sampler.stop()
-
-    tot_ms = sum(s["ms"] for s in steps)
-    null = sum(int(s["tallies"][L]) for s in steps)
-    real = sum(int(s["tallies"][L + 1]) for s in steps)
-    electrons = sum(int(s["n"]) for s in steps)
-    launches = sum(s["launches"] for s in steps)
-    t_launches = sum(s["transport_launches"] for s in steps)
-    t_ms = sum(s["transport_ms"] for s in steps)
-    gfrac = grid_fraction(w.field)
-    fp64 = sum(alg_fp64(s["tallies"], L, w.gas.level_type, has_b, gfrac) for s in steps)
-
-    for i in range(min(args.warmup, 2)):
-        e2e_step(w.seed + 2000 + i)
-    barrier()
-    e2e = [e2e_step(w.seed + i) for i in range(args.steps)]
-    barrier()
-    e2e_s = sum(s["s"] for s in e2e)
-    e2e_coll = sum(int(s["tallies"][L]) + int(s["tallies"][L + 1]) for s in e2e)
-    e2e_d2h = sum(s["d2h"] for s in e2e) / max(len(e2e), 1)
-
-    vals = torch.tensor([tot_ms, e2e_s, t_ms], dtype=torch.float64, device=ctx.device)
-    sums = torch.tensor([null, real, electrons, launches, e2e_coll, fp64, t_launches], dtype=torch.float64, device=ctx.device)
-    if dist is not None:
-        dist.all_reduce(vals, op=dist.ReduceOp.MAX)          # reporting only: max time over ranks, job totals
-        dist.all_reduce(sums, op=dist.ReduceOp.SUM)
-    tot_ms, e2e_s, t_ms_max = (float(x) for x in vals.cpu())
-    null, real, electrons, launches, e2e_coll, fp64_all, t_launches_all = (float(x) for x in sums.cpu())
-    if rank != 0:
-        if dist is not None:
-            dist.destroy_process_group()
-        return
-
-    value = (null + real) / (tot_ms * 1e-3)
-    # roofline of the dominant kernel (transport_kernel), this rank: algorithmic FP64 thread-instructions per launch
-    # / its average launch duration (CUDA events inside avm_run, on the ctx stream)
-    achieved = (fp64 / max(t_launches, 1)) / ((t_ms / max(t_launches, 1)) * 1e-3)
-    roofline = {"bound": "alu", "kernel": "transport_kernel", "achieved": achieved / 1e12, "peak": peak["measured"] / 1e12,
-                "unit": "T FP64 thread-instr/s", "frac": achieved / peak["measured"],
-                "traffic": NCU_CAPTURE.get(w.name, {}).get("traffic"),
-                "traffic_source": "profiles/r1d_transport_ncu.md (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum, one launch)"
-                                  if w.name in NCU_CAPTURE else None,
-                "sass_fp64_per_collision_ncu": NCU_CAPTURE.get(w.name, {}).get("sass_fp64_per_collision"),
-                "fp64_pipe_active_pct_ncu": NCU_CAPTURE.get(w.name, {}).get("fp64_pipe_active_pct"),
-                "peak_source": "measured: avm_fp64_probe DFMA rate on this GPU in this run",
-                "peak_nominal": peak["nominal"] / 1e12,
-                "frac_of_nominal": achieved / peak["nominal"],
-                "alg_fp64_per_collision": fp64 / max(null / world + real / world, 1.0) if world == 1 else None,
-                "launch_ms": t_ms / max(t_launches, 1), "transport_share_of_step": t_ms / max(sum(s["ms"] for s in steps), 1e-9)}
-    if gfrac > 0.0:      # grid maps: the field gather's algorithmic bytes beside the ALU figure (DESIGN.md §6)
-        gb = gfrac * (null + real) / world * GATHER_BYTES_PER_GRID_STEP
-        roofline["field_gather_GBps"] = gb / (t_ms * 1e-3) / 1e9
-        roofline["field_gather_bytes_per_step"] = GATHER_BYTES_PER_GRID_STEP
-        roofline["grid_step_fraction"] = gfrac
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": tot_ms / max(args.steps, 1), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic",
-            "config": {"workload": w.name, "note": w.note, "n_primaries_per_gpu": w.n_primaries, "capacity": w.capacity,
-                       "l2": "256 MiB buffer written between timed iterations", "seed_per_step": "seed + step index",
-                       "parallelism": f"replicas over primaries x{world}, no collective"},
-            "null_per_s": null / (tot_ms * 1e-3), "real_per_s": real / (tot_ms * 1e-3),
-            "avalanches_per_s": world * w.n_primaries * args.steps / (tot_ms * 1e-3),
-            "electrons_per_step": electrons / max(args.steps, 1) / world,
-            "collisions_per_step": (null + real) / max(args.steps, 1) / world,
-            "e2e": {"value": e2e_coll / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(w.n_primaries * 64),
-                    "d2h_bytes_per_step": int(e2e_d2h), "ms_per_step": 1e3 * e2e_s / max(args.steps, 1)},
-            "gpu_launches": int(launches), "roofline": roofline, "clocks": clocks}
-    if world == 1 and not args.no_cpu_baseline:
-        cores = os.cpu_count() or 1
-        n_prim = min(w.n_primaries, args.ref_primaries) if args.ref_primaries > 0 else w.n_primaries
-        o = oracle_leg(w, n_prim, cores)
-        line["cpu_baseline"] = {"value": o["collisions"] / o["seconds"], "unit": UNIT, "cores": cores, "kind": "oracle",
-                                "sample": f"first {n_prim} of {w.n_primaries} primaries of {w.name}, seed {w.seed}, "
-                                          f"{o['collisions']} collisions in {o['seconds']:.2f} s",
-                                "avalanches_per_s": n_prim / o["seconds"]}
-    print(json.dumps(line), flush=True)
+    cores = os.cpu_count() or 1
+    with_cpu = world == 1 and not args.no_cpu_baseline
+    head = HEADLINE if args.workload == "all" else args.workload
+    per = []
+    for name, steps, sample in workload_list(args):
+        e, _ = bench_workload(avm, ctx, torch, dist, name, steps, args.warmup, sample, rank, world, peaks, flush, with_cpu, cores)
+        if e is not None:
+            per.append(e)
+        torch.cuda.empty_cache()
+    if rank == 0:
+        h = next(e for e in per if e["workload"] == head)
+        line = {"metric": METRIC, "value": h["value"], "unit": UNIT, "n_gpus": world, "steps": h["steps"], "warmup": args.warmup,
+                "ms_per_step": h["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic", "config": h["config"],
+                "null_per_s": h["null_per_s"], "real_per_s": h["real_per_s"], "avalanches_per_s": h["avalanches_per_s"],
+                "electrons_per_step": h["electrons_per_step"], "collisions_per_step": h["collisions_per_step"],
+                "e2e": h["e2e"], "gpu_launches": h["gpu_launches"], "roofline": h["roofline"], "clocks": h["clocks"],
+                "headline": f"{head}: the largest BASELINE config by collisions per step that fits the bench budget (DESIGN.md §6); "
+                            "all five configs are in per_config",
+                "measured_peaks": {"fp64_T_thread_instr_per_s": peaks["fp64_measured"] / 1e12, "gather_GBps": peaks["gather_GBps"],
+                                   "smem_random_8B_loads_per_s": peaks["smem_random_8B_loads_per_s"],
+                                   "hbm_copy_GBps_MEASURED_PEAKS": peaks["hbm_copy_GBps_MEASURED_PEAKS"]},
+                "kernel_source_hash": kernel_source_hash()}
+        if "cpu_baseline" in h:
+            line["cpu_baseline"] = h["cpu_baseline"]
+        line["per_config"] = [{k: v for k, v in e.items() if k not in ("config",)} | {"note": e["config"]["note"]} for e in per]
+        print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
 
@@ -338,11 +433,11 @@ def run_ours(args) -> None:
 def main() -> None:
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="config2")
+    ap.add_argument("--workload", default="all")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--ref-primaries", type=int, default=0, help="oracle legs: first n primaries only (0 = all)")
+    ap.add_argument("--ref-primaries", type=int, default=0, help="oracle legs: first n primaries only (0 = the workload's default sample)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -216,6 +216,20 @@ int32_t avm_philox_batch(avm_ctx*, uint64_t seed, int64_t n_items, const uint64_
 int32_t avm_fp64_probe(avm_ctx*, int32_t n_blocks, int32_t n_threads_per_block, int64_t iters, double* sink,
                        float* ms_out /*host*/);
 
+/* Random-gather probe: every thread issues `iters` independent 32-byte (one-sector) loads at random sector indices of
+ * the working set buf[0, bytes), bypassing L1.  With the working set inside L2 it measures the L2-resident random-sector
+ * rate, far beyond L2 the HBM one: the denominators of the field-gather roofline of the map configs (SURVEY.md §7 stage
+ * 0, §8(d): steps/s x 128 B / measured gather bandwidth; PAPER.md:83 for the field data that is gathered).  buf: DEVICE,
+ * 32-byte aligned, contents irrelevant; sink: DEVICE [n_blocks * n_threads_per_block] u64; n_threads_per_block <= 256.
+ * Bytes moved = n_blocks * n_threads_per_block * iters * 32. */
+int32_t avm_gather_probe(avm_ctx*, const void* buf, size_t bytes, int32_t n_blocks, int32_t n_threads_per_block,
+                         int64_t iters, uint64_t* sink, float* ms_out /*host*/);
+/* Shared-memory random-load probe: `iters` random 8-byte loads per thread from a table of table_bytes in dynamic shared
+ * memory (the access pattern of the threshold table, one record per step).  sink as above;
+ * n_threads_per_block <= 512.  Loads = n_blocks * n_threads_per_block * iters. */
+int32_t avm_smem_probe(avm_ctx*, int32_t table_bytes, int32_t n_blocks, int32_t n_threads_per_block, int64_t iters,
+                       uint64_t* sink, float* ms_out /*host*/);
+
 #ifdef __cplusplus
 }
 #endif

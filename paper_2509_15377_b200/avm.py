@@ -27,7 +27,7 @@ MAX_LEVELS, MAX_SLABS = 64, 8
 EXPORTS = ["avm_last_error", "avm_ctx_create", "avm_ctx_destroy", "avm_ctx_sm_count", "avm_gas_bytes",
            "avm_gas_create", "avm_gas_destroy", "avm_gas_nu_hat", "avm_field_create", "avm_field_destroy",
            "avm_field_eval", "avm_run_workspace_bytes", "avm_run", "avm_run_stats", "avm_run_transport_ms", "avm_fetch", "avm_step_batch", "avm_step_batch_form",
-           "avm_philox_batch", "avm_fp64_probe"]
+           "avm_philox_batch", "avm_fp64_probe", "avm_gather_probe", "avm_smem_probe"]
 
 
 class AvmError(RuntimeError):
@@ -74,7 +74,8 @@ _lib.avm_gas_nu_hat.restype = C.c_double
 _lib.avm_gas_nu_hat.argtypes = [C.c_void_p]
 for _n in ("avm_ctx_create", "avm_ctx_destroy", "avm_ctx_sm_count", "avm_gas_create", "avm_gas_destroy",
            "avm_field_create", "avm_field_destroy", "avm_field_eval", "avm_run", "avm_run_stats", "avm_fetch",
-           "avm_step_batch", "avm_step_batch_form", "avm_philox_batch", "avm_fp64_probe", "avm_run_transport_ms"):
+           "avm_step_batch", "avm_step_batch_form", "avm_philox_batch", "avm_fp64_probe", "avm_run_transport_ms",
+           "avm_gather_probe", "avm_smem_probe"):
     getattr(_lib, _n).restype = C.c_int32
 _lib.avm_run_transport_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
 _lib.avm_ctx_create.argtypes = [C.c_int32, C.c_void_p, C.POINTER(C.c_void_p)]
@@ -92,6 +93,8 @@ _lib.avm_fetch.argtypes = [C.c_void_p, C.POINTER(_Outputs), C.c_int64, C.c_int64
 _lib.avm_step_batch.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint64, C.c_double, C.c_int64] + [C.c_void_p] * 9
 _lib.avm_step_batch_form.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint64, C.c_double, C.c_int32, C.c_int32, C.c_int64] + [C.c_void_p] * 9
 _lib.avm_philox_batch.argtypes = [C.c_void_p, C.c_uint64, C.c_int64] + [C.c_void_p] * 5
+_lib.avm_gather_probe.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.c_int32, C.c_int32, C.c_int64, C.c_void_p, C.POINTER(C.c_float)]
+_lib.avm_smem_probe.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_int64, C.c_void_p, C.POINTER(C.c_float)]
 _lib.avm_fp64_probe.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int64, C.c_void_p, C.POINTER(C.c_float)]
 
 
@@ -316,6 +319,27 @@ def fp64_probe(ctx: Context, n_blocks=None, n_threads=256, iters=1 << 16) -> dic
     _check(_lib.avm_fp64_probe(ctx._h, nb, n_threads, iters, _dev(sink), C.byref(ms)))
     n_fma = float(nb) * n_threads * iters * 8
     return {"ms": ms.value, "dfma_per_s": n_fma / (ms.value * 1e-3), "threads": nb * n_threads}
+
+
+def gather_probe(ctx: Context, working_set_bytes: int, iters: int = 2048, blocks_per_sm: int = 8, n_threads: int = 256) -> dict:
+    """Measured random 32-byte-sector gather bandwidth over a working set of the given size (L2-resident or HBM)."""
+    buf = torch.zeros(int(working_set_bytes) // 8, dtype=torch.int64, device=ctx.device)
+    nb = ctx.sm_count * blocks_per_sm
+    sink = ctx.empty(nb * n_threads, torch.int64)
+    ms = C.c_float(0)
+    _check(_lib.avm_gather_probe(ctx._h, _dev(buf), buf.numel() * 8, nb, n_threads, iters, _dev(sink), C.byref(ms)))
+    moved = float(nb) * n_threads * iters * 32
+    return {"ms": ms.value, "GBps": moved / (ms.value * 1e-3) / 1e9, "sectors_per_s": moved / 32 / (ms.value * 1e-3),
+            "working_set_bytes": int(buf.numel() * 8)}
+
+
+def smem_probe(ctx: Context, table_bytes: int = 160000, iters: int = 1 << 14, n_threads: int = 512) -> dict:
+    """Measured shared-memory random 8-byte loads per second, one CTA per SM."""
+    nb = ctx.sm_count
+    sink = ctx.empty(nb * n_threads, torch.int64)
+    ms = C.c_float(0)
+    _check(_lib.avm_smem_probe(ctx._h, int(table_bytes), nb, n_threads, iters, _dev(sink), C.byref(ms)))
+    return {"ms": ms.value, "loads_per_s": float(nb) * n_threads * iters / (ms.value * 1e-3)}
 
 
 class RunBuffers:

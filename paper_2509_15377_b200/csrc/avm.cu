@@ -714,6 +714,37 @@ __global__ void __launch_bounds__(256) fp64_probe_kernel(const long long iters, 
   sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
 }
 
+// Random-gather probes: the denominators of the map configs' roofline (SURVEY.md §7 stage 0, §8(d)).
+// Every thread issues `iters` independent 32-byte loads (one sector, two 16-byte halves) at xorshift-random sector
+// indices of the working set, bypassing L1 (ld.global.cg): the sustained random-sector rate of L2 (working set inside
+// the 126 MB L2) or of HBM (working set far beyond it).
+__global__ void __launch_bounds__(256) gather_probe_kernel(const uint4* __restrict__ buf, const unsigned long long n_sectors,
+                                                          const long long iters, unsigned long long* sink) {
+  unsigned long long s = 0x9E3779B97F4A7C15ull * ((unsigned long long)blockIdx.x * blockDim.x + threadIdx.x + 1ull);
+  unsigned int acc = 0u;
+  for (long long i = 0; i < iters; ++i) {
+    s ^= s << 13; s ^= s >> 7; s ^= s << 17;
+    const unsigned long long j = __umul64hi(s, n_sectors);          // uniform in [0, n_sectors)
+    const uint4 a = __ldcg(buf + 2 * j), b = __ldcg(buf + 2 * j + 1);
+    acc ^= a.x ^ a.w ^ b.y ^ b.z;
+  }
+  sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = acc;
+}
+// Shared-memory random 8-byte loads per second (the 160 KB threshold table's access pattern: one record per step).
+__global__ void __launch_bounds__(512) smem_probe_kernel(const int n_entries, const long long iters, unsigned long long* sink) {
+  extern __shared__ __align__(16) unsigned char s_probe[];
+  unsigned long long* tab = reinterpret_cast<unsigned long long*>(s_probe);
+  for (int i = threadIdx.x; i < n_entries; i += blockDim.x) tab[i] = 0x100000001ull * (unsigned)i;
+  __syncthreads();
+  unsigned int s = 2654435761u * (blockIdx.x * blockDim.x + threadIdx.x + 1u);
+  unsigned long long acc = 0ull;
+  for (long long i = 0; i < iters; ++i) {
+    s ^= s << 13; s ^= s >> 17; s ^= s << 5;
+    acc += tab[__umulhi(s, (unsigned)n_entries)];
+  }
+  sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = acc;
+}
+
 }  // namespace
 
 // =================================================================================================================
@@ -1239,6 +1270,48 @@ int32_t avm_philox_batch(avm_ctx* ctx, uint64_t seed, int64_t n, const uint64_t*
   if (n == 0) return AVM_OK;
   AVM_CUDA(cudaSetDevice(ctx->device));
   AVM_CUDA(launch(ctx, philox_batch_kernel, dim3((unsigned)((n + 255) / 256)), dim3(256), seed, n, id, n_idx, block, words, u));
+  return AVM_OK;
+}
+
+int32_t avm_gather_probe(avm_ctx* ctx, const void* buf, size_t bytes, int32_t n_blocks, int32_t n_threads, int64_t iters,
+                         uint64_t* sink, float* ms_out) {
+  if (!ctx || !buf || bytes < 64 || ((uintptr_t)buf & 31u) || n_blocks < 1 || n_threads < 32 || n_threads > 256 || iters < 1 || !sink || !ms_out)
+    return fail(AVM_ERR_INVALID_ARG, "gather_probe: bad argument");
+  AVM_CUDA(cudaSetDevice(ctx->device));
+  cudaEvent_t e0, e1;
+  AVM_CUDA(cudaEventCreate(&e0));
+  AVM_CUDA(cudaEventCreate(&e1));
+  const unsigned long long n_sectors = bytes / 32;
+  gather_probe_kernel<<<n_blocks, n_threads, 0, ctx->stream>>>((const uint4*)buf, n_sectors, iters / 8 > 0 ? iters / 8 : 1, (unsigned long long*)sink);   // warm-up
+  AVM_CUDA(cudaEventRecord(e0, ctx->stream));
+  gather_probe_kernel<<<n_blocks, n_threads, 0, ctx->stream>>>((const uint4*)buf, n_sectors, iters, (unsigned long long*)sink);
+  AVM_CUDA(cudaEventRecord(e1, ctx->stream));
+  AVM_CUDA(cudaGetLastError());
+  AVM_CUDA(cudaEventSynchronize(e1));
+  AVM_CUDA(cudaEventElapsedTime(ms_out, e0, e1));
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  return AVM_OK;
+}
+
+int32_t avm_smem_probe(avm_ctx* ctx, int32_t table_bytes, int32_t n_blocks, int32_t n_threads, int64_t iters, uint64_t* sink,
+                       float* ms_out) {
+  if (!ctx || table_bytes < 64 || table_bytes > (int32_t)kMaxDynSmem || n_blocks < 1 || n_threads < 32 || n_threads > 512 || iters < 1 || !sink || !ms_out)
+    return fail(AVM_ERR_INVALID_ARG, "smem_probe: bad argument");
+  AVM_CUDA(cudaSetDevice(ctx->device));
+  AVM_CUDA(cudaFuncSetAttribute(smem_probe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, table_bytes));
+  cudaEvent_t e0, e1;
+  AVM_CUDA(cudaEventCreate(&e0));
+  AVM_CUDA(cudaEventCreate(&e1));
+  smem_probe_kernel<<<n_blocks, n_threads, table_bytes, ctx->stream>>>(table_bytes / 8, iters / 8 > 0 ? iters / 8 : 1, (unsigned long long*)sink);
+  AVM_CUDA(cudaEventRecord(e0, ctx->stream));
+  smem_probe_kernel<<<n_blocks, n_threads, table_bytes, ctx->stream>>>(table_bytes / 8, iters, (unsigned long long*)sink);
+  AVM_CUDA(cudaEventRecord(e1, ctx->stream));
+  AVM_CUDA(cudaGetLastError());
+  AVM_CUDA(cudaEventSynchronize(e1));
+  AVM_CUDA(cudaEventElapsedTime(ms_out, e0, e1));
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
   return AVM_OK;
 }
 
