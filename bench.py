@@ -354,11 +354,12 @@ def bench_workload(avm, ctx, torch, dist, name, steps, warmup, sample, rank, wor
                 "launch_ms": t_ms / n_launch, "transport_share_of_step": t_ms / max(tot_ms, 1e-9)}
     if gfrac > 0.0:      # maps: the field gather against the MEASURED random-sector bandwidth; report the lower fraction's bound
         gb = gfrac * (sums[0] + sums[1]) * GATHER_BYTES_PER_GRID_STEP
-        ws = sum(s.nodes.nbytes for s in w.field.slabs if s.kind == 1)
-        key = "hbm_1GiB" if ws > (100 << 20) else "l2_64MB"
-        roofline["gather"] = {"achieved_GBps": gb / (t_ms * 1e-3) / 1e9, "peak_GBps": peaks["gather_GBps"][key],
-                              "peak_kind": f"measured random 32-byte-sector gather, working set {key} (map {ws / 1e6:.0f} MB)",
-                              "frac": gb / (t_ms * 1e-3) / 1e9 / peaks["gather_GBps"][key],
+        # the touched region (the holes' neighbourhood, a few MB per map) stays in L2 / L1 (DRAM traffic is ~3 B per step,
+        # profiles/): the L2-resident random-sector rate is the binding denominator; the HBM one is printed beside it
+        ach = gb / (t_ms * 1e-3) / 1e9
+        roofline["gather"] = {"achieved_GBps": ach, "peak_GBps": peaks["gather_GBps"]["l2_64MB"],
+                              "peak_kind": "measured random 32-byte-sector gather, 64 MB working set (L2-resident), this run",
+                              "frac": ach / peaks["gather_GBps"]["l2_64MB"], "frac_vs_hbm_random_gather": ach / peaks["gather_GBps"]["hbm_1GiB"],
                               "bytes_per_grid_step": GATHER_BYTES_PER_GRID_STEP, "grid_step_fraction": gfrac}
     wall = tot_ms_max * 1e-3
     entry = {"workload": w.name, "value": (null + real) / wall, "unit": UNIT, "steps": steps, "warmup": warmup,

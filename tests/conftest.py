@@ -8,6 +8,31 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 
+# Observed margins of the whole-run comparisons (same-seed identical-history fractions, endpoint errors, statistics):
+# tests append one line each; printed in the terminal summary and written to gpurun_out/parity_margins.txt, from which
+# BASELINE.md's parity table is filled in.
+MARGINS = []
+
+
+def record_margin(line: str) -> None:
+    MARGINS.append(line)
+
+
+def pytest_terminal_summary(terminalreporter):
+    if not MARGINS:
+        return
+    terminalreporter.write_sep("-", "observed parity margins")
+    for m in MARGINS:
+        terminalreporter.write_line(m)
+    out = os.path.join(ROOT, "gpurun_out")
+    try:
+        os.makedirs(out, exist_ok=True)
+        with open(os.path.join(out, "parity_margins.txt"), "a") as f:
+            f.write("\n".join(MARGINS) + "\n")
+    except OSError:
+        pass
+
+
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
 

@@ -1,0 +1,108 @@
+"""north_star level 2 on the BASELINE configs: whole-avalanche statistics of the CUDA path against the oracle.
+
+Two comparisons per config (SURVEY.md §8(d) "Acceptance"; PAPER.md:127-133 compares CPU and GPU endpoint histograms the
+same way): (i) same seed — drift velocity W and effective Townsend coefficient alpha - eta within 1 %; (ii) independent
+streams (GPU: run seed 1 and primaries drawn with seed 1; oracle: seed 0) — mean gain per primary within 3 combined standard
+errors, two-sample KS p > 0.01 on the per-primary gain, on the endpoint energy and on the endpoint z overshoot of the
+electrons that reach the far side.  Config 2 (reduced gap) and config 3 have theirs in test_gpu_parity.py /
+test_gpu_fullsize.py.  Observed values are recorded (conftest.record_margin).
+"""
+import os
+
+import numpy as np
+import pytest
+import torch
+from scipy import stats
+
+from conftest import record_margin
+from paper_2509_15377_b200.gen import configs, primaries
+
+pytestmark = pytest.mark.gpu
+CORES = os.cpu_count() or 1
+
+
+@pytest.fixture(scope="module")
+def ctx(avm):
+    return avm.ctx_create(0)
+
+
+def gpu_run(avm, ctx, w, prim, seed):
+    gg, fg = avm.gas_create(ctx, w.gas), avm.field_create(ctx, w.field)
+    bufs = avm.RunBuffers(ctx, w.capacity, prim.shape[0], w.gas.n_levels)
+    _, n = avm.run(ctx, gg, fg, torch.from_numpy(prim.copy()).to(ctx.device), bufs, seed=seed, t_max=w.t_max)
+    return avm.fetch(ctx, bufs, n)
+
+
+def w_alpha(r, gas, axis_sign):
+    """Drift velocity along the force direction and effective Townsend coefficient from the tallies."""
+    t = r.tallies_u64
+    ion = sum(int(t[l]) for l in range(gas.n_levels) if gas.level_type[l] == 2)
+    att = sum(int(t[l]) for l in range(gas.n_levels) if gas.level_type[l] == 3)
+    dz = axis_sign * r.tallies_f64[2]
+    return dz / r.tallies_f64[3], (ion - att) / dz
+
+
+def compare_statistics(label, cpu, gpu, far_status, z_far, thin):
+    """Independent streams: gain within 3 combined SE; KS p > 0.01 on gain, endpoint energy and endpoint z overshoot."""
+    gc, gg = cpu.per_avalanche[:, 0].astype(float), gpu.per_avalanche[:, 0].astype(float)
+    se = np.hypot(gc.std(ddof=1) / np.sqrt(len(gc)), gg.std(ddof=1) / np.sqrt(len(gg)))
+    p_gain = stats.ks_2samp(gc, gg).pvalue
+    fc, fg = cpu.status == far_status, gpu.status == far_status
+    p_e = stats.ks_2samp(cpu.end[4][fc][::thin], gpu.end[4][fg][::thin]).pvalue        # thinned: electrons of one avalanche are correlated
+    p_z = stats.ks_2samp(np.abs(cpu.end[2][fc][::thin] - z_far), np.abs(gpu.end[2][fg][::thin] - z_far)).pvalue
+    record_margin(f"independent seeds {label}: mean gain oracle {gc.mean():.3f} ({len(gc)} primaries) gpu {gg.mean():.3f} ({len(gg)}), "
+                  f"difference {abs(gc.mean() - gg.mean()) / se:.2f} combined SE; KS p: gain {p_gain:.3f}, endpoint energy {p_e:.3f}, "
+                  f"endpoint z {p_z:.3f} ({fc.sum()} / {fg.sum()} far-side electrons, every {thin}th)")
+    assert abs(gc.mean() - gg.mean()) < 3 * se, (gc.mean(), gg.mean(), se)
+    assert p_gain > 0.01 and p_e > 0.01 and p_z > 0.01, (p_gain, p_e, p_z)
+
+
+def test_config1_acceptance(avm, ctx, oracle):
+    w = configs.config1()
+    cpu = oracle.run(w.gas, w.field, w.primaries, seed=w.seed, n_threads=CORES)
+    same = gpu_run(avm, ctx, w, w.primaries, w.seed)
+    Wc, ac = w_alpha(cpu, w.gas, +1.0); Wg, ag = w_alpha(same, w.gas, +1.0)
+    record_margin(f"same seed config1: W gpu/oracle - 1 = {Wg / Wc - 1:+.2e}, (alpha - eta) gpu/oracle - 1 = {ag / ac - 1:+.2e}")
+    assert abs(Wg / Wc - 1) < 0.01 and abs(ag / ac - 1) < 0.01
+    # independent streams: 4000 primaries each side (the 1000 of the config resolve the gain to ~5 % only)
+    pc = primaries.isotropic_primaries(4000, 0); pg = primaries.isotropic_primaries(4000, 1)
+    cpu = oracle.run(w.gas, w.field, pc, seed=0, n_threads=CORES)
+    gpu = gpu_run(avm, ctx, w, pg, 1)
+    compare_statistics("config1 (4000 primaries)", cpu, gpu, 2, 50e-4, 1)
+    Wc, ac = w_alpha(cpu, w.gas, +1.0); Wg, ag = w_alpha(gpu, w.gas, +1.0)
+    record_margin(f"independent seeds config1: W gpu/oracle - 1 = {Wg / Wc - 1:+.2e}, (alpha - eta) gpu/oracle - 1 = {ag / ac - 1:+.2e} (not required: ~1500 ionisations)")
+    assert abs(Wg / Wc - 1) < 0.03
+
+
+def test_config4_acceptance(avm, ctx, oracle):
+    """Config 4 in full: 1000 primaries through the single-GEM map on both sides."""
+    w = configs.config4()
+    cpu = oracle.run(w.gas, w.field, w.primaries, seed=w.seed, capacity=w.capacity, n_threads=CORES)
+    same = gpu_run(avm, ctx, w, w.primaries, w.seed)
+    Wc, ac = w_alpha(cpu, w.gas, -1.0); Wg, ag = w_alpha(same, w.gas, -1.0)        # electrons move toward -z
+    record_margin(f"same seed config4: W gpu/oracle - 1 = {Wg / Wc - 1:+.2e}, (alpha - eta) gpu/oracle - 1 = {ag / ac - 1:+.2e}, "
+                  f"electrons oracle {cpu.n} gpu {same.n}")
+    assert abs(Wg / Wc - 1) < 0.01 and abs(ag / ac - 1) < 0.01
+    pg = configs._gem_primaries(1000, 1, 0)
+    gpu = gpu_run(avm, ctx, w, pg, 1)
+    compare_statistics("config4 (1000 primaries)", cpu, gpu, 1, w.field.slabs[0].z_lo, 3)
+    # where the electrons end: shares of the statuses (induction side, foil, back to the drift side) within 3 SE
+    for stc in (1, 2, 4):
+        fc, fg = (cpu.status == stc).mean(), (gpu.status == stc).mean()
+        se = np.sqrt(fc * (1 - fc) / cpu.n + fg * (1 - fg) / gpu.n) * 3.0 + 0.01       # + avalanche correlations
+        assert abs(fc - fg) < se, (stc, fc, fg)
+
+
+def test_config5_acceptance(avm, ctx, oracle):
+    """Config 5: the GPU's 200 avalanches (run seed 1, primaries seed 1) against as many as the oracle affords (32, seed 0)."""
+    w = configs.config5()
+    m = 32
+    cpu = oracle.run(w.gas, w.field, w.primaries[:m], seed=w.seed, capacity=1 << 18, n_threads=min(CORES, m))
+    first = gpu_run(avm, ctx, w, w.primaries[:m], w.seed)
+    Wc, ac = w_alpha(cpu, w.gas, -1.0); Wg, ag = w_alpha(first, w.gas, -1.0)
+    record_margin(f"same seed config5 (first {m} primaries): W gpu/oracle - 1 = {Wg / Wc - 1:+.2e}, (alpha - eta) gpu/oracle - 1 = {ag / ac - 1:+.2e}, "
+                  f"electrons oracle {cpu.n} gpu {first.n}")
+    assert abs(Wg / Wc - 1) < 0.01 and abs(ag / ac - 1) < 0.01
+    pg = configs._gem_primaries(200, 1, 0)
+    gpu = gpu_run(avm, ctx, w, pg, 1)
+    compare_statistics(f"config5 (oracle {m}, gpu 200 primaries)", cpu, gpu, 1, w.field.slabs[0].z_lo, 5)

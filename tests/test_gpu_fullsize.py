@@ -1,4 +1,9 @@
-"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (primaries resident on the
+"""Thresholds of the same-seed comparisons = the observed values (gpurun_out/parity_margins.txt, copied into BASELINE.md §4)
+with a stated margin: round 2 observed 100 % identical histories on configs 1-4 in full and on config 5's first 4
+avalanches (99.8 % on its first 6: one electron of 444), endpoint errors of identical histories <= 3.4e-7 (config 4) and
+<= 1.8e-5 (config 5, histories of 2e6 steps); required here: >= 99.5 % / 98 % identical, errors <= 3e-6 / 1e-4.
+
+GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (primaries resident on the
 device, the workload's capacity, default launch shape).
 
 Configs 1, 2 and 4 are small enough for the oracle in full: the whole run is compared electron by electron.  Configs 3
@@ -66,7 +71,7 @@ def test_config2_full_size(avm, ctx, oracle):
     check_invariants(gpu, w)
     cpu = oracle.run(w.gas, w.field, w.primaries, seed=w.seed, capacity=w.capacity, n_threads=CORES)
     assert cpu.n > 100000
-    assert_run_same_seed(cpu, gpu, w.gas.n_levels, min_identical=0.999)
+    assert_run_same_seed(cpu, gpu, w.gas.n_levels, min_identical=0.999, label='config2 full size')
     L = w.gas.n_levels
     assert abs(int(gpu.tallies_u64[L + 3]) / int(cpu.tallies_u64[L + 3]) - 1) < 1e-3
     assert abs(gpu.n / cpu.n - 1) < 1e-3
@@ -82,7 +87,7 @@ def test_config3_time_cut_full_size(avm, ctx, oracle):
     assert (gpu.status == 6).sum() > 0.9 * w.n_primaries               # almost all reach the time cut
     m = 96
     cpu = oracle.run(w.gas, w.field, w.primaries[:m], seed=w.seed, t_max=20.0, n_threads=CORES)
-    assert_run_same_seed(cpu, first_avalanches(gpu, m), w.gas.n_levels, min_identical=0.97, end_rtol=1e-7)
+    assert_run_same_seed(cpu, first_avalanches(gpu, m), w.gas.n_levels, min_identical=0.99, end_rtol=1e-9, label='config3 time cut, first 96 avalanches of the full-size run')
 
 
 def test_config4_full_size(avm, ctx, oracle):
@@ -91,9 +96,9 @@ def test_config4_full_size(avm, ctx, oracle):
     check_invariants(gpu, w)
     cpu = oracle.run(w.gas, w.field, w.primaries, seed=w.seed, capacity=w.capacity, n_threads=CORES)
     assert cpu.n > 5000
-    assert_run_same_seed(cpu, gpu, w.gas.n_levels, min_identical=0.90, end_rtol=1e-6, tail=0.05)
+    assert_run_same_seed(cpu, gpu, w.gas.n_levels, min_identical=0.995, end_rtol=3e-6, label='config4 full size')
     L = w.gas.n_levels
-    assert abs(int(gpu.tallies_u64[L + 3]) / int(cpu.tallies_u64[L + 3]) - 1) < 0.02
+    assert abs(int(gpu.tallies_u64[L + 3]) / int(cpu.tallies_u64[L + 3]) - 1) < 2e-3
 
 
 def test_config5_full_size(avm, ctx, oracle):
@@ -102,7 +107,7 @@ def test_config5_full_size(avm, ctx, oracle):
     check_invariants(gpu, w)
     m = 4
     cpu = oracle.run(w.gas, w.field, w.primaries[:m], seed=w.seed, capacity=1 << 16, n_threads=m)
-    assert_run_same_seed(cpu, first_avalanches(gpu, m), w.gas.n_levels, min_identical=0.80, end_rtol=1e-6, tail=0.05)
+    assert_run_same_seed(cpu, first_avalanches(gpu, m), w.gas.n_levels, min_identical=0.98, end_rtol=1e-4, label='config5 full size, first 4 avalanches')
 
 
 def test_config3_drift_lorentz_angle_and_diffusion(avm, ctx, oracle):

@@ -198,7 +198,7 @@ def test_step_parity_textbook_gases(avm, ctx, oracle):
 
 
 # ---- whole avalanches -------------------------------------------------------------------------------------
-def assert_run_same_seed(cpu, gpu, n_levels, min_identical=0.999, end_rtol=1e-9, tail=0.0, tail_rtol=1e-3):
+def assert_run_same_seed(cpu, gpu, n_levels, min_identical=0.999, end_rtol=1e-9, tail=0.0, tail_rtol=1e-3, label=None):
     """Same seed, same ids: the two runs are the same avalanche electron by electron until rounding flips a
     discrete decision.  Counts must agree exactly for >= min_identical of the electrons.
 
@@ -209,8 +209,18 @@ def assert_run_same_seed(cpu, gpu, n_levels, min_identical=0.999, end_rtol=1e-9,
     (PAPER.md:117); the map tests allow a few electrons of several hundred to reach 1e-5..1e-3."""
     c, g = cpu.sorted_by_id(), gpu.sorted_by_id()
     common, ic, ig = np.intersect1d(c.id, g.id, return_indices=True)
-    assert len(common) >= min_identical * max(c.n, g.n), (c.n, g.n, len(common))
     same = (c.n_steps[ic] == g.n_steps[ig]) & (c.status[ic] == g.status[ig]) & (c.avalanche[ic] == g.avalanche[ig])
+    if label is not None:                        # the observed margins, whatever the thresholds (conftest.record_margin)
+        from conftest import record_margin
+        jc, jg = ic[same], ig[same]
+        e_r = np.abs(c.end[0:3, jc] - g.end[0:3, jg]).max(axis=0) / np.maximum(np.abs(c.end[0:3, jc]).max(), 1e-4) if len(jc) else np.zeros(1)
+        e_t = np.abs(c.end[3, jc] - g.end[3, jg]) / np.maximum(c.end[3, jc], 1e-6) if len(jc) else np.zeros(1)
+        e_e = np.abs(c.end[4, jc] - g.end[4, jg]) / (10 * np.maximum(c.end[4, jc], 1.0)) if len(jc) else np.zeros(1)
+        e_all = np.maximum(np.maximum(e_r, e_t), e_e)
+        record_margin(f"same-seed {label}: electrons cpu {c.n} gpu {g.n}, common ids {len(common) / max(c.n, g.n):.5f}, identical histories "
+                      f"{same.mean():.5f} (required {min_identical}); endpoint error of identical histories: median {np.median(e_all):.2e}, "
+                      f"p99.9 {np.quantile(e_all, 0.999):.2e}, worst {e_all.max():.2e} (end_rtol {end_rtol}, tail {tail})")
+    assert len(common) >= min_identical * max(c.n, g.n), (c.n, g.n, len(common))
     assert same.mean() >= min_identical, same.mean()
     ic, ig = ic[same], ig[same]
     # identical histories: endpoints agree to accumulated rounding (1e-9 of the path scale is generous for the ~1e4-step
@@ -234,7 +244,7 @@ def test_config1_same_seed_identical_avalanches(avm, ctx, oracle, g0):
     p = primaries.isotropic_primaries(1000, 0)
     cpu = oracle.run(g0, fd, p, seed=0)
     gpu = avm.simulate(ctx, avm.gas_create(ctx, g0), avm.field_create(ctx, fd), p, seed=0)
-    frac, n = assert_run_same_seed(cpu, gpu, g0.n_levels)
+    frac, n = assert_run_same_seed(cpu, gpu, g0.n_levels, label='config1 full')
     L = g0.n_levels
     if frac == 1.0 and cpu.n == gpu.n:
         assert np.array_equal(cpu.tallies_u64, gpu.tallies_u64)
@@ -480,10 +490,10 @@ def test_config4_same_seed_run(avm, ctx, oracle, g0, cfg4):
     gpu = avm.simulate(ctx, avm.gas_create(ctx, g0), avm.field_create(ctx, w.field), w.primaries, seed=w.seed,
                        capacity=1 << 15)
     assert cpu.n > 100 and (cpu.status == 4).sum() > 20 and (cpu.status == 1).sum() > 10
-    # ~3e5 steps per electron: a rounding difference can flip one decision in a history; allow a few per cent
-    assert_run_same_seed(cpu, gpu, g0.n_levels, min_identical=0.90, end_rtol=1e-6, tail=0.05)
+    # ~3e5 steps per electron: a rounding difference can flip one decision in a history (observed: none of 281)
+    assert_run_same_seed(cpu, gpu, g0.n_levels, min_identical=0.99, end_rtol=1e-6, label='config4 first 24 primaries')
     L = g0.n_levels
-    assert abs(int(gpu.tallies_u64[L + 3]) / int(cpu.tallies_u64[L + 3]) - 1) < 0.05
+    assert abs(int(gpu.tallies_u64[L + 3]) / int(cpu.tallies_u64[L + 3]) - 1) < 5e-3
     t = gpu.tallies_u64
     assert gpu.n == 24 + int(t[14] + t[15]) and int(gpu.n_steps.sum()) == int(t[L + 3])
 
@@ -505,7 +515,7 @@ def test_config5_triple_gem_same_seed_run(avm, ctx, oracle, g0):
     cpu = oracle.run(w.gas, w.field, w.primaries, seed=w.seed, capacity=1 << 16, n_threads=6)
     gpu = avm.simulate(ctx, avm.gas_create(ctx, g0), fg, w.primaries, seed=w.seed, capacity=1 << 16)
     assert cpu.n > 50
-    assert_run_same_seed(cpu, gpu, g0.n_levels, min_identical=0.80, end_rtol=1e-6, tail=0.05)
+    assert_run_same_seed(cpu, gpu, g0.n_levels, min_identical=0.985, end_rtol=1e-4, label='config5 first 6 primaries')
     # what is unique regardless of rounding-flipped histories: bookkeeping on the GPU result
     L = g0.n_levels
     t = gpu.tallies_u64
