@@ -7,6 +7,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstring>
+#include <limits>
 #include <string>
 #include <thread>
 #include <vector>
@@ -58,12 +59,23 @@ void uniform_pair(uint64_t seed, uint64_t id, uint32_t n, uint32_t block, double
 }
 
 // ---- data ---------------------------------------------------------------------------------------------
+// NEXT-1: the energy-banded null-collision rate, DESIGN.md §3.5 readings N1-N6.  nu[k][j] bounds the
+// total collision rate over every energy an electron that starts a flight in energy band k, under an acceleration of
+// class j, can reach within dtmax[k][j]; a flight drawn longer than dtmax is cut there and counted as a null collision
+// (the exponential is memoryless: thinning with a piecewise-constant majorant is exact).
+struct Majorant {
+  int shift = 0, K = 0, J = 0;
+  std::vector<double> a2;                       // [J]: squared upper edge of acceleration class j
+  std::vector<double> nu, inv_nu, dtmax;        // [K][J+1]; column J = accelerations above every class: global rate, no cut
+};
+
 struct Gas {
   int nb = 0, L = 0;
   double e_max = 0, inv_de = 0, nu_hat = 0, inv_nu_hat = 0;
   const double* cum = nullptr;
   const uint8_t* type = nullptr;
   const double *loss = nullptr, *recoil = nullptr, *w = nullptr;
+  Majorant M;
 };
 
 struct Electron {
@@ -76,9 +88,67 @@ struct Electron {
 
 struct Tally {
   std::vector<uint64_t> level;
-  uint64_t n_null = 0, n_real = 0, n_overflow = 0, n_steps = 0;
+  uint64_t n_null = 0, n_real = 0, n_overflow = 0, n_steps = 0, n_viol = 0;
   double sdx = 0, sdy = 0, sdz = 0, sdt = 0, sloss = 0;
 };
+
+// N1-N4: the table of banded rates.  Bands: 2^shift energy bins each, shift the largest with nb >> shift >= 256 (else 0).
+// Acceleration classes: upper edges A_j = a0 2^(j/2), a0 = kappa x 250 V/cm, j = 0 .. 24 (250 V/cm .. 1.02 MV/cm).
+// For band k (upper energy edge e_hi) and class j: a flight of at most dt = m / nu from an energy <= e_hi ends with speed
+// <= c2 sqrt(e_hi) + A_j dt, i.e. (one bin of slack) in an energy bin <= b_r(nu); with P[b] = max of the total rate over
+// bins 0 .. b and f(nu) = P[b_r(nu)] (non-increasing in nu), nu1 = f(P[last bin of the band]) satisfies nu1 >= f(nu1): a
+// valid bound; it is tightened while f(f(nu)) stays below.  m is the candidate of {1/2, 1, 2, 4, 8, 16} with the fewest
+// expected steps per unit time, nu / (1 - exp(-m)).  The last band also holds the energies above the table (R5), which
+// only the global maximum bounds.
+void build_majorant(Gas& g) {
+  Majorant& M = g.M;
+  const int nb = g.nb;
+  std::vector<double> P(nb);
+  double run = 0.0;
+  for (int b = 0; b < nb; ++b) { run = std::max(run, g.cum[(size_t)b * g.L + g.L - 1]); P[b] = run; }
+  M.shift = 0;
+  while ((nb >> (M.shift + 1)) >= 256) ++M.shift;
+  M.K = (nb + (1 << M.shift) - 1) >> M.shift;
+  M.J = 25;
+  const double a0 = KAPPA * 250.0, de = g.e_max / (double)nb;
+  M.a2.resize(M.J);
+  for (int j = 0; j < M.J; ++j) {
+    M.a2[j] = std::ldexp(a0 * a0, j);             // A_j^2 = a0^2 2^j, exact scaling
+  }
+  const double INF = std::numeric_limits<double>::infinity();
+  const double mc[6] = {0.5, 1.0, 2.0, 4.0, 8.0, 16.0};
+  M.nu.assign((size_t)M.K * (M.J + 1), 0.0); M.inv_nu = M.nu; M.dtmax = M.nu;
+  for (int k = 0; k < M.K; ++k) {
+    const int b_hi = std::min((k + 1) << M.shift, nb) - 1;
+    const double e_hi = (double)(b_hi + 1) * de;
+    for (int j = 0; j <= M.J; ++j) {
+      double nu = P[nb - 1], dtm = INF;
+      if (k < M.K - 1 && j < M.J) {
+        const double A = std::sqrt(M.a2[j]);
+        double best = INF;
+        for (int c = 0; c < 6; ++c) {
+          const double m = mc[c];
+          auto f = [&](double v) {
+            const double dt = m / v;
+            const double sp = C2 * std::sqrt(e_hi) + A * dt;
+            const double sb = (sp * sp * INV_C2SQ) * g.inv_de + 1.0;
+            return P[sb >= (double)(nb - 1) ? nb - 1 : (int)sb];
+          };
+          double v = f(P[b_hi]);
+          for (int it = 0; it < 4; ++it) {
+            const double v2 = f(v);
+            if (v2 < v && f(v2) <= v2) v = v2; else break;
+          }
+          const double cost = v / (1.0 - std::exp(-m));
+          if (v > 0.0 && cost <= best) { best = cost; nu = v; dtm = m / v; }
+        }
+      }
+      if (!(nu > 0.0)) { nu = g.nu_hat; dtm = INF; }
+      const size_t o = (size_t)k * (M.J + 1) + j;
+      M.nu[o] = nu; M.inv_nu[o] = 1.0 / nu; M.dtmax[o] = dtm;
+    }
+  }
+}
 
 bool load_gas(const avmo_gas_desc* d, Gas& g) {
   if (!d || d->n_bins < 1 || d->n_levels < 1 || !(d->e_max_eV > 0) || !d->cum_rate || !d->level_type ||
@@ -100,6 +170,7 @@ bool load_gas(const avmo_gas_desc* d, Gas& g) {
   g.nu_hat = d->nu_hat > 0 ? d->nu_hat : mx;      // R4: one global null-collision rate
   if (!(g.nu_hat > 0) || g.nu_hat < mx) { g_err = "gas: nu_hat must be >= max total rate and > 0"; return false; }
   g.inv_nu_hat = 1.0 / g.nu_hat;
+  build_majorant(g);
   return true;
 }
 
@@ -192,7 +263,7 @@ struct StepOut {
 };
 
 // One step S0-S9 for an in-domain, active electron.
-void step(const Gas& g, const avmo_field_desc* f, uint64_t seed, double t_max, Electron& el, StepOut& so, Tally* tl) {
+void step(const Gas& g, const avmo_field_desc* f, uint64_t seed, double t_max, bool banded, Electron& el, StepOut& so, Tally* tl) {
   so.event = -2; so.bin = -1; so.child = false;
   // S0: field at r (held constant during the flight); B is a run constant.  R3: re-evaluated every step.
   double E[3], m;
@@ -202,8 +273,23 @@ void step(const Gas& g, const avmo_field_desc* f, uint64_t seed, double t_max, E
   const uint32_t n_s = el.n;
   double u1, u2;
   uniform_pair(seed, el.id, n_s, 0, u1, u2);
-  // S2: free-flight time under the null-collision rate nu_hat
-  const double dt = -std::log(u1) * g.inv_nu_hat;
+  // S2: free-flight time under the null-collision rate nu_hat (R4: one global rate) — or, banded (N5), under the rate of
+  // the electron's energy band and this flight's acceleration class, cut at dtmax
+  double nu_hat = g.nu_hat, inv_nu_hat = g.inv_nu_hat, dt_cut = std::numeric_limits<double>::infinity();
+  if (banded) {
+    const Majorant& M = g.M;
+    const double sb0 = el.e * g.inv_de;
+    const int b0 = sb0 >= (double)g.nb ? g.nb - 1 : (int)sb0;
+    const double ax = KAPPA * E[0], ay = KAPPA * E[1], az = KAPPA * E[2];
+    const double a2 = ax * ax + ay * ay + az * az;
+    int j = 0;
+    while (j < M.J && a2 > M.a2[j]) ++j;           // smallest class whose edge covers |a| (J = above all)
+    const size_t o = (size_t)(b0 >> M.shift) * (M.J + 1) + j;
+    nu_hat = M.nu[o]; inv_nu_hat = M.inv_nu[o]; dt_cut = M.dtmax[o];
+  }
+  double dt = -std::log(u1) * inv_nu_hat;
+  const bool cut = dt > dt_cut;
+  if (cut) dt = dt_cut;
   // S3: flight in constant E (and B)
   const double sp = C2 * std::sqrt(el.e);
   const double v0[3] = {sp * el.kx, sp * el.ky, sp * el.kz};
@@ -267,8 +353,11 @@ void step(const Gas& g, const avmo_field_desc* f, uint64_t seed, double t_max, E
   if (sb >= (double)g.nb) { b = g.nb - 1; if (tl) tl->n_overflow++; } else b = (int)sb;
   so.bin = b;
   const double* row = g.cum + (size_t)b * g.L;
-  // S7: null or real (R7: one uniform decides both)
-  const double xr = u2 * g.nu_hat;
+  // S7: null or real (R7: one uniform decides both).  N6: a flight that was cut is a null collision; the band's rate must
+  // bound the total rate of the bin reached (counted when it does not: never, by construction)
+  if (cut) { so.event = -1; if (tl) tl->n_null++; return; }
+  if (tl && row[g.L - 1] > nu_hat) tl->n_viol++;
+  const double xr = u2 * nu_hat;
   if (xr >= row[g.L - 1]) { so.event = -1; if (tl) tl->n_null++; return; }
   // S8: level = smallest index with cum[b][l] > x
   int l = 0;
@@ -332,7 +421,7 @@ struct Record { Electron el; };
 // The avalanche driver: transport until status != 0, push newly created electrons, repeat.
 // Serial: one electron at a time from a stack.  Order is irrelevant because draws are keyed by (id, n).
 void run_range(const Gas& g, const avmo_field_desc* f, const double* prim, int64_t p0, int64_t p1, uint64_t seed,
-               uint64_t id_offset, double t_max, std::vector<Electron>& done, Tally& tl) {
+               uint64_t id_offset, double t_max, bool banded, std::vector<Electron>& done, Tally& tl) {
   std::vector<Electron> stack;
   StepOut so;
   for (int64_t p = p0; p < p1; ++p) {
@@ -354,7 +443,7 @@ void run_range(const Gas& g, const avmo_field_desc* f, const double* prim, int64
       Electron cur = stack.back();
       stack.pop_back();
       while (cur.status == AVMO_ACTIVE) {
-        step(g, f, seed, t_max, cur, so, &tl);
+        step(g, f, seed, t_max, banded, cur, so, &tl);
         if (so.child) stack.push_back(so.c);
       }
       done.push_back(cur);
@@ -367,6 +456,16 @@ void run_range(const Gas& g, const avmo_field_desc* f, const double* prim, int64
 extern "C" {
 
 const char* avmo_last_error(void) { return g_err.c_str(); }
+
+int32_t avmo_majorant(const avmo_gas_desc* gd, int32_t* shape3, double* a2, double* nu, double* dtmax) {
+  Gas g;
+  if (!load_gas(gd, g) || !shape3) return AVMO_ERR_INVALID_ARG;
+  shape3[0] = g.M.K; shape3[1] = g.M.J; shape3[2] = g.M.shift;
+  if (a2) std::copy(g.M.a2.begin(), g.M.a2.end(), a2);
+  if (nu) std::copy(g.M.nu.begin(), g.M.nu.end(), nu);
+  if (dtmax) std::copy(g.M.dtmax.begin(), g.M.dtmax.end(), dtmax);
+  return AVMO_OK;
+}
 
 void avmo_philox(uint64_t seed, uint64_t id, uint32_t n, uint32_t block, uint32_t out[4]) { philox_block(seed, id, n, block, out); }
 
@@ -386,7 +485,7 @@ int32_t avmo_field_eval(const avmo_field_desc* f, int64_t n, const double* r, do
 
 int32_t avmo_step_batch(const avmo_gas_desc* gd, const avmo_field_desc* f, uint64_t seed, double t_max, int64_t n,
                         const double* in, const uint64_t* id, const uint32_t* n_idx, double* out, int32_t* event,
-                        int32_t* status, int32_t* bin, double* child, uint64_t* child_id) {
+                        int32_t* status, int32_t* bin, double* child, uint64_t* child_id, uint32_t flags) {
   Gas g;
   if (!load_gas(gd, g) || !check_field(f)) return AVMO_ERR_INVALID_ARG;
   if (n < 0 || !in || !id || !n_idx || !out || !event || !status || !bin || !child || !child_id) { g_err = "step_batch: null"; return AVMO_ERR_INVALID_ARG; }
@@ -396,7 +495,7 @@ int32_t avmo_step_batch(const avmo_gas_desc* gd, const avmo_field_desc* f, uint6
     el.x = in[i]; el.y = in[n + i]; el.z = in[2 * n + i]; el.t = in[3 * n + i]; el.e = in[4 * n + i];
     el.kx = in[5 * n + i]; el.ky = in[6 * n + i]; el.kz = in[7 * n + i];
     el.id = id[i]; el.n = n_idx[i]; el.aval = 0; el.status = AVMO_ACTIVE;
-    step(g, f, seed, t_max, el, so, nullptr);
+    step(g, f, seed, t_max, (flags & AVMO_BANDED) != 0, el, so, nullptr);
     out[i] = el.x; out[n + i] = el.y; out[2 * n + i] = el.z; out[3 * n + i] = el.t; out[4 * n + i] = el.e;
     out[5 * n + i] = el.kx; out[6 * n + i] = el.ky; out[7 * n + i] = el.kz;
     event[i] = so.event; status[i] = el.status; bin[i] = so.bin;
@@ -418,18 +517,19 @@ int32_t avmo_run(const avmo_gas_desc* gd, const avmo_field_desc* f, const double
   if (!load_gas(gd, g) || !check_field(f)) return AVMO_ERR_INVALID_ARG;
   if (np < 0 || (np > 0 && !prim) || !opts || !o || !n_out || o->capacity < 0) { g_err = "run: null/negative"; return AVMO_ERR_INVALID_ARG; }
   if (np > 0xFFFFFFFFll) { g_err = "run: too many primaries"; return AVMO_ERR_INVALID_ARG; }
+  const bool banded = (opts->flags & AVMO_BANDED) != 0;
   int nt = std::max(1, opts->n_threads);
   nt = (int)std::min<int64_t>(nt, std::max<int64_t>(np, 1));
   std::vector<std::vector<Electron>> done(nt);
   std::vector<Tally> tl(nt);
   for (auto& t : tl) t.level.assign(g.L, 0);
   if (nt == 1) {
-    run_range(g, f, prim, 0, np, opts->seed, opts->id_offset, opts->t_max, done[0], tl[0]);
+    run_range(g, f, prim, 0, np, opts->seed, opts->id_offset, opts->t_max, banded, done[0], tl[0]);
   } else {                       // timed multi-core baseline only: disjoint primary ranges, identical results
     std::vector<std::thread> th;
     for (int t = 0; t < nt; ++t) {
       int64_t p0 = np * t / nt, p1 = np * (t + 1) / nt;
-      th.emplace_back([&, t, p0, p1] { run_range(g, f, prim, p0, p1, opts->seed, opts->id_offset, opts->t_max, done[t], tl[t]); });
+      th.emplace_back([&, t, p0, p1] { run_range(g, f, prim, p0, p1, opts->seed, opts->id_offset, opts->t_max, banded, done[t], tl[t]); });
     }
     for (auto& x : th) x.join();
   }
@@ -460,11 +560,11 @@ int32_t avmo_run(const avmo_gas_desc* gd, const avmo_field_desc* f, const double
   if (o->per_avalanche)
     for (int64_t p = 0; p < np; ++p) o->per_avalanche[3 * p + 1] = o->per_avalanche[3 * p] > 0 ? o->per_avalanche[3 * p] - 1 : 0;
   if (o->tallies_u64) {
-    for (int l = 0; l < g.L + 4; ++l) o->tallies_u64[l] = 0;
+    for (int l = 0; l < g.L + 5; ++l) o->tallies_u64[l] = 0;
     for (auto& t : tl) {
       for (int l = 0; l < g.L; ++l) o->tallies_u64[l] += t.level[l];
       o->tallies_u64[g.L] += t.n_null; o->tallies_u64[g.L + 1] += t.n_real;
-      o->tallies_u64[g.L + 2] += t.n_overflow; o->tallies_u64[g.L + 3] += t.n_steps;
+      o->tallies_u64[g.L + 2] += t.n_overflow; o->tallies_u64[g.L + 3] += t.n_steps; o->tallies_u64[g.L + 4] += t.n_viol;
     }
   }
   if (o->tallies_f64) {

@@ -51,8 +51,12 @@ typedef struct {
 
 typedef struct { const avmo_slab* slabs; int32_t n_slabs; double B[3]; double xy_lo[2], xy_hi[2]; } avmo_field_desc;
 
+/* flags.  AVMO_BANDED: the null-collision rate of a flight is the one of the
+ * electron's energy band and of the flight's acceleration class instead of the global maximum; flights longer than the
+ * band's validity time are cut and count as null collisions.  Same physics, fewer null steps, other random streams. */
+enum { AVMO_BANDED = 1u };
 /* id_offset: primary p gets electron id id_offset + p (shards of one job use disjoint id ranges); avalanche stays p. */
-typedef struct { uint64_t seed; double t_max; int32_t n_threads; uint64_t id_offset; } avmo_run_opts;
+typedef struct { uint64_t seed; double t_max; int32_t n_threads; uint64_t id_offset; uint32_t flags; } avmo_run_opts;
 
 typedef struct {
   int64_t capacity;
@@ -60,7 +64,7 @@ typedef struct {
   double* birth;            /* [5][capacity]: x0,y0,z0,t0,e0 */
   double* end;              /* [8][capacity]: x1,y1,z1,t1,e1,kx,ky,kz */
   uint64_t* per_avalanche;  /* [Np][3]: endpoints, ions, negative ions */
-  uint64_t* tallies_u64;    /* [n_levels+4]: per level, null, real, overflow, steps */
+  uint64_t* tallies_u64;    /* [n_levels+5]: per level, null, real, overflow, steps, banded-rate violations (always 0) */
   double*   tallies_f64;    /* [5]: sum dx,dy,dz over all flights, sum dt, sum energy loss */
 } avmo_outputs;
 
@@ -77,7 +81,11 @@ int32_t avmo_field_eval(const avmo_field_desc*, int64_t n, const double* r, doub
 int32_t avmo_step_batch(const avmo_gas_desc*, const avmo_field_desc*, uint64_t seed, double t_max, int64_t n,
                         const double* state_in, const uint64_t* id, const uint32_t* n_idx,
                         double* state_out, int32_t* event, int32_t* status, int32_t* bin,
-                        double* child_out, uint64_t* child_id);
+                        double* child_out, uint64_t* child_id, uint32_t flags);
+
+/* The table of banded rates built for this gas (pins): shape3 = (K bands, J classes, shift); a2 [J] squared class edges;
+ * nu, dtmax [K][J+1].  Any output pointer may be NULL. */
+int32_t avmo_majorant(const avmo_gas_desc*, int32_t* shape3, double* a2, double* nu, double* dtmax);
 
 /* Whole avalanches: stack driver.  primaries: [Np][8] AoS.  Returns AVMO_ERR_CAPACITY when more than
  * `capacity` electrons are created (outputs then hold the first `capacity` finished ones). */

@@ -47,7 +47,11 @@ class FieldDescC(C.Structure):
 
 
 class RunOpts(C.Structure):
-    _fields_ = [("seed", C.c_uint64), ("t_max", C.c_double), ("n_threads", C.c_int32), ("id_offset", C.c_uint64)]
+    _fields_ = [("seed", C.c_uint64), ("t_max", C.c_double), ("n_threads", C.c_int32), ("id_offset", C.c_uint64),
+                ("flags", C.c_uint32)]
+
+
+BANDED = 1
 
 
 class Outputs(C.Structure):
@@ -65,6 +69,7 @@ def lib():
         _lib.avmo_run.restype = C.c_int32
         _lib.avmo_step_batch.restype = C.c_int32
         _lib.avmo_field_eval.restype = C.c_int32
+        _lib.avmo_majorant.restype = C.c_int32
     return _lib
 
 
@@ -147,7 +152,18 @@ class StepResult:
     child_id: np.ndarray
 
 
-def step_batch(gas, field, seed, state, ids, n_idx, t_max=float("inf")) -> StepResult:
+def majorant(gas):
+    """The banded-rate table of this gas: (a2 [J], nu [K, J+1], dtmax [K, J+1], shift)."""
+    gd, _kg = gas_desc(gas)
+    shp = (C.c_int32 * 3)()
+    assert lib().avmo_majorant(C.byref(gd), shp, None, None, None) == 0
+    K, J, shift = shp[0], shp[1], shp[2]
+    a2 = np.zeros(J); nu = np.zeros((K, J + 1)); dt = np.zeros((K, J + 1))
+    assert lib().avmo_majorant(C.byref(gd), shp, _p(a2), _p(nu), _p(dt)) == 0
+    return a2, nu, dt, shift
+
+
+def step_batch(gas, field, seed, state, ids, n_idx, t_max=float("inf"), flags=0) -> StepResult:
     state = np.ascontiguousarray(state, dtype=np.float64)
     n = state.shape[1]
     ids = np.ascontiguousarray(ids, dtype=np.uint64)
@@ -157,7 +173,7 @@ def step_batch(gas, field, seed, state, ids, n_idx, t_max=float("inf")) -> StepR
     gd, _kg = gas_desc(gas)
     fd, _kf = field_desc(field)
     rc = lib().avmo_step_batch(C.byref(gd), C.byref(fd), C.c_uint64(seed), C.c_double(t_max), C.c_int64(n), _p(state),
-                               _p(ids), _p(n_idx), _p(out), _p(ev), _p(st), _p(bn), _p(ch), _p(cid))
+                               _p(ids), _p(n_idx), _p(out), _p(ev), _p(st), _p(bn), _p(ch), _p(cid), C.c_uint32(flags))
     if rc != 0:
         raise RuntimeError(lib().avmo_last_error().decode())
     return StepResult(out, ev, st, bn, ch, cid)
@@ -176,26 +192,28 @@ class RunResult:
     tallies_u64: np.ndarray     # [L+4]
     tallies_f64: np.ndarray     # [5]
     rc: int = 0
+    n_rate_violations: int = 0  # banded runs: steps whose bin's total rate exceeded the band's rate (always 0)
 
     def sorted_by_id(self):
         o = np.argsort(self.id, kind="stable")
         return RunResult(self.n, self.id[o], self.avalanche[o], self.status[o], self.n_steps[o], self.birth[:, o],
-                         self.end[:, o], self.per_avalanche, self.tallies_u64, self.tallies_f64, self.rc)
+                         self.end[:, o], self.per_avalanche, self.tallies_u64, self.tallies_f64, self.rc,
+                         self.n_rate_violations)
 
 
 def run(gas, field, primaries, seed=0, t_max=float("inf"), capacity=None, n_threads=1, allow_overflow=False,
-        id_offset=0) -> RunResult:
+        id_offset=0, flags=0) -> RunResult:
     prim = np.ascontiguousarray(primaries, dtype=np.float64)
     np_ = prim.shape[0]
     cap = int(capacity if capacity is not None else max(4 * np_, 1 << 16))
     L = gas.n_levels
     ident = np.zeros(cap, dtype=np.uint64); av = np.zeros(cap, dtype=np.uint32); st = np.zeros(cap, dtype=np.int32)
     ns = np.zeros(cap, dtype=np.uint32); birth = np.zeros((5, cap)); end = np.zeros((8, cap))
-    pa = np.zeros((max(np_, 1), 3), dtype=np.uint64); tu = np.zeros(L + 4, dtype=np.uint64); tf = np.zeros(5)
+    pa = np.zeros((max(np_, 1), 3), dtype=np.uint64); tu = np.zeros(L + 5, dtype=np.uint64); tf = np.zeros(5)
     gd, _kg = gas_desc(gas)
     fd, _kf = field_desc(field)
     o = Outputs(cap, _p(ident), _p(av), _p(st), _p(ns), _p(birth), _p(end), _p(pa), _p(tu), _p(tf))
-    opts = RunOpts(int(seed), float(t_max), int(n_threads), int(id_offset))
+    opts = RunOpts(int(seed), float(t_max), int(n_threads), int(id_offset), int(flags))
     n_out = C.c_int64(0)
     rc = lib().avmo_run(C.byref(gd), C.byref(fd), _p(prim), C.c_int64(np_), C.byref(opts), C.byref(o), C.byref(n_out))
     if rc == -2 and not allow_overflow:
@@ -203,4 +221,4 @@ def run(gas, field, primaries, seed=0, t_max=float("inf"), capacity=None, n_thre
     if rc not in (0, -2):
         raise RuntimeError(lib().avmo_last_error().decode())
     n = n_out.value
-    return RunResult(n, ident[:n], av[:n], st[:n], ns[:n], birth[:, :n], end[:, :n], pa[:np_], tu, tf, rc)
+    return RunResult(n, ident[:n], av[:n], st[:n], ns[:n], birth[:, :n], end[:, :n], pa[:np_], tu[:L + 4], tf, rc, int(tu[L + 4]))

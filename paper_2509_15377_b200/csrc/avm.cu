@@ -159,7 +159,8 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
 
   const uint32_t cap = a.cap;
   const size_t ld = cap;
-  // static tickets, CTA-major then warp then lane: the first electrons go one per warp, spread over all SMs
+  // static tickets, CTA-major then warp then lane: the first electrons go one per warp, spread over all SMs (packing them
+  // into one warp per scheduler instead was measured slower on the map configs: DESIGN.md §7)
   constexpr int kWarpsPerCta = THREADS / 32;
   uint32_t ticket = (lane * kWarpsPerCta + warp) * gridDim.x + blockIdx.x;
   bool have = false, dvalid = false;
@@ -199,7 +200,7 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
     }
   };
   // one collision phase for the lanes with a pending real collision, then append their secondaries (a-8, a-9)
-  auto collide_and_append = [&](bool pend, const Pending& pc, bool have_d, const Deflection& dd, int& fin) -> int {
+  auto collide_and_append = [&](const unsigned mask, bool pend, const Pending& pc, bool have_d, const Deflection& dd, int& fin) -> int {
     bool spawn = false;
     Child ch;
     ch.e = 0.0; ch.u6 = 0.5; ch.u7 = 0.0;
@@ -216,12 +217,12 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
         tl.loss += loss;
       }
     }
-    const unsigned sm = __ballot_sync(0xFFFFFFFFu, spawn);
-    if (sm) {                                       // one atomic per warp
+    const unsigned sm = __ballot_sync(mask, spawn);
+    if (sm) {                                       // one atomic per warp (per group of converged lanes)
       const int leader = __ffs(sm) - 1;
       unsigned long long old = 0ull;
       if ((int)lane == leader) old = atomicAdd(&ctl->counters, (unsigned long long)__popc(sm) << 32);
-      old = __shfl_sync(0xFFFFFFFFu, old, leader);
+      old = __shfl_sync(mask, old, leader);
       if (spawn) {
         const uint64_t cs = (old >> 32) + (uint64_t)__popc(sm & lt_mask);
         if (cs < (uint64_t)cap) {
@@ -249,13 +250,13 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
   };
   // retire finished electrons: endpoint write, one atomic per warp for `finished`, one for new tickets; the lane that
   // finishes the last electron raises every CTA's done flag (a-11)
-  auto retire = [&](int fin) {
-    const unsigned fm = __ballot_sync(0xFFFFFFFFu, fin != 0);
+  auto retire = [&](const unsigned mask, int fin) {
+    const unsigned fm = __ballot_sync(mask, fin != 0);
     if (fm) {
       const int leader = __ffs(fm) - 1;
       unsigned int base = 0u;
       if ((int)lane == leader) base = atomicAdd(&ctl->q_head, (unsigned int)__popc(fm));
-      base = __shfl_sync(0xFFFFFFFFu, base, leader);
+      base = __shfl_sync(mask, base, leader);
       if (fin != 0) {
         const double s2 = vx * vx + vy * vy + vz * vz;
         double kx = 0.0, ky = 0.0, kz = 1.0;
@@ -319,7 +320,7 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
         const int fin = tp_batch<FK, HASB, TALLY>(g, f, K, tab, s_lv, s_logtab, wb, t_max, lane, act, have, x, y, z, t, vx, vy, vz,
                                                   id, n, slot, tl, collide_and_append, [](bool, int, int, int, int, int) {});
         dvalid = false;
-        retire(fin);
+        retire(0xFFFFFFFFu, fin);
       }
     } else if (k <= kCoopMax) {
       // ---- serial batch: cooperative draws, then every owner lane walks its electron's steps alone (avm_forms.cuh) ----
@@ -341,8 +342,8 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
       }
       Deflection dd;
       dd.ct = 1.0; dd.st = 0.0; dd.cphi = 1.0; dd.sphi = 0.0;
-      collide_and_append(pend, pc, false, dd, fin);
-      retire(fin);
+      collide_and_append(0xFFFFFFFFu, pend, pc, false, dd, fin);
+      retire(0xFFFFFFFFu, fin);
     }
     // ---- refill idle lanes when the probed ticket has been published ----
     if (probe != -1) refill();
@@ -631,7 +632,7 @@ step_form_batch_kernel(const __grid_constant__ DevGas g, const __grid_constant__
   Tally tl;
   // the output entry a lane is working on: tp_batch gives lane (e, sidx) one step; sb_batch gives the owner lane all steps
   int64_t o_cur = 0;
-  auto collide = [&](bool pend, const Pending& pc, bool have_d, const Deflection& dd, int& fin) -> int {
+  auto collide = [&](const unsigned, bool pend, const Pending& pc, bool have_d, const Deflection& dd, int& fin) -> int {
     int l = -1;
     if (pend) {
       double loss;
@@ -669,7 +670,7 @@ step_form_batch_kernel(const __grid_constant__ DevGas g, const __grid_constant__
     // same step: o_cur is kept one step ahead (the owner lane's next output entry)
     o_cur = have ? i * gl : 0;
     sb_batch<FK, HASB, true>(g, f, K, g.tab, s_logtab, &s_wb[warp], t_max, lane, act, have, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, id,
-                             nn, tl, collide, [&](int fin) { if (fin != 0) have = false; },
+                             nn, tl, collide, [&](const unsigned, int fin) { if (fin != 0) have = false; },
                              [&](int e, int sidx, int ev, int b, int fin) { record(e, sidx, ev, b, fin); o_cur = s_gidx[warp][e] * gl + sidx + 1; });
   }
 }

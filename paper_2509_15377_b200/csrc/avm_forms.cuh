@@ -68,7 +68,7 @@ __device__ __forceinline__ void fw_flight(const DevGas& g, const DevField& f, co
 // stay valid for the next pass from the new base state.  The draws depend on (id, n) only, so this is the sequence of
 // steps S0-S9 the oracle takes, evaluated out of order; T_j differs from the sequential sum by rounding only.
 //
-// collide(pend, pc, have_d, d, fin) -> level: the collision phase for lanes with a pending real collision that is not the
+// collide(mask, pend, pc, have_d, d, fin) -> level: the collision phase for lanes with a pending real collision that is not the
 //   pre-evaluated elastic one (acts on the caller's x .. vz, id, n, which are the same objects as the arguments here).
 // commit(on, e, sidx, ev, bin, fin): called once per pass by every lane; on = this lane's step was taken in this pass,
 //   its result is in x .. vz, n; ev = -1 null, level, or -2 ended before the decision.
@@ -171,7 +171,7 @@ __device__ __forceinline__ int tp_batch(const DevGas& g, const DevField& f, cons
       } else { pend = true; pc.lsel = r; pc.bin = b; }
     }
     if (__any_sync(0xFFFFFFFFu, pend)) {
-      const int lvl = collide(pend, pc, true, dj, fin);
+      const int lvl = collide(0xFFFFFFFFu, pend, pc, true, dj, fin);
       if (pend) evc = lvl;
     }
     commit(taken, e, sidx, evc, b, fin);
@@ -211,15 +211,17 @@ __device__ __forceinline__ int tp_batch(const DevGas& g, const DevField& f, cons
 // For a warp that holds k <= 16 electrons.  All 32 lanes first prepare the draws (Philox block 0 + logarithm, block 1 +
 // deflection angles) of the next B = 32 / k' steps of the k electrons, lane j serving electron j mod k' at step j div k',
 // through the warp's WarpBuf — the draws depend on (id, n) alone, so this is the same as drawing them in place, and draws
-// of steps an electron does not reach are discarded.  Then every owner lane walks through ITS electron's steps on its own:
-// one straight-line block per step — flight (S3-S4), energy bin and threshold record (S6, S7), the S5 predicate with the
-// field lookup at the new position (= S0 of the next step) — and goes straight on when the step was a null collision, with
-// no warp vote, ballot or shuffle in between.  A lane leaves its loop at an event (a real collision pending, or the
-// electron finished); the warp then runs one collision / append / retire phase for the lanes with events, and the loops
-// resume until every electron has used its B steps.
+// of steps an electron does not reach are discarded.  Then every owner lane walks through ITS electron's B steps on its
+// own: one straight-line block per step — flight (S3-S4), energy bin and threshold record (S6, S7), the S5 predicate with
+// the field lookup at the new position (= S0 of the next step) — and, only when the step was not a null collision, one
+// divergent side branch: the collision (with the append of a secondary) or the retirement of the electron.  There is no
+// warp vote, ballot or shuffle on the path of a null step, and a lane never waits for another lane's electron to reach an
+// event: lanes whose step was null wait only while the side branch of the others runs (reconvergence at its end), so a
+// step costs the warp one flight plus, with probability 1 - (null fraction)^k, one collision.
 //
-// collide(pend, pc, have_d, d, fin) -> level; retire(fin): warp-wide, frees the lanes whose electron finished (clears
-// `have`); commit(e, s, ev, bin, fin): step s of the batch of the warp's e-th electron is done, its result is in x .. vz, n.
+// collide(mask, pend, pc, have_d, d, fin) -> level and retire(mask, fin) are called by the lanes with an event only, with
+// mask = the lanes converged at the call (the warp-aggregated atomics inside them run over that mask); retire clears
+// `have`.  commit(e, s, ev, bin, fin): step s of the batch of the warp's e-th electron is done, its result is in x .. vz, n.
 template <int FK, bool HASB, bool TALLY, class Collide, class Retire, class Commit>
 __device__ __forceinline__ void sb_batch(const DevGas& g, const DevField& f, const PhiloxKeys& K,
                                          const ushort4* __restrict__ tab, const double2* __restrict__ s_logtab,
@@ -250,49 +252,40 @@ __device__ __forceinline__ void sb_batch(const DevGas& g, const DevField& f, con
   __syncwarp();
   int s = 0;                                    // this lane's next step of the batch
 #pragma unroll 1
-  for (;;) {
-    int fin = 0, sc = 0;
-    bool pend = false;
-    Pending pc;
-    pc.lsel = 0; pc.bin = -1; pc.xr = 0.0;
-    Deflection dd;
-    dd.ct = 1.0; dd.st = 0.0; dd.cphi = 1.0; dd.sphi = 0.0;
-    if (have) {
-#pragma unroll 1
-      while (s < nb_steps) {
-        const int idx = s * kp + rank;
-        const double dtj = wb->dt[idx];
-        const uint2 u2 = wb->u2w[idx];
-        sc = s; ++s;
-        const double s2 = advance_move<FK, HASB>(f, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dtj);   // S3, S4
-        bool over;
-        const int b = energy_bin(g, s2, over);                                                     // S6 (counts only when S5 passes)
-        int r = decide_filter(tab[b], u2);                                                         // S7 and the head of S8
-        const int st = s5_status<FK>(f, t_max, n, x, y, z, t, Ex, Ey, Ez);                         // S5; the field at r' = S0 of the next step
-        if (st == 0 && r == -1) {                                                                  // null collision: straight on
-          if (TALLY && over) ++tl.over;
-          commit(rank, sc, -1, b, 0);
-          continue;
-        }
-        if (st < 0) { fin = -st; break; }
-        if (TALLY && over) ++tl.over;
+  while (have && s < nb_steps) {
+    const int idx = s * kp + rank;
+    const double dtj = wb->dt[idx];
+    const uint2 u2 = wb->u2w[idx];
+    const double s2 = advance_move<FK, HASB>(f, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dtj);   // S3, S4
+    bool over;
+    const int b = energy_bin(g, s2, over);                                                     // S6 (counts only when S5 passes)
+    int r = decide_filter(tab[b], u2);                                                         // S7 and the head of S8
+    const int st = s5_status<FK>(f, t_max, n, x, y, z, t, Ex, Ey, Ez);                         // S5; the field at r' = S0 of the next step
+    if (TALLY && over && st == 0) ++tl.over;
+    int ev = -1, fin = 0;
+    if (st != 0 || r != -1) {                                                                  // not a plain null collision
+      if (st < 0) { fin = -st; ev = -2; }
+      else {
+        Pending pc;
+        pc.lsel = 0; pc.bin = b; pc.xr = 0.0;
         if (r == -2 || r == 2) {
           pc.xr = to_unit(u2.x, u2.y) * g.nu_hat;
           if (r == -2) r = decide_exact(g, b, pc.xr);
           if (r == 2) prefetch_row(g, b);
         }
-        if (r < 0) { commit(rank, sc, -1, b, 0); continue; }
-        pend = true; pc.lsel = r; pc.bin = b;
-        dd.ct = wb->ct[idx]; dd.st = wb->st[idx]; dd.cphi = wb->cphi[idx]; dd.sphi = wb->sphi[idx];
-        break;
+        if (r >= 0) {
+          pc.lsel = r;
+          Deflection dd;
+          dd.ct = wb->ct[idx]; dd.st = wb->st[idx]; dd.cphi = wb->cphi[idx]; dd.sphi = wb->sphi[idx];
+          ev = collide(__activemask(), true, pc, true, dd, fin);
+        }
       }
+      if (fin != 0) { commit(rank, s, ev, st < 0 ? -1 : b, fin); retire(__activemask(), fin); }
     }
-    int lvl = -1;
-    if (__any_sync(0xFFFFFFFFu, pend)) lvl = collide(pend, pc, true, dd, fin);
-    if (have && (pend || fin != 0)) commit(rank, sc, pend ? lvl : -2, pc.bin, fin);
-    retire(fin);
-    if (!__any_sync(0xFFFFFFFFu, have && s < nb_steps)) break;
+    if (fin == 0) commit(rank, s, ev, b, 0);
+    ++s;
   }
+  __syncwarp();
 }
 
 }  // namespace avm
