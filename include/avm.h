@@ -79,6 +79,12 @@ int32_t avm_gas_create(avm_ctx*, const avm_gas_desc*, void* dev_buf, size_t dev_
 int32_t avm_gas_destroy(avm_gas*);
 /* The resolved null-collision rate [ns^-1]. */
 double avm_gas_nu_hat(const avm_gas*);
+/* The table of energy-banded null-collision rates avm_gas_create built for this gas (AVM_RUN_BANDED; DESIGN.md §3.5,
+ * readings N1-N4, "revisiting the algorithms").  shape3 (HOST) = (K energy bands, J
+ * acceleration classes, shift: a band is 2^shift energy bins); a2: HOST [J] squared upper edges of the classes
+ * [(cm/ns^2)^2]; nu, dtmax: HOST [K][J + 1] rate [ns^-1] and validity time [ns] (+inf = no cut) per band and class, column
+ * J = accelerations above every class.  a2, nu, dtmax may be NULL.  Lets the tests compare the table with the oracle's. */
+int32_t avm_gas_bands(const avm_gas*, int32_t* shape3, double* a2, double* nu, double* dtmax);
 
 /* ---- field: uniform, uniform + B, or regular-grid map(s) (S0, R14, R15) ---------------------------------
  * A stack of z-slabs, ascending and contiguous (slab[i].z_hi == slab[i+1].z_lo).  kind 0: uniform field
@@ -127,7 +133,14 @@ enum {
   /* Launch shape of the transport kernel.  Default: chosen from n_primaries (wide when the primaries alone outnumber
    * the lanes of the latency shape).  Results do not depend on the shape. */
   AVM_RUN_SHAPE_WIDE = 4u,        /* 768 threads per SM: most lanes, for runs that keep them busy */
-  AVM_RUN_SHAPE_LATENCY = 8u      /* 512 threads per SM with time-parallel batches: fewest cycles per step */
+  AVM_RUN_SHAPE_LATENCY = 8u,     /* 512 threads per SM with time-parallel batches: fewest cycles per step */
+  /* Energy-banded null-collision rate (DESIGN.md §3.5 readings N1-N6): the rate of a flight is the
+   * one of the electron's energy band and of the acceleration class of the field at its position (avm_gas_bands) instead
+   * of the global nu_hat; a flight longer than the band's validity time is cut there and ends in a null collision.  The
+   * same physics (thinning with a piecewise-constant majorant is exact) in 1.6-5x fewer steps; the random streams are
+   * consumed differently, so a banded run is compared with a banded oracle run.  Runs take serial batches and full-warp
+   * iterations only (no time-parallel batches: a flight's rate depends on the energy the previous flight ended with). */
+  AVM_RUN_BANDED = 16u
 };
 typedef struct {
   uint64_t seed;
@@ -199,11 +212,11 @@ int32_t avm_step_batch(avm_ctx*, const avm_gas*, const avm_field*, uint64_t seed
  *          For forms 2 and 3 the output arrays have n * gl entries ([8][n * gl] for states): entry i * gl + s = the result of step s of electron i,
  *          in the sense of avm_step_batch (state after the step, event, status, bin, child).  Entries of steps the
  *          electron does not reach (it finished earlier in the batch) are left untouched: pre-fill event with -3.
- * k is ignored for forms 0 and 1. */
+ * k is ignored for forms 0 and 1.  flags: 0 or AVM_RUN_BANDED (forms 1 and 3 only: the forms a banded run takes). */
 int32_t avm_step_batch_form(avm_ctx*, const avm_gas*, const avm_field*, uint64_t seed, double t_max, int32_t form,
                             int32_t k, int64_t n, const double* state_in, const uint64_t* id, const uint32_t* n_idx,
                             double* state_out, int32_t* event, int32_t* status, int32_t* bin, double* child_out,
-                            uint64_t* child_id);
+                            uint64_t* child_id, uint32_t flags);
 
 /* Philox block (seed, id, n, block) -> words[4] and two uniforms, for n_items items.  All arrays DEVICE.
  * Pin C1: lets the tests compare the device generator bit for bit. */

@@ -22,10 +22,10 @@ if not os.path.exists(_SO):
 _lib = C.CDLL(_SO)
 
 OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_CUDA, ERR_STATE = 0, -1, -2, -3, -4
-RUN_PRIMARIES_ON_DEVICE, RUN_NO_TALLIES, RUN_SHAPE_WIDE, RUN_SHAPE_LATENCY = 1, 2, 4, 8
+RUN_PRIMARIES_ON_DEVICE, RUN_NO_TALLIES, RUN_SHAPE_WIDE, RUN_SHAPE_LATENCY, RUN_BANDED = 1, 2, 4, 8, 16
 MAX_LEVELS, MAX_SLABS = 64, 8
 EXPORTS = ["avm_last_error", "avm_ctx_create", "avm_ctx_destroy", "avm_ctx_sm_count", "avm_gas_bytes",
-           "avm_gas_create", "avm_gas_destroy", "avm_gas_nu_hat", "avm_field_create", "avm_field_destroy",
+           "avm_gas_create", "avm_gas_destroy", "avm_gas_nu_hat", "avm_gas_bands", "avm_field_create", "avm_field_destroy",
            "avm_field_eval", "avm_run_workspace_bytes", "avm_run", "avm_run_stats", "avm_run_transport_ms", "avm_fetch", "avm_step_batch", "avm_step_batch_form",
            "avm_philox_batch", "avm_fp64_probe", "avm_gather_probe", "avm_smem_probe"]
 
@@ -72,7 +72,7 @@ _lib.avm_run_workspace_bytes.restype = C.c_size_t
 _lib.avm_run_workspace_bytes.argtypes = [C.c_void_p, C.c_int64]
 _lib.avm_gas_nu_hat.restype = C.c_double
 _lib.avm_gas_nu_hat.argtypes = [C.c_void_p]
-for _n in ("avm_ctx_create", "avm_ctx_destroy", "avm_ctx_sm_count", "avm_gas_create", "avm_gas_destroy",
+for _n in ("avm_ctx_create", "avm_ctx_destroy", "avm_ctx_sm_count", "avm_gas_create", "avm_gas_destroy", "avm_gas_bands",
            "avm_field_create", "avm_field_destroy", "avm_field_eval", "avm_run", "avm_run_stats", "avm_fetch",
            "avm_step_batch", "avm_step_batch_form", "avm_philox_batch", "avm_fp64_probe", "avm_run_transport_ms",
            "avm_gather_probe", "avm_smem_probe"):
@@ -83,6 +83,7 @@ _lib.avm_ctx_destroy.argtypes = [C.c_void_p]
 _lib.avm_ctx_sm_count.argtypes = [C.c_void_p]
 _lib.avm_gas_create.argtypes = [C.c_void_p, C.POINTER(_GasDesc), C.c_void_p, C.c_size_t, C.POINTER(C.c_void_p)]
 _lib.avm_gas_destroy.argtypes = [C.c_void_p]
+_lib.avm_gas_bands.argtypes = [C.c_void_p] + [C.c_void_p] * 4
 _lib.avm_field_create.argtypes = [C.c_void_p, C.POINTER(_FieldDesc), C.POINTER(C.c_void_p)]
 _lib.avm_field_destroy.argtypes = [C.c_void_p]
 _lib.avm_field_eval.argtypes = [C.c_void_p, C.c_void_p, C.c_int64] + [C.c_void_p] * 4
@@ -91,7 +92,7 @@ _lib.avm_run.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int
 _lib.avm_run_stats.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
 _lib.avm_fetch.argtypes = [C.c_void_p, C.POINTER(_Outputs), C.c_int64, C.c_int64, C.c_int32, C.POINTER(_Outputs)]
 _lib.avm_step_batch.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint64, C.c_double, C.c_int64] + [C.c_void_p] * 9
-_lib.avm_step_batch_form.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint64, C.c_double, C.c_int32, C.c_int32, C.c_int64] + [C.c_void_p] * 9
+_lib.avm_step_batch_form.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint64, C.c_double, C.c_int32, C.c_int32, C.c_int64] + [C.c_void_p] * 9 + [C.c_uint32]
 _lib.avm_philox_batch.argtypes = [C.c_void_p, C.c_uint64, C.c_int64] + [C.c_void_p] * 5
 _lib.avm_gather_probe.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.c_int32, C.c_int32, C.c_int64, C.c_void_p, C.POINTER(C.c_float)]
 _lib.avm_smem_probe.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_int64, C.c_void_p, C.POINTER(C.c_float)]
@@ -176,6 +177,15 @@ class Gas:
     @property
     def nu_hat(self) -> float:
         return float(_lib.avm_gas_nu_hat(self._h))
+
+    def bands(self):
+        """avm_gas_bands: (a2 [J], nu [K, J+1], dtmax [K, J+1], shift) — the table of banded null-collision rates."""
+        shp = np.zeros(3, dtype=np.int32)
+        _check(_lib.avm_gas_bands(self._h, _hp(shp), None, None, None))
+        K, J, shift = (int(v) for v in shp)
+        a2 = np.zeros(J); nu = np.zeros((K, J + 1)); dt = np.zeros((K, J + 1))
+        _check(_lib.avm_gas_bands(self._h, _hp(shp), _hp(a2), _hp(nu), _hp(dt)))
+        return a2, nu, dt, shift
 
     def __del__(self):
         try:
@@ -276,7 +286,7 @@ def step_form_lanes(k: int) -> int:
 
 
 def step_batch_form(ctx: Context, gas: Gas, field: Field, seed, state, ids, n_idx, form: int, k: int = 1,
-                    t_max=float("inf")) -> StepResult:
+                    t_max=float("inf"), flags: int = 0) -> StepResult:
     """avm_step_batch_form.  Forms 0 / 1: as step_batch.  Forms 2 / 3: arrays get a trailing axis of gl =
     step_form_lanes(k) steps per electron ([8, n, gl], [n, gl]); steps the batch did not reach have event == -3."""
     st = torch.from_numpy(np.ascontiguousarray(state, dtype=np.float64)).to(ctx.device)
@@ -292,7 +302,8 @@ def step_batch_form(ctx: Context, gas: Gas, field: Field, seed, state, ids, n_id
     ch = torch.zeros((8, m), dtype=torch.float64, device=ctx.device)
     cid = torch.zeros(m, dtype=torch.int64, device=ctx.device)
     _check(_lib.avm_step_batch_form(ctx._h, gas._h, field._h, int(seed), float(t_max), int(form), int(k), n, _dev(st),
-                                    _dev(idt), _dev(nt), _dev(out), _dev(ev), _dev(stt), _dev(bn), _dev(ch), _dev(cid)))
+                                    _dev(idt), _dev(nt), _dev(out), _dev(ev), _dev(stt), _dev(bn), _dev(ch), _dev(cid),
+                                    int(flags)))
     r = StepResult(out.cpu().numpy(), ev.cpu().numpy(), stt.cpu().numpy(), bn.cpu().numpy(), ch.cpu().numpy(),
                    cid.cpu().numpy().view(np.uint64))
     if form >= 2:

@@ -130,7 +130,7 @@ constexpr int kCoopMax = AVM_COOP_MAX;
 #ifndef AVM_SB_UNIFORM
 #define AVM_SB_UNIFORM 0     // 1: serial batches instead of time-parallel ones in one uniform slab without B
 #endif
-template <int FK, bool HASB, bool TALLY, bool SMEMTAB, int THREADS, bool TPB>
+template <int FK, bool HASB, bool TALLY, bool SMEMTAB, int THREADS, bool TPB, bool BANDED>
 __global__ void __launch_bounds__(THREADS, 1)
 transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevField f, const RunArrays a,
                  RunCtl* __restrict__ ctl, const __grid_constant__ PhiloxKeys K, const double t_max,
@@ -145,6 +145,8 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
     s_logtab[i] = make_double2(__longlong_as_double((long long)kLogTab[i].rc), __longlong_as_double((long long)kLogTab[i].L));
   const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
   const ushort4* tab = g.tab;
+  // banded rates (NEXT-1): in one uniform slab the acceleration class is a constant of the run
+  const int jcls = (BANDED && FK == 1) ? accel_class(g, f.slab[0].E[0], f.slab[0].E[1], f.slab[0].E[2]) : 0;
   size_t dyn_off = 0;
   if (SMEMTAB) {                                   // threshold table: 8 bytes per bin, resident in shared memory
     uint2* dst = reinterpret_cast<uint2*>(s_dyn);
@@ -314,7 +316,7 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
     if ((it & 15u) == 0u && ld_relaxed_s32(done) == 2) { stopped = true; break; }
     const int k = __popc(act);
 
-    if (TPB && FK == 1 && (HASB || !AVM_SB_UNIFORM) && k <= kCoopMax) {
+    if (TPB && !BANDED && FK == 1 && (HASB || !AVM_SB_UNIFORM) && k <= kCoopMax) {
       // ---- time-parallel batch (uniform E, optional B): g = 32 / k' lanes per electron (avm_forms.cuh) ----
       if constexpr (FK == 1) {
         const int fin = tp_batch<FK, HASB, TALLY>(g, f, K, tab, s_lv, s_logtab, wb, t_max, lane, act, have, x, y, z, t, vx, vy, vz,
@@ -324,12 +326,12 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
       }
     } else if (k <= kCoopMax) {
       // ---- serial batch: cooperative draws, then every owner lane walks its electron's steps alone (avm_forms.cuh) ----
-      sb_batch<FK, HASB, TALLY>(g, f, K, tab, s_logtab, wb, t_max, lane, act, have, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, id, n, tl,
-                                collide_and_append, retire, [](int, int, int, int, int) {});
+      sb_batch<FK, HASB, TALLY, BANDED>(g, f, K, tab, s_logtab, wb, t_max, lane, act, have, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, id, n, tl,
+                                        collide_and_append, retire, [](int, int, int, int, int) {}, jcls);
       dvalid = false;
     } else {
       // ---- full warp ----
-      if (have && !dvalid) { draw_flight(g, K, s_logtab, id, n, dt, u2w); dvalid = true; }
+      if (have && !dvalid) { draw_flight<BANDED>(g, K, s_logtab, id, n, dt, u2w); dvalid = true; }
       int fin = 0;
       bool pend = false;
       Pending pc;
@@ -337,8 +339,8 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
 #pragma unroll
       for (int fl = 0; fl < kFlights; ++fl) {
         if (have && !pend && fin == 0)
-          fw_flight<FK, HASB, TALLY>(g, f, K, tab, s_logtab, t_max, id, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt, u2w, fin,
-                                           pend, pc, tl);
+          fw_flight<FK, HASB, TALLY, BANDED>(g, f, K, tab, s_logtab, t_max, id, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt, u2w, fin,
+                                             pend, pc, tl, jcls);
       }
       Deflection dd;
       dd.ct = 1.0; dd.st = 0.0; dd.cphi = 1.0; dd.sphi = 0.0;
@@ -498,7 +500,7 @@ __global__ void publish_kernel(const RunCtl* ctl, const int L, unsigned long lon
 // FORM 0: the general sequence draw_flight -> advance -> decide -> collision_step.  FORM 1: the full-warp form of the
 // transport kernel — fw_flight (avm_forms.cuh: advance, decide_filter / decide_exact, the next flight's draws hoisted
 // behind the record load) and the collision phase with the deflection drawn there.
-template <int FK, bool HASB, int FORM>
+template <int FK, bool HASB, int FORM, bool BANDED>
 __global__ void step_batch_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevField f,
                                   const uint64_t seed, const double t_max, const int64_t n,
                                   const double* __restrict__ in, const uint64_t* __restrict__ ids,
@@ -531,7 +533,7 @@ __global__ void step_batch_kernel(const __grid_constant__ DevGas g, const __grid
   const double sp = kC2 * sqrt(e);
   double vx = sp * kx, vy = sp * ky, vz = sp * kz, dt;
   uint2 u2;
-  draw_flight(g, K, s_logtab, id, nn, dt, u2);
+  draw_flight<BANDED>(g, K, s_logtab, id, nn, dt, u2);
   Pending pc;
   pc.lsel = 0; pc.bin = -1; pc.xr = 0.0;
   bool over = false, spawn = false;
@@ -543,8 +545,9 @@ __global__ void step_batch_kernel(const __grid_constant__ DevGas g, const __grid
   if (FORM == 1) {
     bool pend = false;
     Tally tl;
-    fw_flight<FK, HASB, true>(g, f, K, g.tab, s_logtab, t_max, id, nn, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt, u2, st, pend,
-                                    pc, tl);
+    const int jcls = (BANDED && FK == 1) ? accel_class(g, f.slab[0].E[0], f.slab[0].E[1], f.slab[0].E[2]) : 0;
+    fw_flight<FK, HASB, true, BANDED>(g, f, K, g.tab, s_logtab, t_max, id, nn, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt, u2, st, pend,
+                                      pc, tl, jcls);
     over = tl.over != 0u;
     if (st == 0) {
       ev = -1;
@@ -589,7 +592,7 @@ __global__ void step_batch_kernel(const __grid_constant__ DevGas g, const __grid
 // FORMS 2 and 3: one batch per warp — a time-parallel batch (tp_batch) or a serial batch (sb_batch) of avm_forms.cuh — with
 // k electrons per warp on scattered lanes.  Entry i * gl + s of the outputs = step s of electron i, gl = 32 / k' steps per
 // batch; entries the batch does not reach (the electron finished earlier) keep what the caller put there.
-template <int FK, bool HASB, int FORM>
+template <int FK, bool HASB, int FORM, bool BANDED>
 __global__ void __launch_bounds__(128)
 step_form_batch_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevField f, const uint64_t seed,
                        const double t_max, const int64_t n, const int k, const double* __restrict__ in,
@@ -669,9 +672,11 @@ step_form_batch_kernel(const __grid_constant__ DevGas g, const __grid_constant__
     // sb_batch calls commit AFTER a step; the child of a collision is recorded inside collide, before the commit of the
     // same step: o_cur is kept one step ahead (the owner lane's next output entry)
     o_cur = have ? i * gl : 0;
-    sb_batch<FK, HASB, true>(g, f, K, g.tab, s_logtab, &s_wb[warp], t_max, lane, act, have, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, id,
-                             nn, tl, collide, [&](const unsigned, int fin) { if (fin != 0) have = false; },
-                             [&](int e, int sidx, int ev, int b, int fin) { record(e, sidx, ev, b, fin); o_cur = s_gidx[warp][e] * gl + sidx + 1; });
+    const int jcls = (BANDED && FK == 1) ? accel_class(g, f.slab[0].E[0], f.slab[0].E[1], f.slab[0].E[2]) : 0;
+    sb_batch<FK, HASB, true, BANDED>(g, f, K, g.tab, s_logtab, &s_wb[warp], t_max, lane, act, have, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, id,
+                                     nn, tl, collide, [&](const unsigned, int fin) { if (fin != 0) have = false; },
+                                     [&](int e, int sidx, int ev, int b, int fin) { record(e, sidx, ev, b, fin); o_cur = s_gidx[warp][e] * gl + sidx + 1; },
+                                     jcls);
   }
 }
 
@@ -760,9 +765,14 @@ struct avm_ctx {
   cudaEvent_t ev_t0 = nullptr, ev_t1 = nullptr;  // bracket the transport launches of the last avm_run
   float transport_ms = 0.0f;
 };
+struct BandTable {               // NEXT-1: host copy of the banded rates, [K][J + 1] as the readings state them
+  int shift = 0, K = 0, J = 0;
+  std::vector<double> a2, nu, dtmax;
+};
 struct avm_gas {
   DevGas d{};
   double nu_hat = 0.0;
+  BandTable bands;
 };
 struct avm_field {
   DevField d{};
@@ -801,7 +811,10 @@ bool valid_gas(const avm_gas_desc* d, double* max_rate) {
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
-struct GasLayout { size_t nu_tot, head, tab, cum, loss, recoil, w, type, total; };
+struct GasLayout { size_t nu_tot, head, tab, cum, loss, recoil, w, type, band, total; };
+constexpr int kBandClasses = 25;                 // N2: class edges 250 V/cm x 2^(j/2), j = 0 .. 24
+int band_shift(int nb) { int s = 0; while ((nb >> (s + 1)) >= 256) ++s; return s; }   // N1: the most bins per band that leaves >= 256 bands
+int band_count(int nb) { const int s = band_shift(nb); return (nb + (1 << s) - 1) >> s; }
 int padded_levels(int L) { return (L + 1) & ~1; }
 GasLayout gas_layout(int nb, int L) {
   GasLayout g;
@@ -815,8 +828,71 @@ GasLayout gas_layout(int nb, int L) {
   g.recoil = off; off += sizeof(double) * AVM_MAX_LEVELS;
   g.w = off;      off += sizeof(double) * AVM_MAX_LEVELS;
   g.type = off;   off = align_up(off + AVM_MAX_LEVELS, 256);
+  g.band = off;   off = align_up(off + 32 * (size_t)(kBandClasses + 1) * band_count(nb), 256);
   g.total = off;
   return g;
+}
+
+
+// NEXT-1, readings N1-N4 of DESIGN.md §3.5: the table of banded null-collision rates.
+//  N1 bands: 2^shift consecutive energy bins each (band_shift), K = ceil(nb / 2^shift) of them.
+//  N2 acceleration classes: squared upper edges A_j^2 = (kappa 250 V/cm)^2 2^j, j = 0 .. J-1, J = 25; column J = any
+//     stronger field.
+//  N3 reach: an electron that starts a flight with energy below the band's upper edge e_hi under an acceleration <= A_j
+//     has, after a time <= dt, a speed <= c2 sqrt(e_hi) + A_j dt, hence (one bin of slack) an energy bin <= reach(dt); with
+//     M[b] = the largest total rate of bins 0 .. b, the rate of (k, j) for a validity time dt = m / nu is a solution of
+//     nu >= M[reach(m / nu)], found by iterating from M[last bin of the band] and tightened while the next iterate still
+//     bounds its own reach.
+//  N4 m is the one of {1/2, 1, 2, 4, 8, 16} with the smallest nu / (1 - exp(-m)) (steps per unit time, cut flights
+//     included; the last one on ties); the last band (it also holds the energies beyond the table) and column J use the
+//     table's largest rate with no cut.
+void build_bands(const avm_gas_desc* d, double nu_hat, BandTable& T) {
+  const int nb = d->n_bins, L = d->n_levels;
+  const double inf = std::numeric_limits<double>::infinity();
+  const double inv_de = (double)nb / d->e_max_eV, de = d->e_max_eV / (double)nb;
+  std::vector<double> M(nb);
+  for (int b = 0; b < nb; ++b) {
+    const double tot = d->cum_rate[(size_t)b * L + L - 1];
+    M[b] = b == 0 ? (tot > 0.0 ? tot : 0.0) : (tot > M[b - 1] ? tot : M[b - 1]);
+  }
+  T.shift = band_shift(nb); T.K = band_count(nb); T.J = kBandClasses;
+  const int W = T.J + 1;
+  T.a2.resize(T.J);
+  const double a0 = kKappa * 250.0;
+  for (int j = 0; j < T.J; ++j) T.a2[j] = std::ldexp(a0 * a0, j);
+  T.nu.assign((size_t)T.K * W, M[nb - 1]);
+  T.dtmax.assign((size_t)T.K * W, inf);
+  auto reach_rate = [&](double e_hi, double A, double m, double nu) {
+    const double dt = m / nu;
+    const double speed = kC2 * std::sqrt(e_hi) + A * dt;
+    const double sb = (speed * speed * kInvC2Sq) * inv_de + 1.0;
+    return M[sb >= (double)(nb - 1) ? nb - 1 : (int)sb];
+  };
+  static const double m_of[6] = {0.5, 1.0, 2.0, 4.0, 8.0, 16.0};
+  for (int k = 0; k + 1 < T.K; ++k) {
+    int last = ((k + 1) << T.shift) - 1;
+    if (last > nb - 1) last = nb - 1;
+    const double e_hi = (double)(last + 1) * de;
+    for (int j = 0; j < T.J; ++j) {
+      const double A = std::sqrt(T.a2[j]);
+      double best_cost = inf, best_nu = M[nb - 1], best_dt = inf;
+      for (int c = 0; c < 6; ++c) {
+        const double m = m_of[c];
+        double nu = reach_rate(e_hi, A, m, M[last]);
+        for (int it = 0; it < 4; ++it) {
+          const double next = reach_rate(e_hi, A, m, nu);
+          if (!(next < nu && reach_rate(e_hi, A, m, next) <= next)) break;
+          nu = next;
+        }
+        const double cost = nu / (1.0 - std::exp(-m));
+        if (nu > 0.0 && cost <= best_cost) { best_cost = cost; best_nu = nu; best_dt = m / nu; }
+      }
+      T.nu[(size_t)k * W + j] = best_nu;
+      T.dtmax[(size_t)k * W + j] = best_dt;
+    }
+  }
+  for (size_t i = 0; i < T.nu.size(); ++i)
+    if (!(T.nu[i] > 0.0)) { T.nu[i] = nu_hat; T.dtmax[i] = inf; }
 }
 
 template <typename K, typename... Args>
@@ -909,6 +985,24 @@ int32_t avm_gas_create(avm_ctx* ctx, const avm_gas_desc* d, void* dev_buf, size_
       for (int l = L; l < Lp; ++l) cum[(size_t)b * Lp + l] = std::numeric_limits<double>::infinity();
     }
   }
+  BandTable bands;
+  build_bands(d, nu_hat_r, bands);
+  {
+    // device layout [J + 1][K][2 x 16 B]: (1 / nu, dtmax), (nu, rho) with rho = floor(nu / nu_hat 2^32) in the low word
+    unsigned char* bt = h.data() + lay.band;
+    const int W = bands.J + 1;
+    for (int j = 0; j < W; ++j)
+      for (int k = 0; k < bands.K; ++k) {
+        const double nu = bands.nu[(size_t)k * W + j], dtm = bands.dtmax[(size_t)k * W + j];
+        const double inv = 1.0 / nu;
+        double rr = std::floor(nu / nu_hat_r * 4294967296.0);
+        if (rr > 4294967295.0) rr = 4294967295.0;
+        if (rr < 0.0) rr = 0.0;
+        const unsigned long long rho = (unsigned long long)rr;
+        unsigned char* e = bt + 32 * ((size_t)j * bands.K + k);
+        std::memcpy(e, &inv, 8); std::memcpy(e + 8, &dtm, 8); std::memcpy(e + 16, &nu, 8); std::memcpy(e + 24, &rho, 8);
+      }
+  }
   std::memcpy(h.data() + lay.loss, d->level_loss_eV, sizeof(double) * L);
   std::memcpy(h.data() + lay.recoil, d->level_recoil, sizeof(double) * L);
   std::memcpy(h.data() + lay.w, d->level_ob_w_eV, sizeof(double) * L);
@@ -936,12 +1030,26 @@ int32_t avm_gas_create(avm_ctx* ctx, const avm_gas_desc* d, void* dev_buf, size_
   g->d.recoil = (const double*)(base + lay.recoil);
   g->d.w = (const double*)(base + lay.w);
   g->d.type = (const uint8_t*)(base + lay.type);
+  g->d.bshift = bands.shift; g->d.bK = bands.K; g->d.bJ = bands.J;
+  g->d.a0sq = bands.a2[0]; g->d.inv_a0sq = 1.0 / bands.a2[0];
+  g->d.band = (const double2*)(base + lay.band);
+  g->bands = std::move(bands);
   *out = g;
   return AVM_OK;
 }
 
 int32_t avm_gas_destroy(avm_gas* g) { delete g; return AVM_OK; }
 double avm_gas_nu_hat(const avm_gas* g) { return g ? g->nu_hat : 0.0; }
+
+int32_t avm_gas_bands(const avm_gas* g, int32_t* shape3, double* a2, double* nu, double* dtmax) {
+  if (!g || !shape3) return fail(AVM_ERR_INVALID_ARG, "gas_bands: null argument");
+  const BandTable& T = g->bands;
+  shape3[0] = T.K; shape3[1] = T.J; shape3[2] = T.shift;
+  if (a2) std::memcpy(a2, T.a2.data(), sizeof(double) * T.a2.size());
+  if (nu) std::memcpy(nu, T.nu.data(), sizeof(double) * T.nu.size());
+  if (dtmax) std::memcpy(dtmax, T.dtmax.data(), sizeof(double) * T.dtmax.size());
+  return AVM_OK;
+}
 
 int32_t avm_field_create(avm_ctx* ctx, const avm_field_desc* d, avm_field** out) {
   if (!ctx || !out) return fail(AVM_ERR_INVALID_ARG, "field_create: null ctx/out");
@@ -1076,18 +1184,22 @@ namespace {
 typedef void (*TransportFn)(const DevGas, const DevField, const RunArrays, RunCtl*, const PhiloxKeys, const double,
                             const uint32_t, const uint32_t);
 // Tallies are always kept in the hot loop (three per-thread counters); AVM_RUN_NO_TALLIES only skips their publication.
+template <int FK, bool B, int T, bool TPB, bool BANDED>
+TransportFn pick4(bool smemtab) {
+  return smemtab ? transport_kernel<FK, B, true, true, T, TPB, BANDED> : transport_kernel<FK, B, true, false, T, TPB, BANDED>;
+}
 template <int FK, bool B, int T, bool TPB>
-TransportFn pick3(bool smemtab) {
-  return smemtab ? transport_kernel<FK, B, true, true, T, TPB> : transport_kernel<FK, B, true, false, T, TPB>;
+TransportFn pick3(bool smemtab, bool banded) {
+  return banded ? pick4<FK, B, T, TPB, true>(smemtab) : pick4<FK, B, T, TPB, false>(smemtab);
 }
 template <int FK, bool B>
-TransportFn pick2(bool smemtab, bool wide) {
-  return wide ? pick3<FK, B, kThreadsWide, false>(smemtab) : pick3<FK, B, kThreads, true>(smemtab);
+TransportFn pick2(bool smemtab, bool wide, bool banded) {
+  return wide ? pick3<FK, B, kThreadsWide, false>(smemtab, banded) : pick3<FK, B, kThreads, true>(smemtab, banded);
 }
-TransportFn pick_transport(int fk, bool has_b, bool smemtab, bool wide) {
-  if (fk == 1) return has_b ? pick2<1, true>(smemtab, wide) : pick2<1, false>(smemtab, wide);
-  if (fk == 2) return has_b ? pick2<2, true>(smemtab, wide) : pick2<2, false>(smemtab, wide);
-  return has_b ? pick2<0, true>(smemtab, wide) : pick2<0, false>(smemtab, wide);
+TransportFn pick_transport(int fk, bool has_b, bool smemtab, bool wide, bool banded) {
+  if (fk == 1) return has_b ? pick2<1, true>(smemtab, wide, banded) : pick2<1, false>(smemtab, wide, banded);
+  if (fk == 2) return has_b ? pick2<2, true>(smemtab, wide, banded) : pick2<2, false>(smemtab, wide, banded);
+  return has_b ? pick2<0, true>(smemtab, wide, banded) : pick2<0, false>(smemtab, wide, banded);
 }
 }  // namespace
 
@@ -1137,7 +1249,7 @@ int32_t avm_run(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, const 
   const size_t tab_bytes = align_up(sizeof(ushort4) * (size_t)gas->d.nb, 16);
   const bool smemtab = tab_bytes + buf_bytes <= kMaxDynSmem;       // else the threshold table is read through L1
   const size_t dyn_smem = (smemtab ? tab_bytes : 0) + buf_bytes;
-  TransportFn fn = pick_transport(field->fk, field->d.has_B != 0, smemtab, wide);
+  TransportFn fn = pick_transport(field->fk, field->d.has_B != 0, smemtab, wide, (opts->flags & AVM_RUN_BANDED) != 0);
   AVM_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn_smem));
   int occ = 0;
   AVM_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, threads, dyn_smem));
@@ -1223,9 +1335,11 @@ int32_t avm_fetch(avm_ctx* ctx, const avm_outputs* dev, int64_t n, int64_t np, i
 
 int32_t avm_step_batch_form(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, uint64_t seed, double t_max, int32_t form,
                             int32_t k, int64_t n, const double* in, const uint64_t* id, const uint32_t* n_idx, double* out,
-                            int32_t* event, int32_t* status, int32_t* bin, double* child, uint64_t* child_id) {
+                            int32_t* event, int32_t* status, int32_t* bin, double* child, uint64_t* child_id, uint32_t flags) {
   if (!ctx || !gas || !field || n < 0) return fail(AVM_ERR_INVALID_ARG, "step_batch: null argument");
   if (form < 0 || form > 3) return fail(AVM_ERR_INVALID_ARG, "step_batch: form must be 0, 1, 2 or 3");
+  const bool banded = (flags & AVM_RUN_BANDED) != 0;
+  if (banded && form != 1 && form != 3) return fail(AVM_ERR_INVALID_ARG, "step_batch: banded rates run in forms 1 and 3 only (the forms a banded run takes)");
   if (form >= 2 && (k < 1 || k > 16 || n % k != 0)) return fail(AVM_ERR_INVALID_ARG, "step_batch: forms 2 and 3 need 1 <= k <= 16 electrons per warp and n a multiple of k");
   if (form == 2 && !field->uniform1) return fail(AVM_ERR_INVALID_ARG, "step_batch: form 2 (time-parallel batch) needs a field of one uniform slab");
   if (n == 0) return AVM_OK;
@@ -1237,18 +1351,21 @@ int32_t avm_step_batch_form(avm_ctx* ctx, const avm_gas* gas, const avm_field* f
 #define AVM_BARGS gas->d, field->d, seed, t_max, n, (int)k, in, id, n_idx, out, event, status, bin, child, child_id
   if (form == 2) {
     const dim3 grid((unsigned)((n / k + 3) / 4)), block(128);
-    if (b) AVM_CUDA(launch(ctx, step_form_batch_kernel<1, true, 2>, grid, block, AVM_BARGS));
-    else AVM_CUDA(launch(ctx, step_form_batch_kernel<1, false, 2>, grid, block, AVM_BARGS));
+    if (b) AVM_CUDA(launch(ctx, step_form_batch_kernel<1, true, 2, false>, grid, block, AVM_BARGS));
+    else AVM_CUDA(launch(ctx, step_form_batch_kernel<1, false, 2, false>, grid, block, AVM_BARGS));
   } else if (form == 3) {
     const dim3 grid((unsigned)((n / k + 3) / 4)), block(128);
-#define AVM_F3(FK) do { if (b) AVM_CUDA(launch(ctx, step_form_batch_kernel<FK, true, 3>, grid, block, AVM_BARGS)); \
-                        else AVM_CUDA(launch(ctx, step_form_batch_kernel<FK, false, 3>, grid, block, AVM_BARGS)); } while (0)
+#define AVM_F3B(FK, B) do { if (banded) AVM_CUDA(launch(ctx, step_form_batch_kernel<FK, B, 3, true>, grid, block, AVM_BARGS)); \
+                            else AVM_CUDA(launch(ctx, step_form_batch_kernel<FK, B, 3, false>, grid, block, AVM_BARGS)); } while (0)
+#define AVM_F3(FK) do { if (b) AVM_F3B(FK, true); else AVM_F3B(FK, false); } while (0)
     if (fk == 1) AVM_F3(1); else if (fk == 2) AVM_F3(2); else AVM_F3(0);
 #undef AVM_F3
+#undef AVM_F3B
   } else {
     const dim3 grid((unsigned)((n + 127) / 128)), block(128);
-#define AVM_SB(FK, B) do { if (form == 1) AVM_CUDA(launch(ctx, step_batch_kernel<FK, B, 1>, grid, block, AVM_ARGS)); \
-                           else AVM_CUDA(launch(ctx, step_batch_kernel<FK, B, 0>, grid, block, AVM_ARGS)); } while (0)
+#define AVM_SB(FK, B) do { if (form == 1 && banded) AVM_CUDA(launch(ctx, step_batch_kernel<FK, B, 1, true>, grid, block, AVM_ARGS)); \
+                           else if (form == 1) AVM_CUDA(launch(ctx, step_batch_kernel<FK, B, 1, false>, grid, block, AVM_ARGS)); \
+                           else AVM_CUDA(launch(ctx, step_batch_kernel<FK, B, 0, false>, grid, block, AVM_ARGS)); } while (0)
 #define AVM_SBK(FK) do { if (b) AVM_SB(FK, true); else AVM_SB(FK, false); } while (0)
     if (fk == 1) AVM_SBK(1); else if (fk == 2) AVM_SBK(2); else AVM_SBK(0);
 #undef AVM_SBK
@@ -1262,7 +1379,7 @@ int32_t avm_step_batch_form(avm_ctx* ctx, const avm_gas* gas, const avm_field* f
 int32_t avm_step_batch(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, uint64_t seed, double t_max, int64_t n,
                        const double* in, const uint64_t* id, const uint32_t* n_idx, double* out, int32_t* event,
                        int32_t* status, int32_t* bin, double* child, uint64_t* child_id) {
-  return avm_step_batch_form(ctx, gas, field, seed, t_max, 0, 1, n, in, id, n_idx, out, event, status, bin, child, child_id);
+  return avm_step_batch_form(ctx, gas, field, seed, t_max, 0, 1, n, in, id, n_idx, out, event, status, bin, child, child_id, 0u);
 }
 
 int32_t avm_philox_batch(avm_ctx* ctx, uint64_t seed, int64_t n, const uint64_t* id, const uint32_t* n_idx,

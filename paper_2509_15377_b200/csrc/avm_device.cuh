@@ -33,6 +33,11 @@ struct DevGas {
   const double* recoil;   // [L]
   const double* w;        // [L]
   const uint8_t* type;    // [L]
+  // NEXT-1, energy-banded null-collision rate: per acceleration class j and energy band k (2^bshift bins)
+  // the rate nu that bounds the total rate wherever a flight from that band can end within dtmax.
+  int bshift, bK, bJ;
+  double a0sq, inv_a0sq;  // squared edge of class 0, (kappa 250 V/cm)^2; the edge of class j is a0sq 2^j
+  const double2* band;    // [bJ + 1][bK][2]: (1 / nu, dtmax), (nu, floor(nu / nu_hat 2^32) as the low word's bits)
 };
 
 struct DevSlab {
@@ -420,11 +425,47 @@ __device__ __forceinline__ void prefetch_row(const DevGas& g, int b) {
 // top 16 bits, the double is built in the rare exact path.
 struct Pending { int lsel, bin; double xr; };   // lsel: 0 / 1 = level decided from the head record, 2 = scan the row
 
+// BANDED: dt returns -ln(u1); the flight's rate is known only when the flight starts (band_rate).
+template <bool BANDED = false>
 __device__ __forceinline__ void draw_flight(const DevGas& g, const PhiloxKeys& K, const double2* __restrict__ logtab,
                                             uint64_t id, uint32_t n, double& dt, uint2& u2w) {
   const U4 r0 = philox(K, id, n, 0u);                                           // S1
-  dt = -log_unit(to_unit(r0.w0, r0.w1), logtab) * g.inv_nu_hat;                 // S2
+  const double ml = -log_unit(to_unit(r0.w0, r0.w1), logtab);
+  dt = BANDED ? ml : ml * g.inv_nu_hat;                                         // S2
   u2w = make_uint2(r0.w2, r0.w3);
+}
+
+// ---- NEXT-1: the rate of one flight under the energy-banded null-collision method (N5) ---------------
+// Acceleration class of the field E: the number of class edges A_j^2 = a0sq 2^j, j = 0 .. J-1, strictly below |kappa E|^2
+// (J = above every class).  |kappa E|^2 is formed with the oracle's roundings (no contraction), the class from the exponent
+// of a2 / a0sq, corrected by one exact comparison against the neighbouring edge (an edge is a0sq with j added to its exponent).
+__device__ __forceinline__ int accel_class(const DevGas& g, double Ex, double Ey, double Ez) {
+  const double ax = kKappa * Ex, ay = kKappa * Ey, az = kKappa * Ez;
+  const double a2 = __dadd_rn(__dadd_rn(__dmul_rn(ax, ax), __dmul_rn(ay, ay)), __dmul_rn(az, az));
+  const int e = ((__double2hiint(a2 * g.inv_a0sq) >> 20) & 0x7FF) - 1023;
+  int j = min(max(e + 1, 0), g.bJ);
+  const int h0 = __double2hiint(g.a0sq), l0 = __double2loint(g.a0sq);
+  const double below = __hiloint2double(h0 + ((j - 1) << 20), l0), at = __hiloint2double(h0 + (j << 20), l0);
+  if (j > 0 && !(a2 > below)) --j;
+  else if (j < g.bJ && a2 > at) ++j;
+  return j;
+}
+struct BandRate { double inv_nu, dtmax, nu; uint32_t rho; };
+// s2 = |v|^2 at the start of the flight; its energy bin (as energy_bin) >> bshift = the band.
+__device__ __forceinline__ BandRate band_rate(const DevGas& g, double s2, int jcls) {
+  const int braw = __double2int_rz((s2 * kInvC2Sq) * g.inv_de);
+  const int b0 = max(min(braw, g.nb - 1), g.bin_floor);
+  const double2* p = g.band + 2 * ((size_t)jcls * g.bK + (b0 >> g.bshift));
+  const double2 q0 = __ldg(p), q1 = __ldg(p + 1);
+  BandRate r;
+  r.inv_nu = q0.x; r.dtmax = q0.y; r.nu = q1.x; r.rho = (uint32_t)__double2loint(q1.y);
+  return r;
+}
+// The flight time of a banded flight from its -ln(u1): cut at dtmax (a cut flight ends in a null collision, N6).
+__device__ __forceinline__ double banded_dt(const BandRate& br, double mlog, bool& cut) {
+  const double dt = mlog * br.inv_nu;
+  cut = dt > br.dtmax;
+  return cut ? br.dtmax : dt;
 }
 
 // S7 + the common part of S8 for bin b and uniform u2 = to_unit(u2w): -1 = null collision, 0 / 1 = level 0 / 1, 2 = a
@@ -434,8 +475,11 @@ __device__ __forceinline__ void draw_flight(const DevGas& g, const PhiloxKeys& K
 // fp64 product — so the 16-bit filter takes the oracle's decision exactly, and the 2e-4 of the steps that fall inside a
 // band are decided from the exact fp64 record.
 // The 16-bit filter alone, branch-free: -1 / 0 / 1 / 2 as decide(), or -2 when h lies in a band (exact record needed).
-__device__ __forceinline__ int decide_filter(const ushort4 rec, uint2 u2w) {
-  const uint32_t h = u2w.x >> 16;
+// BANDED: the comparison is u2 nu >= cum with the flight's own rate nu = rho nu_hat, rho <= 1: h = floor(u2 rho 2^16) up to
+// [0, 1 + 2^-14) (umulhi of the top words of u2 and rho 2^32), which the +-2 band of the filter still covers.
+template <bool BANDED = false>
+__device__ __forceinline__ int decide_filter(const ushort4 rec, uint2 u2w, uint32_t rho = 0u) {
+  const uint32_t h = BANDED ? (__umulhi(u2w.x, rho) >> 16) : (u2w.x >> 16);
   const uint32_t qt = rec.x, q0 = rec.y, q1 = rec.z;
   const bool null = h >= qt + 2u, l0 = h + 2u <= q0;
   const bool l1 = (h >= q0 + 2u) & (h + 2u <= q1), l2 = (h >= q1 + 2u) & (h + 2u <= qt);

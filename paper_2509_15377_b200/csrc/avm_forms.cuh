@@ -37,21 +37,33 @@ static_assert(sizeof(WarpBuf) == 1920, "WarpBuf");
 // S3-S7 with this flight's pre-drawn (dt, u2w); the draws of the lane's NEXT flight are issued behind the threshold-record
 // load.  On return: fin = finishing status (or 0), pend / pc = a real collision is pending (collision_step follows, in
 // the warp's one collision phase), (dt, u2w) = the next flight's draws.
-template <int FK, bool HASB, bool TALLY>
+// BANDED (NEXT-1): dt carries -ln(u1); the flight's rate comes from the band of the electron's energy and
+// the class of the field at its position (jcls = the class when the field is one uniform slab), a flight longer than the
+// band's dtmax is cut there and ends in a null collision, and the decision compares u2 nu with the flight's own nu.
+template <int FK, bool HASB, bool TALLY, bool BANDED = false>
 __device__ __forceinline__ void fw_flight(const DevGas& g, const DevField& f, const PhiloxKeys& K,
                                           const ushort4* __restrict__ tab, const double2* __restrict__ logtab,
                                           const double t_max, const uint64_t id, uint32_t& n, double& x, double& y,
                                           double& z, double& t, double& vx, double& vy, double& vz, double& Ex, double& Ey,
-                                          double& Ez, double& dt, uint2& u2w, int& fin, bool& pend, Pending& pc, Tally& tl) {
-  bool over = false;
-  const int b = advance<FK, HASB>(g, f, t_max, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt, over);
+                                          double& Ez, double& dt, uint2& u2w, int& fin, bool& pend, Pending& pc, Tally& tl,
+                                          const int jcls = 0) {
+  bool over = false, cut = false;
+  double dtf = dt, nu = g.nu_hat;
+  uint32_t rho = 0u;
+  if (BANDED) {
+    const BandRate br = band_rate(g, vx * vx + vy * vy + vz * vz, FK == 1 ? jcls : accel_class(g, Ex, Ey, Ez));
+    dtf = banded_dt(br, dt, cut);
+    nu = br.nu; rho = br.rho;
+  }
+  const int b = advance<FK, HASB>(g, f, t_max, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dtf, over);
   if (b < 0) { fin = -b; return; }
   const ushort4 rec = tab[b];
   const uint2 u2c = u2w;
-  draw_flight(g, K, logtab, id, n, dt, u2w);          // next flight's draws: independent of the record load
-  int r = decide_filter(rec, u2c);                    // branch-free; the rare outcomes below
+  draw_flight<BANDED>(g, K, logtab, id, n, dt, u2w);  // next flight's draws: independent of the record load
+  int r = decide_filter<BANDED>(rec, u2c, rho);       // branch-free; the rare outcomes below
+  if (BANDED && cut) r = -1;
   if (r == -2 || r == 2) {
-    pc.xr = to_unit(u2c.x, u2c.y) * g.nu_hat;
+    pc.xr = to_unit(u2c.x, u2c.y) * nu;
     if (r == -2) r = decide_exact(g, b, pc.xr);
     if (r == 2) prefetch_row(g, b);
   }
@@ -222,13 +234,14 @@ __device__ __forceinline__ int tp_batch(const DevGas& g, const DevField& f, cons
 // collide(mask, pend, pc, have_d, d, fin) -> level and retire(mask, fin) are called by the lanes with an event only, with
 // mask = the lanes converged at the call (the warp-aggregated atomics inside them run over that mask); retire clears
 // `have`.  commit(e, s, ev, bin, fin): step s of the batch of the warp's e-th electron is done, its result is in x .. vz, n.
-template <int FK, bool HASB, bool TALLY, class Collide, class Retire, class Commit>
+// BANDED: as fw_flight — the exchange area holds -ln(u1) per step, the rate is looked up when the step starts.
+template <int FK, bool HASB, bool TALLY, bool BANDED, class Collide, class Retire, class Commit>
 __device__ __forceinline__ void sb_batch(const DevGas& g, const DevField& f, const PhiloxKeys& K,
                                          const ushort4* __restrict__ tab, const double2* __restrict__ s_logtab,
                                          WarpBuf* __restrict__ wb, const double t_max, const unsigned lane, const unsigned act,
                                          bool& have, double& x, double& y, double& z, double& t, double& vx, double& vy,
                                          double& vz, double& Ex, double& Ey, double& Ez, const uint64_t& id, uint32_t& n,
-                                         Tally& tl, Collide&& collide, Retire&& retire, Commit&& commit) {
+                                         Tally& tl, Collide&& collide, Retire&& retire, Commit&& commit, const int jcls = 0) {
   const unsigned lt_mask = (1u << lane) - 1u;
   const int k = __popc(act);
   const int lg = 32 - __clz(k - 1);             // k' = 2^lg >= k  (k = 1: __clz(0) = 32)
@@ -243,7 +256,7 @@ __device__ __forceinline__ void sb_batch(const DevGas& g, const DevField& f, con
       const uint32_t hn = wb->n[e] + (uint32_t)s;
       double ddt;
       uint2 du2;
-      draw_flight(g, K, s_logtab, hid, hn, ddt, du2);
+      draw_flight<BANDED>(g, K, s_logtab, hid, hn, ddt, du2);
       const Deflection d = deflection_draws(K, hid, hn);
       wb->dt[lane] = ddt; wb->u2w[lane] = du2;
       wb->ct[lane] = d.ct; wb->st[lane] = d.st; wb->cphi[lane] = d.cphi; wb->sphi[lane] = d.sphi;
@@ -254,12 +267,21 @@ __device__ __forceinline__ void sb_batch(const DevGas& g, const DevField& f, con
 #pragma unroll 1
   while (have && s < nb_steps) {
     const int idx = s * kp + rank;
-    const double dtj = wb->dt[idx];
+    double dtj = wb->dt[idx];
     const uint2 u2 = wb->u2w[idx];
+    bool cut = false;
+    double nu = g.nu_hat;
+    uint32_t rho = 0u;
+    if (BANDED) {
+      const BandRate br = band_rate(g, vx * vx + vy * vy + vz * vz, FK == 1 ? jcls : accel_class(g, Ex, Ey, Ez));
+      dtj = banded_dt(br, dtj, cut);
+      nu = br.nu; rho = br.rho;
+    }
     const double s2 = advance_move<FK, HASB>(f, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dtj);   // S3, S4
     bool over;
     const int b = energy_bin(g, s2, over);                                                     // S6 (counts only when S5 passes)
-    int r = decide_filter(tab[b], u2);                                                         // S7 and the head of S8
+    int r = decide_filter<BANDED>(tab[b], u2, rho);                                            // S7 and the head of S8
+    if (BANDED && cut) r = -1;
     const int st = s5_status<FK>(f, t_max, n, x, y, z, t, Ex, Ey, Ez);                         // S5; the field at r' = S0 of the next step
     if (TALLY && over && st == 0) ++tl.over;
     int ev = -1, fin = 0;
@@ -269,7 +291,7 @@ __device__ __forceinline__ void sb_batch(const DevGas& g, const DevField& f, con
         Pending pc;
         pc.lsel = 0; pc.bin = b; pc.xr = 0.0;
         if (r == -2 || r == 2) {
-          pc.xr = to_unit(u2.x, u2.y) * g.nu_hat;
+          pc.xr = to_unit(u2.x, u2.y) * nu;
           if (r == -2) r = decide_exact(g, b, pc.xr);
           if (r == 2) prefetch_row(g, b);
         }
