@@ -284,11 +284,11 @@ def bench_workload(avm, ctx, torch, dist, name, steps, warmup, sample, rank, wor
             dist.barrier()
         torch.cuda.synchronize()
 
-    def device_step(seed):
+    def device_step(seed, flags=0):
         flush.zero_()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
-        _, n = avm.run(ctx, gg, fg, prim_dev, bufs, seed=seed, t_max=w.t_max, id_offset=id_offset)
+        _, n = avm.run(ctx, gg, fg, prim_dev, bufs, seed=seed, t_max=w.t_max, id_offset=id_offset, flags=flags)
         e1.record()
         e1.synchronize()
         t = bufs.tallies_u64.cpu().numpy().view(np.uint64)
@@ -321,6 +321,13 @@ def bench_workload(avm, ctx, torch, dist, name, steps, warmup, sample, rank, wor
     barrier()
     e2e = [e2e_step(w.seed + i) for i in range(steps)]
     barrier()
+    # the same workload under the energy-banded null-collision rate (AVM_RUN_BANDED): same physics in
+    # fewer null steps, so collisions/s falls while avalanches/s rises — reported beside the headline, never as it
+    for i in range(min(warmup, 2)):
+        device_step(w.seed + 3000 + i, avm.RUN_BANDED)
+    barrier()
+    bd = [device_step(w.seed + i, avm.RUN_BANDED) for i in range(steps)]
+    barrier()
 
     gfrac = grid_fraction(w.field)
     tot_ms = sum(s["ms"] for s in st)
@@ -329,13 +336,15 @@ def bench_workload(avm, ctx, torch, dist, name, steps, warmup, sample, rank, wor
             sum(s["launches"] for s in st), sum(int(s["tallies"][L]) + int(s["tallies"][L + 1]) for s in e2e),
             sum(alg_fp64(s["tallies"], L, w.gas.level_type, has_b, gfrac) for s in st), sum(s["transport_launches"] for s in st)]
     e2e_s = sum(s["s"] for s in e2e)
-    vals = torch.tensor([tot_ms, e2e_s, t_ms], dtype=torch.float64, device=ctx.device)
-    sums_t = torch.tensor(sums, dtype=torch.float64, device=ctx.device)
+    bd_ms = sum(s["ms"] for s in bd)
+    bd_sums = [sum(int(s["tallies"][L]) for s in bd), sum(int(s["tallies"][L + 1]) for s in bd), sum(int(s["n"]) for s in bd)]
+    vals = torch.tensor([tot_ms, e2e_s, t_ms, bd_ms], dtype=torch.float64, device=ctx.device)
+    sums_t = torch.tensor(sums + bd_sums, dtype=torch.float64, device=ctx.device)
     if dist is not None:
         dist.all_reduce(vals, op=dist.ReduceOp.MAX)          # reporting only: max time over ranks, job totals
         dist.all_reduce(sums_t, op=dist.ReduceOp.SUM)
-    tot_ms_max, e2e_s_max, _ = (float(x) for x in vals.cpu())
-    null, real, electrons, launches, e2e_coll, _, _ = (float(x) for x in sums_t.cpu())
+    tot_ms_max, e2e_s_max, _, bd_ms_max = (float(x) for x in vals.cpu())
+    null, real, electrons, launches, e2e_coll, _, _, bd_null, bd_real, bd_el = (float(x) for x in sums_t.cpu())
     if rank != 0:
         return None, clocks
     # roofline of the dominant kernel (transport_kernel), this rank: algorithmic units per launch / its average launch
@@ -368,7 +377,13 @@ def bench_workload(avm, ctx, torch, dist, name, steps, warmup, sample, rank, wor
              "collisions_per_step": (null + real) / max(steps, 1) / world, "roofline": roofline,
              "e2e": {"value": e2e_coll / e2e_s_max, "unit": UNIT, "h2d_bytes_per_step": int(w.n_primaries * 64),
                      "d2h_bytes_per_step": int(sum(s["d2h"] for s in e2e) / max(len(e2e), 1)), "ms_per_step": 1e3 * e2e_s_max / max(steps, 1)},
-             "gpu_launches": int(launches), "config": config_dict(w, world), "capacity": w.capacity, "clocks": clocks}
+             "gpu_launches": int(launches), "config": config_dict(w, world), "capacity": w.capacity, "clocks": clocks,
+             "banded": {"what": "same workload with AVM_RUN_BANDED (energy-banded null-collision rate, DESIGN.md §3.5): other random streams, same physics",
+                        "value": (bd_null + bd_real) / (bd_ms_max * 1e-3), "unit": UNIT, "ms_per_step": bd_ms_max / max(steps, 1),
+                        "null_per_s": bd_null / (bd_ms_max * 1e-3), "real_per_s": bd_real / (bd_ms_max * 1e-3),
+                        "avalanches_per_s": world * w.n_primaries * steps / (bd_ms_max * 1e-3),
+                        "electrons_per_step": bd_el / max(steps, 1) / world,
+                        "speedup_avalanches_per_s": tot_ms_max / max(bd_ms_max, 1e-9)}}
     if with_cpu:
         entry["cpu_baseline"] = cpu_baseline_entry(w, sample, cores)
     return entry, clocks
