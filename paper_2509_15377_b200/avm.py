@@ -15,7 +15,7 @@ import numpy as np
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SO = os.path.join(_HERE, "libavm.so")
+_SO = os.environ.get("AVM_LIBRARY") or os.path.join(_HERE, "libavm.so")    # AVM_LIBRARY: the -DAVM_DEBUG build (build.SO_DEBUG)
 if not os.path.exists(_SO):
     raise ImportError(f"{_SO} is missing: build it with `python -m paper_2509_15377_b200.build` "
                       "(nvcc, sm_100a).  There is no CPU fallback.")

@@ -7,6 +7,19 @@
 
 #include "../../include/avm.h"
 
+// -DAVM_DEBUG (python -m paper_2509_15377_b200.build -DAVM_DEBUG -> libavm_debug.so): every table, map, slot, ticket and
+// exchange-area index of the device code is range-checked and the kernel traps on a violation; compute-sanitizer is not
+// available on the GPU pool, so the edge-case and relaunch tests are run once per round against this build.
+#ifdef AVM_DEBUG
+#include <cstdio>
+#define AVM_CHECK(cond)                                                              \
+  do {                                                                               \
+    if (!(cond)) { printf("AVM_CHECK failed: %s (%s:%d)\n", #cond, __FILE__, __LINE__); __trap(); } \
+  } while (0)
+#else
+#define AVM_CHECK(cond) do { } while (0)
+#endif
+
 namespace avm {
 
 // ---- constants (DESIGN.md §3 "Constants"; CODATA-2018 c = 29.9792458 cm/ns, mc^2 = 510998.95 eV) ------------
@@ -105,17 +118,17 @@ __device__ __forceinline__ double to_unit(uint32_t hi, uint32_t lo) {
 // Coefficients live in constant memory so that they enter DFMA as constant-bank operands (an fp64 immediate costs
 // two UMOVs).  Accuracy: a few ulp, far inside the 1e-12 parity tolerance.
 // log1p(r) = r + r^2 (kLog1pC[0] + kLog1pC[1] r + ...), |r| < 2^-7: the first dropped term is r^9/9 < 2e-18 |r|
-__constant__ double kLog1pC[7] = {-1.0 / 2.0, 1.0 / 3.0, -1.0 / 4.0, 1.0 / 5.0, -1.0 / 6.0, 1.0 / 7.0, -1.0 / 8.0};
+static __constant__ double kLog1pC[7] = {-1.0 / 2.0, 1.0 / 3.0, -1.0 / 4.0, 1.0 / 5.0, -1.0 / 6.0, 1.0 / 7.0, -1.0 / 8.0};
 // (rc, L) per 1/128 of the mantissa range — see gen_logtab.py.  Kernels stage it in shared memory.
 struct LogEntry { unsigned long long rc, L; };
-__device__ const LogEntry kLogTab[128] = {
+static __device__ const LogEntry kLogTab[128] = {
 #include "avm_logtab.inc"
 };
 // sin(r pi/2) = r sum_k kSinC[k] r^2k, cos(r pi/2) = sum_k kCosC[k] r^2k (Taylor; |r| <= 1/2: truncation < 5e-17)
-__constant__ double kSinC[8] = {1.5707963267948966, -0.6459640975062463, 0.07969262624616705, -0.004681754135318688,
+static __constant__ double kSinC[8] = {1.5707963267948966, -0.6459640975062463, 0.07969262624616705, -0.004681754135318688,
                                 0.00016044118478735983, -3.598843235212085e-06, 5.692172921967927e-08,
                                 -6.688035109811468e-10};
-__constant__ double kCosC[9] = {1.0, -1.2337005501361697, 0.25366950790104803, -0.02086348076335296,
+static __constant__ double kCosC[9] = {1.0, -1.2337005501361697, 0.25366950790104803, -0.02086348076335296,
                                 0.0009192602748394266, -2.5202042373060607e-05, 4.710874778818172e-07,
                                 -6.386603083791852e-09, 6.565963114979473e-11};
 
@@ -231,6 +244,7 @@ __device__ __forceinline__ bool grid_at(const DevSlab& s, double x, double y, do
   cell_of((z - s.org[2]) * s.inv_h[2], s.nz, k, wz);
   const size_t sy = (size_t)s.nx, sz = (size_t)s.nx * s.ny;
   const size_t o = ((size_t)k * s.ny + j) * s.nx + i;
+  AVM_CHECK(i >= 0 && j >= 0 && k >= 0 && o + sz + sy + 1 < (size_t)s.nx * s.ny * s.nz);
   double ex, ey;
   if (s.nodes64) {
     const double2* p = reinterpret_cast<const double2*>(s.nodes64) + 2 * o;
@@ -455,6 +469,7 @@ struct BandRate { double inv_nu, dtmax, nu; uint32_t rho; };
 __device__ __forceinline__ BandRate band_rate(const DevGas& g, double s2, int jcls) {
   const int braw = __double2int_rz((s2 * kInvC2Sq) * g.inv_de);
   const int b0 = max(min(braw, g.nb - 1), g.bin_floor);
+  AVM_CHECK(jcls >= 0 && jcls <= g.bJ && b0 >= 0 && (b0 >> g.bshift) < g.bK);
   const double2* p = g.band + 2 * ((size_t)jcls * g.bK + (b0 >> g.bshift));
   const double2 q0 = __ldg(p), q1 = __ldg(p + 1);
   BandRate r;
@@ -626,6 +641,7 @@ __device__ __forceinline__ int collision_step(const DevGas& g, const LevelPar* _
                                               double& vx, double& vy, double& vz, int& status, bool& spawn, Child& ch,
                                               double& loss) {
   const int l = p.lsel < 2 ? p.lsel : select_level_from2(g, p.bin, p.xr);     // S8
+  AVM_CHECK(l >= 0 && l < g.L && p.bin >= 0 && p.bin < g.nb);
   const LevelPar par = lv[l];
   status = 0; spawn = false; loss = 0.0;
   if (par.type == AVM_ATTACHMENT) { status = AVM_ATTACHED; return l; }         // S9a

@@ -57,6 +57,7 @@ __device__ __forceinline__ void fw_flight(const DevGas& g, const DevField& f, co
   }
   const int b = advance<FK, HASB>(g, f, t_max, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dtf, over);
   if (b < 0) { fin = -b; return; }
+  AVM_CHECK(b < g.nb);
   const ushort4 rec = tab[b];
   const uint2 u2c = u2w;
   draw_flight<BANDED>(g, K, logtab, id, n, dt, u2w);  // next flight's draws: independent of the record load
@@ -99,6 +100,7 @@ __device__ __forceinline__ int tp_batch(const DevGas& g, const DevField& f, cons
   const int kp = 1 << lg, gl = 32 >> lg;        // gl = lanes (steps per batch) of one electron
   const int rank = __popc(act & lt_mask);
   const int e = (int)lane & (kp - 1), sidx = (int)lane >> lg;
+  AVM_CHECK(k >= 1 && k <= 16 && (!have || rank < 16));
   if (have) {
     wb->bsv[rank][0] = make_double2(x, y); wb->bsv[rank][1] = make_double2(z, t);
     wb->bsv[rank][2] = make_double2(vx, vy); wb->bsv[rank][3] = make_double2(vz, 0.0);
@@ -153,6 +155,7 @@ __device__ __forceinline__ int tp_batch(const DevGas& g, const DevField& f, cons
       n = n + 1u;
       const bool ok = uniform_continues(f, t_max, n, x, y, z, t);
       b = energy_bin(g, s2, over);
+      AVM_CHECK(b >= 0 && b < g.nb);
       r = decide_filter(tab[b], u2j);
       const LevelPar par = s_lv[r == 1 ? 1 : 0];
       fvx = vx; fvy = vy; fvz = vz;
@@ -267,6 +270,7 @@ __device__ __forceinline__ void sb_batch(const DevGas& g, const DevField& f, con
 #pragma unroll 1
   while (have && s < nb_steps) {
     const int idx = s * kp + rank;
+    AVM_CHECK(idx >= 0 && idx < 32 && rank < 16);
     double dtj = wb->dt[idx];
     const uint2 u2 = wb->u2w[idx];
     bool cut = false;
@@ -280,6 +284,7 @@ __device__ __forceinline__ void sb_batch(const DevGas& g, const DevField& f, con
     const double s2 = advance_move<FK, HASB>(f, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dtj);   // S3, S4
     bool over;
     const int b = energy_bin(g, s2, over);                                                     // S6 (counts only when S5 passes)
+    AVM_CHECK(b >= 0 && b < g.nb);
     int r = decide_filter<BANDED>(tab[b], u2, rho);                                            // S7 and the head of S8
     if (BANDED && cut) r = -1;
     const int st = s5_status<FK>(f, t_max, n, x, y, z, t, Ex, Ey, Ez);                         // S5; the field at r' = S0 of the next step
