@@ -75,6 +75,8 @@ struct Gas {
   const double* cum = nullptr;
   const uint8_t* type = nullptr;
   const double *loss = nullptr, *recoil = nullptr, *w = nullptr;
+  const double *xi = nullptr, *pen_p = nullptr, *pen_e = nullptr;   // NEXT-3: X1, X2
+  double kT = 0.0;                                                  // X3
   Majorant M;
 };
 
@@ -88,7 +90,7 @@ struct Electron {
 
 struct Tally {
   std::vector<uint64_t> level;
-  uint64_t n_null = 0, n_real = 0, n_overflow = 0, n_steps = 0, n_viol = 0;
+  uint64_t n_null = 0, n_real = 0, n_overflow = 0, n_steps = 0, n_viol = 0, n_penning = 0;
   double sdx = 0, sdy = 0, sdz = 0, sdt = 0, sloss = 0;
 };
 
@@ -167,6 +169,13 @@ bool load_gas(const avmo_gas_desc* d, Gas& g) {
     mx = std::max(mx, prev);
   }
   for (int l = 0; l < g.L; ++l) if (g.type[l] > 3) { g_err = "gas: bad level type"; return false; }
+  g.xi = d->scat_xi; g.pen_p = d->level_penning_prob; g.pen_e = d->level_penning_eV; g.kT = d->kT_eV;
+  if (g.xi)
+    for (size_t i = 0; i < (size_t)g.nb * g.L; ++i) if (!(g.xi[i] > -1.0 && g.xi[i] < 1.0)) { g_err = "gas: scat_xi outside (-1, 1)"; return false; }
+  if ((g.pen_p != nullptr) != (g.pen_e != nullptr)) { g_err = "gas: Penning probability and energy come together"; return false; }
+  if (g.pen_p)
+    for (int l = 0; l < g.L; ++l) if (!(g.pen_p[l] >= 0.0 && g.pen_p[l] <= 1.0) || !(g.pen_e[l] >= 0.0)) { g_err = "gas: Penning parameters"; return false; }
+  if (!(g.kT >= 0.0)) { g_err = "gas: kT < 0"; return false; }
   g.nu_hat = d->nu_hat > 0 ? d->nu_hat : mx;      // R4: one global null-collision rate
   if (!(g.nu_hat > 0) || g.nu_hat < mx) { g_err = "gas: nu_hat must be >= max total rate and > 0"; return false; }
   g.inv_nu_hat = 1.0 / g.nu_hat;
@@ -369,18 +378,69 @@ void step(const Gas& g, const avmo_field_desc* f, uint64_t seed, double t_max, b
   // S9b: deflection angles
   double u3, u4;
   uniform_pair(seed, el.id, n_s, 1, u3, u4);
-  const double ct = 1.0 - 2.0 * u3;
-  const double st = 2.0 * std::sqrt(u3 * (1.0 - u3));
+  double ct = 1.0 - 2.0 * u3;
+  double st = 2.0 * std::sqrt(u3 * (1.0 - u3));
+  if (g.xi) {
+    // X1: forward-peaked deflection, cos(theta) = (c0 + xi) / (1 + xi c0) with c0 = 1 - 2 u3 uniform in (-1, 1) and xi the
+    // table entry of this bin and level; sin(theta) in the cancellation-free form sqrt((1 - ct)(1 + ct)) =
+    // 2 sqrt(u3 (1 - u3)) sqrt(1 - xi^2) / (1 + xi c0)
+    const double xi = g.xi[(size_t)b * g.L + l];
+    const double den = 1.0 + xi * ct;
+    st = st * std::sqrt(1.0 - xi * xi) / den;
+    ct = (ct + xi) / den;
+  }
   const double phi = TWO_PI * u4;
   const double sphi = std::sin(phi), cphi = std::cos(phi);
   // S9c: energy after the collision
   double e2;
-  if (g.type[l] == AVMO_ELASTIC) {
+  bool thermal = false;
+  double V[3] = {0.0, 0.0, 0.0};
+  if (g.type[l] == AVMO_ELASTIC && g.kT > 0.0 && g.recoil[l] > 0.0) {
+    // X3: the gas atom moves.  Its velocity components are normal with variance kT / M, M / m = 2 / r (R9's order):
+    // sigma = c2 sqrt(kT r / 4); Box-Muller from blocks 2 and 3.  The cold-gas collision (S9b-S9d) is applied to the
+    // electron's velocity RELATIVE to the atom, w = v' - V, and the atom's velocity is added back.
+    double u5, u6, u7, u8;
+    uniform_pair(seed, el.id, n_s, 2, u5, u6);
+    uniform_pair(seed, el.id, n_s, 3, u7, u8);
+    const double sigma = C2 * std::sqrt(g.kT * g.recoil[l] * 0.25);
+    const double ra = std::sqrt(-2.0 * std::log(u5)), rb = std::sqrt(-2.0 * std::log(u7));
+    V[0] = sigma * ra * std::cos(TWO_PI * u6);
+    V[1] = sigma * ra * std::sin(TWO_PI * u6);
+    V[2] = sigma * rb * std::cos(TWO_PI * u8);
+    const double w[3] = {v1[0] - V[0], v1[1] - V[1], v1[2] - V[2]};
+    const double w2 = w[0] * w[0] + w[1] * w[1] + w[2] * w[2];
+    const double ew = std::max(w2 * INV_C2SQ, EPS_FLOOR);
+    if (w2 > 0.0) { const double nrm = std::sqrt(w2); k1[0] = w[0] / nrm; k1[1] = w[1] / nrm; k1[2] = w[2] / nrm; }
+    e2 = ew * (1.0 - g.recoil[l] * (1.0 - ct));                    // relative-frame energy after the collision
+    thermal = true;
+  } else if (g.type[l] == AVMO_ELASTIC) {
     e2 = e1 * (1.0 - g.recoil[l] * (1.0 - ct));                    // R9
     if (tl) tl->sloss += e1 - e2;
   } else if (g.type[l] == AVMO_EXCITATION) {
     e2 = std::max(e1 - g.loss[l], EPS_FLOOR);                      // R11
     if (tl) tl->sloss += e1 - e2;
+    if (g.pen_p && g.pen_p[l] > 0.0) {
+      // X2: Penning transfer — with probability p_l the excited atom ionises the admixture: one more electron at r', t'
+      // with energy u8 x (available energy), isotropic direction from (u6, u7), id hashed like an ionisation's child
+      double u5, u6, u7, u8;
+      uniform_pair(seed, el.id, n_s, 2, u5, u6);
+      uniform_pair(seed, el.id, n_s, 3, u7, u8);
+      if (u5 < g.pen_p[l]) {
+        Electron& c = so.c;
+        c.x = r1[0]; c.y = r1[1]; c.z = r1[2]; c.t = t1;
+        c.e = std::max(u8 * g.pen_e[l], EPS_FLOOR);
+        const double sc = 2.0 * std::sqrt(u6 * (1.0 - u6));
+        const double pc = TWO_PI * u7;
+        c.kx = sc * std::cos(pc); c.ky = sc * std::sin(pc); c.kz = 1.0 - 2.0 * u6;
+        uint32_t wd[4];
+        philox_block(seed, el.id, n_s, BLOCK_CHILD_ID, wd);
+        c.id = (uint64_t)wd[0] + ((uint64_t)wd[1] << 32);
+        c.n = 0; c.aval = el.aval; c.status = AVMO_ACTIVE;
+        c.birth[0] = c.x; c.birth[1] = c.y; c.birth[2] = c.z; c.birth[3] = c.t; c.birth[4] = c.e;
+        so.child = true;
+        if (tl) tl->n_penning++;
+      }
+    }
   } else {                                                         // ionisation, R10 (Opal-Peterson-Beaty)
     double u5, u6, u7, u8;
     uniform_pair(seed, el.id, n_s, 2, u5, u6);
@@ -414,6 +474,15 @@ void step(const Gas& g, const avmo_field_desc* f, uint64_t seed, double t_max, b
   for (int i = 0; i < 3; ++i) k2[i] = ct * k1[i] + st * (cphi * b1[i] + sphi * b2[i]);
   const double nk = std::sqrt(k2[0] * k2[0] + k2[1] * k2[1] + k2[2] * k2[2]);
   el.kx = k2[0] / nk; el.ky = k2[1] / nk; el.kz = k2[2] / nk;
+  if (thermal) {
+    // X3, back to the laboratory frame: v'' = c2 sqrt(e2) k'' + V; energy and direction from v''
+    const double sw = C2 * std::sqrt(e2);
+    const double v2[3] = {sw * el.kx + V[0], sw * el.ky + V[1], sw * el.kz + V[2]};
+    const double s22 = v2[0] * v2[0] + v2[1] * v2[1] + v2[2] * v2[2];
+    el.e = std::max(s22 * INV_C2SQ, EPS_FLOOR);
+    if (s22 > 0.0) { const double nrm = std::sqrt(s22); el.kx = v2[0] / nrm; el.ky = v2[1] / nrm; el.kz = v2[2] / nrm; }
+    if (tl) tl->sloss += e1 - el.e;
+  }
 }
 
 struct Record { Electron el; };
@@ -560,11 +629,12 @@ int32_t avmo_run(const avmo_gas_desc* gd, const avmo_field_desc* f, const double
   if (o->per_avalanche)
     for (int64_t p = 0; p < np; ++p) o->per_avalanche[3 * p + 1] = o->per_avalanche[3 * p] > 0 ? o->per_avalanche[3 * p] - 1 : 0;
   if (o->tallies_u64) {
-    for (int l = 0; l < g.L + 5; ++l) o->tallies_u64[l] = 0;
+    for (int l = 0; l < g.L + 6; ++l) o->tallies_u64[l] = 0;
     for (auto& t : tl) {
       for (int l = 0; l < g.L; ++l) o->tallies_u64[l] += t.level[l];
       o->tallies_u64[g.L] += t.n_null; o->tallies_u64[g.L + 1] += t.n_real;
-      o->tallies_u64[g.L + 2] += t.n_overflow; o->tallies_u64[g.L + 3] += t.n_steps; o->tallies_u64[g.L + 4] += t.n_viol;
+      o->tallies_u64[g.L + 2] += t.n_overflow; o->tallies_u64[g.L + 3] += t.n_steps; o->tallies_u64[g.L + 4] += t.n_penning;
+      o->tallies_u64[g.L + 5] += t.n_viol;
     }
   }
   if (o->tallies_f64) {

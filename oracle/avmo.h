@@ -38,6 +38,11 @@ typedef struct {
   const double*  level_recoil;
   const double*  level_ob_w_eV;
   double nu_hat;                  /* <= 0: max_b cum_rate[b][L-1] */
+  /* NEXT-3 (DESIGN.md §3.6 readings X1-X3); every one optional (NULL / 0 = the base model R8, R9): */
+  const double*  scat_xi;            /* X1 [n_bins][n_levels]: forward-scattering parameter xi in (-1, 1) of S9b, 0 = isotropic */
+  const double*  level_penning_prob; /* X2 [n_levels]: probability that an excitation of the level ionises the admixture */
+  const double*  level_penning_eV;   /* X2 [n_levels]: energy available to that electron (excitation energy - ionisation potential) */
+  double kT_eV;                      /* X3: gas temperature (0.02526 eV at 293.15 K); 0 = cold gas */
 } avmo_gas_desc;
 
 typedef struct {
@@ -64,7 +69,7 @@ typedef struct {
   double* birth;            /* [5][capacity]: x0,y0,z0,t0,e0 */
   double* end;              /* [8][capacity]: x1,y1,z1,t1,e1,kx,ky,kz */
   uint64_t* per_avalanche;  /* [Np][3]: endpoints, ions, negative ions */
-  uint64_t* tallies_u64;    /* [n_levels+5]: per level, null, real, overflow, steps, banded-rate violations (always 0) */
+  uint64_t* tallies_u64;    /* [n_levels+6]: per level, null, real, overflow, steps, Penning transfers, banded-rate violations (always 0) */
   double*   tallies_f64;    /* [5]: sum dx,dy,dz over all flights, sum dt, sum energy loss */
 } avmo_outputs;
 

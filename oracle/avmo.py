@@ -31,7 +31,9 @@ def build(force: bool = False) -> str:
 class GasDesc(C.Structure):
     _fields_ = [("n_bins", C.c_int32), ("e_max_eV", C.c_double), ("n_levels", C.c_int32),
                 ("cum_rate", C.c_void_p), ("level_type", C.c_void_p), ("level_loss_eV", C.c_void_p),
-                ("level_recoil", C.c_void_p), ("level_ob_w_eV", C.c_void_p), ("nu_hat", C.c_double)]
+                ("level_recoil", C.c_void_p), ("level_ob_w_eV", C.c_void_p), ("nu_hat", C.c_double),
+                ("scat_xi", C.c_void_p), ("level_penning_prob", C.c_void_p), ("level_penning_eV", C.c_void_p),
+                ("kT_eV", C.c_double)]
 
 
 class SlabDesc(C.Structure):
@@ -92,8 +94,17 @@ def gas_desc(gas) -> tuple:
     rc = np.ascontiguousarray(gas.level_recoil, dtype=np.float64)
     w = np.ascontiguousarray(gas.level_ob_w, dtype=np.float64)
     k.refs += [cum, ty, lo, rc, w]
+    opt = []
+    for name in ("scat_xi", "level_penning_prob", "level_penning_eV"):      # NEXT-3 extensions: optional
+        a = getattr(gas, name, None)
+        if a is None:
+            opt.append(None)
+        else:
+            a = np.ascontiguousarray(a, dtype=np.float64)
+            k.refs.append(a)
+            opt.append(_p(a).value)
     d = GasDesc(int(gas.n_bins), float(gas.e_max), int(cum.shape[1]), _p(cum).value, _p(ty).value, _p(lo).value,
-                _p(rc).value, _p(w).value, float(gas.nu_hat))
+                _p(rc).value, _p(w).value, float(gas.nu_hat), opt[0], opt[1], opt[2], float(getattr(gas, "kT_eV", 0.0)))
     return d, k
 
 
@@ -189,7 +200,7 @@ class RunResult:
     birth: np.ndarray           # [5, n]
     end: np.ndarray             # [8, n]
     per_avalanche: np.ndarray   # [Np, 3]
-    tallies_u64: np.ndarray     # [L+4]
+    tallies_u64: np.ndarray     # [L+5]: per level, null, real, overflow, steps, Penning transfers
     tallies_f64: np.ndarray     # [5]
     rc: int = 0
     n_rate_violations: int = 0  # banded runs: steps whose bin's total rate exceeded the band's rate (always 0)
@@ -209,7 +220,7 @@ def run(gas, field, primaries, seed=0, t_max=float("inf"), capacity=None, n_thre
     L = gas.n_levels
     ident = np.zeros(cap, dtype=np.uint64); av = np.zeros(cap, dtype=np.uint32); st = np.zeros(cap, dtype=np.int32)
     ns = np.zeros(cap, dtype=np.uint32); birth = np.zeros((5, cap)); end = np.zeros((8, cap))
-    pa = np.zeros((max(np_, 1), 3), dtype=np.uint64); tu = np.zeros(L + 5, dtype=np.uint64); tf = np.zeros(5)
+    pa = np.zeros((max(np_, 1), 3), dtype=np.uint64); tu = np.zeros(L + 6, dtype=np.uint64); tf = np.zeros(5)
     gd, _kg = gas_desc(gas)
     fd, _kf = field_desc(field)
     o = Outputs(cap, _p(ident), _p(av), _p(st), _p(ns), _p(birth), _p(end), _p(pa), _p(tu), _p(tf))
@@ -221,4 +232,4 @@ def run(gas, field, primaries, seed=0, t_max=float("inf"), capacity=None, n_thre
     if rc not in (0, -2):
         raise RuntimeError(lib().avmo_last_error().decode())
     n = n_out.value
-    return RunResult(n, ident[:n], av[:n], st[:n], ns[:n], birth[:, :n], end[:, :n], pa[:np_], tu[:L + 4], tf, rc, int(tu[L + 4]))
+    return RunResult(n, ident[:n], av[:n], st[:n], ns[:n], birth[:, :n], end[:, :n], pa[:np_], tu[:L + 5], tf, rc, int(tu[L + 5]))

@@ -38,6 +38,11 @@ class GasTable:
     level_ob_w: np.ndarray      # [n_levels] float64, eV
     nu_hat: float = 0.0         # <= 0: use max_b cum_rate[b, -1]
     names: list = field(default_factory=list)
+    # NEXT-3 extensions, all optional:
+    scat_xi: np.ndarray = None             # [n_bins, n_levels] forward-scattering parameter in (-1, 1); None = isotropic
+    level_penning_prob: np.ndarray = None  # [n_levels] Penning transfer probability of an excitation level
+    level_penning_eV: np.ndarray = None    # [n_levels] energy available to the Penning electron
+    kT_eV: float = 0.0                     # gas temperature; 0 = cold gas (R8)
 
     @property
     def n_levels(self) -> int:
