@@ -70,6 +70,13 @@ typedef struct {
   const double* level_recoil;     /* host [n_levels]: r = 2mM/(m+M)^2 (elastic) */
   const double* level_ob_w_eV;    /* host [n_levels]: Opal-Beaty w (ionisation) */
   double nu_hat;
+  /* NEXT-3 (DESIGN.md §3.6 readings X1-X3; PAPER.md:121 for Penning transfer, the feature the paper had to
+   * switch off).  All optional: NULL / 0 = the base model (isotropic deflection R9, no transfer, cold gas R8). */
+  const double* scat_xi;            /* host [n_bins][n_levels]: forward-scattering parameter xi in (-1, 1) of the bin and
+                                     * level: cos(theta) = (c0 + xi) / (1 + xi c0), c0 = 1 - 2 u3 (0 = isotropic) */
+  const double* level_penning_prob; /* host [n_levels]: probability that an excitation of the level ionises the admixture */
+  const double* level_penning_eV;   /* host [n_levels]: energy available to that electron (its energy is uniform in it) */
+  double kT_eV;                     /* gas temperature for elastic collisions (0.02526 eV at 293.15 K); 0 = cold gas */
 } avm_gas_desc;
 /* Bytes of device memory avm_gas_create needs for this table (0 on an invalid description). */
 size_t avm_gas_bytes(const avm_gas_desc*);
@@ -169,7 +176,7 @@ typedef struct {
   double* birth;                  /* [5][capacity]: x0, y0, z0, t0, e0; may be NULL */
   double* end;                    /* [8][capacity]: x1, y1, z1, t1, e1, kx, ky, kz */
   uint64_t* per_avalanche;        /* [n_primaries][3]: endpoints, ions (= endpoints - 1), negative ions; may be NULL */
-  uint64_t* tallies_u64;          /* [n_levels + 4]: per level, null, real, energy overflow, steps; may be NULL */
+  uint64_t* tallies_u64;          /* [n_levels + 5]: per level, null, real, energy overflow, steps, Penning transfers; may be NULL */
   double* tallies_f64;            /* [5]: sum dx, dy, dz over all flights, sum dt, sum energy loss; may be NULL */
 } avm_outputs;
 size_t avm_run_workspace_bytes(const avm_ctx*, int64_t capacity);

@@ -39,7 +39,9 @@ class AvmError(RuntimeError):
 class _GasDesc(C.Structure):
     _fields_ = [("n_bins", C.c_int32), ("e_max_eV", C.c_double), ("n_levels", C.c_int32),
                 ("cum_rate", C.c_void_p), ("level_type", C.c_void_p), ("level_loss_eV", C.c_void_p),
-                ("level_recoil", C.c_void_p), ("level_ob_w_eV", C.c_void_p), ("nu_hat", C.c_double)]
+                ("level_recoil", C.c_void_p), ("level_ob_w_eV", C.c_void_p), ("nu_hat", C.c_double),
+                ("scat_xi", C.c_void_p), ("level_penning_prob", C.c_void_p), ("level_penning_eV", C.c_void_p),
+                ("kT_eV", C.c_double)]
 
 
 class _Slab(C.Structure):
@@ -164,8 +166,11 @@ class Gas:
         w = np.ascontiguousarray(table.level_ob_w, dtype=np.float64)
         self.n_levels = int(cum.shape[1])
         self.n_bins = int(cum.shape[0])
+        opt = [None if getattr(table, k, None) is None else np.ascontiguousarray(getattr(table, k), dtype=np.float64)
+               for k in ("scat_xi", "level_penning_prob", "level_penning_eV")]              # NEXT-3 extensions (optional)
         d = _GasDesc(self.n_bins, float(table.e_max), self.n_levels, _hp(cum).value, _hp(ty).value, _hp(lo).value,
-                     _hp(rc).value, _hp(w).value, float(table.nu_hat))
+                     _hp(rc).value, _hp(w).value, float(table.nu_hat), *[None if a is None else _hp(a).value for a in opt],
+                     float(getattr(table, "kT_eV", 0.0)))
         nbytes = int(_lib.avm_gas_bytes(C.byref(d)))
         if nbytes == 0:
             raise AvmError(ERR_INVALID_ARG, "gas: invalid description")
@@ -368,7 +373,7 @@ class RunBuffers:
         self.birth = ctx.empty((5, cap), torch.float64)
         self.end = ctx.empty((8, cap), torch.float64)
         self.per_avalanche = ctx.empty((max(self.n_primaries, 1), 3), torch.int64)
-        self.tallies_u64 = ctx.empty(n_levels + 4, torch.int64)
+        self.tallies_u64 = ctx.empty(n_levels + 5, torch.int64)
         self.tallies_f64 = ctx.empty(5, torch.float64)
 
     def c_struct(self) -> _Outputs:
@@ -389,7 +394,7 @@ class HostBuffers:
         self.id = mk(cap, torch.int64); self.avalanche = mk(cap, torch.int32); self.status = mk(cap, torch.int32)
         self.n_steps = mk(cap, torch.int32); self.birth = mk((5, cap), torch.float64); self.end = mk((8, cap), torch.float64)
         self.per_avalanche = mk((max(self.n_primaries, 1), 3), torch.int64)
-        self.tallies_u64 = mk(n_levels + 4, torch.int64); self.tallies_f64 = mk(5, torch.float64)
+        self.tallies_u64 = mk(n_levels + 5, torch.int64); self.tallies_f64 = mk(5, torch.float64)
 
     def c_struct(self) -> _Outputs:
         p = lambda t: C.c_void_p(t.data_ptr())
@@ -407,7 +412,7 @@ class RunResult:
     birth: np.ndarray           # [5, n]
     end: np.ndarray             # [8, n]
     per_avalanche: np.ndarray   # [Np, 3]
-    tallies_u64: np.ndarray     # [L+4]
+    tallies_u64: np.ndarray     # [L+5]: per level, null, real, overflow, steps, Penning transfers
     tallies_f64: np.ndarray     # [5]
     rc: int = 0
 

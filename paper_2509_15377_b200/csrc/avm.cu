@@ -129,6 +129,7 @@ __global__ void publish_kernel(const RunCtl* ctl, const int L, unsigned long lon
       tallies_u64[L] = ctl->n_steps - ctl->n_real - ctl->n_term;  // null collisions
       tallies_u64[L + 1] = ctl->n_real;
       tallies_u64[L + 2] = ctl->n_overflow; tallies_u64[L + 3] = ctl->n_steps;
+      tallies_u64[L + 4] = ctl->n_penning;
     }
     if (tallies_f64) {
       for (int c = 0; c < 4; ++c) tallies_f64[c] = ctl->sum_d[c];
@@ -444,6 +445,14 @@ bool valid_gas(const avm_gas_desc* d, double* max_rate) {
     if (d->level_type[l] > 3) { g_err = "gas: bad level type"; return false; }
     if (d->level_type[l] == AVM_IONISATION && !(d->level_ob_w_eV[l] > 0)) { g_err = "gas: ionisation level needs w > 0"; return false; }
   }
+  if (d->scat_xi)
+    for (size_t i = 0; i < (size_t)d->n_bins * L; ++i)
+      if (!(d->scat_xi[i] > -1.0 && d->scat_xi[i] < 1.0)) { g_err = "gas: scat_xi outside (-1, 1)"; return false; }
+  if ((d->level_penning_prob != nullptr) != (d->level_penning_eV != nullptr)) { g_err = "gas: Penning probability and energy come together"; return false; }
+  if (d->level_penning_prob)
+    for (int l = 0; l < L; ++l)
+      if (!(d->level_penning_prob[l] >= 0.0 && d->level_penning_prob[l] <= 1.0) || !(d->level_penning_eV[l] >= 0.0)) { g_err = "gas: Penning parameters"; return false; }
+  if (!(d->kT_eV >= 0.0)) { g_err = "gas: kT < 0"; return false; }
   if (!(mx > 0.0) && !(d->nu_hat > 0.0)) { g_err = "gas: all rates are zero"; return false; }
   if (d->nu_hat > 0.0 && d->nu_hat < mx) { g_err = "gas: nu_hat below the maximum total rate"; return false; }
   if (max_rate) *max_rate = mx;
@@ -452,12 +461,12 @@ bool valid_gas(const avm_gas_desc* d, double* max_rate) {
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
-struct GasLayout { size_t nu_tot, head, tab, cum, loss, recoil, w, type, band, total; };
+struct GasLayout { size_t nu_tot, head, tab, cum, loss, recoil, w, type, band, pen_p, pen_e, xi, total; };
 constexpr int kBandClasses = 25;                 // N2: class edges 250 V/cm x 2^(j/2), j = 0 .. 24
 int band_shift(int nb) { int s = 0; while ((nb >> (s + 1)) >= 256) ++s; return s; }   // N1: the most bins per band that leaves >= 256 bands
 int band_count(int nb) { const int s = band_shift(nb); return (nb + (1 << s) - 1) >> s; }
 int padded_levels(int L) { return (L + 1) & ~1; }
-GasLayout gas_layout(int nb, int L) {
+GasLayout gas_layout(int nb, int L, bool with_xi) {
   GasLayout g;
   const int Lp = padded_levels(L);
   size_t off = 0;
@@ -470,6 +479,9 @@ GasLayout gas_layout(int nb, int L) {
   g.w = off;      off += sizeof(double) * AVM_MAX_LEVELS;
   g.type = off;   off = align_up(off + AVM_MAX_LEVELS, 256);
   g.band = off;   off = align_up(off + 32 * (size_t)(kBandClasses + 1) * band_count(nb), 256);
+  g.pen_p = off;  off += sizeof(double) * AVM_MAX_LEVELS;
+  g.pen_e = off;  off = align_up(off + sizeof(double) * AVM_MAX_LEVELS, 256);
+  g.xi = off;     if (with_xi) off = align_up(off + sizeof(double) * (size_t)nb * L, 256);
   g.total = off;
   return g;
 }
@@ -586,7 +598,7 @@ int32_t avm_ctx_sm_count(const avm_ctx* c) { return c ? c->sm_count : 0; }
 
 size_t avm_gas_bytes(const avm_gas_desc* d) {
   if (!d || d->n_bins < 1 || d->n_levels < 1 || d->n_levels > AVM_MAX_LEVELS) return 0;
-  return gas_layout(d->n_bins, d->n_levels).total;
+  return gas_layout(d->n_bins, d->n_levels, d->scat_xi != nullptr).total;
 }
 
 int32_t avm_gas_create(avm_ctx* ctx, const avm_gas_desc* d, void* dev_buf, size_t dev_bytes, avm_gas** out) {
@@ -595,7 +607,7 @@ int32_t avm_gas_create(avm_ctx* ctx, const avm_gas_desc* d, void* dev_buf, size_
   double mx = 0.0;
   if (!valid_gas(d, &mx)) return AVM_ERR_INVALID_ARG;
   const int nb = d->n_bins, L = d->n_levels;
-  const GasLayout lay = gas_layout(nb, L);
+  const GasLayout lay = gas_layout(nb, L, d->scat_xi != nullptr);
   if (!dev_buf || dev_bytes < lay.total || ((uintptr_t)dev_buf & 255u)) return fail(AVM_ERR_INVALID_ARG, "gas_create: device buffer null, too small or not 256-byte aligned");
   std::vector<unsigned char> h(lay.total, 0);
   double* nu_tot = (double*)(h.data() + lay.nu_tot);
@@ -648,6 +660,11 @@ int32_t avm_gas_create(avm_ctx* ctx, const avm_gas_desc* d, void* dev_buf, size_
   std::memcpy(h.data() + lay.recoil, d->level_recoil, sizeof(double) * L);
   std::memcpy(h.data() + lay.w, d->level_ob_w_eV, sizeof(double) * L);
   std::memcpy(h.data() + lay.type, d->level_type, L);
+  if (d->level_penning_prob) {
+    std::memcpy(h.data() + lay.pen_p, d->level_penning_prob, sizeof(double) * L);
+    std::memcpy(h.data() + lay.pen_e, d->level_penning_eV, sizeof(double) * L);
+  }
+  if (d->scat_xi) std::memcpy(h.data() + lay.xi, d->scat_xi, sizeof(double) * (size_t)nb * L);
   AVM_CUDA(cudaSetDevice(ctx->device));
   AVM_CUDA(cudaMemcpyAsync(dev_buf, h.data(), lay.total, cudaMemcpyHostToDevice, ctx->stream));
   AVM_CUDA(cudaStreamSynchronize(ctx->stream));
@@ -671,6 +688,11 @@ int32_t avm_gas_create(avm_ctx* ctx, const avm_gas_desc* d, void* dev_buf, size_
   g->d.recoil = (const double*)(base + lay.recoil);
   g->d.w = (const double*)(base + lay.w);
   g->d.type = (const uint8_t*)(base + lay.type);
+  g->d.pen_p = (const double*)(base + lay.pen_p);
+  g->d.pen_e = (const double*)(base + lay.pen_e);
+  g->d.xi = d->scat_xi ? (const double*)(base + lay.xi) : nullptr;
+  g->d.kT = d->kT_eV;
+  g->d.ext = (d->scat_xi ? 1 : 0) | (d->kT_eV > 0.0 ? 2 : 0);
   g->d.bshift = bands.shift; g->d.bK = bands.K; g->d.bJ = bands.J;
   g->d.a0sq = bands.a2[0]; g->d.inv_a0sq = 1.0 / bands.a2[0];
   g->d.band = (const double2*)(base + lay.band);
@@ -952,7 +974,7 @@ int32_t avm_fetch(avm_ctx* ctx, const avm_outputs* dev, int64_t n, int64_t np, i
       AVM_CUDA(cudaMemcpy2DAsync(host->end, sizeof(double) * host->capacity, dev->end, sizeof(double) * dev->capacity, sizeof(double) * n, 8, cudaMemcpyDeviceToHost, st));
   }
   if (host->per_avalanche && dev->per_avalanche && np > 0) AVM_D2H(host->per_avalanche, dev->per_avalanche, sizeof(uint64_t) * 3 * np);
-  if (host->tallies_u64 && dev->tallies_u64 && n_levels > 0) AVM_D2H(host->tallies_u64, dev->tallies_u64, sizeof(uint64_t) * (n_levels + 4));
+  if (host->tallies_u64 && dev->tallies_u64 && n_levels > 0) AVM_D2H(host->tallies_u64, dev->tallies_u64, sizeof(uint64_t) * (n_levels + 5));
   if (host->tallies_f64 && dev->tallies_f64) AVM_D2H(host->tallies_f64, dev->tallies_f64, sizeof(double) * 5);
 #undef AVM_D2H
   AVM_CUDA(cudaStreamSynchronize(st));

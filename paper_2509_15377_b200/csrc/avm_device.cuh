@@ -51,6 +51,12 @@ struct DevGas {
   int bshift, bK, bJ;
   double a0sq, inv_a0sq;  // squared edge of class 0, (kappa 250 V/cm)^2; the edge of class j is a0sq 2^j
   const double2* band;    // [bJ + 1][bK][2]: (1 / nu, dtmax), (nu, floor(nu / nu_hat 2^32) as the low word's bits)
+  // NEXT-3: X1 forward-scattering table, X2 Penning parameters per level, X3 gas temperature
+  const double* xi;       // [nb][L] or null (isotropic)
+  const double* pen_p;    // [AVM_MAX_LEVELS] transfer probability (0 where none)
+  const double* pen_e;    // [AVM_MAX_LEVELS] energy available to the Penning electron
+  double kT;              // 0 = cold gas
+  int ext;                // bit 0: xi given, bit 1: kT > 0 — the speculative elastic collision of the time-parallel batches is off
 };
 
 struct DevSlab {
@@ -355,7 +361,7 @@ __device__ __forceinline__ void flight(const DevField& f, double Ex, double Ey, 
 struct Child { double e, u6, u7; };   // secondary: energy and the two uniforms of its isotropic direction
 
 // Level parameters as the kernels keep them in shared memory: two 16-byte loads per collision.
-struct __align__(16) LevelPar { double loss, recoil, w; int type, pad; };
+struct __align__(16) LevelPar { double loss, recoil, w; int type, pad; double pen_p, pen_e; };
 
 __device__ __forceinline__ void stage_levels(const DevGas& g, LevelPar* s_lv) {
   for (int l = threadIdx.x; l < AVM_MAX_LEVELS; l += blockDim.x) {
@@ -363,6 +369,7 @@ __device__ __forceinline__ void stage_levels(const DevGas& g, LevelPar* s_lv) {
     LevelPar p;
     p.loss = in ? g.loss[l] : 0.0; p.recoil = in ? g.recoil[l] : 0.0; p.w = in ? g.w[l] : 1.0;
     p.type = in ? g.type[l] : 0; p.pad = 0;
+    p.pen_p = in ? g.pen_p[l] : 0.0; p.pen_e = in ? g.pen_e[l] : 0.0;
     s_lv[l] = p;
   }
 }
@@ -646,6 +653,12 @@ __device__ __forceinline__ int collision_step(const DevGas& g, const LevelPar* _
   status = 0; spawn = false; loss = 0.0;
   if (par.type == AVM_ATTACHMENT) { status = AVM_ATTACHED; return l; }         // S9a
   if (!have_d) d = deflection_draws(K, id, n - 1u);                            // S9b
+  if (g.xi) {                                     // X1: cos(theta) = (c0 + xi) / (1 + xi c0), sin(theta) cancellation-free
+    const double xi = __ldg(g.xi + (size_t)p.bin * g.L + l);
+    const double den = 1.0 + xi * d.ct;
+    d.st = d.st * sqrt(1.0 - xi * xi) / den;
+    d.ct = (d.ct + xi) / den;
+  }
   double s2 = vx * vx + vy * vy + vz * vz;
   if (!(s2 >= 1e-280)) {                          // v' = 0 (never in practice): direction +z, energy at the floor
     vx = 0.0; vy = 0.0; vz = kC2 * 1e-5; s2 = vz * vz;
@@ -653,6 +666,29 @@ __device__ __forceinline__ int collision_step(const DevGas& g, const LevelPar* _
   double e1 = s2 * kInvC2Sq;
   if (e1 < kEpsFloor) e1 = kEpsFloor;
   double e2;                                                                    // S9c
+  if (par.type == AVM_ELASTIC && g.kT > 0.0 && par.recoil > 0.0) {
+    // X3: the atom moves with velocity V (normal components, sigma = c2 sqrt(kT r / 4), Box-Muller from blocks 2 and 3);
+    // the cold-gas collision acts on the relative velocity w = v' - V, then V is added back.  Rare path: library math.
+    const U4 r2 = philox(K, id, n - 1u, 2u);
+    const U4 r3 = philox(K, id, n - 1u, 3u);
+    const double u5 = to_unit(r2.w0, r2.w1), u6 = to_unit(r2.w2, r2.w3), u7 = to_unit(r3.w0, r3.w1), u8 = to_unit(r3.w2, r3.w3);
+    const double sigma = kC2 * sqrt(g.kT * par.recoil * 0.25);
+    const double ra = sqrt(-2.0 * log(u5)), rb = sqrt(-2.0 * log(u7));
+    double s6, c6, s8, c8;
+    sincos_2pi(u6, s6, c6);
+    sincos_2pi(u8, s8, c8);
+    const double Vx = sigma * ra * c6, Vy = sigma * ra * s6, Vz = sigma * rb * c8;
+    double wx = vx - Vx, wy = vy - Vy, wz = vz - Vz;
+    double w2 = wx * wx + wy * wy + wz * wz;
+    if (!(w2 >= 1e-280)) { wx = 0.0; wy = 0.0; wz = kC2 * 1e-5; w2 = wz * wz; }
+    double ew = w2 * kInvC2Sq;
+    if (ew < kEpsFloor) ew = kEpsFloor;
+    const double e2w = ew * (1.0 - par.recoil * (1.0 - d.ct));
+    rotate_scale(d, w2, e2w, wx, wy, wz);
+    vx = wx + Vx; vy = wy + Vy; vz = wz + Vz;
+    loss = e1 - fmax((vx * vx + vy * vy + vz * vz) * kInvC2Sq, kEpsFloor);
+    return l;
+  }
   if (par.type == AVM_ELASTIC) {
     e2 = e1 * (1.0 - par.recoil * (1.0 - d.ct));
     loss = e1 - e2;
@@ -660,6 +696,16 @@ __device__ __forceinline__ int collision_step(const DevGas& g, const LevelPar* _
     e2 = e1 - par.loss;
     if (!(e2 > kEpsFloor)) e2 = kEpsFloor;
     loss = e1 - e2;
+    if (par.pen_p > 0.0) {                        // X2: Penning transfer — one more electron with probability pen_p
+      const U4 r2 = philox(K, id, n - 1u, 2u);
+      if (to_unit(r2.w0, r2.w1) < par.pen_p) {
+        const U4 r3 = philox(K, id, n - 1u, 3u);
+        ch.u6 = to_unit(r2.w2, r2.w3);
+        ch.u7 = to_unit(r3.w0, r3.w1);
+        ch.e = fmax(to_unit(r3.w2, r3.w3) * par.pen_e, kEpsFloor);
+        spawn = true;
+      }
+    }
   } else {   // ionisation: Opal-Peterson-Beaty sharing (R10)
     const U4 r2 = philox(K, id, n - 1u, 2u);
     const U4 r3 = philox(K, id, n - 1u, 3u);

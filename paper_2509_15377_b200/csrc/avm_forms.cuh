@@ -12,7 +12,7 @@
 namespace avm {
 
 // Per-thread tallies of the hot loop (warp-reduced at the end of the launch); null counts are derived (finalize_kernel).
-struct Tally { uint32_t real = 0u, l0 = 0u, over = 0u; double loss = 0.0; };
+struct Tally { uint32_t real = 0u, l0 = 0u, over = 0u, pen = 0u; double loss = 0.0; };
 
 // Per-warp exchange area (shared memory).
 struct WarpBuf {
@@ -160,7 +160,7 @@ __device__ __forceinline__ int tp_batch(const DevGas& g, const DevField& f, cons
       const LevelPar par = s_lv[r == 1 ? 1 : 0];
       fvx = vx; fvy = vy; fvz = vz;
       floss = elastic_collision(par.recoil, dj, s2, fvx, fvy, fvz);
-      fast = ok & ((r == 0) | (r == 1)) & (par.type == AVM_ELASTIC) & (s2 >= 1e-280);
+      fast = ok & ((r == 0) | (r == 1)) & (par.type == AVM_ELASTIC) & (s2 >= 1e-280) & (g.ext == 0);
       if (!ok) {
         b = uniform_exit_status(f, t_max, x, y, z, t);
       } else if (r == -2 || r == 2) {

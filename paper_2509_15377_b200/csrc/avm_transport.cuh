@@ -58,7 +58,7 @@ struct RunCtl {
   unsigned int q_head;           // tickets handed out beyond the static ones (own 128-byte line)
   unsigned int dropped;          // children that did not fit in `capacity`
   unsigned char pad1[120];
-  unsigned long long n_real, n_overflow;
+  unsigned long long n_real, n_overflow, n_penning;
   unsigned long long n_steps;    // sum over electrons of their collision index n (finalize_kernel)
   unsigned long long n_term;     // electrons whose last step ended before the null/real decision (status 1-4, 6, 7)
   unsigned long long level[AVM_MAX_LEVELS];
@@ -202,6 +202,7 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
         if (l == 0) ++tl.l0;
         else if (l > 1) atomicAdd(&s_hist[l], 1u);
         tl.loss += loss;
+        if (spawn && s_lv[l].type == AVM_EXCITATION) ++tl.pen;       // X2: a Penning transfer
       }
     }
     const unsigned sm = __ballot_sync(mask, spawn);
@@ -356,17 +357,19 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
   }
   if (TALLY) {
     // warp reduce the per-thread counters, one atomic per warp; rare-level histogram per CTA
-    unsigned long long v0 = tl.real, v1 = tl.l0, v3 = tl.over;
+    unsigned long long v0 = tl.real, v1 = tl.l0, v3 = tl.over, v5 = tl.pen;
     double v4 = tl.loss;
 #pragma unroll
     for (int o2 = 16; o2 > 0; o2 >>= 1) {
       v0 += __shfl_down_sync(0xFFFFFFFFu, v0, o2); v1 += __shfl_down_sync(0xFFFFFFFFu, v1, o2);
       v3 += __shfl_down_sync(0xFFFFFFFFu, v3, o2); v4 += __shfl_down_sync(0xFFFFFFFFu, v4, o2);
+      v5 += __shfl_down_sync(0xFFFFFFFFu, v5, o2);
     }
     if (lane == 0u) {
       if (v0) atomicAdd(&ctl->n_real, v0);
       if (v1) atomicAdd(&ctl->level[0], v1);
       if (v3) atomicAdd(&ctl->n_overflow, v3);
+      if (v5) atomicAdd(&ctl->n_penning, v5);
       if (v4 != 0.0) atomicAdd(&ctl->sum_loss, v4);
     }
     __syncthreads();
