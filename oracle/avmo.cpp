@@ -86,6 +86,7 @@ struct Electron {
   uint32_t n, aval;
   int32_t status;
   double birth[5];
+  bool primary = false;
 };
 
 struct Tally {
@@ -272,7 +273,24 @@ struct StepOut {
 };
 
 // One step S0-S9 for an in-domain, active electron.
-void step(const Gas& g, const avmo_field_desc* f, uint64_t seed, double t_max, bool banded, Electron& el, StepOut& so, Tally* tl) {
+// W1: the weighting field at r: E_w, zero outside its description (mask and B ignored).
+void weighting_at(const avmo_field_desc* wf, double x, double y, double z, double Ew[3]) {
+  double m;
+  Ew[0] = Ew[1] = Ew[2] = 0.0;
+  double e[3];
+  if (field_at(wf, x, y, z, e, m) >= 0) { Ew[0] = e[0]; Ew[1] = e[1]; Ew[2] = e[2]; }
+}
+// W2: charge q moved from r0 to r1 in a step that starts at time t: q E_w(at) . (r1 - r0) into the bin of t.
+void induce(const avmo_signal* sg, double* acc, double q, const double at[3], const double r0[3], const double r1[3], double t) {
+  double Ew[3];
+  weighting_at(sg->weighting, at[0], at[1], at[2], Ew);
+  const double dq = q * (Ew[0] * (r1[0] - r0[0]) + Ew[1] * (r1[1] - r0[1]) + Ew[2] * (r1[2] - r0[2]));
+  const double sb = std::floor((t - sg->t0) / sg->dt_bin);
+  if (sb >= 0.0 && sb < (double)sg->n_bins) acc[(int)sb] += dq;
+}
+
+void step(const Gas& g, const avmo_field_desc* f, uint64_t seed, double t_max, bool banded, Electron& el, StepOut& so, Tally* tl,
+          const avmo_signal* sgn = nullptr, double* sig_acc = nullptr) {
   so.event = -2; so.bin = -1; so.child = false;
   // S0: field at r (held constant during the flight); B is a run constant.  R3: re-evaluated every step.
   double E[3], m;
@@ -337,6 +355,7 @@ void step(const Gas& g, const avmo_field_desc* f, uint64_t seed, double t_max, b
       r1[i] = r0[i] + vpar[i] * dt + 0.5 * apar[i] * dt * dt + vd[i] * dt + (w0[i] * sn + bxw[i] * vers) / omega;
     }
   }
+  if (sgn) induce(sgn, sig_acc, -1.0, r0, r0, r1, el.t);   // W2: every flight, the last one of an electron included
   // S4: new energy, direction, time, counter
   const double s2 = v1[0] * v1[0] + v1[1] * v1[1] + v1[2] * v1[2];
   const double e1 = std::max(s2 * INV_C2SQ, EPS_FLOOR);
@@ -435,7 +454,7 @@ void step(const Gas& g, const avmo_field_desc* f, uint64_t seed, double t_max, b
         uint32_t wd[4];
         philox_block(seed, el.id, n_s, BLOCK_CHILD_ID, wd);
         c.id = (uint64_t)wd[0] + ((uint64_t)wd[1] << 32);
-        c.n = 0; c.aval = el.aval; c.status = AVMO_ACTIVE;
+        c.n = 0; c.aval = el.aval; c.status = AVMO_ACTIVE; c.primary = false;
         c.birth[0] = c.x; c.birth[1] = c.y; c.birth[2] = c.z; c.birth[3] = c.t; c.birth[4] = c.e;
         so.child = true;
         if (tl) tl->n_penning++;
@@ -458,7 +477,7 @@ void step(const Gas& g, const avmo_field_desc* f, uint64_t seed, double t_max, b
     uint32_t wd[4];
     philox_block(seed, el.id, n_s, BLOCK_CHILD_ID, wd);             // R16: schedule-independent child id
     c.id = (uint64_t)wd[0] + ((uint64_t)wd[1] << 32);
-    c.n = 0; c.aval = el.aval; c.status = AVMO_ACTIVE;
+    c.n = 0; c.aval = el.aval; c.status = AVMO_ACTIVE; c.primary = false;
     c.birth[0] = c.x; c.birth[1] = c.y; c.birth[2] = c.z; c.birth[3] = c.t; c.birth[4] = c.e;
     so.child = true;
     if (tl) tl->sloss += e1 - e2 - c.e;
@@ -490,7 +509,8 @@ struct Record { Electron el; };
 // The avalanche driver: transport until status != 0, push newly created electrons, repeat.
 // Serial: one electron at a time from a stack.  Order is irrelevant because draws are keyed by (id, n).
 void run_range(const Gas& g, const avmo_field_desc* f, const double* prim, int64_t p0, int64_t p1, uint64_t seed,
-               uint64_t id_offset, double t_max, bool banded, std::vector<Electron>& done, Tally& tl) {
+               uint64_t id_offset, double t_max, bool banded, std::vector<Electron>& done, Tally& tl,
+               const avmo_signal* sg = nullptr, double* sig_acc = nullptr) {
   std::vector<Electron> stack;
   StepOut so;
   for (int64_t p = p0; p < p1; ++p) {
@@ -499,7 +519,7 @@ void run_range(const Gas& g, const avmo_field_desc* f, const double* prim, int64
     el.x = q[0]; el.y = q[1]; el.z = q[2]; el.t = q[3]; el.e = std::max(q[4], EPS_FLOOR);
     double nk = std::sqrt(q[5] * q[5] + q[6] * q[6] + q[7] * q[7]);
     if (!(nk > 0)) { el.kx = 0; el.ky = 0; el.kz = 1; } else { el.kx = q[5] / nk; el.ky = q[6] / nk; el.kz = q[7] / nk; }
-    el.id = id_offset + (uint64_t)p; el.n = 0; el.aval = (uint32_t)p; el.status = AVMO_ACTIVE;
+    el.id = id_offset + (uint64_t)p; el.n = 0; el.aval = (uint32_t)p; el.status = AVMO_ACTIVE; el.primary = true;
     el.birth[0] = el.x; el.birth[1] = el.y; el.birth[2] = el.z; el.birth[3] = el.t; el.birth[4] = el.e;
     // a-1: reject out-of-domain primaries (status set, endpoint = birth point)
     double E[3], m;
@@ -512,7 +532,7 @@ void run_range(const Gas& g, const avmo_field_desc* f, const double* prim, int64
       Electron cur = stack.back();
       stack.pop_back();
       while (cur.status == AVMO_ACTIVE) {
-        step(g, f, seed, t_max, banded, cur, so, &tl);
+        step(g, f, seed, t_max, banded, cur, so, &tl, sg, sig_acc);
         if (so.child) stack.push_back(so.c);
       }
       done.push_back(cur);
@@ -580,6 +600,57 @@ int32_t avmo_step_batch(const avmo_gas_desc* gd, const avmo_field_desc* f, uint6
   return AVMO_OK;
 }
 
+int32_t avmo_ion_drift(const avmo_field_desc* f, const avmo_signal* sg, const avmo_ion_opts* io, int64_t n, int64_t n_prim,
+                       int64_t ldb, const double* birth, int64_t lde, const double* end, const int32_t* status,
+                       double* ion_end, int32_t* ion_status, uint32_t* ion_steps) {
+  if (!check_field(f) || !io || n < 0 || !birth || !end || !status || !ion_end || !ion_status || !ion_steps) { g_err = "ion_drift: null"; return AVMO_ERR_INVALID_ARG; }
+  if (!(io->step_cm > 0) || !(io->mobility_pos > 0) || !(io->mobility_neg > 0) || io->max_steps < 1) { g_err = "ion_drift: options"; return AVMO_ERR_INVALID_ARG; }
+  if (sg && (!sg->weighting || !check_field(sg->weighting) || !(sg->dt_bin > 0) || sg->n_bins < 1 || !sg->signal)) { g_err = "ion_drift: signal description"; return AVMO_ERR_INVALID_ARG; }
+  const int64_t N = 2 * n;
+  for (int64_t i = 0; i < N; ++i) {
+    const int64_t s = i < n ? i : i - n;
+    const bool pos = i < n;
+    ion_status[i] = -1; ion_steps[i] = 0;
+    for (int c = 0; c < 4; ++c) ion_end[c * N + i] = 0.0;
+    if (pos ? s < n_prim : status[s] != AVMO_ATTACHED) continue;           // W3: which ions exist
+    double r[3], t;
+    if (pos) { r[0] = birth[s]; r[1] = birth[ldb + s]; r[2] = birth[2 * ldb + s]; t = birth[3 * ldb + s]; }
+    else { r[0] = end[s]; r[1] = end[lde + s]; r[2] = end[2 * lde + s]; t = end[3 * lde + s]; }
+    const double q = pos ? 1.0 : -1.0, mu = pos ? io->mobility_pos : io->mobility_neg;
+    int st = AVMO_ACTIVE;
+    uint32_t ns = 0;
+    double E[3], m;
+    int si = field_at(f, r[0], r[1], r[2], E, m);
+    if (si < 0) st = -si; else if (m < 0.5) st = AVMO_MATERIAL;
+    while (st == AVMO_ACTIVE) {                                              // W4: explicit midpoint, fixed step length
+      if (ns >= (uint32_t)io->max_steps) { st = AVMO_STEP_LIMIT; break; }
+      const double k1[3] = {q * mu * E[0], q * mu * E[1], q * mu * E[2]};
+      const double n1 = std::sqrt(k1[0] * k1[0] + k1[1] * k1[1] + k1[2] * k1[2]);
+      if (!(n1 > 0.0)) { st = AVMO_STEP_LIMIT; break; }
+      const double hh = 0.5 * io->step_cm / n1;
+      const double rm[3] = {r[0] + hh * k1[0], r[1] + hh * k1[1], r[2] + hh * k1[2]};
+      double Em[3], mm;
+      if (field_at(f, rm[0], rm[1], rm[2], Em, mm) < 0) { Em[0] = E[0]; Em[1] = E[1]; Em[2] = E[2]; }   // midpoint outside: Euler step
+      const double k2[3] = {q * mu * Em[0], q * mu * Em[1], q * mu * Em[2]};
+      const double n2 = std::sqrt(k2[0] * k2[0] + k2[1] * k2[1] + k2[2] * k2[2]);
+      if (!(n2 > 0.0)) { st = AVMO_STEP_LIMIT; break; }
+      const double h2 = io->step_cm / n2;
+      const double r1[3] = {r[0] + h2 * k2[0], r[1] + h2 * k2[1], r[2] + h2 * k2[2]};
+      if (sg) induce(sg, sg->signal, q, rm, r, r1, t);
+      r[0] = r1[0]; r[1] = r1[1]; r[2] = r1[2];
+      t = t + h2;
+      ++ns;
+      si = field_at(f, r[0], r[1], r[2], E, m);
+      if (si < 0) st = -si;
+      else if (m < 0.5) st = AVMO_MATERIAL;
+      else if (t > io->t_max) st = AVMO_TIME_LIMIT;
+    }
+    ion_end[i] = r[0]; ion_end[N + i] = r[1]; ion_end[2 * N + i] = r[2]; ion_end[3 * N + i] = t;
+    ion_status[i] = st; ion_steps[i] = ns;
+  }
+  return AVMO_OK;
+}
+
 int32_t avmo_run(const avmo_gas_desc* gd, const avmo_field_desc* f, const double* prim, int64_t np,
                  const avmo_run_opts* opts, avmo_outputs* o, int64_t* n_out) {
   Gas g;
@@ -592,24 +663,33 @@ int32_t avmo_run(const avmo_gas_desc* gd, const avmo_field_desc* f, const double
   std::vector<std::vector<Electron>> done(nt);
   std::vector<Tally> tl(nt);
   for (auto& t : tl) t.level.assign(g.L, 0);
+  const avmo_signal* sg = opts->signal;
+  if (sg && (!sg->weighting || !check_field(sg->weighting) || !(sg->dt_bin > 0) || sg->n_bins < 1 || !sg->signal)) { g_err = "run: signal description"; return AVMO_ERR_INVALID_ARG; }
+  std::vector<std::vector<double>> sacc(nt);
+  if (sg) for (auto& a : sacc) a.assign(sg->n_bins, 0.0);
   if (nt == 1) {
-    run_range(g, f, prim, 0, np, opts->seed, opts->id_offset, opts->t_max, banded, done[0], tl[0]);
+    run_range(g, f, prim, 0, np, opts->seed, opts->id_offset, opts->t_max, banded, done[0], tl[0], sg, sg ? sacc[0].data() : nullptr);
   } else {                       // timed multi-core baseline only: disjoint primary ranges, identical results
     std::vector<std::thread> th;
     for (int t = 0; t < nt; ++t) {
       int64_t p0 = np * t / nt, p1 = np * (t + 1) / nt;
-      th.emplace_back([&, t, p0, p1] { run_range(g, f, prim, p0, p1, opts->seed, opts->id_offset, opts->t_max, banded, done[t], tl[t]); });
+      th.emplace_back([&, t, p0, p1] { run_range(g, f, prim, p0, p1, opts->seed, opts->id_offset, opts->t_max, banded, done[t], tl[t], sg, sg ? sacc[t].data() : nullptr); });
     }
     for (auto& x : th) x.join();
   }
+  if (sg) for (auto& a : sacc) for (int i = 0; i < sg->n_bins; ++i) sg->signal[i] += a[i];
   // outputs
   int64_t total = 0;
   for (auto& d : done) total += (int64_t)d.size();
   const int64_t cap = o->capacity;
   if (o->per_avalanche) std::memset(o->per_avalanche, 0, sizeof(uint64_t) * 3 * (size_t)np);
+  // entries in creation order as far as it is defined: the primaries first, in primary order (threads own ascending
+  // ranges), then the secondaries (order unspecified; compare after sorting by id, R17)
   int64_t w = 0;
+  for (int pass = 0; pass < 2; ++pass)
   for (auto& d : done)
     for (auto& el : d) {
+      if (el.primary != (pass == 0)) continue;
       if (o->per_avalanche) {                 // a-12 / C11: ions = ionisations = endpoints - 1 per avalanche
         o->per_avalanche[3 * (size_t)el.aval + 0]++;
         if (el.status == AVMO_ATTACHED) o->per_avalanche[3 * (size_t)el.aval + 2]++;

@@ -60,8 +60,27 @@ typedef struct { const avmo_slab* slabs; int32_t n_slabs; double B[3]; double xy
  * electron's energy band and of the flight's acceleration class instead of the global maximum; flights longer than the
  * band's validity time are cut and count as null collisions.  Same physics, fewer null steps, other random streams. */
 enum { AVMO_BANDED = 1u };
+/* NEXT-4 (DESIGN.md §3.7 readings W1-W4): induced-signal accumulation (Shockley-Ramo).  weighting = the
+ * weighting field E_w [1/cm] of the read-out electrode as a field description (mask and B ignored; outside it E_w = 0).
+ * Every flight r -> r' that starts at time t adds q E_w(r) . (r' - r), q = -1, to signal[floor((t - t0) / dt_bin)] (flights
+ * starting outside the bins are dropped).  signal: [n_bins] induced charge per bin in units of e, ADDED to. */
+typedef struct { const avmo_field_desc* weighting; double t0, dt_bin; int32_t n_bins; double* signal; } avmo_signal;
 /* id_offset: primary p gets electron id id_offset + p (shards of one job use disjoint id ranges); avalanche stays p. */
-typedef struct { uint64_t seed; double t_max; int32_t n_threads; uint64_t id_offset; uint32_t flags; } avmo_run_opts;
+typedef struct { uint64_t seed; double t_max; int32_t n_threads; uint64_t id_offset; uint32_t flags;
+                 const avmo_signal* signal; /* NULL: none */ } avmo_run_opts;
+
+/* Ion drift (W3, W4): every electron s >= n_primaries left a positive ion at its birth point, every attached electron
+ * (status 5) a negative ion at its endpoint.  Ion i = s (positive) or n + s (negative) of 2 n entries; status -1 = no such
+ * ion.  An ion of charge q moves with v = q mu E(r) (mu: mobility [cm^2 / (V ns)], constant), integrated by the explicit
+ * midpoint rule in steps of fixed LENGTH step_cm: k1 = v(r), r_m = r + (step/2) k1/|k1|, k2 = v(r_m), r' = r + step k2/|k2|,
+ * dt = step / |k2|; it stops at the first sampled point outside the domain (status 1-3), inside material (4), after t_max
+ * (6), after max_steps or where the field vanishes (7).  With a signal, each step adds q E_w(r_m) . (r' - r) to the bin of
+ * the step's start time.  ion_end: [4][2n] x, y, z, t. */
+typedef struct { double mobility_pos, mobility_neg, step_cm, t_max; int32_t max_steps; } avmo_ion_opts;
+int32_t avmo_ion_drift(const avmo_field_desc* field, const avmo_signal* signal, const avmo_ion_opts* opts, int64_t n,
+                       int64_t n_primaries, int64_t ld_birth, const double* birth /*[5][ld]*/, int64_t ld_end,
+                       const double* end /*[8][ld]*/, const int32_t* status, double* ion_end, int32_t* ion_status,
+                       uint32_t* ion_steps);
 
 typedef struct {
   int64_t capacity;

@@ -48,9 +48,19 @@ class FieldDescC(C.Structure):
                 ("xy_lo", C.c_double * 2), ("xy_hi", C.c_double * 2)]
 
 
+class SignalC(C.Structure):
+    _fields_ = [("weighting", C.POINTER(FieldDescC)), ("t0", C.c_double), ("dt_bin", C.c_double), ("n_bins", C.c_int32),
+                ("signal", C.c_void_p)]
+
+
+class IonOpts(C.Structure):
+    _fields_ = [("mobility_pos", C.c_double), ("mobility_neg", C.c_double), ("step_cm", C.c_double), ("t_max", C.c_double),
+                ("max_steps", C.c_int32)]
+
+
 class RunOpts(C.Structure):
     _fields_ = [("seed", C.c_uint64), ("t_max", C.c_double), ("n_threads", C.c_int32), ("id_offset", C.c_uint64),
-                ("flags", C.c_uint32)]
+                ("flags", C.c_uint32), ("signal", C.POINTER(SignalC))]
 
 
 BANDED = 1
@@ -72,6 +82,7 @@ def lib():
         _lib.avmo_step_batch.restype = C.c_int32
         _lib.avmo_field_eval.restype = C.c_int32
         _lib.avmo_majorant.restype = C.c_int32
+        _lib.avmo_ion_drift.restype = C.c_int32
     return _lib
 
 
@@ -204,16 +215,25 @@ class RunResult:
     tallies_f64: np.ndarray     # [5]
     rc: int = 0
     n_rate_violations: int = 0  # banded runs: steps whose bin's total rate exceeded the band's rate (always 0)
+    signal: np.ndarray = None   # induced charge per time bin [e] when a signal description was given
 
     def sorted_by_id(self):
         o = np.argsort(self.id, kind="stable")
         return RunResult(self.n, self.id[o], self.avalanche[o], self.status[o], self.n_steps[o], self.birth[:, o],
                          self.end[:, o], self.per_avalanche, self.tallies_u64, self.tallies_f64, self.rc,
-                         self.n_rate_violations)
+                         self.n_rate_violations, self.signal)
+
+
+def _signal_c(weighting, t0, dt_bin, signal):
+    wd, kw = field_desc(weighting)
+    s = SignalC(C.pointer(wd), float(t0), float(dt_bin), int(signal.shape[0]), _p(signal).value)
+    return s, (wd, kw)
 
 
 def run(gas, field, primaries, seed=0, t_max=float("inf"), capacity=None, n_threads=1, allow_overflow=False,
-        id_offset=0, flags=0) -> RunResult:
+        id_offset=0, flags=0, signal=None) -> RunResult:
+    """signal: None or (weighting FieldDesc, t0, dt_bin, n_bins) — the induced charge per time bin is returned in
+    RunResult.signal (NEXT-4)."""
     prim = np.ascontiguousarray(primaries, dtype=np.float64)
     np_ = prim.shape[0]
     cap = int(capacity if capacity is not None else max(4 * np_, 1 << 16))
@@ -224,7 +244,11 @@ def run(gas, field, primaries, seed=0, t_max=float("inf"), capacity=None, n_thre
     gd, _kg = gas_desc(gas)
     fd, _kf = field_desc(field)
     o = Outputs(cap, _p(ident), _p(av), _p(st), _p(ns), _p(birth), _p(end), _p(pa), _p(tu), _p(tf))
-    opts = RunOpts(int(seed), float(t_max), int(n_threads), int(id_offset), int(flags))
+    sig_arr, sig_c, _ks = None, None, None
+    if signal is not None:
+        sig_arr = np.zeros(int(signal[3]))
+        sig_c, _ks = _signal_c(signal[0], signal[1], signal[2], sig_arr)
+    opts = RunOpts(int(seed), float(t_max), int(n_threads), int(id_offset), int(flags), C.pointer(sig_c) if sig_c is not None else None)
     n_out = C.c_int64(0)
     rc = lib().avmo_run(C.byref(gd), C.byref(fd), _p(prim), C.c_int64(np_), C.byref(opts), C.byref(o), C.byref(n_out))
     if rc == -2 and not allow_overflow:
@@ -232,4 +256,32 @@ def run(gas, field, primaries, seed=0, t_max=float("inf"), capacity=None, n_thre
     if rc not in (0, -2):
         raise RuntimeError(lib().avmo_last_error().decode())
     n = n_out.value
-    return RunResult(n, ident[:n], av[:n], st[:n], ns[:n], birth[:, :n], end[:, :n], pa[:np_], tu[:L + 5], tf, rc, int(tu[L + 5]))
+    return RunResult(n, ident[:n], av[:n], st[:n], ns[:n], birth[:, :n], end[:, :n], pa[:np_], tu[:L + 5], tf, rc, int(tu[L + 5]), sig_arr)
+
+
+@dataclass
+class IonResult:
+    end: np.ndarray        # [4, 2n]: x, y, z, t; entry s = positive ion born with electron s, n + s = negative ion of electron s
+    status: np.ndarray     # [2n]; -1 = no such ion
+    n_steps: np.ndarray
+    signal: np.ndarray = None
+
+
+def ion_drift(field, run_result, n_primaries, mobility_pos, mobility_neg, step_cm, t_max=float("inf"), max_steps=1 << 20,
+              signal=None) -> IonResult:
+    r = run_result
+    n = int(r.n)
+    birth = np.ascontiguousarray(r.birth, dtype=np.float64); end = np.ascontiguousarray(r.end, dtype=np.float64)
+    status = np.ascontiguousarray(r.status, dtype=np.int32)
+    ie = np.zeros((4, 2 * n)); ist = np.zeros(2 * n, dtype=np.int32); ins = np.zeros(2 * n, dtype=np.uint32)
+    fd, _kf = field_desc(field)
+    sig_arr, sig_c, _ks = None, None, None
+    if signal is not None:
+        sig_arr = np.zeros(int(signal[3]))
+        sig_c, _ks = _signal_c(signal[0], signal[1], signal[2], sig_arr)
+    io = IonOpts(float(mobility_pos), float(mobility_neg), float(step_cm), float(t_max), int(max_steps))
+    rc = lib().avmo_ion_drift(C.byref(fd), C.byref(sig_c) if sig_c is not None else None, C.byref(io), C.c_int64(n), C.c_int64(n_primaries),
+                              C.c_int64(birth.shape[1]), _p(birth), C.c_int64(end.shape[1]), _p(end), _p(status), _p(ie), _p(ist), _p(ins))
+    if rc != 0:
+        raise RuntimeError(lib().avmo_last_error().decode())
+    return IonResult(ie, ist, ins, sig_arr)
