@@ -149,6 +149,19 @@ enum {
    * iterations only (no time-parallel batches: a flight's rate depends on the energy the previous flight ended with). */
   AVM_RUN_BANDED = 16u
 };
+/* NEXT-4 ("induced-signal accumulation (weighting-field dot velocity per flight) and ion drift";
+ * what the endpoints feed; DESIGN.md §3.7 readings W1-W4).  weighting: the weighting field E_w [1/cm] of the
+ * read-out electrode as an avm_field (uniform slabs or grid maps; mask and B ignored; E_w = 0 outside it).  Every step
+ * r -> r' of a charge q [e] that starts at time t adds q E_w . (r' - r) to signal_dev[floor((t - t0) / dt_bin)]; steps that
+ * start outside the bins are dropped.  Electron flights: q = -1, E_w at r.  signal_dev: DEVICE [n_bins] doubles, ADDED to
+ * (the caller zeroes it); induced charge per bin, current = charge / dt_bin. */
+typedef struct {
+  const avm_field* weighting;
+  double t0, dt_bin;
+  int32_t n_bins;
+  double* signal_dev;
+} avm_signal;
+
 typedef struct {
   uint64_t seed;
   double t_max;                   /* ns; electrons with t > t_max stop with status 6 (+inf: none) */
@@ -157,6 +170,7 @@ typedef struct {
                                    * reaches it stops the launch, live electrons are parked, the host relaunches */
   uint64_t id_offset;             /* id of primary 0 (replicas / shards of one job use disjoint ranges) */
   int32_t max_ctas;               /* 0 = one CTA per SM; else at most this many CTAs (results do not depend on it) */
+  const avm_signal* signal;       /* HOST struct or NULL: accumulate the electrons' induced signal during the run */
 } avm_run_opts;
 
 /* Caller-provided DEVICE buffers; `capacity` = maximum number of electrons ever created (primaries +
@@ -190,6 +204,19 @@ int32_t avm_run_stats(const avm_ctx*, int64_t* n_kernel_launches, int64_t* n_tra
 /* Device time [ms] of the transport-kernel launches of the last avm_run on this context, summed (CUDA events
  * recorded on the context's stream around each launch).  *ms_out is HOST.  bench.py's roofline uses it. */
 int32_t avm_run_transport_ms(const avm_ctx*, float* ms_out);
+
+/* Ion drift after a run (W3, W4).  Every electron s >= n_primaries left a positive ion at its birth point, every attached
+ * electron (status 5) a negative ion at its endpoint.  Ion i = s (positive) or n + s (negative) of 2 n entries; status -1 =
+ * no such ion.  An ion of charge q moves with v = q mu E(r), mu the mobility [cm^2 / (V ns)], integrated by the explicit
+ * midpoint rule in steps of fixed LENGTH step_cm (k1 = v(r), r_m = r + (step/2) k1/|k1|, k2 = v(r_m), r' = r + step k2/|k2|,
+ * dt = step / |k2|); it stops at the first sampled point outside the domain (status 1-3), inside material (4), after t_max
+ * (6), after max_steps or where the field vanishes (7).  With a signal, each step adds q E_w(r_m) . (r' - r) to the bin of the
+ * step's start time.  run: the avm_outputs of the finished avm_run (birth, end, status DEVICE arrays are read; n = its
+ * endpoint count).  ion_end: DEVICE [4][2n] x, y, z, t; ion_status: DEVICE [2n]; ion_steps: DEVICE [2n].  Asynchronous on
+ * the context's stream. */
+typedef struct { double mobility_pos, mobility_neg, step_cm, t_max; int32_t max_steps; } avm_ion_opts;
+int32_t avm_ion_drift(avm_ctx*, const avm_field* field, const avm_signal* signal, const avm_ion_opts*, const avm_outputs* run,
+                      int64_t n, int64_t n_primaries, double* ion_end, int32_t* ion_status, uint32_t* ion_steps);
 
 /* Device -> host copy of the first n entries of every non-NULL array of `host` from the same-named array of
  * `dev` ("retrieve the electron endpoints").  `host` is an avm_outputs whose pointers are HOST

@@ -26,7 +26,7 @@ RUN_PRIMARIES_ON_DEVICE, RUN_NO_TALLIES, RUN_SHAPE_WIDE, RUN_SHAPE_LATENCY, RUN_
 MAX_LEVELS, MAX_SLABS = 64, 8
 EXPORTS = ["avm_last_error", "avm_ctx_create", "avm_ctx_destroy", "avm_ctx_sm_count", "avm_gas_bytes",
            "avm_gas_create", "avm_gas_destroy", "avm_gas_nu_hat", "avm_gas_bands", "avm_field_create", "avm_field_destroy",
-           "avm_field_eval", "avm_run_workspace_bytes", "avm_run", "avm_run_stats", "avm_run_transport_ms", "avm_fetch", "avm_step_batch", "avm_step_batch_form",
+           "avm_field_eval", "avm_run_workspace_bytes", "avm_run", "avm_run_stats", "avm_run_transport_ms", "avm_fetch", "avm_ion_drift", "avm_step_batch", "avm_step_batch_form",
            "avm_philox_batch", "avm_fp64_probe", "avm_gather_probe", "avm_smem_probe"]
 
 
@@ -56,9 +56,20 @@ class _FieldDesc(C.Structure):
                 ("xy_lo", C.c_double * 2), ("xy_hi", C.c_double * 2)]
 
 
+class _Signal(C.Structure):
+    _fields_ = [("weighting", C.c_void_p), ("t0", C.c_double), ("dt_bin", C.c_double), ("n_bins", C.c_int32),
+                ("signal_dev", C.c_void_p)]
+
+
+class _IonOpts(C.Structure):
+    _fields_ = [("mobility_pos", C.c_double), ("mobility_neg", C.c_double), ("step_cm", C.c_double), ("t_max", C.c_double),
+                ("max_steps", C.c_int32)]
+
+
 class _RunOpts(C.Structure):
     _fields_ = [("seed", C.c_uint64), ("t_max", C.c_double), ("flags", C.c_uint32),
-                ("max_iters_per_launch", C.c_uint32), ("id_offset", C.c_uint64), ("max_ctas", C.c_int32)]
+                ("max_iters_per_launch", C.c_uint32), ("id_offset", C.c_uint64), ("max_ctas", C.c_int32),
+                ("signal", C.POINTER(_Signal))]
 
 
 class _Outputs(C.Structure):
@@ -75,7 +86,7 @@ _lib.avm_run_workspace_bytes.argtypes = [C.c_void_p, C.c_int64]
 _lib.avm_gas_nu_hat.restype = C.c_double
 _lib.avm_gas_nu_hat.argtypes = [C.c_void_p]
 for _n in ("avm_ctx_create", "avm_ctx_destroy", "avm_ctx_sm_count", "avm_gas_create", "avm_gas_destroy", "avm_gas_bands",
-           "avm_field_create", "avm_field_destroy", "avm_field_eval", "avm_run", "avm_run_stats", "avm_fetch",
+           "avm_field_create", "avm_field_destroy", "avm_field_eval", "avm_run", "avm_run_stats", "avm_fetch", "avm_ion_drift",
            "avm_step_batch", "avm_step_batch_form", "avm_philox_batch", "avm_fp64_probe", "avm_run_transport_ms",
            "avm_gather_probe", "avm_smem_probe"):
     getattr(_lib, _n).restype = C.c_int32
@@ -91,6 +102,8 @@ _lib.avm_field_destroy.argtypes = [C.c_void_p]
 _lib.avm_field_eval.argtypes = [C.c_void_p, C.c_void_p, C.c_int64] + [C.c_void_p] * 4
 _lib.avm_run.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(_RunOpts),
                          C.POINTER(_Outputs), C.POINTER(C.c_int64)]
+_lib.avm_ion_drift.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_Signal), C.POINTER(_IonOpts), C.POINTER(_Outputs), C.c_int64, C.c_int64,
+                               C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.avm_run_stats.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
 _lib.avm_fetch.argtypes = [C.c_void_p, C.POINTER(_Outputs), C.c_int64, C.c_int64, C.c_int32, C.POINTER(_Outputs)]
 _lib.avm_step_batch.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint64, C.c_double, C.c_int64] + [C.c_void_p] * 9
@@ -422,9 +435,19 @@ class RunResult:
                          self.end[:, o], self.per_avalanche, self.tallies_u64, self.tallies_f64, self.rc)
 
 
+def _signal_struct(signal):
+    """signal = (weighting Field, t0, dt_bin, float64 CUDA tensor [n_bins]) -> avm_signal (or None)."""
+    if signal is None:
+        return None
+    wf, t0, dt_bin, arr = signal
+    assert arr.is_cuda and arr.dtype == torch.float64 and arr.is_contiguous()
+    return _Signal(wf._h, float(t0), float(dt_bin), int(arr.numel()), arr.data_ptr())
+
+
 def run(ctx: Context, gas: Gas, field: Field, primaries, bufs: RunBuffers, seed=0, t_max=float("inf"), flags=0,
-        max_iters_per_launch=0, id_offset=0, max_ctas=0, allow_overflow=False) -> tuple:
+        max_iters_per_launch=0, id_offset=0, max_ctas=0, allow_overflow=False, signal=None) -> tuple:
     """avm_run.  primaries: numpy/CPU tensor [Np, 8] (H2D inside the call) or a CUDA tensor (flag set here).
+    signal: None or (weighting Field, t0, dt_bin, float64 CUDA tensor [n_bins], added to) — the induced signal (NEXT-4).
     Returns (rc, n_endpoints); outputs stay in `bufs` on the device."""
     if isinstance(primaries, torch.Tensor) and primaries.is_cuda:
         p = primaries.contiguous()
@@ -438,7 +461,9 @@ def run(ctx: Context, gas: Gas, field: Field, primaries, bufs: RunBuffers, seed=
     else:
         p = np.ascontiguousarray(primaries, dtype=np.float64)
         ptr, np_ = _hp(p), p.shape[0]
-    opts = _RunOpts(int(seed), float(t_max), int(flags), int(max_iters_per_launch), int(id_offset), int(max_ctas))
+    sg = _signal_struct(signal)
+    opts = _RunOpts(int(seed), float(t_max), int(flags), int(max_iters_per_launch), int(id_offset), int(max_ctas),
+                    C.pointer(sg) if sg is not None else None)
     o = bufs.c_struct()
     n_out = C.c_int64(0)
     rc = _lib.avm_run(ctx._h, gas._h, field._h, ptr, np_, C.byref(opts), C.byref(o), C.byref(n_out))
@@ -469,6 +494,26 @@ def fetch(ctx: Context, bufs: RunBuffers, n: int, host: Optional[HostBuffers] = 
     return RunResult(n, u64(host.id)[:n], host.avalanche.numpy().view(np.uint32)[:n], host.status.numpy()[:n],
                      host.n_steps.numpy().view(np.uint32)[:n], host.birth.numpy()[:, :n], host.end.numpy()[:, :n],
                      u64(host.per_avalanche)[:bufs.n_primaries], u64(host.tallies_u64), host.tallies_f64.numpy())
+
+
+@dataclass
+class IonResult:
+    end: np.ndarray        # [4, 2n]: x, y, z, t; entry s = positive ion born with electron s, n + s = negative ion of electron s
+    status: np.ndarray     # [2n]; -1 = no such ion
+    n_steps: np.ndarray
+
+
+def ion_drift(ctx: Context, field: Field, bufs: RunBuffers, n: int, mobility_pos, mobility_neg, step_cm, t_max=float("inf"),
+              max_steps=1 << 20, signal=None) -> IonResult:
+    """avm_ion_drift on the outputs of a finished run (still on the device in `bufs`)."""
+    ie = ctx.empty((4, 2 * max(n, 1)), torch.float64); ist = ctx.empty(2 * max(n, 1), torch.int32); ins = ctx.empty(2 * max(n, 1), torch.int32)
+    sg = _signal_struct(signal)
+    io = _IonOpts(float(mobility_pos), float(mobility_neg), float(step_cm), float(t_max), int(max_steps))
+    o = bufs.c_struct()
+    _check(_lib.avm_ion_drift(ctx._h, field._h, C.byref(sg) if sg is not None else None, C.byref(io), C.byref(o), int(n),
+                              int(bufs.n_primaries), _dev(ie), _dev(ist), _dev(ins)))
+    torch.cuda.synchronize(ctx.device)
+    return IonResult(ie.cpu().numpy()[:, :2 * n], ist.cpu().numpy()[:2 * n], ins.cpu().numpy().view(np.uint32)[:2 * n])
 
 
 def simulate(ctx: Context, gas: Gas, field: Field, primaries, seed=0, t_max=float("inf"), capacity=None, **kw) -> RunResult:

@@ -308,18 +308,76 @@ step_form_batch_kernel(const __grid_constant__ DevGas g, const __grid_constant__
     event[o] = ev; status[o] = fin; bin[o] = b < 0 ? -1 : b;
   };
   if constexpr (FORM == 2) {
-    tp_batch<FK, HASB, true>(g, f, K, g.tab, s_lv, s_logtab, &s_wb[warp], t_max, lane, act, have, x, y, z, t, vx, vy, vz, id, nn,
+    tp_batch<FK, HASB, true, false>(g, f, K, g.tab, s_lv, s_logtab, &s_wb[warp], t_max, lane, act, have, x, y, z, t, vx, vy, vz, id, nn,
                              slot, tl, collide, [&](bool on, int e, int sidx, int ev, int b, int fin) { if (on) record(e, sidx, ev, b, fin); });
   } else {
     // sb_batch calls commit AFTER a step; the child of a collision is recorded inside collide, before the commit of the
     // same step: o_cur is kept one step ahead (the owner lane's next output entry)
     o_cur = have ? i * gl : 0;
     const int jcls = (BANDED && FK == 1) ? accel_class(g, f.slab[0].E[0], f.slab[0].E[1], f.slab[0].E[2]) : 0;
-    sb_batch<FK, HASB, true, BANDED>(g, f, K, g.tab, s_logtab, &s_wb[warp], t_max, lane, act, have, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, id,
+    sb_batch<FK, HASB, true, BANDED, false>(g, f, K, g.tab, s_logtab, &s_wb[warp], t_max, lane, act, have, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, id,
                                      nn, tl, collide, [&](const unsigned, int fin) { if (fin != 0) have = false; },
                                      [&](int e, int sidx, int ev, int b, int fin) { record(e, sidx, ev, b, fin); o_cur = s_gidx[warp][e] * gl + sidx + 1; },
                                      jcls);
   }
+}
+
+// ---- NEXT-4: ion drift (W3-W4) ---------------------------------------------------------------------------
+// One thread per possible ion: i < n = the positive ion left where electron i was born (none for the primaries), i >= n =
+// the negative ion of electron i - n if it was attached.  Explicit midpoint along q mu E in steps of fixed length.
+struct IonOpts { double mu_pos, mu_neg, step, t_max; int max_steps; };
+template <bool SIGNAL>
+__global__ void __launch_bounds__(256)
+ion_drift_kernel(const __grid_constant__ DevField f, const __grid_constant__ DevSignal sig, const IonOpts io, const RunArrays a,
+                 const uint32_t n, const uint32_t n_prim, double* __restrict__ ion_end, int32_t* __restrict__ ion_status,
+                 uint32_t* __restrict__ ion_steps) {
+  const size_t N = 2 * (size_t)n, ld = a.cap;
+  SigAcc sacc;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (size_t)gridDim.x * blockDim.x) {
+    const uint32_t s = i < n ? (uint32_t)i : (uint32_t)(i - n);
+    const bool pos = i < n;
+    int st = -1;
+    uint32_t ns = 0u;
+    double x = 0.0, y = 0.0, z = 0.0, t = 0.0;
+    if (pos ? s >= n_prim : a.status[s] == AVM_ATTACHED) {                  // W3: which ions exist
+      const double* src = pos ? a.birth : a.end;
+      x = src[s]; y = src[ld + s]; z = src[2 * ld + s]; t = src[3 * ld + s];
+      const double q = pos ? 1.0 : -1.0, qmu = q * (pos ? io.mu_pos : io.mu_neg);
+      double Ex, Ey, Ez, m;
+      int si = field_at<0>(f, x, y, z, Ex, Ey, Ez, m);
+      st = si < 0 ? -si : (m < 0.5 ? AVM_MATERIAL : AVM_ACTIVE);
+      while (st == AVM_ACTIVE) {
+        if (ns >= (uint32_t)io.max_steps) { st = AVM_STEP_LIMIT; break; }
+        const double k1x = qmu * Ex, k1y = qmu * Ey, k1z = qmu * Ez;
+        const double n1 = sqrt(k1x * k1x + k1y * k1y + k1z * k1z);
+        if (!(n1 > 0.0)) { st = AVM_STEP_LIMIT; break; }
+        const double hh = 0.5 * io.step / n1;
+        const double mx = x + hh * k1x, my = y + hh * k1y, mz = z + hh * k1z;
+        double Emx, Emy, Emz, mm;
+        if (field_at<0>(f, mx, my, mz, Emx, Emy, Emz, mm) < 0) { Emx = Ex; Emy = Ey; Emz = Ez; }   // midpoint outside: Euler step
+        const double k2x = qmu * Emx, k2y = qmu * Emy, k2z = qmu * Emz;
+        const double n2 = sqrt(k2x * k2x + k2y * k2y + k2z * k2z);
+        if (!(n2 > 0.0)) { st = AVM_STEP_LIMIT; break; }
+        const double h2 = io.step / n2;
+        const double nx = x + h2 * k2x, ny = y + h2 * k2y, nz = z + h2 * k2z;
+        if (SIGNAL) {
+          double wx, wy, wz;
+          weighting_at(sig, mx, my, mz, wx, wy, wz);
+          sig_add(sig, sacc, q * (wx * (nx - x) + wy * (ny - y) + wz * (nz - z)), t);
+        }
+        x = nx; y = ny; z = nz;
+        t = t + h2;
+        ++ns;
+        si = field_at<0>(f, x, y, z, Ex, Ey, Ez, m);
+        if (si < 0) st = -si;
+        else if (m < 0.5) st = AVM_MATERIAL;
+        else if (t > io.t_max) st = AVM_TIME_LIMIT;
+      }
+    }
+    ion_end[i] = x; ion_end[N + i] = y; ion_end[2 * N + i] = z; ion_end[3 * N + i] = t;
+    ion_status[i] = st; ion_steps[i] = ns;
+  }
+  if (SIGNAL) sig_flush(sig, sacc);
 }
 
 // Widened copy of a grid map: node i's float4 (Ex, Ey, Ez, mask) -> four doubles, exactly (avm_slab.nodes_f64_dev).
@@ -844,10 +902,20 @@ int32_t avm_run_transport_ms(const avm_ctx* c, float* ms_out) {
 }  // extern "C"
 
 namespace {
-TransportFn pick_transport(int fk, bool has_b, bool smemtab, bool wide, bool banded) {
-  if (fk == 1) return has_b ? pick_transport_inst<1, true>(smemtab, wide, banded) : pick_transport_inst<1, false>(smemtab, wide, banded);
-  if (fk == 2) return has_b ? pick_transport_inst<2, true>(smemtab, wide, banded) : pick_transport_inst<2, false>(smemtab, wide, banded);
-  return has_b ? pick_transport_inst<0, true>(smemtab, wide, banded) : pick_transport_inst<0, false>(smemtab, wide, banded);
+TransportFn pick_transport(int fk, bool has_b, bool smemtab, bool wide, bool banded, bool signal) {
+  if (fk == 1) return has_b ? pick_transport_inst<1, true>(smemtab, wide, banded, signal) : pick_transport_inst<1, false>(smemtab, wide, banded, signal);
+  if (fk == 2) return has_b ? pick_transport_inst<2, true>(smemtab, wide, banded, signal) : pick_transport_inst<2, false>(smemtab, wide, banded, signal);
+  return has_b ? pick_transport_inst<0, true>(smemtab, wide, banded, signal) : pick_transport_inst<0, false>(smemtab, wide, banded, signal);
+}
+// W1: the device form of a signal description (validated); false with g_err set when it is unusable.
+bool make_signal(const avm_signal* s, DevSignal& D) {
+  std::memset(&D, 0, sizeof(D));
+  if (!s) return true;
+  if (!s->weighting || !(s->dt_bin > 0.0) || s->n_bins < 1 || !s->signal_dev || !std::isfinite(s->t0)) { g_err = "signal: weighting field, dt_bin > 0, n_bins >= 1 and a device array are required"; return false; }
+  D.wf = s->weighting->d;
+  D.t0 = s->t0; D.inv_dt = 1.0 / s->dt_bin; D.n_bins = s->n_bins; D.uniform1 = s->weighting->uniform1 ? 1 : 0;
+  D.out = s->signal_dev;
+  return true;
 }
 }  // namespace
 
@@ -897,7 +965,10 @@ int32_t avm_run(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, const 
   const size_t tab_bytes = align_up(sizeof(ushort4) * (size_t)gas->d.nb, 16);
   const bool smemtab = tab_bytes + buf_bytes <= kMaxDynSmem;       // else the threshold table is read through L1
   const size_t dyn_smem = (smemtab ? tab_bytes : 0) + buf_bytes;
-  TransportFn fn = pick_transport(field->fk, field->d.has_B != 0, smemtab, wide, (opts->flags & AVM_RUN_BANDED) != 0);
+  DevSignal dsig;
+  if (!make_signal(opts->signal, dsig)) return AVM_ERR_INVALID_ARG;
+  TransportFn fn = pick_transport(field->fk, field->d.has_B != 0, smemtab, wide, (opts->flags & AVM_RUN_BANDED) != 0, opts->signal != nullptr);
+  if (!fn) return fail(AVM_ERR_INVALID_ARG, "run: a signal needs the threshold table in shared memory (at most ~24000 energy bins)");
   AVM_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn_smem));
   int occ = 0;
   AVM_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, threads, dyn_smem));
@@ -924,7 +995,7 @@ int32_t avm_run(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, const 
       ctx->transport_ms += ms;
     }
     AVM_CUDA(cudaEventRecord(ctx->ev_t0, st));
-    fn<<<grid, threads, dyn_smem, st>>>(gas->d, field->d, a, ctl, philox_keys(opts->seed), opts->t_max, max_iters, n_static);
+    fn<<<grid, threads, dyn_smem, st>>>(gas->d, field->d, a, ctl, philox_keys(opts->seed), opts->t_max, max_iters, n_static, dsig);
     AVM_CUDA(cudaGetLastError());
     AVM_CUDA(cudaEventRecord(ctx->ev_t1, st));
     ctx->n_kernel_launches++; ctx->n_transport_launches++;
@@ -955,6 +1026,28 @@ int32_t avm_run(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, const 
   dropped = *(unsigned int*)(ctx->h_counters + 1);
   *n_out = n_end;
   if (dropped) return fail(AVM_ERR_CAPACITY, "run: capacity exceeded, " + std::to_string(dropped) + " secondaries dropped");
+  return AVM_OK;
+}
+
+int32_t avm_ion_drift(avm_ctx* ctx, const avm_field* field, const avm_signal* signal, const avm_ion_opts* io, const avm_outputs* run,
+                      int64_t n, int64_t n_primaries, double* ion_end, int32_t* ion_status, uint32_t* ion_steps) {
+  if (!ctx || !field || !io || !run || n < 0 || n_primaries < 0) return fail(AVM_ERR_INVALID_ARG, "ion_drift: null argument");
+  if (!(io->step_cm > 0.0) || !(io->mobility_pos > 0.0) || !(io->mobility_neg > 0.0) || io->max_steps < 1) return fail(AVM_ERR_INVALID_ARG, "ion_drift: step, mobilities and max_steps must be positive");
+  if (n == 0) return AVM_OK;
+  if (n > run->capacity || !run->birth || !run->end || !run->status || !ion_end || !ion_status || !ion_steps) return fail(AVM_ERR_INVALID_ARG, "ion_drift: run outputs (birth, end, status) and the ion arrays are required");
+  DevSignal dsig;
+  if (!make_signal(signal, dsig)) return AVM_ERR_INVALID_ARG;
+  AVM_CUDA(cudaSetDevice(ctx->device));
+  RunArrays a;
+  a.cap = (uint32_t)run->capacity; a.id = run->id; a.aval = run->avalanche; a.status = run->status; a.nsteps = run->n_steps;
+  a.birth = run->birth; a.end = run->end;
+  IonOpts o;
+  o.mu_pos = io->mobility_pos; o.mu_neg = io->mobility_neg; o.step = io->step_cm; o.t_max = io->t_max; o.max_steps = io->max_steps;
+  unsigned blocks = (unsigned)((2 * n + 255) / 256);
+  const unsigned maxb = (unsigned)ctx->sm_count * 8u;
+  if (blocks > maxb) blocks = maxb;
+  if (signal) AVM_CUDA(launch(ctx, ion_drift_kernel<true>, dim3(blocks), dim3(256), field->d, dsig, o, a, (uint32_t)n, (uint32_t)n_primaries, ion_end, ion_status, ion_steps));
+  else AVM_CUDA(launch(ctx, ion_drift_kernel<false>, dim3(blocks), dim3(256), field->d, dsig, o, a, (uint32_t)n, (uint32_t)n_primaries, ion_end, ion_status, ion_steps));
   return AVM_OK;
 }
 

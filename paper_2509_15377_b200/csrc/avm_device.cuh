@@ -313,6 +313,36 @@ __device__ __forceinline__ int field_at(const DevField& f, double x, double y, d
   return si;
 }
 
+// ---- NEXT-4: induced signal (W1-W2) ----------------------------------------------------------------------
+// wf = the weighting field E_w [1/cm] of the read-out electrode as a field description (mask and B ignored; E_w = 0 outside
+// it).  A step r -> r' of a charge q that starts at time t adds q E_w(at) . (r' - r) to out[floor((t - t0) / dt_bin)].
+struct DevSignal {
+  DevField wf;
+  double t0, inv_dt;
+  int n_bins, uniform1;     // uniform1: wf is one uniform slab
+  double* out;              // [n_bins]
+};
+__device__ __forceinline__ void weighting_at(const DevSignal& s, double x, double y, double z, double& wx, double& wy, double& wz) {
+  double ex = 0.0, ey = 0.0, ez = 0.0, m;
+  const int si = s.uniform1 ? field_at<1>(s.wf, x, y, z, ex, ey, ez, m) : field_at<0>(s.wf, x, y, z, ex, ey, ez, m);
+  const bool in = si >= 0;
+  wx = in ? ex : 0.0; wy = in ? ey : 0.0; wz = in ? ez : 0.0;
+}
+// Per-thread accumulator: contributions to one time bin are summed in a register and flushed with one atomicAdd when the
+// bin changes (a bin holds ~100 flights) and at the end of the launch.  Any thread may hold any electron's contributions:
+// the signal is a plain sum.
+struct SigAcc { int bin = -1; double q = 0.0; };
+__device__ __forceinline__ void sig_flush(const DevSignal& s, SigAcc& a) {
+  if (a.bin >= 0 && a.q != 0.0) atomicAdd(s.out + a.bin, a.q);
+  a.q = 0.0;
+}
+__device__ __forceinline__ void sig_add(const DevSignal& s, SigAcc& a, double dq, double t) {
+  const double sb = floor((t - s.t0) * s.inv_dt);
+  const int b = (sb >= 0.0 && sb < (double)s.n_bins) ? (int)sb : -1;
+  if (b != a.bin) { sig_flush(s, a); a.bin = b; }
+  if (b >= 0) a.q += dq;
+}
+
 // ---- S2-S3: free flight of duration dt in constant E (and B) from (r, v) ---------------------------------
 // UNIFORM1: E is the run constant of slab 0 and the arguments Ex, Ey, Ez are ignored (a, E x B drift and a-parallel
 // come precomputed from DevField).

@@ -40,13 +40,14 @@ static_assert(sizeof(WarpBuf) == 1920, "WarpBuf");
 // BANDED (NEXT-1): dt carries -ln(u1); the flight's rate comes from the band of the electron's energy and
 // the class of the field at its position (jcls = the class when the field is one uniform slab), a flight longer than the
 // band's dtmax is cut there and ends in a null collision, and the decision compares u2 nu with the flight's own nu.
-template <int FK, bool HASB, bool TALLY, bool BANDED = false>
+// SIGNAL (NEXT-4): the flight's induced charge -E_w(r) . (r' - r) goes to the bin of its start time.
+template <int FK, bool HASB, bool TALLY, bool BANDED = false, bool SIGNAL = false>
 __device__ __forceinline__ void fw_flight(const DevGas& g, const DevField& f, const PhiloxKeys& K,
                                           const ushort4* __restrict__ tab, const double2* __restrict__ logtab,
                                           const double t_max, const uint64_t id, uint32_t& n, double& x, double& y,
                                           double& z, double& t, double& vx, double& vy, double& vz, double& Ex, double& Ey,
                                           double& Ez, double& dt, uint2& u2w, int& fin, bool& pend, Pending& pc, Tally& tl,
-                                          const int jcls = 0) {
+                                          const int jcls = 0, const DevSignal* sig = nullptr, SigAcc* sacc = nullptr) {
   bool over = false, cut = false;
   double dtf = dt, nu = g.nu_hat;
   uint32_t rho = 0u;
@@ -55,7 +56,10 @@ __device__ __forceinline__ void fw_flight(const DevGas& g, const DevField& f, co
     dtf = banded_dt(br, dt, cut);
     nu = br.nu; rho = br.rho;
   }
+  double sx0 = 0.0, sy0 = 0.0, sz0 = 0.0, st0 = 0.0, swx = 0.0, swy = 0.0, swz = 0.0;
+  if (SIGNAL) { sx0 = x; sy0 = y; sz0 = z; st0 = t; weighting_at(*sig, x, y, z, swx, swy, swz); }
   const int b = advance<FK, HASB>(g, f, t_max, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dtf, over);
+  if (SIGNAL) sig_add(*sig, *sacc, -(swx * (x - sx0) + swy * (y - sy0) + swz * (z - sz0)), st0);
   if (b < 0) { fin = -b; return; }
   AVM_CHECK(b < g.nb);
   const ushort4 rec = tab[b];
@@ -86,13 +90,14 @@ __device__ __forceinline__ void fw_flight(const DevGas& g, const DevField& f, co
 // commit(on, e, sidx, ev, bin, fin): called once per pass by every lane; on = this lane's step was taken in this pass,
 //   its result is in x .. vz, n; ev = -1 null, level, or -2 ended before the decision.
 // Returns the finishing status of the lane's own electron (0 = still active); its state is back in x .. vz, id, n, slot.
-template <int FK, bool HASB, bool TALLY, class Collide, class Commit>
+template <int FK, bool HASB, bool TALLY, bool SIGNAL, class Collide, class Commit>
 __device__ __forceinline__ int tp_batch(const DevGas& g, const DevField& f, const PhiloxKeys& K,
                                         const ushort4* __restrict__ tab, const LevelPar* __restrict__ s_lv,
                                         const double2* __restrict__ s_logtab, WarpBuf* __restrict__ wb, const double t_max,
                                         const unsigned lane, const unsigned act, const bool have, double& x, double& y,
                                         double& z, double& t, double& vx, double& vy, double& vz, uint64_t& id, uint32_t& n,
-                                        uint32_t& slot, Tally& tl, Collide&& collide, Commit&& commit) {
+                                        uint32_t& slot, Tally& tl, Collide&& collide, Commit&& commit,
+                                        const DevSignal* sig = nullptr, SigAcc* sacc = nullptr) {
   static_assert(FK == 1, "time-parallel batches need a constant field: one uniform slab");
   const unsigned lt_mask = (1u << lane) - 1u;
   const int k = __popc(act);
@@ -173,6 +178,18 @@ __device__ __forceinline__ int tp_batch(const DevGas& g, const DevField& f, cons
     const unsigned evm = __ballot_sync(0xFFFFFFFFu, ev) & gmask;
     const int fl = __ffs(evm) - 1;                       // the group's first step that is not null, or -1
     const bool taken = valid && (fl < 0 || (int)lane <= fl);   // this lane's step is one the electron really takes
+    if (SIGNAL) {
+      // the flight of step s starts where step s - 1 ended: the lane kp below (same electron), or the base state
+      const double px = __shfl_up_sync(0xFFFFFFFFu, x, kp), py = __shfl_up_sync(0xFFFFFFFFu, y, kp);
+      const double pz = __shfl_up_sync(0xFFFFFFFFu, z, kp), pt = __shfl_up_sync(0xFFFFFFFFu, t, kp);
+      if (taken) {
+        const bool first = sidx == cur;
+        const double sx0 = first ? bx : px, sy0 = first ? by : py, sz0 = first ? bz : pz, st0 = first ? bt : pt;
+        double swx, swy, swz;
+        weighting_at(*sig, sx0, sy0, sz0, swx, swy, swz);
+        sig_add(*sig, *sacc, -(swx * (x - sx0) + swy * (y - sy0) + swz * (z - sz0)), st0);
+      }
+    }
     // S6 counts an energy overflow only for a step that passes S5 (reaches the bin lookup)
     if (TALLY && taken && over && b >= 0) ++tl.over;
     int fin = 0, evc = -1;
@@ -238,13 +255,14 @@ __device__ __forceinline__ int tp_batch(const DevGas& g, const DevField& f, cons
 // mask = the lanes converged at the call (the warp-aggregated atomics inside them run over that mask); retire clears
 // `have`.  commit(e, s, ev, bin, fin): step s of the batch of the warp's e-th electron is done, its result is in x .. vz, n.
 // BANDED: as fw_flight — the exchange area holds -ln(u1) per step, the rate is looked up when the step starts.
-template <int FK, bool HASB, bool TALLY, bool BANDED, class Collide, class Retire, class Commit>
+template <int FK, bool HASB, bool TALLY, bool BANDED, bool SIGNAL, class Collide, class Retire, class Commit>
 __device__ __forceinline__ void sb_batch(const DevGas& g, const DevField& f, const PhiloxKeys& K,
                                          const ushort4* __restrict__ tab, const double2* __restrict__ s_logtab,
                                          WarpBuf* __restrict__ wb, const double t_max, const unsigned lane, const unsigned act,
                                          bool& have, double& x, double& y, double& z, double& t, double& vx, double& vy,
                                          double& vz, double& Ex, double& Ey, double& Ez, const uint64_t& id, uint32_t& n,
-                                         Tally& tl, Collide&& collide, Retire&& retire, Commit&& commit, const int jcls = 0) {
+                                         Tally& tl, Collide&& collide, Retire&& retire, Commit&& commit, const int jcls = 0,
+                                         const DevSignal* sig = nullptr, SigAcc* sacc = nullptr) {
   const unsigned lt_mask = (1u << lane) - 1u;
   const int k = __popc(act);
   const int lg = 32 - __clz(k - 1);             // k' = 2^lg >= k  (k = 1: __clz(0) = 32)
@@ -281,7 +299,10 @@ __device__ __forceinline__ void sb_batch(const DevGas& g, const DevField& f, con
       dtj = banded_dt(br, dtj, cut);
       nu = br.nu; rho = br.rho;
     }
+    double sx0 = 0.0, sy0 = 0.0, sz0 = 0.0, st0 = 0.0, swx = 0.0, swy = 0.0, swz = 0.0;
+    if (SIGNAL) { sx0 = x; sy0 = y; sz0 = z; st0 = t; weighting_at(*sig, x, y, z, swx, swy, swz); }
     const double s2 = advance_move<FK, HASB>(f, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dtj);   // S3, S4
+    if (SIGNAL) sig_add(*sig, *sacc, -(swx * (x - sx0) + swy * (y - sy0) + swz * (z - sz0)), st0);
     bool over;
     const int b = energy_bin(g, s2, over);                                                     // S6 (counts only when S5 passes)
     AVM_CHECK(b >= 0 && b < g.nb);

@@ -40,7 +40,7 @@ constexpr int64_t kStageElectrons = 1 << 18;   // primaries staged per H2D chunk
 constexpr int kMaxGrid = 1024;                 // done flags, one 32-byte sector per CTA
 constexpr size_t kDoneOffset = 4096;
 constexpr size_t kCtlBytes = kDoneOffset + (size_t)kMaxGrid * 32;
-constexpr size_t kMaxDynSmem = 227 * 1024 - 4096;   // static shared memory (level parameters) comes on top
+constexpr size_t kMaxDynSmem = 227 * 1024 - 6144;   // static shared memory (level parameters, logarithm table: 5.4 KB) comes on top
 
 struct RunArrays {
   uint32_t cap;
@@ -114,11 +114,11 @@ constexpr int kCoopMax = AVM_COOP_MAX;
 #ifndef AVM_SB_UNIFORM
 #define AVM_SB_UNIFORM 0     // 1: serial batches instead of time-parallel ones in one uniform slab without B
 #endif
-template <int FK, bool HASB, bool TALLY, bool SMEMTAB, int THREADS, bool TPB, bool BANDED>
+template <int FK, bool HASB, bool TALLY, bool SMEMTAB, int THREADS, bool TPB, bool BANDED, bool SIGNAL>
 __global__ void __launch_bounds__(THREADS, 1)
 transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevField f, const RunArrays a,
                  RunCtl* __restrict__ ctl, const __grid_constant__ PhiloxKeys K, const double t_max,
-                 const uint32_t max_iters, const uint32_t n_static_tickets) {
+                 const uint32_t max_iters, const uint32_t n_static_tickets, const __grid_constant__ DevSignal sig) {
   extern __shared__ __align__(16) unsigned char s_dyn[];
   __shared__ LevelPar s_lv[AVM_MAX_LEVELS];
   __shared__ double2 s_logtab[128];
@@ -155,6 +155,7 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
   uint64_t id = 0;
   uint32_t n = 0, slot = 0;
   Tally tl;                                       // tallies kept per thread; null counts are derived (finalize_kernel)
+  SigAcc sacc;                                    // NEXT-4: this thread's pending contribution to one time bin of the signal
   uint32_t backoff = 250u;
   const unsigned lt_mask = (1u << lane) - 1u;
 
@@ -307,15 +308,15 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
     if (TPB && !BANDED && FK == 1 && (HASB || !AVM_SB_UNIFORM) && k <= kCoopMax) {
       // ---- time-parallel batch (uniform E, optional B): g = 32 / k' lanes per electron (avm_forms.cuh) ----
       if constexpr (FK == 1) {
-        const int fin = tp_batch<FK, HASB, TALLY>(g, f, K, tab, s_lv, s_logtab, wb, t_max, lane, act, have, x, y, z, t, vx, vy, vz,
-                                                  id, n, slot, tl, collide_and_append, [](bool, int, int, int, int, int) {});
+        const int fin = tp_batch<FK, HASB, TALLY, SIGNAL>(g, f, K, tab, s_lv, s_logtab, wb, t_max, lane, act, have, x, y, z, t, vx, vy, vz,
+                                                          id, n, slot, tl, collide_and_append, [](bool, int, int, int, int, int) {}, &sig, &sacc);
         dvalid = false;
         retire(0xFFFFFFFFu, fin);
       }
     } else if (k <= kCoopMax) {
       // ---- serial batch: cooperative draws, then every owner lane walks its electron's steps alone (avm_forms.cuh) ----
-      sb_batch<FK, HASB, TALLY, BANDED>(g, f, K, tab, s_logtab, wb, t_max, lane, act, have, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, id, n, tl,
-                                        collide_and_append, retire, [](int, int, int, int, int) {}, jcls);
+      sb_batch<FK, HASB, TALLY, BANDED, SIGNAL>(g, f, K, tab, s_logtab, wb, t_max, lane, act, have, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, id, n, tl,
+                                                collide_and_append, retire, [](int, int, int, int, int) {}, jcls, &sig, &sacc);
       dvalid = false;
     } else {
       // ---- full warp ----
@@ -327,8 +328,8 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
 #pragma unroll
       for (int fl = 0; fl < kFlights; ++fl) {
         if (have && !pend && fin == 0)
-          fw_flight<FK, HASB, TALLY, BANDED>(g, f, K, tab, s_logtab, t_max, id, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt, u2w, fin,
-                                             pend, pc, tl, jcls);
+          fw_flight<FK, HASB, TALLY, BANDED, SIGNAL>(g, f, K, tab, s_logtab, t_max, id, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt, u2w, fin,
+                                                     pend, pc, tl, jcls, &sig, &sacc);
       }
       Deflection dd;
       dd.ct = 1.0; dd.st = 0.0; dd.cphi = 1.0; dd.sphi = 0.0;
@@ -355,6 +356,7 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
     a.end[5 * ld + slot] = kx; a.end[6 * ld + slot] = ky; a.end[7 * ld + slot] = kz;
     a.nsteps[slot] = n;
   }
+  if (SIGNAL) sig_flush(sig, sacc);
   if (TALLY) {
     // warp reduce the per-thread counters, one atomic per warp; rare-level histogram per CTA
     unsigned long long v0 = tl.real, v1 = tl.l0, v3 = tl.over, v5 = tl.pen;
@@ -379,9 +381,10 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
 }
 
 typedef void (*TransportFn)(const DevGas, const DevField, const RunArrays, RunCtl*, const PhiloxKeys, const double,
-                            const uint32_t, const uint32_t);
-// Defined (explicit specialisation) in avm_transport_inst.cu, one translation unit per (FK, B).
+                            const uint32_t, const uint32_t, const DevSignal);
+// Defined (explicit specialisation) in avm_transport_inst.cu, one translation unit per (FK, B).  signal with the threshold
+// table outside shared memory (more than ~24000 energy bins) is not instantiated: nullptr.
 template <int FK, bool B>
-TransportFn pick_transport_inst(bool smemtab, bool wide, bool banded);
+TransportFn pick_transport_inst(bool smemtab, bool wide, bool banded, bool signal);
 
 }  // namespace avm

@@ -10,20 +10,21 @@
 namespace avm {
 namespace {
 template <int FK, bool B, int T, bool TPB, bool BANDED>
-TransportFn pick4(bool smemtab) {
-  return smemtab ? transport_kernel<FK, B, true, true, T, TPB, BANDED> : transport_kernel<FK, B, true, false, T, TPB, BANDED>;
+TransportFn pick4(bool smemtab, bool signal) {
+  if (signal) return smemtab ? transport_kernel<FK, B, true, true, T, TPB, BANDED, true> : nullptr;
+  return smemtab ? transport_kernel<FK, B, true, true, T, TPB, BANDED, false> : transport_kernel<FK, B, true, false, T, TPB, BANDED, false>;
 }
 template <int FK, bool B, int T, bool TPB>
-TransportFn pick3(bool smemtab, bool banded) {
-  return banded ? pick4<FK, B, T, TPB, true>(smemtab) : pick4<FK, B, T, TPB, false>(smemtab);
+TransportFn pick3(bool smemtab, bool banded, bool signal) {
+  return banded ? pick4<FK, B, T, TPB, true>(smemtab, signal) : pick4<FK, B, T, TPB, false>(smemtab, signal);
 }
 }  // namespace
 
 template <>
-TransportFn pick_transport_inst<AVM_INST_FK, (AVM_INST_B != 0)>(bool smemtab, bool wide, bool banded) {
+TransportFn pick_transport_inst<AVM_INST_FK, (AVM_INST_B != 0)>(bool smemtab, bool wide, bool banded, bool signal) {
   constexpr int FK = AVM_INST_FK;
   constexpr bool B = AVM_INST_B != 0;
-  return wide ? pick3<FK, B, kThreadsWide, false>(smemtab, banded) : pick3<FK, B, kThreads, true>(smemtab, banded);
+  return wide ? pick3<FK, B, kThreadsWide, false>(smemtab, banded, signal) : pick3<FK, B, kThreads, true>(smemtab, banded, signal);
 }
 
 }  // namespace avm

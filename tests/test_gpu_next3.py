@@ -168,11 +168,12 @@ def test_next3_full_warps_and_config2_same_seed(avm, ctx, oracle, g0):
     gpu = avm.simulate(ctx, avm.gas_create(ctx, g), avm.field_create(ctx, fd), w.primaries, seed=0, capacity=1 << 20)
     assert cpu.n > 20000
     assert_run_same_seed(cpu, gpu, g.n_levels, min_identical=0.999, label="NEXT-3 config2 field, 80 um gap, 16 primaries")
-    # thermalisation on the device: no field, constant collision frequency, 293 K — <eps> = 3/2 kT (1 - r/2) (oracle pin X3)
+    # thermalisation on the device: no field, constant collision frequency, 293 K — <eps> = thermal_mean (oracle pin X3)
     gt = gas.constant_elastic(400.0, 0.04, n_bins=64, e_max=10.0); gt.kT_eV = 0.02526
     p = primaries.isotropic_primaries(80000, 61, e_scale=1.0)
     fd = fields.uniform_gap((0, 0, 0), -1e6, 1e6)
     r = avm.simulate(ctx, avm.gas_create(ctx, gt), avm.field_create(ctx, fd), p, seed=61, t_max=1.2, capacity=80000)
     e = r.end[4]
-    exact = 1.5 * gt.kT_eV * (1 - 0.02)
+    from test_oracle_pins_next3 import thermal_mean
+    exact = thermal_mean(gt.kT_eV, 0.04)
     assert abs(e.mean() - exact) < 4 * e.std(ddof=1) / np.sqrt(len(e)), (e.mean(), exact)
