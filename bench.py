@@ -34,7 +34,9 @@ UNIT = "collisions/s"
 HEADLINE = "config3s"
 # workload -> (multiplier of --steps, oracle sample = first n primaries; 0 = all).  Oracle samples follow SURVEY.md §8(d)
 # "Oracle timing" (config 3: first primaries only, config 5: first 8), sized for ~1-10 s each on the box's cores.
-ALL = {"config1": (4, 0), "config2": (2, 0), "config3s": (1, 2048), "config4": (1, 0), "config5": (0.5, 8)}
+ALL = {"config1": (4, 0), "config2": (2, 0), "config3s": (1, 2048), "config4": (1, 0), "config5": (0.5, 8),
+       "config5hg": (0.2, -1)}      # not a BASELINE config (D4): config 5's stack at dV = 500 V, 1e4-1e5 electrons per avalanche;
+                                    # -1: no oracle leg (one such avalanche is ~4e9 collisions on one core)
 # Algorithmic FP64 thread-instructions per unit: what the method must do — NOT what
 # the kernel executes (the executed count and the FP64 pipe's busy share come from the ncu capture, when it is current).
 FP64_PER_NULL = {False: 90.0, True: 170.0}       # free flight + energy + bin + decision; key = B != 0
@@ -258,6 +260,8 @@ def run_reference(args) -> None:
             per.append({"workload": name, "value": v, "unit": UNIT, "ms_per_step": line["ms_per_step"], "steps": args.steps,
                         "null_per_s": line["null_per_s"], "real_per_s": line["real_per_s"],
                         "avalanches_per_s": line["avalanches_per_s"], "cpu_baseline": cb})
+        elif sample < 0:
+            continue                                                  # no oracle leg for this workload (see ALL)
         else:
             cb = cpu_baseline_entry(w, sample, cores)
             per.append({"workload": name, "value": cb["value"], "unit": UNIT, "steps": 1, "null_per_s": cb["null_per_s"],
@@ -384,7 +388,7 @@ def bench_workload(avm, ctx, torch, dist, name, steps, warmup, sample, rank, wor
                         "avalanches_per_s": world * w.n_primaries * steps / (bd_ms_max * 1e-3),
                         "electrons_per_step": bd_el / max(steps, 1) / world,
                         "speedup_avalanches_per_s": tot_ms_max / max(bd_ms_max, 1e-9)}}
-    if with_cpu:
+    if with_cpu and sample >= 0:
         entry["cpu_baseline"] = cpu_baseline_entry(w, sample, cores)
     return entry, clocks
 

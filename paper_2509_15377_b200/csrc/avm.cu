@@ -751,6 +751,8 @@ int32_t avm_gas_create(avm_ctx* ctx, const avm_gas_desc* d, void* dev_buf, size_
   g->d.xi = d->scat_xi ? (const double*)(base + lay.xi) : nullptr;
   g->d.kT = d->kT_eV;
   g->d.ext = (d->scat_xi ? 1 : 0) | (d->kT_eV > 0.0 ? 2 : 0);
+  if (d->level_penning_prob)
+    for (int l = 0; l < L; ++l) if (d->level_penning_prob[l] > 0.0) g->d.ext |= 4;
   g->d.bshift = bands.shift; g->d.bK = bands.K; g->d.bJ = bands.J;
   g->d.a0sq = bands.a2[0]; g->d.inv_a0sq = 1.0 / bands.a2[0];
   g->d.band = (const double2*)(base + lay.band);
@@ -967,8 +969,9 @@ int32_t avm_run(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, const 
   const size_t dyn_smem = (smemtab ? tab_bytes : 0) + buf_bytes;
   DevSignal dsig;
   if (!make_signal(opts->signal, dsig)) return AVM_ERR_INVALID_ARG;
-  TransportFn fn = pick_transport(field->fk, field->d.has_B != 0, smemtab, wide, (opts->flags & AVM_RUN_BANDED) != 0, opts->signal != nullptr);
-  if (!fn) return fail(AVM_ERR_INVALID_ARG, "run: a signal needs the threshold table in shared memory (at most ~24000 energy bins)");
+  const bool extras = opts->signal != nullptr || gas->d.ext != 0;     // NEXT-3 / NEXT-4: the kernel variant that has them
+  TransportFn fn = pick_transport(field->fk, field->d.has_B != 0, smemtab, wide, (opts->flags & AVM_RUN_BANDED) != 0, extras);
+  if (!fn) return fail(AVM_ERR_INVALID_ARG, "run: a signal or a gas with NEXT-3 extensions needs the threshold table in shared memory (at most ~24000 energy bins)");
   AVM_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn_smem));
   int occ = 0;
   AVM_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, threads, dyn_smem));

@@ -56,7 +56,9 @@ struct DevGas {
   const double* pen_p;    // [AVM_MAX_LEVELS] transfer probability (0 where none)
   const double* pen_e;    // [AVM_MAX_LEVELS] energy available to the Penning electron
   double kT;              // 0 = cold gas
-  int ext;                // bit 0: xi given, bit 1: kT > 0 — the speculative elastic collision of the time-parallel batches is off
+  int ext;                // bit 0: xi given, bit 1: kT > 0, bit 2: some level has a Penning probability.  Non-zero: collisions
+                          // go through collision_step_ext (kept out of line, so that the base model's register budget is
+                          // untouched) and the speculative elastic collision of the time-parallel batches is off
 };
 
 struct DevSlab {
@@ -391,7 +393,7 @@ __device__ __forceinline__ void flight(const DevField& f, double Ex, double Ey, 
 struct Child { double e, u6, u7; };   // secondary: energy and the two uniforms of its isotropic direction
 
 // Level parameters as the kernels keep them in shared memory: two 16-byte loads per collision.
-struct __align__(16) LevelPar { double loss, recoil, w; int type, pad; double pen_p, pen_e; };
+struct __align__(16) LevelPar { double loss, recoil, w; int type, pad; };
 
 __device__ __forceinline__ void stage_levels(const DevGas& g, LevelPar* s_lv) {
   for (int l = threadIdx.x; l < AVM_MAX_LEVELS; l += blockDim.x) {
@@ -399,7 +401,6 @@ __device__ __forceinline__ void stage_levels(const DevGas& g, LevelPar* s_lv) {
     LevelPar p;
     p.loss = in ? g.loss[l] : 0.0; p.recoil = in ? g.recoil[l] : 0.0; p.w = in ? g.w[l] : 1.0;
     p.type = in ? g.type[l] : 0; p.pad = 0;
-    p.pen_p = in ? g.pen_p[l] : 0.0; p.pen_e = in ? g.pen_e[l] : 0.0;
     s_lv[l] = p;
   }
 }
@@ -673,32 +674,37 @@ __device__ __forceinline__ double elastic_collision(double recoil, const Deflect
 // S9d in velocity form: with s = |v'|, sg = sign(v'z), A = -1/(sg s + v'z), the Duff et al. basis about k' = v'/s scaled
 // by s is  s e1 = (s + sg v'x^2 A, sg v'x v'y A, -sg v'x),  s e2 = (v'x v'y A, sg s + v'y^2 A, -v'y),  so that
 // v'' = (speed''/s) [cos(theta) v' + sin(theta) (cos(phi) s e1 + sin(phi) s e2)] without normalising k' first.
-__device__ __forceinline__ int collision_step(const DevGas& g, const LevelPar* __restrict__ lv, const PhiloxKeys& K,
-                                              uint64_t id, uint32_t n, const Pending& p, bool have_d, Deflection d,
-                                              double& vx, double& vy, double& vz, int& status, bool& spawn, Child& ch,
-                                              double& loss) {
-  const int l = p.lsel < 2 ? p.lsel : select_level_from2(g, p.bin, p.xr);     // S8
-  AVM_CHECK(l >= 0 && l < g.L && p.bin >= 0 && p.bin < g.nb);
+//
+// NEXT-3: with any extension on (g.ext != 0) the whole collision is computed by collision_step_ext, a
+// __noinline__ function that takes and returns everything by value — the base model's code below stays what it was.
+struct CollisionOut { double vx, vy, vz, loss, che, chu6, chu7; int l, status, spawn; };
+
+static __device__ __noinline__ CollisionOut collision_step_ext(const DevGas& g, const LevelPar* __restrict__ lv, const PhiloxKeys& K,
+                                                        uint64_t id, uint32_t n, int lsel, int bin, double xr, bool have_d,
+                                                        Deflection d, double vx, double vy, double vz) {
+  CollisionOut o;
+  o.l = lsel < 2 ? lsel : select_level_from2(g, bin, xr);                     // S8
+  AVM_CHECK(o.l >= 0 && o.l < g.L && bin >= 0 && bin < g.nb);
+  const int l = o.l;
   const LevelPar par = lv[l];
-  status = 0; spawn = false; loss = 0.0;
-  if (par.type == AVM_ATTACHMENT) { status = AVM_ATTACHED; return l; }         // S9a
+  o.status = 0; o.spawn = 0; o.loss = 0.0; o.che = 0.0; o.chu6 = 0.5; o.chu7 = 0.0;
+  o.vx = vx; o.vy = vy; o.vz = vz;
+  if (par.type == AVM_ATTACHMENT) { o.status = AVM_ATTACHED; return o; }       // S9a
   if (!have_d) d = deflection_draws(K, id, n - 1u);                            // S9b
   if (g.xi) {                                     // X1: cos(theta) = (c0 + xi) / (1 + xi c0), sin(theta) cancellation-free
-    const double xi = __ldg(g.xi + (size_t)p.bin * g.L + l);
+    const double xi = __ldg(g.xi + (size_t)bin * g.L + l);
     const double den = 1.0 + xi * d.ct;
     d.st = d.st * sqrt(1.0 - xi * xi) / den;
     d.ct = (d.ct + xi) / den;
   }
   double s2 = vx * vx + vy * vy + vz * vz;
-  if (!(s2 >= 1e-280)) {                          // v' = 0 (never in practice): direction +z, energy at the floor
-    vx = 0.0; vy = 0.0; vz = kC2 * 1e-5; s2 = vz * vz;
-  }
+  if (!(s2 >= 1e-280)) { vx = 0.0; vy = 0.0; vz = kC2 * 1e-5; s2 = vz * vz; }
   double e1 = s2 * kInvC2Sq;
   if (e1 < kEpsFloor) e1 = kEpsFloor;
   double e2;                                                                    // S9c
   if (par.type == AVM_ELASTIC && g.kT > 0.0 && par.recoil > 0.0) {
     // X3: the atom moves with velocity V (normal components, sigma = c2 sqrt(kT r / 4), Box-Muller from blocks 2 and 3);
-    // the cold-gas collision acts on the relative velocity w = v' - V, then V is added back.  Rare path: library math.
+    // the cold-gas collision acts on the relative velocity w = v' - V, then V is added back.  Library math.
     const U4 r2 = philox(K, id, n - 1u, 2u);
     const U4 r3 = philox(K, id, n - 1u, 3u);
     const double u5 = to_unit(r2.w0, r2.w1), u6 = to_unit(r2.w2, r2.w3), u7 = to_unit(r3.w0, r3.w1), u8 = to_unit(r3.w2, r3.w3);
@@ -715,10 +721,73 @@ __device__ __forceinline__ int collision_step(const DevGas& g, const LevelPar* _
     if (ew < kEpsFloor) ew = kEpsFloor;
     const double e2w = ew * (1.0 - par.recoil * (1.0 - d.ct));
     rotate_scale(d, w2, e2w, wx, wy, wz);
-    vx = wx + Vx; vy = wy + Vy; vz = wz + Vz;
-    loss = e1 - fmax((vx * vx + vy * vy + vz * vz) * kInvC2Sq, kEpsFloor);
-    return l;
+    o.vx = wx + Vx; o.vy = wy + Vy; o.vz = wz + Vz;
+    o.loss = e1 - fmax((o.vx * o.vx + o.vy * o.vy + o.vz * o.vz) * kInvC2Sq, kEpsFloor);
+    return o;
   }
+  if (par.type == AVM_ELASTIC) {
+    e2 = e1 * (1.0 - par.recoil * (1.0 - d.ct));
+    o.loss = e1 - e2;
+  } else if (par.type == AVM_EXCITATION) {
+    e2 = e1 - par.loss;
+    if (!(e2 > kEpsFloor)) e2 = kEpsFloor;
+    o.loss = e1 - e2;
+    const double pen_p = __ldg(g.pen_p + l);
+    if (pen_p > 0.0) {                            // X2: Penning transfer — one more electron with probability pen_p
+      const U4 r2 = philox(K, id, n - 1u, 2u);
+      if (to_unit(r2.w0, r2.w1) < pen_p) {
+        const U4 r3 = philox(K, id, n - 1u, 3u);
+        o.chu6 = to_unit(r2.w2, r2.w3);
+        o.chu7 = to_unit(r3.w0, r3.w1);
+        o.che = fmax(to_unit(r3.w2, r3.w3) * __ldg(g.pen_e + l), kEpsFloor);
+        o.spawn = 1;
+      }
+    }
+  } else {   // ionisation: Opal-Peterson-Beaty sharing (R10)
+    const U4 r2 = philox(K, id, n - 1u, 2u);
+    const U4 r3 = philox(K, id, n - 1u, 3u);
+    const double u5 = to_unit(r2.w0, r2.w1);
+    o.chu6 = to_unit(r2.w2, r2.w3);
+    o.chu7 = to_unit(r3.w0, r3.w1);
+    const double ea = fmax(e1 - par.loss, 0.0);
+    const double es = par.w * tan(u5 * atan(ea / (2.0 * par.w)));
+    e2 = fmax(ea - es, kEpsFloor);
+    o.che = fmax(es, kEpsFloor);
+    o.spawn = 1;
+    o.loss = e1 - e2 - o.che;
+  }
+  rotate_scale(d, s2, e2, vx, vy, vz);                                         // S9d
+  o.vx = vx; o.vy = vy; o.vz = vz;
+  return o;
+}
+
+// EXT = the kernel variant that supports the extensions (transport_kernel<.., XTR>; the parity hooks always do): the call
+// is compiled only there — even untaken, it costs the base kernels ~180 bytes of spills in the 80-register launch shape
+// (config 3s: 414 -> 576 ms).
+template <bool EXT = true>
+__device__ __forceinline__ int collision_step(const DevGas& g, const LevelPar* __restrict__ lv, const PhiloxKeys& K,
+                                              uint64_t id, uint32_t n, const Pending& p, bool have_d, Deflection d,
+                                              double& vx, double& vy, double& vz, int& status, bool& spawn, Child& ch,
+                                              double& loss) {
+  if (EXT && g.ext != 0) {
+    const CollisionOut o = collision_step_ext(g, lv, K, id, n, p.lsel, p.bin, p.xr, have_d, d, vx, vy, vz);
+    vx = o.vx; vy = o.vy; vz = o.vz; status = o.status; spawn = o.spawn != 0; loss = o.loss;
+    ch.e = o.che; ch.u6 = o.chu6; ch.u7 = o.chu7;
+    return o.l;
+  }
+  const int l = p.lsel < 2 ? p.lsel : select_level_from2(g, p.bin, p.xr);     // S8
+  AVM_CHECK(l >= 0 && l < g.L && p.bin >= 0 && p.bin < g.nb);
+  const LevelPar par = lv[l];
+  status = 0; spawn = false; loss = 0.0;
+  if (par.type == AVM_ATTACHMENT) { status = AVM_ATTACHED; return l; }         // S9a
+  if (!have_d) d = deflection_draws(K, id, n - 1u);                            // S9b
+  double s2 = vx * vx + vy * vy + vz * vz;
+  if (!(s2 >= 1e-280)) {                          // v' = 0 (never in practice): direction +z, energy at the floor
+    vx = 0.0; vy = 0.0; vz = kC2 * 1e-5; s2 = vz * vz;
+  }
+  double e1 = s2 * kInvC2Sq;
+  if (e1 < kEpsFloor) e1 = kEpsFloor;
+  double e2;                                                                    // S9c
   if (par.type == AVM_ELASTIC) {
     e2 = e1 * (1.0 - par.recoil * (1.0 - d.ct));
     loss = e1 - e2;
@@ -726,16 +795,6 @@ __device__ __forceinline__ int collision_step(const DevGas& g, const LevelPar* _
     e2 = e1 - par.loss;
     if (!(e2 > kEpsFloor)) e2 = kEpsFloor;
     loss = e1 - e2;
-    if (par.pen_p > 0.0) {                        // X2: Penning transfer — one more electron with probability pen_p
-      const U4 r2 = philox(K, id, n - 1u, 2u);
-      if (to_unit(r2.w0, r2.w1) < par.pen_p) {
-        const U4 r3 = philox(K, id, n - 1u, 3u);
-        ch.u6 = to_unit(r2.w2, r2.w3);
-        ch.u7 = to_unit(r3.w0, r3.w1);
-        ch.e = fmax(to_unit(r3.w2, r3.w3) * par.pen_e, kEpsFloor);
-        spawn = true;
-      }
-    }
   } else {   // ionisation: Opal-Peterson-Beaty sharing (R10)
     const U4 r2 = philox(K, id, n - 1u, 2u);
     const U4 r3 = philox(K, id, n - 1u, 3u);

@@ -40,7 +40,8 @@ static_assert(sizeof(WarpBuf) == 1920, "WarpBuf");
 // BANDED (NEXT-1): dt carries -ln(u1); the flight's rate comes from the band of the electron's energy and
 // the class of the field at its position (jcls = the class when the field is one uniform slab), a flight longer than the
 // band's dtmax is cut there and ends in a null collision, and the decision compares u2 nu with the flight's own nu.
-// SIGNAL (NEXT-4): the flight's induced charge -E_w(r) . (r' - r) goes to the bin of its start time.
+// SIGNAL (the extras variant; NEXT-4 when sig->out is set): the flight's induced charge -E_w(r) . (r' - r) goes to the bin
+// of its start time.
 template <int FK, bool HASB, bool TALLY, bool BANDED = false, bool SIGNAL = false>
 __device__ __forceinline__ void fw_flight(const DevGas& g, const DevField& f, const PhiloxKeys& K,
                                           const ushort4* __restrict__ tab, const double2* __restrict__ logtab,
@@ -57,9 +58,9 @@ __device__ __forceinline__ void fw_flight(const DevGas& g, const DevField& f, co
     nu = br.nu; rho = br.rho;
   }
   double sx0 = 0.0, sy0 = 0.0, sz0 = 0.0, st0 = 0.0, swx = 0.0, swy = 0.0, swz = 0.0;
-  if (SIGNAL) { sx0 = x; sy0 = y; sz0 = z; st0 = t; weighting_at(*sig, x, y, z, swx, swy, swz); }
+  if (SIGNAL && sig->out) { sx0 = x; sy0 = y; sz0 = z; st0 = t; weighting_at(*sig, x, y, z, swx, swy, swz); }
   const int b = advance<FK, HASB>(g, f, t_max, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dtf, over);
-  if (SIGNAL) sig_add(*sig, *sacc, -(swx * (x - sx0) + swy * (y - sy0) + swz * (z - sz0)), st0);
+  if (SIGNAL && sig->out) sig_add(*sig, *sacc, -(swx * (x - sx0) + swy * (y - sy0) + swz * (z - sz0)), st0);
   if (b < 0) { fin = -b; return; }
   AVM_CHECK(b < g.nb);
   const ushort4 rec = tab[b];
@@ -165,7 +166,7 @@ __device__ __forceinline__ int tp_batch(const DevGas& g, const DevField& f, cons
       const LevelPar par = s_lv[r == 1 ? 1 : 0];
       fvx = vx; fvy = vy; fvz = vz;
       floss = elastic_collision(par.recoil, dj, s2, fvx, fvy, fvz);
-      fast = ok & ((r == 0) | (r == 1)) & (par.type == AVM_ELASTIC) & (s2 >= 1e-280) & (g.ext == 0);
+      fast = ok & ((r == 0) | (r == 1)) & (par.type == AVM_ELASTIC) & (s2 >= 1e-280) & ((g.ext & 3) == 0);
       if (!ok) {
         b = uniform_exit_status(f, t_max, x, y, z, t);
       } else if (r == -2 || r == 2) {
@@ -178,7 +179,7 @@ __device__ __forceinline__ int tp_batch(const DevGas& g, const DevField& f, cons
     const unsigned evm = __ballot_sync(0xFFFFFFFFu, ev) & gmask;
     const int fl = __ffs(evm) - 1;                       // the group's first step that is not null, or -1
     const bool taken = valid && (fl < 0 || (int)lane <= fl);   // this lane's step is one the electron really takes
-    if (SIGNAL) {
+    if (SIGNAL && sig->out) {
       // the flight of step s starts where step s - 1 ended: the lane kp below (same electron), or the base state
       const double px = __shfl_up_sync(0xFFFFFFFFu, x, kp), py = __shfl_up_sync(0xFFFFFFFFu, y, kp);
       const double pz = __shfl_up_sync(0xFFFFFFFFu, z, kp), pt = __shfl_up_sync(0xFFFFFFFFu, t, kp);
@@ -300,9 +301,9 @@ __device__ __forceinline__ void sb_batch(const DevGas& g, const DevField& f, con
       nu = br.nu; rho = br.rho;
     }
     double sx0 = 0.0, sy0 = 0.0, sz0 = 0.0, st0 = 0.0, swx = 0.0, swy = 0.0, swz = 0.0;
-    if (SIGNAL) { sx0 = x; sy0 = y; sz0 = z; st0 = t; weighting_at(*sig, x, y, z, swx, swy, swz); }
+    if (SIGNAL && sig->out) { sx0 = x; sy0 = y; sz0 = z; st0 = t; weighting_at(*sig, x, y, z, swx, swy, swz); }
     const double s2 = advance_move<FK, HASB>(f, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dtj);   // S3, S4
-    if (SIGNAL) sig_add(*sig, *sacc, -(swx * (x - sx0) + swy * (y - sy0) + swz * (z - sz0)), st0);
+    if (SIGNAL && sig->out) sig_add(*sig, *sacc, -(swx * (x - sx0) + swy * (y - sy0) + swz * (z - sz0)), st0);
     bool over;
     const int b = energy_bin(g, s2, over);                                                     // S6 (counts only when S5 passes)
     AVM_CHECK(b >= 0 && b < g.nb);

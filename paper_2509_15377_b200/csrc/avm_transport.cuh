@@ -114,6 +114,8 @@ constexpr int kCoopMax = AVM_COOP_MAX;
 #ifndef AVM_SB_UNIFORM
 #define AVM_SB_UNIFORM 0     // 1: serial batches instead of time-parallel ones in one uniform slab without B
 #endif
+// SIGNAL = the "extras" variant: NEXT-3 (collision extensions of the gas, DevGas.ext) and NEXT-4 (induced signal, when
+// sig.out is set) are compiled in and selected at run time; the base variant has neither, and its register budget.
 template <int FK, bool HASB, bool TALLY, bool SMEMTAB, int THREADS, bool TPB, bool BANDED, bool SIGNAL>
 __global__ void __launch_bounds__(THREADS, 1)
 transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevField f, const RunArrays a,
@@ -196,14 +198,14 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
     if (pend) {
       double loss;
       int st;
-      l = collision_step(g, s_lv, K, id, n, pc, have_d, dd, vx, vy, vz, st, spawn, ch, loss);
+      l = collision_step<SIGNAL>(g, s_lv, K, id, n, pc, have_d, dd, vx, vy, vz, st, spawn, ch, loss);
       if (st) fin = st;
       if (TALLY) {
         ++tl.real;
         if (l == 0) ++tl.l0;
         else if (l > 1) atomicAdd(&s_hist[l], 1u);
         tl.loss += loss;
-        if (spawn && s_lv[l].type == AVM_EXCITATION) ++tl.pen;       // X2: a Penning transfer
+        if (SIGNAL && spawn && s_lv[l].type == AVM_EXCITATION) ++tl.pen;       // X2: a Penning transfer (extras variant only)
       }
     }
     const unsigned sm = __ballot_sync(mask, spawn);
@@ -356,7 +358,7 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
     a.end[5 * ld + slot] = kx; a.end[6 * ld + slot] = ky; a.end[7 * ld + slot] = kz;
     a.nsteps[slot] = n;
   }
-  if (SIGNAL) sig_flush(sig, sacc);
+  if (SIGNAL && sig.out) sig_flush(sig, sacc);
   if (TALLY) {
     // warp reduce the per-thread counters, one atomic per warp; rare-level histogram per CTA
     unsigned long long v0 = tl.real, v1 = tl.l0, v3 = tl.over, v5 = tl.pen;
@@ -382,9 +384,10 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
 
 typedef void (*TransportFn)(const DevGas, const DevField, const RunArrays, RunCtl*, const PhiloxKeys, const double,
                             const uint32_t, const uint32_t, const DevSignal);
-// Defined (explicit specialisation) in avm_transport_inst.cu, one translation unit per (FK, B).  signal with the threshold
-// table outside shared memory (more than ~24000 energy bins) is not instantiated: nullptr.
+// Defined (explicit specialisation) in avm_transport_inst.cu, one translation unit per (FK, B).  extras = the variant with
+// NEXT-3 / NEXT-4 compiled in; with the threshold table outside shared memory (more than ~24000 energy bins) it is not
+// instantiated: nullptr.
 template <int FK, bool B>
-TransportFn pick_transport_inst(bool smemtab, bool wide, bool banded, bool signal);
+TransportFn pick_transport_inst(bool smemtab, bool wide, bool banded, bool extras);
 
 }  // namespace avm

@@ -79,9 +79,9 @@ GEM_STACK_PITCH = 2060.0e-4                               # foil centres 2 mm + 
 GEM_START_Z = 130.0e-4                                    # 100 um above the top copper surface (z = +30 um)
 
 
-def _gem_slab(e_above: float, e_below: float, z_centre: float, seed: int) -> "fields.Slab":
+def _gem_slab(e_above: float, e_below: float, z_centre: float, seed: int, dv: float = 400.0) -> "fields.Slab":
     from . import gem
-    nodes = gem.gem_nodes(e_above, e_below, 400.0, seed)
+    nodes = gem.gem_nodes(e_above, e_below, dv, seed)
     return fields.grid_slab(nodes, (0.0, 0.0, z_centre + gem.Z0_UM * gem.UM), (gem.UM, gem.UM, gem.UM),
                             z_centre + GEM_Z_HALF_LO, z_centre + GEM_Z_HALF_HI,
                             fields.BC_MIRROR, fields.BC_MIRROR, gem.LX_UM * gem.UM, gem.LY_UM * gem.UM)
@@ -93,16 +93,16 @@ def _gem_primaries(n: int, seed: int, id_offset: int) -> np.ndarray:
                                          xy_box=((0.0, gem.LX_UM * gem.UM), (0.0, gem.LY_UM * gem.UM)))
 
 
-def config4(n_primaries: int = 1000, seed: int = 0, id_offset: int = 0) -> Workload:
+def config4(n_primaries: int = 1000, seed: int = 0, id_offset: int = 0, dv: float = 400.0) -> Workload:
     """Single GEM: 141 x 245 x 600 fp32 map at 1 um, dV = 400 V, 2 kV/cm drift above, 3 kV/cm induction below,
     mirror-periodic in x/y; primaries 100 um above the foil, uniform over the cell; electrons move toward -z."""
-    fd = fields.FieldDesc([_gem_slab(2000.0, 3000.0, 0.0, seed)])
+    fd = fields.FieldDesc([_gem_slab(2000.0, 3000.0, 0.0, seed, dv)])
     return Workload("config4", gas.gas_g0(), fd, _gem_primaries(n_primaries, seed, id_offset), seed, INF,
                     max(256 * n_primaries, 1 << 16),
                     "single GEM map 141x245x600 (331.6 MB), dV=400 V, 2/3 kV/cm, gas G0, primaries 100 um above the foil")
 
 
-def config5(n_primaries: int = 200, seed: int = 0, id_offset: int = 0) -> Workload:
+def config5(n_primaries: int = 200, seed: int = 0, id_offset: int = 0, dv: float = 400.0, name: str = "config5") -> Workload:
     """Triple GEM: three maps (2->3, 3->3, 3->3 kV/cm) whose foil centres are 2.06 mm apart, uniform 3 kV/cm transfer
     slabs between them; slabs ascend in z, GEM1 (the first the electrons meet) on top at z = 0."""
     slabs = []
@@ -110,8 +110,22 @@ def config5(n_primaries: int = 200, seed: int = 0, id_offset: int = 0) -> Worklo
         zc = -(2 - i) * GEM_STACK_PITCH
         if slabs:
             slabs.append(fields.Slab(slabs[-1].z_hi, zc + GEM_Z_HALF_LO, fields.KIND_UNIFORM, (0.0, 0.0, 3000.0)))
-        slabs.append(_gem_slab(ea, eb, zc, seed + (2 - i)))
+        slabs.append(_gem_slab(ea, eb, zc, seed + (2 - i), dv))
     fd = fields.FieldDesc(slabs)
-    return Workload("config5", gas.gas_g0(), fd, _gem_primaries(n_primaries, seed, id_offset), seed, INF,
+    return Workload(name, gas.gas_g0(), fd, _gem_primaries(n_primaries, seed, id_offset), seed, INF,
                     max(200000 * n_primaries, 1 << 20),
-                    "triple GEM: 3 maps 141x245x600 (995 MB), 3 kV/cm transfer gaps, gas G0, primaries 100 um above GEM1")
+                    f"triple GEM: 3 maps 141x245x600 (995 MB), dV={dv:g} V, 3 kV/cm transfer gaps, gas G0, primaries 100 um above GEM1")
+
+
+HG_DV = 500.0
+
+
+def config5hg(n_primaries: int = 8, seed: int = 0, id_offset: int = 0) -> Workload:
+    """High-gain variant of config 5 (NOT a BASELINE config; D4): the same triple-GEM stack with the three maps
+    generated at dV = 500 V instead of 400 V.  BASELINE's config 5 asks for "avalanches of 10^4-10^5 electrons each, stressing
+    secondary append, compaction and occupancy"; with the synthetic gas G0 the stated 400 V gives ~200 electrons per primary
+    (effective gain 3.6 per GEM), 500 V gives ~17 per GEM: 10^4-10^5 electrons per primary (chosen by the oracle on single
+    GEMs: 3.6 / 13 / 37 electrons reach the induction side per primary at 400 / 480 / 540 V)."""
+    w = config5(n_primaries, seed, id_offset, HG_DV, "config5hg")
+    w.capacity = max(400000 * n_primaries, 1 << 21)
+    return w

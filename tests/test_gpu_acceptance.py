@@ -42,8 +42,10 @@ def w_alpha(r, gas, axis_sign):
     return dz / r.tallies_f64[3], (ion - att) / dz
 
 
-def compare_statistics(label, cpu, gpu, far_status, z_far, thin):
-    """Independent streams: gain within 3 combined SE; KS p > 0.01 on gain, endpoint energy and endpoint z overshoot."""
+def compare_statistics(label, cpu, gpu, far_status, z_far, thin, z_overshoot=True):
+    """Independent streams: gain within 3 combined SE; KS p > 0.01 on gain, endpoint energy and endpoint z overshoot.
+    z_overshoot=False: the two sides use different null-collision rates — the endpoint is the first sampled point outside
+    (R13), so the overshoot beyond the plane scales with the last flight's length, i.e. with 1 / nu_hat: not comparable."""
     gc, gg = cpu.per_avalanche[:, 0].astype(float), gpu.per_avalanche[:, 0].astype(float)
     se = np.hypot(gc.std(ddof=1) / np.sqrt(len(gc)), gg.std(ddof=1) / np.sqrt(len(gg)))
     p_gain = stats.ks_2samp(gc, gg).pvalue
@@ -54,7 +56,7 @@ def compare_statistics(label, cpu, gpu, far_status, z_far, thin):
                   f"difference {abs(gc.mean() - gg.mean()) / se:.2f} combined SE; KS p: gain {p_gain:.3f}, endpoint energy {p_e:.3f}, "
                   f"endpoint z {p_z:.3f} ({fc.sum()} / {fg.sum()} far-side electrons, every {thin}th)")
     assert abs(gc.mean() - gg.mean()) < 3 * se, (gc.mean(), gg.mean(), se)
-    assert p_gain > 0.01 and p_e > 0.01 and p_z > 0.01, (p_gain, p_e, p_z)
+    assert p_gain > 0.01 and p_e > 0.01 and (p_z > 0.01 or not z_overshoot), (p_gain, p_e, p_z)
 
 
 def test_config1_acceptance(avm, ctx, oracle):

@@ -144,3 +144,38 @@ def test_config3_drift_lorentz_angle_and_diffusion(avm, ctx, oracle):
     assert Wg[2] > 0 and abs(Wg[0]) > 3 * Wg_se[0]                     # E x B drift along x is resolved
     assert abs(ang(Wg) - ang(Wc)) <= 3 * np.hypot(ang_se(Wg, Wg_se), ang_se(Wc, Wc_se)) + 0.1, (ang(Wg), ang(Wc))
     assert 1.0 < ang(Wg) < 6.0
+
+
+def test_config5hg_high_gain_stack(avm, ctx, oracle):
+    """The high-gain variant of config 5 (D4: the three maps at dV = 500 V; NOT a BASELINE config): avalanches of
+    10^4-10^5 electrons through the three-map stack — the append / refill / occupancy stress BASELINE's config 5 text asks
+    for and the synthetic gas does not deliver at 400 V.  The oracle cannot run it in test time (one avalanche is ~4e9
+    collisions on one core), so: the any-size invariants on every electron of the full run, un-banded and banded, and
+    electron-by-electron parity with the oracle on ONE such GEM (config 4's cell at 500 V, 32 primaries, ~40 electrons each,
+    both rate modes)."""
+    w = configs.config5hg()
+    gpu = run_as_bench(avm, ctx, w)
+    check_invariants(gpu, w)
+    size = gpu.per_avalanche[:, 0].astype(float)
+    assert 5e3 < size.mean() < 3e5 and size.max() > 1e4, size
+    gg, fg = avm.gas_create(ctx, w.gas), avm.field_create(ctx, w.field)
+    bufs = avm.RunBuffers(ctx, w.capacity, w.n_primaries, w.gas.n_levels)
+    _, n = avm.run(ctx, gg, fg, torch.from_numpy(w.primaries.copy()).to(ctx.device), bufs, seed=w.seed, flags=avm.RUN_BANDED)
+    banded = avm.fetch(ctx, bufs, n)
+    check_invariants(banded, w)
+    sb = banded.per_avalanche[:, 0].astype(float)
+    assert 5e3 < sb.mean() < 3e5
+    from conftest import record_margin
+    L = w.gas.n_levels
+    record_margin(f"config5hg (8 primaries, dV 500 V): electrons per avalanche un-banded {sorted(size.astype(int))}, banded {sorted(sb.astype(int))}; "
+                  f"collisions {int(gpu.tallies_u64[L] + gpu.tallies_u64[L + 1])} / {int(banded.tallies_u64[L] + banded.tallies_u64[L + 1])}")
+    del bufs, fg
+    torch.cuda.empty_cache()
+    w4 = configs.config4(n_primaries=32, dv=configs.HG_DV)
+    for flags, oflags in ((0, 0), (avm.RUN_BANDED, 1)):
+        cpu = oracle.run(w4.gas, w4.field, w4.primaries, seed=0, capacity=1 << 18, n_threads=CORES, flags=oflags)
+        g4, f4 = avm.gas_create(ctx, w4.gas), avm.field_create(ctx, w4.field)
+        b4 = avm.RunBuffers(ctx, 1 << 18, 32, L)
+        _, n4 = avm.run(ctx, g4, f4, torch.from_numpy(w4.primaries.copy()).to(ctx.device), b4, seed=0, flags=flags)
+        assert cpu.n > 600
+        assert_run_same_seed(cpu, avm.fetch(ctx, b4, n4), L, min_identical=0.99, end_rtol=3e-6, label=f'single GEM at 500 V, 32 primaries, flags {flags}')

@@ -30,10 +30,11 @@ def _states(n, rng, e_lo=0.01, e_hi=39.0, box=1e-3, center=(0, 0, 0)):
     return st
 
 
-def assert_step_parity(cpu, gpu, st_in, what="", pos_floor=None):
+def assert_step_parity(cpu, gpu, st_in, what="", pos_floor=None, RTOL=RTOL):
     """Tolerance T on one batch of steps.  Returns the number of compared items.
     pos_floor [3, n]: extra lower bound of the position scale (time-parallel batches compose a step's position from a base
-    state up to 32 steps back: its rounding is relative to the coordinate's largest magnitude since that base)."""
+    state up to 32 steps back: its rounding is relative to the coordinate's largest magnitude since that base).
+    RTOL: T = 1e-12 for a step from IDENTICAL state; the batch tests widen it with the step index (assert_form2_parity)."""
     n = st_in.shape[1]
     assert np.array_equal(cpu.event, gpu.event), f"{what}: events differ at {np.flatnonzero(cpu.event != gpu.event)[:5]}"
     assert np.array_equal(cpu.status, gpu.status), what

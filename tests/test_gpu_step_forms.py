@@ -141,7 +141,11 @@ def oracle_sequence(oracle, g, fd, seed, st, ids, n0, gl, t_max):
 def assert_form2_parity(avm, cpu, st_in, gpu, gl, what, composed=False):
     """composed (form 2): a step's position is the composed flight from the batch's base state, so its rounding is relative
     to the coordinate's largest magnitude since the batch began (the oracle's sequential sum carries the same absolute
-    rounding); form 3 steps sequentially and needs no such allowance."""
+    rounding); form 3 steps sequentially and needs no such allowance.
+    Step s of a batch starts from each side's OWN result of step s - 1, not from identical state: the two inputs already
+    differ by the accumulated rounding of s steps (each within T), which the field gradients of a random map carry forward.
+    The bound therefore grows with the step index: T (1 + s / 8) — 1e-12 at the batch's first step, 4.9e-12 at its 32nd
+    (observed worst: 1.2e-12 at step 30 on a random map with B)."""
     assert np.array_equal(cpu.event == -3, gpu.event == -3), f"{what}: the batches reach different steps"
     total = 0
     run_max = np.zeros((3, st_in.shape[1]))
@@ -152,7 +156,8 @@ def assert_form2_parity(avm, cpu, st_in, gpu, gl, what, composed=False):
             continue
         c = type(cpu)(cpu.state[:, sel, s], cpu.event[sel, s], cpu.status[sel, s], cpu.bin[sel, s], cpu.child[:, sel, s], cpu.child_id[sel, s])
         g = type(cpu)(gpu.state[:, sel, s], gpu.event[sel, s], gpu.status[sel, s], gpu.bin[sel, s], gpu.child[:, sel, s], gpu.child_id[sel, s])
-        total += assert_step_parity(c, g, st_in[:, sel, s], f"{what} step {s}", pos_floor=run_max[:, sel] if composed else None)
+        total += assert_step_parity(c, g, st_in[:, sel, s], f"{what} step {s}", pos_floor=run_max[:, sel] if composed else None,
+                                    RTOL=1e-12 * (1.0 + s / 8.0))
     return total
 
 
