@@ -8,6 +8,7 @@
 #include <cmath>
 #include <cstring>
 #include <limits>
+#include <memory>
 #include <string>
 #include <thread>
 #include <vector>
@@ -199,8 +200,125 @@ bool check_field(const avmo_field_desc* f) {
       if (s.bc_x < 0 || s.bc_x > 2 || s.bc_y < 0 || s.bc_y > 2) { g_err = "field: bc"; return false; }
       if (s.bc_x && !(s.period_x > 0 && s.period_x <= (s.nx - 1) * s.spacing[0] * (1 + 1e-12))) { g_err = "field: period_x"; return false; }
       if (s.bc_y && !(s.period_y > 0 && s.period_y <= (s.ny - 1) * s.spacing[1] * (1 + 1e-12))) { g_err = "field: period_y"; return false; }
+    } else if (s.kind == 2) {
+      if (s.n_tets < 1 || s.n_mesh_nodes < 4 || !s.node_xyz || !s.node_V || !s.tet_nodes || !s.tet_gas) { g_err = "field: mesh arrays"; return false; }
+      for (int64_t i = 0; i < s.n_tets * 10; ++i) if (s.tet_nodes[i] < 0 || s.tet_nodes[i] >= s.n_mesh_nodes) { g_err = "field: mesh node index"; return false; }
+      if (s.bc_x < 0 || s.bc_x > 2 || s.bc_y < 0 || s.bc_y > 2) { g_err = "field: bc"; return false; }
+      if ((s.bc_x && !(s.period_x > 0)) || (s.bc_y && !(s.period_y > 0))) { g_err = "field: period"; return false; }
     } else if (s.kind != 0) { g_err = "field: kind"; return false; }
   }
+  return true;
+}
+
+// ---- NEXT-2: unstructured tetrahedral maps ----------------------------------------------------------
+// F2: the element that contains a point.  Definition: element e contains r when its four barycentric coordinates are all
+// >= -1e-10 (interior points belong to exactly one element; on a shared face, the lowest index wins).  Brute force over
+// all elements is that definition; the bucket grid below only skips elements whose bounding box cannot contain r, and
+// keeps each bucket's candidates in ascending order, so it returns the same element (pinned against brute force).
+const double TET_TOL = 1e-10;
+
+// barycentric coordinates of r in the tetrahedron with vertices p[0..3] (Cramer's rule on the edge matrix)
+bool barycentric(const double* p0, const double* p1, const double* p2, const double* p3, const double r[3], double lam[4]) {
+  const double a[3] = {p0[0] - p3[0], p0[1] - p3[1], p0[2] - p3[2]};
+  const double b[3] = {p1[0] - p3[0], p1[1] - p3[1], p1[2] - p3[2]};
+  const double c[3] = {p2[0] - p3[0], p2[1] - p3[1], p2[2] - p3[2]};
+  const double q[3] = {r[0] - p3[0], r[1] - p3[1], r[2] - p3[2]};
+  auto det3 = [](const double* u, const double* v, const double* w) {
+    return u[0] * (v[1] * w[2] - v[2] * w[1]) - u[1] * (v[0] * w[2] - v[2] * w[0]) + u[2] * (v[0] * w[1] - v[1] * w[0]);
+  };
+  const double D = det3(a, b, c);
+  if (D == 0.0) return false;
+  lam[0] = det3(q, b, c) / D;
+  lam[1] = det3(a, q, c) / D;
+  lam[2] = det3(a, b, q) / D;
+  lam[3] = 1.0 - lam[0] - lam[1] - lam[2];
+  return true;
+}
+
+struct MeshIndex {
+  double lo[3], inv[3];
+  int n[3];
+  std::vector<int64_t> off;
+  std::vector<int32_t> list;
+};
+
+std::unique_ptr<MeshIndex> build_mesh_index(const avmo_slab& s) {
+  auto M = std::make_unique<MeshIndex>();
+  double hi[3];
+  for (int a = 0; a < 3; ++a) { M->lo[a] = 1e300; hi[a] = -1e300; }
+  for (int64_t e = 0; e < s.n_tets; ++e)
+    for (int v = 0; v < 4; ++v)
+      for (int a = 0; a < 3; ++a) {
+        const double x = s.node_xyz[3 * (size_t)s.tet_nodes[10 * e + v] + a];
+        M->lo[a] = std::min(M->lo[a], x); hi[a] = std::max(hi[a], x);
+      }
+  const double per_axis = std::cbrt((double)s.n_tets / 4.0);
+  for (int a = 0; a < 3; ++a) {
+    const double ext = std::max(hi[a] - M->lo[a], 1e-300);
+    const double vol_share = ext / std::cbrt(std::max((hi[0] - M->lo[0]) * (hi[1] - M->lo[1]) * (hi[2] - M->lo[2]), 1e-300));
+    M->n[a] = std::max(1, std::min(512, (int)(per_axis * vol_share)));
+    M->inv[a] = M->n[a] / ext;
+  }
+  const size_t nc = (size_t)M->n[0] * M->n[1] * M->n[2];
+  std::vector<std::vector<int32_t>> buckets(nc);
+  for (int64_t e = 0; e < s.n_tets; ++e) {                     // ascending e: every bucket's list is ascending
+    int c0[3], c1[3];
+    for (int a = 0; a < 3; ++a) {
+      double mn = 1e300, mx = -1e300;
+      for (int v = 0; v < 4; ++v) { const double x = s.node_xyz[3 * (size_t)s.tet_nodes[10 * e + v] + a]; mn = std::min(mn, x); mx = std::max(mx, x); }
+      const double pad = 1e-9 * (mx - mn) + 1e-300;
+      c0[a] = std::max(0, std::min(M->n[a] - 1, (int)std::floor((mn - pad - M->lo[a]) * M->inv[a])));
+      c1[a] = std::max(0, std::min(M->n[a] - 1, (int)std::floor((mx + pad - M->lo[a]) * M->inv[a])));
+    }
+    for (int k = c0[2]; k <= c1[2]; ++k) for (int j = c0[1]; j <= c1[1]; ++j) for (int i = c0[0]; i <= c1[0]; ++i)
+      buckets[((size_t)k * M->n[1] + j) * M->n[0] + i].push_back((int32_t)e);
+  }
+  M->off.assign(nc + 1, 0);
+  for (size_t c = 0; c < nc; ++c) M->off[c + 1] = M->off[c] + (int64_t)buckets[c].size();
+  M->list.reserve((size_t)M->off[nc]);
+  for (auto& b : buckets) M->list.insert(M->list.end(), b.begin(), b.end());
+  return M;
+}
+
+// An avmo_field_desc with the mesh indices of its kind-2 slabs (built once per entry call).
+struct PreparedField : avmo_field_desc {
+  std::vector<std::unique_ptr<MeshIndex>> mesh;
+  bool prepared = true;
+  explicit PreparedField(const avmo_field_desc* f) : avmo_field_desc(*f) {
+    mesh.resize(f->n_slabs);
+    for (int i = 0; i < f->n_slabs; ++i) if (f->slabs[i].kind == 2) mesh[i] = build_mesh_index(f->slabs[i]);
+  }
+};
+
+// F1: potential gradient of a 10-node tetrahedron at barycentric point lam; element test and evaluation in one.
+// Returns true when the element contains r.
+bool tet_eval(const avmo_slab& s, int64_t e, const double r[3], double E[3], double& mask) {
+  const int32_t* nd = s.tet_nodes + 10 * e;
+  const double* p[4];
+  for (int v = 0; v < 4; ++v) p[v] = s.node_xyz + 3 * (size_t)nd[v];
+  double lam[4];
+  if (!barycentric(p[0], p[1], p[2], p[3], r, lam)) return false;
+  for (int v = 0; v < 4; ++v) if (!(lam[v] >= -TET_TOL)) return false;
+  // grad lambda_a: lambda is affine; recover its gradient from unit displacements
+  double g[4][3];
+  for (int a = 0; a < 3; ++a) {
+    double rp[3] = {r[0], r[1], r[2]}, lp[4];
+    rp[a] += 1.0;
+    barycentric(p[0], p[1], p[2], p[3], rp, lp);
+    for (int v = 0; v < 4; ++v) g[v][a] = lp[v] - lam[v];
+  }
+  static const int EA[6] = {0, 0, 0, 1, 1, 2}, EB[6] = {1, 2, 3, 2, 3, 3};
+  double grad[3] = {0.0, 0.0, 0.0};
+  for (int v = 0; v < 4; ++v) {
+    const double c = s.node_V[nd[v]] * (4.0 * lam[v] - 1.0);                    // d/dl [l (2l - 1)] = 4l - 1
+    for (int a = 0; a < 3; ++a) grad[a] += c * g[v][a];
+  }
+  for (int k = 0; k < 6; ++k) {
+    const double V = 4.0 * s.node_V[nd[4 + k]];                                 // N = 4 l_a l_b
+    for (int a = 0; a < 3; ++a) grad[a] += V * (lam[EB[k]] * g[EA[k]][a] + lam[EA[k]] * g[EB[k]][a]);
+  }
+  E[0] = -grad[0]; E[1] = -grad[1]; E[2] = -grad[2];
+  mask = s.tet_gas[e] ? 1.0 : 0.0;
   return true;
 }
 
@@ -239,6 +357,32 @@ int field_at(const avmo_field_desc* f, double x, double y, double z, double E[3]
   for (int i = 0; i < ns; ++i) if (z < S[i].z_hi) { si = i; break; }
   const avmo_slab& s = S[si];
   if (s.kind == 0) { E[0] = s.E[0]; E[1] = s.E[1]; E[2] = s.E[2]; mask = 1.0; return si; }
+  if (s.kind == 2) {
+    // F3: fold x, y as for a grid (bc none: no fold and no range: a point in no element is solid), look the element up
+    double qx = x - s.origin[0], qy = y - s.origin[1];
+    bool fx = false, fy = false;
+    if (s.bc_x) fold(x, s.origin[0], 1.0, 2, s.bc_x, s.period_x, qx, fx);
+    if (s.bc_y) fold(y, s.origin[1], 1.0, 2, s.bc_y, s.period_y, qy, fy);
+    const double r[3] = {qx, qy, z - s.origin[2]};
+    const MeshIndex& M = *static_cast<const PreparedField*>(f)->mesh[si];
+    E[0] = E[1] = E[2] = 0.0; mask = 0.0;
+    int c[3];
+    bool inside = true;
+    for (int a = 0; a < 3; ++a) {
+      const double u = (r[a] - M.lo[a]) * M.inv[a];
+      c[a] = (int)std::floor(u);
+      if (c[a] == M.n[a] && u <= (double)M.n[a] * (1.0 + 1e-12)) c[a] = M.n[a] - 1;
+      if (c[a] < 0 || c[a] >= M.n[a]) inside = false;
+    }
+    if (inside) {
+      const size_t cell = ((size_t)c[2] * M.n[1] + c[1]) * M.n[0] + c[0];
+      for (int64_t q = M.off[cell]; q < M.off[cell + 1]; ++q)
+        if (tet_eval(s, M.list[q], r, E, mask)) break;
+    }
+    if (fx) E[0] = -E[0];
+    if (fy) E[1] = -E[1];
+    return si;
+  }
   double qx, qy; bool fx, fy;
   if (!fold(x, s.origin[0], s.spacing[0], s.nx, s.bc_x, s.period_x, qx, fx)) return -AVMO_LEFT_XY;
   if (!fold(y, s.origin[1], s.spacing[1], s.ny, s.bc_y, s.period_y, qy, fy)) return -AVMO_LEFT_XY;
@@ -564,6 +708,8 @@ void avmo_uniform_pair(uint64_t seed, uint64_t id, uint32_t n, uint32_t block, d
 
 int32_t avmo_field_eval(const avmo_field_desc* f, int64_t n, const double* r, double* E, double* mask, int32_t* slab) {
   if (!check_field(f) || n < 0 || !r || !E || !mask || !slab) return AVMO_ERR_INVALID_ARG;
+  const PreparedField pf(f);
+  f = &pf;
   for (int64_t i = 0; i < n; ++i) {
     double e[3] = {0, 0, 0}, m = 0;
     int si = field_at(f, r[i], r[n + i], r[2 * n + i], e, m);
@@ -578,6 +724,8 @@ int32_t avmo_step_batch(const avmo_gas_desc* gd, const avmo_field_desc* f, uint6
   Gas g;
   if (!load_gas(gd, g) || !check_field(f)) return AVMO_ERR_INVALID_ARG;
   if (n < 0 || !in || !id || !n_idx || !out || !event || !status || !bin || !child || !child_id) { g_err = "step_batch: null"; return AVMO_ERR_INVALID_ARG; }
+  const PreparedField pf(f);
+  f = &pf;
   StepOut so;
   for (int64_t i = 0; i < n; ++i) {
     Electron el;
@@ -606,6 +754,11 @@ int32_t avmo_ion_drift(const avmo_field_desc* f, const avmo_signal* sg, const av
   if (!check_field(f) || !io || n < 0 || !birth || !end || !status || !ion_end || !ion_status || !ion_steps) { g_err = "ion_drift: null"; return AVMO_ERR_INVALID_ARG; }
   if (!(io->step_cm > 0) || !(io->mobility_pos > 0) || !(io->mobility_neg > 0) || io->max_steps < 1) { g_err = "ion_drift: options"; return AVMO_ERR_INVALID_ARG; }
   if (sg && (!sg->weighting || !check_field(sg->weighting) || !(sg->dt_bin > 0) || sg->n_bins < 1 || !sg->signal)) { g_err = "ion_drift: signal description"; return AVMO_ERR_INVALID_ARG; }
+  const PreparedField pf(f);
+  f = &pf;
+  std::unique_ptr<PreparedField> pw;
+  avmo_signal sg_local;
+  if (sg) { pw = std::make_unique<PreparedField>(sg->weighting); sg_local = *sg; sg_local.weighting = pw.get(); sg = &sg_local; }
   const int64_t N = 2 * n;
   for (int64_t i = 0; i < N; ++i) {
     const int64_t s = i < n ? i : i - n;
@@ -665,6 +818,11 @@ int32_t avmo_run(const avmo_gas_desc* gd, const avmo_field_desc* f, const double
   for (auto& t : tl) t.level.assign(g.L, 0);
   const avmo_signal* sg = opts->signal;
   if (sg && (!sg->weighting || !check_field(sg->weighting) || !(sg->dt_bin > 0) || sg->n_bins < 1 || !sg->signal)) { g_err = "run: signal description"; return AVMO_ERR_INVALID_ARG; }
+  const PreparedField pf(f);
+  f = &pf;
+  std::unique_ptr<PreparedField> pw;
+  avmo_signal sg_local;
+  if (sg) { pw = std::make_unique<PreparedField>(sg->weighting); sg_local = *sg; sg_local.weighting = pw.get(); sg = &sg_local; }
   std::vector<std::vector<double>> sacc(nt);
   if (sg) for (auto& a : sacc) a.assign(sg->n_bins, 0.0);
   if (nt == 1) {

@@ -52,6 +52,17 @@ typedef struct {
   int32_t nx, ny, nz;  double origin[3], spacing[3];
   int32_t bc_x, bc_y;                          /* 0 none, 1 periodic, 2 mirror */
   double period_x, period_y;
+  /* kind 2 (NEXT-2; DESIGN.md §3.8 readings F1-F4): an unstructured mesh of 10-node (quadratic)
+   * tetrahedra with straight edges, as ANSYS SOLID123 exports them.  Coordinates are relative to `origin`
+   * (x, y after the fold of bc_x / bc_y, as for a grid).  tet_nodes[e] = 4 vertices then the mid-edge nodes of edges
+   * (0,1) (0,2) (0,3) (1,2) (1,3) (2,3); node_V = potential [V] at every node; tet_gas[e] = 1 gas, 0 solid.  Inside an
+   * element V = sum_i V_i N_i(lambda), N_vertex = l(2l - 1), N_edge = 4 l_a l_b, E = -grad V; the mask is the element's flag;
+   * a point of the slab inside no element is solid (an unmeshed electrode). */
+  int64_t n_mesh_nodes, n_tets;
+  const double* node_xyz;                      /* [n_mesh_nodes][3] */
+  const double* node_V;                        /* [n_mesh_nodes] */
+  const int32_t* tet_nodes;                    /* [n_tets][10] */
+  const uint8_t* tet_gas;                      /* [n_tets] */
 } avmo_slab;
 
 typedef struct { const avmo_slab* slabs; int32_t n_slabs; double B[3]; double xy_lo[2], xy_hi[2]; } avmo_field_desc;

@@ -40,7 +40,9 @@ class SlabDesc(C.Structure):
     _fields_ = [("z_lo", C.c_double), ("z_hi", C.c_double), ("kind", C.c_int32), ("E", C.c_double * 3),
                 ("nodes", C.c_void_p), ("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
                 ("origin", C.c_double * 3), ("spacing", C.c_double * 3), ("bc_x", C.c_int32), ("bc_y", C.c_int32),
-                ("period_x", C.c_double), ("period_y", C.c_double)]
+                ("period_x", C.c_double), ("period_y", C.c_double),
+                ("n_mesh_nodes", C.c_int64), ("n_tets", C.c_int64), ("node_xyz", C.c_void_p), ("node_V", C.c_void_p),
+                ("tet_nodes", C.c_void_p), ("tet_gas", C.c_void_p)]
 
 
 class FieldDescC(C.Structure):
@@ -135,6 +137,13 @@ def field_desc(field) -> tuple:
         a.origin[:] = s.origin
         a.spacing[:] = s.spacing
         a.bc_x, a.bc_y, a.period_x, a.period_y = s.bc_x, s.bc_y, s.period_x, s.period_y
+        m = getattr(s, "mesh", None)
+        if m is not None:                       # kind 2: unstructured tetrahedral map (NEXT-2)
+            xyz = np.ascontiguousarray(m.node_xyz, dtype=np.float64); v = np.ascontiguousarray(m.node_V, dtype=np.float64)
+            tn = np.ascontiguousarray(m.tet_nodes, dtype=np.int32); tg = np.ascontiguousarray(m.tet_gas, dtype=np.uint8)
+            k.refs += [xyz, v, tn, tg]
+            a.n_mesh_nodes, a.n_tets = xyz.shape[0], tn.shape[0]
+            a.node_xyz, a.node_V, a.tet_nodes, a.tet_gas = _p(xyz).value, _p(v).value, _p(tn).value, _p(tg).value
     k.refs.append(arr)
     d = FieldDescC(arr, n, (C.c_double * 3)(*field.B), (C.c_double * 2)(*field.xy_lo), (C.c_double * 2)(*field.xy_hi))
     return d, k

@@ -25,6 +25,9 @@ namespace avm {
 #ifndef AVM_FLIGHTS
 #define AVM_FLIGHTS 2
 #endif
+#ifndef AVM_TICKET_PACK
+#define AVM_TICKET_PACK 1
+#endif
 #ifndef AVM_COOP_MAX
 #define AVM_COOP_MAX 8
 #endif
@@ -150,7 +153,8 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
   // static tickets, CTA-major then warp then lane: the first electrons go one per warp, spread over all SMs (packing them
   // into one warp per scheduler instead was measured slower on the map configs: DESIGN.md §7)
   constexpr int kWarpsPerCta = THREADS / 32;
-  uint32_t ticket = (lane * kWarpsPerCta + warp) * gridDim.x + blockIdx.x;
+  constexpr uint32_t kPack = AVM_TICKET_PACK;
+  uint32_t ticket = (((lane / kPack) * kWarpsPerCta + warp) * kPack + lane % kPack) * gridDim.x + blockIdx.x;
   bool have = false, dvalid = false;
   double x = 0, y = 0, z = 0, t = 0, vx = 0, vy = 0, vz = 0, Ex = 0, Ey = 0, Ez = 0, dt = 0;
   uint2 u2w = make_uint2(0u, 0u);

@@ -11,9 +11,20 @@ from typing import Optional
 
 import numpy as np
 
-KIND_UNIFORM, KIND_GRID = 0, 1
+KIND_UNIFORM, KIND_GRID, KIND_TETMESH = 0, 1, 2
 BC_NONE, BC_PERIODIC, BC_MIRROR = 0, 1, 2
 INF = float("inf")
+
+
+@dataclass
+class TetMesh:
+    """Unstructured mesh of 10-node (quadratic, straight-edged) tetrahedra with node potentials (NEXT-2; the element type
+    of the paper's ANSYS maps).  tet_nodes[e] = 4 vertices, then the mid-edge nodes of edges (0,1) (0,2) (0,3)
+    (1,2) (1,3) (2,3).  Coordinates are relative to the slab's origin."""
+    node_xyz: np.ndarray        # [n_nodes, 3] float64, cm
+    node_V: np.ndarray          # [n_nodes] float64, volt
+    tet_nodes: np.ndarray       # [n_tets, 10] int32
+    tet_gas: np.ndarray         # [n_tets] uint8: 1 gas, 0 solid
 
 
 @dataclass
@@ -29,6 +40,7 @@ class Slab:
     bc_y: int = BC_NONE
     period_x: float = 0.0
     period_y: float = 0.0
+    mesh: Optional[TetMesh] = None           # kind 2
 
     @property
     def shape(self):
@@ -56,3 +68,8 @@ def grid_slab(nodes, origin, spacing, z_lo, z_hi, bc_x=BC_NONE, bc_y=BC_NONE, pe
     assert nodes.ndim == 4 and nodes.shape[3] == 4
     return Slab(float(z_lo), float(z_hi), KIND_GRID, (0.0, 0.0, 0.0), nodes, tuple(map(float, origin)),
                 tuple(map(float, spacing)), int(bc_x), int(bc_y), float(period_x), float(period_y))
+
+
+def tet_slab(mesh: TetMesh, origin, z_lo, z_hi, bc_x=BC_NONE, bc_y=BC_NONE, period_x=0.0, period_y=0.0) -> Slab:
+    return Slab(float(z_lo), float(z_hi), KIND_TETMESH, (0.0, 0.0, 0.0), None, tuple(map(float, origin)), (1.0, 1.0, 1.0),
+                int(bc_x), int(bc_y), float(period_x), float(period_y), mesh)
