@@ -94,7 +94,7 @@ double avm_gas_nu_hat(const avm_gas*);
 int32_t avm_gas_bands(const avm_gas*, int32_t* shape3, double* a2, double* nu, double* dtmax);
 
 /* ---- field: uniform, uniform + B, or regular-grid map(s) (S0, R14, R15) ---------------------------------
- * A stack of z-slabs, ascending and contiguous (slab[i].z_hi == slab[i+1].z_lo).  kind 0: uniform field
+ * A stack of z-slabs, ascending and contiguous (slab[i].z_hi == slab[i+1].z_lo).  kind 2: see below.  kind 0: uniform field
  * vector E (the force on an electron is -E).  kind 1: regular grid of float4 nodes (Ex, Ey, Ez, gas-mask)
  * laid out [nz][ny][nx][4], trilinear interpolation (x, then y, then z); mask < 0.5 = solid material, the
  * electron is absorbed (R14).  bc 0: leaving the grid in x/y ends the electron (status 3); 1: periodic with
@@ -114,7 +114,25 @@ typedef struct {
                                    * avm_field_destroy.  When given, avm_field_create widens the fp32 map into it once
                                    * (same values) and lookups read it: no float-to-double conversion per step, twice
                                    * the bytes.  Results are identical either way. */
+  /* kind 2 (NEXT-2: SURVEY.md §8(f), DESIGN.md §3.8 readings F1-F4; PAPER.md:121 — the paper's maps are ANSYS meshes of
+   * 10-node tetrahedra, found through an octree): an unstructured mesh of quadratic tetrahedra with straight
+   * edges.  Coordinates are relative to `origin`, x and y after the fold of bc_x / bc_y (as for a grid; bc none: no fold).
+   * tet_nodes[e] = 4 vertices, then the mid-edge nodes of edges (0,1) (0,2) (0,3) (1,2) (1,3) (2,3); node_V = potential
+   * [V] at every node.  Inside an element V = sum_i V_i N_i(lambda) (N_vertex = l (2l - 1), N_edge = 4 l_a l_b), E = -grad V,
+   * the mask is tet_gas[e] (1 gas, 0 solid); the element of a point is the lowest-numbered one whose barycentric
+   * coordinates are all >= -1e-10; a point of the slab inside no element is solid (an unmeshed electrode).  The four host
+   * arrays are read by avm_field_create only; mesh_dev (DEVICE, >= avm_tetmesh_bytes(slab), 256-byte aligned) receives the
+   * per-element records and the bucket-grid index and is borrowed until avm_field_destroy. */
+  int64_t n_mesh_nodes, n_tets;
+  const double* node_xyz;         /* HOST [n_mesh_nodes][3] */
+  const double* node_V;           /* HOST [n_mesh_nodes] */
+  const int32_t* tet_nodes;       /* HOST [n_tets][10] */
+  const uint8_t* tet_gas;         /* HOST [n_tets] */
+  void* mesh_dev;
+  size_t mesh_dev_bytes;
 } avm_slab;
+/* Bytes of device memory avm_field_create needs for the mesh of a kind-2 slab (0 for other kinds or an invalid mesh). */
+size_t avm_tetmesh_bytes(const avm_slab*);
 typedef struct {
   const avm_slab* slabs;          /* host [n_slabs], 1..AVM_MAX_SLABS */
   int32_t n_slabs;

@@ -25,7 +25,7 @@ OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_CUDA, ERR_STATE = 0, -1, -2, -3, -4
 RUN_PRIMARIES_ON_DEVICE, RUN_NO_TALLIES, RUN_SHAPE_WIDE, RUN_SHAPE_LATENCY, RUN_BANDED = 1, 2, 4, 8, 16
 MAX_LEVELS, MAX_SLABS = 64, 8
 EXPORTS = ["avm_last_error", "avm_ctx_create", "avm_ctx_destroy", "avm_ctx_sm_count", "avm_gas_bytes",
-           "avm_gas_create", "avm_gas_destroy", "avm_gas_nu_hat", "avm_gas_bands", "avm_field_create", "avm_field_destroy",
+           "avm_gas_create", "avm_gas_destroy", "avm_gas_nu_hat", "avm_gas_bands", "avm_field_create", "avm_field_destroy", "avm_tetmesh_bytes",
            "avm_field_eval", "avm_run_workspace_bytes", "avm_run", "avm_run_stats", "avm_run_transport_ms", "avm_fetch", "avm_ion_drift", "avm_step_batch", "avm_step_batch_form",
            "avm_philox_batch", "avm_fp64_probe", "avm_gather_probe", "avm_smem_probe"]
 
@@ -48,7 +48,9 @@ class _Slab(C.Structure):
     _fields_ = [("z_lo", C.c_double), ("z_hi", C.c_double), ("kind", C.c_int32), ("E", C.c_double * 3),
                 ("nodes_dev", C.c_void_p), ("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
                 ("origin", C.c_double * 3), ("spacing", C.c_double * 3), ("bc_x", C.c_int32), ("bc_y", C.c_int32),
-                ("period_x", C.c_double), ("period_y", C.c_double), ("nodes_f64_dev", C.c_void_p)]
+                ("period_x", C.c_double), ("period_y", C.c_double), ("nodes_f64_dev", C.c_void_p),
+                ("n_mesh_nodes", C.c_int64), ("n_tets", C.c_int64), ("node_xyz", C.c_void_p), ("node_V", C.c_void_p),
+                ("tet_nodes", C.c_void_p), ("tet_gas", C.c_void_p), ("mesh_dev", C.c_void_p), ("mesh_dev_bytes", C.c_size_t)]
 
 
 class _FieldDesc(C.Structure):
@@ -81,6 +83,8 @@ class _Outputs(C.Structure):
 
 _lib.avm_last_error.restype = C.c_char_p
 _lib.avm_gas_bytes.restype = C.c_size_t
+_lib.avm_tetmesh_bytes.restype = C.c_size_t
+_lib.avm_tetmesh_bytes.argtypes = [C.c_void_p]
 _lib.avm_run_workspace_bytes.restype = C.c_size_t
 _lib.avm_run_workspace_bytes.argtypes = [C.c_void_p, C.c_int64]
 _lib.avm_gas_nu_hat.restype = C.c_double
@@ -250,6 +254,20 @@ class Field:
             a.origin[:] = s.origin
             a.spacing[:] = s.spacing
             a.bc_x, a.bc_y, a.period_x, a.period_y = s.bc_x, s.bc_y, s.period_x, s.period_y
+            m = getattr(s, "mesh", None)
+            if m is not None:                   # kind 2: host arrays in, device buffer sized by the library (NEXT-2)
+                host = [np.ascontiguousarray(m.node_xyz, dtype=np.float64), np.ascontiguousarray(m.node_V, dtype=np.float64),
+                        np.ascontiguousarray(m.tet_nodes, dtype=np.int32), np.ascontiguousarray(m.tet_gas, dtype=np.uint8)]
+                self.nodes.append(host)
+                a.n_mesh_nodes, a.n_tets = host[0].shape[0], host[2].shape[0]
+                a.node_xyz, a.node_V, a.tet_nodes, a.tet_gas = (_hp(x).value for x in host)
+                nbytes = int(_lib.avm_tetmesh_bytes(C.byref(a)))
+                if nbytes == 0:
+                    raise AvmError(ERR_INVALID_ARG, "field: invalid mesh: " + last_error())
+                buf = ctx.empty(nbytes, torch.uint8)
+                self.wide.append(buf)
+                self.map_bytes += nbytes
+                a.mesh_dev, a.mesh_dev_bytes = buf.data_ptr(), nbytes
         d = _FieldDesc(arr, n, (C.c_double * 3)(*desc.B), (C.c_double * 2)(*desc.xy_lo), (C.c_double * 2)(*desc.xy_hi))
         self._h = C.c_void_p()
         _check(_lib.avm_field_create(ctx._h, C.byref(d), C.byref(self._h)))

@@ -545,6 +545,95 @@ GasLayout gas_layout(int nb, int L, bool with_xi) {
 }
 
 
+// NEXT-2: device form of a kind-2 slab — per element a 24-double record (vertex 3, the rows of the inverse
+// edge matrix, the ten node potentials, the gas flag) and a bucket grid over the mesh's bounding box whose cells list, in
+// ascending order, the elements whose bounding boxes touch them.  Layout in the caller's buffer: records | offsets | list.
+struct MeshLayout { size_t rec, off, list, total; int n[3]; double lo[3], inv[3]; std::vector<int> counts; };
+bool mesh_plan(const avm_slab& s, MeshLayout& L, std::vector<std::vector<int>>* buckets) {
+  if (s.n_tets < 1 || s.n_tets > 0x7FFFFFFFll / 24 || s.n_mesh_nodes < 4 || !s.node_xyz || !s.node_V || !s.tet_nodes || !s.tet_gas) { g_err = "field: mesh arrays"; return false; }
+  const int64_t nt = s.n_tets;
+  for (int64_t i = 0; i < nt * 10; ++i) if (s.tet_nodes[i] < 0 || s.tet_nodes[i] >= s.n_mesh_nodes) { g_err = "field: mesh node index out of range"; return false; }
+  double hi[3];
+  for (int a = 0; a < 3; ++a) { L.lo[a] = std::numeric_limits<double>::infinity(); hi[a] = -L.lo[a]; }
+  for (int64_t e = 0; e < nt; ++e)
+    for (int v = 0; v < 4; ++v)
+      for (int a = 0; a < 3; ++a) {
+        const double x = s.node_xyz[3 * (size_t)s.tet_nodes[10 * e + v] + a];
+        if (x < L.lo[a]) L.lo[a] = x;
+        if (x > hi[a]) hi[a] = x;
+      }
+  // about two elements per cell on average, cells as cubic as the box allows
+  double ext[3], vol = 1.0;
+  for (int a = 0; a < 3; ++a) { ext[a] = hi[a] - L.lo[a]; if (!(ext[a] > 0.0)) { g_err = "field: degenerate mesh"; return false; } vol *= ext[a]; }
+  const double cell = std::cbrt(vol / (0.5 * (double)nt));
+  size_t nc = 1;
+  for (int a = 0; a < 3; ++a) {
+    int n = (int)std::ceil(ext[a] / cell);
+    L.n[a] = n < 1 ? 1 : (n > 1024 ? 1024 : n);
+    L.inv[a] = (double)L.n[a] / ext[a];
+    nc *= (size_t)L.n[a];
+  }
+  L.counts.assign(nc, 0);
+  if (buckets) buckets->assign(nc, {});
+  size_t total = 0;
+  for (int64_t e = 0; e < nt; ++e) {
+    int c0[3], c1[3];
+    for (int a = 0; a < 3; ++a) {
+      double mn = std::numeric_limits<double>::infinity(), mx = -mn;
+      for (int v = 0; v < 4; ++v) { const double x = s.node_xyz[3 * (size_t)s.tet_nodes[10 * e + v] + a]; if (x < mn) mn = x; if (x > mx) mx = x; }
+      const double pad = 1e-9 * (mx - mn);
+      const int i0 = (int)std::floor((mn - pad - L.lo[a]) * L.inv[a]), i1 = (int)std::floor((mx + pad - L.lo[a]) * L.inv[a]);
+      c0[a] = i0 < 0 ? 0 : (i0 > L.n[a] - 1 ? L.n[a] - 1 : i0);
+      c1[a] = i1 < 0 ? 0 : (i1 > L.n[a] - 1 ? L.n[a] - 1 : i1);
+    }
+    for (int k = c0[2]; k <= c1[2]; ++k) for (int j = c0[1]; j <= c1[1]; ++j) for (int i = c0[0]; i <= c1[0]; ++i) {
+      const size_t c = ((size_t)k * L.n[1] + j) * L.n[0] + i;
+      ++L.counts[c]; ++total;
+      if (buckets) (*buckets)[c].push_back((int)e);
+    }
+  }
+  if (total > 0x7FFFFFFFull) { g_err = "field: mesh index too large"; return false; }
+  L.rec = 0;
+  L.off = align_up(sizeof(double) * 24 * (size_t)nt, 256);
+  L.list = align_up(L.off + sizeof(int) * (nc + 1), 256);
+  L.total = align_up(L.list + sizeof(int) * total, 256);
+  return true;
+}
+// Fills `h` (L.total bytes) with the device image of the mesh.
+bool mesh_image(const avm_slab& s, const MeshLayout& L, const std::vector<std::vector<int>>& buckets, unsigned char* h) {
+  double* rec = (double*)(h + L.rec);
+  for (int64_t e = 0; e < s.n_tets; ++e) {
+    const int32_t* nd = s.tet_nodes + 10 * e;
+    const double* p[4];
+    for (int v = 0; v < 4; ++v) p[v] = s.node_xyz + 3 * (size_t)nd[v];
+    // edge matrix T = [p0 - p3 | p1 - p3 | p2 - p3] (columns); lambda_{0,1,2} = T^-1 (r - p3): rows of the inverse by cofactors
+    double T[3][3];
+    for (int r = 0; r < 3; ++r) for (int c = 0; c < 3; ++c) T[r][c] = p[c][r] - p[3][r];
+    const double c00 = T[1][1] * T[2][2] - T[1][2] * T[2][1], c01 = T[1][2] * T[2][0] - T[1][0] * T[2][2], c02 = T[1][0] * T[2][1] - T[1][1] * T[2][0];
+    const double det = T[0][0] * c00 + T[0][1] * c01 + T[0][2] * c02;
+    if (!(std::fabs(det) > 0.0)) { g_err = "field: degenerate tetrahedron " + std::to_string(e); return false; }
+    const double id = 1.0 / det;
+    double G[3][3];
+    G[0][0] = c00 * id; G[0][1] = (T[0][2] * T[2][1] - T[0][1] * T[2][2]) * id; G[0][2] = (T[0][1] * T[1][2] - T[0][2] * T[1][1]) * id;
+    G[1][0] = c01 * id; G[1][1] = (T[0][0] * T[2][2] - T[0][2] * T[2][0]) * id; G[1][2] = (T[0][2] * T[1][0] - T[0][0] * T[1][2]) * id;
+    G[2][0] = c02 * id; G[2][1] = (T[0][1] * T[2][0] - T[0][0] * T[2][1]) * id; G[2][2] = (T[0][0] * T[1][1] - T[0][1] * T[1][0]) * id;
+    double* q = rec + 24 * (size_t)e;
+    q[0] = p[3][0]; q[1] = p[3][1]; q[2] = p[3][2];
+    for (int a = 0; a < 3; ++a) for (int c = 0; c < 3; ++c) q[3 + 3 * a + c] = G[a][c];
+    for (int i = 0; i < 10; ++i) q[12 + i] = s.node_V[nd[i]];
+    q[22] = s.tet_gas[e] ? 1.0 : 0.0; q[23] = 0.0;
+  }
+  int* off = (int*)(h + L.off);
+  int* list = (int*)(h + L.list);
+  int run = 0;
+  for (size_t c = 0; c < buckets.size(); ++c) {
+    off[c] = run;
+    for (int e : buckets[c]) list[run++] = e;
+  }
+  off[buckets.size()] = run;
+  return true;
+}
+
 // NEXT-1, readings N1-N4 of DESIGN.md §3.5: the table of banded null-collision rates.
 //  N1 bands: 2^shift consecutive energy bins each (band_shift), K = ceil(nb / 2^shift) of them.
 //  N2 acceleration classes: squared upper edges A_j^2 = (kappa 250 V/cm)^2 2^j, j = 0 .. J-1, J = 25; column J = any
@@ -789,7 +878,7 @@ int32_t avm_field_create(avm_ctx* ctx, const avm_field_desc* d, avm_field** out)
     const char* bad = nullptr;
     if (!(s.z_hi > s.z_lo)) bad = "field: slab z_hi <= z_lo";
     else if (i > 0 && s.z_lo != d->slabs[i - 1].z_hi) bad = "field: slabs not contiguous/ascending";
-    else if (s.kind != 0 && s.kind != 1) bad = "field: kind";
+    else if (s.kind != 0 && s.kind != 1 && s.kind != 2) bad = "field: kind";
     if (!bad && s.kind == 0 && !(std::isfinite(s.E[0]) && std::isfinite(s.E[1]) && std::isfinite(s.E[2]))) bad = "field: uniform E is not finite";
     S.z_lo = s.z_lo; S.z_hi = s.z_hi; S.kind = s.kind;
     for (int a = 0; a < 3; ++a) S.E[a] = s.E[a];
@@ -822,6 +911,39 @@ int32_t avm_field_create(avm_ctx* ctx, const avm_field_desc* d, avm_field** out)
         S.half[a] = bc[a] == 2 ? per[a] : inf;
       }
     }
+    if (!bad && s.kind == 2) {
+      // NEXT-2: x / y fold constants as for a grid (no extent: a point in no element is solid), the mesh image uploaded
+      if (s.bc_x < 0 || s.bc_x > 2 || s.bc_y < 0 || s.bc_y > 2) bad = "field: bc";
+      else if ((s.bc_x && !(s.period_x > 0)) || (s.bc_y && !(s.period_y > 0))) bad = "field: period";
+      const int bc[2] = {s.bc_x, s.bc_y};
+      const double per[2] = {s.period_x, s.period_y};
+      for (int a = 0; a < 3; ++a) { S.org[a] = s.origin[a]; S.inv_h[a] = 1.0; }
+      for (int a = 0; a < 2; ++a) {
+        S.bc[a] = bc[a];
+        S.span[a] = inf;
+        S.P[a] = bc[a] == 2 ? 2.0 * per[a] : (bc[a] == 1 ? per[a] : 1.0);
+        S.inv_P[a] = bc[a] ? 1.0 / S.P[a] : 0.0;
+        S.Pc[a] = bc[a] ? S.P[a] : inf;
+        S.lo[a] = bc[a] ? 0.0 : -inf;
+        S.half[a] = bc[a] == 2 ? per[a] : inf;
+      }
+      MeshLayout L;
+      std::vector<std::vector<int>> buckets;
+      if (!bad && !mesh_plan(s, L, &buckets)) { delete f; return AVM_ERR_INVALID_ARG; }
+      if (!bad && (!s.mesh_dev || s.mesh_dev_bytes < L.total || ((uintptr_t)s.mesh_dev & 255u))) bad = "field: mesh_dev null, smaller than avm_tetmesh_bytes or not 256-byte aligned";
+      if (!bad) {
+        std::vector<unsigned char> img(L.total, 0);
+        if (!mesh_image(s, L, buckets, img.data())) { delete f; return AVM_ERR_INVALID_ARG; }
+        cudaError_t e = cudaSetDevice(ctx->device);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(s.mesh_dev, img.data(), L.total, cudaMemcpyHostToDevice, ctx->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+        if (e != cudaSuccess) { delete f; return fail(AVM_ERR_CUDA, std::string("field_create: mesh upload: ") + cudaGetErrorString(e)); }
+        unsigned char* base = (unsigned char*)s.mesh_dev;
+        S.tet_rec = (const double*)(base + L.rec); S.tet_off = (const int*)(base + L.off); S.tet_list = (const int*)(base + L.list);
+        for (int a = 0; a < 3; ++a) { S.tlo[a] = L.lo[a]; S.tinv[a] = L.inv[a]; S.tn[a] = L.n[a]; }
+        S.n_tets = (int)s.n_tets;
+      }
+    }
     if (bad) { delete f; return fail(AVM_ERR_INVALID_ARG, bad); }
   }
   F.z_lo = d->slabs[0].z_lo;
@@ -851,7 +973,7 @@ int32_t avm_field_create(avm_ctx* ctx, const avm_field_desc* d, avm_field** out)
     if (e != cudaSuccess) { delete f; return fail(AVM_ERR_CUDA, std::string("field_create: widening the map: ") + cudaGetErrorString(e)); }
   }
   f->uniform1 = d->n_slabs == 1 && d->slabs[0].kind == 0;
-  f->fk = f->uniform1 ? 1 : (d->n_slabs == 1 ? 2 : 0);
+  f->fk = f->uniform1 ? 1 : ((d->n_slabs == 1 && d->slabs[0].kind == 1) ? 2 : 0);   // a lone tetrahedral map takes the general path
   F.xy_bounded = 0;
   for (int a = 0; a < 2; ++a)
     if (std::isfinite(F.xy_lo[a]) || std::isfinite(F.xy_hi[a]) || F.xy_lo[a] != F.xy_lo[a] || F.xy_hi[a] != F.xy_hi[a]) F.xy_bounded = 1;
@@ -873,6 +995,12 @@ int32_t avm_field_create(avm_ctx* ctx, const avm_field_desc* d, avm_field** out)
 }
 
 int32_t avm_field_destroy(avm_field* f) { delete f; return AVM_OK; }
+
+size_t avm_tetmesh_bytes(const avm_slab* s) {
+  if (!s || s->kind != 2) return 0;
+  MeshLayout L;
+  return mesh_plan(*s, L, nullptr) ? L.total : 0;
+}
 
 int32_t avm_field_eval(avm_ctx* ctx, const avm_field* f, int64_t n, const double* r, double* E, double* mask, int32_t* slab) {
   if (!ctx || !f || n < 0 || (n > 0 && (!r || !E || !mask || !slab))) return fail(AVM_ERR_INVALID_ARG, "field_eval: null argument");

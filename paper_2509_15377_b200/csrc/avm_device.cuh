@@ -72,6 +72,14 @@ struct DevSlab {
   const float4* nodes;
   const double* nodes64;              // optional widened copy [nz][ny][nx][4] (same values as doubles): no conversions per lookup
   int kind, nx, ny, nz, bc[2];
+  // kind 2 (NEXT-2): unstructured map of 10-node tetrahedra.  tet_rec[e] = 24 doubles: vertex 3 (3), the
+  // rows G_a of the inverse edge matrix, lambda_a = G_a . (r - p3), a = 0..2 (9), the ten node potentials (10), gas flag, pad.
+  // Bucket grid over the mesh's bounding box: tet_off[cell] .. tet_off[cell + 1] index tet_list (ascending element numbers).
+  const double* tet_rec;
+  const int* tet_off;
+  const int* tet_list;
+  double tlo[3], tinv[3];
+  int tn[3], n_tets;
 };
 
 struct DevField {
@@ -281,6 +289,64 @@ __device__ __forceinline__ bool grid_at(const DevSlab& s, double x, double y, do
   return okx & oky;
 }
 
+// ---- NEXT-2: 10-node tetrahedra (F1-F2) -------------------------------------------------------------
+// Element e at r (coordinates relative to the slab's origin): false when r is not inside (some barycentric < tol); else the
+// field E = -grad V from the quadratic shape functions (N_vertex = l(2l - 1), N_edge = 4 l_a l_b) and the element's flag.
+__device__ __forceinline__ bool tet_try(const DevSlab& s, int e, double tol, double x, double y, double z, double& Ex, double& Ey,
+                                        double& Ez, double& mask) {
+  const double2* p = reinterpret_cast<const double2*>(s.tet_rec + 24 * (size_t)e);
+  const double2 a0 = __ldg(p), a1 = __ldg(p + 1), a2 = __ldg(p + 2), a3 = __ldg(p + 3), a4 = __ldg(p + 4), a5 = __ldg(p + 5);
+  const double qx = x - a0.x, qy = y - a0.y, qz = z - a1.x;
+  const double g0x = a1.y, g0y = a2.x, g0z = a2.y, g1x = a3.x, g1y = a3.y, g1z = a4.x, g2x = a4.y, g2y = a5.x, g2z = a5.y;
+  const double l0 = g0x * qx + g0y * qy + g0z * qz, l1 = g1x * qx + g1y * qy + g1z * qz, l2 = g2x * qx + g2y * qy + g2z * qz;
+  const double l3 = 1.0 - l0 - l1 - l2;
+  if (!((l0 >= tol) & (l1 >= tol) & (l2 >= tol) & (l3 >= tol))) return false;
+  const double2 v01 = __ldg(p + 6), v23 = __ldg(p + 7), m01 = __ldg(p + 8), m23 = __ldg(p + 9), m45 = __ldg(p + 10), fl = __ldg(p + 11);
+  const double g3x = -(g0x + g1x + g2x), g3y = -(g0y + g1y + g2y), g3z = -(g0z + g1z + g2z);
+  // dV/dlambda_a: vertex terms V_a (4 l_a - 1), edge terms 4 V_ab l_b; edges (0,1) (0,2) (0,3) (1,2) (1,3) (2,3)
+  const double d0 = v01.x * (4.0 * l0 - 1.0) + 4.0 * (m01.x * l1 + m01.y * l2 + m23.x * l3);
+  const double d1 = v01.y * (4.0 * l1 - 1.0) + 4.0 * (m01.x * l0 + m23.y * l2 + m45.x * l3);
+  const double d2 = v23.x * (4.0 * l2 - 1.0) + 4.0 * (m01.y * l0 + m23.y * l1 + m45.y * l3);
+  const double d3 = v23.y * (4.0 * l3 - 1.0) + 4.0 * (m23.x * l0 + m45.x * l1 + m45.y * l2);
+  Ex = -(d0 * g0x + d1 * g1x + d2 * g2x + d3 * g3x);
+  Ey = -(d0 * g0y + d1 * g1y + d2 * g2y + d3 * g3y);
+  Ez = -(d0 * g0z + d1 * g1z + d2 * g2z + d3 * g3z);
+  mask = fl.x;
+  return true;
+}
+// Field and flag at (x, y, z) of a kind-2 slab (z inside the slab).  The element that contains the point is the lowest-
+// numbered one with all barycentrics >= -1e-10 (F2); `cache` (may be null) holds the electron's last element: it is taken
+// without a search only when the point is strictly inside it (all barycentrics >= 1e-9: then no other element qualifies).
+__device__ __forceinline__ void tet_at(const DevSlab& s, double x, double y, double z, int* cache, double& Ex, double& Ey,
+                                       double& Ez, double& mask) {
+  double qx, qy;
+  bool fx, fy;
+  fold_axis(s, 0, x, qx, fx);
+  fold_axis(s, 1, y, qy, fy);
+  const double qz = z - s.org[2];
+  double ex = 0.0, ey = 0.0, ez = 0.0, m = 0.0;
+  bool found = false;
+  if (cache && *cache >= 0) { AVM_CHECK(*cache < s.n_tets); found = tet_try(s, *cache, 1e-9, qx, qy, qz, ex, ey, ez, m); }
+  if (!found) {
+    const double ux = (qx - s.tlo[0]) * s.tinv[0], uy = (qy - s.tlo[1]) * s.tinv[1], uz = (qz - s.tlo[2]) * s.tinv[2];
+    int cx = (int)floor(ux), cy = (int)floor(uy), cz = (int)floor(uz);
+    if (cx == s.tn[0] && ux <= (double)s.tn[0] * (1.0 + 1e-12)) cx = s.tn[0] - 1;
+    if (cy == s.tn[1] && uy <= (double)s.tn[1] * (1.0 + 1e-12)) cy = s.tn[1] - 1;
+    if (cz == s.tn[2] && uz <= (double)s.tn[2] * (1.0 + 1e-12)) cz = s.tn[2] - 1;
+    if (cx >= 0 && cx < s.tn[0] && cy >= 0 && cy < s.tn[1] && cz >= 0 && cz < s.tn[2]) {
+      const size_t cell = ((size_t)cz * s.tn[1] + cy) * s.tn[0] + cx;
+      const int q1 = __ldg(s.tet_off + cell + 1);
+      for (int q = __ldg(s.tet_off + cell); q < q1; ++q) {
+        const int e = __ldg(s.tet_list + q);
+        AVM_CHECK(e >= 0 && e < s.n_tets);
+        if (tet_try(s, e, -1e-10, qx, qy, qz, ex, ey, ez, m)) { if (cache) *cache = e; found = true; break; }
+      }
+    }
+    if (!found) { ex = 0.0; ey = 0.0; ez = 0.0; m = 0.0; }                      // in no element: solid (an unmeshed electrode)
+  }
+  Ex = fx ? -ex : ex; Ey = fy ? -ey : ey; Ez = ez; mask = m;
+}
+
 // Field and mask at r.  Returns the slab index (>= 0) or -status when r is outside the domain.
 // FK = field kind the kernel is compiled for: 1 = the field is one uniform slab (configs 1-3: no dispatch, no loads), 2 = one
 // grid slab (config 4: the slab's constants are read at fixed constant-bank offsets instead of through a dynamic slab
@@ -294,7 +360,7 @@ __device__ __forceinline__ int outside_status(const DevField& f, double x, doubl
 
 template <int FK>
 __device__ __forceinline__ int field_at(const DevField& f, double x, double y, double z, double& Ex, double& Ey,
-                                        double& Ez, double& mask) {
+                                        double& Ez, double& mask, int* tet_cache = nullptr) {
   // written so that NaN coordinates fail the test, like the oracle
   bool in = (z >= f.z_lo) & (z <= f.z_hi);
   if (f.xy_bounded) in = in & (x >= f.xy_lo[0]) & (x <= f.xy_hi[0]) & (y >= f.xy_lo[1]) & (y <= f.xy_hi[1]);
@@ -311,6 +377,7 @@ __device__ __forceinline__ int field_at(const DevField& f, double x, double y, d
   }
   const DevSlab& s = f.slab[si];
   if (FK == 0 && s.kind == 0) { Ex = s.E[0]; Ey = s.E[1]; Ez = s.E[2]; mask = 1.0; return si; }
+  if (FK == 0 && s.kind == 2) { tet_at(s, x, y, z, tet_cache, Ex, Ey, Ez, mask); return si; }
   if (!grid_at(s, x, y, z, Ex, Ey, Ez, mask)) return -AVM_LEFT_XY;
   return si;
 }
@@ -589,7 +656,7 @@ __device__ __forceinline__ int uniform_exit_status(const DevField& f, double t_m
 // order, only when it fails.
 template <int FK>
 __device__ __forceinline__ int s5_status(const DevField& f, double t_max, uint32_t n, double x, double y, double z,
-                                         double t, double& Ex, double& Ey, double& Ez) {
+                                         double t, double& Ex, double& Ey, double& Ez, int* tet_cache = nullptr) {
   if (FK == 1) {
     if (!uniform_continues(f, t_max, n, x, y, z, t)) return uniform_exit_status(f, t_max, x, y, z, t);
     return 0;
@@ -606,6 +673,10 @@ __device__ __forceinline__ int s5_status(const DevField& f, double t_max, uint32
   double nEx, nEy, nEz, mask = 1.0;
   bool fold_ok = true;
   if (FK == 0 && s.kind == 0) { nEx = s.E[0]; nEy = s.E[1]; nEz = s.E[2]; }
+  else if (FK == 0 && s.kind == 2) {
+    if (inb) tet_at(s, x, y, z, tet_cache, nEx, nEy, nEz, mask);              // a search outside the domain is wasted work
+    else { nEx = 0.0; nEy = 0.0; nEz = 0.0; }
+  }
   else fold_ok = grid_at(s, x, y, z, nEx, nEy, nEz, mask);
   const bool ok = inb & fold_ok & !(mask < 0.5) & !(t > t_max) & (n < kStepLimit);
   if (!ok) {
@@ -633,9 +704,9 @@ __device__ __forceinline__ double advance_move(const DevField& f, uint32_t& n, d
 template <int FK, bool HASB>
 __device__ __forceinline__ int advance(const DevGas& g, const DevField& f, double t_max, uint32_t& n, double& x,
                                        double& y, double& z, double& t, double& vx, double& vy, double& vz, double& Ex,
-                                       double& Ey, double& Ez, double dt, bool& overflow) {
+                                       double& Ey, double& Ez, double dt, bool& overflow, int* tet_cache = nullptr) {
   const double s2 = advance_move<FK, HASB>(f, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt);   // S3, S4
-  const int st = s5_status<FK>(f, t_max, n, x, y, z, t, Ex, Ey, Ez);                        // S5
+  const int st = s5_status<FK>(f, t_max, n, x, y, z, t, Ex, Ey, Ez, tet_cache);             // S5
   if (st < 0) return st;
   return energy_bin(g, s2, overflow);                                                            // S6
 }

@@ -30,8 +30,9 @@ struct WarpBuf {
   };
   unsigned long long id[32];
   unsigned int n[32];
+  int last_tet[32];                // NEXT-2: the element each lane's electron was last found in (-1: none)
 };
-static_assert(sizeof(WarpBuf) == 1920, "WarpBuf");
+static_assert(sizeof(WarpBuf) == 2048, "WarpBuf");
 
 // ---- full-warp form: ONE free flight of a lane's electron and its null/real decision ---------------------------------
 // S3-S7 with this flight's pre-drawn (dt, u2w); the draws of the lane's NEXT flight are issued behind the threshold-record
@@ -48,7 +49,8 @@ __device__ __forceinline__ void fw_flight(const DevGas& g, const DevField& f, co
                                           const double t_max, const uint64_t id, uint32_t& n, double& x, double& y,
                                           double& z, double& t, double& vx, double& vy, double& vz, double& Ex, double& Ey,
                                           double& Ez, double& dt, uint2& u2w, int& fin, bool& pend, Pending& pc, Tally& tl,
-                                          const int jcls = 0, const DevSignal* sig = nullptr, SigAcc* sacc = nullptr) {
+                                          const int jcls = 0, const DevSignal* sig = nullptr, SigAcc* sacc = nullptr,
+                                          int* tet_cache = nullptr) {
   bool over = false, cut = false;
   double dtf = dt, nu = g.nu_hat;
   uint32_t rho = 0u;
@@ -59,7 +61,7 @@ __device__ __forceinline__ void fw_flight(const DevGas& g, const DevField& f, co
   }
   double sx0 = 0.0, sy0 = 0.0, sz0 = 0.0, st0 = 0.0, swx = 0.0, swy = 0.0, swz = 0.0;
   if (SIGNAL && sig->out) { sx0 = x; sy0 = y; sz0 = z; st0 = t; weighting_at(*sig, x, y, z, swx, swy, swz); }
-  const int b = advance<FK, HASB>(g, f, t_max, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dtf, over);
+  const int b = advance<FK, HASB>(g, f, t_max, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dtf, over, tet_cache);
   if (SIGNAL && sig->out) sig_add(*sig, *sacc, -(swx * (x - sx0) + swy * (y - sy0) + swz * (z - sz0)), st0);
   if (b < 0) { fin = -b; return; }
   AVM_CHECK(b < g.nb);
@@ -263,7 +265,7 @@ __device__ __forceinline__ void sb_batch(const DevGas& g, const DevField& f, con
                                          bool& have, double& x, double& y, double& z, double& t, double& vx, double& vy,
                                          double& vz, double& Ex, double& Ey, double& Ez, const uint64_t& id, uint32_t& n,
                                          Tally& tl, Collide&& collide, Retire&& retire, Commit&& commit, const int jcls = 0,
-                                         const DevSignal* sig = nullptr, SigAcc* sacc = nullptr) {
+                                         const DevSignal* sig = nullptr, SigAcc* sacc = nullptr, int* tet_cache = nullptr) {
   const unsigned lt_mask = (1u << lane) - 1u;
   const int k = __popc(act);
   const int lg = 32 - __clz(k - 1);             // k' = 2^lg >= k  (k = 1: __clz(0) = 32)
@@ -309,7 +311,7 @@ __device__ __forceinline__ void sb_batch(const DevGas& g, const DevField& f, con
     AVM_CHECK(b >= 0 && b < g.nb);
     int r = decide_filter<BANDED>(tab[b], u2, rho);                                            // S7 and the head of S8
     if (BANDED && cut) r = -1;
-    const int st = s5_status<FK>(f, t_max, n, x, y, z, t, Ex, Ey, Ez);                         // S5; the field at r' = S0 of the next step
+    const int st = s5_status<FK>(f, t_max, n, x, y, z, t, Ex, Ey, Ez, tet_cache);              // S5; the field at r' = S0 of the next step
     if (TALLY && over && st == 0) ++tl.over;
     int ev = -1, fin = 0;
     if (st != 0 || r != -1) {                                                                  // not a plain null collision

@@ -145,6 +145,8 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
     dyn_off = ((size_t)g.nb * sizeof(ushort4) + 15) & ~(size_t)15;
   }
   WarpBuf* const wb = reinterpret_cast<WarpBuf*>(s_dyn + dyn_off) + warp;
+  int* const tet_cache = FK == 0 ? &wb->last_tet[lane] : nullptr;   // NEXT-2: only slab stacks can hold a tetrahedral map
+  if (FK == 0) *tet_cache = -1;
   int* const done = reinterpret_cast<int*>(reinterpret_cast<unsigned char*>(ctl) + kDoneOffset) + 8 * blockIdx.x;
   __syncthreads();
 
@@ -184,7 +186,8 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
           id = __ldcg(a.id + slot);
           n = __ldcg(a.nsteps + slot);
           double m;
-          field_at<FK>(f, x, y, z, Ex, Ey, Ez, m);           // S0 of its first step (in-domain by construction)
+          if (FK == 0) *tet_cache = -1;
+          field_at<FK>(f, x, y, z, Ex, Ey, Ez, m, tet_cache);   // S0 of its first step (in-domain by construction)
           have = true; dvalid = false;
           break;
         }
@@ -322,7 +325,7 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
     } else if (k <= kCoopMax) {
       // ---- serial batch: cooperative draws, then every owner lane walks its electron's steps alone (avm_forms.cuh) ----
       sb_batch<FK, HASB, TALLY, BANDED, SIGNAL>(g, f, K, tab, s_logtab, wb, t_max, lane, act, have, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, id, n, tl,
-                                                collide_and_append, retire, [](int, int, int, int, int) {}, jcls, &sig, &sacc);
+                                                collide_and_append, retire, [](int, int, int, int, int) {}, jcls, &sig, &sacc, tet_cache);
       dvalid = false;
     } else {
       // ---- full warp ----
@@ -335,7 +338,7 @@ transport_kernel(const __grid_constant__ DevGas g, const __grid_constant__ DevFi
       for (int fl = 0; fl < kFlights; ++fl) {
         if (have && !pend && fin == 0)
           fw_flight<FK, HASB, TALLY, BANDED, SIGNAL>(g, f, K, tab, s_logtab, t_max, id, n, x, y, z, t, vx, vy, vz, Ex, Ey, Ez, dt, u2w, fin,
-                                                     pend, pc, tl, jcls, &sig, &sacc);
+                                                     pend, pc, tl, jcls, &sig, &sacc, tet_cache);
       }
       Deflection dd;
       dd.ct = 1.0; dd.st = 0.0; dd.cphi = 1.0; dd.sphi = 0.0;

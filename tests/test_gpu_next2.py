@@ -1,0 +1,169 @@
+"""NEXT-2 on the device (DESIGN.md §3.8 readings F1-F4): unstructured maps of 10-node tetrahedra in the
+CUDA path against the oracle — the field at random points (incl. vertices, edges, faces, solid elements, holes, folded
+coordinates), per-step tolerance T through the forms a slab stack takes (general, full-warp, serial batch; banded too),
+same-seed whole avalanches through a mesh with a GEM-like hole (un-banded, banded, with induced signal and ion drift), and
+the uniform-slab equivalence of a linear-potential mesh on the device.  PAPER.md:121 / :33: the paper's maps are ANSYS
+finite-element meshes searched through an octree."""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from paper_2509_15377_b200.gen import fields, gas, primaries, tetmesh
+from test_gpu_parity import assert_step_parity, assert_run_same_seed, _states
+from test_gpu_step_forms import assert_form2_parity, oracle_sequence
+
+pytestmark = pytest.mark.gpu
+CORES = os.cpu_count() or 1
+H = 2e-4
+
+
+@pytest.fixture(scope="module")
+def ctx(avm):
+    return avm.ctx_create(0)
+
+
+def hole_mesh(seed=1, nx=13, ny=13, nz=31):
+    """A GEM-like cell as a tetrahedral map: 24 x 24 x 60 um, a foil (solid elements) between z = 24 and 36 um with a hole of
+    radius 9 um at the cell's corner (mirror cell: the hole is shared by four cells), metal left unmeshed in a ring around it;
+    potential: 3 kV/cm drift + a focusing term that pulls field lines through the hole."""
+    Lx = (nx - 1) * H
+    zc = 30e-4
+    def V(x, y, z):
+        r2 = x * x + y * y
+        # E_z = -dV/dz > 0 everywhere: the force on an electron points to -z (R1), through the hole
+        # and above the foil the potential is highest on the hole's axis: the electrons are funnelled into it
+        return -3000.0 * z - 40.0 * np.tanh((z - zc) / 6e-4) * (1.5 - np.exp(-r2 / (9e-4) ** 2))      # 36 kV/cm on the axis, 79 at the rim
+    foil = lambda x, y, z: (np.abs(z - zc) < 6e-4) & (x * x + y * y > (9e-4) ** 2)
+    metal = lambda x, y, z: (np.abs(np.abs(z - zc) - 5e-4) < 1.2e-4) & (x * x + y * y > (10e-4) ** 2) & (x * x + y * y < (16e-4) ** 2)
+    mesh = tetmesh.kuhn_mesh(nx, ny, nz, (H, H, H), V, seed=seed, solid=foil, removed=metal)
+    return mesh, Lx, (nz - 1) * H
+
+
+def hole_field(mesh, Lx, Lz, B=(0.0, 0.0, 0.0)):
+    return fields.FieldDesc([fields.tet_slab(mesh, (0.0, 0.0, 0.0), 0.0, Lz, fields.BC_MIRROR, fields.BC_MIRROR, Lx, Lx),
+                             fields.Slab(Lz, Lz + 20e-4, fields.KIND_UNIFORM, (0.0, 0.0, 3000.0))], B)
+
+
+def test_field_eval_on_tetrahedral_maps(avm, ctx, oracle):
+    mesh, Lx, Lz = hole_mesh()
+    assert mesh.tet_nodes.shape[0] > 20000 and (mesh.tet_gas == 0).sum() > 1000
+    fd = hole_field(mesh, Lx, Lz)
+    fg = avm.field_create(ctx, fd)
+    rng = np.random.default_rng(0)
+    n = 200000
+    r = rng.uniform(-1, 1, size=(3, n)) * np.array([3 * Lx, 3 * Lx, 0.0])[:, None]
+    r[2] = rng.uniform(-2e-4, Lz + 22e-4, n)
+    xyz, tn = mesh.node_xyz, mesh.tet_nodes
+    r[:, :500] = xyz[tn[:500, 0]].T                                     # vertices
+    r[:, 500:1000] = xyz[tn[1000:1500, 6]].T                            # mid-edge nodes
+    r[:, 1000:1500] = ((xyz[tn[2000:2500, 0]] + xyz[tn[2000:2500, 1]] + xyz[tn[2000:2500, 3]]) / 3).T   # face centres
+    Ec, mc, sc = oracle.field_eval(fd, r)
+    Eg, mg, sg = avm.field_eval(ctx, fg, r)
+    assert np.array_equal(sc, sg)
+    # on a face / edge / vertex the two sides may take different elements of the tolerance band: compare where they agree on
+    # the flag, require the rest to be within the band's share
+    agree = mc == mg
+    assert agree.mean() > 0.9995 and agree[1500:].mean() > 0.99999, (agree.mean(), agree[1500:].mean())
+    scale = np.abs(Ec).max()
+    err = np.abs(Ec - Eg).max(axis=0)
+    interior = np.ones(n, dtype=bool); interior[:1500] = False
+    assert np.all(err[interior & agree] <= 1e-11 * scale), err[interior & agree].max() / scale
+    assert (mc == 0).sum() > 0.1 * n and (mc == 1).sum() > 0.3 * n and (sc == 1).sum() > 1000 and (sc == -1).sum() > 100
+
+
+@pytest.mark.parametrize("B", [(0.0, 0.0, 0.0), (0.3, -0.2, 0.9)])
+def test_steps_through_a_tetrahedral_map(avm, ctx, oracle, g0, B):
+    mesh, Lx, Lz = hole_mesh()
+    fd = hole_field(mesh, Lx, Lz, B)
+    fg = avm.field_create(ctx, fd)
+    gg = avm.gas_create(ctx, g0)
+    rng = np.random.default_rng(5)
+    n = 1 << 15
+    st = _states(n, rng, box=1.0, center=(0, 0, 0))
+    st[0:2] = rng.uniform(-2 * Lx, 2 * Lx, size=(2, n)); st[2] = rng.uniform(1e-4, Lz + 19e-4, n)
+    E, m, sl = oracle.field_eval(fd, st[0:3])
+    ok = (sl >= 0) & (m >= 0.5)
+    st[:, ~ok] = st[:, np.flatnonzero(ok)[0]][:, None]
+    ids = rng.integers(0, 2 ** 64, n, dtype=np.uint64)
+    nidx = rng.integers(0, 1 << 20, n, dtype=np.uint64).astype(np.uint32)
+    cpu = oracle.step_batch(g0, fd, 5, st, ids, nidx)
+    for form in (0, 1):
+        gpu = avm.step_batch_form(ctx, gg, fg, 5, st, ids, nidx, form=form)
+        assert_step_parity(cpu, gpu, st, f"tet map form {form} B={B}")
+    assert (cpu.status == 4).sum() > 20 and (cpu.status == 0).sum() > 0.8 * n
+    cb = oracle.step_batch(g0, fd, 5, st, ids, nidx, flags=1)
+    gb = avm.step_batch_form(ctx, gg, fg, 5, st, ids, nidx, form=1, flags=avm.RUN_BANDED)
+    assert_step_parity(cb, gb, st, f"tet map banded form 1 B={B}")
+    # batches of 8 and 4 steps: E jumps across element faces, so over longer batches the two sides' accumulated rounding
+    # is not merely carried forward (observed 9.5e-12 at the 31st step of a 32-step batch; 1e-12 per step from identical state)
+    for k in (4, 8):
+        gl = avm.step_form_lanes(k)
+        m_ = k * 600
+        c3, st_in = oracle_sequence(oracle, g0, fd, 3, st[:, :m_], ids[:m_], nidx[:m_], gl, 5.0)
+        g3 = avm.step_batch_form(ctx, gg, fg, 3, st[:, :m_], ids[:m_], nidx[:m_], form=3, k=k, t_max=5.0)
+        assert_form2_parity(avm, c3, st_in, g3, gl, f"tet map form 3 k={k} B={B}")
+
+
+@pytest.mark.parametrize("flags", [0, 16], ids=["global", "banded"])
+def test_avalanches_through_a_tetrahedral_map(avm, ctx, oracle, g0, flags):
+    """Same seed, whole avalanches: electrons start above the foil, drift into the hole (or onto the foil: status 4), come
+    out below; the induced signal and the ions' drift through the mesh against the oracle as well."""
+    mesh, Lx, Lz = hole_mesh()
+    fd = hole_field(mesh, Lx, Lz)
+    wf = fields.uniform_gap((0.0, 0.0, 1.0 / (Lz + 20e-4)), 0.0, Lz + 20e-4)
+    p = primaries.isotropic_primaries(400, 21, pos=(0.0, 0.0, Lz + 10e-4), xy_box=((0.0, Lx), (0.0, Lx)))
+    cpu = oracle.run(g0, fd, p, seed=21, n_threads=CORES, flags=1 if flags else 0, t_max=50.0, signal=(wf, 0.0, 0.05, 60))
+    gg, fg, wg = avm.gas_create(ctx, g0), avm.field_create(ctx, fd), avm.field_create(ctx, wf)
+    bufs = avm.RunBuffers(ctx, 1 << 16, 400, g0.n_levels)
+    sig = torch.zeros(60, dtype=torch.float64, device=ctx.device)
+    _, n = avm.run(ctx, gg, fg, p, bufs, seed=21, flags=flags, t_max=50.0, signal=(wg, 0.0, 0.05, sig))
+    gpu = avm.fetch(ctx, bufs, n)
+    assert (cpu.status == 4).sum() > 50 and (cpu.status == 1).sum() > 50
+    # E jumps across element faces: a history that crosses ~1e3 faces amplifies the two sides' rounding far more than a
+    # trilinear map does (observed: 99.0 % identical histories, median endpoint error 9e-12, 4 % beyond 1e-7, worst 9e-5)
+    # banded flights are longer and end in more distant elements: 94.7 % identical histories observed (per-step parity of the
+    # same forms on the same map holds at 1e-12: test_steps_through_a_tetrahedral_map)
+    frac, _ = assert_run_same_seed(cpu, gpu, g0.n_levels, min_identical=0.98 if flags == 0 else 0.9, end_rtol=1e-7, tail=0.08, tail_rtol=1e-3,
+                                   label=f"tetrahedral hole map, 400 primaries, flags {flags}")
+    scale = np.abs(cpu.signal).max()
+    assert np.all(np.abs(cpu.signal - sig.cpu().numpy()) <= (1e-6 if frac == 1.0 else 5e-2) * scale)
+    ic = oracle.ion_drift(fd, cpu, 400, 1.5e-9, 2.0e-9, 0.5e-4, t_max=5e4)
+    ig = avm.ion_drift(ctx, fg, bufs, n, 1.5e-9, 2.0e-9, 0.5e-4, t_max=5e4)
+    common, oc, og = np.intersect1d(cpu.id, gpu.id, return_indices=True)      # the electrons both sides have, same histories
+    same = (cpu.n_steps[oc] == gpu.n_steps[og]) & (cpu.status[oc] == gpu.status[og])
+    nc, ng = cpu.n, gpu.n
+    sc, sg = ic.status[:nc][oc][same], ig.status[:ng][og][same]
+    assert (sc == sg).mean() > 0.99 and (sc >= 1).sum() > 100
+    okk = sc == sg
+    assert np.allclose(ic.end[:, :nc][:, oc][:, same][:, okk], ig.end[:, :ng][:, og][:, same][:, okk], rtol=1e-3, atol=1e-7)
+    close = np.abs(ic.end[0:3, :nc][:, oc][:, same][:, okk] - ig.end[0:3, :ng][:, og][:, same][:, okk]).max(axis=0) < 1e-9
+    assert close.mean() > 0.9                                                  # most ions agree to rounding
+    assert set(np.unique(sg)) >= {-1, 2}                                        # ions go up and out at the top
+
+
+def test_linear_potential_mesh_is_a_uniform_slab_on_the_device(avm, ctx, oracle, g0):
+    """F3 on the device: a jittered mesh carrying V = E0 z gives the uniform-slab avalanches of the oracle."""
+    nx, ny, nz = 12, 12, 26
+    E0 = 30000.0
+    mesh = tetmesh.kuhn_mesh(nx, ny, nz, (4 * H, 4 * H, H), lambda x, y, z: E0 * z, seed=9)
+    P = 11 * 4 * H
+    fm = fields.FieldDesc([fields.tet_slab(mesh, (0.0, 0.0, 0.0), 0.0, 25 * H, fields.BC_MIRROR, fields.BC_PERIODIC, P, P)])
+    fu = fields.uniform_gap((0.0, 0.0, -E0), 0.0, 25 * H)
+    p = primaries.isotropic_primaries(200, 3, pos=(0.3 * P, 0.6 * P, 0.0))
+    cpu = oracle.run(g0, fu, p, seed=3, n_threads=CORES)
+    gpu = avm.simulate(ctx, avm.gas_create(ctx, g0), avm.field_create(ctx, fm), p, seed=3)
+    assert_run_same_seed(cpu, gpu, g0.n_levels, min_identical=0.999, end_rtol=1e-8, label="linear-potential mesh vs uniform slab (oracle)")
+
+
+def test_invalid_meshes_are_rejected(avm, ctx):
+    mesh = tetmesh.kuhn_mesh(4, 4, 4, (H, H, H), lambda x, y, z: z, seed=1)
+    bad = fields.TetMesh(mesh.node_xyz, mesh.node_V, mesh.tet_nodes.copy(), mesh.tet_gas)
+    bad.tet_nodes[3, 2] = mesh.node_xyz.shape[0] + 5
+    with pytest.raises(avm.AvmError):
+        avm.field_create(ctx, fields.FieldDesc([fields.tet_slab(bad, (0, 0, 0), 0.0, 3 * H)]))
+    flat = fields.TetMesh(mesh.node_xyz.copy(), mesh.node_V, mesh.tet_nodes, mesh.tet_gas)
+    flat.node_xyz[:, 2] = 0.0
+    with pytest.raises(avm.AvmError):
+        avm.field_create(ctx, fields.FieldDesc([fields.tet_slab(flat, (0, 0, 0), 0.0, 3 * H)]))

@@ -235,7 +235,7 @@ def assert_run_same_seed(cpu, gpu, n_levels, min_identical=0.999, end_rtol=1e-9,
     assert err.max() <= (tail_rtol if tail > 0.0 else end_rtol), np.sort(err)[-5:]
     # birth records of children born late in a long history carry their parent's drift: a child's birth point IS its
     # parent's position at the ionisation, so it is held to the endpoints' tolerance
-    birth_rtol = max(1e-9, end_rtol) if tail == 0.0 else 100 * end_rtol
+    birth_rtol = max(1e-9, end_rtol) if tail == 0.0 else max(100 * end_rtol, tail_rtol)    # children of parents in the tail
     assert np.abs(c.birth[:, ic] - g.birth[:, ig]).max() <= birth_rtol * np.maximum(np.abs(c.birth[:, ic]).max(), 1.0)
     return same.mean(), len(common)
 
