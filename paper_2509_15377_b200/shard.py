@@ -3,7 +3,7 @@
 Avalanches are independent and every random number is keyed by (electron id, collision index), so a job of Np
 primaries partitions over ranks by primary range with NO data-path collective: rank r runs primaries [p0, p1) with
 `id_offset = job_id_offset + p0` and gets bit-identical avalanches to the ones the single-rank job computes for those
-primaries.  What is exchanged is the result only: one all-reduce of the tallies (<= (L + 4) u64 + 5 f64) and a gather of
+primaries.  What is exchanged is the result only: one all-reduce of the tallies (<= (L + 5) u64 + 5 f64) and a gather of
 the endpoint columns and per-avalanche counts.  Works with any torch.distributed backend ("nccl" with device tensors
 on the GPU box, "gloo" with CPU tensors in the tests); nothing here touches the transport arithmetic.
 """
