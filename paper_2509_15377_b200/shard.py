@@ -55,6 +55,15 @@ def merge_tallies(tallies_u64: np.ndarray, tallies_f64: np.ndarray, dist, device
     return tu.cpu().numpy().view(np.uint64), tf.cpu().numpy()
 
 
+def merge_signal(signal: np.ndarray, dist, device=None) -> np.ndarray:
+    """Sum of the shards' induced-signal histograms (NEXT-4; the signal is a plain sum over electrons, so the whole job's
+    histogram is the all-reduce of the shards' — same bins on every rank)."""
+    dev = _dev(dist, device)
+    t = torch.from_numpy(np.ascontiguousarray(signal, dtype=np.float64).copy()).to(dev)
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return t.cpu().numpy()
+
+
 def _gather_rows(local: np.ndarray, counts: list, dist, dev) -> np.ndarray:
     """all_gather of arrays whose LAST axis has a per-rank length (padded to the maximum, trimmed after)."""
     world, rank = dist.get_world_size(), dist.get_rank()

@@ -3,7 +3,8 @@
 The host-side plumbing (paper_2509_15377_b200.shard: partition, id offsets, tally all-reduce, endpoint gather) is what
 runs here; each rank's shard is computed by the oracle standing in for the GPU (tests may call oracle/), so the merged
 result must be IDENTICAL to the whole job computed in one piece — the property the multi-GPU design rests on
-(draws keyed by electron id, no data-path collective).
+(draws keyed by electron id, no data-path collective).  The shards run with banded rates and an induced signal: the
+banded streams are keyed by electron id as well, and the job's histogram is the all-reduce of the shards'.
 """
 import os
 import socket
@@ -53,12 +54,14 @@ def _worker(rank: int, world: int, port: int, n_prim: int, out_dir: str):
         fd = fields.uniform_gap((0.0, 0.0, -45000.0), 0.0, 60e-4)
         prim = primaries.isotropic_primaries(n_prim, 3)
         p0, p1 = shard.shard_range(n_prim, rank, world)
-        local = avmo.run(g0, fd, prim[p0:p1], seed=3, id_offset=p0, capacity=1 << 16)
+        wf = fields.uniform_gap((0.0, 0.0, 1.0 / 60e-4), 0.0, 60e-4)
+        local = avmo.run(g0, fd, prim[p0:p1], seed=3, id_offset=p0, capacity=1 << 16, flags=avmo.BANDED, signal=(wf, 0.0, 0.01, 40))
         merged = shard.merge_run(local, p0, n_prim, dist)
+        signal = shard.merge_signal(local.signal, dist)
         np.savez(os.path.join(out_dir, f"merged_{rank}.npz"), n=merged.n, id=merged.id, avalanche=merged.avalanche,
                  status=merged.status, n_steps=merged.n_steps, birth=merged.birth, end=merged.end,
                  per_avalanche=merged.per_avalanche, tallies_u64=merged.tallies_u64, tallies_f64=merged.tallies_f64,
-                 n_per_rank=np.array(merged.n_per_rank))
+                 n_per_rank=np.array(merged.n_per_rank), signal=signal)
     finally:
         dist.destroy_process_group()
 
@@ -72,7 +75,8 @@ def test_two_rank_gloo_job_equals_single_rank_job(tmp_path):
     mp.spawn(_worker, args=(world, _free_port(), n_prim, str(tmp_path)), nprocs=world, join=True)
     g0 = gas.gas_g0()
     fd = fields.uniform_gap((0.0, 0.0, -45000.0), 0.0, 60e-4)
-    whole = avmo.run(g0, fd, primaries.isotropic_primaries(n_prim, 3), seed=3, capacity=1 << 16)
+    wf = fields.uniform_gap((0.0, 0.0, 1.0 / 60e-4), 0.0, 60e-4)
+    whole = avmo.run(g0, fd, primaries.isotropic_primaries(n_prim, 3), seed=3, capacity=1 << 16, flags=avmo.BANDED, signal=(wf, 0.0, 0.01, 40))
     assert whole.n > 2 * n_prim                      # the avalanches multiply: secondaries cross the gather too
     m = [np.load(os.path.join(tmp_path, f"merged_{r}.npz")) for r in range(world)]
     for key in m[0].files:                           # every rank assembled the same job result
@@ -87,4 +91,5 @@ def test_two_rank_gloo_job_equals_single_rank_job(tmp_path):
     assert np.array_equal(whole.end[:, oc], r["end"][:, om])
     assert np.array_equal(whole.per_avalanche, r["per_avalanche"])
     assert np.array_equal(whole.tallies_u64, r["tallies_u64"])
-    assert np.allclose(whole.tallies_f64, r["tallies_f64"], rtol=1e-12, atol=0)   # sums in a different order
+    assert np.allclose(whole.tallies_f64, r["tallies_f64"], rtol=1e-12, atol=1e-14)   # sums in a different order (dx, dy cancel to ~1e-5)
+    assert np.abs(whole.signal).max() > 1.0 and np.allclose(whole.signal, r["signal"], rtol=1e-12, atol=1e-13)   # NEXT-4 histogram
