@@ -11,7 +11,8 @@
  * R1-R20 and steps S0-S9 of SURVEY.md §8(c), restated in DESIGN.md §3; the functions below cite them.
  *
  * Units: cm, ns, eV, V/cm, tesla.  All arithmetic fp64; grid nodes are fp32 storage, fp64 arithmetic.
- * All pointers are HOST pointers.  Parity status of each function: see DESIGN.md §5 (pins C1-C17);
+ * All pointers are HOST pointers.  Parity status of each function: see DESIGN.md §5 (pins C1-C17 of the base model; the
+ * NEXT rows' pins: tests/test_oracle_pins_banded.py, _next2.py, _next3.py, _next4.py — every function has a pin);
  * absolute values of the synthetic-gas results (gain, alpha, W of configs 1-5) are "parity unpinned"
  * (no reference values exist anywhere) — they are pinned GPU-vs-oracle only.
  */
