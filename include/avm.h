@@ -217,6 +217,41 @@ size_t avm_run_workspace_bytes(const avm_ctx*, int64_t capacity);
  * electrons that fit (children that did not fit are dropped and counted in the message). */
 int32_t avm_run(avm_ctx*, const avm_gas*, const avm_field*, const double* primaries, int64_t n_primaries,
                 const avm_run_opts*, const avm_outputs*, int64_t* n_endpoints_out);
+/* avm_run for callers that have no device workspace to give.
+ *
+ * Who this is for.  avm_run needs a `workspace`: scratch in device memory that the persistent transport kernel uses for
+ * its run-control block (live / created electron counters, the ticket queue head, per-CTA stop flags, the tally
+ * accumulators) and that stages the primaries' host-to-device copy.  Normally the caller allocates it next to the output
+ * arrays.  Some callers cannot: a plug-in that is handed its output buffers by a host framework and is forbidden to call
+ * the CUDA allocator itself; a service whose memory pool is sized and frozen at start-up; code that runs where
+ * cudaMalloc would synchronise the device or is simply not permitted.  For them the library carries ONE fixed scratch
+ * block of its own: a file-scope `static __device__` array in the library image, avm_run_static_bytes() bytes (4 MiB +
+ * 36 KiB), which every GPU that loads the library holds from module load until the process exits, used or not.
+ *
+ * What it does.  Exactly avm_run — same kernels, same arguments, same results, same return codes — except that
+ * outputs->workspace and outputs->workspace_bytes are IGNORED (pass NULL / 0) and the built-in block is used instead.
+ * All input and output arrays are still the caller's.  The call itself allocates nothing: no cudaMalloc, cudaFree, or
+ * library routine that allocates device memory is reached from it.
+ *
+ * Limit.  outputs->capacity <= AVM_RUN_STATIC_MAX_CAPACITY (65536 electrons, primaries + secondaries: the staging part of
+ * the block is sized for that many primaries).  A larger capacity fails at once with AVM_ERR_INVALID_ARG and a message
+ * that names the limit; nothing is queued.  Use avm_run with your own workspace for bigger runs.
+ *
+ * First call on a device.  The array's device address is looked up (cudaGetSymbolAddress, with the context's device
+ * current) the first time the entry point is called for that device, and remembered.  Make that first call outside any
+ * CUDA stream capture.
+ *
+ * Sharing.  There is one block per GPU and every avm_run_static call on that GPU uses it, whatever the context or the
+ * stream.  It still holds the previous call's contents when the next one starts; the call re-zeroes the run-control part
+ * on its stream before any kernel reads it, and the staging part is overwritten before it is read, so nothing of an
+ * earlier run leaks into a later one.  Because avm_run synchronises its stream before it returns, calls made one after
+ * the other from one host thread never overlap.  Calls issued from different host threads of one process to the same
+ * GPU at the same time DO overlap on the device and race on the block: serialise them yourself.  (Separate processes
+ * each load their own copy of the library image, so they do not share a block.) */
+enum { AVM_RUN_STATIC_MAX_CAPACITY = 65536 };
+size_t avm_run_static_bytes(void);
+int32_t avm_run_static(avm_ctx*, const avm_gas*, const avm_field*, const double* primaries, int64_t n_primaries,
+                       const avm_run_opts*, const avm_outputs*, int64_t* n_endpoints_out);
 /* Launch statistics of the last avm_run on this context: kernels launched, persistent-kernel launches. */
 int32_t avm_run_stats(const avm_ctx*, int64_t* n_kernel_launches, int64_t* n_transport_launches);
 /* Device time [ms] of the transport-kernel launches of the last avm_run on this context, summed (CUDA events

@@ -24,9 +24,10 @@ _lib = C.CDLL(_SO)
 OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_CUDA, ERR_STATE = 0, -1, -2, -3, -4
 RUN_PRIMARIES_ON_DEVICE, RUN_NO_TALLIES, RUN_SHAPE_WIDE, RUN_SHAPE_LATENCY, RUN_BANDED = 1, 2, 4, 8, 16
 MAX_LEVELS, MAX_SLABS = 64, 8
+RUN_STATIC_MAX_CAPACITY = 65536     # AVM_RUN_STATIC_MAX_CAPACITY: largest `capacity` run_static accepts
 EXPORTS = ["avm_last_error", "avm_ctx_create", "avm_ctx_destroy", "avm_ctx_sm_count", "avm_gas_bytes",
            "avm_gas_create", "avm_gas_destroy", "avm_gas_nu_hat", "avm_gas_bands", "avm_field_create", "avm_field_destroy", "avm_tetmesh_bytes",
-           "avm_field_eval", "avm_run_workspace_bytes", "avm_run", "avm_run_stats", "avm_run_transport_ms", "avm_fetch", "avm_ion_drift", "avm_step_batch", "avm_step_batch_form",
+           "avm_field_eval", "avm_run_workspace_bytes", "avm_run", "avm_run_static", "avm_run_static_bytes", "avm_run_stats", "avm_run_transport_ms", "avm_fetch", "avm_ion_drift", "avm_step_batch", "avm_step_batch_form",
            "avm_philox_batch", "avm_fp64_probe", "avm_gather_probe", "avm_smem_probe"]
 
 
@@ -106,6 +107,10 @@ _lib.avm_field_destroy.argtypes = [C.c_void_p]
 _lib.avm_field_eval.argtypes = [C.c_void_p, C.c_void_p, C.c_int64] + [C.c_void_p] * 4
 _lib.avm_run.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(_RunOpts),
                          C.POINTER(_Outputs), C.POINTER(C.c_int64)]
+_lib.avm_run_static.restype = C.c_int32
+_lib.avm_run_static.argtypes = list(_lib.avm_run.argtypes)
+_lib.avm_run_static_bytes.restype = C.c_size_t
+_lib.avm_run_static_bytes.argtypes = []
 _lib.avm_ion_drift.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_Signal), C.POINTER(_IonOpts), C.POINTER(_Outputs), C.c_int64, C.c_int64,
                                C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.avm_run_stats.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
@@ -485,6 +490,43 @@ def run(ctx: Context, gas: Gas, field: Field, primaries, bufs: RunBuffers, seed=
     o = bufs.c_struct()
     n_out = C.c_int64(0)
     rc = _lib.avm_run(ctx._h, gas._h, field._h, ptr, np_, C.byref(opts), C.byref(o), C.byref(n_out))
+    _check(rc, allow=(ERR_CAPACITY,) if allow_overflow else ())
+    return rc, int(n_out.value)
+
+
+def run_static_bytes() -> int:
+    """avm_run_static_bytes: size of the scratch block built into libavm.so (held by every GPU that loads it)."""
+    return int(_lib.avm_run_static_bytes())
+
+
+def run_static(ctx: Context, gas: Gas, field: Field, primaries, bufs: RunBuffers, seed=0, t_max=float("inf"), flags=0,
+               max_iters_per_launch=0, id_offset=0, max_ctas=0, allow_overflow=False, signal=None) -> tuple:
+    """avm_run_static: the same run as `run`, for callers that cannot allocate device memory for a workspace (a plug-in
+    whose host framework owns the allocator, a service with a memory pool frozen at start-up).  The transport kernel's
+    scratch lives in a fixed block inside the library instead, so `bufs.workspace` is not passed at all (NULL / 0 go
+    down); inputs and outputs are still the caller's tensors.  Limit: bufs.capacity <= RUN_STATIC_MAX_CAPACITY (65536
+    electrons), beyond it the call raises AvmError (INVALID_ARG) and nothing runs.  One block per GPU, shared by every
+    call: calls from several host threads to one GPU must be serialised by the caller.  The first call on a device looks
+    the block's address up; make it outside any stream capture.  Returns (rc, n_endpoints) like `run`."""
+    if isinstance(primaries, torch.Tensor) and primaries.is_cuda:
+        p = primaries.contiguous()
+        assert p.dtype == torch.float64
+        flags |= RUN_PRIMARIES_ON_DEVICE
+        ptr, np_ = C.c_void_p(p.data_ptr()), p.shape[0]
+    elif isinstance(primaries, torch.Tensor):
+        p = primaries.contiguous()
+        assert p.dtype == torch.float64
+        ptr, np_ = C.c_void_p(p.data_ptr()), p.shape[0]
+    else:
+        p = np.ascontiguousarray(primaries, dtype=np.float64)
+        ptr, np_ = _hp(p), p.shape[0]
+    sg = _signal_struct(signal)
+    opts = _RunOpts(int(seed), float(t_max), int(flags), int(max_iters_per_launch), int(id_offset), int(max_ctas),
+                    C.pointer(sg) if sg is not None else None)
+    o = bufs.c_struct()
+    o.workspace, o.workspace_bytes = None, 0          # ignored by the entry point; passed as NULL to show it
+    n_out = C.c_int64(0)
+    rc = _lib.avm_run_static(ctx._h, gas._h, field._h, ptr, np_, C.byref(opts), C.byref(o), C.byref(n_out))
     _check(rc, allow=(ERR_CAPACITY,) if allow_overflow else ())
     return rc, int(n_out.value)
 

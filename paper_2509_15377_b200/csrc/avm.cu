@@ -10,6 +10,7 @@
 #include <cstdio>
 #include <cstring>
 #include <limits>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -1321,6 +1322,60 @@ int32_t avm_fp64_probe(avm_ctx* ctx, int32_t n_blocks, int32_t n_threads, int64_
   cudaEventDestroy(e0);
   cudaEventDestroy(e1);
   return AVM_OK;
+}
+
+}  // extern "C"
+
+// ---- avm_run_static: avm_run on the library's own scratch block (include/avm.h) -----------------------------------------
+// For callers that may not allocate device memory (plug-ins given their buffers by a host framework, services with a pool
+// frozen at start-up): the workspace avm_run asks for — run-control block of the persistent transport kernel + staging
+// area of the primaries — lives in the array below instead of a caller buffer.  It is part of the library image, so every
+// GPU that loads libavm holds these bytes until the process exits.
+namespace {
+constexpr int64_t kStaticMaxCapacity = AVM_RUN_STATIC_MAX_CAPACITY;
+constexpr size_t kStaticWsBytes = kCtlBytes + (size_t)kStaticMaxCapacity * 8 * sizeof(double);   // 36 KiB + 4 MiB
+static_assert(kStaticMaxCapacity <= kStageElectrons, "the staging part is sized per electron only up to kStageElectrons");
+static __device__ __align__(256) unsigned char g_static_ws[kStaticWsBytes];
+
+// In host code `g_static_ws` is only a handle for the runtime, not memory a kernel can use: the device address has to be
+// asked for, once per device, with that device current.  Device code could name the array directly; the kernels here get
+// it as the `ctl` / `stage` pointers avm_run derives from the workspace, so only the host needs the address.
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mu;
+void* g_static_ws_addr[kStaticMaxDevices] = {};   // guarded by g_static_mu
+}  // namespace
+
+extern "C" {
+
+size_t avm_run_static_bytes(void) { return kStaticWsBytes; }
+
+int32_t avm_run_static(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, const double* primaries, int64_t np,
+                       const avm_run_opts* opts, const avm_outputs* o, int64_t* n_out) {
+  if (!ctx || !gas || !field || !opts || !o || !n_out) return fail(AVM_ERR_INVALID_ARG, "run_static: null argument");
+  *n_out = 0;
+  if (o->capacity > kStaticMaxCapacity)
+    return fail(AVM_ERR_INVALID_ARG, "run_static: capacity " + std::to_string(o->capacity) + " exceeds AVM_RUN_STATIC_MAX_CAPACITY (" +
+                                     std::to_string(kStaticMaxCapacity) + " electrons, the size of the built-in scratch block); use avm_run with a caller-provided workspace");
+  if (ctx->device < 0 || ctx->device >= kStaticMaxDevices) return fail(AVM_ERR_INVALID_ARG, "run_static: device ordinal beyond the 64 this entry point keeps an address for");
+  AVM_CUDA(cudaSetDevice(ctx->device));
+  void* ws = nullptr;
+  {
+    // First call on this device: resolve the array's address there (not inside a stream capture — see avm.h).
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_ws_addr[ctx->device]) {
+      void* p = nullptr;
+      AVM_CUDA(cudaGetSymbolAddress(&p, g_static_ws));
+      if (!p || ((uintptr_t)p & 255u)) return fail(AVM_ERR_CUDA, "run_static: the scratch block has no usable device address");
+      g_static_ws_addr[ctx->device] = p;
+    }
+    ws = g_static_ws_addr[ctx->device];
+  }
+  // The block still holds the previous call's counters, flags and staged primaries.  avm_run zeroes the run-control part
+  // on the stream before its first kernel and writes the staging part before reading it, so nothing else is cleared here.
+  avm_outputs w = *o;
+  w.workspace = ws;
+  w.workspace_bytes = kStaticWsBytes;
+  return avm_run(ctx, gas, field, primaries, np, opts, &w, n_out);
 }
 
 }  // extern "C"
