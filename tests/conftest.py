@@ -9,9 +9,19 @@ if ROOT not in sys.path:
 
 
 # Observed margins of the whole-run comparisons (same-seed identical-history fractions, endpoint errors, statistics):
-# tests append one line each; printed in the terminal summary and written to gpurun_out/parity_margins.txt, from which
-# BASELINE.md's parity table is filled in.
+# tests append one line each; printed in the terminal summary and written to gpurun_out/parity_margins.txt (overwritten by
+# every session and stamped with its command line, so the file always holds ONE run), from which BASELINE.md's parity table
+# is filled in.
 MARGINS = []
+
+
+def _git_head() -> str:
+    """HEAD of the tree the tests ran on ("unknown" on the GPU box, whose snapshot has no .git)."""
+    try:
+        import subprocess
+        return subprocess.run(["git", "rev-parse", "--short", "HEAD"], cwd=ROOT, capture_output=True, text=True, timeout=10).stdout.strip() or "unknown"
+    except Exception:
+        return "unknown"
 
 
 def record_margin(line: str) -> None:
@@ -27,7 +37,8 @@ def pytest_terminal_summary(terminalreporter):
     out = os.path.join(ROOT, "gpurun_out")
     try:
         os.makedirs(out, exist_ok=True)
-        with open(os.path.join(out, "parity_margins.txt"), "a") as f:
+        with open(os.path.join(out, "parity_margins.txt"), "w") as f:          # one run per file: never mixed with older code's lines
+            f.write(f"# pytest session at git {_git_head()}; args: {' '.join(sys.argv[1:])}\n")
             f.write("\n".join(MARGINS) + "\n")
     except OSError:
         pass
