@@ -326,7 +326,10 @@ __device__ __forceinline__ void tet_at(const DevSlab& s, double x, double y, dou
   const double qz = z - s.org[2];
   double ex = 0.0, ey = 0.0, ez = 0.0, m = 0.0;
   bool found = false;
-  if (cache && *cache >= 0) { AVM_CHECK(*cache < s.n_tets); found = tet_try(s, *cache, 1e-9, qx, qy, qz, ex, ey, ez, m); }
+  // The cached index is a hint and may stem from ANOTHER kind-2 slab of the stack (the electron crossed a slab plane since):
+  // strictly inside element e of this slab the answer is e whatever made us try it first, so a foreign hint is harmless —
+  // provided it indexes this slab's records at all (slabs differ in n_tets; checked in every build, not only AVM_DEBUG).
+  if (cache && *cache >= 0 && *cache < s.n_tets) found = tet_try(s, *cache, 1e-9, qx, qy, qz, ex, ey, ez, m);
   if (!found) {
     const double ux = (qx - s.tlo[0]) * s.tinv[0], uy = (qy - s.tlo[1]) * s.tinv[1], uz = (qz - s.tlo[2]) * s.tinv[2];
     int cx = (int)floor(ux), cy = (int)floor(uy), cz = (int)floor(uz);
