@@ -169,7 +169,8 @@ enum {
 };
 /* NEXT-4 ("induced-signal accumulation (weighting-field dot velocity per flight) and ion drift";
  * what the endpoints feed; DESIGN.md §3.7 readings W1-W4).  weighting: the weighting field E_w [1/cm] of the
- * read-out electrode as an avm_field (uniform slabs or grid maps; mask and B ignored; E_w = 0 outside it).  Every step
+ * read-out electrode as an avm_field (uniform slabs or grid maps only — a field with a tetrahedral slab is refused with
+ * AVM_ERR_INVALID_ARG; mask and B ignored; E_w = 0 outside it).  Every step
  * r -> r' of a charge q [e] that starts at time t adds q E_w . (r' - r) to signal_dev[floor((t - t0) / dt_bin)]; steps that
  * start outside the bins are dropped.  Electron flights: q = -1, E_w at r.  signal_dev: DEVICE [n_bins] doubles, ADDED to
  * (the caller zeroes it); induced charge per bin, current = charge / dt_bin. */
@@ -214,7 +215,9 @@ typedef struct {
 size_t avm_run_workspace_bytes(const avm_ctx*, int64_t capacity);
 /* Runs all avalanches to completion.  *n_endpoints_out = electrons created = endpoints written (<= capacity).
  * AVM_ERR_CAPACITY: more than `capacity` electrons would exist; the run still terminates, outputs hold the
- * electrons that fit (children that did not fit are dropped and counted in the message). */
+ * electrons that fit (children that did not fit are dropped and counted in the message).
+ * A signal or a gas with NEXT-3 extensions needs the kernel variant that keeps the threshold table in shared memory: gases of
+ * more than ~24000 energy bins are refused for those runs (AVM_ERR_INVALID_ARG, before anything is queued). */
 int32_t avm_run(avm_ctx*, const avm_gas*, const avm_field*, const double* primaries, int64_t n_primaries,
                 const avm_run_opts*, const avm_outputs*, int64_t* n_endpoints_out);
 /* avm_run for callers that have no device workspace to give.
@@ -266,7 +269,8 @@ int32_t avm_run_transport_ms(const avm_ctx*, float* ms_out);
  * (6), after max_steps or where the field vanishes (7).  With a signal, each step adds q E_w(r_m) . (r' - r) to the bin of the
  * step's start time.  run: the avm_outputs of the finished avm_run (birth, end, status DEVICE arrays are read; n = its
  * endpoint count).  ion_end: DEVICE [4][2n] x, y, z, t; ion_status: DEVICE [2n]; ion_steps: DEVICE [2n].  Asynchronous on
- * the context's stream. */
+ * the context's stream.  n_primaries <= n <= run->capacity is required; slots whose status is <= 0 (no finished electron:
+ * n was larger than the run's endpoint count) yield no ion (status -1). */
 typedef struct { double mobility_pos, mobility_neg, step_cm, t_max; int32_t max_steps; } avm_ion_opts;
 int32_t avm_ion_drift(avm_ctx*, const avm_field* field, const avm_signal* signal, const avm_ion_opts*, const avm_outputs* run,
                       int64_t n, int64_t n_primaries, double* ion_end, int32_t* ion_status, uint32_t* ion_steps);

@@ -340,7 +340,8 @@ ion_drift_kernel(const __grid_constant__ DevField f, const __grid_constant__ Dev
     int st = -1;
     uint32_t ns = 0u;
     double x = 0.0, y = 0.0, z = 0.0, t = 0.0;
-    if (pos ? s >= n_prim : a.status[s] == AVM_ATTACHED) {                  // W3: which ions exist
+    const int32_t est = a.status[s];                                         // <= 0: the slot holds no finished electron
+    if (est > 0 && (pos ? s >= n_prim : est == AVM_ATTACHED)) {              // W3: which ions exist
       const double* src = pos ? a.birth : a.end;
       x = src[s]; y = src[ld + s]; z = src[2 * ld + s]; t = src[3 * ld + s];
       const double q = pos ? 1.0 : -1.0, qmu = q * (pos ? io.mu_pos : io.mu_neg);
@@ -1043,6 +1044,8 @@ bool make_signal(const avm_signal* s, DevSignal& D) {
   std::memset(&D, 0, sizeof(D));
   if (!s) return true;
   if (!s->weighting || !(s->dt_bin > 0.0) || s->n_bins < 1 || !s->signal_dev || !std::isfinite(s->t0)) { g_err = "signal: weighting field, dt_bin > 0, n_bins >= 1 and a device array are required"; return false; }
+  for (int i = 0; i < s->weighting->d.n_slabs; ++i)
+    if (s->weighting->d.slab[i].kind == 2) { g_err = "signal: the weighting field must consist of uniform slabs and grid maps (a tetrahedral slab, kind 2, is not accepted here)"; return false; }
   D.wf = s->weighting->d;
   D.t0 = s->t0; D.inv_dt = 1.0 / s->dt_bin; D.n_bins = s->n_bins; D.uniform1 = s->weighting->uniform1 ? 1 : 0;
   D.out = s->signal_dev;
@@ -1062,6 +1065,20 @@ int32_t avm_run(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, const 
   if (o->tallies_f64 && !o->birth) return fail(AVM_ERR_INVALID_ARG, "run: tallies_f64 needs birth");
   if (!o->workspace || o->workspace_bytes < avm_run_workspace_bytes(ctx, o->capacity) || ((uintptr_t)o->workspace & 255u))
     return fail(AVM_ERR_INVALID_ARG, "run: workspace null, too small or not 256-byte aligned");
+  // Launch shape and kernel variant first: a combination without a variant is refused before any work is queued.
+  bool wide = np > (int64_t)ctx->sm_count * kThreads;            // the primaries alone outnumber the latency shape's lanes
+  if (opts->flags & AVM_RUN_SHAPE_WIDE) wide = true;
+  if (opts->flags & AVM_RUN_SHAPE_LATENCY) wide = false;
+  const int threads = wide ? kThreadsWide : kThreads;
+  const size_t buf_bytes = sizeof(WarpBuf) * (size_t)(threads / 32);
+  const size_t tab_bytes = align_up(sizeof(ushort4) * (size_t)gas->d.nb, 16);
+  const bool smemtab = tab_bytes + buf_bytes <= kMaxDynSmem;       // else the threshold table is read through L1
+  const size_t dyn_smem = (smemtab ? tab_bytes : 0) + buf_bytes;
+  DevSignal dsig;
+  if (!make_signal(opts->signal, dsig)) return AVM_ERR_INVALID_ARG;
+  const bool extras = opts->signal != nullptr || gas->d.ext != 0;     // NEXT-3 / NEXT-4: the kernel variant that has them
+  TransportFn fn = pick_transport(field->fk, field->d.has_B != 0, smemtab, wide, (opts->flags & AVM_RUN_BANDED) != 0, extras);
+  if (!fn) return fail(AVM_ERR_INVALID_ARG, "run: a signal or a gas with NEXT-3 extensions needs the threshold table in shared memory (at most ~24000 energy bins)");
   AVM_CUDA(cudaSetDevice(ctx->device));
   ctx->n_kernel_launches = 0; ctx->n_transport_launches = 0; ctx->transport_ms = 0.0f;
   cudaStream_t st = ctx->stream;
@@ -1088,19 +1105,6 @@ int32_t avm_run(avm_ctx* ctx, const avm_gas* gas, const avm_field* field, const 
     else AVM_CUDA(launch(ctx, inject_kernel<0>, grid, dim3(256), field->d, a, ctl, src, (uint32_t)p0, (uint32_t)cnt, opts->id_offset, opts->t_max));
   }
   // persistent transport (a-2 .. a-11)
-  bool wide = np > (int64_t)ctx->sm_count * kThreads;            // the primaries alone outnumber the latency shape's lanes
-  if (opts->flags & AVM_RUN_SHAPE_WIDE) wide = true;
-  if (opts->flags & AVM_RUN_SHAPE_LATENCY) wide = false;
-  const int threads = wide ? kThreadsWide : kThreads;
-  const size_t buf_bytes = sizeof(WarpBuf) * (size_t)(threads / 32);
-  const size_t tab_bytes = align_up(sizeof(ushort4) * (size_t)gas->d.nb, 16);
-  const bool smemtab = tab_bytes + buf_bytes <= kMaxDynSmem;       // else the threshold table is read through L1
-  const size_t dyn_smem = (smemtab ? tab_bytes : 0) + buf_bytes;
-  DevSignal dsig;
-  if (!make_signal(opts->signal, dsig)) return AVM_ERR_INVALID_ARG;
-  const bool extras = opts->signal != nullptr || gas->d.ext != 0;     // NEXT-3 / NEXT-4: the kernel variant that has them
-  TransportFn fn = pick_transport(field->fk, field->d.has_B != 0, smemtab, wide, (opts->flags & AVM_RUN_BANDED) != 0, extras);
-  if (!fn) return fail(AVM_ERR_INVALID_ARG, "run: a signal or a gas with NEXT-3 extensions needs the threshold table in shared memory (at most ~24000 energy bins)");
   AVM_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn_smem));
   int occ = 0;
   AVM_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, threads, dyn_smem));
@@ -1165,6 +1169,7 @@ int32_t avm_ion_drift(avm_ctx* ctx, const avm_field* field, const avm_signal* si
                       int64_t n, int64_t n_primaries, double* ion_end, int32_t* ion_status, uint32_t* ion_steps) {
   if (!ctx || !field || !io || !run || n < 0 || n_primaries < 0) return fail(AVM_ERR_INVALID_ARG, "ion_drift: null argument");
   if (!(io->step_cm > 0.0) || !(io->mobility_pos > 0.0) || !(io->mobility_neg > 0.0) || io->max_steps < 1) return fail(AVM_ERR_INVALID_ARG, "ion_drift: step, mobilities and max_steps must be positive");
+  if (n_primaries > n) return fail(AVM_ERR_INVALID_ARG, "ion_drift: n_primaries exceeds n (n = the endpoint count avm_run returned, primaries included)");
   if (n == 0) return AVM_OK;
   if (n > run->capacity || !run->birth || !run->end || !run->status || !ion_end || !ion_status || !ion_steps) return fail(AVM_ERR_INVALID_ARG, "ion_drift: run outputs (birth, end, status) and the ion arrays are required");
   DevSignal dsig;

@@ -163,3 +163,55 @@ def test_signal_and_ions_invalid_arguments(avm, ctx, g0):
     _, n = avm.run(ctx, gg, fg, p, bufs)
     with pytest.raises(avm.AvmError):
         avm.ion_drift(ctx, fg, bufs, n, 1e-9, 1e-9, 0.0)                  # step = 0
+
+
+def test_ion_drift_ignores_slots_that_hold_no_electron(avm, ctx, g0):
+    """avm_ion_drift with n beyond the run's endpoint count (slots of status -1 with stale birth values) produces no ions
+    there; n_primaries > n is refused."""
+    from paper_2509_15377_b200.gen import tetmesh
+    fd = fields.uniform_gap((0.0, 0.0, -30000.0), 0.0, 50e-4)
+    gg, fg = avm.gas_create(ctx, g0), avm.field_create(ctx, fd)
+    bufs = avm.RunBuffers(ctx, 1 << 12, 200, g0.n_levels)
+    bufs.birth.fill_(10e-4)                                                  # stale slots would look like ions born mid-gap
+    bufs.end.fill_(10e-4)
+    p = primaries.isotropic_primaries(200, 2)
+    _, n = avm.run(ctx, gg, fg, p, bufs, seed=2)
+    assert 200 < n < (1 << 12) - 64
+    a = avm.ion_drift(ctx, fg, bufs, n, 1.5e-9, 2.0e-9, 0.25e-4)
+    b = avm.ion_drift(ctx, fg, bufs, n + 64, 1.5e-9, 2.0e-9, 0.25e-4)
+    m = n + 64
+    assert np.all(b.status[n:m] == -1) and np.all(b.status[m + n:] == -1) and np.all(b.n_steps[n:m] == 0)
+    assert np.array_equal(a.status[:n], b.status[:n]) and np.array_equal(a.status[n:], b.status[m:m + n])
+    assert np.array_equal(a.end[:, :n], b.end[:, :n]) and (a.status[:n] >= 1).sum() == n - 200
+    with pytest.raises(avm.AvmError) as e:
+        avm.ion_drift(ctx, fg, avm.RunBuffers(ctx, 1 << 12, n + 1, g0.n_levels), n, 1.5e-9, 2.0e-9, 0.25e-4)   # n_primaries = n + 1
+    assert "n_primaries" in str(e.value)
+    # a tetrahedral weighting field is refused (uniform slabs and grid maps only), for runs and for ion drift alike
+    mesh = tetmesh.kuhn_mesh(4, 4, 4, (20e-4, 20e-4, 20e-4), lambda x, y, z: z, seed=1)
+    wt = avm.field_create(ctx, fields.FieldDesc([fields.tet_slab(mesh, (0, 0, 0), 0.0, 60e-4)]))
+    sig = torch.zeros(8, dtype=torch.float64, device=ctx.device)
+    for call in (lambda: avm.run(ctx, gg, fg, p, bufs, seed=2, signal=(wt, 0.0, 1.0, sig)),
+                 lambda: avm.ion_drift(ctx, fg, bufs, n, 1.5e-9, 2.0e-9, 0.25e-4, signal=(wt, 0.0, 1.0, sig))):
+        with pytest.raises(avm.AvmError) as e:
+            call()
+        assert "weighting" in str(e.value)
+
+
+def test_extras_on_a_table_too_large_for_shared_memory_are_refused_before_any_work(avm, ctx):
+    """A signal (or a NEXT-3 gas) needs the kernel variant with the threshold table in shared memory (at most ~24000
+    energy bins).  Beyond that avm_run refuses BEFORE it queues anything: the output arrays are untouched.  The same gas without
+    a signal runs (the table is then read through L1)."""
+    g = gas.gas_g0(n_bins=30000)
+    fd = fields.uniform_gap((0.0, 0.0, -30000.0), 0.0, 50e-4)
+    gg, fg = avm.gas_create(ctx, g), avm.field_create(ctx, fd)
+    bufs = avm.RunBuffers(ctx, 1 << 12, 50, g.n_levels)
+    bufs.status.fill_(-7)
+    p = primaries.isotropic_primaries(50, 3)
+    sig = torch.zeros(8, dtype=torch.float64, device=ctx.device)
+    with pytest.raises(avm.AvmError) as e:
+        avm.run(ctx, gg, fg, p, bufs, seed=3, signal=(fg, 0.0, 1.0, sig))
+    assert "shared memory" in str(e.value)
+    torch.cuda.synchronize()
+    assert bool((bufs.status == -7).all()) and float(sig.abs().sum()) == 0.0
+    _, n = avm.run(ctx, gg, fg, p, bufs, seed=3)
+    assert n >= 50 and bool((bufs.status[:n] >= 1).all())
