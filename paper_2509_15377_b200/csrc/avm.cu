@@ -604,6 +604,18 @@ bool mesh_plan(const avm_slab& s, MeshLayout& L, std::vector<std::vector<int>>* 
 // Fills `h` (L.total bytes) with the device image of the mesh.
 bool mesh_image(const avm_slab& s, const MeshLayout& L, const std::vector<std::vector<int>>& buckets, unsigned char* h) {
   double* rec = (double*)(h + L.rec);
+  // Largest element extent of the mesh (bounding-box diagonal over the four vertices): scales the per-element margin of the
+  // device's last-element shortcut below.
+  double d_max = 0.0;
+  for (int64_t e = 0; e < s.n_tets; ++e) {
+    double d2 = 0.0;
+    for (int a = 0; a < 3; ++a) {
+      double mn = std::numeric_limits<double>::infinity(), mx = -mn;
+      for (int v = 0; v < 4; ++v) { const double x = s.node_xyz[3 * (size_t)s.tet_nodes[10 * e + v] + a]; if (x < mn) mn = x; if (x > mx) mx = x; }
+      d2 += (mx - mn) * (mx - mn);
+    }
+    if (d2 > d_max * d_max) d_max = std::sqrt(d2);
+  }
   for (int64_t e = 0; e < s.n_tets; ++e) {
     const int32_t* nd = s.tet_nodes + 10 * e;
     const double* p[4];
@@ -623,7 +635,22 @@ bool mesh_image(const avm_slab& s, const MeshLayout& L, const std::vector<std::v
     q[0] = p[3][0]; q[1] = p[3][1]; q[2] = p[3][2];
     for (int a = 0; a < 3; ++a) for (int c = 0; c < 3; ++c) q[3 + 3 * a + c] = G[a][c];
     for (int i = 0; i < 10; ++i) q[12 + i] = s.node_V[nd[i]];
-    q[22] = s.tet_gas[e] ? 1.0 : 0.0; q[23] = 0.0;
+    q[22] = s.tet_gas[e] ? 1.0 : 0.0;
+    // Margin of the last-element shortcut (tet_at): a point whose barycentrics in THIS element are all >= q[23] lies at least
+    // q[23] h_min inside it (h_min = its smallest height = 1 / max |grad lambda_i|).  Another element e' of a valid mesh does
+    // not overlap it, so the point is at least that far outside e'; a point with all barycentrics of e' >= -eps is within
+    // 8 eps D' of e' (D' = its extent: clip the negative coordinates and renormalise), so e' fails F2's test (eps = 1e-10)
+    // whenever q[23] h_min > 8e-10 D'.  With D' <= d_max: q[23] = 1e-9 max(1, d_max / h_min) holds for ANY grading of the mesh.
+    double g_max = 0.0;
+    for (int a = 0; a < 4; ++a) {
+      double gx, gy, gz;
+      if (a < 3) { gx = G[a][0]; gy = G[a][1]; gz = G[a][2]; }
+      else { gx = -(G[0][0] + G[1][0] + G[2][0]); gy = -(G[0][1] + G[1][1] + G[2][1]); gz = -(G[0][2] + G[1][2] + G[2][2]); }
+      const double gn = std::sqrt(gx * gx + gy * gy + gz * gz);
+      if (gn > g_max) g_max = gn;
+    }
+    const double ratio = d_max * g_max;                       // d_max / h_min
+    q[23] = 1e-9 * (ratio > 1.0 ? ratio : 1.0);
   }
   int* off = (int*)(h + L.off);
   int* list = (int*)(h + L.list);

@@ -292,9 +292,12 @@ __device__ __forceinline__ bool grid_at(const DevSlab& s, double x, double y, do
 // ---- NEXT-2: 10-node tetrahedra (F1-F2) -------------------------------------------------------------
 // Element e at r (coordinates relative to the slab's origin): false when r is not inside (some barycentric < tol); else the
 // field E = -grad V from the quadratic shape functions (N_vertex = l(2l - 1), N_edge = 4 l_a l_b) and the element's flag.
+// OWN_MARGIN: `tol` is ignored and the element's own shortcut margin (record word 23, written by mesh_image) is used.
+template <bool OWN_MARGIN = false>
 __device__ __forceinline__ bool tet_try(const DevSlab& s, int e, double tol, double x, double y, double z, double& Ex, double& Ey,
                                         double& Ez, double& mask) {
   const double2* p = reinterpret_cast<const double2*>(s.tet_rec + 24 * (size_t)e);
+  if (OWN_MARGIN) tol = __ldg(p + 11).y;
   const double2 a0 = __ldg(p), a1 = __ldg(p + 1), a2 = __ldg(p + 2), a3 = __ldg(p + 3), a4 = __ldg(p + 4), a5 = __ldg(p + 5);
   const double qx = x - a0.x, qy = y - a0.y, qz = z - a1.x;
   const double g0x = a1.y, g0y = a2.x, g0z = a2.y, g1x = a3.x, g1y = a3.y, g1z = a4.x, g2x = a4.y, g2y = a5.x, g2z = a5.y;
@@ -316,7 +319,9 @@ __device__ __forceinline__ bool tet_try(const DevSlab& s, int e, double tol, dou
 }
 // Field and flag at (x, y, z) of a kind-2 slab (z inside the slab).  The element that contains the point is the lowest-
 // numbered one with all barycentrics >= -1e-10 (F2); `cache` (may be null) holds the electron's last element: it is taken
-// without a search only when the point is strictly inside it (all barycentrics >= 1e-9: then no other element qualifies).
+// without a search only when the point is strictly inside it: all barycentrics >= the element's own margin, 1e-9 scaled by
+// (largest element extent of the mesh) / (this element's smallest height) — then no other element passes F2's test, however
+// strongly the mesh is graded (derivation at mesh_image in avm.cu).
 __device__ __forceinline__ void tet_at(const DevSlab& s, double x, double y, double z, int* cache, double& Ex, double& Ey,
                                        double& Ez, double& mask) {
   double qx, qy;
@@ -329,7 +334,7 @@ __device__ __forceinline__ void tet_at(const DevSlab& s, double x, double y, dou
   // The cached index is a hint and may stem from ANOTHER kind-2 slab of the stack (the electron crossed a slab plane since):
   // strictly inside element e of this slab the answer is e whatever made us try it first, so a foreign hint is harmless —
   // provided it indexes this slab's records at all (slabs differ in n_tets; checked in every build, not only AVM_DEBUG).
-  if (cache && *cache >= 0 && *cache < s.n_tets) found = tet_try(s, *cache, 1e-9, qx, qy, qz, ex, ey, ez, m);
+  if (cache && *cache >= 0 && *cache < s.n_tets) found = tet_try<true>(s, *cache, 0.0, qx, qy, qz, ex, ey, ez, m);
   if (!found) {
     const double ux = (qx - s.tlo[0]) * s.tinv[0], uy = (qy - s.tlo[1]) * s.tinv[1], uz = (qz - s.tlo[2]) * s.tinv[2];
     int cx = (int)floor(ux), cy = (int)floor(uy), cz = (int)floor(uz);

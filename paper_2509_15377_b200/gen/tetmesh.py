@@ -19,10 +19,14 @@ from .fields import TetMesh
 MESH_KEY_XOR = 0x54455421
 
 
-def kuhn_mesh(nx: int, ny: int, nz: int, h, potential, seed: int = 0, jitter: float = 0.25, solid=None, removed=None) -> TetMesh:
+def kuhn_mesh(nx: int, ny: int, nz: int, h, potential, seed: int = 0, jitter: float = 0.25, solid=None, removed=None,
+              warp=None) -> TetMesh:
     """(nx, ny, nz) lattice points with spacings h = (hx, hy, hz); interior points displaced by jitter x h x (2u - 1), u from
     Philox (the boundary stays flat, so the mesh fills its box).  potential(x, y, z) -> V; solid(x, y, z) -> bool at element
-    centroids; removed(x, y, z) -> bool at centroids (those elements are dropped)."""
+    centroids; removed(x, y, z) -> bool at centroids (those elements are dropped).  warp(x, y, z) -> (x, y, z): an
+    orientation-preserving map applied to the jittered lattice points before anything else is derived from them (a GRADED
+    mesh: e.g. a piecewise-linear stretch of z puts elements ten times taller next to thin ones); edges stay straight, the
+    mid-edge nodes are the midpoints of the warped vertices."""
     hx, hy, hz = (float(v) for v in h)
     K, J, I = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
     ids = (K * ny + J) * nx + I
@@ -32,6 +36,9 @@ def kuhn_mesh(nx: int, ny: int, nz: int, h, potential, seed: int = 0, jitter: fl
     interior = ((I > 0) & (I < nx - 1) & (J > 0) & (J < ny - 1) & (K > 0) & (K < nz - 1)).reshape(-1)
     for a, hh in enumerate((hx, hy, hz)):
         pts[:, a] += np.where(interior, jitter * hh * (2.0 * u[a] - 1.0), 0.0)
+    if warp is not None:
+        wx, wy, wz = warp(pts[:, 0], pts[:, 1], pts[:, 2])
+        pts = np.stack([wx, wy, wz], axis=1).astype(np.float64)
     # six tetrahedra per cell: the paths from corner 000 to corner 111 along the axes in every order
     tets = []
     base = ids[:-1, :-1, :-1].reshape(-1)

@@ -205,6 +205,56 @@ def test_two_stacked_tetrahedral_slabs_of_different_size(avm, ctx, oracle, g0):
                              label=f"two stacked tetrahedral slabs, 300 primaries, flags {flags}")
 
 
+def test_graded_tetrahedral_mesh(avm, ctx, oracle, g0):
+    """A strongly graded mesh: the lower half of the lattice is squeezed 20-fold in z, so flat elements (2 um x 2 um x 0.1 um)
+    meet elements 20 times taller across the plane between them.  The device's last-element shortcut uses a per-element margin
+    scaled by (largest extent of the mesh) / (the element's smallest height) — DESIGN.md F2 — so that F2's lowest-index rule
+    holds whatever the grading; here: field at 2e5 points, per-step tolerance T in forms 0, 1 and 3 (the form that carries
+    the hint from step to step), and same-seed avalanches against the oracle, whose search has no shortcut."""
+    nx, ny, nz = 9, 9, 41
+    Lz = (nz - 1) * H
+    zm, sq = 0.5 * Lz, 20.0
+    zt = zm / sq                                                                # the squeezed half ends here
+    warp = lambda x, y, z: (x, y, np.where(z < zm, z / sq, zt + (z - zm) * (Lz - zt) / (Lz - zm)))
+    E0 = 40000.0
+    V = lambda x, y, z: -E0 * z * (1.0 + 30.0 * z) + 4.0e8 * (x ** 3 - 3.0 * x * y * y) * (1.0 + 50.0 * z)   # not quadratic: E jumps across faces
+    mesh = tetmesh.kuhn_mesh(nx, ny, nz, (H, H, H), V, seed=6, warp=warp)
+    xyz, tn = mesh.node_xyz, mesh.tet_nodes
+    hz = xyz[tn[:, :4], 2].max(axis=1) - xyz[tn[:, :4], 2].min(axis=1)
+    assert hz.max() / hz.min() > 25.0                                           # graded indeed
+    P = (nx - 1) * H
+    fd = fields.FieldDesc([fields.tet_slab(mesh, (0.0, 0.0, 0.0), 0.0, Lz, fields.BC_MIRROR, fields.BC_MIRROR, P, P)])
+    gg, fg = avm.gas_create(ctx, g0), avm.field_create(ctx, fd)
+    rng = np.random.default_rng(3)
+    n = 200000
+    r = np.zeros((3, n)); r[0:2] = rng.uniform(-2 * P, 2 * P, size=(2, n)); r[2] = rng.uniform(0.0, Lz, n)
+    r[2, : n // 2] = rng.uniform(0.0, 3 * zt, n // 2)                           # half of them in and just above the flat elements
+    Ec, mc, sc = oracle.field_eval(fd, r); Eg, mg, sg = avm.field_eval(ctx, fg, r)
+    assert np.array_equal(sc, sg) and np.array_equal(mc, mg)
+    assert np.all(np.abs(Ec - Eg).max(axis=0) <= 1e-11 * np.abs(Ec).max())
+    m_ = 1 << 14
+    st = _states(m_, rng, box=1.0)
+    st[0:3] = r[:, :m_]; st[2] = np.clip(st[2], 1e-7, Lz - 1e-7)
+    st[2, : m_ // 4] = zt + rng.uniform(-1, 1, m_ // 4) * 2e-6                  # flights across the plane where the sizes jump
+    ids = rng.integers(0, 2 ** 64, m_, dtype=np.uint64)
+    nidx = rng.integers(0, 1 << 20, m_, dtype=np.uint64).astype(np.uint32)
+    cpu = oracle.step_batch(g0, fd, 6, st, ids, nidx)
+    for form in (0, 1):
+        assert_step_parity(cpu, avm.step_batch_form(ctx, gg, fg, 6, st, ids, nidx, form=form), st, f"graded mesh form {form}")
+    for k in (4, 8):
+        gl = avm.step_form_lanes(k)
+        c3, st_in = oracle_sequence(oracle, g0, fd, 3, st[:, :k * 512], ids[:k * 512], nidx[:k * 512], gl, 5.0)
+        g3 = avm.step_batch_form(ctx, gg, fg, 3, st[:, :k * 512], ids[:k * 512], nidx[:k * 512], form=3, k=k, t_max=5.0)
+        assert_form2_parity(avm, c3, st_in, g3, gl, f"graded mesh form 3 k={k}")
+    p = primaries.isotropic_primaries(300, 17, pos=(0.0, 0.0, Lz - 2e-4), xy_box=((0.0, P), (0.0, P)))
+    cr = oracle.run(g0, fd, p, seed=17, n_threads=CORES)
+    gr = avm.simulate(ctx, gg, fg, p, seed=17)
+    assert cr.n > 600 and (cr.status == 1).sum() > 300
+    # observed on B200: 100 % identical histories of 8201 electrons, worst endpoint error 2.4e-5 (E jumps across faces)
+    assert_run_same_seed(cr, gr, g0.n_levels, min_identical=0.99, end_rtol=1e-7, tail=0.08, tail_rtol=1e-3,
+                         label="graded tetrahedral mesh (20x size jump), 300 primaries")
+
+
 def test_invalid_meshes_are_rejected(avm, ctx):
     mesh = tetmesh.kuhn_mesh(4, 4, 4, (H, H, H), lambda x, y, z: z, seed=1)
     bad = fields.TetMesh(mesh.node_xyz, mesh.node_V, mesh.tet_nodes.copy(), mesh.tet_gas)
