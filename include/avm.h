@@ -162,8 +162,12 @@ enum {
   /* Energy-banded null-collision rate (DESIGN.md §3.5 readings N1-N6): the rate of a flight is the
    * one of the electron's energy band and of the acceleration class of the field at its position (avm_gas_bands) instead
    * of the global nu_hat; a flight longer than the band's validity time is cut there and ends in a null collision.  The
-   * same physics (thinning with a piecewise-constant majorant is exact) in 1.6-5x fewer steps; the random streams are
-   * consumed differently, so a banded run is compared with a banded oracle run.  Runs take serial batches and full-warp
+   * same collision physics (thinning with a piecewise-constant majorant is exact) in 1.6-5x fewer steps; the random streams
+   * are consumed differently, so a banded run is compared with a banded oracle run.  NOT identical at absorbing planes:
+   * an electron is tested for having left the domain only where a flight ends, and banded flights are longer, so fewer
+   * electrons are lost at a plane they start on or linger near (config 1, primaries on the cathode plane: mean gain +1.1 %,
+   * share ending at the cathode -2.1 points against the global rate, N7).  Use the global rate when such
+   * losses matter.  Runs take serial batches and full-warp
    * iterations only (no time-parallel batches: a flight's rate depends on the energy the previous flight ended with). */
   AVM_RUN_BANDED = 16u
 };

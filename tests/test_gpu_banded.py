@@ -2,7 +2,7 @@
 CUDA path against the banded oracle (oracle flag AVMO_BANDED) — the table of rates bit for bit, per-step tolerance T (1e-12)
 through the two step forms a banded run takes (form 1 full-warp, form 3 serial batch), cut flights, uniforms constructed
 inside the bands of the 16-bit filter with the flight's own rate, same-seed whole runs, and the statistics of a banded GPU
-run against the UN-banded oracle (the same physics through other random streams).
+run against the UN-banded oracle (the same collision physics through other random streams — boundary losses differ, DESIGN.md §3.5 N7).
 """
 import os
 
@@ -285,7 +285,8 @@ def test_banded_config2_and_config4_same_seed(avm, ctx, oracle):
 
 
 def test_banded_statistics_against_the_unbanded_oracle(avm, ctx, oracle):
-    """The banded CUDA run and the UN-banded oracle draw different random streams for the same physics: mean gain within 3
+    """The banded CUDA run and the UN-banded oracle draw different random streams for the same collision physics (NOT the same losses at the start plane: DESIGN.md §3.5 N7 —
+    which is why the endpoint-z distribution is not compared here and why 4000 primaries do not resolve the 1 % gain shift): mean gain within 3
     combined SE, KS p > 0.01 on gain / endpoint energy / endpoint z, drift velocity within 1 % (config 1, 4000 primaries
     a side; config 4 in full)."""
     from test_gpu_acceptance import compare_statistics, w_alpha
