@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py — electron-collisions/s (real + null) of the avalanche hot path on B200, with its roofline.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload all|config1|config2|config3s|config4|config5|...]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload all|config1|config2|config3s|config3|config4|config4x16|config5|...]
   python bench.py --impl reference ...     # the oracle on the host cores
 
 A "step" is one pass of the whole hot path (avm_run: primary injection, persistent transport kernel with secondary
@@ -35,8 +35,14 @@ HEADLINE = "config3s"
 # workload -> (multiplier of --steps, oracle sample = first n primaries; 0 = all).  Oracle samples follow SURVEY.md §8(d)
 # "Oracle timing" (config 3: first primaries only, config 5: first 8), sized for ~1-10 s each on the box's cores.
 ALL = {"config1": (4, 0), "config2": (2, 0), "config3s": (1, 2048), "config4": (1, 0), "config5": (0.5, 8),
-       "config5hg": (0.2, -1)}      # not a BASELINE config (D4): config 5's stack at dV = 500 V, 1e4-1e5 electrons per avalanche;
+       "config5hg": (0.2, -1),      # not a BASELINE config (D4): config 5's stack at dV = 500 V, 1e4-1e5 electrons per avalanche;
                                     # -1: no oracle leg (one such avalanche is ~4e9 collisions on one core)
+       # HEAVY entries (multiplier 0): ONE timed run each, un-banded and banded, no warm-up of their own (the kernels are warm
+       # from the entries before them and one run lasts seconds), no e2e leg — stated in the entry's `timing`.
+       "config3": (0, 8),           # BASELINE config 3 AS STATED: 1 cm gap, no time cut, ~1.3e12 steps (~28 s; ~13 s banded)
+       "config4x16": (0, -1),       # replicated variants that show the map path's throughput asymptote
+       "config4x64": (0, -1)}
+HEAVY = {k for k, (m, _) in ALL.items() if m == 0}
 # Algorithmic FP64 thread-instructions per unit: what the method must do — NOT what
 # the kernel executes (the executed count and the FP64 pipe's busy share come from the ncu capture, when it is current).
 FP64_PER_NULL = {False: 90.0, True: 170.0}       # free flight + energy + bin + decision; key = B != 0
@@ -90,6 +96,8 @@ def make_workload(name: str, rank: int = 0):
         w = configs.config3(n_primaries=100000, t_max=20.0, id_offset=rank * 100000)
         w.name = "config3s"
         w.note += "; time cut t_max=20 ns"
+    elif name == "config3":                       # as BASELINE states it: no time cut
+        w = configs.config3(n_primaries=100000, id_offset=rank * 100000)
     elif name == "config4":
         w = configs.config4(id_offset=rank * 1000)
     elif name.startswith("config4x"):
@@ -210,18 +218,28 @@ def oracle_leg(w, n_prim: int, threads: int) -> dict:
             "electrons": int(r.n), "primaries": int(n_prim)}
 
 
-def cpu_baseline_entry(w, sample: int, cores: int) -> dict:
+def cpu_baseline_entry(w, sample: int, cores: int, one_core: bool = False) -> dict:
     n_prim = min(w.n_primaries, sample) if sample > 0 else w.n_primaries
     o = oracle_leg(w, n_prim, cores)
-    return {"value": o["collisions"] / o["seconds"], "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"first {n_prim} of {w.n_primaries} primaries of {w.name}, seed {w.seed}, {cores} threads over disjoint "
-                      f"primary ranges, {o['collisions']} collisions in {o['seconds']:.2f} s",
-            "avalanches_per_s": n_prim / o["seconds"], "null_per_s": o["null"] / o["seconds"], "real_per_s": o["real"] / o["seconds"]}
+    out = {"value": o["collisions"] / o["seconds"], "unit": UNIT, "cores": cores, "kind": "oracle",
+           "sample": f"first {n_prim} of {w.n_primaries} primaries of {w.name}, seed {w.seed}, {cores} threads over disjoint "
+                     f"primary ranges, {o['collisions']} collisions in {o['seconds']:.2f} s",
+           "avalanches_per_s": n_prim / o["seconds"], "null_per_s": o["null"] / o["seconds"], "real_per_s": o["real"] / o["seconds"]}
+    if one_core:
+        # SURVEY §8(d) "Oracle timing": the serial figure in the same harness — one thread on a sample sized to ~the same
+        # seconds (1/cores of the primaries, at least one)
+        n1 = max(1, n_prim // max(cores, 1))
+        o1 = oracle_leg(w, n1, 1)
+        out["one_core"] = {"value": o1["collisions"] / o1["seconds"], "unit": UNIT, "cores": 1,
+                           "sample": f"first {n1} primaries, 1 thread, {o1['collisions']} collisions in {o1['seconds']:.2f} s",
+                           "ns_per_collision": 1e9 * o1["seconds"] / max(o1["collisions"], 1)}
+    return out
 
 
 def workload_list(args):
     if args.workload == "all":
-        return [(nm, max(1, int(round(args.steps * mult))), smp) for nm, (mult, smp) in ALL.items()]
+        return [(nm, max(1, int(round(args.steps * mult))), smp) for nm, (mult, smp) in ALL.items()
+                if not (args.skip_heavy and nm in HEAVY)]
     smp = args.ref_primaries if args.ref_primaries > 0 else ALL.get(args.workload, (1, 0))[1]
     return [(args.workload, args.steps, smp)]
 
@@ -270,7 +288,7 @@ def run_reference(args) -> None:
     print(json.dumps(line), flush=True)
 
 
-def bench_workload(avm, ctx, torch, dist, name, steps, warmup, sample, rank, world, peaks, flush, with_cpu, cores):
+def bench_workload(avm, ctx, torch, dist, name, steps, warmup, sample, rank, world, peaks, flush, with_cpu, cores, head_name=None):
     """W warm-ups + exactly `steps` timed steps of one workload (device-timed, inputs resident) and the same through the
     user's call with host buffers (e2e); returns its per_config entry (rank 0) and the clock samples of the timed region."""
     w = make_workload(name, rank)
@@ -312,6 +330,9 @@ def bench_workload(avm, ctx, torch, dist, name, steps, warmup, sample, rank, wor
         d2h = n * per_el + host.per_avalanche.numel() * 8 + host.tallies_u64.numel() * 8 + host.tallies_f64.numel() * 8
         return {"s": dt, "n": n, "tallies": res.tallies_u64.copy(), "d2h": d2h}
 
+    heavy = name in HEAVY
+    if heavy:
+        warmup = 0
     for i in range(warmup):
         device_step(w.seed + 1000 + i)
     sampler = ClockSampler(ctx.device.index or 0)
@@ -323,9 +344,9 @@ def bench_workload(avm, ctx, torch, dist, name, steps, warmup, sample, rank, wor
     for i in range(min(warmup, 2)):
         e2e_step(w.seed + 2000 + i)
     barrier()
-    e2e = [e2e_step(w.seed + i) for i in range(steps)]
+    e2e = [] if heavy else [e2e_step(w.seed + i) for i in range(steps)]
     barrier()
-    # the same workload under the energy-banded null-collision rate (AVM_RUN_BANDED): same physics in
+    # the same workload under the energy-banded null-collision rate (AVM_RUN_BANDED): same collision physics (boundary losses differ: DESIGN.md §3.5 N7) in
     # fewer null steps, so collisions/s falls while avalanches/s rises — reported beside the headline, never as it
     for i in range(min(warmup, 2)):
         device_step(w.seed + 3000 + i, avm.RUN_BANDED)
@@ -339,7 +360,7 @@ def bench_workload(avm, ctx, torch, dist, name, steps, warmup, sample, rank, wor
     sums = [sum(int(s["tallies"][L]) for s in st), sum(int(s["tallies"][L + 1]) for s in st), sum(int(s["n"]) for s in st),
             sum(s["launches"] for s in st), sum(int(s["tallies"][L]) + int(s["tallies"][L + 1]) for s in e2e),
             sum(alg_fp64(s["tallies"], L, w.gas.level_type, has_b, gfrac) for s in st), sum(s["transport_launches"] for s in st)]
-    e2e_s = sum(s["s"] for s in e2e)
+    e2e_s = sum(s["s"] for s in e2e) if e2e else 1.0
     bd_ms = sum(s["ms"] for s in bd)
     bd_sums = [sum(int(s["tallies"][L]) for s in bd), sum(int(s["tallies"][L + 1]) for s in bd), sum(int(s["n"]) for s in bd)]
     vals = torch.tensor([tot_ms, e2e_s, t_ms, bd_ms], dtype=torch.float64, device=ctx.device)
@@ -364,6 +385,13 @@ def bench_workload(avm, ctx, torch, dist, name, steps, warmup, sample, rank, wor
                 "fp64_pipe_active_pct_ncu": cap["fp64_pipe_active_pct_ncu"], "ncu_source": cap["ncu_source"],
                 "peak_source": "measured: avm_fp64_probe DFMA rate on this GPU in this run", "peak_nominal": peaks["fp64_nominal"] / 1e12,
                 "alg_fp64_per_collision": sums[5] / max(sums[0] + sums[1], 1.0),
+                # the three readings of "how busy is the FP64 pipe", side by side: algorithmic work / peak (frac, above), the
+                # FP64 thread-instructions the kernel EXECUTES (ncu, per collision) x this run's collisions / time / peak, and
+                # the share of cycles the FP64 pipe is busy (ncu).  The last two are null when the capture is stale.
+                "frac_algorithmic": achieved / peaks["fp64_measured"],
+                "frac_executed_lanes": (None if cap["sass_fp64_per_collision_ncu"] is None else
+                                        cap["sass_fp64_per_collision_ncu"] * (sums[0] + sums[1]) / (t_ms * 1e-3) / peaks["fp64_measured"]),
+                "frac_pipe_busy": None if cap["fp64_pipe_active_pct_ncu"] is None else cap["fp64_pipe_active_pct_ncu"] / 100.0,
                 "launch_ms": t_ms / n_launch, "transport_share_of_step": t_ms / max(tot_ms, 1e-9)}
     if gfrac > 0.0:      # maps: the field gather against the MEASURED random-sector bandwidth; report the lower fraction's bound
         gb = gfrac * (sums[0] + sums[1]) * GATHER_BYTES_PER_GRID_STEP
@@ -379,17 +407,24 @@ def bench_workload(avm, ctx, torch, dist, name, steps, warmup, sample, rank, wor
              "ms_per_step": tot_ms_max / max(steps, 1), "null_per_s": null / wall, "real_per_s": real / wall,
              "avalanches_per_s": world * w.n_primaries * steps / wall, "electrons_per_step": electrons / max(steps, 1) / world,
              "collisions_per_step": (null + real) / max(steps, 1) / world, "roofline": roofline,
-             "e2e": {"value": e2e_coll / e2e_s_max, "unit": UNIT, "h2d_bytes_per_step": int(w.n_primaries * 64),
-                     "d2h_bytes_per_step": int(sum(s["d2h"] for s in e2e) / max(len(e2e), 1)), "ms_per_step": 1e3 * e2e_s_max / max(steps, 1)},
+             "e2e": (None if heavy else
+                     {"value": e2e_coll / e2e_s_max, "unit": UNIT, "h2d_bytes_per_step": int(w.n_primaries * 64),
+                      "d2h_bytes_per_step": int(sum(s["d2h"] for s in e2e) / max(len(e2e), 1)), "ms_per_step": 1e3 * e2e_s_max / max(steps, 1)}),
              "gpu_launches": int(launches), "config": config_dict(w, world), "capacity": w.capacity, "clocks": clocks,
-             "banded": {"what": "same workload with AVM_RUN_BANDED (energy-banded null-collision rate, DESIGN.md §3.5): other random streams, same physics",
+             "banded": {"what": "same workload with AVM_RUN_BANDED (energy-banded null-collision rate, DESIGN.md §3.5): other random streams; the same collision "
+                                "physics, but termination is tested at sampled points only (R13), so longer flights lose fewer electrons at absorbing "
+                                "planes (config 1, oracle alone: gain +1.1 %, cathode share -2.1 points; DESIGN.md §3.5 N7) — not a like-for-like speed-up there",
                         "value": (bd_null + bd_real) / (bd_ms_max * 1e-3), "unit": UNIT, "ms_per_step": bd_ms_max / max(steps, 1),
                         "null_per_s": bd_null / (bd_ms_max * 1e-3), "real_per_s": bd_real / (bd_ms_max * 1e-3),
                         "avalanches_per_s": world * w.n_primaries * steps / (bd_ms_max * 1e-3),
                         "electrons_per_step": bd_el / max(steps, 1) / world,
                         "speedup_avalanches_per_s": tot_ms_max / max(bd_ms_max, 1e-9)}}
+    if heavy:
+        entry["timing"] = ("heavy entry: ONE timed run un-banded and ONE banded, device-timed like the others (CUDA events, inputs resident, "
+                           "L2 flushed before), no warm-up runs of its own (kernels and clocks are warm from the preceding entries; one run "
+                           "lasts seconds) and no e2e leg (host copies are < 0.1 % of such a run: see config3s / config4)")
     if with_cpu and sample >= 0:
-        entry["cpu_baseline"] = cpu_baseline_entry(w, sample, cores)
+        entry["cpu_baseline"] = cpu_baseline_entry(w, sample, cores, one_core=(name == head_name))
     return entry, clocks
 
 
@@ -424,7 +459,7 @@ def run_ours(args) -> None:
     head = HEADLINE if args.workload == "all" else args.workload
     per = []
     for name, steps, sample in workload_list(args):
-        e, _ = bench_workload(avm, ctx, torch, dist, name, steps, args.warmup, sample, rank, world, peaks, flush, with_cpu, cores)
+        e, _ = bench_workload(avm, ctx, torch, dist, name, steps, args.warmup, sample, rank, world, peaks, flush, with_cpu, cores, head_name=head)
         if e is not None:
             per.append(e)
         torch.cuda.empty_cache()
@@ -459,6 +494,7 @@ def main() -> None:
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-primaries", type=int, default=0, help="oracle legs: first n primaries only (0 = the workload's default sample)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--skip-heavy", action="store_true", help="--workload all without the single-run heavy entries (config3 in full, config4x16/x64)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
