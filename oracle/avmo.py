@@ -14,18 +14,25 @@ from dataclasses import dataclass
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SO = os.path.join(_HERE, "libavmo.so")
+_SO_SAN = os.path.join(_HERE, "libavmo_san.so")        # build(sanitize=True): the same source under ASan + UBSan
+# AVMO_SANITIZED=1 makes this process load the sanitizer build (the process must then run with libasan preloaded:
+# tests/test_oracle_sanitizers.py does that in a subprocess)
+_SANITIZED = os.environ.get("AVMO_SANITIZED") == "1"
+_SO = _SO_SAN if _SANITIZED else os.path.join(_HERE, "libavmo.so")
 _lib = None
 
 
-def build(force: bool = False) -> str:
+def build(force: bool = False, sanitize: bool = _SANITIZED) -> str:
+    """sanitize: -fsanitize=address,undefined (the oracle under ASan / UBSan), every report fatal."""
     src = os.path.join(_HERE, "avmo.cpp")
     hdr = os.path.join(_HERE, "avmo.h")
-    if not force and os.path.exists(_SO) and os.path.getmtime(_SO) >= max(os.path.getmtime(src), os.path.getmtime(hdr)):
-        return _SO
-    cmd = ["g++", "-O2", "-ffp-contract=off", "-std=c++17", "-shared", "-fPIC", "-pthread", "-o", _SO, src]
+    so = _SO_SAN if sanitize else os.path.join(_HERE, "libavmo.so")
+    if not force and os.path.exists(so) and os.path.getmtime(so) >= max(os.path.getmtime(src), os.path.getmtime(hdr)):
+        return so
+    opt = ["-O1", "-g", "-fno-omit-frame-pointer", "-fsanitize=address,undefined", "-fno-sanitize-recover=all"] if sanitize else ["-O2"]
+    cmd = ["g++"] + opt + ["-ffp-contract=off", "-std=c++17", "-shared", "-fPIC", "-pthread", "-o", so, src]
     subprocess.run(cmd, check=True, cwd=_HERE)
-    return _SO
+    return so
 
 
 class GasDesc(C.Structure):
