@@ -154,7 +154,7 @@ int32_t avm_field_eval(avm_ctx*, const avm_field*, int64_t n, const double* r, d
  * its birth point with the corresponding status. */
 enum {
   AVM_RUN_PRIMARIES_ON_DEVICE = 1u,
-  AVM_RUN_NO_TALLIES = 2u,        /* accepted for compatibility: the hot loop's tallies are three per-thread counters */
+  /* bit 2u is unused (it was AVM_RUN_NO_TALLIES, a flag without effect: tallies are three per-thread counters) */
   /* Launch shape of the transport kernel.  Default: chosen from n_primaries (wide when the primaries alone outnumber
    * the lanes of the latency shape).  Results do not depend on the shape. */
   AVM_RUN_SHAPE_WIDE = 4u,        /* 768 threads per SM: most lanes, for runs that keep them busy */

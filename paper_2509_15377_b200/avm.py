@@ -22,7 +22,7 @@ if not os.path.exists(_SO):
 _lib = C.CDLL(_SO)
 
 OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_CUDA, ERR_STATE = 0, -1, -2, -3, -4
-RUN_PRIMARIES_ON_DEVICE, RUN_NO_TALLIES, RUN_SHAPE_WIDE, RUN_SHAPE_LATENCY, RUN_BANDED = 1, 2, 4, 8, 16
+RUN_PRIMARIES_ON_DEVICE, RUN_SHAPE_WIDE, RUN_SHAPE_LATENCY, RUN_BANDED = 1, 4, 8, 16
 MAX_LEVELS, MAX_SLABS = 64, 8
 RUN_STATIC_MAX_CAPACITY = 65536     # AVM_RUN_STATIC_MAX_CAPACITY: largest `capacity` run_static accepts
 EXPORTS = ["avm_last_error", "avm_ctx_create", "avm_ctx_destroy", "avm_ctx_sm_count", "avm_gas_bytes",
